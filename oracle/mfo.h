@@ -1,0 +1,133 @@
+/* mfo.h -- C API of the ORACLE (test infrastructure, NOT the product).
+ *
+ * Plain, slow, fp64 CPU restatement of the MadFlow leading-order integrand hot path
+ * (arxiv 2105.10529; PAPER.md:29,59 pipeline "random numbers -> phase space -> matrix element ->
+ * histogram accumulation", PAPER.md:47,67,69 structure of the matrix element).  The paper prints no
+ * formulas; every step follows the reading listed in DESIGN.md ("Readings", items O1-O11 / A1-A24,
+ * taken from SURVEY.md section 8(c)).
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may use
+ * anything under oracle/.  It shares no code, header, table or constant generator with the CUDA
+ * path (paper_2105_10529_b200/csrc); the struct definitions below are the oracle's own.
+ *
+ * All pointers are HOST pointers.  All functions return 0 on success, <0 on error.
+ */
+#ifndef MFO_H
+#define MFO_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { MFO_OK = 0, MFO_EINVAL = -1, MFO_ENOMEM = -2, MFO_ESTATE = -4, MFO_EUNSUPPORTED = -5 };
+enum { MFO_EE_MUMU = 0, MFO_GG_TT = 1, MFO_GG_TTG = 2, MFO_GG_TTGG = 3 };
+
+typedef struct {
+  int32_t  process;            /* MFO_*                                                          */
+  uint64_t seed;               /* Philox key (O1)                                                */
+  uint32_t n_bins;             /* VEGAS bins per dimension (50)                                  */
+  double   alpha_damp;         /* VEGAS damping exponent (1.5)                                   */
+  double   sqrt_s, m_top, alpha_s, alpha_em, mu_f;
+  double   ptmin_g, etamax_g, drmin_gg;   /* cuts; <= 0 disables                                 */
+  double   gev2_to_pb;         /* 0.3894e9                                                       */
+  const double *pdf_xf;        /* host [nx][nq] row-major table of x*g(x,Q^2); must not be NULL  */
+  uint32_t pdf_nx, pdf_nq;
+  double   pdf_xmin, pdf_xmax, pdf_qmin, pdf_qmax;
+} mfo_config_t;
+
+typedef struct {               /* host buffers owned by the caller; NULL = skip                  */
+  double  *weight;             /* [n]  F_i = w_i f_i  (t_i * N)                                  */
+  double  *x;                  /* [n][d]  VEGAS points                                           */
+  uint8_t *bins;               /* [n][d]                                                         */
+  double  *momenta;            /* [n][2+n_final][4] (E,px,py,pz), partonic CM frame              */
+  double  *me2;                /* [n]  |M|^2 averaged/summed, before the symmetry factor         */
+  double  *pdf;                /* [n][2]  xg(x1), xg(x2)                                         */
+  uint8_t *pass;               /* [n]  1 if the event passed the cuts                            */
+} mfo_eval_out_t;
+
+typedef struct { double integral, sigma; uint64_t n_events, n_pass, n_nonfinite; } mfo_iter_t;
+typedef struct { double integral, sigma, chi2_dof; uint32_t n_iter; } mfo_result_t;
+typedef struct mfo_vegas mfo_vegas_t;
+
+/* ---- the path (same calls as the product's C-ABI, on host memory) ---------------------------- */
+int mfo_vegas_create(const mfo_config_t *cfg, mfo_vegas_t **out);
+int mfo_vegas_destroy(mfo_vegas_t *h);
+int mfo_ndim(const mfo_vegas_t *h, uint32_t *d, uint32_t *n_final);
+int mfo_integrand_eval(mfo_vegas_t *h, uint32_t iteration, uint64_t first_event, uint64_t n_events,
+                       const mfo_eval_out_t *out, int n_threads);
+int mfo_vegas_iterate(mfo_vegas_t *h, uint64_t n_events, int n_threads, mfo_iter_t *out);
+int mfo_result(mfo_vegas_t *h, mfo_result_t *out);
+int mfo_get_grid(mfo_vegas_t *h, double *edges /* [d][n_bins+1] */);
+int mfo_set_grid(mfo_vegas_t *h, const double *edges);
+/* raw sums of the last iteration: acc[0]=sum t, acc[1]=sum t^2, acc[2+j*nb+k]=H[j][k] (O9) */
+int mfo_get_accum(mfo_vegas_t *h, double *acc /* [2 + d*n_bins] */);
+/* accumulate events [first, first+n) of an iteration of n_total events into acc (adds; O9);
+ * counts[0] += n_pass, counts[1] += n_nonfinite.  Used by the sharding tests. */
+int mfo_vegas_accumulate(mfo_vegas_t *h, uint32_t iteration, uint64_t first_event, uint64_t n_events,
+                         uint64_t n_total, int n_threads, double *acc, uint64_t *counts);
+/* finish an iteration from raw sums (O10): record (I, sigma), refine the grid */
+int mfo_vegas_finalize(mfo_vegas_t *h, const double *acc, uint64_t n_total, uint64_t n_pass,
+                       uint64_t n_nonfinite, mfo_iter_t *out);
+int mfo_max_threads(void);
+
+/* ---- single steps, exported so that the tests can pin each one ------------------------------- */
+/* O1 */
+void mfo_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+void mfo_uniforms(uint64_t seed, uint32_t iteration, uint64_t event, uint32_t d, double *u);
+/* O2 */
+void mfo_vegas_map(const double *edges, uint32_t d, uint32_t nb, const double *u,
+                   double *x, uint8_t *bins, double *jac);
+/* O10 refinement of one set of edges [d][nb+1] from H [d][nb] */
+void mfo_refine(const double *edges_in, const double *H, uint32_t d, uint32_t nb, double alpha,
+                double *edges_out);
+/* O11 */
+void mfo_combine(const double *I, const double *sig, uint32_t n, mfo_result_t *out);
+/* O3: y0,y1 -> x1,x2,shat,Jx */
+void mfo_x_map(double y0, double y1, double s, double shat_min, double *x1, double *x2,
+               double *shat, double *jx);
+/* O4: n-body phase space from 3n-4 numbers. p0: massless momenta [n][4], k: massive [n][4],
+ * Mint[n] intermediate masses (Mint[0]=sqrt(shat)), out3 = {W0, Wm, xi}; returns Newton steps */
+int mfo_phase_space(uint32_t n, double shat, const double *masses, const double *rs,
+                    double *p0, double *k, double *Mint, double *out3);
+/* O5 */
+double mfo_pdf_interp(const double *xf, uint32_t nx, uint32_t nq, double xmin, double xmax,
+                      double qmin, double qmax, double x, double q2);
+/* O6.2: kind 0 = u (incoming fermion), 1 = v (outgoing antifermion); out = 4 complex (re,im) */
+void mfo_wf_fermion(int kind, const double p[4], double m, int lambda, double out[8]);
+/* polarisation vector eps(p,lambda) (not conjugated); out = 4 complex, upper index */
+void mfo_wf_vector(const double p[4], int lambda, double out[8]);
+/* gamma^mu in the chiral representation, out[mu][r][c] complex -> [4][4][4][2] */
+void mfo_gamma(double out[128]);
+/* O6.6: colour matrix numerators over the common denominator, [nf][nf], nf = ng! */
+int mfo_colour_matrix(uint32_t ng, double *numer, double *denom);
+/* SU(3): T^a (a=0..7) as [8][3][3][2] and f^{abc} as [8][8][8] */
+void mfo_su3(double *T, double *f);
+/* O6.5 counts: diagrams, colour-stripped sub-amplitudes, flows */
+int mfo_diagram_counts(uint32_t ng, uint32_t *ndiag, uint32_t *nsub, uint32_t *nflow);
+/* O6: |M|^2 averaged over initial and summed over final helicities/colours (before S_f) at the
+ * given momenta [2+n_final][4] (incoming k1,k2 then final), algorithm A (diagram list + flows) */
+int mfo_me2(int process, const double *mom, double m_top, double alpha_s, double alpha_em,
+            double *out);
+/* same with the literal colour-dressed recursion (algorithm B) and explicit colour sum;
+ * hel_only >= 0 restricts the helicity sum to that single combination index                    */
+int mfo_me2_literal(int process, const double *mom, double m_top, double alpha_s, int hel_only,
+                    double *out);
+/* algorithm A for one helicity combination hel[2+n_final] (+-1): jamp[nf] complex, and the
+ * colour-summed |M|^2 of that helicity (no averaging).  ward_leg >= 0 replaces that gluon leg's
+ * polarisation by its momentum (P19).                                                          */
+int mfo_jamps(int process, const double *mom, double m_top, double alpha_s, const int *hel,
+              int ward_leg, double *jamp /* [nf][2] */, double *me2_hel);
+/* algorithm B amplitude iM for explicit colours: col_g[ng] in 0..7, c3,c4 in 0..2 */
+int mfo_amp_literal(int process, const double *mom, double m_top, double alpha_s, const int *hel,
+                    const int *col_g, int c3, int c4, int ward_leg, double out[2]);
+/* O7: cuts on final gluons in the lab frame; obs = {pt_i, eta_i (per gluon)..., dR} */
+int mfo_cuts(uint32_t n_gluons, const double *kg /* [n_gluons][4] */, double x1, double x2,
+             double ptmin, double etamax, double drmin, double *obs);
+/* O4.3 */
+double mfo_w0(uint32_t n, double shat);
+const char *mfo_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,119 @@
+/* madflow_b200.h -- C-ABI boundary of the B200-native MadFlow leading-order integrand path.
+ *
+ * The operation: "integrate an event-parallel integrand with an adaptive importance-sampling
+ * integrator, entirely on the device" (PAPER.md:15 parallelism over events; PAPER.md:29 the four
+ * ingredients: integrator, PDF interpolation, phase space + cuts, matrix element
+ * VegasFlow/PDFFlow; PAPER.md:59 pipeline "random numbers -> phase-space kinematics -> matrix
+ * element -> histogram accumulation"; PAPER.md:85 everything stays in GPU memory).  The paper prints
+ * no formulas; the arithmetic of every step is the reading listed in DESIGN.md (O1-O11, A1-A24).
+ *
+ * Conventions
+ *  - Every function returns MF_OK (0) or a negative MF_E* code; none throws or exits.  A message for
+ *    the last error of the calling thread is available from mf_last_error().
+ *  - mf_vegas_t is opaque and owned by the library (create/destroy).  The library owns its scratch
+ *    (per-block partial sums, grid edges, iteration records) in device memory.
+ *  - Pointers in mf_config_t and the "host_*" arguments are HOST pointers.  Pointers inside
+ *    mf_eval_out_t are DEVICE pointers owned by the caller (e.g. torch tensors' data_ptr()).
+ *  - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Work is
+ *    only enqueued; a call synchronises the stream only where stated.
+ *  - Event indices are global within an iteration: evaluating [0,N) in one call or in chunks gives
+ *    identical per-event values (counter-based RNG, reading A1).
+ *  - There is no CPU fallback: without a CUDA device every compute call returns MF_ECUDA.
+ */
+#ifndef MADFLOW_B200_H
+#define MADFLOW_B200_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mf_vegas mf_vegas_t;
+
+enum { MF_OK = 0, MF_EINVAL = -1, MF_ENOMEM = -2, MF_ECUDA = -3, MF_ESTATE = -4, MF_EUNSUPPORTED = -5 };
+/* processes (BASELINE.json configs 0-3) */
+enum { MF_EE_MUMU = 0, MF_GG_TT = 1, MF_GG_TTG = 2, MF_GG_TTGG = 3 };
+
+typedef struct {
+  uint32_t struct_size;      /* = sizeof(mf_config_t); ABI check                                     */
+  int32_t  process;          /* MF_EE_MUMU .. MF_GG_TTGG                                             */
+  int32_t  precision;        /* 64 (fp64, the path) ; 32 -> MF_EUNSUPPORTED in this build            */
+  int32_t  device;           /* CUDA ordinal                                                         */
+  uint64_t seed;             /* Philox key (reading A1)                                              */
+  uint32_t n_bins;           /* VEGAS bins per dimension, 1..64 (configs: 50)                        */
+  uint32_t reserved0;
+  double   alpha_damp;       /* VEGAS damping exponent (1.5)                                         */
+  double   sqrt_s;           /* collider energy, GeV (config 0: the fixed e+e- energy)               */
+  double   m_top, alpha_s, alpha_em, mu_f;
+  double   ptmin_g, etamax_g, drmin_gg;   /* cuts on final gluons, lab frame; <= 0 disables (O7)     */
+  double   gev2_to_pb;       /* 0.3894e9 (reading A11)                                               */
+  const double *pdf_xf;      /* HOST [pdf_nx][pdf_nq] row-major table of x*g(x,Q^2); copied at       */
+                             /* create; required for processes 1-3, ignored for process 0            */
+  uint32_t pdf_nx, pdf_nq;   /* knots, uniform in ln x resp. ln Q^2; nx*nq*8 bytes <= 160 KB         */
+  double   pdf_xmin, pdf_xmax, pdf_qmin, pdf_qmax;
+} mf_config_t;
+
+/* Optional per-event outputs of mf_integrand_eval.  DEVICE pointers, caller-owned, NULL = skip.     */
+typedef struct {
+  double  *weight;           /* [n]  F_i = w_i f_i (= t_i * N), pb; 0 for events failing the cuts    */
+  double  *x;                /* [n][d]  VEGAS points y_j (O2)                                         */
+  uint8_t *bins;             /* [n][d]  VEGAS bin indices k_j                                         */
+  double  *momenta;          /* [n][2+n_final][4]  (E,px,py,pz), partonic CM frame, incoming first   */
+  double  *me2;              /* [n]  |M|^2 averaged/summed, before the symmetry factor; 0 if cut     */
+  double  *pdf;              /* [n][2]  xg(x1,muF^2), xg(x2,muF^2)                                    */
+  uint8_t *pass;             /* [n]  1 if the event passed the cuts                                  */
+} mf_eval_out_t;
+
+typedef struct { double integral, sigma; uint64_t n_events, n_pass, n_nonfinite; float kernel_ms; } mf_iter_t;
+typedef struct { double integral, sigma, chi2_dof; uint32_t n_iter; } mf_result_t;
+
+/* Validate cfg, copy it and the PDF table, allocate device state, set the uniform grid.  No kernel
+ * work.  Errors: MF_EINVAL (bad field, kinematics outside the PDF grid), MF_EUNSUPPORTED
+ * (precision != 64), MF_ECUDA (no device / allocation failure).                                    */
+int mf_vegas_create(const mf_config_t *cfg, mf_vegas_t **out);
+int mf_vegas_destroy(mf_vegas_t *h);
+/* d = VEGAS dimensions (2 for process 0, else 2 + 3 n_final - 4), n_final = final-state particles */
+int mf_ndim(const mf_vegas_t *h, uint32_t *d, uint32_t *n_final);
+
+/* S1-S8 for events [first_event, first_event + n_events) of iteration `iteration` on the CURRENT
+ * grid; writes the requested per-event records.  No grid update, no reduction, no host sync.       */
+int mf_integrand_eval(mf_vegas_t *h, uint32_t iteration, uint64_t first_event, uint64_t n_events,
+                      const mf_eval_out_t *out, void *cuda_stream);
+
+/* One VEGAS iteration of n_events (>= 2) events: S1-S9 fused in one kernel (no per-event global
+ * traffic), then S10 in a one-block finalize kernel: I, sigma, grid refinement, record appended on
+ * the device.  Enqueue only, unless host_out_or_null != NULL: then the stream is synchronised and
+ * the iteration record (with the device time of the two kernels) is returned.                      */
+int mf_vegas_iterate(mf_vegas_t *h, uint64_t n_events, void *cuda_stream, mf_iter_t *host_out_or_null);
+
+/* Sharded form of one iteration (multi-GPU): accumulate events
+ * [first_event, first_event+n_events) of an iteration of n_total events into the handle's raw sums
+ * (device, [2 + d*n_bins] doubles + 2 counters); read / overwrite the raw sums from the host (the
+ * caller all-reduces them); finish the iteration from the raw sums.  mf_vegas_iterate ==
+ * accumulate(0, n, n) + finalize.                                                                   */
+int mf_vegas_accumulate(mf_vegas_t *h, uint64_t first_event, uint64_t n_events, uint64_t n_total,
+                        void *cuda_stream);
+int mf_get_accum(mf_vegas_t *h, double *host_acc /* [2 + d*n_bins] */, uint64_t *host_counts /* [2] */);
+int mf_set_accum(mf_vegas_t *h, const double *host_acc, const uint64_t *host_counts);
+int mf_vegas_finalize(mf_vegas_t *h, uint64_t n_total, void *cuda_stream, mf_iter_t *host_out_or_null);
+
+/* O11 combination over all iterations so far; synchronises the last-used stream.  MF_ESTATE if no
+ * iteration has been run.                                                                           */
+int mf_result(mf_vegas_t *h, mf_result_t *host_out);
+/* per-iteration records; host_out[n_iter] must hold at least max_iter entries; *n_iter = stored    */
+int mf_get_iterations(mf_vegas_t *h, mf_iter_t *host_out, uint32_t max_iter, uint32_t *n_iter);
+int mf_get_grid(mf_vegas_t *h, double *host_edges /* [d][n_bins+1] */);
+int mf_set_grid(mf_vegas_t *h, const double *host_edges);   /* edges must start at 0, end at 1, increase */
+/* Launch geometry of the fused kernel: blocks per SM (0 = library default) and threads per block
+ * (0 = default).  Results are deterministic for a fixed geometry.                                  */
+int mf_set_launch(mf_vegas_t *h, uint32_t blocks_per_sm, uint32_t threads_per_block);
+/* Exact add/mul/fma counts per event of the generated |M|^2 code of the handle's process
+ * (generator-counted): flops = add + mul + 2 fma.                    */
+int mf_me_flops(const mf_vegas_t *h, uint64_t *n_add, uint64_t *n_mul, uint64_t *n_fma);
+/* Register-resident DFMA-chain microbenchmark on `device`: measured fp64 FLOP/s (roofline peak).   */
+int mf_fp64_peak(int32_t device, double seconds, double *host_flops_per_s);
+const char *mf_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

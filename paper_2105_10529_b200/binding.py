@@ -1,0 +1,214 @@
+"""Thin ctypes binding of the C-ABI library (include/madflow_b200.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of libmadflow_b200.so; PyTorch is used by callers
+for device memory and streams (tensors' data_ptr(), torch.cuda.current_stream()).  There is no CPU
+path: if the library is missing or no CUDA device is present the calls raise.
+"""
+import ctypes as C
+import os
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmadflow_b200.so")
+
+MF_OK, MF_EINVAL, MF_ENOMEM, MF_ECUDA, MF_ESTATE, MF_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
+EXPORTS = ["mf_vegas_create", "mf_vegas_destroy", "mf_ndim", "mf_integrand_eval", "mf_vegas_iterate",
+           "mf_vegas_accumulate", "mf_get_accum", "mf_set_accum", "mf_vegas_finalize", "mf_result",
+           "mf_get_iterations", "mf_get_grid", "mf_set_grid", "mf_set_launch", "mf_me_flops",
+           "mf_fp64_peak", "mf_last_error"]
+
+
+class MfError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("madflow_b200 error %d: %s" % (code, msg))
+        self.code = code
+
+
+class Config(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("process", C.c_int32), ("precision", C.c_int32),
+                ("device", C.c_int32), ("seed", C.c_uint64), ("n_bins", C.c_uint32), ("reserved0", C.c_uint32),
+                ("alpha_damp", C.c_double), ("sqrt_s", C.c_double), ("m_top", C.c_double),
+                ("alpha_s", C.c_double), ("alpha_em", C.c_double), ("mu_f", C.c_double),
+                ("ptmin_g", C.c_double), ("etamax_g", C.c_double), ("drmin_gg", C.c_double),
+                ("gev2_to_pb", C.c_double), ("pdf_xf", C.POINTER(C.c_double)),
+                ("pdf_nx", C.c_uint32), ("pdf_nq", C.c_uint32), ("pdf_xmin", C.c_double),
+                ("pdf_xmax", C.c_double), ("pdf_qmin", C.c_double), ("pdf_qmax", C.c_double)]
+
+
+class EvalOut(C.Structure):
+    _fields_ = [("weight", C.c_void_p), ("x", C.c_void_p), ("bins", C.c_void_p), ("momenta", C.c_void_p),
+                ("me2", C.c_void_p), ("pdf", C.c_void_p), ("pass_", C.c_void_p)]
+
+
+class Iter(C.Structure):
+    _fields_ = [("integral", C.c_double), ("sigma", C.c_double), ("n_events", C.c_uint64),
+                ("n_pass", C.c_uint64), ("n_nonfinite", C.c_uint64), ("kernel_ms", C.c_float)]
+
+
+class Result(C.Structure):
+    _fields_ = [("integral", C.c_double), ("sigma", C.c_double), ("chi2_dof", C.c_double), ("n_iter", C.c_uint32)]
+
+
+def make_config(cfg: dict):
+    """dict (paper_2105_10529_b200.workloads.config) -> (Config, keep-alive host PDF array)"""
+    c = Config()
+    c.struct_size = C.sizeof(Config)
+    for k in ("process", "precision", "device", "seed", "n_bins", "alpha_damp", "sqrt_s", "m_top", "alpha_s",
+              "alpha_em", "mu_f", "ptmin_g", "etamax_g", "drmin_gg", "gev2_to_pb", "pdf_xmin", "pdf_xmax",
+              "pdf_qmin", "pdf_qmax"):
+        setattr(c, k, cfg[k])
+    pdf = None
+    if cfg.get("pdf_xf") is not None:
+        pdf = np.ascontiguousarray(cfg["pdf_xf"], dtype=np.float64)
+        c.pdf_xf = pdf.ctypes.data_as(C.POINTER(C.c_double))
+        c.pdf_nx, c.pdf_nq = pdf.shape
+    return c, pdf
+
+
+_lib = None
+
+
+def lib():
+    """Load libmadflow_b200.so (built in-tree by __graft_entry__.build()); fail loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError("CUDA library %s is missing: run `python -c 'import __graft_entry__ as g; g.build()'`"
+                               " (there is no CPU fallback)" % LIB_PATH)
+        L = C.CDLL(LIB_PATH)
+        L.mf_last_error.restype = C.c_char_p
+        vp, u32, u64 = C.c_void_p, C.c_uint32, C.c_uint64
+        L.mf_vegas_create.argtypes = [C.POINTER(Config), C.POINTER(vp)]
+        L.mf_vegas_destroy.argtypes = [vp]
+        L.mf_ndim.argtypes = [vp, C.POINTER(u32), C.POINTER(u32)]
+        L.mf_integrand_eval.argtypes = [vp, u32, u64, u64, C.POINTER(EvalOut), vp]
+        L.mf_vegas_iterate.argtypes = [vp, u64, vp, C.POINTER(Iter)]
+        L.mf_vegas_accumulate.argtypes = [vp, u64, u64, u64, vp]
+        L.mf_get_accum.argtypes = [vp, vp, vp]
+        L.mf_set_accum.argtypes = [vp, vp, vp]
+        L.mf_vegas_finalize.argtypes = [vp, u64, vp, C.POINTER(Iter)]
+        L.mf_result.argtypes = [vp, C.POINTER(Result)]
+        L.mf_get_iterations.argtypes = [vp, vp, u32, C.POINTER(u32)]
+        L.mf_get_grid.argtypes = [vp, vp]
+        L.mf_set_grid.argtypes = [vp, vp]
+        L.mf_set_launch.argtypes = [vp, u32, u32]
+        L.mf_me_flops.argtypes = [vp, C.POINTER(u64), C.POINTER(u64), C.POINTER(u64)]
+        L.mf_fp64_peak.argtypes = [C.c_int32, C.c_double, C.POINTER(C.c_double)]
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != 0:
+        raise MfError(rc, lib().mf_last_error().decode())
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    return C.c_void_p(int(stream))
+
+
+class Vegas:
+    """mf_vegas_t handle.  Methods carry the names of the C calls."""
+
+    def __init__(self, cfg: dict):
+        self._cfg, self._pdf = make_config(cfg)
+        self._h = C.c_void_p()
+        _check(lib().mf_vegas_create(C.byref(self._cfg), C.byref(self._h)))
+        d, nf = C.c_uint32(), C.c_uint32()
+        _check(lib().mf_ndim(self._h, C.byref(d), C.byref(nf)))
+        self.d, self.n_final, self.n_bins = d.value, nf.value, cfg["n_bins"]
+        self.device = cfg.get("device", 0)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().mf_vegas_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def integrand_eval(self, iteration, first_event, n_events, debug=False, stream=None):
+        """mf_integrand_eval: returns a dict of torch tensors on the handle's device"""
+        import torch
+        dev = torch.device("cuda", self.device)
+        n, d, nl = int(n_events), self.d, 2 + self.n_final
+        out = dict(weight=torch.empty(n, dtype=torch.float64, device=dev))
+        if debug:
+            out.update(x=torch.empty((n, d), dtype=torch.float64, device=dev),
+                       bins=torch.empty((n, d), dtype=torch.uint8, device=dev),
+                       momenta=torch.empty((n, nl, 4), dtype=torch.float64, device=dev),
+                       me2=torch.empty(n, dtype=torch.float64, device=dev),
+                       pdf=torch.empty((n, 2), dtype=torch.float64, device=dev),
+                       pass_=torch.empty(n, dtype=torch.uint8, device=dev))
+        eo = EvalOut(**{k: (v.data_ptr() if n else None) for k, v in out.items()})
+        with torch.cuda.device(dev):
+            _check(lib().mf_integrand_eval(self._h, iteration, int(first_event), n, C.byref(eo), _stream_ptr(stream)))
+        return out
+
+    def integrand_eval_into(self, iteration, first_event, n_events, weight_ptr, stream=None):
+        """mf_integrand_eval writing only the weights to a caller-owned device pointer"""
+        eo = EvalOut(weight=weight_ptr)
+        _check(lib().mf_integrand_eval(self._h, iteration, int(first_event), int(n_events), C.byref(eo), _stream_ptr(stream)))
+
+    def vegas_iterate(self, n_events, stream=None, sync=True):
+        it = Iter()
+        _check(lib().mf_vegas_iterate(self._h, int(n_events), _stream_ptr(stream), C.byref(it) if sync else None))
+        return _iter_dict(it) if sync else None
+
+    def vegas_accumulate(self, first_event, n_events, n_total, stream=None):
+        _check(lib().mf_vegas_accumulate(self._h, int(first_event), int(n_events), int(n_total), _stream_ptr(stream)))
+
+    def get_accum(self):
+        acc = np.zeros(2 + self.d * self.n_bins); cnt = np.zeros(2, np.uint64)
+        _check(lib().mf_get_accum(self._h, acc.ctypes.data, cnt.ctypes.data))
+        return acc, cnt
+
+    def set_accum(self, acc, counts):
+        acc = np.ascontiguousarray(acc, dtype=np.float64); cnt = np.ascontiguousarray(counts, dtype=np.uint64)
+        _check(lib().mf_set_accum(self._h, acc.ctypes.data, cnt.ctypes.data))
+
+    def vegas_finalize(self, n_total, stream=None, sync=True):
+        it = Iter()
+        _check(lib().mf_vegas_finalize(self._h, int(n_total), _stream_ptr(stream), C.byref(it) if sync else None))
+        return _iter_dict(it) if sync else None
+
+    def result(self):
+        r = Result()
+        _check(lib().mf_result(self._h, C.byref(r)))
+        return dict(integral=r.integral, sigma=r.sigma, chi2_dof=r.chi2_dof, n_iter=r.n_iter)
+
+    def get_iterations(self, max_iter=1024):
+        arr = (Iter * max_iter)(); n = C.c_uint32()
+        _check(lib().mf_get_iterations(self._h, C.cast(arr, C.c_void_p), max_iter, C.byref(n)))
+        return [_iter_dict(arr[i]) for i in range(n.value)]
+
+    def get_grid(self):
+        e = np.zeros((self.d, self.n_bins + 1))
+        _check(lib().mf_get_grid(self._h, e.ctypes.data))
+        return e
+
+    def set_grid(self, edges):
+        e = np.ascontiguousarray(edges, dtype=np.float64)
+        assert e.shape == (self.d, self.n_bins + 1)
+        _check(lib().mf_set_grid(self._h, e.ctypes.data))
+
+    def set_launch(self, blocks_per_sm=0, threads_per_block=0):
+        _check(lib().mf_set_launch(self._h, blocks_per_sm, threads_per_block))
+
+    def me_flops(self):
+        a, m, f = C.c_uint64(), C.c_uint64(), C.c_uint64()
+        _check(lib().mf_me_flops(self._h, C.byref(a), C.byref(m), C.byref(f)))
+        return dict(add=a.value, mul=m.value, fma=f.value, flops=a.value + m.value + 2 * f.value)
+
+
+def _iter_dict(it):
+    return dict(integral=it.integral, sigma=it.sigma, n_events=it.n_events, n_pass=it.n_pass,
+                n_nonfinite=it.n_nonfinite, kernel_ms=it.kernel_ms)
+
+
+def fp64_peak(device=0, seconds=0.5):
+    v = C.c_double()
+    _check(lib().mf_fp64_peak(device, seconds, C.byref(v)))
+    return v.value

@@ -1,0 +1,291 @@
+// mf_device.cuh -- per-event device functions of the LO integrand path, steps S1-S8
+// ("generation of random numbers, computation of the phase space kinematics, matrix
+// element evaluation and histogram accumulation"; PAPER.md:29 PDF interpolation, phase space with
+// fiducial cuts, matrix element).  The paper prints no formulas: each function states the DESIGN.md
+// reading (O1-O8) it implements.  One event per thread, everything in registers; the VEGAS edges
+// and the PDF table are read from shared memory.
+//
+// Functions are marked MF_HD so that tests/ can compile this very file for the host with g++ and
+// check the per-event arithmetic against the oracle without a GPU (test harness only: the product
+// library has no CPU path).
+#pragma once
+#include <stdint.h>
+#include <math.h>
+
+#if defined(__CUDACC__)
+#define MF_HD __host__ __device__ __forceinline__
+#define MF_DEVFN __device__ __forceinline__
+#else
+#define MF_HD static inline
+#define MF_DEVFN static inline
+static inline void sincospi(double x, double* s, double* c) { *s = sin(M_PI * x); *c = cos(M_PI * x); }
+static inline double rsqrt(double x) { return 1.0 / sqrt(x); }
+#endif
+
+#define MF_DMAX 10          // VEGAS dimensions of the largest process (gg -> tt~gg)
+#define MF_NBMAX 64         // bins per dimension
+#define MF_PI 3.14159265358979323846
+
+// run constants of one handle (kernel parameter)
+struct MfParams {
+  int32_t process, d, n_final, nb;
+  uint32_t key0, key1;                  // Philox key = (seed lo, seed hi)        (A1)
+  double s, ltau0, m_top;               // collider s, ln(shat_min / s)            (O3)
+  double me_pref;                       // g_s^(2 ng) / 256 * generator scale, or e^4/4 (O6)
+  double ptmin, etamax, drmin;          // cuts (O7)
+  double wconst;                        // S_f * K / 2  (O8: F = ... S_f W_PS K / (2 shat))
+  double pdf_lx0, pdf_ihx, pdf_lq0, pdf_ihq, pdf_lq;   // ln xmin, 1/h_x, ln qmin^2, 1/h_q, ln muF^2
+  int32_t pdf_nx, pdf_nq;
+};
+
+// ---- S1: Philox4x32-10 (Salmon et al. SC'11), reading O1/A1 ----------------------------------
+MF_HD uint32_t mf_mulhi32(uint32_t a, uint32_t b) {
+#if defined(__CUDA_ARCH__)
+  return __umulhi(a, b);
+#else
+  return (uint32_t)(((uint64_t)a * b) >> 32);
+#endif
+}
+
+MF_HD void mf_philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1,
+                     uint32_t o[4]) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint32_t h0 = mf_mulhi32(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+    const uint32_t h1 = mf_mulhi32(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+    c0 = h1 ^ c1 ^ k0; c1 = l1; c2 = h0 ^ c3 ^ k1; c3 = l0;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  o[0] = c0; o[1] = c1; o[2] = c2; o[3] = c3;
+}
+
+// 52-bit uniform in (0,1): u = ((X >> 12) + 0.5) 2^-52, exact in fp64 (A1)
+MF_HD double mf_u52(uint32_t lo, uint32_t hi) {
+  const uint64_t X = ((uint64_t)hi << 32) | lo;
+  return ((double)(X >> 12) + 0.5) * 0x1p-52;
+}
+
+// d uniforms of event `ev`: counter = (ev lo, ev hi, block j, iteration); block j -> dims 2j, 2j+1
+template <int D>
+MF_HD void mf_uniforms(const MfParams& P, uint32_t iteration, uint64_t ev, double u[D]) {
+#pragma unroll
+  for (int j = 0; 2 * j < D; ++j) {
+    uint32_t o[4];
+    mf_philox((uint32_t)ev, (uint32_t)(ev >> 32), (uint32_t)j, iteration, P.key0, P.key1, o);
+    u[2 * j] = mf_u52(o[0], o[1]);
+    if (2 * j + 1 < D) u[2 * j + 1] = mf_u52(o[2], o[3]);
+  }
+}
+
+// ---- S2: VEGAS map (O2): k = min(floor(u nb), nb-1); y = e_k + (u nb - k) D_k; J = prod nb D_k --
+template <int D>
+MF_HD double mf_vegas_map(const double* edges, int nb, const double u[D], double y[D], int bin[D]) {
+  double J = 1.0;
+  const double dnb = (double)nb;
+#pragma unroll
+  for (int j = 0; j < D; ++j) {
+    const double* e = edges + j * (nb + 1);
+    const double t = u[j] * dnb;
+    int k = (int)t;
+    k = k > nb - 1 ? nb - 1 : k;
+    const double e0 = e[k], delta = e[k + 1] - e0;
+    y[j] = e0 + (t - (double)k) * delta;
+    bin[j] = k;
+    J *= dnb * delta;
+  }
+  return J;
+}
+
+// ---- S3: parton fractions (O3): tau = tau0^(1-y0), x1 = tau^y1, x2 = tau/x1 -------------------
+MF_HD void mf_x_map(const MfParams& P, double y0, double y1, double& x1, double& x2, double& shat,
+                    double& jx) {
+  const double ltau = (1.0 - y0) * P.ltau0;
+  const double tau = exp(ltau);
+  x1 = exp(y1 * ltau);
+  x2 = tau / x1;
+  shat = tau * P.s;
+  jx = tau * P.ltau0 * ltau;            // tau (-ln tau0)(-ln tau)
+}
+
+// ---- S4: phase space (O4): 3n-4-random sequential-decay RAMBO + massive rescaling ---------------
+// mass fraction: solve r = (k+1) w^k - k w^(k+1) for w = u^2 in (0,1), k = n - i (closed form, then
+// two Newton steps on the polynomial so that the root does not depend on acos/cos rounding)
+MF_HD double mf_mass_fraction_sq(int k, double r) {
+  double w;
+  if (k == 1) {                                   // 2w - w^2 = r
+    w = r / (1.0 + sqrt(1.0 - r));
+#pragma unroll
+    for (int it = 0; it < 2; ++it) w -= (w * (2.0 - w) - r) / (2.0 * (1.0 - w));
+  } else {                                        // 3w^2 - 2w^3 = r,  w = 1/2 + cos((2pi - acos(1-2r))/3)
+    w = 0.5 + cos((2.0 * MF_PI - acos(1.0 - 2.0 * r)) * (1.0 / 3.0));
+#pragma unroll
+    for (int it = 0; it < 2; ++it) w -= (w * w * (3.0 - 2.0 * w) - r) / (6.0 * w * (1.0 - w));
+  }
+  return w;
+}
+
+// boost p from the rest frame of Q (mass M known analytically) to the frame in which Q is given
+MF_HD void mf_boost(const double Q[4], double M, const double p[4], double out[4]) {
+  const double Ep = (Q[0] * p[0] + Q[1] * p[1] + Q[2] * p[2] + Q[3] * p[3]) / M;
+  const double f = (p[0] + Ep) / (Q[0] + M);
+  out[0] = Ep; out[1] = p[1] + Q[1] * f; out[2] = p[2] + Q[2] * f; out[3] = p[3] + Q[3] * f;
+}
+
+// W0(n, shat) = (pi/2)^(n-1) shat^(n-2) / ((n-1)!(n-2)!) (2pi)^(4-3n)
+template <int N>
+MF_HD double mf_w0(double shat) {
+  if (N == 2) return 1.0 / (8.0 * MF_PI);
+  if (N == 3) return shat / (256.0 * MF_PI * MF_PI * MF_PI);
+  return shat * shat / (24576.0 * MF_PI * MF_PI * MF_PI * MF_PI * MF_PI);
+}
+
+// rs[3N-4] -> massive momenta k[N][4] (t, t~, g...) in the partonic CM frame; returns W0 * Wm.
+// masses: m for particles 0,1 (0 for the massless 2-body case), 0 for the rest.
+template <int N>
+MF_HD double mf_phase_space(double shat, double m, const double* rs, double k[N][4]) {
+  const double rts = sqrt(shat);
+  double M[N + 1];
+  M[1] = rts; M[N] = 0.0;
+#pragma unroll
+  for (int i = 2; i + 1 <= N; ++i) M[i] = sqrt(mf_mass_fraction_sq(N - i, rs[i - 2])) * M[i - 1];
+  double Q[4] = {rts, 0.0, 0.0, 0.0};
+#pragma unroll
+  for (int i = 2; i <= N; ++i) {
+    const double ct = 2.0 * rs[N - 6 + 2 * i] - 1.0;
+    double sp, cp;
+    sincospi(2.0 * rs[N - 5 + 2 * i], &sp, &cp);
+    const double st = sqrt(1.0 - ct * ct);
+    const double q = (M[i - 1] * M[i - 1] - M[i] * M[i]) / (2.0 * M[i - 1]);
+    const double pr[4] = {q, q * st * cp, q * st * sp, q * ct};
+    const double Qr[4] = {sqrt(q * q + M[i] * M[i]), -pr[1], -pr[2], -pr[3]};
+    if (i == 2) {
+#pragma unroll
+      for (int c = 0; c < 4; ++c) { k[0][c] = pr[c]; Q[c] = Qr[c]; }
+    } else {
+      double Qn[4];
+      mf_boost(Q, M[i - 1], pr, k[i - 2]);
+      mf_boost(Q, M[i - 1], Qr, Qn);
+#pragma unroll
+      for (int c = 0; c < 4; ++c) Q[c] = Qn[c];
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < 4; ++c) k[N - 1][c] = Q[c];
+  const double W0 = mf_w0<N>(shat);
+  if (m == 0.0) return W0;
+  // massive rescaling: sum_i sqrt(m_i^2 + xi^2 E_i^2) = sqrt(shat); Newton from
+  // xi0 = sqrt(1 - (sum m / sqrt shat)^2), fixed 6 steps (A7); N = 2: xi0 is the exact root
+  const double m2 = m * m;
+  const double r0 = 2.0 * m / rts;
+  double xi = sqrt(1.0 - r0 * r0);
+  if (N > 2) {
+#pragma unroll 1
+    for (int it = 0; it < 6; ++it) {
+      double F = -rts, dF = 0.0;
+#pragma unroll
+      for (int i = 0; i < N; ++i) {
+        const double e0 = k[i][0];
+        const double E = (i < 2) ? sqrt(m2 + xi * xi * e0 * e0) : xi * e0;
+        F += E; dF += xi * e0 * e0 / E;
+      }
+      xi -= F / dF;
+    }
+  }
+  double prod = 1.0, den = 0.0;
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    const double kabs = xi * k[i][0];
+    const double E = (i < 2) ? sqrt(m2 + kabs * kabs) : kabs;
+    prod *= kabs / E; den += kabs * kabs / E;
+    k[i][0] = E; k[i][1] *= xi; k[i][2] *= xi; k[i][3] *= xi;
+  }
+  double xp = xi;                                // xi^(2N-3)
+#pragma unroll
+  for (int i = 1; i < 2 * N - 3; ++i) xp *= xi;
+  return W0 * (xp * prod * rts / den);
+}
+
+// ---- S6: PDF (O5): cubic Hermite in (ln x, ln Q^2) on the tabulated xf, node slope = mean of the
+// two secants, one-sided at the ends.  On uniform knots h*d_i = (f_{i+1}-f_{i-1})/2, so no division.
+MF_HD double mf_hermite(double fm1, double f0, double f1, double f2, bool has_m1, bool has_p2, double t) {
+  const double hd0 = has_m1 ? 0.5 * (f1 - fm1) : (f1 - f0);
+  const double hd1 = has_p2 ? 0.5 * (f2 - f0) : (f1 - f0);
+  const double t2 = t * t, t3 = t2 * t;
+  return (2.0 * t3 - 3.0 * t2 + 1.0) * f0 + (t3 - 2.0 * t2 + t) * hd0 + (3.0 * t2 - 2.0 * t3) * f1 + (t3 - t2) * hd1;
+}
+
+// xf(x, Q^2) from the table `tab` [nx][nq] (shared memory on the device); lq = ln Q^2
+MF_HD double mf_pdf(const MfParams& P, const double* tab, double x, double lq) {
+  const int nx = P.pdf_nx, nq = P.pdf_nq;
+  const double fx = (log(x) - P.pdf_lx0) * P.pdf_ihx, fq = (lq - P.pdf_lq0) * P.pdf_ihq;
+  int ix = (int)floor(fx), iq = (int)floor(fq);
+  ix = ix < 0 ? 0 : (ix > nx - 2 ? nx - 2 : ix);
+  iq = iq < 0 ? 0 : (iq > nq - 2 ? nq - 2 : iq);
+  double tx = fx - (double)ix, tq = fq - (double)iq;
+  tx = tx < 0.0 ? 0.0 : (tx > 1.0 ? 1.0 : tx);     // clamp: no extrapolation
+  tq = tq < 0.0 ? 0.0 : (tq > 1.0 ? 1.0 : tq);
+  const bool xm = ix > 0, xp = ix + 2 < nx, qm = iq > 0, qp = iq + 2 < nq;
+  const int r0 = (xm ? ix - 1 : ix) * nq, r1 = ix * nq, r2 = (ix + 1) * nq, r3 = (xp ? ix + 2 : ix + 1) * nq;
+  double row[4];
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {                     // Q^2 rows iq-1 .. iq+2 (clamped where absent)
+    int q = iq - 1 + c;
+    q = q < 0 ? 0 : (q > nq - 1 ? nq - 1 : q);
+    row[c] = mf_hermite(tab[r0 + q], tab[r1 + q], tab[r2 + q], tab[r3 + q], xm, xp, tx);
+  }
+  return mf_hermite(row[0], row[1], row[2], row[3], qm, qp, tq);
+}
+
+// ---- S5: cuts (O7): final gluons only, lab frame; eta_lab = atanh(kz/|k|) + ln(x1/x2)/2 -----------
+template <int NGL>
+MF_HD bool mf_cuts(const MfParams& P, const double kg[][4], double x1, double x2) {
+  if (NGL == 0) return true;
+  const double yb = 0.5 * log(x1 / x2);
+  bool pass = true;
+  double eta[NGL > 0 ? NGL : 1], phi[NGL > 0 ? NGL : 1];
+#pragma unroll
+  for (int i = 0; i < NGL; ++i) {
+    const double pt2 = kg[i][1] * kg[i][1] + kg[i][2] * kg[i][2];
+    const double pt = sqrt(pt2), kabs = sqrt(pt2 + kg[i][3] * kg[i][3]);
+    eta[i] = atanh(kg[i][3] / kabs) + yb;
+    if (P.ptmin > 0.0 && !(pt > P.ptmin)) pass = false;
+    if (P.etamax > 0.0 && !(fabs(eta[i]) < P.etamax)) pass = false;
+  }
+  if (NGL == 2 && P.drmin > 0.0) {
+    phi[0] = atan2(kg[0][2], kg[0][1]);
+    phi[1] = atan2(kg[1][2], kg[1][1]);
+    double dphi = phi[0] - phi[1];
+    if (dphi > MF_PI) dphi -= 2.0 * MF_PI;
+    if (dphi <= -MF_PI) dphi += 2.0 * MF_PI;
+    const double deta = eta[0] - eta[1];
+    if (!(sqrt(deta * deta + dphi * dphi) > P.drmin)) pass = false;
+  }
+  return pass;
+}
+
+// ---- S7a: external-wavefunction ingredients (O6.2), the "conditional control statements" of
+// PAPER.md:69.  Fermion: w+ = sqrt(E+|p|), w- = m/w+, and N*(|p|+pz, px, py) of the two-spinors
+// chi+ = N(|p|+pz, px+i py), chi- = N(-px+i py, |p|+pz); the generated code builds u, v from them.
+MF_HD void mf_fermion_ing(const double p[4], double m, double o[5]) {
+  const double pt2 = p[1] * p[1] + p[2] * p[2];
+  const double pabs = sqrt(pt2 + p[3] * p[3]);
+  o[0] = sqrt(p[0] + pabs);
+  o[1] = (m == 0.0) ? 0.0 : m / o[0];
+  if (pabs < 1e-12 * fabs(p[0]) || (pt2 == 0.0 && p[3] < 0.0)) {   // pz = -|p| branch
+    o[2] = 0.0; o[3] = 1.0; o[4] = 0.0;
+  } else {
+    const double ppz = (p[3] >= 0.0) ? pabs + p[3] : pt2 / (pabs - p[3]);   // no cancellation
+    const double N = rsqrt(2.0 * pabs * ppz);
+    o[2] = N * ppz; o[3] = N * p[1]; o[4] = N * p[2];
+  }
+}
+// Gluon: eps(k,lam) = (-lam eps1 - i eps2)/sqrt2; o = (eps1x, eps1y, eps1z, eps2x, eps2y)/sqrt2
+MF_HD void mf_gluon_ing(const double k[4], double o[5]) {
+  const double pt2 = k[1] * k[1] + k[2] * k[2];
+  const double r2 = 0.70710678118654752440;
+  if (pt2 == 0.0) { o[0] = r2; o[1] = 0.0; o[2] = 0.0; o[3] = 0.0; o[4] = (k[3] >= 0.0) ? r2 : -r2; return; }
+  const double pt = sqrt(pt2), kabs = sqrt(pt2 + k[3] * k[3]);
+  const double ipt = r2 / pt, ik = 1.0 / kabs;
+  o[0] = k[1] * k[3] * ipt * ik; o[1] = k[2] * k[3] * ipt * ik; o[2] = -pt * ik * r2;
+  o[3] = -k[2] * ipt; o[4] = k[1] * ipt;
+}

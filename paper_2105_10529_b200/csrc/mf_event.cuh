@@ -1,0 +1,111 @@
+// mf_event.cuh -- one event, S1 -> S8 (PAPER.md:59 pipeline), for the four processes of
+// BASELINE.json configs 0-3.  Returns F = w*f (pb), the weight before the 1/N (reading O8):
+//   config 0   : F = J_V |M|^2 (1/(8 pi)) K / (2 s)
+//   configs 1-3: F = J_V J_x f_g(x1) f_g(x2) |M|^2 S_f W_0 W_m Theta_cuts K / (2 shat)
+#pragma once
+#include "mf_device.cuh"
+#include "generated/mf_me2_ee_mumu.cuh"
+#include "generated/mf_me2_gg_tt.cuh"
+#include "generated/mf_me2_gg_ttg.cuh"
+#include "generated/mf_me2_gg_ttgg.cuh"
+
+template <int PROC> struct MfProc;
+template <> struct MfProc<0> { static const int D = 2, N = 2, NGL = 0; };
+template <> struct MfProc<1> { static const int D = 4, N = 2, NGL = 0; };
+template <> struct MfProc<2> { static const int D = 7, N = 3, NGL = 1; };
+template <> struct MfProc<3> { static const int D = 10, N = 4, NGL = 2; };
+
+// optional per-event record (mf_integrand_eval's debug outputs)
+struct MfEventRec {
+  double y[MF_DMAX];
+  double mom[6][4];
+  double me2, pdf[2];
+  int pass;
+};
+
+// inputs of the generated gg -> t t~ + gluons code: [E, mt, p3, p4, t-ingredients, t~-ingredients,
+// then for every final gluon: k, polarisation ingredients] (order fixed by gen/amplitudes.py)
+template <int N>
+MF_HD void mf_me_inputs_gg(double rts, double mt, const double k[N][4], double* in) {
+  in[0] = 0.5 * rts; in[1] = mt;
+#pragma unroll
+  for (int c = 0; c < 4; ++c) { in[2 + c] = k[0][c]; in[6 + c] = k[1][c]; }
+  mf_fermion_ing(k[0], mt, in + 10);
+  mf_fermion_ing(k[1], mt, in + 15);
+#pragma unroll
+  for (int g = 2; g < N; ++g) {
+#pragma unroll
+    for (int c = 0; c < 4; ++c) in[20 + 9 * (g - 2) + c] = k[g][c];
+    mf_gluon_ing(k[g], in + 24 + 9 * (g - 2));
+  }
+}
+
+template <int PROC>
+MF_HD double mf_me2(const MfParams& P, double rts, const double k[MfProc<PROC>::N][4]) {
+  if (PROC == 0) {
+    static_assert(MF_ME2_EE_MUMU_NIN == 20, "generator input layout changed");
+    double in[20];
+    const double E = 0.5 * rts;
+    const double pa[4] = {E, 0.0, 0.0, E}, pb[4] = {E, 0.0, 0.0, -E};
+    mf_fermion_ing(pa, 0.0, in); mf_fermion_ing(pb, 0.0, in + 5);
+    mf_fermion_ing(k[0], 0.0, in + 10); mf_fermion_ing(k[1], 0.0, in + 15);
+    return P.me_pref * mf_me2_ee_mumu(in) / (rts * rts * rts * rts);      // e^4/4 * sum |L.R|^2 / s^2
+  } else if (PROC == 1) {
+    static_assert(MF_ME2_GG_TT_NIN == 20, "generator input layout changed");
+    double in[20];
+    mf_me_inputs_gg<2>(rts, P.m_top, (const double(*)[4])k, in);
+    return P.me_pref * mf_me2_gg_tt(in);
+  } else if (PROC == 2) {
+    static_assert(MF_ME2_GG_TTG_NIN == 29, "generator input layout changed");
+    double in[29];
+    mf_me_inputs_gg<3>(rts, P.m_top, (const double(*)[4])k, in);
+    return P.me_pref * mf_me2_gg_ttg(in);
+  } else {
+    static_assert(MF_ME2_GG_TTGG_NIN == 38, "generator input layout changed");
+    double in[38];
+    mf_me_inputs_gg<4>(rts, P.m_top, (const double(*)[4])k, in);
+    return P.me_pref * mf_me2_gg_ttgg(in);
+  }
+}
+
+// One event.  edges: [d][nb+1], pdf_tab: [nx][nq] (both in shared memory on the device).
+// bin[] receives the VEGAS bins (needed by the histogram); rec (nullable) the debug record.
+template <int PROC, bool REC>
+MF_HD double mf_event(const MfParams& P, const double* edges, const double* pdf_tab,
+                      uint32_t iteration, uint64_t ev, int bin[MfProc<PROC>::D], bool& pass,
+                      MfEventRec* rec) {
+  constexpr int D = MfProc<PROC>::D, N = MfProc<PROC>::N, NGL = MfProc<PROC>::NGL;
+  double u[D], y[D];
+  mf_uniforms<D>(P, iteration, ev, u);                                   // S1
+  const double JV = mf_vegas_map<D>(edges, P.nb, u, y, bin);             // S2
+  double x1 = 1.0, x2 = 1.0, shat = P.s, jx = 1.0;
+  if (PROC != 0) mf_x_map(P, y[0], y[1], x1, x2, shat, jx);              // S3
+  double k[N][4];
+  const double wps = mf_phase_space<N>(shat, PROC == 0 ? 0.0 : P.m_top, y + (PROC == 0 ? 0 : 2), k);   // S4
+  const double rts = sqrt(shat);
+  pass = mf_cuts<NGL>(P, (const double(*)[4])(&k[0][0] + 8), x1, x2);   // S5 (final gluons = k[2..])
+  double f1 = 1.0, f2 = 1.0, xf1 = 0.0, xf2 = 0.0;
+  if (PROC != 0) {                                                       // S6
+    xf1 = mf_pdf(P, pdf_tab, x1, P.pdf_lq);
+    xf2 = mf_pdf(P, pdf_tab, x2, P.pdf_lq);
+    f1 = xf1 / x1; f2 = xf2 / x2;
+  }
+  double me2 = 0.0, F = 0.0;
+  if (pass) {
+    me2 = mf_me2<PROC>(P, rts, k);                                       // S7
+    F = JV * jx * f1 * f2 * me2 * wps * P.wconst / shat;                 // S8
+  }
+  if (REC) {
+#pragma unroll
+    for (int j = 0; j < D; ++j) rec->y[j] = y[j];
+    const double E = 0.5 * rts;
+    rec->mom[0][0] = E; rec->mom[0][1] = 0.0; rec->mom[0][2] = 0.0; rec->mom[0][3] = E;
+    rec->mom[1][0] = E; rec->mom[1][1] = 0.0; rec->mom[1][2] = 0.0; rec->mom[1][3] = -E;
+#pragma unroll
+    for (int i = 0; i < N; ++i)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) rec->mom[2 + i][c] = k[i][c];
+    rec->me2 = me2; rec->pdf[0] = xf1; rec->pdf[1] = xf2; rec->pass = pass ? 1 : 0;
+  }
+  return F;
+}

@@ -1,0 +1,66 @@
+// mf_params.h -- host-side validation of mf_config_t and derivation of the kernel constants
+// (MfParams).  Used by the C-ABI (mf_api.cu); the test harness includes it as well.
+#pragma once
+#include "../../include/madflow_b200.h"
+#include "mf_event.cuh"
+#include <string>
+
+static inline int mf_process_shape(int process, int* d, int* n_final, int* ng) {
+  static const int nf[4] = {2, 2, 3, 4};
+  if (process < 0 || process > 3) return -1;
+  *n_final = nf[process];
+  *d = (process == MF_EE_MUMU) ? 2 : 2 + 3 * nf[process] - 4;
+  *ng = (process == MF_EE_MUMU) ? 0 : nf[process];      // gluon legs of gg -> t t~ + (n_final-2) g
+  return 0;
+}
+
+// returns MF_OK or MF_EINVAL / MF_EUNSUPPORTED with a message in err
+static inline int mf_fill_params(const mf_config_t* c, MfParams* P, std::string& err) {
+  if (!c) { err = "cfg is NULL"; return MF_EINVAL; }
+  if (c->struct_size != sizeof(mf_config_t)) { err = "struct_size mismatch (ABI)"; return MF_EINVAL; }
+  int d, nfin, ng;
+  if (mf_process_shape(c->process, &d, &nfin, &ng)) { err = "unknown process"; return MF_EINVAL; }
+  if (c->precision != 64) { err = "only precision 64 is built"; return MF_EUNSUPPORTED; }
+  if (c->n_bins < 1 || c->n_bins > MF_NBMAX) { err = "n_bins must be in 1..64"; return MF_EINVAL; }
+  if (!(c->sqrt_s > 0.0)) { err = "sqrt_s must be positive"; return MF_EINVAL; }
+  if (!(c->alpha_damp >= 0.0)) { err = "alpha_damp must be >= 0"; return MF_EINVAL; }
+  if (!(c->gev2_to_pb > 0.0)) { err = "gev2_to_pb must be positive"; return MF_EINVAL; }
+  MfParams p = {};
+  p.process = c->process; p.d = d; p.n_final = nfin; p.nb = (int)c->n_bins;
+  p.key0 = (uint32_t)c->seed; p.key1 = (uint32_t)(c->seed >> 32);
+  p.s = c->sqrt_s * c->sqrt_s; p.m_top = c->m_top;
+  p.ptmin = c->ptmin_g; p.etamax = c->etamax_g; p.drmin = c->drmin_gg;
+  const double PI = 3.14159265358979323846;
+  if (c->process == MF_EE_MUMU) {
+    if (!(c->alpha_em > 0.0)) { err = "alpha_em must be positive"; return MF_EINVAL; }
+    const double e2 = 4.0 * PI * c->alpha_em;
+    p.me_pref = e2 * e2 * MF_ME2_EE_MUMU_SCALE;         // e^4 / 4 (spin average, A12)
+    p.wconst = c->gev2_to_pb / 2.0;
+    p.ltau0 = 0.0;
+  } else {
+    if (!(c->m_top > 0.0) || !(c->alpha_s > 0.0)) { err = "m_top and alpha_s must be positive"; return MF_EINVAL; }
+    if (!c->pdf_xf || c->pdf_nx < 2 || c->pdf_nq < 2) { err = "pdf grid required"; return MF_EINVAL; }
+    if ((uint64_t)c->pdf_nx * c->pdf_nq * 8ull > 160ull * 1024ull) { err = "pdf grid larger than 160 KB"; return MF_EINVAL; }
+    if (!(c->pdf_xmin > 0.0 && c->pdf_xmax > c->pdf_xmin && c->pdf_qmin > 0.0 && c->pdf_qmax > c->pdf_qmin)) { err = "bad pdf ranges"; return MF_EINVAL; }
+    const int ngl = nfin - 2;
+    const double thr = 2.0 * c->m_top + ngl * (c->ptmin_g > 0.0 ? c->ptmin_g : 0.0);   // O3: shat_min
+    const double tau0 = thr * thr / p.s;
+    if (!(tau0 < 1.0) || tau0 < c->pdf_xmin || c->mu_f < c->pdf_qmin || c->mu_f > c->pdf_qmax) {
+      err = "kinematics outside the PDF grid"; return MF_EINVAL;
+    }
+    p.ltau0 = log(tau0);
+    double gs2n = 1.0;
+    for (int i = 0; i < ng; ++i) gs2n *= 4.0 * PI * c->alpha_s;
+    const double scale = (c->process == MF_GG_TT) ? MF_ME2_GG_TT_SCALE : (c->process == MF_GG_TTG) ? MF_ME2_GG_TTG_SCALE : MF_ME2_GG_TTGG_SCALE;
+    p.me_pref = gs2n / 256.0 * scale;                   // 1/4 helicities x 1/64 colours (A12)
+    p.wconst = (ngl == 2 ? 0.5 : 1.0) * c->gev2_to_pb / 2.0;
+    p.pdf_nx = (int)c->pdf_nx; p.pdf_nq = (int)c->pdf_nq;
+    p.pdf_lx0 = log(c->pdf_xmin);
+    p.pdf_ihx = (double)(c->pdf_nx - 1) / (log(c->pdf_xmax) - p.pdf_lx0);
+    p.pdf_lq0 = log(c->pdf_qmin * c->pdf_qmin);
+    p.pdf_ihq = (double)(c->pdf_nq - 1) / (log(c->pdf_qmax * c->pdf_qmax) - p.pdf_lq0);
+    p.pdf_lq = log(c->mu_f * c->mu_f);
+  }
+  *P = p;
+  return MF_OK;
+}

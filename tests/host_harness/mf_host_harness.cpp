@@ -1,0 +1,36 @@
+// TEST HARNESS ONLY (never part of the product library): compiles the product's per-event device
+// functions (csrc/mf_event.cuh, including the generated |M|^2 code) for the host with g++, so that
+// the CPU test-suite can check that arithmetic event by event against the oracle without a GPU.
+#include "../../paper_2105_10529_b200/csrc/mf_event.cuh"
+#include "../../paper_2105_10529_b200/csrc/mf_params.h"
+#include <cstring>
+
+template <int PROC>
+static double run(const MfParams& P, const double* edges, const double* pdf, uint32_t it, uint64_t ev,
+                  int* bins, int* pass, double* rec_out) {
+  int bin[MfProc<PROC>::D]; bool ok; MfEventRec rec;
+  std::memset(&rec, 0, sizeof rec);
+  double F = mf_event<PROC, true>(P, edges, pdf, it, ev, bin, ok, &rec);
+  for (int j = 0; j < MfProc<PROC>::D; ++j) bins[j] = bin[j];
+  *pass = ok;
+  // rec_out: y[10], mom[24], me2, pdf[2]
+  std::memcpy(rec_out, rec.y, sizeof(double) * 10);
+  std::memcpy(rec_out + 10, rec.mom, sizeof(double) * 24);
+  rec_out[34] = rec.me2; rec_out[35] = rec.pdf[0]; rec_out[36] = rec.pdf[1];
+  return F;
+}
+
+extern "C" double mfh_event(const MfParams* P, const double* edges, const double* pdf, uint32_t it,
+                            uint64_t ev, int* bins, int* pass, double* rec_out) {
+  switch (P->process) {
+    case 0: return run<0>(*P, edges, pdf, it, ev, bins, pass, rec_out);
+    case 1: return run<1>(*P, edges, pdf, it, ev, bins, pass, rec_out);
+    case 2: return run<2>(*P, edges, pdf, it, ev, bins, pass, rec_out);
+#ifndef MFH_NO_TTGG
+    case 3: return run<3>(*P, edges, pdf, it, ev, bins, pass, rec_out);
+#endif
+  }
+  return -1.0;
+}
+extern "C" int mfh_params_size(void) { return (int)sizeof(MfParams); }
+extern "C" int mfh_fill_params(const mf_config_t* c, MfParams* P) { std::string e; return mf_fill_params(c, P, e); }

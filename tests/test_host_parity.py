@@ -1,0 +1,66 @@
+"""CPU check of the product's per-event arithmetic (csrc/mf_event.cuh + generated |M|^2 code),
+compiled for the host by tests/host_harness (test harness only), against the oracle, event by
+event on the same seeded inputs.  The GPU parity tests proper are in test_gpu_parity.py."""
+import ctypes as C
+import os
+import subprocess
+import numpy as np
+import pytest
+
+from paper_2105_10529_b200 import workloads as W
+from paper_2105_10529_b200.binding import Config, make_config
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+SRC = os.path.join(ROOT, "tests", "host_harness", "mf_host_harness.cpp")
+LIB = os.path.join(ROOT, "tests", "host_harness", "libmfh.so")
+
+
+@pytest.fixture(scope="module")
+def harness():
+    from paper_2105_10529_b200.gen.__main__ import main as gen_main
+    gen_main()
+    deps = [SRC] + [os.path.join(ROOT, "paper_2105_10529_b200", "csrc", f) for f in ("mf_event.cuh", "mf_device.cuh", "mf_params.h")]
+    if not os.path.exists(LIB) or any(os.path.getmtime(LIB) < os.path.getmtime(p) for p in deps):
+        subprocess.check_call(["g++", "-O1", "-std=c++17", "-fPIC", "-shared", "-o", LIB, SRC])
+    lib = C.CDLL(LIB)
+    lib.mfh_event.restype = C.c_double
+    lib.mfh_event.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.mfh_fill_params.argtypes = [C.POINTER(Config), C.c_void_p]
+    return lib
+
+
+def random_grid(d, nb, seed):
+    rng = np.random.default_rng(seed)
+    w = rng.uniform(0.3, 1.7, size=(d, nb))
+    e = np.concatenate([np.zeros((d, 1)), np.cumsum(w, axis=1) / w.sum(axis=1, keepdims=True)], axis=1)
+    e[:, -1] = 1.0
+    return e
+
+
+@pytest.mark.parametrize("proc,n,tol", [(0, 300, 1e-12), (1, 300, 1e-11), (2, 300, 1e-10), (3, 40, 1e-10)])
+def test_host_compiled_event_matches_oracle(mfo, harness, proc, n, tol):
+    cfg = W.config(proc, seed=7)
+    c, pdf = make_config(cfg)
+    P = C.create_string_buffer(harness.mfh_params_size())
+    assert harness.mfh_fill_params(C.byref(c), P) == 0
+    orc = mfo.Vegas(cfg)
+    edges = random_grid(orc.d, 50, 11 + proc)
+    orc.set_grid(edges)
+    ref = orc.eval(2, 1000, n)
+    d, nl = orc.d, 2 + orc.n_final
+    bins = np.zeros(16, np.int32); ok = np.zeros(1, np.int32); rec = np.zeros(37)
+    worst = 0.0
+    for i in range(n):
+        F = harness.mfh_event(P, edges.ctypes.data, pdf.ctypes.data if pdf is not None else None, 2, 1000 + i,
+                              bins.ctypes.data, ok.ctypes.data, rec.ctypes.data)
+        assert list(bins[:d]) == list(ref["bins"][i])
+        assert ok[0] == ref["pass_"][i]
+        np.testing.assert_allclose(rec[:d], ref["x"][i], rtol=1e-14, atol=0)
+        np.testing.assert_allclose(rec[10:10 + 4 * nl].reshape(nl, 4), ref["momenta"][i], rtol=1e-11, atol=1e-9)
+        if proc:
+            np.testing.assert_allclose(rec[35:37], ref["pdf"][i], rtol=1e-12, atol=1e-15)   # interpolant ~0 near x -> 1: absolute
+        if ref["weight"][i] != 0:
+            worst = max(worst, abs(F / ref["weight"][i] - 1), abs(rec[34] / ref["me2"][i] - 1))
+        else:
+            assert F == 0.0
+    assert worst < tol, worst

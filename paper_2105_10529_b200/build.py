@@ -1,0 +1,55 @@
+"""In-tree build of libmadflow_b200.so for sm_100a: run the amplitude generator, compile the C-ABI
+and the four per-process kernel objects in parallel with nvcc, link.  `python -m
+paper_2105_10529_b200.build [--force]`."""
+import os
+import subprocess
+import sys
+from concurrent.futures import ThreadPoolExecutor
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
+LIB = os.path.join(HERE, "libmadflow_b200.so")
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+              "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+
+
+def _newer(target, deps):
+    return os.path.exists(target) and all(os.path.getmtime(target) >= os.path.getmtime(d) for d in deps)
+
+
+def build(force=False, verbose=False):
+    from .gen.__main__ import main as gen_main
+    gen_main()
+    os.makedirs(OBJ, exist_ok=True)
+    hdrs = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cuh", ".h"))]
+    hdrs += [os.path.join(CSRC, "generated", f) for f in os.listdir(os.path.join(CSRC, "generated"))]
+    hdrs += [os.path.join(os.path.dirname(HERE), "include", "madflow_b200.h"), os.path.abspath(__file__)]
+    jobs = [("mf_api.o", os.path.join(CSRC, "mf_api.cu"), [])]
+    jobs += [("mf_proc%d.o" % p, os.path.join(CSRC, "mf_proc.cu"), ["-DMF_PROC=%d" % p]) for p in range(4)]
+
+    def compile_one(job):
+        obj, src, extra = job
+        out = os.path.join(OBJ, obj)
+        if not force and _newer(out, hdrs + [src]):
+            return obj, "up to date"
+        r = subprocess.run(["nvcc"] + NVCC_FLAGS + extra + ["-c", src, "-o", out], capture_output=True, text=True)
+        with open(out + ".log", "w") as f:
+            f.write(r.stdout + r.stderr)
+        if r.returncode != 0:
+            raise RuntimeError("nvcc failed for %s:\n%s" % (obj, (r.stdout + r.stderr)[-4000:]))
+        return obj, "compiled"
+
+    with ThreadPoolExecutor(max_workers=5) as ex:
+        results = list(ex.map(compile_one, jobs))
+    objs = [os.path.join(OBJ, j[0]) for j in jobs]
+    if force or not _newer(LIB, objs):
+        subprocess.check_call(["nvcc", "-shared", "-o", LIB] + objs + ["-gencode", "arch=compute_100a,code=sm_100a"])
+    if verbose:
+        for obj, what in results:
+            print(obj, what)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose=True))

@@ -1,0 +1,328 @@
+// mf_api.cu -- the C-ABI of include/madflow_b200.h: handle management and kernel launches.
+// Host code only validates, allocates and enqueues; every step of the path runs in the kernels of
+// mf_kernels.cuh.  No CPU fallback: without a device every compute call returns MF_ECUDA.
+#include "../../include/madflow_b200.h"
+#include "mf_small_kernels.cuh"
+#include "mf_proc.h"
+#include "mf_params.h"
+#include <string>
+#include <vector>
+#include <new>
+#include <cstring>
+#include <cstdio>
+
+static thread_local std::string g_err;
+extern "C" const char* mf_last_error(void) { return g_err.c_str(); }
+
+static int fail(int code, const std::string& msg) { g_err = msg; return code; }
+#define MF_CUDA(call)                                                                              \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess) return fail(MF_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); \
+  } while (0)
+
+struct mf_vegas {
+  mf_config_t cfg;
+  MfParams P;
+  int device, n_sm;
+  int na;                              // 2 + d*nb
+  size_t smem_iter, smem_eval;
+  int occ_iter, occ_eval;              // resident blocks per SM of the two kernels
+  uint32_t blocks_per_sm, threads;     // user override (0 = default)
+  int max_blocks;
+  double *d_edges, *d_pdf, *d_partial, *d_acc;
+  unsigned long long *d_pcount, *d_counts;
+  MfDevState* d_state;
+  const MfProcOps* ops;               // per-process kernels (one translation unit each)
+  uint32_t iteration;                  // iterations finalized so far (= Philox counter word 3)
+  cudaStream_t last_stream;
+  cudaEvent_t ev0, ev1;
+  bool timing_armed;
+};
+
+static size_t iter_smem_bytes(const MfParams& P, int threads) {
+  const int nw = threads / 32;
+  return sizeof(double) * ((size_t)P.d * (P.nb + 1) + (size_t)P.pdf_nx * P.pdf_nq + (size_t)nw * P.d * P.nb + (size_t)nw * 4);
+}
+
+extern "C" int mf_vegas_create(const mf_config_t* cfg, mf_vegas_t** out) {
+  if (!out) return fail(MF_EINVAL, "out is NULL");
+  *out = nullptr;
+  MfParams P;
+  std::string err;
+  int rc = mf_fill_params(cfg, &P, err);
+  if (rc) return fail(rc, err);
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+    return fail(MF_ECUDA, "no CUDA device (this library has no CPU path)");
+  if (cfg->device < 0 || cfg->device >= ndev) return fail(MF_EINVAL, "device ordinal out of range");
+  mf_vegas* h = new (std::nothrow) mf_vegas();
+  if (!h) return fail(MF_ENOMEM, "host allocation failed");
+  std::memset(h, 0, sizeof *h);
+  h->cfg = *cfg; h->cfg.pdf_xf = nullptr; h->P = P; h->device = cfg->device;
+  h->na = 2 + P.d * P.nb;
+#define MF_CREATE_CUDA(call)                                                     \
+  do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { std::string m_ = std::string(#call) + ": " + cudaGetErrorString(e_); mf_vegas_destroy(h); return fail(MF_ECUDA, m_); } } while (0)
+  MF_CREATE_CUDA(cudaSetDevice(h->device));
+  MF_CREATE_CUDA(cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device));
+  h->smem_iter = iter_smem_bytes(P, MF_THREADS);
+  h->smem_eval = sizeof(double) * ((size_t)P.d * (P.nb + 1) + (size_t)P.pdf_nx * P.pdf_nq);
+  h->ops = mf_proc_ops(P.process);
+  MF_CREATE_CUDA(h->ops->setup(h->smem_iter, h->smem_eval, &h->occ_iter, &h->occ_eval));
+  if (h->occ_iter < 1 || h->occ_eval < 1) { mf_vegas_destroy(h); return fail(MF_ECUDA, "kernel does not fit on an SM"); }
+  h->max_blocks = h->n_sm * 32;
+  const size_t ne = (size_t)P.d * (P.nb + 1), npdf = (size_t)P.pdf_nx * P.pdf_nq;
+  MF_CREATE_CUDA(cudaMalloc(&h->d_edges, ne * sizeof(double)));
+  MF_CREATE_CUDA(cudaMalloc(&h->d_pdf, (npdf ? npdf : 1) * sizeof(double)));
+  MF_CREATE_CUDA(cudaMalloc(&h->d_partial, (size_t)h->max_blocks * h->na * sizeof(double)));
+  MF_CREATE_CUDA(cudaMalloc(&h->d_pcount, (size_t)h->max_blocks * 2 * sizeof(unsigned long long)));
+  MF_CREATE_CUDA(cudaMalloc(&h->d_acc, h->na * sizeof(double)));
+  MF_CREATE_CUDA(cudaMalloc(&h->d_counts, 2 * sizeof(unsigned long long)));
+  MF_CREATE_CUDA(cudaMalloc(&h->d_state, sizeof(MfDevState)));
+  MF_CREATE_CUDA(cudaMemset(h->d_state, 0, sizeof(MfDevState)));
+  MF_CREATE_CUDA(cudaMemset(h->d_acc, 0, h->na * sizeof(double)));
+  MF_CREATE_CUDA(cudaMemset(h->d_counts, 0, 2 * sizeof(unsigned long long)));
+  std::vector<double> e(ne);
+  for (int j = 0; j < P.d; ++j)
+    for (int k = 0; k <= P.nb; ++k) e[(size_t)j * (P.nb + 1) + k] = (double)k / (double)P.nb;
+  MF_CREATE_CUDA(cudaMemcpy(h->d_edges, e.data(), ne * sizeof(double), cudaMemcpyHostToDevice));
+  if (npdf) MF_CREATE_CUDA(cudaMemcpy(h->d_pdf, cfg->pdf_xf, npdf * sizeof(double), cudaMemcpyHostToDevice));
+  MF_CREATE_CUDA(cudaEventCreate(&h->ev0));
+  MF_CREATE_CUDA(cudaEventCreate(&h->ev1));
+  *out = h;
+  return MF_OK;
+}
+
+extern "C" int mf_vegas_destroy(mf_vegas_t* h) {
+  if (!h) return MF_OK;
+  cudaSetDevice(h->device);
+  cudaFree(h->d_edges); cudaFree(h->d_pdf); cudaFree(h->d_partial); cudaFree(h->d_pcount);
+  cudaFree(h->d_acc); cudaFree(h->d_counts); cudaFree(h->d_state);
+  if (h->ev0) cudaEventDestroy(h->ev0);
+  if (h->ev1) cudaEventDestroy(h->ev1);
+  delete h;
+  return MF_OK;
+}
+
+extern "C" int mf_ndim(const mf_vegas_t* h, uint32_t* d, uint32_t* n_final) {
+  if (!h) return fail(MF_EINVAL, "handle is NULL");
+  if (d) *d = (uint32_t)h->P.d;
+  if (n_final) *n_final = (uint32_t)h->P.n_final;
+  return MF_OK;
+}
+
+extern "C" int mf_set_launch(mf_vegas_t* h, uint32_t blocks_per_sm, uint32_t threads_per_block) {
+  if (!h) return fail(MF_EINVAL, "handle is NULL");
+  if (threads_per_block != 0 && threads_per_block != MF_THREADS)
+    return fail(MF_EINVAL, "threads_per_block must be 0 or 128 in this build");
+  if (blocks_per_sm > 32) return fail(MF_EINVAL, "blocks_per_sm must be <= 32");
+  h->blocks_per_sm = blocks_per_sm; h->threads = threads_per_block;
+  return MF_OK;
+}
+
+static int grid_for(const mf_vegas* h, unsigned long long n, int occ) {
+  const int per_sm = h->blocks_per_sm ? (int)h->blocks_per_sm : occ;
+  unsigned long long want = (n + MF_THREADS - 1) / MF_THREADS;
+  unsigned long long cap = (unsigned long long)h->n_sm * per_sm;     // whole waves of resident CTAs
+  if (cap > (unsigned long long)h->max_blocks) cap = h->max_blocks;
+  unsigned long long g = want < cap ? want : cap;
+  return (int)(g ? g : 1);
+}
+
+extern "C" int mf_integrand_eval(mf_vegas_t* h, uint32_t iteration, uint64_t first_event, uint64_t n_events,
+                                 const mf_eval_out_t* out, void* cuda_stream) {
+  if (!h || !out) return fail(MF_EINVAL, "null argument");
+  if (n_events == 0) return MF_OK;
+  if (!out->weight && !out->x && !out->bins && !out->momenta && !out->me2 && !out->pdf && !out->pass)
+    return fail(MF_EINVAL, "no output buffer requested");
+  MF_CUDA(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  MfEvalOutDev o = {out->weight, out->x, out->bins, out->momenta, out->me2, out->pdf, out->pass};
+  const bool rec = out->x || out->momenta || out->me2 || out->pdf;
+  MF_CUDA(h->ops->eval(h->P, h->d_edges, h->d_pdf, iteration, first_event, n_events, o, rec,
+                       grid_for(h, n_events, h->occ_eval), h->smem_eval, st));
+  h->last_stream = st;
+  return MF_OK;
+}
+
+extern "C" int mf_vegas_accumulate(mf_vegas_t* h, uint64_t first_event, uint64_t n_events, uint64_t n_total,
+                                   void* cuda_stream) {
+  if (!h) return fail(MF_EINVAL, "handle is NULL");
+  if (n_total < 2 || n_events > n_total || first_event > n_total - n_events)
+    return fail(MF_EINVAL, "event range outside the iteration");
+  if (n_events == 0) return MF_OK;
+  MF_CUDA(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int grid = grid_for(h, n_events, h->occ_iter);
+  MF_CUDA(h->ops->iterate(h->P, h->d_edges, h->d_pdf, h->iteration, first_event, n_events, (double)n_total,
+                          h->d_partial, h->d_pcount, grid, h->smem_iter, st));
+  mf_reduce_kernel<<<(h->na + 127) / 128, 128, 0, st>>>(h->d_partial, h->d_pcount, grid, h->na, h->d_acc, h->d_counts);
+  MF_CUDA(cudaGetLastError());
+  h->last_stream = st;
+  return MF_OK;
+}
+
+static int fetch_iter(mf_vegas* h, uint32_t idx, mf_iter_t* o) {
+  MfDevState* s = h->d_state;
+  MF_CUDA(cudaMemcpy(&o->integral, &s->it_I[idx], sizeof(double), cudaMemcpyDeviceToHost));
+  MF_CUDA(cudaMemcpy(&o->sigma, &s->it_sig[idx], sizeof(double), cudaMemcpyDeviceToHost));
+  unsigned long long v[3];
+  MF_CUDA(cudaMemcpy(&v[0], &s->it_n[idx], sizeof(v[0]), cudaMemcpyDeviceToHost));
+  MF_CUDA(cudaMemcpy(&v[1], &s->it_pass[idx], sizeof(v[0]), cudaMemcpyDeviceToHost));
+  MF_CUDA(cudaMemcpy(&v[2], &s->it_bad[idx], sizeof(v[0]), cudaMemcpyDeviceToHost));
+  o->n_events = v[0]; o->n_pass = v[1]; o->n_nonfinite = v[2]; o->kernel_ms = 0.0f;
+  return MF_OK;
+}
+
+extern "C" int mf_vegas_finalize(mf_vegas_t* h, uint64_t n_total, void* cuda_stream, mf_iter_t* host_out) {
+  if (!h) return fail(MF_EINVAL, "handle is NULL");
+  if (n_total < 2) return fail(MF_EINVAL, "an iteration needs at least 2 events");
+  if (h->iteration >= MF_MAX_ITER) return fail(MF_ESTATE, "too many iterations (1024)");
+  MF_CUDA(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  mf_finalize_kernel<<<1, 32, 0, st>>>(h->P, h->cfg.alpha_damp, (double)n_total, n_total, h->d_acc, h->d_counts,
+                                        h->d_edges, h->d_state);
+  MF_CUDA(cudaGetLastError());
+  // the raw sums stay readable (mf_get_accum) until the next iteration starts
+  const uint32_t idx = h->iteration++;
+  h->last_stream = st;
+  if (host_out) {
+    float ms = 0.0f;
+    if (h->timing_armed) { MF_CUDA(cudaEventRecord(h->ev1, st)); }
+    MF_CUDA(cudaStreamSynchronize(st));
+    if (h->timing_armed) { MF_CUDA(cudaEventElapsedTime(&ms, h->ev0, h->ev1)); }
+    int rc = fetch_iter(h, idx, host_out);
+    if (rc) return rc;
+    host_out->kernel_ms = ms;
+  }
+  h->timing_armed = false;
+  return MF_OK;
+}
+
+static int zero_accum(mf_vegas* h, cudaStream_t st) {
+  MF_CUDA(cudaMemsetAsync(h->d_acc, 0, h->na * sizeof(double), st));
+  MF_CUDA(cudaMemsetAsync(h->d_counts, 0, 2 * sizeof(unsigned long long), st));
+  return MF_OK;
+}
+
+extern "C" int mf_vegas_iterate(mf_vegas_t* h, uint64_t n_events, void* cuda_stream, mf_iter_t* host_out) {
+  if (!h) return fail(MF_EINVAL, "handle is NULL");
+  if (n_events < 2) return fail(MF_EINVAL, "an iteration needs at least 2 events");
+  if (h->iteration >= MF_MAX_ITER) return fail(MF_ESTATE, "too many iterations (1024)");
+  MF_CUDA(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (host_out) { MF_CUDA(cudaEventRecord(h->ev0, st)); h->timing_armed = true; }
+  int rc = zero_accum(h, st);
+  if (rc) return rc;
+  rc = mf_vegas_accumulate(h, 0, n_events, n_events, cuda_stream);
+  if (rc) return rc;
+  return mf_vegas_finalize(h, n_events, cuda_stream, host_out);
+}
+
+extern "C" int mf_get_accum(mf_vegas_t* h, double* host_acc, uint64_t* host_counts) {
+  if (!h || !host_acc) return fail(MF_EINVAL, "null argument");
+  MF_CUDA(cudaSetDevice(h->device));
+  MF_CUDA(cudaStreamSynchronize(h->last_stream));
+  MF_CUDA(cudaMemcpy(host_acc, h->d_acc, h->na * sizeof(double), cudaMemcpyDeviceToHost));
+  if (host_counts) MF_CUDA(cudaMemcpy(host_counts, h->d_counts, 2 * sizeof(uint64_t), cudaMemcpyDeviceToHost));
+  return MF_OK;
+}
+
+extern "C" int mf_set_accum(mf_vegas_t* h, const double* host_acc, const uint64_t* host_counts) {
+  if (!h || !host_acc) return fail(MF_EINVAL, "null argument");
+  MF_CUDA(cudaSetDevice(h->device));
+  MF_CUDA(cudaStreamSynchronize(h->last_stream));
+  MF_CUDA(cudaMemcpy(h->d_acc, host_acc, h->na * sizeof(double), cudaMemcpyHostToDevice));
+  if (host_counts) MF_CUDA(cudaMemcpy(h->d_counts, host_counts, 2 * sizeof(uint64_t), cudaMemcpyHostToDevice));
+  return MF_OK;
+}
+
+extern "C" int mf_result(mf_vegas_t* h, mf_result_t* host_out) {
+  if (!h || !host_out) return fail(MF_EINVAL, "null argument");
+  if (h->iteration == 0) return fail(MF_ESTATE, "no iteration has been run");
+  MF_CUDA(cudaSetDevice(h->device));
+  mf_combine_kernel<<<1, 32, 0, h->last_stream>>>(h->d_state);
+  MF_CUDA(cudaGetLastError());
+  MF_CUDA(cudaStreamSynchronize(h->last_stream));
+  double r[3];
+  MF_CUDA(cudaMemcpy(r, &h->d_state->res_I, 3 * sizeof(double), cudaMemcpyDeviceToHost));
+  host_out->integral = r[0]; host_out->sigma = r[1]; host_out->chi2_dof = r[2]; host_out->n_iter = h->iteration;
+  return MF_OK;
+}
+
+extern "C" int mf_get_iterations(mf_vegas_t* h, mf_iter_t* host_out, uint32_t max_iter, uint32_t* n_iter) {
+  if (!h || !host_out || !n_iter) return fail(MF_EINVAL, "null argument");
+  MF_CUDA(cudaSetDevice(h->device));
+  MF_CUDA(cudaStreamSynchronize(h->last_stream));
+  uint32_t n = h->iteration < max_iter ? h->iteration : max_iter;
+  for (uint32_t i = 0; i < n; ++i) { int rc = fetch_iter(h, i, &host_out[i]); if (rc) return rc; }
+  *n_iter = n;
+  return MF_OK;
+}
+
+extern "C" int mf_get_grid(mf_vegas_t* h, double* host_edges) {
+  if (!h || !host_edges) return fail(MF_EINVAL, "null argument");
+  MF_CUDA(cudaSetDevice(h->device));
+  MF_CUDA(cudaStreamSynchronize(h->last_stream));
+  MF_CUDA(cudaMemcpy(host_edges, h->d_edges, (size_t)h->P.d * (h->P.nb + 1) * sizeof(double), cudaMemcpyDeviceToHost));
+  return MF_OK;
+}
+
+extern "C" int mf_set_grid(mf_vegas_t* h, const double* e) {
+  if (!h || !e) return fail(MF_EINVAL, "null argument");
+  const int nb = h->P.nb;
+  for (int j = 0; j < h->P.d; ++j) {
+    const double* r = e + (size_t)j * (nb + 1);
+    if (r[0] != 0.0 || r[nb] != 1.0) return fail(MF_EINVAL, "edges must start at 0 and end at 1");
+    for (int k = 0; k < nb; ++k) if (!(r[k + 1] > r[k])) return fail(MF_EINVAL, "edges not increasing");
+  }
+  MF_CUDA(cudaSetDevice(h->device));
+  MF_CUDA(cudaStreamSynchronize(h->last_stream));
+  MF_CUDA(cudaMemcpy(h->d_edges, e, (size_t)h->P.d * (nb + 1) * sizeof(double), cudaMemcpyHostToDevice));
+  return MF_OK;
+}
+
+extern "C" int mf_me_flops(const mf_vegas_t* h, uint64_t* n_add, uint64_t* n_mul, uint64_t* n_fma) {
+  if (!h) return fail(MF_EINVAL, "handle is NULL");
+  static const uint64_t T[4][3] = {{MF_ME2_EE_MUMU_NADD, MF_ME2_EE_MUMU_NMUL, MF_ME2_EE_MUMU_NFMA},
+                                   {MF_ME2_GG_TT_NADD, MF_ME2_GG_TT_NMUL, MF_ME2_GG_TT_NFMA},
+                                   {MF_ME2_GG_TTG_NADD, MF_ME2_GG_TTG_NMUL, MF_ME2_GG_TTG_NFMA},
+                                   {MF_ME2_GG_TTGG_NADD, MF_ME2_GG_TTGG_NMUL, MF_ME2_GG_TTGG_NFMA}};
+  if (n_add) *n_add = T[h->P.process][0];
+  if (n_mul) *n_mul = T[h->P.process][1];
+  if (n_fma) *n_fma = T[h->P.process][2];
+  return MF_OK;
+}
+
+extern "C" int mf_fp64_peak(int32_t device, double seconds, double* host_flops_per_s) {
+  if (!host_flops_per_s || !(seconds > 0.0)) return fail(MF_EINVAL, "bad argument");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return fail(MF_ECUDA, "no such CUDA device");
+  MF_CUDA(cudaSetDevice(device));
+  int n_sm = 0;
+  MF_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device));
+  const int grid = n_sm * 4, threads = 256, iters = 4096;
+  double* d_out = nullptr;
+  MF_CUDA(cudaMalloc(&d_out, (size_t)grid * threads * sizeof(double)));
+  cudaEvent_t a, b;
+  MF_CUDA(cudaEventCreate(&a)); MF_CUDA(cudaEventCreate(&b));
+  mf_dfma_kernel<<<grid, threads>>>(d_out, iters, 0.999999, 1e-6);          // warm-up
+  MF_CUDA(cudaDeviceSynchronize());
+  const double flops_per_launch = 2.0 * MF_DFMA_PER_ITER * (double)iters * grid * threads;
+  double best = 0.0, spent = 0.0;
+  int reps = 0;
+  while (spent < seconds * 1e3 && reps < 10000) {
+    MF_CUDA(cudaEventRecord(a));
+    mf_dfma_kernel<<<grid, threads>>>(d_out, iters, 0.999999, 1e-6);
+    MF_CUDA(cudaEventRecord(b));
+    MF_CUDA(cudaEventSynchronize(b));
+    float ms = 0.0f;
+    MF_CUDA(cudaEventElapsedTime(&ms, a, b));
+    spent += ms; ++reps;
+    const double f = flops_per_launch / (ms * 1e-3);
+    if (f > best) best = f;
+  }
+  cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(d_out);
+  *host_flops_per_s = best;
+  return MF_OK;
+}

@@ -13,7 +13,7 @@
 #include <math.h>
 
 #if defined(__CUDACC__)
-#define MF_HD __host__ __device__ __forceinline__
+#define MF_HD __device__ __forceinline__
 #define MF_DEVFN __device__ __forceinline__
 #else
 #define MF_HD static inline

@@ -1,0 +1,35 @@
+// mf_kernels.cuh -- the CUDA kernels of the path (sm_100a):
+//   mf_iterate_kernel  S1-S9 fused: one event per thread in registers, persistent grid (a multiple of
+//                      the 148 SMs), per-thread running sums, per-warp shared-memory histograms,
+//                      fixed-order block reduction -> one partial record per block (no atomics, so
+//                      the result is bit-reproducible for a fixed launch geometry; reading A22)
+//   mf_eval_kernel     S1-S8 with per-event outputs (the parity entry point mf_integrand_eval)
+//   mf_reduce_kernel   fixed-order sum of the per-block partials into the handle's raw sums
+//   mf_finalize_kernel S10: I, sigma, VEGAS grid refinement, iteration record (one block)
+//   mf_combine_kernel  O11: inverse-variance combination over iterations
+//   mf_dfma_kernel     register-resident DFMA chains: the measured fp64 roofline peak
+// These are FP64-pipe-bound straight-line kernels (no dense contraction): no tensor cores, no TMA;
+// the only staged data are the 2.9-4.1 KB of VEGAS edges and the 40 KB PDF table in shared memory.
+#pragma once
+#include <cuda_runtime.h>
+#include "mf_event.cuh"
+
+#define MF_THREADS 128
+#define MF_MAX_ITER 1024
+
+template <int PROC> struct MfLaunch { static const int MINB = 4; };
+template <> struct MfLaunch<2> { static const int MINB = 2; };
+template <> struct MfLaunch<3> { static const int MINB = 2; };
+
+struct MfEvalOutDev {
+  double* weight; double* x; uint8_t* bins; double* momenta; double* me2; double* pdf; uint8_t* pass;
+};
+
+// device-resident integrator state that the kernels update
+struct MfDevState {
+  double it_I[MF_MAX_ITER], it_sig[MF_MAX_ITER];
+  unsigned long long it_n[MF_MAX_ITER], it_pass[MF_MAX_ITER], it_bad[MF_MAX_ITER];
+  unsigned int n_iter;
+  double res_I, res_sig, res_chi2;
+};
+

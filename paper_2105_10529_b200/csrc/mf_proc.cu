@@ -1,0 +1,170 @@
+// mf_proc.cu -- the two per-process kernels (fused iteration, per-event evaluation), compiled once
+// per process with -DMF_PROC=0..3 so that the four |M|^2 codes build in parallel.
+#include "mf_kernels.cuh"
+#include "mf_proc.h"
+#ifndef MF_PROC
+#error "compile with -DMF_PROC=0..3"
+#endif
+
+__device__ __forceinline__ void mf_stage_tables(const MfParams& P, const double* g_edges, const double* g_pdf,
+                                                double* s_edges, double* s_pdf) {
+  const int ne = P.d * (P.nb + 1), np = P.pdf_nx * P.pdf_nq;
+  for (int i = threadIdx.x; i < ne; i += blockDim.x) s_edges[i] = g_edges[i];
+  for (int i = threadIdx.x; i < np; i += blockDim.x) s_pdf[i] = g_pdf[i];
+}
+
+// ---- S1-S9 fused ---------------------------------------------------------------------------------
+// partial: [gridDim.x][2 + d*nb] doubles, pcount: [gridDim.x][2] (n_pass, n_nonfinite)
+template <int PROC>
+__global__ void __launch_bounds__(MF_THREADS, MfLaunch<PROC>::MINB)
+mf_iterate_kernel(const MfParams P, const double* __restrict__ g_edges, const double* __restrict__ g_pdf,
+                  uint32_t iteration, unsigned long long first, unsigned long long n, double n_total,
+                  double* __restrict__ partial, unsigned long long* __restrict__ pcount) {
+  constexpr int D = MfProc<PROC>::D;
+  extern __shared__ double smem[];
+  const int nb = P.nb, nh = D * nb, nw = blockDim.x >> 5;
+  double* s_edges = smem;
+  double* s_pdf = s_edges + D * (nb + 1);
+  double* s_hist = s_pdf + P.pdf_nx * P.pdf_nq;          // [nw][D*nb]
+  double* s_red = s_hist + nw * nh;                      // [nw][4]
+  mf_stage_tables(P, g_edges, g_pdf, s_edges, s_pdf);
+  for (int i = threadIdx.x; i < nw * nh; i += blockDim.x) s_hist[i] = 0.0;
+  __syncthreads();
+
+  const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+  const unsigned lt_mask = (1u << lane) - 1u;
+  double* hw = s_hist + warp * nh;
+  double s1 = 0.0, s2 = 0.0;
+  unsigned long long n_pass = 0, n_bad = 0;
+  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+  for (unsigned long long base = (unsigned long long)blockIdx.x * blockDim.x + (threadIdx.x & ~31u);
+       base < n; base += stride) {                       // warp-uniform trip count
+    const unsigned long long i = base + lane;
+    const bool valid = i < n;
+    int bin[D];
+    bool pass = false;
+    double F = 0.0;
+    if (valid) F = mf_event<PROC, false>(P, s_edges, s_pdf, iteration, first + i, bin, pass, nullptr);
+    if (!isfinite(F)) { F = 0.0; ++n_bad; }              // A20
+    if (valid && pass) ++n_pass;
+    const double t = F / n_total, t2 = t * t;            // O9: t_i = F_i / N
+    s1 += t; s2 += t2;
+    // per-warp histogram H[j][k] += t^2, lanes that share a bin are served in lane order
+    const bool contrib = valid && t2 != 0.0;
+#pragma unroll
+    for (int j = 0; j < D; ++j) {
+      const unsigned key = contrib ? (unsigned)bin[j] : 64u + lane;
+      const unsigned peers = __match_any_sync(0xffffffffu, key);
+      const unsigned rank = __popc(peers & lt_mask);
+      const unsigned maxr = __reduce_max_sync(0xffffffffu, rank);
+      for (unsigned r = 0; r <= maxr; ++r) {
+        if (contrib && rank == r) hw[j * nb + key] += t2;
+        __syncwarp();
+      }
+    }
+  }
+  // fixed-order reductions: xor-butterfly inside the warp, warps in index order inside the block
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+    s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+    n_pass += __shfl_xor_sync(0xffffffffu, n_pass, o);
+    n_bad += __shfl_xor_sync(0xffffffffu, n_bad, o);
+  }
+  if (lane == 0) {
+    s_red[warp * 4 + 0] = s1; s_red[warp * 4 + 1] = s2;
+    s_red[warp * 4 + 2] = __longlong_as_double((long long)n_pass);
+    s_red[warp * 4 + 3] = __longlong_as_double((long long)n_bad);
+  }
+  __syncthreads();
+  double* out = partial + (size_t)blockIdx.x * (2 + nh);
+  for (int e = threadIdx.x; e < nh; e += blockDim.x) {
+    double s = 0.0;
+    for (int w = 0; w < nw; ++w) s += s_hist[w * nh + e];
+    out[2 + e] = s;
+  }
+  if (threadIdx.x == 0) {
+    double a = 0.0, b = 0.0; unsigned long long c = 0, d2 = 0;
+    for (int w = 0; w < nw; ++w) {
+      a += s_red[w * 4 + 0]; b += s_red[w * 4 + 1];
+      c += (unsigned long long)__double_as_longlong(s_red[w * 4 + 2]);
+      d2 += (unsigned long long)__double_as_longlong(s_red[w * 4 + 3]);
+    }
+    out[0] = a; out[1] = b;
+    pcount[2 * blockIdx.x] = c; pcount[2 * blockIdx.x + 1] = d2;
+  }
+}
+
+// ---- S1-S8 with per-event outputs -------------------------------------------------------------------
+template <int PROC, bool REC>
+__global__ void __launch_bounds__(MF_THREADS, MfLaunch<PROC>::MINB)
+mf_eval_kernel(const MfParams P, const double* __restrict__ g_edges, const double* __restrict__ g_pdf,
+               uint32_t iteration, unsigned long long first, unsigned long long n, MfEvalOutDev o) {
+  constexpr int D = MfProc<PROC>::D, NL = 2 + MfProc<PROC>::N;
+  extern __shared__ double smem[];
+  double* s_edges = smem;
+  double* s_pdf = s_edges + D * (P.nb + 1);
+  mf_stage_tables(P, g_edges, g_pdf, s_edges, s_pdf);
+  __syncthreads();
+  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    int bin[D];
+    bool pass;
+    MfEventRec rec;
+    double F = mf_event<PROC, REC>(P, s_edges, s_pdf, iteration, first + i, bin, pass, REC ? &rec : nullptr);
+    if (!isfinite(F)) F = 0.0;
+    if (o.weight) o.weight[i] = F;
+    if (o.bins) {
+#pragma unroll
+      for (int j = 0; j < D; ++j) o.bins[i * D + j] = (uint8_t)bin[j];
+    }
+    if (o.pass) o.pass[i] = pass ? 1 : 0;
+    if (REC) {
+      if (o.x) {
+#pragma unroll
+        for (int j = 0; j < D; ++j) o.x[i * D + j] = rec.y[j];
+      }
+      if (o.momenta) {
+#pragma unroll
+        for (int l = 0; l < NL; ++l)
+#pragma unroll
+          for (int c = 0; c < 4; ++c) o.momenta[(i * NL + l) * 4 + c] = rec.mom[l][c];
+      }
+      if (o.me2) o.me2[i] = rec.me2;
+      if (o.pdf) { o.pdf[2 * i] = rec.pdf[0]; o.pdf[2 * i + 1] = rec.pdf[1]; }
+    }
+  }
+}
+
+
+static cudaError_t proc_setup(size_t smem_iter, size_t smem_eval, int* occ_iter, int* occ_eval) {
+  cudaError_t e;
+  e = cudaFuncSetAttribute(mf_iterate_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_iter);
+  if (e) return e;
+  e = cudaFuncSetAttribute(mf_eval_kernel<MF_PROC, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_eval);
+  if (e) return e;
+  e = cudaFuncSetAttribute(mf_eval_kernel<MF_PROC, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_eval);
+  if (e) return e;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_iter, mf_iterate_kernel<MF_PROC>, MF_THREADS, smem_iter);
+  if (e) return e;
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_eval, mf_eval_kernel<MF_PROC, false>, MF_THREADS, smem_eval);
+}
+
+static cudaError_t proc_eval(const MfParams& P, const double* edges, const double* pdf, uint32_t iteration,
+                             unsigned long long first, unsigned long long n, const MfEvalOutDev& o, bool rec,
+                             int grid, size_t smem, cudaStream_t st) {
+  if (rec) mf_eval_kernel<MF_PROC, true><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, o);
+  else mf_eval_kernel<MF_PROC, false><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, o);
+  return cudaGetLastError();
+}
+
+static cudaError_t proc_iterate(const MfParams& P, const double* edges, const double* pdf, uint32_t iteration,
+                                unsigned long long first, unsigned long long n, double n_total, double* partial,
+                                unsigned long long* pcount, int grid, size_t smem, cudaStream_t st) {
+  mf_iterate_kernel<MF_PROC><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount);
+  return cudaGetLastError();
+}
+
+#define MF_CAT_(a, b) a##b
+#define MF_CAT(a, b) MF_CAT_(a, b)
+extern const MfProcOps MF_CAT(mf_ops_, MF_PROC) = {proc_setup, proc_eval, proc_iterate};

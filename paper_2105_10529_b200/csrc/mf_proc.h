@@ -1,0 +1,18 @@
+// mf_proc.h -- host-side table of the per-process kernel launchers (mf_proc.cu, one object per process)
+#pragma once
+#include <cuda_runtime.h>
+#include "mf_kernels.cuh"
+
+struct MfProcOps {
+  cudaError_t (*setup)(size_t smem_iter, size_t smem_eval, int* occ_iter, int* occ_eval);
+  cudaError_t (*eval)(const MfParams& P, const double* edges, const double* pdf, uint32_t iteration,
+                      unsigned long long first, unsigned long long n, const MfEvalOutDev& o, bool rec, int grid,
+                      size_t smem, cudaStream_t st);
+  cudaError_t (*iterate)(const MfParams& P, const double* edges, const double* pdf, uint32_t iteration,
+                         unsigned long long first, unsigned long long n, double n_total, double* partial,
+                         unsigned long long* pcount, int grid, size_t smem, cudaStream_t st);
+};
+extern const MfProcOps mf_ops_0, mf_ops_1, mf_ops_2, mf_ops_3;
+static inline const MfProcOps* mf_proc_ops(int process) {
+  return process == 0 ? &mf_ops_0 : process == 1 ? &mf_ops_1 : process == 2 ? &mf_ops_2 : &mf_ops_3;
+}

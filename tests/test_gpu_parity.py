@@ -1,0 +1,180 @@
+"""GPU parity tests proper: the CUDA path, called through the C-ABI (ctypes binding), against the
+oracle element by element on the same seeded inputs.  Tolerances (BASELINE.json north_star):
+1e-10 relative per event and on the integrals in fp64; integer work (bins, pass flags) bit-exact."""
+import numpy as np
+import pytest
+
+from paper_2105_10529_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+RTOL_EVENT = 1e-10
+RTOL_INT = 1e-10
+
+
+@pytest.fixture(scope="module")
+def mf():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2105_10529_b200 import binding
+    binding.lib()
+    return binding
+
+
+def random_grid(d, nb, seed):
+    rng = np.random.default_rng(seed)
+    w = rng.uniform(0.3, 1.7, size=(d, nb))
+    e = np.concatenate([np.zeros((d, 1)), np.cumsum(w, axis=1) / w.sum(axis=1, keepdims=True)], axis=1)
+    e[:, -1] = 1.0
+    return e
+
+
+def compare_events(out, ref, proc):
+    g = {k: v.cpu().numpy() for k, v in out.items()}
+    assert (g["bins"] == ref["bins"]).all()
+    assert (g["pass_"] == ref["pass_"]).all()
+    np.testing.assert_allclose(g["x"], ref["x"], rtol=1e-14, atol=0)
+    np.testing.assert_allclose(g["momenta"], ref["momenta"], rtol=1e-11, atol=1e-9)
+    if proc:
+        np.testing.assert_allclose(g["pdf"], ref["pdf"], rtol=1e-12, atol=1e-15)
+    nz = ref["weight"] != 0
+    assert (g["weight"][~nz] == 0).all()
+    rel_w = np.abs(g["weight"][nz] / ref["weight"][nz] - 1)
+    rel_m = np.abs(g["me2"][nz] / ref["me2"][nz] - 1)
+    assert rel_m.max() < RTOL_EVENT, rel_m.max()
+    assert rel_w.max() < RTOL_EVENT, rel_w.max()
+
+
+# sizes span several 128-thread tiles and a ragged tail; iteration/first_event exercise the counter
+@pytest.mark.parametrize("proc,n", [(0, 5003), (1, 5003), (2, 3001), (3, 333)])
+def test_per_event_parity_uniform_and_adapted_grid(mf, mfo, proc, n):
+    cfg = W.config(proc, seed=W.CONFIGS[proc]["seed"])
+    gpu, orc = mf.Vegas(cfg), mfo.Vegas(cfg)
+    ref = orc.eval(0, 0, n, n_threads=mfo.max_threads())
+    compare_events(gpu.integrand_eval(0, 0, n, debug=True), ref, proc)
+    e = random_grid(orc.d, 50, 100 + proc)
+    gpu.set_grid(e); orc.set_grid(e)
+    np.testing.assert_array_equal(gpu.get_grid(), e)
+    ref = orc.eval(3, 2**33 + 17, n, n_threads=mfo.max_threads())
+    compare_events(gpu.integrand_eval(3, 2**33 + 17, n, debug=True), ref, proc)
+
+
+def test_chunking_invariance(mf):
+    """event indices are global: one call == concatenated chunks, bit for bit"""
+    cfg = W.config(W.GG_TTG, seed=1)
+    gpu = mf.Vegas(cfg)
+    a = gpu.integrand_eval(0, 0, 10000)["weight"].cpu().numpy()
+    b = np.concatenate([gpu.integrand_eval(0, s, m)["weight"].cpu().numpy() for s, m in ((0, 1), (1, 4095), (4096, 5904))])
+    assert (a == b).all()
+
+
+@pytest.mark.parametrize("proc,n_iter,n", [(0, 3, 100_000), (1, 3, 40_000), (2, 2, 20_000), (3, 2, 1_500)])
+def test_iteration_parity(mf, mfo, proc, n_iter, n):
+    """fused kernel + finalize vs the oracle: I, sigma, raw sums, histogram, refined grid, counters"""
+    cfg = W.config(proc, seed=W.CONFIGS[proc]["seed"])
+    gpu, orc = mf.Vegas(cfg), mfo.Vegas(cfg)
+    for it in range(n_iter):
+        g = gpu.vegas_iterate(n)
+        o = orc.iterate(n, n_threads=mfo.max_threads())
+        assert g["n_events"] == n and g["n_pass"] == o["n_pass"] and g["n_nonfinite"] == 0 == o["n_nonfinite"]
+        assert abs(g["integral"] / o["integral"] - 1) < RTOL_INT
+        assert abs(g["sigma"] / o["sigma"] - 1) < 1e-8          # sigma^2 = N S2 - I^2 cancels ~2 digits
+        acc, cnt = gpu.get_accum()
+        np.testing.assert_allclose(acc, orc.get_accum(), rtol=RTOL_INT, atol=1e-300)
+        np.testing.assert_allclose(gpu.get_grid(), orc.get_grid(), rtol=0, atol=1e-11)
+        gpu.set_grid(orc.get_grid())          # keep the two in lock-step for the next iteration
+    rg, ro = gpu.result(), orc.result()
+    assert rg["n_iter"] == n_iter
+    for k in ("integral", "sigma"):
+        assert abs(rg[k] / ro[k] - 1) < 1e-8
+    assert abs(rg["chi2_dof"] - ro["chi2_dof"]) < 1e-6 * max(1.0, ro["chi2_dof"])
+
+
+def test_config0_cross_section(mf):
+    """config 0 end to end on the GPU: sigma = 4 pi alpha^2/(3s) K = 9.290793339943443 pb"""
+    c = W.CONFIGS[0]
+    gpu = mf.Vegas(W.config(0, seed=c["seed"]))
+    for _ in range(c["n_iter"]):
+        gpu.vegas_iterate(c["n_events"])
+    r = gpu.result()
+    assert abs(r["integral"] - 9.290793339943443) < 5 * r["sigma"] and r["sigma"] < 2e-3
+
+
+def test_config1_cross_section_and_closed_form(mf):
+    """config 1 at full size: per-event |M|^2 vs the closed form of gg -> tt~ (sampled), sigma vs quadrature"""
+    c = W.CONFIGS[1]
+    cfg = W.config(1, seed=c["seed"])
+    gpu = mf.Vegas(cfg)
+    out = gpu.integrand_eval(0, 0, 20000, debug=True)
+    mom = out["momenta"].cpu().numpy(); me2 = out["me2"].cpu().numpy()
+    shat = 4 * mom[:, 0, 0] ** 2
+    dot = lambda a, b: a[:, 0] * b[:, 0] - (a[:, 1:] * b[:, 1:]).sum(1)
+    t1 = 2 * dot(mom[:, 0], mom[:, 2]) / shat; t2 = 2 * dot(mom[:, 1], mom[:, 2]) / shat
+    rho = 4 * cfg["m_top"] ** 2 / shat
+    gs4 = (4 * np.pi * cfg["alpha_s"]) ** 2
+    closed = gs4 * (1 / (6 * t1 * t2) - 3.0 / 8) * (t1 ** 2 + t2 ** 2 + rho - rho ** 2 / (4 * t1 * t2))
+    assert np.abs(me2 / closed - 1).max() < 1e-10
+    for _ in range(c["n_iter"]):
+        gpu.vegas_iterate(c["n_events"])
+    r = gpu.result()
+    assert abs(r["integral"] - 1074.393) < 5 * r["sigma"] + 0.02 and r["sigma"] < 0.5
+
+
+def test_full_size_launch_sampled_parity(mf, mfo):
+    """gg->tt~g at BASELINE's 1e7 events in the launch configuration bench.py times: integrals of
+    the fused kernel == sums of the eval kernel's weights; sampled events == oracle"""
+    import torch
+    cfg = W.config(W.GG_TTG, seed=0)
+    n = 10_000_000
+    gpu, orc = mf.Vegas(cfg), mfo.Vegas(cfg)
+    g = gpu.vegas_iterate(n)
+    acc, cnt = gpu.get_accum()
+    gpu2 = mf.Vegas(cfg)
+    w = gpu2.integrand_eval(0, 0, n)["weight"]
+    t = w / n
+    assert abs(float(t.sum()) / acc[0] - 1) < 1e-10 and abs(float((t * t).sum()) / acc[1] - 1) < 1e-10
+    assert int((w != 0).sum()) <= cnt[0] <= n and g["n_nonfinite"] == 0
+    idx = [0, 1, 127, 128, 4097, 999_999, 5_000_001, n - 1]
+    for i in idx:
+        ref = orc.eval(0, i, 1)["weight"][0]
+        got = float(w[i])
+        assert (ref == 0 and got == 0) or abs(got / ref - 1) < RTOL_EVENT
+
+
+def test_sharded_accumulate_equals_iterate(mf):
+    """mf_vegas_accumulate over two event ranges + finalize == mf_vegas_iterate (to summation order)"""
+    cfg = W.config(W.GG_TT, seed=5)
+    n = 50_000
+    a, b = mf.Vegas(cfg), mf.Vegas(cfg)
+    ia = a.vegas_iterate(n)
+    acc0 = np.zeros(2 + b.d * b.n_bins); b.set_accum(acc0, np.zeros(2, np.uint64))
+    b.vegas_accumulate(0, 20_000, n); b.vegas_accumulate(20_000, 30_000, n)
+    ib = b.vegas_finalize(n)
+    assert abs(ia["integral"] / ib["integral"] - 1) < 1e-13 and ia["n_pass"] == ib["n_pass"]
+    np.testing.assert_allclose(a.get_grid(), b.get_grid(), rtol=0, atol=1e-13)
+
+
+def test_errors_and_edge_cases(mf):
+    cfg = W.config(W.GG_TT)
+    gpu = mf.Vegas(cfg)
+    with pytest.raises(mf.MfError) as e:
+        gpu.result()
+    assert e.value.code == mf.MF_ESTATE
+    with pytest.raises(mf.MfError):
+        gpu.vegas_iterate(1)
+    out = gpu.integrand_eval(0, 0, 0)            # empty input
+    assert out["weight"].numel() == 0
+    one = gpu.integrand_eval(0, 5, 1)["weight"]  # single event (ragged warp)
+    assert one.shape == (1,)
+    bad = dict(cfg); bad["precision"] = 32
+    with pytest.raises(mf.MfError) as e:
+        mf.Vegas(bad)
+    assert e.value.code == mf.MF_EUNSUPPORTED
+    bad = dict(cfg); bad["sqrt_s"] = 300.0       # below threshold: kinematics outside the grid
+    with pytest.raises(mf.MfError) as e:
+        mf.Vegas(bad)
+    assert e.value.code == mf.MF_EINVAL
+    g = gpu.get_grid(); g[0, 3] = g[0, 2]
+    with pytest.raises(mf.MfError):
+        gpu.set_grid(g)
+    gpu.vegas_iterate(2)                          # minimum iteration
+    assert gpu.result()["n_iter"] == 1

@@ -82,7 +82,7 @@ int mf_integrand_eval(mf_vegas_t *h, uint32_t iteration, uint64_t first_event, u
 /* One VEGAS iteration of n_events (>= 2) events: S1-S9 fused in one kernel (no per-event global
  * traffic), then S10 in a one-block finalize kernel: I, sigma, grid refinement, record appended on
  * the device.  Enqueue only, unless host_out_or_null != NULL: then the stream is synchronised and
- * the iteration record (with the device time of the two kernels) is returned.                      */
+ * the iteration record (kernel_ms = device time of the fused kernel) is returned.                            */
 int mf_vegas_iterate(mf_vegas_t *h, uint64_t n_events, void *cuda_stream, mf_iter_t *host_out_or_null);
 
 /* Sharded form of one iteration (multi-GPU): accumulate events
@@ -106,6 +106,10 @@ int mf_set_grid(mf_vegas_t *h, const double *host_edges);   /* edges must start 
 /* Launch geometry of the fused kernel: blocks per SM (0 = library default) and threads per block
  * (0 = default).  Results are deterministic for a fixed geometry.                                  */
 int mf_set_launch(mf_vegas_t *h, uint32_t blocks_per_sm, uint32_t threads_per_block);
+/* Device times (CUDA events on the caller's stream): of the fused S1-S9 kernel of the last
+ * mf_vegas_accumulate / mf_vegas_iterate, and of the whole last mf_vegas_iterate (memsets + fused
+ * kernel + reduce + finalize).  Waits for those events to complete.                                 */
+int mf_last_kernel_ms(const mf_vegas_t *h, float *fused_kernel_ms, float *iteration_ms);
 /* Exact add/mul/fma counts per event of the generated |M|^2 code of the handle's process
  * (generator-counted): flops = add + mul + 2 fma.                    */
 int mf_me_flops(const mf_vegas_t *h, uint64_t *n_add, uint64_t *n_mul, uint64_t *n_fma);

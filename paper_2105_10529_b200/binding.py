@@ -15,7 +15,7 @@ MF_OK, MF_EINVAL, MF_ENOMEM, MF_ECUDA, MF_ESTATE, MF_EUNSUPPORTED = 0, -1, -2, -
 EXPORTS = ["mf_vegas_create", "mf_vegas_destroy", "mf_ndim", "mf_integrand_eval", "mf_vegas_iterate",
            "mf_vegas_accumulate", "mf_get_accum", "mf_set_accum", "mf_vegas_finalize", "mf_result",
            "mf_get_iterations", "mf_get_grid", "mf_set_grid", "mf_set_launch", "mf_me_flops",
-           "mf_fp64_peak", "mf_last_error"]
+           "mf_fp64_peak", "mf_last_kernel_ms", "mf_last_error"]
 
 
 class MfError(RuntimeError):
@@ -93,6 +93,7 @@ def lib():
         L.mf_set_grid.argtypes = [vp, vp]
         L.mf_set_launch.argtypes = [vp, u32, u32]
         L.mf_me_flops.argtypes = [vp, C.POINTER(u64), C.POINTER(u64), C.POINTER(u64)]
+        L.mf_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
         L.mf_fp64_peak.argtypes = [C.c_int32, C.c_double, C.POINTER(C.c_double)]
         _lib = L
     return _lib
@@ -196,6 +197,11 @@ class Vegas:
 
     def set_launch(self, blocks_per_sm=0, threads_per_block=0):
         _check(lib().mf_set_launch(self._h, blocks_per_sm, threads_per_block))
+
+    def last_kernel_ms(self):
+        a, b = C.c_float(), C.c_float()
+        _check(lib().mf_last_kernel_ms(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
 
     def me_flops(self):
         a, m, f = C.c_uint64(), C.c_uint64(), C.c_uint64()

@@ -22,16 +22,17 @@ def build(force=False, verbose=False):
     from .gen.__main__ import main as gen_main
     gen_main()
     os.makedirs(OBJ, exist_ok=True)
-    hdrs = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cuh", ".h"))]
-    hdrs += [os.path.join(CSRC, "generated", f) for f in os.listdir(os.path.join(CSRC, "generated"))]
-    hdrs += [os.path.join(os.path.dirname(HERE), "include", "madflow_b200.h"), os.path.abspath(__file__)]
+    gen = [os.path.join(CSRC, "generated", f) for f in os.listdir(os.path.join(CSRC, "generated"))]
+    kern = gen + [os.path.join(CSRC, f) for f in ("mf_device.cuh", "mf_event.cuh", "mf_kernels.cuh", "mf_proc.h")]
+    api = kern + [os.path.join(CSRC, f) for f in ("mf_small_kernels.cuh", "mf_params.h")]
+    api += [os.path.join(os.path.dirname(HERE), "include", "madflow_b200.h")]
     jobs = [("mf_api.o", os.path.join(CSRC, "mf_api.cu"), [])]
     jobs += [("mf_proc%d.o" % p, os.path.join(CSRC, "mf_proc.cu"), ["-DMF_PROC=%d" % p]) for p in range(4)]
 
     def compile_one(job):
         obj, src, extra = job
         out = os.path.join(OBJ, obj)
-        if not force and _newer(out, hdrs + [src]):
+        if not force and _newer(out, (api if obj == "mf_api.o" else kern) + [src]):
             return obj, "up to date"
         r = subprocess.run(["nvcc"] + NVCC_FLAGS + extra + ["-c", src, "-o", out], capture_output=True, text=True)
         with open(out + ".log", "w") as f:

@@ -36,8 +36,8 @@ struct mf_vegas {
   const MfProcOps* ops;               // per-process kernels (one translation unit each)
   uint32_t iteration;                  // iterations finalized so far (= Philox counter word 3)
   cudaStream_t last_stream;
-  cudaEvent_t ev0, ev1;
-  bool timing_armed;
+  cudaEvent_t ev0, ev1, evk0, evk1;   // iteration start/end, fused-kernel start/end
+  bool have_k, have_it;                // events recorded (fused kernel / whole iteration)
 };
 
 static size_t iter_smem_bytes(const MfParams& P, int threads) {
@@ -89,6 +89,8 @@ extern "C" int mf_vegas_create(const mf_config_t* cfg, mf_vegas_t** out) {
   if (npdf) MF_CREATE_CUDA(cudaMemcpy(h->d_pdf, cfg->pdf_xf, npdf * sizeof(double), cudaMemcpyHostToDevice));
   MF_CREATE_CUDA(cudaEventCreate(&h->ev0));
   MF_CREATE_CUDA(cudaEventCreate(&h->ev1));
+  MF_CREATE_CUDA(cudaEventCreate(&h->evk0));
+  MF_CREATE_CUDA(cudaEventCreate(&h->evk1));
   *out = h;
   return MF_OK;
 }
@@ -100,6 +102,8 @@ extern "C" int mf_vegas_destroy(mf_vegas_t* h) {
   cudaFree(h->d_acc); cudaFree(h->d_counts); cudaFree(h->d_state);
   if (h->ev0) cudaEventDestroy(h->ev0);
   if (h->ev1) cudaEventDestroy(h->ev1);
+  if (h->evk0) cudaEventDestroy(h->evk0);
+  if (h->evk1) cudaEventDestroy(h->evk1);
   delete h;
   return MF_OK;
 }
@@ -154,8 +158,11 @@ extern "C" int mf_vegas_accumulate(mf_vegas_t* h, uint64_t first_event, uint64_t
   MF_CUDA(cudaSetDevice(h->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int grid = grid_for(h, n_events, h->occ_iter);
+  MF_CUDA(cudaEventRecord(h->evk0, st));
   MF_CUDA(h->ops->iterate(h->P, h->d_edges, h->d_pdf, h->iteration, first_event, n_events, (double)n_total,
                           h->d_partial, h->d_pcount, grid, h->smem_iter, st));
+  MF_CUDA(cudaEventRecord(h->evk1, st));
+  h->have_k = true;
   mf_reduce_kernel<<<(h->na + 127) / 128, 128, 0, st>>>(h->d_partial, h->d_pcount, grid, h->na, h->d_acc, h->d_counts);
   MF_CUDA(cudaGetLastError());
   h->last_stream = st;
@@ -187,15 +194,11 @@ extern "C" int mf_vegas_finalize(mf_vegas_t* h, uint64_t n_total, void* cuda_str
   const uint32_t idx = h->iteration++;
   h->last_stream = st;
   if (host_out) {
-    float ms = 0.0f;
-    if (h->timing_armed) { MF_CUDA(cudaEventRecord(h->ev1, st)); }
     MF_CUDA(cudaStreamSynchronize(st));
-    if (h->timing_armed) { MF_CUDA(cudaEventElapsedTime(&ms, h->ev0, h->ev1)); }
     int rc = fetch_iter(h, idx, host_out);
     if (rc) return rc;
-    host_out->kernel_ms = ms;
+    if (h->have_k) MF_CUDA(cudaEventElapsedTime(&host_out->kernel_ms, h->evk0, h->evk1));
   }
-  h->timing_armed = false;
   return MF_OK;
 }
 
@@ -211,12 +214,35 @@ extern "C" int mf_vegas_iterate(mf_vegas_t* h, uint64_t n_events, void* cuda_str
   if (h->iteration >= MF_MAX_ITER) return fail(MF_ESTATE, "too many iterations (1024)");
   MF_CUDA(cudaSetDevice(h->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (host_out) { MF_CUDA(cudaEventRecord(h->ev0, st)); h->timing_armed = true; }
+  MF_CUDA(cudaEventRecord(h->ev0, st));
   int rc = zero_accum(h, st);
   if (rc) return rc;
   rc = mf_vegas_accumulate(h, 0, n_events, n_events, cuda_stream);
   if (rc) return rc;
-  return mf_vegas_finalize(h, n_events, cuda_stream, host_out);
+  rc = mf_vegas_finalize(h, n_events, cuda_stream, nullptr);
+  if (rc) return rc;
+  MF_CUDA(cudaEventRecord(h->ev1, st));
+  h->have_it = true;
+  if (host_out) {
+    MF_CUDA(cudaStreamSynchronize(st));
+    rc = fetch_iter(h, h->iteration - 1, host_out);
+    if (rc) return rc;
+    MF_CUDA(cudaEventElapsedTime(&host_out->kernel_ms, h->evk0, h->evk1));
+  }
+  return MF_OK;
+}
+
+extern "C" int mf_last_kernel_ms(const mf_vegas_t* h, float* fused_kernel_ms, float* iteration_ms) {
+  if (!h) return fail(MF_EINVAL, "handle is NULL");
+  if (fused_kernel_ms) {
+    *fused_kernel_ms = 0.0f;
+    if (h->have_k) { MF_CUDA(cudaEventSynchronize(h->evk1)); MF_CUDA(cudaEventElapsedTime(fused_kernel_ms, h->evk0, h->evk1)); }
+  }
+  if (iteration_ms) {
+    *iteration_ms = 0.0f;
+    if (h->have_it) { MF_CUDA(cudaEventSynchronize(h->ev1)); MF_CUDA(cudaEventElapsedTime(iteration_ms, h->ev0, h->ev1)); }
+  }
+  return MF_OK;
 }
 
 extern "C" int mf_get_accum(mf_vegas_t* h, double* host_acc, uint64_t* host_counts) {

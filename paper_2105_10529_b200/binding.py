@@ -9,7 +9,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libmadflow_b200.so")
+LIB_PATH = os.environ.get("MF_LIB", os.path.join(_HERE, "libmadflow_b200.so"))   # MF_LIB: tuning variants
 
 MF_OK, MF_EINVAL, MF_ENOMEM, MF_ECUDA, MF_ESTATE, MF_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 EXPORTS = ["mf_vegas_create", "mf_vegas_destroy", "mf_ndim", "mf_integrand_eval", "mf_vegas_iterate",

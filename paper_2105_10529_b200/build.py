@@ -18,23 +18,27 @@ def _newer(target, deps):
     return os.path.exists(target) and all(os.path.getmtime(target) >= os.path.getmtime(d) for d in deps)
 
 
-def build(force=False, verbose=False):
+def build(force=False, verbose=False, extra_flags=(), tag="", only=(0, 1, 2, 3)):
+    """tag/extra_flags/only: tuning variants (objects and library get the tag as a suffix)"""
+    global OBJ, LIB
+    obj_dir = OBJ + tag
+    lib = LIB if not tag else LIB.replace(".so", tag + ".so")
     from .gen.__main__ import main as gen_main
     gen_main()
-    os.makedirs(OBJ, exist_ok=True)
+    os.makedirs(obj_dir, exist_ok=True)
     gen = [os.path.join(CSRC, "generated", f) for f in os.listdir(os.path.join(CSRC, "generated"))]
     kern = gen + [os.path.join(CSRC, f) for f in ("mf_device.cuh", "mf_event.cuh", "mf_kernels.cuh", "mf_proc.h")]
     api = kern + [os.path.join(CSRC, f) for f in ("mf_small_kernels.cuh", "mf_params.h")]
     api += [os.path.join(os.path.dirname(HERE), "include", "madflow_b200.h")]
     jobs = [("mf_api.o", os.path.join(CSRC, "mf_api.cu"), [])]
-    jobs += [("mf_proc%d.o" % p, os.path.join(CSRC, "mf_proc.cu"), ["-DMF_PROC=%d" % p]) for p in range(4)]
+    jobs += [("mf_proc%d.o" % p, os.path.join(CSRC, "mf_proc.cu" if p in only else "mf_proc_stub.cu"), ["-DMF_PROC=%d" % p]) for p in range(4)]
 
     def compile_one(job):
         obj, src, extra = job
-        out = os.path.join(OBJ, obj)
+        out = os.path.join(obj_dir, obj)
         if not force and _newer(out, (api if obj == "mf_api.o" else kern) + [src]):
             return obj, "up to date"
-        r = subprocess.run(["nvcc"] + NVCC_FLAGS + extra + ["-c", src, "-o", out], capture_output=True, text=True)
+        r = subprocess.run(["nvcc"] + NVCC_FLAGS + list(extra_flags) + extra + ["-c", src, "-o", out], capture_output=True, text=True)
         with open(out + ".log", "w") as f:
             f.write(r.stdout + r.stderr)
         if r.returncode != 0:
@@ -43,13 +47,13 @@ def build(force=False, verbose=False):
 
     with ThreadPoolExecutor(max_workers=5) as ex:
         results = list(ex.map(compile_one, jobs))
-    objs = [os.path.join(OBJ, j[0]) for j in jobs]
-    if force or not _newer(LIB, objs):
-        subprocess.check_call(["nvcc", "-shared", "-o", LIB] + objs + ["-gencode", "arch=compute_100a,code=sm_100a"])
+    objs = [os.path.join(obj_dir, j[0]) for j in jobs]
+    if force or not _newer(lib, objs):
+        subprocess.check_call(["nvcc", "-shared", "-o", lib] + objs + ["-gencode", "arch=compute_100a,code=sm_100a"])
     if verbose:
         for obj, what in results:
             print(obj, what)
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":

@@ -91,10 +91,9 @@ MF_HD double mf_event(const MfParams& P, const double* edges, const double* pdf_
     f1 = xf1 / x1; f2 = xf2 / x2;
   }
   double me2 = 0.0, F = 0.0;
-  if (pass) {
-    me2 = mf_me2<PROC>(P, rts, k);                                       // S7
-    F = JV * jx * f1 * f2 * me2 * wps * P.wconst / shat;                 // S8
-  }
+  if (MF_UNIFORM_ME || pass) me2 = mf_me2<PROC>(P, rts, k);              // S7
+  if (pass) F = JV * jx * f1 * f2 * me2 * wps * P.wconst / shat;         // S8
+  else me2 = 0.0;
   if (REC) {
 #pragma unroll
     for (int j = 0; j < D; ++j) rec->y[j] = y[j];

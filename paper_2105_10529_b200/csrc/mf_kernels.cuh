@@ -14,12 +14,17 @@
 #include <cuda_runtime.h>
 #include "mf_event.cuh"
 
+#ifndef MF_THREADS
 #define MF_THREADS 128
+#endif
 #define MF_MAX_ITER 1024
+#ifndef MF_MINB_HEAVY
+#define MF_MINB_HEAVY 2              // resident blocks per SM the heavy kernels (tt~g, tt~gg) are compiled for
+#endif
 
-template <int PROC> struct MfLaunch { static const int MINB = 4; };
-template <> struct MfLaunch<2> { static const int MINB = 2; };
-template <> struct MfLaunch<3> { static const int MINB = 2; };
+template <int PROC> struct MfLaunch { static const int MINB = 512 / MF_THREADS; };
+template <> struct MfLaunch<2> { static const int MINB = MF_MINB_HEAVY; };
+template <> struct MfLaunch<3> { static const int MINB = MF_MINB_HEAVY; };
 
 struct MfEvalOutDev {
   double* weight; double* x; uint8_t* bins; double* momenta; double* me2; double* pdf; uint8_t* pass;

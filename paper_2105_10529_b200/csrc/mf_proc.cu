@@ -37,14 +37,19 @@ mf_iterate_kernel(const MfParams P, const double* __restrict__ g_edges, const do
   double s1 = 0.0, s2 = 0.0;
   unsigned long long n_pass = 0, n_bad = 0;
   const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
-  for (unsigned long long base = (unsigned long long)blockIdx.x * blockDim.x + (threadIdx.x & ~31u);
-       base < n; base += stride) {                       // warp-uniform trip count
-    const unsigned long long i = base + lane;
+  const unsigned long long tbase = MF_UNIFORM_ME ? 0u : (threadIdx.x & ~31u);   // block- or warp-uniform trips
+  for (unsigned long long base = (unsigned long long)blockIdx.x * blockDim.x + tbase; base < n; base += stride) {
+    const unsigned long long i = base + (MF_UNIFORM_ME ? threadIdx.x : lane);
     const bool valid = i < n;
     int bin[D];
     bool pass = false;
     double F = 0.0;
-    if (valid) F = mf_event<PROC, false>(P, s_edges, s_pdf, iteration, first + i, bin, pass, nullptr);
+    if (MF_UNIFORM_ME) {                                 // every thread runs the event (barriers inside);
+      F = mf_event<PROC, false>(P, s_edges, s_pdf, iteration, first + (valid ? i : n - 1), bin, pass, nullptr);
+      if (!valid) { F = 0.0; pass = false; }             // lanes past the end recompute event n-1, discarded
+    } else if (valid) {
+      F = mf_event<PROC, false>(P, s_edges, s_pdf, iteration, first + i, bin, pass, nullptr);
+    }
     if (!isfinite(F)) { F = 0.0; ++n_bad; }              // A20
     if (valid && pass) ++n_pass;
     const double t = F / n_total, t2 = t * t;            // O9: t_i = F_i / N
@@ -107,7 +112,9 @@ mf_eval_kernel(const MfParams P, const double* __restrict__ g_edges, const doubl
   mf_stage_tables(P, g_edges, g_pdf, s_edges, s_pdf);
   __syncthreads();
   const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
-  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+  for (unsigned long long base = (unsigned long long)blockIdx.x * blockDim.x; base < n; base += stride) {
+    unsigned long long i = base + threadIdx.x;           // block-uniform trip count (barriers inside the event)
+    if (i >= n) { if (!MF_UNIFORM_ME) break; i = n - 1; }   // tail lanes recompute event n-1 (same values written)
     int bin[D];
     bool pass;
     MfEventRec rec;

@@ -401,7 +401,11 @@ def emit_function(gen, fname):
         L.append("  for (int ih = 0; ih < %d; ++ih) {" % nh)
         for b, l in enumerate(reversed(gen.loop_legs)):
             L.append("    const double lam%d = (ih & %d) ? 1.0 : -1.0;" % (l, 1 << b))
-        L += g.emit([out], True, indent="    ")
+        body = g.emit([out], True, indent="    ")
+        for i, line in enumerate(body):      # barrier points: keep the block's warps on the same I-cache lines
+            if i % 64 == 0:
+                L.append("    MF_SYNC_POINT(%d);" % (i // 64))
+            L.append(line)
         L.append("    acc += %s;" % g.ref(out))
         L.append("  }")
         L.append("  return acc;")

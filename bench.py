@@ -31,7 +31,7 @@ FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # SMs x DFMA lanes x 2 
 
 
 class ClockSampler:
-    """nvidia-smi clocks/throttle reasons sampled every 200 ms while the timed region runs"""
+    """nvidia-smi clocks/throttle reasons sampled every 50 ms while the warm-up, timed and e2e regions run"""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
@@ -39,7 +39,7 @@ class ClockSampler:
         self.rows, self.p = [], None
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", uuid, "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
-                                       "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                                       "-lms", "50"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
         except OSError:
@@ -140,10 +140,11 @@ def run_ours(args, rank, local_rank, world):
         else:
             sharding.sharded_iterate(h, n_total, rank, world, dist, dev)
 
+    # clocks are sampled from the first warm-up step to the end of the end-to-end region (same load)
+    sampler = ClockSampler(uuid) if rank == 0 else None
     for _ in range(args.warmup):
         step()
     barrier()
-    sampler = ClockSampler(uuid) if rank == 0 else None
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     kernel_ms, pass_frac = [], []
     e0.record()
@@ -157,7 +158,6 @@ def run_ours(args, rank, local_rank, world):
         t = torch.tensor([ms], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t.item())
-    clocks = sampler.stop() if sampler else None
     its = h.get_iterations()
     pass_frac = [it["n_pass"] / it["n_events"] for it in its[-args.steps:]]
     value = n_total * args.steps / (ms * 1e-3)
@@ -179,6 +179,7 @@ def run_ours(args, rank, local_rank, world):
         t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_s = float(t.item())
+    clocks = sampler.stop() if sampler else None
     peak_after = binding.fp64_peak(local_rank, 0.3)
     res = h.result()
     if rank != 0:

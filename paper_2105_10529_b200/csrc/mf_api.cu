@@ -118,7 +118,7 @@ extern "C" int mf_ndim(const mf_vegas_t* h, uint32_t* d, uint32_t* n_final) {
 extern "C" int mf_set_launch(mf_vegas_t* h, uint32_t blocks_per_sm, uint32_t threads_per_block) {
   if (!h) return fail(MF_EINVAL, "handle is NULL");
   if (threads_per_block != 0 && threads_per_block != MF_THREADS)
-    return fail(MF_EINVAL, "threads_per_block must be 0 or 128 in this build");
+    return fail(MF_EINVAL, "threads_per_block must be 0 or the built MF_THREADS (256)");
   if (blocks_per_sm > 32) return fail(MF_EINVAL, "blocks_per_sm must be <= 32");
   h->blocks_per_sm = blocks_per_sm; h->threads = threads_per_block;
   return MF_OK;

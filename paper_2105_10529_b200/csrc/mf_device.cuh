@@ -28,7 +28,7 @@ static inline double rsqrt(double x) { return 1.0 / sqrt(x); }
 // line body is larger than the 32 KB L1.5 I-cache).  Requires the |M|^2 code to be executed by every
 // thread of the block (MF_UNIFORM_ME), which costs nothing: a warp runs it whenever one lane passes.
 #ifndef MF_SYNC_EVERY
-#define MF_SYNC_EVERY 0
+#define MF_SYNC_EVERY 4
 #endif
 #if defined(__CUDA_ARCH__)
 #define MF_SYNC_POINT(i) do { if (MF_SYNC_EVERY > 0 && (i) % (MF_SYNC_EVERY > 0 ? MF_SYNC_EVERY : 1) == 0) __syncthreads(); } while (0)

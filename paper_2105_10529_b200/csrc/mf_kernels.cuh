@@ -14,12 +14,15 @@
 #include <cuda_runtime.h>
 #include "mf_event.cuh"
 
+// Launch shape (tuned on B200, profiles/r1_tuning.md): one 256-thread CTA per SM for the heavy
+// processes (255 registers/thread, 8 warps/SM) whose warps are kept on the same instruction-cache
+// lines by the barrier points of the generated code (MF_SYNC_EVERY in mf_device.cuh).
 #ifndef MF_THREADS
-#define MF_THREADS 128
+#define MF_THREADS 256
 #endif
 #define MF_MAX_ITER 1024
 #ifndef MF_MINB_HEAVY
-#define MF_MINB_HEAVY 2              // resident blocks per SM the heavy kernels (tt~g, tt~gg) are compiled for
+#define MF_MINB_HEAVY 1              // resident blocks per SM the heavy kernels (tt~g, tt~gg) are compiled for
 #endif
 
 template <int PROC> struct MfLaunch { static const int MINB = 512 / MF_THREADS; };

@@ -21,6 +21,7 @@ derivation is written out in DESIGN.md.  The parity relation |M(-lambda)|^2 = |M
 """
 import itertools
 import math
+import os
 import numpy as np
 from .dag import Dag, R, Cx, csum_prod
 
@@ -431,7 +432,15 @@ PROCESSES = {
 }
 
 
+# loop-invariant values with a cone of at most this many operations are recomputed in the loop body
+# (Dag.demote_cheap); tuned on B200, see DESIGN.md "Kernels / S7"
+DEMOTE = {"mf_me2_gg_ttg": int(os.environ.get("MF_GEN_DEMOTE_TTG", "0")),
+          "mf_me2_gg_ttgg": int(os.environ.get("MF_GEN_DEMOTE_TTGG", "0"))}
+
+
 def generate(fname):
     gen = PROCESSES[fname]()
     gen.build()
+    if DEMOTE.get(fname, 0) > 0:
+        gen.g.demote_cheap([gen.out], DEMOTE[fname])
     return gen

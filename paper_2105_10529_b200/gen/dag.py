@@ -167,6 +167,36 @@ class Dag:
             acc = self.fma(a, b, acc)
         return acc
 
+    def demote_cheap(self, outputs, max_cost):
+        """Limit loop-invariant hoisting: an invariant node whose whole cone (down to the inputs) has
+        at most max_cost operations and no reciprocal is recomputed inside the loop instead of being
+        kept in a register across it (the hoisted values otherwise outnumber the register file)."""
+        mark = self.live(outputs)
+        cone = [None] * len(self.nodes)
+        for i, (op, *_r) in enumerate(self.nodes):
+            if not mark[i] or self.dep[i]:
+                continue
+            if op in ("in", "sym"):
+                cone[i] = frozenset()
+                continue
+            c = {i}
+            big = op == "rcp"
+            for o in self._operands(i):
+                if cone[o] is None:
+                    big = True
+                else:
+                    c |= cone[o]
+            cone[i] = None if (big or len(c) > max_cost) else frozenset(c)
+        stay = [False] * len(self.nodes)          # cheap nodes that a hoisted (expensive) node needs
+        for i in range(len(self.nodes) - 1, -1, -1):
+            if mark[i] and not self.dep[i] and (cone[i] is None or stay[i]):
+                for o in self._operands(i):
+                    stay[o] = True
+        for i in range(len(self.nodes)):
+            if (mark[i] and not self.dep[i] and cone[i] is not None and not stay[i]
+                    and self.nodes[i][0] not in ("in", "sym")):
+                self.dep[i] = True
+
     # ---- analysis ------------------------------------------------------------------------------
     def _operands(self, i):
         op, a, b, c = self.nodes[i]

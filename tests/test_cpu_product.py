@@ -1,0 +1,113 @@
+"""CPU-side tests of the product's host logic: the C-ABI library loads and exports every symbol the
+header declares (no compute calls without a GPU), argument validation, the build-time amplitude
+generator evaluated numerically against the oracle, and the sharded-iteration plumbing under gloo."""
+import ctypes as C
+import math
+import os
+import re
+import numpy as np
+import pytest
+
+from paper_2105_10529_b200 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def binding():
+    from paper_2105_10529_b200 import build, binding as b
+    build.build()
+    b.lib()
+    return b
+
+
+def test_library_exports_every_declared_symbol(binding):
+    hdr = open(os.path.join(ROOT, "include", "madflow_b200.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(mf_[a-z0-9_]+)\s*\(", hdr))
+    assert {"mf_vegas_create", "mf_integrand_eval", "mf_vegas_iterate", "mf_result"} <= declared
+    lib = binding.lib()
+    for name in sorted(declared):
+        assert getattr(lib, name) is not None, name
+    assert declared == set(binding.EXPORTS)
+
+
+def test_argument_validation_and_no_cpu_path(binding):
+    import torch
+    lib = binding.lib()
+    h = C.c_void_p()
+    cfg, pdf = binding.make_config(W.config(W.GG_TTG))
+    cfg.n_bins = 100                                   # invalid: validated before any device work
+    assert lib.mf_vegas_create(C.byref(cfg), C.byref(h)) == binding.MF_EINVAL
+    assert b"n_bins" in lib.mf_last_error()
+    cfg, pdf = binding.make_config(W.config(W.GG_TTG))
+    cfg.struct_size = 8
+    assert lib.mf_vegas_create(C.byref(cfg), C.byref(h)) == binding.MF_EINVAL
+    cfg, pdf = binding.make_config(W.config(W.GG_TTG))
+    cfg.precision = 32
+    assert lib.mf_vegas_create(C.byref(cfg), C.byref(h)) == binding.MF_EUNSUPPORTED
+    if not torch.cuda.is_available():                  # no CPU fallback: a valid config fails loudly
+        cfg, pdf = binding.make_config(W.config(W.GG_TTG))
+        assert lib.mf_vegas_create(C.byref(cfg), C.byref(h)) == binding.MF_ECUDA
+        assert b"no CUDA device" in lib.mf_last_error()
+        with pytest.raises(binding.MfError):
+            binding.Vegas(W.config(W.GG_TT))
+    assert lib.mf_result(None, None) == binding.MF_EINVAL
+
+
+# ---- the amplitude generator, evaluated with NumPy, against the oracle -----------------------------
+def _ferm(p, m):
+    E, px, py, pz = p
+    pabs = math.sqrt(px * px + py * py + pz * pz); pt2 = px * px + py * py
+    wp = math.sqrt(E + pabs); wm = 0.0 if m == 0 else m / wp
+    if pabs < 1e-12 * abs(E) or (pt2 == 0 and pz < 0):
+        return wp, wm, 0.0, 1.0, 0.0
+    ppz = pabs + pz if pz >= 0 else pt2 / (pabs - pz)
+    N = 1 / math.sqrt(2 * pabs * ppz)
+    return wp, wm, N * ppz, N * px, N * py
+
+
+def _glu(k):
+    E, px, py, pz = k
+    pt = math.hypot(px, py); pabs = math.sqrt(px * px + py * py + pz * pz); s = 1 / math.sqrt(2)
+    return px * pz / (pabs * pt) * s, py * pz / (pabs * pt) * s, -pt / pabs * s, -py / pt * s, px / pt * s
+
+
+def _inputs(gen, mom, mt=173.0):
+    v = dict(E=mom[0][0], mt=mt)
+    for n, c in zip(("p3e", "p3x", "p3y", "p3z"), mom[2]): v[n] = c
+    for n, c in zip(("p4e", "p4x", "p4y", "p4z"), mom[3]): v[n] = c
+    for n, c in zip(("wp", "wm", "c0", "cx", "cy"), _ferm(mom[2], mt)): v["t_" + n] = c
+    for n, c in zip(("wp", "wm", "c0", "cx", "cy"), _ferm(mom[3], mt)): v["b_" + n] = c
+    for l in range(2, gen.ng):
+        for n, c in zip("exyz", mom[2 + l]): v["k%d%s" % (l, n)] = c
+        for n, c in zip(("e1x", "e1y", "e1z", "e2x", "e2y"), _glu(mom[2 + l])): v["g%d_%s" % (l, n)] = c
+    return v
+
+
+@pytest.mark.parametrize("proc,fname,n", [(1, "mf_me2_gg_tt", 2), (2, "mf_me2_gg_ttg", 3), (3, "mf_me2_gg_ttgg", 4)])
+def test_generated_amplitude_dag_matches_oracle(mfo, proc, fname, n):
+    from paper_2105_10529_b200.gen import amplitudes as A
+    gen = A.generate(fname)
+    text, tot = A.emit_function(gen, fname)
+    assert "%s_NFMA %dull" % (fname.upper(), tot["fma"]) in text
+    gs2 = 4 * math.pi * 0.118
+    rng = np.random.default_rng(17 + proc)
+    for trial in range(4 if proc < 3 else 2):
+        rts = rng.uniform(450, 4000)
+        ps = mfo.phase_space(n, rts * rts, [173.0, 173.0] + [0.0] * (n - 2), rng.uniform(0.03, 0.97, 3 * n - 4))
+        mom = np.zeros((2 + n, 4)); mom[0] = [rts / 2, 0, 0, rts / 2]; mom[1] = [rts / 2, 0, 0, -rts / 2]; mom[2:] = ps["k"]
+        ref = mfo.me2(proc, mom)
+        val = float(A.evaluate(gen, _inputs(gen, mom))) * gen.scale * gs2 ** n / 256
+        assert abs(val / ref - 1) < 1e-11
+
+
+def test_generator_colour_matrices_match_golden():
+    from paper_2105_10529_b200.gen import amplitudes as A
+    from conftest import read_golden
+    g = read_golden("points.txt")
+    for ng in (2, 3, 4):
+        num, den, perms = A.colour_matrix(ng)
+        assert den == int(g["C%d_den" % ng][0])
+        assert list(num[0]) == [int(v) for v in g["C%d_row0" % ng]]
+        assert (num == num.T).all()

@@ -1,0 +1,77 @@
+"""World-size-2 gloo test (CPU) of the sharded-iteration plumbing (paper_2105_10529_b200/sharding.py):
+event ranges, the one all-reduce of the raw sums, identical grids on every rank.  The device handle is
+replaced by an adapter over the oracle (same method names as the C-ABI binding)."""
+import os
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+from paper_2105_10529_b200 import sharding, workloads as W
+
+
+class OracleHandle:
+    """binding.Vegas look-alike on host memory (tests only)"""
+
+    def __init__(self, cfg):
+        from oracle import mfo
+        self.v = mfo.Vegas(cfg)
+        self.d, self.n_bins = self.v.d, self.v.n_bins
+        self.iteration = 0
+        self.acc = np.zeros(2 + self.d * self.n_bins); self.cnt = np.zeros(2, np.uint64)
+
+    def set_accum(self, acc, counts):
+        self.acc = np.array(acc, dtype=np.float64); self.cnt = np.array(counts, dtype=np.uint64)
+
+    def get_accum(self):
+        return self.acc.copy(), self.cnt.copy()
+
+    def vegas_accumulate(self, first, n, n_total, stream=None):
+        acc, cnt = self.v.accumulate(self.iteration, first, n, n_total, n_threads=2, acc=self.acc.copy())
+        self.acc = acc; self.cnt = self.cnt + cnt
+
+    def vegas_finalize(self, n_total, stream=None):
+        self.iteration += 1
+        return self.v.finalize(self.acc, n_total, self.cnt[0], self.cnt[1])
+
+
+def test_shard_ranges_cover_the_iteration():
+    for n, world in ((10, 3), (10_000_000, 8), (7, 8), (1, 2)):
+        spans = [sharding.shard_range(n, r, world) for r in range(world)]
+        assert spans[0][0] == 0 and sum(c for _, c in spans) == n
+        for (f0, c0), (f1, _) in zip(spans, spans[1:]):
+            assert f0 + c0 == f1
+
+
+def _worker(rank, world, port, q):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    h = OracleHandle(W.config(W.GG_TT, seed=3))
+    out = []
+    for _ in range(2):
+        it = sharding.sharded_iterate(h, 6001, rank, world, dist)
+        out.append((it["integral"], it["sigma"], it["n_pass"]))
+    q.put((rank, out, h.v.get_grid()))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_rank_iteration_matches_single_process(mfo):
+    port = 29500 + os.getpid() % 2000
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = sorted([q.get(timeout=300) for _ in procs], key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    single = mfo.Vegas(W.config(W.GG_TT, seed=3))
+    ref = [single.iterate(6001, n_threads=2) for _ in range(2)]
+    for rank, out, grid in got:
+        for (I, s, npass), r in zip(out, ref):
+            assert abs(I / r["integral"] - 1) < 1e-12 and abs(s / r["sigma"] - 1) < 1e-9 and npass == r["n_pass"]
+        np.testing.assert_allclose(grid, single.get_grid(), rtol=0, atol=1e-13)
+    np.testing.assert_array_equal(got[0][2], got[1][2])      # every rank holds the same grid, bit for bit

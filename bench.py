@@ -205,7 +205,7 @@ def run_ours(args, rank, local_rank, world):
                 "d2h_bytes_per_step": grid_bytes + 40},
         "gpu_launches": 3 * args.steps,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                     "traffic": None, "kernel": "mf_iterate_kernel<2>", "kernel_ms": k_ms,
+                     "traffic": None, "kernel": "mf_iterate_compact_kernel<2>", "kernel_ms": k_ms,
                      "flops_per_event": flops["flops"], "fma_fraction_of_ops": flops["fma"] / (flops["add"] + flops["mul"] + flops["fma"]),
                      "peak_source": "measured DFMA-chain microbenchmark (mf_fp64_peak), max of before/after the timed region",
                      "peak_before": peak_before / 1e12, "peak_after": peak_after / 1e12,

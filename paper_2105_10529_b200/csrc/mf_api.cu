@@ -40,11 +40,6 @@ struct mf_vegas {
   bool have_k, have_it;                // events recorded (fused kernel / whole iteration)
 };
 
-static size_t iter_smem_bytes(const MfParams& P, int threads) {
-  const int nw = threads / 32;
-  return sizeof(double) * ((size_t)P.d * (P.nb + 1) + (size_t)P.pdf_nx * P.pdf_nq + (size_t)nw * P.d * P.nb + (size_t)nw * 4);
-}
-
 extern "C" int mf_vegas_create(const mf_config_t* cfg, mf_vegas_t** out) {
   if (!out) return fail(MF_EINVAL, "out is NULL");
   *out = nullptr;
@@ -65,10 +60,8 @@ extern "C" int mf_vegas_create(const mf_config_t* cfg, mf_vegas_t** out) {
   do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { std::string m_ = std::string(#call) + ": " + cudaGetErrorString(e_); mf_vegas_destroy(h); return fail(MF_ECUDA, m_); } } while (0)
   MF_CREATE_CUDA(cudaSetDevice(h->device));
   MF_CREATE_CUDA(cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device));
-  h->smem_iter = iter_smem_bytes(P, MF_THREADS);
-  h->smem_eval = sizeof(double) * ((size_t)P.d * (P.nb + 1) + (size_t)P.pdf_nx * P.pdf_nq);
   h->ops = mf_proc_ops(P.process);
-  MF_CREATE_CUDA(h->ops->setup(h->smem_iter, h->smem_eval, &h->occ_iter, &h->occ_eval));
+  MF_CREATE_CUDA(h->ops->setup(P, &h->smem_iter, &h->smem_eval, &h->occ_iter, &h->occ_eval));
   if (h->occ_iter < 1 || h->occ_eval < 1) { mf_vegas_destroy(h); return fail(MF_ECUDA, "kernel does not fit on an SM"); }
   h->max_blocks = h->n_sm * 32;
   const size_t ne = (size_t)P.d * (P.nb + 1), npdf = (size_t)P.pdf_nx * P.pdf_nq;

@@ -35,6 +35,13 @@ static inline double rsqrt(double x) { return 1.0 / sqrt(x); }
 #else
 #define MF_SYNC_POINT(i) do { } while (0)
 #endif
+// opaque identity on a double: stops the compiler from hoisting what is computed from it out of the
+// helicity loop (the generator decides what is hoisted: gen/dag.py Dag.plan)
+#if defined(__CUDA_ARCH__)
+#define MF_LAUNDER(x) asm volatile("" : "+d"(x))
+#else
+#define MF_LAUNDER(x) do { } while (0)
+#endif
 #ifndef MF_UNIFORM_ME
 #define MF_UNIFORM_ME (MF_SYNC_EVERY > 0)
 #endif

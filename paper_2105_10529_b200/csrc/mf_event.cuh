@@ -71,32 +71,30 @@ MF_HD double mf_me2(const MfParams& P, double rts, const double k[MfProc<PROC>::
   }
 }
 
-// One event.  edges: [d][nb+1], pdf_tab: [nx][nq] (both in shared memory on the device).
-// bin[] receives the VEGAS bins (needed by the histogram); rec (nullable) the debug record.
+// Front end of one event, S1-S6 + the weight prefactor: F = pref * |M|^2 for a passing event with
+//   config 0   : pref = J_V (1/(8 pi)) K / (2 s)
+//   configs 1-3: pref = J_V J_x f_g(x1) f_g(x2) S_f W_0 W_m K / (2 shat)
+// edges: [d][nb+1], pdf_tab: [nx][nq] (both in shared memory on the device).  Returns the cut flag.
 template <int PROC, bool REC>
-MF_HD double mf_event(const MfParams& P, const double* edges, const double* pdf_tab,
-                      uint32_t iteration, uint64_t ev, int bin[MfProc<PROC>::D], bool& pass,
-                      MfEventRec* rec) {
+MF_HD bool mf_event_front(const MfParams& P, const double* edges, const double* pdf_tab, uint32_t iteration,
+                          uint64_t ev, int bin[MfProc<PROC>::D], double k[MfProc<PROC>::N][4], double& rts,
+                          double& pref, MfEventRec* rec) {
   constexpr int D = MfProc<PROC>::D, N = MfProc<PROC>::N, NGL = MfProc<PROC>::NGL;
   double u[D], y[D];
   mf_uniforms<D>(P, iteration, ev, u);                                   // S1
   const double JV = mf_vegas_map<D>(edges, P.nb, u, y, bin);             // S2
   double x1 = 1.0, x2 = 1.0, shat = P.s, jx = 1.0;
   if (PROC != 0) mf_x_map(P, y[0], y[1], x1, x2, shat, jx);              // S3
-  double k[N][4];
   const double wps = mf_phase_space<N>(shat, PROC == 0 ? 0.0 : P.m_top, y + (PROC == 0 ? 0 : 2), k);   // S4
-  const double rts = sqrt(shat);
-  pass = mf_cuts<NGL>(P, (const double(*)[4])(&k[0][0] + 8), x1, x2);   // S5 (final gluons = k[2..])
+  rts = sqrt(shat);
+  const bool pass = mf_cuts<NGL>(P, (const double(*)[4])(&k[0][0] + 8), x1, x2);   // S5 (final gluons = k[2..])
   double f1 = 1.0, f2 = 1.0, xf1 = 0.0, xf2 = 0.0;
-  if (PROC != 0) {                                                       // S6
+  if (PROC != 0 && (REC || pass)) {                                      // S6
     xf1 = mf_pdf(P, pdf_tab, x1, P.pdf_lq);
     xf2 = mf_pdf(P, pdf_tab, x2, P.pdf_lq);
     f1 = xf1 / x1; f2 = xf2 / x2;
   }
-  double me2 = 0.0, F = 0.0;
-  if (MF_UNIFORM_ME || pass) me2 = mf_me2<PROC>(P, rts, k);              // S7
-  if (pass) F = JV * jx * f1 * f2 * me2 * wps * P.wconst / shat;         // S8
-  else me2 = 0.0;
+  pref = JV * jx * f1 * f2 * wps * P.wconst / shat;                      // S8 without |M|^2
   if (REC) {
 #pragma unroll
     for (int j = 0; j < D; ++j) rec->y[j] = y[j];
@@ -107,7 +105,23 @@ MF_HD double mf_event(const MfParams& P, const double* edges, const double* pdf_
     for (int i = 0; i < N; ++i)
 #pragma unroll
       for (int c = 0; c < 4; ++c) rec->mom[2 + i][c] = k[i][c];
-    rec->me2 = me2; rec->pdf[0] = xf1; rec->pdf[1] = xf2; rec->pass = pass ? 1 : 0;
+    rec->pdf[0] = xf1; rec->pdf[1] = xf2; rec->pass = pass ? 1 : 0;
   }
-  return F;
+  return pass;
+}
+
+// One whole event: front end, then S7 and S8.  bin[] receives the VEGAS bins; rec (nullable) the
+// debug record.
+template <int PROC, bool REC>
+MF_HD double mf_event(const MfParams& P, const double* edges, const double* pdf_tab,
+                      uint32_t iteration, uint64_t ev, int bin[MfProc<PROC>::D], bool& pass,
+                      MfEventRec* rec) {
+  constexpr int N = MfProc<PROC>::N;
+  double k[N][4], rts, pref;
+  pass = mf_event_front<PROC, REC>(P, edges, pdf_tab, iteration, ev, bin, k, rts, pref, rec);
+  double me2 = 0.0;
+  if (MF_UNIFORM_ME || pass) me2 = mf_me2<PROC>(P, rts, k);              // S7
+  if (!pass) me2 = 0.0;
+  if (REC) rec->me2 = me2;
+  return pass ? pref * me2 : 0.0;                                        // S8
 }

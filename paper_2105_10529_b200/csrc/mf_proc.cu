@@ -100,6 +100,132 @@ mf_iterate_kernel(const MfParams P, const double* __restrict__ g_edges, const do
   }
 }
 
+// ---- S1-S9 fused, with CTA-level compaction of the events that pass the cuts -------------------------
+// Phase A: every thread runs the front end (S1-S6) of one event; the passing ones are appended, in
+// event order (ballot + prefix over the warps, so the order is deterministic), to a queue in shared
+// memory holding {momenta, sqrt(shat), weight prefactor, bins}.  Phase B: once the queue holds a full
+// CTA of events (or the input is exhausted) every thread takes one entry and runs S7-S9.  All lanes
+// of every warp then carry a passing event through the |M|^2 code (no idle lanes at an 85 % pass
+// rate), and all threads reach the barrier points inside it.
+template <int PROC>
+__global__ void __launch_bounds__(MF_THREADS, MfLaunch<PROC>::MINB)
+mf_iterate_compact_kernel(const MfParams P, const double* __restrict__ g_edges, const double* __restrict__ g_pdf,
+                          uint32_t iteration, unsigned long long first, unsigned long long n, double n_total,
+                          double* __restrict__ partial, unsigned long long* __restrict__ pcount) {
+  constexpr int D = MfProc<PROC>::D, N = MfProc<PROC>::N, NF = 4 * N + 3, T = MF_THREADS, CAP = 2 * MF_THREADS;
+  extern __shared__ double smem[];
+  const int nb = P.nb, nh = D * nb, nw = T >> 5;
+  double* s_edges = smem;
+  double* s_pdf = s_edges + D * (nb + 1);
+  double* s_hist = s_pdf + P.pdf_nx * P.pdf_nq;          // [nw][D*nb]
+  double* s_red = s_hist + nw * nh;                      // [nw][4]
+  double* s_q = s_red + nw * 4;                          // [NF][CAP] field-major queue
+  int* s_wtot = (int*)(s_q + NF * CAP);                  // [nw]
+  mf_stage_tables(P, g_edges, g_pdf, s_edges, s_pdf);
+  for (int i = threadIdx.x; i < nw * nh; i += T) s_hist[i] = 0.0;
+  __syncthreads();
+
+  const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  const unsigned lt_mask = (1u << lane) - 1u;
+  double* hw = s_hist + warp * nh;
+  double s1 = 0.0, s2 = 0.0;
+  unsigned long long n_pass = 0, n_bad = 0;
+  const unsigned long long nchunks = (n + T - 1) / T;
+  unsigned long long chunk = blockIdx.x;
+  int qhead = 0, qcount = 0;                             // block-uniform
+  while (true) {
+    while (qcount < T && chunk < nchunks) {              // ---- phase A
+      const unsigned long long i = chunk * T + tid;
+      bool pass = false;
+      int bin[D];
+      double k[N][4], rts, pref;
+      if (i < n) pass = mf_event_front<PROC, false>(P, s_edges, s_pdf, iteration, first + i, bin, k, rts, pref, nullptr);
+      const unsigned bal = __ballot_sync(0xffffffffu, pass);
+      if (lane == 0) s_wtot[warp] = __popc(bal);
+      __syncthreads();
+      int base = 0, tot = 0;
+      for (int w = 0; w < nw; ++w) { const int c = s_wtot[w]; base += (w < (int)warp) ? c : 0; tot += c; }
+      if (pass) {
+        ++n_pass;
+        const int slot = (qhead + qcount + base + __popc(bal & lt_mask)) % CAP;
+#pragma unroll
+        for (int p = 0; p < N; ++p)
+#pragma unroll
+          for (int c = 0; c < 4; ++c) s_q[(4 * p + c) * CAP + slot] = k[p][c];
+        s_q[(4 * N) * CAP + slot] = rts;
+        s_q[(4 * N + 1) * CAP + slot] = pref;
+        unsigned long long packed = 0;                   // D <= 10 bins of 6 bits
+#pragma unroll
+        for (int j = 0; j < D; ++j) packed |= (unsigned long long)bin[j] << (6 * j);
+        s_q[(4 * N + 2) * CAP + slot] = __longlong_as_double((long long)packed);
+      }
+      __syncthreads();
+      qcount += tot;
+      chunk += gridDim.x;
+    }
+    if (qcount == 0) break;
+    const int m = qcount < T ? qcount : T;               // ---- phase B
+    const bool have = (int)tid < m;
+    const int slot = (qhead + (have ? (int)tid : 0)) % CAP;
+    double k[N][4];
+#pragma unroll
+    for (int p = 0; p < N; ++p)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) k[p][c] = s_q[(4 * p + c) * CAP + slot];
+    const double rts = s_q[(4 * N) * CAP + slot], pref = s_q[(4 * N + 1) * CAP + slot];
+    const unsigned long long packed = (unsigned long long)__double_as_longlong(s_q[(4 * N + 2) * CAP + slot]);
+    __syncthreads();                                     // queue entries are in registers before anyone refills
+    double F = pref * mf_me2<PROC>(P, rts, k);           // S7, S8 (every thread: barrier points inside)
+    if (!have) F = 0.0;
+    if (!isfinite(F)) { F = 0.0; ++n_bad; }
+    const double t = F / n_total, t2 = t * t;
+    s1 += t; s2 += t2;
+    const bool contrib = have && t2 != 0.0;
+#pragma unroll
+    for (int j = 0; j < D; ++j) {
+      const unsigned key = contrib ? (unsigned)((packed >> (6 * j)) & 63ull) : 64u + lane;
+      const unsigned peers = __match_any_sync(0xffffffffu, key);
+      const unsigned rank = __popc(peers & lt_mask);
+      const unsigned maxr = __reduce_max_sync(0xffffffffu, rank);
+      for (unsigned r = 0; r <= maxr; ++r) {
+        if (contrib && rank == r) hw[j * nb + key] += t2;
+        __syncwarp();
+      }
+    }
+    qhead = (qhead + m) % CAP;
+    qcount -= m;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+    s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+    n_pass += __shfl_xor_sync(0xffffffffu, n_pass, o);
+    n_bad += __shfl_xor_sync(0xffffffffu, n_bad, o);
+  }
+  if (lane == 0) {
+    s_red[warp * 4 + 0] = s1; s_red[warp * 4 + 1] = s2;
+    s_red[warp * 4 + 2] = __longlong_as_double((long long)n_pass);
+    s_red[warp * 4 + 3] = __longlong_as_double((long long)n_bad);
+  }
+  __syncthreads();
+  double* out = partial + (size_t)blockIdx.x * (2 + nh);
+  for (int e = tid; e < nh; e += T) {
+    double s = 0.0;
+    for (int w = 0; w < nw; ++w) s += s_hist[w * nh + e];
+    out[2 + e] = s;
+  }
+  if (tid == 0) {
+    double a = 0.0, b = 0.0; unsigned long long c = 0, d2 = 0;
+    for (int w = 0; w < nw; ++w) {
+      a += s_red[w * 4 + 0]; b += s_red[w * 4 + 1];
+      c += (unsigned long long)__double_as_longlong(s_red[w * 4 + 2]);
+      d2 += (unsigned long long)__double_as_longlong(s_red[w * 4 + 3]);
+    }
+    out[0] = a; out[1] = b;
+    pcount[2 * blockIdx.x] = c; pcount[2 * blockIdx.x + 1] = d2;
+  }
+}
+
 // ---- S1-S8 with per-event outputs -------------------------------------------------------------------
 template <int PROC, bool REC>
 __global__ void __launch_bounds__(MF_THREADS, MfLaunch<PROC>::MINB)
@@ -144,19 +270,34 @@ mf_eval_kernel(const MfParams P, const double* __restrict__ g_edges, const doubl
 }
 
 
-static cudaError_t proc_setup(size_t smem_iter, size_t smem_eval, int* occ_iter, int* occ_eval) {
-  cudaError_t e;
-  e = cudaFuncSetAttribute(mf_iterate_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_iter);
-  if (e) return e;
-  e = cudaFuncSetAttribute(mf_eval_kernel<MF_PROC, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_eval);
-  if (e) return e;
-  e = cudaFuncSetAttribute(mf_eval_kernel<MF_PROC, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_eval);
-  if (e) return e;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_iter, mf_iterate_kernel<MF_PROC>, MF_THREADS, smem_iter);
-  if (e) return e;
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_eval, mf_eval_kernel<MF_PROC, false>, MF_THREADS, smem_eval);
-}
+#ifndef MF_COMPACT
+#define MF_COMPACT 1                 // CTA-level compaction of passing events for the processes with cuts
+#endif
+static constexpr bool kCompact = MF_COMPACT && MfProc<MF_PROC>::NGL > 0;
 
+static cudaError_t proc_setup(const MfParams& P, size_t* smem_iter, size_t* smem_eval, int* occ_iter, int* occ_eval) {
+  const size_t tables = (size_t)P.d * (P.nb + 1) + (size_t)P.pdf_nx * P.pdf_nq;
+  const size_t nw = MF_THREADS / 32;
+  *smem_eval = sizeof(double) * tables;
+  *smem_iter = sizeof(double) * (tables + nw * P.d * P.nb + nw * 4);
+  if (kCompact) *smem_iter += sizeof(double) * (4 * MfProc<MF_PROC>::N + 3) * 2 * MF_THREADS + sizeof(int) * nw;
+  cudaError_t e;
+  if (kCompact) {
+    e = cudaFuncSetAttribute(mf_iterate_compact_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem_iter);
+    if (e) return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_iter, mf_iterate_compact_kernel<MF_PROC>, MF_THREADS, *smem_iter);
+  } else {
+    e = cudaFuncSetAttribute(mf_iterate_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem_iter);
+    if (e) return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_iter, mf_iterate_kernel<MF_PROC>, MF_THREADS, *smem_iter);
+  }
+  if (e) return e;
+  e = cudaFuncSetAttribute(mf_eval_kernel<MF_PROC, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem_eval);
+  if (e) return e;
+  e = cudaFuncSetAttribute(mf_eval_kernel<MF_PROC, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem_eval);
+  if (e) return e;
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_eval, mf_eval_kernel<MF_PROC, false>, MF_THREADS, *smem_eval);
+}
 static cudaError_t proc_eval(const MfParams& P, const double* edges, const double* pdf, uint32_t iteration,
                              unsigned long long first, unsigned long long n, const MfEvalOutDev& o, bool rec,
                              int grid, size_t smem, cudaStream_t st) {
@@ -168,7 +309,10 @@ static cudaError_t proc_eval(const MfParams& P, const double* edges, const doubl
 static cudaError_t proc_iterate(const MfParams& P, const double* edges, const double* pdf, uint32_t iteration,
                                 unsigned long long first, unsigned long long n, double n_total, double* partial,
                                 unsigned long long* pcount, int grid, size_t smem, cudaStream_t st) {
-  mf_iterate_kernel<MF_PROC><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount);
+  if (kCompact)
+    mf_iterate_compact_kernel<MF_PROC><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount);
+  else
+    mf_iterate_kernel<MF_PROC><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount);
   return cudaGetLastError();
 }
 

@@ -4,7 +4,7 @@
 #include "mf_kernels.cuh"
 
 struct MfProcOps {
-  cudaError_t (*setup)(size_t smem_iter, size_t smem_eval, int* occ_iter, int* occ_eval);
+  cudaError_t (*setup)(const MfParams& P, size_t* smem_iter, size_t* smem_eval, int* occ_iter, int* occ_eval);
   cudaError_t (*eval)(const MfParams& P, const double* edges, const double* pdf, uint32_t iteration,
                       unsigned long long first, unsigned long long n, const MfEvalOutDev& o, bool rec, int grid,
                       size_t smem, cudaStream_t st);

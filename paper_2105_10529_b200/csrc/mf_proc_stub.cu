@@ -1,6 +1,6 @@
 // mf_proc_stub.cu -- placeholder ops table for a process left out of a tuning build (build.py only=...)
 #include "mf_proc.h"
-static cudaError_t s_setup(size_t, size_t, int*, int*) { return cudaErrorNotSupported; }
+static cudaError_t s_setup(const MfParams&, size_t*, size_t*, int*, int*) { return cudaErrorNotSupported; }
 static cudaError_t s_eval(const MfParams&, const double*, const double*, uint32_t, unsigned long long, unsigned long long,
                           const MfEvalOutDev&, bool, int, size_t, cudaStream_t) { return cudaErrorNotSupported; }
 static cudaError_t s_iter(const MfParams&, const double*, const double*, uint32_t, unsigned long long, unsigned long long,

@@ -102,7 +102,10 @@ def slash_terms(s, psi):
 class Gen:
     """gg -> t tbar + (ng-2) g.  Gluon legs 0,1 incoming along +z/-z, legs 2.. outgoing."""
 
-    def __init__(self, ng, loop_legs=(), parity=True):
+    def __init__(self, ng, loop_legs=(), parity=True, loop_lam4=False):
+        """loop_legs: gluon legs whose helicity is a run-time loop symbol; loop_lam4: the antitop
+        helicity is a loop symbol too (leg id 4 in the loop list; v(lam4) is blended arithmetically)"""
+        self.loop_lam4 = loop_lam4
         self.ng, self.g = ng, Dag()
         g = self.g
         self.loop_legs = tuple(loop_legs)
@@ -124,6 +127,7 @@ class Gen:
             self.K.append([-c for c in k])
             self.g_ing.append([inp("g%d_%s" % (l, n)) for n in ("e1x", "e1y", "e1z", "e2x", "e2y")])
         self.lam_sym = {l: g.sym("lam%d" % l) for l in self.loop_legs}
+        self.lam4_sym = g.sym("lam9") if loop_lam4 else None
         self._P, self._j, self._sl, self._chi = {}, {}, {}, {}
 
     def _inp(self, name):
@@ -161,6 +165,10 @@ class Gen:
         return [u[2].conj(), u[3].conj(), u[0].conj(), u[1].conj()]      # u^dagger gamma^0
 
     def v4(self, lam):
+        if isinstance(lam, R):       # symbolic: v = (1+lam)/2 v(+) + (1-lam)/2 v(-)
+            vp, vm = self.v4(1), self.v4(-1)
+            sp, sm = 0.5 * lam + 0.5, 0.5 - 0.5 * lam
+            return [Cx(self.g.sop([(sp, a.re), (sm, b.re)]), self.g.sop([(sp, a.im), (sm, b.im)])) for a, b in zip(vp, vm)]
         wp, wm, cp, cm = self._chi_pm(self.b_ing)
         if lam > 0:      # v(+) = (-w+ chi- ; w- chi-)
             return [-(cm[0] * wp), -(cm[1] * wp), cm[0] * wm, cm[1] * wm]
@@ -243,7 +251,7 @@ class Gen:
 
     def chi(self, tau, hel, lam4):
         tau = tuple(tau)
-        key = (tau, tuple(id(hel[l]) if isinstance(hel[l], R) else hel[l] for l in tau), lam4)
+        key = (tau, tuple(id(hel[l]) if isinstance(hel[l], R) else hel[l] for l in tau), id(lam4) if isinstance(lam4, R) else lam4)
         if key in self._chi:
             return self._chi[key]
         g = self.g
@@ -301,7 +309,7 @@ class Gen:
             if self.parity:
                 hel[0] = 1
             hel.update(dict(zip(free, combo)))
-            for lam4 in (1, -1):
+            for lam4 in ((self.lam4_sym,) if self.loop_lam4 else (1, -1)):
                 amps = {1: [], -1: []}
                 for sg in perms:
                     a = self.partial_amps(sg, hel, lam4)
@@ -311,6 +319,8 @@ class Gen:
                     total = total + self.colour_form(amps[lam3], num)
         self.out = total
         self.scale = (2.0 if self.parity else 1.0) / den
+        if self.loop_lam4:
+            self.loop_legs = self.loop_legs + (9,)          # symbol lam9 = antitop helicity
         self.loop_assign = list(itertools.product((-1.0, 1.0), repeat=len(self.loop_legs)))
         return total
 
@@ -374,17 +384,25 @@ class GenEE:
 def emit_function(gen, fname):
     """CUDA/C++ text of `double fname(const double* in)` plus the flop-count macros."""
     g, out = gen.g, gen.out
-    pro = g.counts([out], dep_only=False)
-    body = g.counts([out], dep_only=True)
     nh = len(gen.loop_assign)
-    if not gen.loop_legs:           # no loop: everything is "prologue"
+    looped = bool(gen.loop_legs)
+    pro_ids, body_ids, hoisted = g.plan([out], getattr(gen, "max_hoist_cost", None) if looped else None)
+    pro, body = g.count_list(pro_ids), g.count_list(body_ids)
+    if not looped:
         tot = {k: pro[k] + body[k] for k in pro}
     else:
         tot = {k: pro[k] + nh * (body[k] + (1 if k == "add" else 0)) for k in pro}
+    emitted = dict(tot)
+    if looped:      # ALGORITHMIC count = every loop invariant computed once (recomputation is not counted)
+        p0, b0, _h = g.plan([out], None)
+        c0, c1 = g.count_list(p0), g.count_list(b0)
+        tot = {k: c0[k] + nh * (c1[k] + (1 if k == "add" else 0)) for k in c0}
     U = fname.upper()
     L = ["// GENERATED by paper_2105_10529_b200/gen/amplitudes.py -- do not edit.",
-         "// per event: %d add, %d mul, %d fma, %d rcp  (flops = add + mul + 2 fma = %d)"
+         "// per event (algorithmic): %d add, %d mul, %d fma, %d rcp  (flops = add + mul + 2 fma = %d)"
          % (tot["add"], tot["mul"], tot["fma"], tot["rcp"], tot["add"] + tot["mul"] + 2 * tot["fma"]),
+         "// emitted (cheap loop invariants recomputed per helicity-loop trip): %d add, %d mul, %d fma"
+         % (emitted["add"], emitted["mul"], emitted["fma"]),
          "#define %s_NADD %dull" % (U, tot["add"]), "#define %s_NMUL %dull" % (U, tot["mul"]),
          "#define %s_NFMA %dull" % (U, tot["fma"]), "#define %s_NIN %d" % (U, len(gen.input_names)),
          "#define %s_SCALE %r" % (U, gen.scale)]
@@ -392,26 +410,52 @@ def emit_function(gen, fname):
     L.append("MF_DEVFN double %s(const double* __restrict__ in) {" % fname)
     for i, n in enumerate(gen.input_names):
         L.append("  const double %s = in[%d];" % (n, i))
-    if not gen.loop_legs:
-        L += g.emit([out], False) + g.emit([out], True)
-        L.append("  return %s;" % g.ref(out))
+    leaf = lambda j: g.nodes[j][0] in ("in", "sym")
+    pname = lambda j: g.names[j] if leaf(j) else "p%d" % j
+    if not looped:
+        ids = sorted(set(pro_ids) | set(body_ids))
+        for i, line in enumerate(g.emit_list(ids, pname, "p")):
+            if i % 64 == 0 and len(ids) > 1024:
+                L.append("  MF_SYNC_POINT(%d);" % (i // 64))
+            L.append(line)
+        L.append("  return %s;" % _ref(g, out, pname))
     else:
-        L += g.emit([out], False)
+        L += g.emit_list(pro_ids, pname, "p")
         L.append("  double acc = 0.0;")
         L.append("#pragma unroll 1")
         L.append("  for (int ih = 0; ih < %d; ++ih) {" % nh)
         for b, l in enumerate(reversed(gen.loop_legs)):
             L.append("    const double lam%d = (ih & %d) ? 1.0 : -1.0;" % (l, 1 << b))
-        body = g.emit([out], True, indent="    ")
-        for i, line in enumerate(body):      # barrier points: keep the block's warps on the same I-cache lines
+        launder = getattr(gen, "max_hoist_cost", None) is not None
+        used_inputs = sorted({o for i in body_ids for o in g._operands(i) if g.nodes[o][0] == "in"})
+        if launder:       # opaque copies: keeps NVVM from hoisting the cheap invariants out again
+            for j in used_inputs:
+                L.append("    double %s_l = %s; MF_LAUNDER(%s_l);" % (g.names[j], g.names[j], g.names[j]))
+
+        def bname(j):
+            if g.nodes[j][0] == "in":
+                return g.names[j] + ("_l" if launder else "")
+            if g.nodes[j][0] == "sym":
+                return g.names[j]
+            return "p%d" % j if (j in hoisted and not g.dep[j] and j not in body_set) else "v%d" % j
+
+        body_set = set(body_ids)
+        body_lines = g.emit_list(body_ids, bname, "v", indent="    ")
+        for i, line in enumerate(body_lines):      # barrier points: keep the block's warps on the same I-cache lines
             if i % 64 == 0:
                 L.append("    MF_SYNC_POINT(%d);" % (i // 64))
             L.append(line)
-        L.append("    acc += %s;" % g.ref(out))
+        L.append("    acc += %s;" % _ref(g, out, bname))
         L.append("  }")
         L.append("  return acc;")
     L.append("}")
     return "\n".join(L) + "\n", tot
+
+
+def _ref(g, r, name):
+    if r.n is None:
+        return g._k(r.c)
+    return name(r.n) if r.s > 0 else "-" + name(r.n)
 
 
 def evaluate(gen, inputs):
@@ -424,17 +468,23 @@ def evaluate(gen, inputs):
     return total
 
 
+def _legs(env, default):
+    v = os.environ.get(env)
+    return default if v is None else tuple(int(x) for x in v.split(",") if x != "")
+
+
 PROCESSES = {
     "mf_me2_ee_mumu": lambda: GenEE(),
     "mf_me2_gg_tt": lambda: Gen(2, loop_legs=(), parity=True),
-    "mf_me2_gg_ttg": lambda: Gen(3, loop_legs=(1, 2), parity=True),
+    "mf_me2_gg_ttg": lambda: Gen(3, loop_legs=_legs("MF_GEN_TTG_LOOP", (1, 2)), parity=True,
+                                 loop_lam4=os.environ.get("MF_GEN_TTG_LAM4", "0") == "1"),
     "mf_me2_gg_ttgg": lambda: Gen(4, loop_legs=(1, 2, 3), parity=True),
 }
 
 
 # loop-invariant values with a cone of at most this many operations are recomputed in the loop body
 # (Dag.demote_cheap); tuned on B200, see DESIGN.md "Kernels / S7"
-DEMOTE = {"mf_me2_gg_ttg": int(os.environ.get("MF_GEN_DEMOTE_TTG", "0")),
+DEMOTE = {"mf_me2_gg_ttg": int(os.environ.get("MF_GEN_DEMOTE_TTG", "6")),
           "mf_me2_gg_ttgg": int(os.environ.get("MF_GEN_DEMOTE_TTGG", "0"))}
 
 
@@ -442,5 +492,5 @@ def generate(fname):
     gen = PROCESSES[fname]()
     gen.build()
     if DEMOTE.get(fname, 0) > 0:
-        gen.g.demote_cheap([gen.out], DEMOTE[fname])
+        gen.max_hoist_cost = DEMOTE[fname]
     return gen

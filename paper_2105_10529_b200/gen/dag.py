@@ -167,35 +167,55 @@ class Dag:
             acc = self.fma(a, b, acc)
         return acc
 
-    def demote_cheap(self, outputs, max_cost):
-        """Limit loop-invariant hoisting: an invariant node whose whole cone (down to the inputs) has
-        at most max_cost operations and no reciprocal is recomputed inside the loop instead of being
-        kept in a register across it (the hoisted values otherwise outnumber the register file)."""
+    def plan(self, outputs, max_cost=None):
+        """Split the live nodes into (prologue, body, hoisted).  max_cost None: every loop-invariant
+        node is hoisted.  Otherwise only EXPENSIVE invariants (cone with a reciprocal or more than
+        max_cost operations) that the body uses are hoisted; cheap ones are recomputed inside the
+        loop (and also in the prologue where a hoisted node needs them), because hoisting everything
+        keeps more values alive across the loop than the register file holds."""
         mark = self.live(outputs)
-        cone = [None] * len(self.nodes)
-        for i, (op, *_r) in enumerate(self.nodes):
-            if not mark[i] or self.dep[i]:
+        ids = [i for i in range(len(self.nodes)) if mark[i]]
+        leaf = lambda i: self.nodes[i][0] in ("in", "sym")
+        if max_cost is None:
+            pro = [i for i in ids if not self.dep[i] and not leaf(i)]
+            body = [i for i in ids if self.dep[i] and not leaf(i)]
+            return pro, body, set(pro)
+        cone = {}
+        for i in ids:
+            if self.dep[i]:
                 continue
-            if op in ("in", "sym"):
+            if leaf(i):
                 cone[i] = frozenset()
                 continue
-            c = {i}
-            big = op == "rcp"
+            c, big = {i}, self.nodes[i][0] == "rcp"
             for o in self._operands(i):
                 if cone[o] is None:
                     big = True
                 else:
                     c |= cone[o]
             cone[i] = None if (big or len(c) > max_cost) else frozenset(c)
-        stay = [False] * len(self.nodes)          # cheap nodes that a hoisted (expensive) node needs
-        for i in range(len(self.nodes) - 1, -1, -1):
-            if mark[i] and not self.dep[i] and (cone[i] is None or stay[i]):
-                for o in self._operands(i):
-                    stay[o] = True
-        for i in range(len(self.nodes)):
-            if (mark[i] and not self.dep[i] and cone[i] is not None and not stay[i]
-                    and self.nodes[i][0] not in ("in", "sym")):
-                self.dep[i] = True
+        body, hoisted = set(), set()
+        stack = [i for i in ids if self.dep[i] and not leaf(i)]
+        while stack:
+            i = stack.pop()
+            if i in body:
+                continue
+            body.add(i)
+            for o in self._operands(i):
+                if self.dep[o] or leaf(o):
+                    continue
+                if cone[o] is None:
+                    hoisted.add(o)
+                else:
+                    stack.append(o)
+        pro, stack = set(), list(hoisted)
+        while stack:
+            i = stack.pop()
+            if i in pro or leaf(i):
+                continue
+            pro.add(i)
+            stack.extend(self._operands(i))
+        return sorted(pro), sorted(body), hoisted
 
     # ---- analysis ------------------------------------------------------------------------------
     def _operands(self, i):
@@ -237,6 +257,25 @@ class Dag:
             elif op == "rcp":
                 c["rcp"] += 1
         return c
+
+    def count_list(self, ids):
+        c = dict(add=0, mul=0, fma=0, rcp=0)
+        for i in ids:
+            op = self.nodes[i][0]
+            if op in ("add", "sub", "addk"):
+                c["add"] += 1
+            elif op in ("mul", "mulk"):
+                c["mul"] += 1
+            elif op in ("fma", "fms"):
+                c["fma"] += 1
+            elif op == "rcp":
+                c["rcp"] += 1
+        return c
+
+    def emit_list(self, ids, name, prefix, indent="  "):
+        """C statements for the given nodes (ascending id = topological order); name(j) gives the C
+        identifier of operand j"""
+        return ["%sconst double %s%d = %s;" % (indent, prefix, i, self._expr(i, name)) for i in ids]
 
     # ---- emission ------------------------------------------------------------------------------
     @staticmethod

@@ -123,6 +123,8 @@ def run_ours(args, rank, local_rank, world):
     n, n_total = args.events, args.events * world
     cfg = W.config(W.GG_TTG, seed=0, device=local_rank)
     h = binding.Vegas(cfg)
+    staged = args.path == "staged"
+    h.set_path(staged)
     flops = h.me_flops()
     uuid = "GPU-" + str(torch.cuda.get_device_properties(dev).uuid)
     peak_before = binding.fp64_peak(local_rank, 0.3)
@@ -146,11 +148,13 @@ def run_ours(args, rank, local_rank, world):
         step()
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    kernel_ms, pass_frac = [], []
+    kernel_ms, pass_frac, stage_ms = [], [], []
     e0.record()
     for _ in range(args.steps):
         step()
-        kernel_ms.append(h.last_kernel_ms()[0])        # waits for this step's fused kernel (event sync)
+        kernel_ms.append(h.last_kernel_ms()[0])        # waits for this step's dominant kernel (event sync)
+        if staged:
+            stage_ms.append(h.last_stage_ms())
     e1.record()
     barrier()
     ms = e0.elapsed_time(e1)
@@ -196,22 +200,28 @@ def run_ours(args, rank, local_rank, world):
         "config": {"workload": "configs[2]: pp->tt~g via gg->tt~g (16 diagrams, 6x6 colour matrix), massive 3-body RAMBO + "
                                "Newton, cuts pT>30 |eta|<2.5, VEGAS 7 dims x 50 bins, seed 0, successive iterations of one run",
                    "events_per_step_per_gpu": n, "pass_fraction": float(np.mean(pass_frac)),
-                   "l2": "flushed between steps (256 MiB memset inside the timed region); the path has no HBM inputs "
-                         "beyond 46 KB of tables", "parallelism": "event ranges over %d GPU(s), 1 all-reduce of 352 "
+                   "path": args.path,
+                   "l2": "flushed between steps (256 MiB memset inside the timed region); inputs are 46 KB of tables; "
+                         "the staged path passes ~1.0 GB of event records per step through HBM (> 126 MB L2)", "parallelism": "event ranges over %d GPU(s), 1 all-reduce of 352 "
                          "doubles per iteration" % world if world > 1 else "1 GPU",
                    "integral_pb": res["integral"], "sigma_pb": res["sigma"]},
         "clocks": clocks,
         "e2e": {"value": n_total * args.steps / e2e_s, "unit": "events/s", "h2d_bytes_per_step": grid_bytes,
                 "d2h_bytes_per_step": grid_bytes + 40},
-        "gpu_launches": 3 * args.steps,
+        "gpu_launches": (5 if staged else 3) * args.steps,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                     "traffic": None, "kernel": "mf_iterate_compact_kernel<2>", "kernel_ms": k_ms,
+                     "traffic": None, "kernel": "mf_me_kernel<2>" if staged else "mf_iterate_compact_kernel<2>", "kernel_ms": k_ms,
                      "flops_per_event": flops["flops"], "fma_fraction_of_ops": flops["fma"] / (flops["add"] + flops["mul"] + flops["fma"]),
                      "peak_source": "measured DFMA-chain microbenchmark (mf_fp64_peak), max of before/after the timed region",
                      "peak_before": peak_before / 1e12, "peak_after": peak_after / 1e12,
                      "peak_nominal": FP64_NOMINAL_TFLOPS, "frac_nominal": achieved / FP64_NOMINAL_TFLOPS,
                      "note": "algorithmic flops = generator-counted |M|^2 add+mul+2*fma per passing event; front end not counted"},
     }
+    if staged:
+        out["roofline"]["stages_ms"] = {k: float(np.mean([m[k] for m in stage_ms])) for k in ("front", "me", "reduce")}
+        rec_bytes = 15 * 8 * n_pass                                        # 4*3+3 doubles per passing event
+        out["roofline"]["front_stage_hbm_gbps"] = rec_bytes / (out["roofline"]["stages_ms"]["front"] * 1e-3) / 1e9
+        out["roofline"]["reduce_stage_hbm_gbps"] = 16 * n_pass / (out["roofline"]["stages_ms"]["reduce"] * 1e-3) / 1e9
     if world == 1 and not args.no_cpu_baseline:
         from oracle import mfo
         mfo.build()
@@ -230,6 +240,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--events", type=int, default=N_EVENTS, help="events per iteration per GPU")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--path", default="staged", choices=["staged", "fused"],
+                    help="staged: front end / |M|^2 / reductions as three kernels (default); fused: one kernel")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

@@ -79,10 +79,15 @@ int mf_ndim(const mf_vegas_t *h, uint32_t *d, uint32_t *n_final);
 int mf_integrand_eval(mf_vegas_t *h, uint32_t iteration, uint64_t first_event, uint64_t n_events,
                       const mf_eval_out_t *out, void *cuda_stream);
 
-/* One VEGAS iteration of n_events (>= 2) events: S1-S9 fused in one kernel (no per-event global
- * traffic), then S10 in a one-block finalize kernel: I, sigma, grid refinement, record appended on
- * the device.  Enqueue only, unless host_out_or_null != NULL: then the stream is synchronised and
- * the iteration record (kernel_ms = device time of the fused kernel) is returned.                            */
+/* One VEGAS iteration of n_events (>= 2) events (random numbers -> phase space -> matrix
+ * element -> accumulation), then S10 in a one-block finalize kernel: I, sigma, grid refinement, record
+ * appended on the device.  S1-S9 run either FUSED in one kernel (no per-event global traffic; the only
+ * path of processes 0 and 1) or STAGED (default for processes 2 and 3, mf_set_path): front end,
+ * |M|^2 and reductions as three kernels, each at its own occupancy, with 4 n_final + 3 doubles per
+ * cut-passing event passed through a library-owned device workspace (grown on demand, at most 2^24
+ * events per launch; larger iterations are processed in slices).  Enqueue only, unless
+ * host_out_or_null != NULL: then the stream is synchronised and the iteration record (kernel_ms =
+ * device time of the dominant kernel: fused kernel or |M|^2 stage) is returned.                      */
 int mf_vegas_iterate(mf_vegas_t *h, uint64_t n_events, void *cuda_stream, mf_iter_t *host_out_or_null);
 
 /* Sharded form of one iteration (multi-GPU): accumulate events
@@ -106,7 +111,15 @@ int mf_set_grid(mf_vegas_t *h, const double *host_edges);   /* edges must start 
 /* Launch geometry of the fused kernel: blocks per SM (0 = library default) and threads per block
  * (0 = default).  Results are deterministic for a fixed geometry.                                  */
 int mf_set_launch(mf_vegas_t *h, uint32_t blocks_per_sm, uint32_t threads_per_block);
-/* Device times (CUDA events on the caller's stream): of the fused S1-S9 kernel of the last
+/* Select the iteration path: staged != 0 -> staged (MF_EUNSUPPORTED for processes 0 and 1, which
+ * only have the fused kernel), 0 -> fused.  Both give the same per-event values; the summation
+ * order (hence the last bits of the sums) differs.                                                   */
+int mf_set_path(mf_vegas_t *h, int32_t staged);
+/* Device times of the three stages (front end, |M|^2, reductions; ms3[3], host) of the last staged
+ * launch.  MF_ESTATE if the last accumulate ran the fused path.  Waits for the events.              */
+int mf_last_stage_ms(const mf_vegas_t *h, float *ms3);
+/* Device times (CUDA events on the caller's stream): of the dominant S1-S9 kernel (fused kernel, or
+ * the |M|^2 stage of the staged path) of the last
  * mf_vegas_accumulate / mf_vegas_iterate, and of the whole last mf_vegas_iterate (memsets + fused
  * kernel + reduce + finalize).  Waits for those events to complete.                                 */
 int mf_last_kernel_ms(const mf_vegas_t *h, float *fused_kernel_ms, float *iteration_ms);

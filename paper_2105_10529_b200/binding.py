@@ -15,7 +15,7 @@ MF_OK, MF_EINVAL, MF_ENOMEM, MF_ECUDA, MF_ESTATE, MF_EUNSUPPORTED = 0, -1, -2, -
 EXPORTS = ["mf_vegas_create", "mf_vegas_destroy", "mf_ndim", "mf_integrand_eval", "mf_vegas_iterate",
            "mf_vegas_accumulate", "mf_get_accum", "mf_set_accum", "mf_vegas_finalize", "mf_result",
            "mf_get_iterations", "mf_get_grid", "mf_set_grid", "mf_set_launch", "mf_me_flops",
-           "mf_fp64_peak", "mf_last_kernel_ms", "mf_last_error"]
+           "mf_fp64_peak", "mf_last_kernel_ms", "mf_last_error", "mf_set_path", "mf_last_stage_ms"]
 
 
 class MfError(RuntimeError):
@@ -92,6 +92,8 @@ def lib():
         L.mf_get_grid.argtypes = [vp, vp]
         L.mf_set_grid.argtypes = [vp, vp]
         L.mf_set_launch.argtypes = [vp, u32, u32]
+        L.mf_set_path.argtypes = [vp, C.c_int32]
+        L.mf_last_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
         L.mf_me_flops.argtypes = [vp, C.POINTER(u64), C.POINTER(u64), C.POINTER(u64)]
         L.mf_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
         L.mf_fp64_peak.argtypes = [C.c_int32, C.c_double, C.POINTER(C.c_double)]
@@ -197,6 +199,14 @@ class Vegas:
 
     def set_launch(self, blocks_per_sm=0, threads_per_block=0):
         _check(lib().mf_set_launch(self._h, blocks_per_sm, threads_per_block))
+
+    def set_path(self, staged):
+        _check(lib().mf_set_path(self._h, 1 if staged else 0))
+
+    def last_stage_ms(self):
+        ms = (C.c_float * 3)()
+        _check(lib().mf_last_stage_ms(self._h, ms))
+        return dict(front=ms[0], me=ms[1], reduce=ms[2])
 
     def last_kernel_ms(self):
         a, b = C.c_float(), C.c_float()

@@ -38,7 +38,14 @@ struct mf_vegas {
   cudaStream_t last_stream;
   cudaEvent_t ev0, ev1, evk0, evk1;   // iteration start/end, fused-kernel start/end
   bool have_k, have_it;                // events recorded (fused kernel / whole iteration)
+  // staged path (heavy processes): records of the passing events go through HBM between the stages
+  int rec_fields, occ_front, occ_hist; // rec_fields = 0: the process has the fused path only
+  bool use_staged, have_stage;
+  MfStageWs ws;
+  size_t ws_doubles, ws_regions;       // allocated sizes
+  cudaEvent_t evs[4];                  // front start / |M|^2 start / |M|^2 end / reductions end
 };
+#define MF_STAGE_MAX_EVENTS (1ull << 24)   // events per staged launch (<= 2.1-2.6 GB of records)
 
 extern "C" int mf_vegas_create(const mf_config_t* cfg, mf_vegas_t** out) {
   if (!out) return fail(MF_EINVAL, "out is NULL");
@@ -63,6 +70,9 @@ extern "C" int mf_vegas_create(const mf_config_t* cfg, mf_vegas_t** out) {
   h->ops = mf_proc_ops(P.process);
   MF_CREATE_CUDA(h->ops->setup(P, &h->smem_iter, &h->smem_eval, &h->occ_iter, &h->occ_eval));
   if (h->occ_iter < 1 || h->occ_eval < 1) { mf_vegas_destroy(h); return fail(MF_ECUDA, "kernel does not fit on an SM"); }
+  MF_CREATE_CUDA(h->ops->staged_setup(P, &h->rec_fields, &h->occ_front, &h->occ_hist));
+  if (h->rec_fields && (h->occ_front < 1 || h->occ_hist < 1)) { mf_vegas_destroy(h); return fail(MF_ECUDA, "staged kernel does not fit on an SM"); }
+  h->use_staged = h->rec_fields > 0;
   h->max_blocks = h->n_sm * 32;
   const size_t ne = (size_t)P.d * (P.nb + 1), npdf = (size_t)P.pdf_nx * P.pdf_nq;
   MF_CREATE_CUDA(cudaMalloc(&h->d_edges, ne * sizeof(double)));
@@ -84,6 +94,7 @@ extern "C" int mf_vegas_create(const mf_config_t* cfg, mf_vegas_t** out) {
   MF_CREATE_CUDA(cudaEventCreate(&h->ev1));
   MF_CREATE_CUDA(cudaEventCreate(&h->evk0));
   MF_CREATE_CUDA(cudaEventCreate(&h->evk1));
+  for (int i = 0; i < 4; ++i) MF_CREATE_CUDA(cudaEventCreate(&h->evs[i]));
   *out = h;
   return MF_OK;
 }
@@ -93,6 +104,8 @@ extern "C" int mf_vegas_destroy(mf_vegas_t* h) {
   cudaSetDevice(h->device);
   cudaFree(h->d_edges); cudaFree(h->d_pdf); cudaFree(h->d_partial); cudaFree(h->d_pcount);
   cudaFree(h->d_acc); cudaFree(h->d_counts); cudaFree(h->d_state);
+  cudaFree(h->ws.rec); cudaFree(h->ws.count);
+  for (int i = 0; i < 4; ++i) if (h->evs[i]) cudaEventDestroy(h->evs[i]);
   if (h->ev0) cudaEventDestroy(h->ev0);
   if (h->ev1) cudaEventDestroy(h->ev1);
   if (h->evk0) cudaEventDestroy(h->evk0);
@@ -142,6 +155,35 @@ extern "C" int mf_integrand_eval(mf_vegas_t* h, uint32_t iteration, uint64_t fir
   return MF_OK;
 }
 
+extern "C" int mf_set_path(mf_vegas_t* h, int32_t staged) {
+  if (!h) return fail(MF_EINVAL, "handle is NULL");
+  if (staged && !h->rec_fields) return fail(MF_EUNSUPPORTED, "this process has the fused path only");
+  h->use_staged = staged != 0;
+  return MF_OK;
+}
+
+// workspace of one staged launch of n events: regions of `cap` consecutive events (a multiple of the
+// CTA size), about 4 front-end CTAs per resident slot so that the front-end grid fills whole waves
+static int ensure_ws(mf_vegas* h, unsigned long long n) {
+  const unsigned long long target = (unsigned long long)h->n_sm * h->occ_front * 4;
+  unsigned long long cap = (n + target - 1) / target;
+  cap = (cap + MF_THREADS - 1) / MF_THREADS * MF_THREADS;
+  const unsigned long long regions = (n + cap - 1) / cap;
+  const size_t need = (size_t)regions * h->rec_fields * cap;
+  if (need > h->ws_doubles) {
+    if (h->ws.rec) { MF_CUDA(cudaFree(h->ws.rec)); h->ws.rec = nullptr; h->ws_doubles = 0; }
+    MF_CUDA(cudaMalloc(&h->ws.rec, need * sizeof(double)));
+    h->ws_doubles = need;
+  }
+  if (regions > h->ws_regions) {
+    if (h->ws.count) { MF_CUDA(cudaFree(h->ws.count)); h->ws.count = nullptr; h->ws_regions = 0; }
+    MF_CUDA(cudaMalloc(&h->ws.count, regions * sizeof(unsigned int)));
+    h->ws_regions = regions;
+  }
+  h->ws.cap = cap; h->ws.regions = (int)regions;
+  return MF_OK;
+}
+
 extern "C" int mf_vegas_accumulate(mf_vegas_t* h, uint64_t first_event, uint64_t n_events, uint64_t n_total,
                                    void* cuda_stream) {
   if (!h) return fail(MF_EINVAL, "handle is NULL");
@@ -150,15 +192,42 @@ extern "C" int mf_vegas_accumulate(mf_vegas_t* h, uint64_t first_event, uint64_t
   if (n_events == 0) return MF_OK;
   MF_CUDA(cudaSetDevice(h->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (h->use_staged) {
+    for (uint64_t done = 0; done < n_events; done += MF_STAGE_MAX_EVENTS) {
+      const uint64_t m = n_events - done < MF_STAGE_MAX_EVENTS ? n_events - done : MF_STAGE_MAX_EVENTS;
+      int rc = ensure_ws(h, m);
+      if (rc) return rc;
+      const int per_sm = h->blocks_per_sm ? (int)h->blocks_per_sm : h->occ_iter;
+      const int grid_me = h->n_sm * per_sm;
+      int grid_hist = h->n_sm * h->occ_hist;
+      if (grid_hist > h->ws.regions) grid_hist = h->ws.regions;
+      if (grid_hist > h->max_blocks) grid_hist = h->max_blocks;
+      MF_CUDA(h->ops->staged(h->P, h->d_edges, h->d_pdf, h->iteration, first_event + done, m, (double)n_total, h->ws,
+                             h->d_partial, h->d_pcount, grid_me, grid_hist, st, h->evs));
+      mf_reduce_kernel<<<(h->na + 127) / 128, 128, 0, st>>>(h->d_partial, h->d_pcount, grid_hist, h->na, h->d_acc, h->d_counts);
+      MF_CUDA(cudaGetLastError());
+    }
+    h->have_stage = true; h->have_k = false;
+    h->last_stream = st;
+    return MF_OK;
+  }
   const int grid = grid_for(h, n_events, h->occ_iter);
   MF_CUDA(cudaEventRecord(h->evk0, st));
   MF_CUDA(h->ops->iterate(h->P, h->d_edges, h->d_pdf, h->iteration, first_event, n_events, (double)n_total,
                           h->d_partial, h->d_pcount, grid, h->smem_iter, st));
   MF_CUDA(cudaEventRecord(h->evk1, st));
-  h->have_k = true;
+  h->have_k = true; h->have_stage = false;
   mf_reduce_kernel<<<(h->na + 127) / 128, 128, 0, st>>>(h->d_partial, h->d_pcount, grid, h->na, h->d_acc, h->d_counts);
   MF_CUDA(cudaGetLastError());
   h->last_stream = st;
+  return MF_OK;
+}
+
+// duration of the dominant kernel of the last accumulate: the fused kernel, or the |M|^2 stage
+static int dominant_ms(mf_vegas* h, float* ms) {
+  *ms = 0.0f;
+  if (h->have_stage) MF_CUDA(cudaEventElapsedTime(ms, h->evs[1], h->evs[2]));
+  else if (h->have_k) MF_CUDA(cudaEventElapsedTime(ms, h->evk0, h->evk1));
   return MF_OK;
 }
 
@@ -190,7 +259,8 @@ extern "C" int mf_vegas_finalize(mf_vegas_t* h, uint64_t n_total, void* cuda_str
     MF_CUDA(cudaStreamSynchronize(st));
     int rc = fetch_iter(h, idx, host_out);
     if (rc) return rc;
-    if (h->have_k) MF_CUDA(cudaEventElapsedTime(&host_out->kernel_ms, h->evk0, h->evk1));
+    rc = dominant_ms(h, &host_out->kernel_ms);
+    if (rc) return rc;
   }
   return MF_OK;
 }
@@ -220,8 +290,18 @@ extern "C" int mf_vegas_iterate(mf_vegas_t* h, uint64_t n_events, void* cuda_str
     MF_CUDA(cudaStreamSynchronize(st));
     rc = fetch_iter(h, h->iteration - 1, host_out);
     if (rc) return rc;
-    MF_CUDA(cudaEventElapsedTime(&host_out->kernel_ms, h->evk0, h->evk1));
+    rc = dominant_ms(h, &host_out->kernel_ms);
+    if (rc) return rc;
   }
+  return MF_OK;
+}
+
+extern "C" int mf_last_stage_ms(const mf_vegas_t* h, float* ms3) {
+  if (!h || !ms3) return fail(MF_EINVAL, "null argument");
+  ms3[0] = ms3[1] = ms3[2] = 0.0f;
+  if (!h->have_stage) return fail(MF_ESTATE, "the last accumulate did not run the staged path");
+  MF_CUDA(cudaEventSynchronize(h->evs[3]));
+  for (int i = 0; i < 3; ++i) MF_CUDA(cudaEventElapsedTime(&ms3[i], h->evs[i], h->evs[i + 1]));
   return MF_OK;
 }
 
@@ -229,7 +309,8 @@ extern "C" int mf_last_kernel_ms(const mf_vegas_t* h, float* fused_kernel_ms, fl
   if (!h) return fail(MF_EINVAL, "handle is NULL");
   if (fused_kernel_ms) {
     *fused_kernel_ms = 0.0f;
-    if (h->have_k) { MF_CUDA(cudaEventSynchronize(h->evk1)); MF_CUDA(cudaEventElapsedTime(fused_kernel_ms, h->evk0, h->evk1)); }
+    if (h->have_stage) { MF_CUDA(cudaEventSynchronize(h->evs[2])); MF_CUDA(cudaEventElapsedTime(fused_kernel_ms, h->evs[1], h->evs[2])); }
+    else if (h->have_k) { MF_CUDA(cudaEventSynchronize(h->evk1)); MF_CUDA(cudaEventElapsedTime(fused_kernel_ms, h->evk0, h->evk1)); }
   }
   if (iteration_ms) {
     *iteration_ms = 0.0f;

@@ -226,6 +226,183 @@ mf_iterate_compact_kernel(const MfParams P, const double* __restrict__ g_edges, 
   }
 }
 
+// ---- staged iteration for the heavy processes: front end -> |M|^2 -> reductions, through HBM --------
+// The fused kernels above run the front end (S1-S6) at the occupancy of the |M|^2 code (255 registers,
+// 2 warps per scheduler), where it is latency-bound: 21 % of the fused kernel's time for 12 % of its
+// FP64 instructions (profiles/r1_v2_iterate_ttg_ncu.md).  The staged path gives every stage its own
+// launch shape and passes 4N+3 doubles per PASSING event through HBM (1.0 GB written + 1.0 GB read per
+// 1e7 events, ~0.3 ms at the measured 6.5 TB/s):
+//   mf_front_kernel  one CTA per REGION of `cap` consecutive events: S1-S6 and the weight prefactor,
+//                    ordered compaction (ballot + prefix over the warps) of the passing events into
+//                    the region's record block rec[region][field][cap] (field-major: coalesced)
+//   mf_me_kernel     persistent, one 256-thread CTA per SM: an exclusive prefix over the region counts
+//                    maps a dense index over ALL passing events to (region, entry), so every lane of
+//                    every warp carries a passing event through S7; writes F = pref |M|^2 in place
+//   mf_hist_kernel   S9: sum t, sum t^2 and the d x nb histogram in fixed order from (F, packed bins)
+// Field order of a record: k[N][4], sqrt(shat), pref (-> F), packed bins (6 bits per dimension).
+template <int PROC>
+__global__ void __launch_bounds__(MF_THREADS, 2)
+mf_front_kernel(const MfParams P, const double* __restrict__ g_edges, const double* __restrict__ g_pdf,
+                uint32_t iteration, unsigned long long first, unsigned long long n, unsigned long long cap,
+                double* __restrict__ rec, unsigned int* __restrict__ count) {
+  constexpr int D = MfProc<PROC>::D, N = MfProc<PROC>::N, NF = 4 * N + 3, T = MF_THREADS;
+  extern __shared__ double smem[];
+  double* s_edges = smem;
+  double* s_pdf = s_edges + D * (P.nb + 1);
+  int* s_wtot = (int*)(s_pdf + P.pdf_nx * P.pdf_nq);    // [T/32]
+  mf_stage_tables(P, g_edges, g_pdf, s_edges, s_pdf);
+  __syncthreads();
+  const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  const unsigned lt_mask = (1u << lane) - 1u;
+  const unsigned long long lo = (unsigned long long)blockIdx.x * cap;
+  const unsigned long long hi = lo + cap < n ? lo + cap : n;
+  double* R = rec + (size_t)blockIdx.x * NF * cap;
+  unsigned filled = 0;                                   // block-uniform
+  for (unsigned long long base = lo; base < hi; base += T) {
+    const unsigned long long i = base + tid;
+    bool pass = false;
+    int bin[D];
+    double k[N][4], rts, pref;
+    if (i < hi) pass = mf_event_front<PROC, false>(P, s_edges, s_pdf, iteration, first + i, bin, k, rts, pref, nullptr);
+    const unsigned bal = __ballot_sync(0xffffffffu, pass);
+    if (lane == 0) s_wtot[warp] = __popc(bal);
+    __syncthreads();
+    unsigned before = 0, tot = 0;
+#pragma unroll
+    for (int w = 0; w < T / 32; ++w) { const unsigned c = s_wtot[w]; before += (w < (int)warp) ? c : 0u; tot += c; }
+    if (pass) {
+      const size_t slot = filled + before + __popc(bal & lt_mask);
+#pragma unroll
+      for (int p = 0; p < N; ++p)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) R[(size_t)(4 * p + c) * cap + slot] = k[p][c];
+      R[(size_t)(4 * N) * cap + slot] = rts;
+      R[(size_t)(4 * N + 1) * cap + slot] = pref;
+      unsigned long long packed = 0;                     // D <= 10 bins of 6 bits
+#pragma unroll
+      for (int j = 0; j < D; ++j) packed |= (unsigned long long)bin[j] << (6 * j);
+      R[(size_t)(4 * N + 2) * cap + slot] = __longlong_as_double((long long)packed);
+    }
+    __syncthreads();
+    filled += tot;
+  }
+  if (tid == 0) count[blockIdx.x] = filled;
+}
+
+template <int PROC>
+__global__ void __launch_bounds__(MF_THREADS, MfLaunch<PROC>::MINB)
+mf_me_kernel(const MfParams P, double* __restrict__ rec, const unsigned int* __restrict__ count, int regions,
+             unsigned long long cap) {
+  constexpr int N = MfProc<PROC>::N, NF = 4 * N + 3, T = MF_THREADS;
+  extern __shared__ unsigned int s_pre[];                // [regions + 1] exclusive prefix, then s_part[T]
+  unsigned int* s_part = s_pre + regions + 1;
+  const unsigned tid = threadIdx.x;
+  {                                                      // block scan over the region counts
+    const int per = (regions + T - 1) / T, a = tid * per, b = (a + per < regions) ? a + per : regions;
+    unsigned s = 0;
+    for (int r = a; r < b; ++r) s += count[r];
+    s_part[tid] = s;
+    __syncthreads();
+    unsigned off = 0;
+    for (unsigned t = 0; t < tid; ++t) off += s_part[t];
+    for (int r = a; r < b; ++r) { s_pre[r] = off; off += count[r]; }
+    if (tid == T - 1) s_pre[regions] = off;
+    __syncthreads();
+  }
+  const unsigned M = s_pre[regions];
+  const unsigned nchunks = (M + T - 1) / T;
+  for (unsigned q = blockIdx.x; q < nchunks; q += gridDim.x) {     // block-uniform trips (barriers in S7)
+    const unsigned lin = q * T + tid;
+    const bool have = lin < M;
+    const unsigned l = have ? lin : M - 1;               // lanes past the end recompute the last event
+    int lo = 0, hi = regions;
+    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (s_pre[mid] <= l) lo = mid; else hi = mid; }
+    double* R = rec + (size_t)lo * NF * cap + (l - s_pre[lo]);
+    double k[N][4];
+#pragma unroll
+    for (int p = 0; p < N; ++p)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) k[p][c] = R[(size_t)(4 * p + c) * cap];
+    const double rts = R[(size_t)(4 * N) * cap], pref = R[(size_t)(4 * N + 1) * cap];
+    const double F = pref * mf_me2<PROC>(P, rts, k);     // S7, S8
+    if (have) R[(size_t)(4 * N + 1) * cap] = F;
+  }
+}
+
+template <int PROC>
+__global__ void __launch_bounds__(MF_THREADS)
+mf_hist_kernel(const MfParams P, const double* __restrict__ rec, const unsigned int* __restrict__ count, int regions,
+               unsigned long long cap, double n_total, double* __restrict__ partial,
+               unsigned long long* __restrict__ pcount) {
+  constexpr int D = MfProc<PROC>::D, N = MfProc<PROC>::N, NF = 4 * N + 3, T = MF_THREADS;
+  extern __shared__ double smem[];
+  const int nb = P.nb, nh = D * nb, nw = T >> 5;
+  double* s_hist = smem;                                 // [nw][D*nb]
+  double* s_red = s_hist + nw * nh;                      // [nw][4]
+  for (int i = threadIdx.x; i < nw * nh; i += T) s_hist[i] = 0.0;
+  __syncthreads();
+  const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  const unsigned lt_mask = (1u << lane) - 1u;
+  double* hw = s_hist + warp * nh;
+  double s1 = 0.0, s2 = 0.0;
+  unsigned long long n_pass = 0, n_bad = 0;
+  for (int r = blockIdx.x; r < regions; r += gridDim.x) {
+    const unsigned c = count[r];
+    const double* R = rec + (size_t)r * NF * cap;
+    for (unsigned e0 = warp * 32u; e0 < c; e0 += T) {    // warp-uniform trips
+      const unsigned e = e0 + lane;
+      const bool have = e < c;
+      double F = have ? R[(size_t)(4 * N + 1) * cap + e] : 0.0;
+      const unsigned long long packed = have ? (unsigned long long)__double_as_longlong(R[(size_t)(4 * N + 2) * cap + e]) : 0ull;
+      if (have) ++n_pass;
+      if (!isfinite(F)) { F = 0.0; ++n_bad; }            // A20
+      const double t = F / n_total, t2 = t * t;          // O9
+      s1 += t; s2 += t2;
+      const bool contrib = have && t2 != 0.0;
+#pragma unroll
+      for (int j = 0; j < D; ++j) {
+        const unsigned key = contrib ? (unsigned)((packed >> (6 * j)) & 63ull) : 64u + lane;
+        const unsigned peers = __match_any_sync(0xffffffffu, key);
+        const unsigned rank = __popc(peers & lt_mask);
+        const unsigned maxr = __reduce_max_sync(0xffffffffu, rank);
+        for (unsigned rr = 0; rr <= maxr; ++rr) {
+          if (contrib && rank == rr) hw[j * nb + key] += t2;
+          __syncwarp();
+        }
+      }
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+    s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+    n_pass += __shfl_xor_sync(0xffffffffu, n_pass, o);
+    n_bad += __shfl_xor_sync(0xffffffffu, n_bad, o);
+  }
+  if (lane == 0) {
+    s_red[warp * 4 + 0] = s1; s_red[warp * 4 + 1] = s2;
+    s_red[warp * 4 + 2] = __longlong_as_double((long long)n_pass);
+    s_red[warp * 4 + 3] = __longlong_as_double((long long)n_bad);
+  }
+  __syncthreads();
+  double* out = partial + (size_t)blockIdx.x * (2 + nh);
+  for (int e = tid; e < nh; e += T) {
+    double s = 0.0;
+    for (int w = 0; w < nw; ++w) s += s_hist[w * nh + e];
+    out[2 + e] = s;
+  }
+  if (tid == 0) {
+    double a = 0.0, b = 0.0; unsigned long long c = 0, d2 = 0;
+    for (int w = 0; w < nw; ++w) {
+      a += s_red[w * 4 + 0]; b += s_red[w * 4 + 1];
+      c += (unsigned long long)__double_as_longlong(s_red[w * 4 + 2]);
+      d2 += (unsigned long long)__double_as_longlong(s_red[w * 4 + 3]);
+    }
+    out[0] = a; out[1] = b;
+    pcount[2 * blockIdx.x] = c; pcount[2 * blockIdx.x + 1] = d2;
+  }
+}
+
 // ---- S1-S8 with per-event outputs -------------------------------------------------------------------
 template <int PROC, bool REC>
 __global__ void __launch_bounds__(MF_THREADS, MfLaunch<PROC>::MINB)
@@ -316,6 +493,52 @@ static cudaError_t proc_iterate(const MfParams& P, const double* edges, const do
   return cudaGetLastError();
 }
 
+// ---- staged path: launches ---------------------------------------------------------------------------
+#ifndef MF_STAGED
+#define MF_STAGED 1                  // heavy processes (with cuts) iterate through the staged path
+#endif
+static constexpr bool kStaged = MF_STAGED && MfProc<MF_PROC>::NGL > 0;
+static constexpr int kRecFields = 4 * MfProc<MF_PROC>::N + 3;
+
+static size_t front_smem(const MfParams& P) {
+  return sizeof(double) * ((size_t)P.d * (P.nb + 1) + (size_t)P.pdf_nx * P.pdf_nq) + sizeof(int) * (MF_THREADS / 32);
+}
+static size_t hist_smem(const MfParams& P) { return sizeof(double) * (MF_THREADS / 32) * ((size_t)P.d * P.nb + 4); }
+
+static cudaError_t proc_staged_setup(const MfParams& P, int* rec_fields, int* occ_front, int* occ_hist) {
+  *rec_fields = kStaged ? kRecFields : 0;
+  *occ_front = *occ_hist = 0;
+  if (!kStaged) return cudaSuccess;
+  cudaError_t e = cudaFuncSetAttribute(mf_front_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)front_smem(P));
+  if (e) return e;
+  e = cudaFuncSetAttribute(mf_me_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+  if (e) return e;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_front, mf_front_kernel<MF_PROC>, MF_THREADS, front_smem(P));
+  if (e) return e;
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_hist, mf_hist_kernel<MF_PROC>, MF_THREADS, hist_smem(P));
+}
+
+// ev (nullable): 4 events recorded at front start / |M|^2 start / |M|^2 end / reductions end
+static cudaError_t proc_staged(const MfParams& P, const double* edges, const double* pdf, uint32_t iteration,
+                               unsigned long long first, unsigned long long n, double n_total, const MfStageWs& ws,
+                               double* partial, unsigned long long* pcount, int grid_me, int grid_hist,
+                               cudaStream_t st, cudaEvent_t* ev) {
+  if (!kStaged) return cudaErrorNotSupported;
+  cudaError_t e;
+  if (ev && (e = cudaEventRecord(ev[0], st))) return e;
+  mf_front_kernel<MF_PROC><<<ws.regions, MF_THREADS, front_smem(P), st>>>(P, edges, pdf, iteration, first, n, ws.cap, ws.rec, ws.count);
+  if ((e = cudaGetLastError())) return e;
+  if (ev && (e = cudaEventRecord(ev[1], st))) return e;
+  const size_t sm = sizeof(unsigned int) * ((size_t)ws.regions + 1 + MF_THREADS);
+  mf_me_kernel<MF_PROC><<<grid_me, MF_THREADS, sm, st>>>(P, ws.rec, ws.count, ws.regions, ws.cap);
+  if ((e = cudaGetLastError())) return e;
+  if (ev && (e = cudaEventRecord(ev[2], st))) return e;
+  mf_hist_kernel<MF_PROC><<<grid_hist, MF_THREADS, hist_smem(P), st>>>(P, ws.rec, ws.count, ws.regions, ws.cap, n_total, partial, pcount);
+  if ((e = cudaGetLastError())) return e;
+  if (ev && (e = cudaEventRecord(ev[3], st))) return e;
+  return cudaSuccess;
+}
+
 #define MF_CAT_(a, b) a##b
 #define MF_CAT(a, b) MF_CAT_(a, b)
-extern const MfProcOps MF_CAT(mf_ops_, MF_PROC) = {proc_setup, proc_eval, proc_iterate};
+extern const MfProcOps MF_CAT(mf_ops_, MF_PROC) = {proc_setup, proc_eval, proc_iterate, proc_staged_setup, proc_staged};

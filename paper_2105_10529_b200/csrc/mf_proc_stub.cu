@@ -7,4 +7,9 @@ static cudaError_t s_iter(const MfParams&, const double*, const double*, uint32_
                           double, double*, unsigned long long*, int, size_t, cudaStream_t) { return cudaErrorNotSupported; }
 #define MF_CAT_(a, b) a##b
 #define MF_CAT(a, b) MF_CAT_(a, b)
-extern const MfProcOps MF_CAT(mf_ops_, MF_PROC) = {s_setup, s_eval, s_iter};
+static cudaError_t s_ssetup(const MfParams&, int*, int*, int*) { return cudaErrorNotSupported; }
+static cudaError_t s_staged(const MfParams&, const double*, const double*, uint32_t, unsigned long long, unsigned long long,
+                            double, const MfStageWs&, double*, unsigned long long*, int, int, cudaStream_t, cudaEvent_t*) {
+  return cudaErrorNotSupported;
+}
+extern const MfProcOps MF_CAT(mf_ops_, MF_PROC) = {s_setup, s_eval, s_iter, s_ssetup, s_staged};

@@ -140,6 +140,39 @@ def test_full_size_launch_sampled_parity(mf, mfo):
         assert (ref == 0 and got == 0) or abs(got / ref - 1) < RTOL_EVENT
 
 
+@pytest.mark.parametrize("proc,n", [(2, 70_001), (3, 5_003)])
+def test_staged_path_equals_fused_path(mf, proc, n):
+    """the staged iteration (front end -> |M|^2 -> reductions through HBM records) and the fused kernel
+    evaluate the same events: equal counters, sums equal to summation order, same refined grid"""
+    cfg = W.config(proc, seed=2)
+    a, b = mf.Vegas(cfg), mf.Vegas(cfg)
+    b.set_path(False)
+    for _ in range(2):
+        ia, ib = a.vegas_iterate(n), b.vegas_iterate(n)
+        assert ia["n_pass"] == ib["n_pass"] and ia["n_nonfinite"] == 0 == ib["n_nonfinite"]
+        np.testing.assert_allclose(a.get_accum()[0], b.get_accum()[0], rtol=1e-12, atol=1e-300)
+        np.testing.assert_allclose(a.get_grid(), b.get_grid(), rtol=0, atol=1e-13)
+    st = a.last_stage_ms()
+    assert st["front"] > 0 and st["me"] > 0 and st["reduce"] > 0
+    with pytest.raises(mf.MfError) as e:
+        mf.Vegas(W.config(W.GG_TT)).set_path(True)
+    assert e.value.code == mf.MF_EUNSUPPORTED
+
+
+def test_staged_path_slices_large_iterations(mf):
+    """more than 2^24 events per iteration: the staged path runs in slices that reuse the workspace;
+    raw sums == sums of the eval kernel's per-event weights"""
+    cfg = W.config(W.GG_TTG, seed=1)
+    n = (1 << 24) + 12_345
+    gpu = mf.Vegas(cfg)
+    g = gpu.vegas_iterate(n)
+    acc, cnt = gpu.get_accum()
+    w = mf.Vegas(cfg).integrand_eval(0, 0, n)["weight"]
+    t = w / n
+    assert abs(float(t.sum()) / acc[0] - 1) < 1e-10 and abs(float((t * t).sum()) / acc[1] - 1) < 1e-10
+    assert int((w != 0).sum()) <= cnt[0] <= n and g["n_events"] == n
+
+
 def test_sharded_accumulate_equals_iterate(mf):
     """mf_vegas_accumulate over two event ranges + finalize == mf_vegas_iterate (to summation order)"""
     cfg = W.config(W.GG_TT, seed=5)

@@ -204,7 +204,7 @@ extern "C" int mf_vegas_accumulate(mf_vegas_t* h, uint64_t first_event, uint64_t
       if (grid_hist > h->max_blocks) grid_hist = h->max_blocks;
       MF_CUDA(h->ops->staged(h->P, h->d_edges, h->d_pdf, h->iteration, first_event + done, m, (double)n_total, h->ws,
                              h->d_partial, h->d_pcount, grid_me, grid_hist, st, h->evs));
-      mf_reduce_kernel<<<(h->na + 127) / 128, 128, 0, st>>>(h->d_partial, h->d_pcount, grid_hist, h->na, h->d_acc, h->d_counts);
+      mf_reduce_kernel<<<(h->na + 2 + 7) / 8, MF_REDUCE_THREADS, 0, st>>>(h->d_partial, h->d_pcount, grid_hist, h->na, h->d_acc, h->d_counts);
       MF_CUDA(cudaGetLastError());
     }
     h->have_stage = true; h->have_k = false;
@@ -217,7 +217,7 @@ extern "C" int mf_vegas_accumulate(mf_vegas_t* h, uint64_t first_event, uint64_t
                           h->d_partial, h->d_pcount, grid, h->smem_iter, st));
   MF_CUDA(cudaEventRecord(h->evk1, st));
   h->have_k = true; h->have_stage = false;
-  mf_reduce_kernel<<<(h->na + 127) / 128, 128, 0, st>>>(h->d_partial, h->d_pcount, grid, h->na, h->d_acc, h->d_counts);
+  mf_reduce_kernel<<<(h->na + 2 + 7) / 8, MF_REDUCE_THREADS, 0, st>>>(h->d_partial, h->d_pcount, grid, h->na, h->d_acc, h->d_counts);
   MF_CUDA(cudaGetLastError());
   h->last_stream = st;
   return MF_OK;
@@ -249,7 +249,7 @@ extern "C" int mf_vegas_finalize(mf_vegas_t* h, uint64_t n_total, void* cuda_str
   if (h->iteration >= MF_MAX_ITER) return fail(MF_ESTATE, "too many iterations (1024)");
   MF_CUDA(cudaSetDevice(h->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  mf_finalize_kernel<<<1, 32, 0, st>>>(h->P, h->cfg.alpha_damp, (double)n_total, n_total, h->d_acc, h->d_counts,
+  mf_finalize_kernel<<<1, 32 * h->P.d, 0, st>>>(h->P, h->cfg.alpha_damp, (double)n_total, n_total, h->d_acc, h->d_counts,
                                         h->d_edges, h->d_state);
   MF_CUDA(cudaGetLastError());
   // the raw sums stay readable (mf_get_accum) until the next iteration starts

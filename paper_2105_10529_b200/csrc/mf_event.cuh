@@ -83,15 +83,15 @@ MF_HD bool mf_event_front(const MfParams& P, const double* edges, const double* 
   double u[D], y[D];
   mf_uniforms<D>(P, iteration, ev, u);                                   // S1
   const double JV = mf_vegas_map<D>(edges, P.nb, u, y, bin);             // S2
-  double x1 = 1.0, x2 = 1.0, shat = P.s, jx = 1.0;
-  if (PROC != 0) mf_x_map(P, y[0], y[1], x1, x2, shat, jx);              // S3
+  double x1 = 1.0, x2 = 1.0, shat = P.s, jx = 1.0, lx1 = 0.0, lx2 = 0.0;
+  if (PROC != 0) mf_x_map(P, y[0], y[1], x1, x2, shat, jx, lx1, lx2);    // S3
   const double wps = mf_phase_space<N>(shat, PROC == 0 ? 0.0 : P.m_top, y + (PROC == 0 ? 0 : 2), k);   // S4
   rts = sqrt(shat);
   const bool pass = mf_cuts<NGL>(P, (const double(*)[4])(&k[0][0] + 8), x1, x2);   // S5 (final gluons = k[2..])
   double f1 = 1.0, f2 = 1.0, xf1 = 0.0, xf2 = 0.0;
   if (PROC != 0 && (REC || pass)) {                                      // S6
-    xf1 = mf_pdf(P, pdf_tab, x1, P.pdf_lq);
-    xf2 = mf_pdf(P, pdf_tab, x2, P.pdf_lq);
+    xf1 = mf_pdf(P, pdf_tab, lx1, P.pdf_lq);
+    xf2 = mf_pdf(P, pdf_tab, lx2, P.pdf_lq);
     f1 = xf1 / x1; f2 = xf2 / x2;
   }
   pref = JV * jx * f1 * f2 * wps * P.wconst / shat;                      // S8 without |M|^2

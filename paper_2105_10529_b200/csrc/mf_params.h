@@ -30,6 +30,7 @@ static inline int mf_fill_params(const mf_config_t* c, MfParams* P, std::string&
   p.key0 = (uint32_t)c->seed; p.key1 = (uint32_t)(c->seed >> 32);
   p.s = c->sqrt_s * c->sqrt_s; p.m_top = c->m_top;
   p.ptmin = c->ptmin_g; p.etamax = c->etamax_g; p.drmin = c->drmin_gg;
+  p.tanh_etamax = c->etamax_g > 0.0 ? tanh(c->etamax_g) : 1.0;
   const double PI = 3.14159265358979323846;
   if (c->process == MF_EE_MUMU) {
     if (!(c->alpha_em > 0.0)) { err = "alpha_em must be positive"; return MF_EINVAL; }

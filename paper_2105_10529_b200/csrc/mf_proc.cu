@@ -13,6 +13,40 @@ __device__ __forceinline__ void mf_stage_tables(const MfParams& P, const double*
   for (int i = threadIdx.x; i < np; i += blockDim.x) s_pdf[i] = g_pdf[i];
 }
 
+// ---- S9: per-warp histogram update in fixed order -------------------------------------------------------
+// H[j][bin_j] += t2 for every contributing lane of the warp, lanes that share a bin served in lane order
+// (so the sum order is fixed: reading A22).  The peer masks come from six ballots per dimension (one per
+// key bit) instead of match.any, whose latency (~800 cycles under load, profiles/r1_v3_staged_ncu.md)
+// dominated the reduction stage; the ranks of all dimensions are resolved first so that each round
+// issues D independent shared-memory updates.
+template <int D>
+__device__ __forceinline__ void mf_hist_add(double* __restrict__ hw, int nb, unsigned long long packed, bool contrib,
+                                            double t2, unsigned lt_mask) {
+  const unsigned full = 0xffffffffu;
+  const unsigned cmask = __ballot_sync(full, contrib);
+  if (cmask == 0u) return;                               // warp-uniform
+  unsigned rank[D], key[D], maxrank = 0;
+#pragma unroll
+  for (int j = 0; j < D; ++j) {
+    key[j] = (unsigned)((packed >> (6 * j)) & 63ull);
+    unsigned peers = cmask;
+#pragma unroll
+    for (int b = 0; b < 6; ++b) {
+      const bool bit = (key[j] >> b) & 1u;
+      const unsigned bal = __ballot_sync(full, bit);
+      peers &= bit ? bal : ~bal;
+    }
+    rank[j] = __popc(peers & lt_mask);
+    maxrank = rank[j] > maxrank ? rank[j] : maxrank;
+  }
+  for (unsigned r = 0; __any_sync(full, contrib && maxrank >= r); ++r) {      // ranks are < 32
+#pragma unroll
+    for (int j = 0; j < D; ++j)
+      if (contrib && rank[j] == r) hw[j * nb + key[j]] += t2;
+    __syncwarp();
+  }
+}
+
 // ---- S1-S9 fused ---------------------------------------------------------------------------------
 // partial: [gridDim.x][2 + d*nb] doubles, pcount: [gridDim.x][2] (n_pass, n_nonfinite)
 template <int PROC>
@@ -55,18 +89,10 @@ mf_iterate_kernel(const MfParams P, const double* __restrict__ g_edges, const do
     const double t = F / n_total, t2 = t * t;            // O9: t_i = F_i / N
     s1 += t; s2 += t2;
     // per-warp histogram H[j][k] += t^2, lanes that share a bin are served in lane order
-    const bool contrib = valid && t2 != 0.0;
+    unsigned long long packed = 0;
 #pragma unroll
-    for (int j = 0; j < D; ++j) {
-      const unsigned key = contrib ? (unsigned)bin[j] : 64u + lane;
-      const unsigned peers = __match_any_sync(0xffffffffu, key);
-      const unsigned rank = __popc(peers & lt_mask);
-      const unsigned maxr = __reduce_max_sync(0xffffffffu, rank);
-      for (unsigned r = 0; r <= maxr; ++r) {
-        if (contrib && rank == r) hw[j * nb + key] += t2;
-        __syncwarp();
-      }
-    }
+    for (int j = 0; j < D; ++j) packed |= (unsigned long long)bin[j] << (6 * j);
+    mf_hist_add<D>(hw, nb, packed, valid && t2 != 0.0, t2, lt_mask);
   }
   // fixed-order reductions: xor-butterfly inside the warp, warps in index order inside the block
 #pragma unroll
@@ -181,17 +207,7 @@ mf_iterate_compact_kernel(const MfParams P, const double* __restrict__ g_edges, 
     const double t = F / n_total, t2 = t * t;
     s1 += t; s2 += t2;
     const bool contrib = have && t2 != 0.0;
-#pragma unroll
-    for (int j = 0; j < D; ++j) {
-      const unsigned key = contrib ? (unsigned)((packed >> (6 * j)) & 63ull) : 64u + lane;
-      const unsigned peers = __match_any_sync(0xffffffffu, key);
-      const unsigned rank = __popc(peers & lt_mask);
-      const unsigned maxr = __reduce_max_sync(0xffffffffu, rank);
-      for (unsigned r = 0; r <= maxr; ++r) {
-        if (contrib && rank == r) hw[j * nb + key] += t2;
-        __syncwarp();
-      }
-    }
+    mf_hist_add<D>(hw, nb, packed, contrib, t2, lt_mask);
     qhead = (qhead + m) % CAP;
     qcount -= m;
   }
@@ -359,17 +375,7 @@ mf_hist_kernel(const MfParams P, const double* __restrict__ rec, const unsigned 
       const double t = F / n_total, t2 = t * t;          // O9
       s1 += t; s2 += t2;
       const bool contrib = have && t2 != 0.0;
-#pragma unroll
-      for (int j = 0; j < D; ++j) {
-        const unsigned key = contrib ? (unsigned)((packed >> (6 * j)) & 63ull) : 64u + lane;
-        const unsigned peers = __match_any_sync(0xffffffffu, key);
-        const unsigned rank = __popc(peers & lt_mask);
-        const unsigned maxr = __reduce_max_sync(0xffffffffu, rank);
-        for (unsigned rr = 0; rr <= maxr; ++rr) {
-          if (contrib && rank == rr) hw[j * nb + key] += t2;
-          __syncwarp();
-        }
-      }
+      mf_hist_add<D>(hw, nb, packed, contrib, t2, lt_mask);
     }
   }
 #pragma unroll

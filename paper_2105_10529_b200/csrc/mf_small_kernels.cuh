@@ -4,29 +4,39 @@
 #include "mf_kernels.cuh"
 
 // ---- fixed-order sum of per-block partials into the raw sums (adds: sharded accumulation) -----------
-__global__ void mf_reduce_kernel(const double* __restrict__ partial, const unsigned long long* __restrict__ pcount,
-                                 int nblocks, int na, double* __restrict__ acc, unsigned long long* __restrict__ counts) {
-  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+// one warp per output element: lane l adds partials l, l+32, ... in order, then a xor-butterfly
+// (fixed order: bit-reproducible for a fixed number of partials).  Launch: ceil((na+2)/8) CTAs of 256.
+#define MF_REDUCE_THREADS 256
+__global__ void __launch_bounds__(MF_REDUCE_THREADS)
+mf_reduce_kernel(const double* __restrict__ partial, const unsigned long long* __restrict__ pcount,
+                 int nblocks, int na, double* __restrict__ acc, unsigned long long* __restrict__ counts) {
+  const int e = blockIdx.x * (MF_REDUCE_THREADS / 32) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
   if (e < na) {
     double s = 0.0;
-    for (int b = 0; b < nblocks; ++b) s += partial[(size_t)b * na + e];
-    acc[e] += s;
-  }
-  if (e < 2) {
+    for (int b = lane; b < nblocks; b += 32) s += partial[(size_t)b * na + e];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane == 0) acc[e] += s;
+  } else if (e < na + 2) {
     unsigned long long c = 0;
-    for (int b = 0; b < nblocks; ++b) c += pcount[2 * b + e];
-    counts[e] += c;
+    for (int b = lane; b < nblocks; b += 32) c += pcount[2 * b + (e - na)];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+    if (lane == 0) counts[e - na] += c;
   }
 }
 
 // ---- S10 (O10): sigma_I^2 = max(0, (N S2 - I^2)/(N-1)); Lepage refinement of every dimension --------
-// one block; thread j < d refines dimension j: smooth (3-point, 2-point at the ends), normalise,
-// floor 1e-30, compress r = ((s-1)/ln s)^alpha, re-bin so that each new bin holds sum(r)/nb.
+// one block of d warps; warp j refines dimension j: smooth (3-point, 2-point at the ends), normalise,
+// floor 1e-30, compress r = ((s-1)/ln s)^alpha (lanes work on bins lane, lane+32: the pow/log are the
+// expensive part), then lane 0 re-bins so that each new bin holds sum(r)/nb.  Sums over bins are
+// taken serially by every lane from shared memory (fixed order).
 __global__ void mf_finalize_kernel(const MfParams P, double alpha, double n_total, unsigned long long n_events,
                                    const double* __restrict__ acc, const unsigned long long* __restrict__ counts,
                                    double* __restrict__ edges, MfDevState* __restrict__ st) {
-  const int j = threadIdx.x, nb = P.nb;
-  if (j == 0) {
+  __shared__ double s_r[MF_DMAX][MF_NBMAX], s_e[MF_DMAX][MF_NBMAX + 1];
+  const int j = threadIdx.x >> 5, lane = threadIdx.x & 31, nb = P.nb;
+  if (threadIdx.x == 0) {
     const double I = acc[0], S2 = acc[1];
     double var = (n_total * S2 - I * I) / (n_total - 1.0);
     var = var > 0.0 ? var : 0.0;
@@ -40,25 +50,31 @@ __global__ void mf_finalize_kernel(const MfParams P, double alpha, double n_tota
   if (j >= P.d) return;
   const double* h = acc + 2 + j * nb;
   double* e = edges + j * (nb + 1);
-  double r[MF_NBMAX], eo[MF_NBMAX + 1];
-  double tot = 0.0;
-  for (int k = 0; k < nb; ++k) {
+  double* r = s_r[j];
+  double* eo = s_e[j];
+  for (int k = lane; k < nb; k += 32) {
     double s;
     if (nb == 1) s = h[0];
     else if (k == 0) s = (h[0] + h[1]) * 0.5;
     else if (k == nb - 1) s = (h[nb - 2] + h[nb - 1]) * 0.5;
     else s = (h[k - 1] + h[k] + h[k + 1]) / 3.0;
-    r[k] = s; tot += s;
+    r[k] = s;
   }
-  if (!(tot > 0.0)) return;                               // nothing sampled here: keep this grid
-  double rtot = 0.0;
-  for (int k = 0; k < nb; ++k) {
+  for (int k = lane; k <= nb; k += 32) eo[k] = e[k];
+  __syncwarp();
+  double tot = 0.0;
+  for (int k = 0; k < nb; ++k) tot += r[k];
+  if (!(tot > 0.0)) return;                               // nothing sampled here: keep this grid (warp-uniform)
+  __syncwarp();
+  for (int k = lane; k < nb; k += 32) {
     double s = r[k] / tot;
     s = s < 1e-30 ? 1e-30 : s;
     r[k] = (s == 1.0) ? 1.0 : pow((s - 1.0) / log(s), alpha);
-    rtot += r[k];
   }
-  for (int k = 0; k <= nb; ++k) eo[k] = e[k];
+  __syncwarp();
+  if (lane != 0) return;
+  double rtot = 0.0;
+  for (int k = 0; k < nb; ++k) rtot += r[k];
   double cum = 0.0;
   int k = 0;
   for (int m = 1; m < nb; ++m) {

@@ -41,7 +41,12 @@ def compare_events(out, ref, proc):
     rel_w = np.abs(g["weight"][nz] / ref["weight"][nz] - 1)
     rel_m = np.abs(g["me2"][nz] / ref["me2"][nz] - 1)
     assert rel_m.max() < RTOL_EVENT, rel_m.max()
-    assert rel_w.max() < RTOL_EVENT, rel_w.max()
+    # the weight carries xf(x1) xf(x2); where the interpolant crosses zero (x -> 1)
+    # its absolute rounding error (1e-15, the bound used on the PDF values above) sets the relative one
+    tol_w = np.full(int(nz.sum()), RTOL_EVENT)
+    if proc:
+        tol_w = tol_w + (1e-15 / np.abs(ref["pdf"][nz])).sum(axis=1)
+    assert (rel_w < tol_w).all(), (rel_w / tol_w).max()
 
 
 # sizes span several 128-thread tiles and a ragged tail; iteration/first_event exercise the counter

@@ -28,10 +28,16 @@ static inline double rsqrt(double x) { return 1.0 / sqrt(x); }
 // line body is larger than the 32 KB L1.5 I-cache).  Requires the |M|^2 code to be executed by every
 // thread of the block (MF_UNIFORM_ME), which costs nothing: a warp runs it whenever one lane passes.
 #ifndef MF_SYNC_EVERY
-#define MF_SYNC_EVERY 4
+#define MF_SYNC_EVERY 16
 #endif
+#define MF_GROUP_THREADS 128
 #if defined(__CUDA_ARCH__)
-#define MF_SYNC_POINT(i) do { if (MF_SYNC_EVERY > 0 && (i) % (MF_SYNC_EVERY > 0 ? MF_SYNC_EVERY : 1) == 0) __syncthreads(); } while (0)
+// barrier points of the generated |M|^2 code: the warps of one 128-thread GROUP (one warp per SM
+// sub-partition) stay on the same instruction-cache lines; the two groups of a 256-thread CTA use
+// their own named barrier so that they can run out of phase (mf_me_kernel staggers them: while one
+// group is in its per-event prologue the other keeps the FP64 pipe busy).
+#define MF_GROUP_SYNC() asm volatile("bar.sync %0, 128;" :: "r"(1 + (int)(threadIdx.x >> 7)) : "memory")
+#define MF_SYNC_POINT(i) do { if (MF_SYNC_EVERY > 0 && (i) % (MF_SYNC_EVERY > 0 ? MF_SYNC_EVERY : 1) == 0) MF_GROUP_SYNC(); } while (0)
 #else
 #define MF_SYNC_POINT(i) do { } while (0)
 #endif

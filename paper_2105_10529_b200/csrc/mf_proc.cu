@@ -256,8 +256,11 @@ mf_iterate_compact_kernel(const MfParams P, const double* __restrict__ g_edges, 
 //                    every warp carries a passing event through S7; writes F = pref |M|^2 in place
 //   mf_hist_kernel   S9: sum t, sum t^2 and the d x nb histogram in fixed order from (F, packed bins)
 // Field order of a record: k[N][4], sqrt(shat), pref (-> F), packed bins (6 bits per dimension).
+#ifndef MF_FRONT_MINB
+#define MF_FRONT_MINB 2              // resident CTAs per SM the front end is compiled for
+#endif
 template <int PROC>
-__global__ void __launch_bounds__(MF_THREADS, 2)
+__global__ void __launch_bounds__(MF_THREADS, MF_FRONT_MINB)
 mf_front_kernel(const MfParams P, const double* __restrict__ g_edges, const double* __restrict__ g_pdf,
                 uint32_t iteration, unsigned long long first, unsigned long long n, unsigned long long cap,
                 double* __restrict__ rec, unsigned int* __restrict__ count) {
@@ -305,11 +308,17 @@ mf_front_kernel(const MfParams P, const double* __restrict__ g_edges, const doub
   if (tid == 0) count[blockIdx.x] = filled;
 }
 
+#ifndef MF_ME_STAGGER
+#define MF_ME_STAGGER 14000          // cycles by which the second group of the |M|^2 CTA starts late (~half a chunk)
+#endif
+#ifndef MF_ME_THREADS
+#define MF_ME_THREADS 256            // CTA size of the |M|^2 stage (one CTA per SM; registers = 65536 / threads)
+#endif
 template <int PROC>
-__global__ void __launch_bounds__(MF_THREADS, MfLaunch<PROC>::MINB)
+__global__ void __launch_bounds__(MF_ME_THREADS, 1)
 mf_me_kernel(const MfParams P, double* __restrict__ rec, const unsigned int* __restrict__ count, int regions,
              unsigned long long cap) {
-  constexpr int N = MfProc<PROC>::N, NF = 4 * N + 3, T = MF_THREADS;
+  constexpr int N = MfProc<PROC>::N, NF = 4 * N + 3, T = MF_ME_THREADS;
   extern __shared__ unsigned int s_pre[];                // [regions + 1] exclusive prefix, then s_part[T]
   unsigned int* s_part = s_pre + regions + 1;
   const unsigned tid = threadIdx.x;
@@ -326,9 +335,16 @@ mf_me_kernel(const MfParams P, double* __restrict__ rec, const unsigned int* __r
     __syncthreads();
   }
   const unsigned M = s_pre[regions];
-  const unsigned nchunks = (M + T - 1) / T;
-  for (unsigned q = blockIdx.x; q < nchunks; q += gridDim.x) {     // block-uniform trips (barriers in S7)
-    const unsigned lin = q * T + tid;
+  // chunks of one GROUP (128 threads, own named barrier inside S7); group 1 starts MF_ME_STAGGER cycles
+  // late so that the groups' per-event prologues (record load, ingredients, reciprocals) do not coincide
+  constexpr unsigned G = MF_GROUP_THREADS, NG = T / G;
+  const unsigned group = tid / G, gtid = tid % G;
+  const unsigned nchunks = (M + G - 1) / G;
+#if MF_ME_STAGGER > 0
+  if (group > 0) { const long long t0 = clock64(); while (clock64() - t0 < (long long)MF_ME_STAGGER * group) { } }
+#endif
+  for (unsigned q = blockIdx.x * NG + group; q < nchunks; q += gridDim.x * NG) {   // group-uniform trips
+    const unsigned lin = q * G + gtid;
     const bool have = lin < M;
     const unsigned l = have ? lin : M - 1;               // lanes past the end recompute the last event
     int lo = 0, hi = regions;
@@ -457,6 +473,7 @@ mf_eval_kernel(const MfParams P, const double* __restrict__ g_edges, const doubl
 #define MF_COMPACT 1                 // CTA-level compaction of passing events for the processes with cuts
 #endif
 static constexpr bool kCompact = MF_COMPACT && MfProc<MF_PROC>::NGL > 0;
+static constexpr bool kEvalOne = MfProc<MF_PROC>::NGL > 0;
 
 static cudaError_t proc_setup(const MfParams& P, size_t* smem_iter, size_t* smem_eval, int* occ_iter, int* occ_eval) {
   const size_t tables = (size_t)P.d * (P.nb + 1) + (size_t)P.pdf_nx * P.pdf_nq;
@@ -465,7 +482,7 @@ static cudaError_t proc_setup(const MfParams& P, size_t* smem_iter, size_t* smem
   *smem_iter = sizeof(double) * (tables + nw * P.d * P.nb + nw * 4);
   if (kCompact) *smem_iter += sizeof(double) * (4 * MfProc<MF_PROC>::N + 3) * 2 * MF_THREADS + sizeof(int) * nw;
   cudaError_t e;
-  if (kCompact) {
+  if constexpr (kCompact) {
     e = cudaFuncSetAttribute(mf_iterate_compact_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem_iter);
     if (e) return e;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_iter, mf_iterate_compact_kernel<MF_PROC>, MF_THREADS, *smem_iter);
@@ -475,16 +492,20 @@ static cudaError_t proc_setup(const MfParams& P, size_t* smem_iter, size_t* smem
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_iter, mf_iterate_kernel<MF_PROC>, MF_THREADS, *smem_iter);
   }
   if (e) return e;
-  e = cudaFuncSetAttribute(mf_eval_kernel<MF_PROC, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem_eval);
-  if (e) return e;
+  if constexpr (!kEvalOne) {
+    e = cudaFuncSetAttribute(mf_eval_kernel<MF_PROC, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem_eval);
+    if (e) return e;
+  }
   e = cudaFuncSetAttribute(mf_eval_kernel<MF_PROC, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem_eval);
   if (e) return e;
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_eval, mf_eval_kernel<MF_PROC, false>, MF_THREADS, *smem_eval);
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_eval, mf_eval_kernel<MF_PROC, true>, MF_THREADS, *smem_eval);
 }
 static cudaError_t proc_eval(const MfParams& P, const double* edges, const double* pdf, uint32_t iteration,
                              unsigned long long first, unsigned long long n, const MfEvalOutDev& o, bool rec,
                              int grid, size_t smem, cudaStream_t st) {
-  if (rec) mf_eval_kernel<MF_PROC, true><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, o);
+  // heavy processes build one eval kernel only (the recording one: each output is written if requested)
+  if constexpr (kEvalOne) mf_eval_kernel<MF_PROC, true><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, o);
+  else if (rec) mf_eval_kernel<MF_PROC, true><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, o);
   else mf_eval_kernel<MF_PROC, false><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, o);
   return cudaGetLastError();
 }
@@ -492,7 +513,7 @@ static cudaError_t proc_eval(const MfParams& P, const double* edges, const doubl
 static cudaError_t proc_iterate(const MfParams& P, const double* edges, const double* pdf, uint32_t iteration,
                                 unsigned long long first, unsigned long long n, double n_total, double* partial,
                                 unsigned long long* pcount, int grid, size_t smem, cudaStream_t st) {
-  if (kCompact)
+  if constexpr (kCompact)
     mf_iterate_compact_kernel<MF_PROC><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount);
   else
     mf_iterate_kernel<MF_PROC><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount);
@@ -514,7 +535,8 @@ static size_t hist_smem(const MfParams& P) { return sizeof(double) * (MF_THREADS
 static cudaError_t proc_staged_setup(const MfParams& P, int* rec_fields, int* occ_front, int* occ_hist) {
   *rec_fields = kStaged ? kRecFields : 0;
   *occ_front = *occ_hist = 0;
-  if (!kStaged) return cudaSuccess;
+  if constexpr (!kStaged) return cudaSuccess;
+  else {
   cudaError_t e = cudaFuncSetAttribute(mf_front_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)front_smem(P));
   if (e) return e;
   e = cudaFuncSetAttribute(mf_me_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
@@ -522,6 +544,7 @@ static cudaError_t proc_staged_setup(const MfParams& P, int* rec_fields, int* oc
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_front, mf_front_kernel<MF_PROC>, MF_THREADS, front_smem(P));
   if (e) return e;
   return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_hist, mf_hist_kernel<MF_PROC>, MF_THREADS, hist_smem(P));
+  }
 }
 
 // ev (nullable): 4 events recorded at front start / |M|^2 start / |M|^2 end / reductions end
@@ -529,20 +552,22 @@ static cudaError_t proc_staged(const MfParams& P, const double* edges, const dou
                                unsigned long long first, unsigned long long n, double n_total, const MfStageWs& ws,
                                double* partial, unsigned long long* pcount, int grid_me, int grid_hist,
                                cudaStream_t st, cudaEvent_t* ev) {
-  if (!kStaged) return cudaErrorNotSupported;
+  if constexpr (!kStaged) return cudaErrorNotSupported;
+  else {
   cudaError_t e;
   if (ev && (e = cudaEventRecord(ev[0], st))) return e;
   mf_front_kernel<MF_PROC><<<ws.regions, MF_THREADS, front_smem(P), st>>>(P, edges, pdf, iteration, first, n, ws.cap, ws.rec, ws.count);
   if ((e = cudaGetLastError())) return e;
   if (ev && (e = cudaEventRecord(ev[1], st))) return e;
-  const size_t sm = sizeof(unsigned int) * ((size_t)ws.regions + 1 + MF_THREADS);
-  mf_me_kernel<MF_PROC><<<grid_me, MF_THREADS, sm, st>>>(P, ws.rec, ws.count, ws.regions, ws.cap);
+  const size_t sm = sizeof(unsigned int) * ((size_t)ws.regions + 1 + MF_ME_THREADS);
+  mf_me_kernel<MF_PROC><<<grid_me, MF_ME_THREADS, sm, st>>>(P, ws.rec, ws.count, ws.regions, ws.cap);
   if ((e = cudaGetLastError())) return e;
   if (ev && (e = cudaEventRecord(ev[2], st))) return e;
   mf_hist_kernel<MF_PROC><<<grid_hist, MF_THREADS, hist_smem(P), st>>>(P, ws.rec, ws.count, ws.regions, ws.cap, n_total, partial, pcount);
   if ((e = cudaGetLastError())) return e;
   if (ev && (e = cudaEventRecord(ev[3], st))) return e;
   return cudaSuccess;
+  }
 }
 
 #define MF_CAT_(a, b) a##b

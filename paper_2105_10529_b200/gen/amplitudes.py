@@ -440,6 +440,7 @@ def emit_function(gen, fname):
             return "p%d" % j if (j in hoisted and not g.dep[j] and j not in body_set) else "v%d" % j
 
         body_set = set(body_ids)
+        body_ids = g.schedule(body_ids, SCHED_WINDOW, SCHED_DISTANCE)
         body_lines = g.emit_list(body_ids, bname, "v", indent="    ")
         for i, line in enumerate(body_lines):      # barrier points: keep the block's warps on the same I-cache lines
             if i % 64 == 0:
@@ -486,6 +487,11 @@ PROCESSES = {
 # (Dag.demote_cheap); tuned on B200, see DESIGN.md "Kernels / S7"
 DEMOTE = {"mf_me2_gg_ttg": int(os.environ.get("MF_GEN_DEMOTE_TTG", "6")),
           "mf_me2_gg_ttgg": int(os.environ.get("MF_GEN_DEMOTE_TTGG", "0"))}
+
+
+# emission order of the helicity-loop body (Dag.schedule): window 0 = creation order
+SCHED_WINDOW = int(os.environ.get("MF_GEN_SCHED_WINDOW", "48"))
+SCHED_DISTANCE = int(os.environ.get("MF_GEN_SCHED_DISTANCE", "5"))
 
 
 def generate(fname):

@@ -217,6 +217,64 @@ class Dag:
             stack.extend(self._operands(i))
         return sorted(pro), sorted(body), hoisted
 
+    # ---- emission order ------------------------------------------------------------------------
+    def _factors(self, i):
+        """node ids of the multiplicands of a mul/fma node (the operands that can sit in a reuse slot)"""
+        op, a, b, c = self.nodes[i]
+        if op == "mul":
+            return (a, b)
+        if op == "mulk":
+            return (a,)
+        if op in ("fma", "fms"):
+            return (a[2],) if a[0] == "k" else (a[1], a[2])
+        return ()
+
+    def schedule(self, ids, window=48, distance=3):
+        """Reorder `ids` (a topologically ordered list) for the FP64 pipe of sm_100: a DFMA whose three
+        64-bit register operands are all fresh takes 3 register-read cycles instead of the pipe's 2
+        (profiles/r1_dfma_operands.md: 25 instead of 34 TFLOP/s), one that shares a multiplicand with
+        the previous instruction reads it from the operand-reuse cache.  Greedy list scheduling inside
+        a sliding window of `window` statements (bounds the extra register pressure): prefer a ready
+        statement that (1) does not depend on the last `distance` emitted statements (DFMA latency is
+        ~4 issue slots), (2) shares a multiplicand with the previous statement, (3) comes first in
+        the original order."""
+        if window <= 1:
+            return list(ids)
+        idset = set(ids)
+        pos = {n: k for k, n in enumerate(ids)}
+        deps = {n: [o for o in set(self._operands(n)) if o in idset] for n in ids}
+        fac = {n: set(self._factors(n)) for n in ids}
+        users = {n: [] for n in ids}
+        for n in ids:
+            for o in deps[n]:
+                users[o].append(n)
+        waiting = {n: len(deps[n]) for n in ids}
+        ready = {n for n in ids if waiting[n] == 0}
+        out, done, ptr = [], set(), 0
+        while len(out) < len(ids):
+            while ids[ptr] in done:
+                ptr += 1
+            lim = ptr + window
+            recent = set(out[-distance:]) if distance > 0 else set()
+            prev = fac[out[-1]] if out else set()
+            best, bs = None, None
+            for n in ready:
+                if pos[n] >= lim:
+                    continue
+                sc = (not any(d in recent for d in deps[n]), bool(fac[n] & prev), -pos[n])
+                if bs is None or sc > bs:
+                    best, bs = n, sc
+            if best is None:                       # nothing ready inside the window: take the first ready one
+                best = min(ready, key=lambda n: pos[n])
+            ready.discard(best)
+            done.add(best)
+            out.append(best)
+            for u in users[best]:
+                waiting[u] -= 1
+                if waiting[u] == 0:
+                    ready.add(u)
+        return out
+
     # ---- analysis ------------------------------------------------------------------------------
     def _operands(self, i):
         op, a, b, c = self.nodes[i]

@@ -28,6 +28,7 @@ import numpy as np
 METRIC = "integrand events/sec (fp64) gg->ttbar g, 1e7 events/iteration/GPU"
 N_EVENTS = 10_000_000
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # SMs x DFMA lanes x 2 x max clock
+ME_KERNEL_DRAM_BYTES = 1.0452e9                          # ncu --set full capture of mf_me_kernel<2> (profiles/r1_v9_staged_ncu.md)
 
 
 class ClockSampler:
@@ -39,7 +40,7 @@ class ClockSampler:
         self.rows, self.p = [], None
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", uuid, "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
-                                       "-lms", "50"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                                       "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
         except OSError:
@@ -210,7 +211,9 @@ def run_ours(args, rank, local_rank, world):
                 "d2h_bytes_per_step": grid_bytes + 40},
         "gpu_launches": (5 if staged else 3) * args.steps,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                     "traffic": None, "kernel": "mf_me_kernel<2>" if staged else "mf_iterate_compact_kernel<2>", "kernel_ms": k_ms,
+                     "traffic": ME_KERNEL_DRAM_BYTES if staged else None,
+                     "traffic_source": "profiles/r1_v9_staged_ncu.md (dram__bytes_read.sum + dram__bytes_write.sum of one mf_me_kernel<2> launch; algorithmic: 120 B per passing event = %.3e B)" % (120.0 * n_pass) if staged else None,
+                     "kernel": "mf_me_kernel<2>" if staged else "mf_iterate_compact_kernel<2>", "kernel_ms": k_ms,
                      "flops_per_event": flops["flops"], "fma_fraction_of_ops": flops["fma"] / (flops["add"] + flops["mul"] + flops["fma"]),
                      "peak_source": "measured DFMA-chain microbenchmark (mf_fp64_peak), max of before/after the timed region",
                      "peak_before": peak_before / 1e12, "peak_after": peak_after / 1e12,
@@ -232,14 +235,56 @@ def run_ours(args, rank, local_rank, world):
     print(json.dumps(out))
 
 
+def run_sweep(args):
+    """BASELINE.json configs[4]: throughput sweep of the gg -> tt~g integrand of config 2 over events per
+    launch (1e4 .. 1e8, 1e8 in slices of 2^24 events), uniform grid, single iteration, seed 1, fp64 (the
+    optional fp32 variant is not built).  One JSON line with one entry per size."""
+    import torch
+    from paper_2105_10529_b200 import binding, workloads as W
+    binding.lib()
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    peak = binding.fp64_peak(0, 0.3) / 1e12
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    rows = []
+    for n in (10_000, 100_000, 1_000_000, 10_000_000, 100_000_000):
+        reps = 5 if n <= 10_000_000 else 2
+        h = binding.Vegas(W.config(W.GG_TTG, seed=1))
+        h.set_path(args.path == "staged")
+        uniform = h.get_grid()
+        h.vegas_accumulate(0, min(n, 1 << 24), n)                          # warm-up: allocates the staged workspace
+        flops = h.me_flops()["flops"]
+        best = None
+        for _ in range(reps):
+            h.set_grid(uniform)                                            # every repetition on the uniform grid
+            flush.zero_()
+            torch.cuda.synchronize()
+            r = h.vegas_iterate(n, sync=True)
+            k_ms, it_ms = h.last_kernel_ms()
+            st = h.last_stage_ms() if args.path == "staged" and n <= (1 << 24) else None
+            if best is None or it_ms < best["iteration_ms"]:
+                best = {"events": n, "iteration_ms": it_ms, "events_per_s": n / (it_ms * 1e-3), "n_pass": r["n_pass"],
+                        "integral_pb": r["integral"], "sigma_pb": r["sigma"], "stages_ms": st,
+                        "whole_path_tflops": flops * r["n_pass"] / (it_ms * 1e-3) / 1e12}
+                if st:
+                    best["me_tflops"] = flops * r["n_pass"] / (st["me"] * 1e-3) / 1e12
+                    best["me_frac_of_peak"] = best["me_tflops"] / peak
+                    best["reduce_stage_gbps"] = 16.0 * r["n_pass"] / (st["reduce"] * 1e-3) / 1e9
+                    best["front_stage_gbps"] = 120.0 * r["n_pass"] / (st["front"] * 1e-3) / 1e9
+        rows.append(best)
+    print(json.dumps({"metric": "throughput sweep, gg->ttbar g integrand (configs[4])", "unit": "events/s", "dtype": "f64",
+                      "path": args.path, "fp64_peak_tflops": peak, "fp32_variant": "not built (DESIGN.md A24)", "sweep": rows}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--events", type=int, default=N_EVENTS, help="events per iteration per GPU")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="configs[4]: events-per-launch sweep of the gg->tt~g integrand (1 GPU)")
     ap.add_argument("--path", default="staged", choices=["staged", "fused"],
                     help="staged: front end / |M|^2 / reductions as three kernels (default); fused: one kernel")
     args = ap.parse_args()
@@ -248,6 +293,10 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.impl == "reference":
         run_reference(args, rank)
+        return
+    if args.sweep:
+        if rank == 0:
+            run_sweep(args)
         return
     run_ours(args, rank, local_rank, world)
     if world > 1:

@@ -38,8 +38,15 @@ static inline double rsqrt(double x) { return 1.0 / sqrt(x); }
 // group is in its per-event prologue the other keeps the FP64 pipe busy).
 #define MF_GROUP_SYNC() asm volatile("bar.sync %0, 128;" :: "r"(1 + (int)(threadIdx.x >> 7)) : "memory")
 #define MF_SYNC_POINT(i) do { if (MF_SYNC_EVERY > 0 && (i) % (MF_SYNC_EVERY > 0 ? MF_SYNC_EVERY : 1) == 0) MF_GROUP_SYNC(); } while (0)
+// gg -> tt~gg: the loop body is ~0.5 MB of SASS, instruction fetch is the bottleneck: all eight warps of the
+// CTA stay together (whole-CTA barrier, every MF_SYNC_EVERY_WIDE-th point) and stream it once
+#ifndef MF_SYNC_EVERY_WIDE
+#define MF_SYNC_EVERY_WIDE 4
+#endif
+#define MF_SYNC_POINT_W(i) do { if ((i) % MF_SYNC_EVERY_WIDE == 0) __syncthreads(); } while (0)
 #else
 #define MF_SYNC_POINT(i) do { } while (0)
+#define MF_SYNC_POINT_W(i) do { } while (0)
 #endif
 // opaque identity on a double: stops the compiler from hoisting what is computed from it out of the
 // helicity loop (the generator decides what is hoisted: gen/dag.py Dag.plan)

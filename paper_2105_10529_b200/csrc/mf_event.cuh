@@ -13,10 +13,11 @@
 #include "generated/mf_me2_gg_ttgg.cuh"
 
 template <int PROC> struct MfProc;
-template <> struct MfProc<0> { static const int D = 2, N = 2, NGL = 0; };
-template <> struct MfProc<1> { static const int D = 4, N = 2, NGL = 0; };
-template <> struct MfProc<2> { static const int D = 7, N = 3, NGL = 1; };
-template <> struct MfProc<3> { static const int D = 10, N = 4, NGL = 2; };
+// GROUP: threads that share the barrier points of the generated |M|^2 code (mf_device.cuh)
+template <> struct MfProc<0> { static const int D = 2, N = 2, NGL = 0, GROUP = 128; };
+template <> struct MfProc<1> { static const int D = 4, N = 2, NGL = 0, GROUP = 128; };
+template <> struct MfProc<2> { static const int D = 7, N = 3, NGL = 1, GROUP = 128; };
+template <> struct MfProc<3> { static const int D = 10, N = 4, NGL = 2, GROUP = 256; };
 
 // optional per-event record (mf_integrand_eval's debug outputs)
 struct MfEventRec {

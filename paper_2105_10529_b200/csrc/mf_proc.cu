@@ -257,7 +257,7 @@ mf_iterate_compact_kernel(const MfParams P, const double* __restrict__ g_edges, 
 //   mf_hist_kernel   S9: sum t, sum t^2 and the d x nb histogram in fixed order from (F, packed bins)
 // Field order of a record: k[N][4], sqrt(shat), pref (-> F), packed bins (6 bits per dimension).
 #ifndef MF_FRONT_MINB
-#define MF_FRONT_MINB 2              // resident CTAs per SM the front end is compiled for
+#define MF_FRONT_MINB 3              // resident CTAs per SM the front end is compiled for (80 registers; tuned, profiles/r1_tuning.md)
 #endif
 template <int PROC>
 __global__ void __launch_bounds__(MF_THREADS, MF_FRONT_MINB)
@@ -337,7 +337,7 @@ mf_me_kernel(const MfParams P, double* __restrict__ rec, const unsigned int* __r
   const unsigned M = s_pre[regions];
   // chunks of one GROUP (128 threads, own named barrier inside S7); group 1 starts MF_ME_STAGGER cycles
   // late so that the groups' per-event prologues (record load, ingredients, reciprocals) do not coincide
-  constexpr unsigned G = MF_GROUP_THREADS, NG = T / G;
+  constexpr unsigned G = MfProc<PROC>::GROUP, NG = T / G;
   const unsigned group = tid / G, gtid = tid % G;
   const unsigned nchunks = (M + G - 1) / G;
 #if MF_ME_STAGGER > 0

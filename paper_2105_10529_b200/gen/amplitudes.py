@@ -384,6 +384,7 @@ class GenEE:
 def emit_function(gen, fname):
     """CUDA/C++ text of `double fname(const double* in)` plus the flop-count macros."""
     g, out = gen.g, gen.out
+    sync = SYNC_MACRO.get(fname, "MF_SYNC_POINT")
     nh = len(gen.loop_assign)
     looped = bool(gen.loop_legs)
     pro_ids, body_ids, hoisted = g.plan([out], getattr(gen, "max_hoist_cost", None) if looped else None)
@@ -416,7 +417,7 @@ def emit_function(gen, fname):
         ids = sorted(set(pro_ids) | set(body_ids))
         for i, line in enumerate(g.emit_list(ids, pname, "p")):
             if i % 64 == 0 and len(ids) > 1024:
-                L.append("  MF_SYNC_POINT(%d);" % (i // 64))
+                L.append("  %s(%d);" % (sync, i // 64))
             L.append(line)
         L.append("  return %s;" % _ref(g, out, pname))
     else:
@@ -444,7 +445,7 @@ def emit_function(gen, fname):
         body_lines = g.emit_list(body_ids, bname, "v", indent="    ")
         for i, line in enumerate(body_lines):      # barrier points: keep the block's warps on the same I-cache lines
             if i % 64 == 0:
-                L.append("    MF_SYNC_POINT(%d);" % (i // 64))
+                L.append("    %s(%d);" % (sync, i // 64))
             L.append(line)
         L.append("    acc += %s;" % _ref(g, out, bname))
         L.append("  }")
@@ -488,6 +489,9 @@ PROCESSES = {
 DEMOTE = {"mf_me2_gg_ttg": int(os.environ.get("MF_GEN_DEMOTE_TTG", "6")),
           "mf_me2_gg_ttgg": int(os.environ.get("MF_GEN_DEMOTE_TTGG", "0"))}
 
+
+# barrier-point macro of the generated code (csrc/mf_device.cuh): 128-thread groups, or the whole CTA
+SYNC_MACRO = {"mf_me2_gg_ttgg": "MF_SYNC_POINT_W"}
 
 # emission order of the helicity-loop body (Dag.schedule): window 0 = creation order
 SCHED_WINDOW = int(os.environ.get("MF_GEN_SCHED_WINDOW", "48"))

@@ -10,7 +10,10 @@
 #define MF_GEN_TTG "generated/mf_me2_gg_ttg.cuh"
 #endif
 #include MF_GEN_TTG
-#include "generated/mf_me2_gg_ttgg.cuh"
+#ifndef MF_GEN_TTGG
+#define MF_GEN_TTGG "generated/mf_me2_gg_ttgg.cuh"
+#endif
+#include MF_GEN_TTGG
 
 template <int PROC> struct MfProc;
 // GROUP: threads that share the barrier points of the generated |M|^2 code (mf_device.cuh)

@@ -102,9 +102,15 @@ def slash_terms(s, psi):
 class Gen:
     """gg -> t tbar + (ng-2) g.  Gluon legs 0,1 incoming along +z/-z, legs 2.. outgoing."""
 
-    def __init__(self, ng, loop_legs=(), parity=True, loop_lam4=False):
+    def __init__(self, ng, loop_legs=(), parity=True, loop_lam4=False, basis="circular"):
         """loop_legs: gluon legs whose helicity is a run-time loop symbol; loop_lam4: the antitop
-        helicity is a loop symbol too (leg id 4 in the loop list; v(lam4) is blended arithmetically)"""
+        helicity is a loop symbol too (leg id 4 in the loop list; v(lam4) is blended arithmetically).
+        basis: "circular" = helicity states eps(k, +-1) of O6.2; "linear" = the two REAL polarisation
+        vectors eps1, eps2 of O6.2 (label +1 -> eps1, -1 -> eps2).  The spin sum over a gluon is the
+        same in any orthonormal basis of its two physical polarisations (sum_lam eps_lam^mu
+        eps_lam^nu* = eps1^mu eps1^nu + eps2^mu eps2^nu), and with real vectors every gluon current
+        is real: the DAG drops the imaginary parts as structural zeros."""
+        self.basis = basis
         self.loop_lam4 = loop_lam4
         self.ng, self.g = ng, Dag()
         g = self.g
@@ -139,6 +145,8 @@ class Gen:
         """e_g: eps(k,lam) for incoming legs, eps^*(k,lam) for outgoing; lam is +-1 or a symbol R"""
         g = self.g
         z = Cx(g.const(0.0), g.const(0.0))
+        if self.basis == "linear":
+            return self.pol_linear(leg, lam)
         lamR = lam if isinstance(lam, R) else g.const(float(lam))
         if leg == 0:      # k along +z: eps = (0, -lam/sqrt2, -i/sqrt2, 0)
             return [z, Cx(-lamR * SQ2I, g.const(0.0)), Cx(g.const(0.0), g.const(-SQ2I)), z]
@@ -146,6 +154,25 @@ class Gen:
             return [z, Cx(-lamR * SQ2I, g.const(0.0)), Cx(g.const(0.0), g.const(SQ2I)), z]
         e1x, e1y, e1z, e2x, e2y = self.g_ing[leg]      # already divided by sqrt 2
         return [z, Cx(-lamR * e1x, e2x), Cx(-lamR * e1y, e2y), Cx(-lamR * e1z, g.const(0.0))]
+
+    def pol_linear(self, leg, lam):
+        """real polarisation vectors: label +1 -> eps1, -1 -> eps2 (O6.2: eps1 = (0, kx kz, ky kz, -kT^2)/(|k| kT),
+        eps2 = (0, -ky, kx, 0)/kT; kT = 0: eps1 = x, eps2 = sgn(kz) y).  Incoming legs: unit vectors;
+        outgoing legs: the ingredients are eps_i/sqrt2 (the factor 2 per outgoing gluon goes into
+        `scale`).  A loop symbol lam = +-1 selects by blending: s1 = (1+lam)/2, s2 = (1-lam)/2."""
+        g = self.g
+        zero = g.const(0.0)
+        z = Cx(zero, zero)
+        re = lambda x: Cx(x, zero)
+        if isinstance(lam, R):
+            s1, s2 = 0.5 * lam + 0.5, 0.5 - 0.5 * lam
+        else:
+            s1, s2 = g.const(1.0 if lam > 0 else 0.0), g.const(0.0 if lam > 0 else 1.0)
+        if leg in (0, 1):
+            sg = 1.0 if leg == 0 else -1.0
+            return [z, re(s1), re(s2 * sg), z]
+        e1x, e1y, e1z, e2x, e2y = self.g_ing[leg]
+        return [z, re(g.sop([(s1, e1x), (s2, e2x)])), re(g.sop([(s1, e1y), (s2, e2y)])), re(s1 * e1z)]
 
     @staticmethod
     def _chi_pm(ing):
@@ -302,14 +329,20 @@ class Gen:
         |M|^2_avg = g_s^{2 ng}/256 * scale * sum_{loop assignments} body"""
         ng = self.ng
         num, den, perms = colour_matrix(ng)
-        free = [l for l in range(ng) if l not in self.loop_legs and not (self.parity and l == 0)]
+        # parity: circular basis |M(-lam)|^2 = |M(lam)|^2 (colour-summed) fixes the helicity of gluon 0;
+        # linear basis: real polarisation vectors are their own conjugates, so flipping the two quark
+        # helicities conjugates every partial amplitude: the antitop helicity is fixed instead
+        linear = self.basis == "linear"
+        fix0 = self.parity and not linear
+        free = [l for l in range(ng) if l not in self.loop_legs and not (fix0 and l == 0)]
+        lam4s = (self.lam4_sym,) if self.loop_lam4 else ((1,) if (self.parity and linear) else (1, -1))
         total = self.g.const(0.0)
         for combo in itertools.product((1, -1), repeat=len(free)):
             hel = dict(self.lam_sym)
-            if self.parity:
+            if fix0:
                 hel[0] = 1
             hel.update(dict(zip(free, combo)))
-            for lam4 in ((self.lam4_sym,) if self.loop_lam4 else (1, -1)):
+            for lam4 in lam4s:
                 amps = {1: [], -1: []}
                 for sg in perms:
                     a = self.partial_amps(sg, hel, lam4)
@@ -318,7 +351,7 @@ class Gen:
                 for lam3 in (1, -1):
                     total = total + self.colour_form(amps[lam3], num)
         self.out = total
-        self.scale = (2.0 if self.parity else 1.0) / den
+        self.scale = (2.0 if self.parity else 1.0) / den * (2.0 ** (ng - 2) if linear else 1.0)
         if self.loop_lam4:
             self.loop_legs = self.loop_legs + (9,)          # symbol lam9 = antitop helicity
         self.loop_assign = list(itertools.product((-1.0, 1.0), repeat=len(self.loop_legs)))
@@ -475,12 +508,13 @@ def _legs(env, default):
     return default if v is None else tuple(int(x) for x in v.split(",") if x != "")
 
 
+BASIS = os.environ.get("MF_GEN_BASIS", "linear")
 PROCESSES = {
     "mf_me2_ee_mumu": lambda: GenEE(),
-    "mf_me2_gg_tt": lambda: Gen(2, loop_legs=(), parity=True),
-    "mf_me2_gg_ttg": lambda: Gen(3, loop_legs=_legs("MF_GEN_TTG_LOOP", (1, 2)), parity=True,
-                                 loop_lam4=os.environ.get("MF_GEN_TTG_LAM4", "0") == "1"),
-    "mf_me2_gg_ttgg": lambda: Gen(4, loop_legs=(1, 2, 3), parity=True),
+    "mf_me2_gg_tt": lambda: Gen(2, loop_legs=(), parity=True, basis="circular"),      # 514 flops (linear: 715)
+    "mf_me2_gg_ttg": lambda: Gen(3, loop_legs=_legs("MF_GEN_TTG_LOOP", (0, 2)), parity=True,
+                                 loop_lam4=os.environ.get("MF_GEN_TTG_LAM4", "0") == "1", basis=BASIS),
+    "mf_me2_gg_ttgg": lambda: Gen(4, loop_legs=_legs("MF_GEN_TTGG_LOOP", (1, 2, 3)), parity=True, basis=BASIS),
 }
 
 

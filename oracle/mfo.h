@@ -10,6 +10,12 @@
  * anything under oracle/.  It shares no code, header, table or constant generator with the CUDA
  * path (paper_2105_10529_b200/csrc); the struct definitions below are the oracle's own.
  *
+ * Pins (what the functions below are checked against, other than themselves): tests/test_oracle_core.py,
+ * tests/test_oracle_me.py, tests/test_oracle_crosscheck.py and the fixtures in tests/golden/ -- listed in
+ * DESIGN.md section 4.  Parity unpinned: none of the functions; of the RESULTS, the absolute cross
+ * sections of configs 2 and 3 (no closed form, no value in the paper) are pinned factor by factor and,
+ * as a whole, only within the Monte Carlo error of the independent-generator cross-check (2.7 % / 12 %).
+ *
  * All pointers are HOST pointers.  All functions return 0 on success, <0 on error.
  */
 #ifndef MFO_H

@@ -1,0 +1,100 @@
+"""Pin P30: the absolute cross sections of configs 2 and 3 (gg -> tt~g, gg -> tt~gg with
+cuts) have no closed form and no value in the paper.  Cross-check of the oracle's whole weight chain: the same integrand
+integrated through an INDEPENDENT phase-space generator -- textbook RAMBO with 4n uniforms (Kleiss,
+Stirling, Ellis 1986) followed by the massive rescaling, restated here in NumPy -- must give the same
+cross section as the oracle's VEGAS run (3n-4-random sequential generator) within the Monte Carlo error.
+Only the squared matrix element, the PDF interpolant and the cut decision are taken from the oracle
+(each pinned on its own in test_oracle_me.py / test_oracle_core.py)."""
+import math
+from concurrent.futures import ThreadPoolExecutor
+
+import numpy as np
+import pytest
+
+from paper_2105_10529_b200 import workloads as W
+
+
+def classic_rambo(rng, n, rts, count):
+    """massless momenta [count][n][4] in the CM frame, flat in phase space; weight is the constant W0"""
+    c = 2.0 * rng.random((count, n)) - 1.0
+    phi = 2.0 * math.pi * rng.random((count, n))
+    f = -np.log(rng.random((count, n)) * rng.random((count, n)))
+    s = np.sqrt(1.0 - c * c)
+    q = np.stack([f, f * s * np.cos(phi), f * s * np.sin(phi), f * c], axis=-1)
+    Q = q.sum(axis=1)
+    M = np.sqrt(Q[:, 0] ** 2 - (Q[:, 1:] ** 2).sum(axis=1))
+    b = -Q[:, 1:] / M[:, None]
+    x = rts / M
+    gam = Q[:, 0] / M
+    a = 1.0 / (1.0 + gam)
+    bq = (b[:, None, :] * q[:, :, 1:]).sum(axis=-1)
+    p = np.empty_like(q)
+    p[:, :, 0] = x[:, None] * (gam[:, None] * q[:, :, 0] + bq)
+    p[:, :, 1:] = x[:, None, None] * (q[:, :, 1:] + b[:, None, :] * q[:, :, :1] + (a[:, None] * bq)[:, :, None] * b[:, None, :])
+    return p
+
+
+def massive(p, masses, rts):
+    """RAMBO's rescaling: xi with sum sqrt(m^2 + xi^2 E^2) = rts (Newton), weight W_m of reading O4.4"""
+    n = p.shape[1]
+    e0 = p[:, :, 0]
+    m = np.asarray(masses)[None, :]
+    xi = np.sqrt(1.0 - (m.sum() / rts) ** 2)
+    for _ in range(12):
+        E = np.sqrt(m ** 2 + (xi[:, None] * e0) ** 2)
+        xi = xi - (E.sum(axis=1) - rts) / (xi[:, None] * e0 ** 2 / E).sum(axis=1)
+    E = np.sqrt(m ** 2 + (xi[:, None] * e0) ** 2)
+    k = p * xi[:, None, None]
+    k[:, :, 0] = E
+    kabs = xi[:, None] * e0
+    wm = xi ** (2 * n - 3) * np.prod(kabs / E, axis=1) * rts / (kabs ** 2 / E).sum(axis=1)
+    return k, wm
+
+
+@pytest.mark.parametrize("proc,n,count,n_vegas", [(W.GG_TTG, 3, 48_000, 60_000), (W.GG_TTGG, 4, 9_000, 10_000)])
+def test_cross_section_through_classic_rambo(mfo, proc, n, count, n_vegas):
+    cfg = W.config(proc, seed=0)
+    rng = np.random.default_rng(20260511)
+    s = cfg["sqrt_s"] ** 2
+    mt = cfg["m_top"]
+    shat_min = (2 * mt + (n - 2) * cfg["ptmin_g"]) ** 2
+    ltau0 = math.log(shat_min / s)
+    y0, y1 = rng.random(count), rng.random(count)
+    ltau = (1.0 - y0) * ltau0
+    tau = np.exp(ltau)
+    x1 = np.exp(y1 * ltau)
+    x2 = tau / x1
+    jx = tau * ltau0 * ltau
+    shat = tau * s
+    rts = np.sqrt(shat)
+    p = classic_rambo(rng, n, rts, count)
+    k, wm = massive(p, [mt, mt] + [0.0] * (n - 2), rts)
+    assert np.abs(k.sum(axis=1)[:, 0] - rts).max() < 1e-8 * rts.max() and np.abs(k.sum(axis=1)[:, 1:]).max() < 1e-8 * rts.max()
+    w0 = (math.pi / 2) ** (n - 1) * shat ** (n - 2) / (math.factorial(n - 1) * math.factorial(n - 2)) * (2 * math.pi) ** (4 - 3 * n)
+    xf = cfg["pdf_xf"]
+    q2 = cfg["mu_f"] ** 2
+
+    sym = 0.5 if n == 4 else 1.0                      # two identical final gluons (reading A12)
+
+    def one(i):
+        ok, _ = mfo.cuts(k[i, 2:], x1[i], x2[i], cfg["ptmin_g"], cfg["etamax_g"], cfg["drmin_gg"])
+        if not ok:
+            return 0.0
+        mom = np.zeros((2 + n, 4))
+        mom[0] = [rts[i] / 2, 0, 0, rts[i] / 2]
+        mom[1] = [rts[i] / 2, 0, 0, -rts[i] / 2]
+        mom[2:] = k[i]
+        f1 = mfo.pdf_interp(xf, W.PDF_XMIN, W.PDF_XMAX, W.PDF_QMIN, W.PDF_QMAX, x1[i], q2) / x1[i]
+        f2 = mfo.pdf_interp(xf, W.PDF_XMIN, W.PDF_XMAX, W.PDF_QMIN, W.PDF_QMAX, x2[i], q2) / x2[i]
+        return jx[i] * f1 * f2 * mfo.me2(proc, mom, mt, cfg["alpha_s"]) * sym * w0[i] * wm[i] * cfg["gev2_to_pb"] / (2 * shat[i])
+
+    with ThreadPoolExecutor(mfo.max_threads()) as ex:
+        F = np.array(list(ex.map(one, range(count))))
+    I1, e1 = F.mean(), F.std(ddof=1) / math.sqrt(count)
+    orc = mfo.Vegas(cfg)
+    for _ in range(3):
+        orc.iterate(n_vegas, n_threads=mfo.max_threads())
+    r = orc.result()
+    print("classic RAMBO: %.2f +- %.2f pb; oracle VEGAS: %.2f +- %.2f pb" % (I1, e1, r["integral"], r["sigma"]))
+    assert e1 < (0.05 if n == 3 else 0.15) * I1, (I1, e1)        # the pin is as sharp as this error: 2.7 % / 12 %
+    assert abs(I1 - r["integral"]) < 4.0 * math.hypot(e1, r["sigma"]), (I1, e1, r)

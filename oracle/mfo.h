@@ -74,6 +74,22 @@ int mfo_vegas_accumulate(mfo_vegas_t *h, uint32_t iteration, uint64_t first_even
 /* finish an iteration from raw sums (O10): record (I, sigma), refine the grid */
 int mfo_vegas_finalize(mfo_vegas_t *h, const double *acc, uint64_t n_total, uint64_t n_pass,
                        uint64_t n_nonfinite, mfo_iter_t *out);
+/* Observable histograms filled in the same pass as the integral ("histogram accumulation";
+ * the differential cross section in the top-quark pT is the paper's physics plot; SURVEY
+ * section 8(f) item 1).  Plain definition: for every event i of [first, first+n) with weight F_i != 0,
+ * t_i = F_i / n_total, the observable v_i is computed from the final-state momenta (partonic CM frame;
+ * all kinds are invariant under the boost along the beam) and
+ *   b = n_bins      if v < lo        (underflow slot)
+ *   b = n_bins + 1  if v >= hi       (overflow slot)
+ *   b = floor((v - lo) / (hi - lo) * n_bins)  otherwise (clamped to n_bins - 1),
+ *   sum[o][b] += t_i,  sum2[o][b] += t_i^2          (long double sums; arrays [n_obs][n_bins + 2], ADDED to).
+ * kinds: 0 = pT of final particle 1 (top / mu-), 1 = pT of final particle 2 (antitop / mu+),
+ *        2 = invariant mass of particles 1+2, 3 = pT of final particle 3 (first gluon; processes 2, 3). */
+enum { MFO_OBS_PT_1 = 0, MFO_OBS_PT_2 = 1, MFO_OBS_M_12 = 2, MFO_OBS_PT_3 = 3 };
+typedef struct { int32_t kind; uint32_t n_bins; double lo, hi; } mfo_observable_t;
+int mfo_observable_hist(mfo_vegas_t *h, uint32_t iteration, uint64_t first_event, uint64_t n_events,
+                        uint64_t n_total, int n_threads, const mfo_observable_t *obs, uint32_t n_obs,
+                        double *sum, double *sum2);
 int mfo_max_threads(void);
 
 /* ---- single steps, exported so that the tests can pin each one ------------------------------- */

@@ -42,6 +42,10 @@ class Iter(C.Structure):
                 ("n_pass", C.c_uint64), ("n_nonfinite", C.c_uint64)]
 
 
+class Observable(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("n_bins", C.c_uint32), ("lo", C.c_double), ("hi", C.c_double)]
+
+
 class Result(C.Structure):
     _fields_ = [("integral", C.c_double), ("sigma", C.c_double), ("chi2_dof", C.c_double), ("n_iter", C.c_uint32)]
 
@@ -77,6 +81,8 @@ def lib():
         _lib.mfo_vegas_iterate.argtypes = [C.c_void_p, C.c_uint64, C.c_int, C.c_void_p]
         _lib.mfo_vegas_accumulate.argtypes = [C.c_void_p, C.c_uint32, C.c_uint64, C.c_uint64, C.c_uint64, C.c_int,
                                               C.c_void_p, C.c_void_p]
+        _lib.mfo_observable_hist.argtypes = [C.c_void_p, C.c_uint32, C.c_uint64, C.c_uint64, C.c_uint64, C.c_int,
+                                             C.c_void_p, C.c_uint32, C.c_void_p, C.c_void_p]
         _lib.mfo_vegas_finalize.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint64, C.c_void_p]
         for f in ("mfo_vegas_destroy", "mfo_result", "mfo_get_grid", "mfo_set_grid", "mfo_get_accum", "mfo_ndim"):
             getattr(_lib, f).argtypes = [C.c_void_p] + [C.c_void_p] * (2 if f == "mfo_ndim" else 0 if f == "mfo_vegas_destroy" else 1)
@@ -249,6 +255,19 @@ class Vegas:
 
     def set_grid(self, e):
         e = _f64(e); _check(lib().mfo_set_grid(self._h, _p(e)))
+
+    def observable_hist(self, iteration, first, n, n_total, obs, n_threads=1):
+        """obs: list of (kind, n_bins, lo, hi); returns a list of (sum, sum2) arrays of n_bins + 2 slots
+        (the last two: underflow, overflow) for the events [first, first+n) of `iteration` on the current grid"""
+        arr = (Observable * len(obs))(*[Observable(int(k), int(nb), float(lo), float(hi)) for k, nb, lo, hi in obs])
+        tot = sum(int(o[1]) + 2 for o in obs)
+        s1, s2 = np.zeros(tot), np.zeros(tot)
+        _check(lib().mfo_observable_hist(self._h, iteration, first, n, n_total, n_threads, arr, len(obs), _p(s1), _p(s2)))
+        out, off = [], 0
+        for o in obs:
+            m = int(o[1]) + 2
+            out.append((s1[off:off + m].copy(), s2[off:off + m].copy())); off += m
+        return out
 
     def get_accum(self):
         a = np.zeros(2 + self.d * self.n_bins); _check(lib().mfo_get_accum(self._h, _p(a))); return a

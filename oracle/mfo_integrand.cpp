@@ -143,6 +143,55 @@ extern "C" int mfo_vegas_accumulate(mfo_vegas_t *h, uint32_t iteration, uint64_t
   return MFO_OK;
 }
 
+// Observable histograms ("histogram accumulation"): the plain definition of mfo.h
+static double observable(int kind, const double *k /* final momenta [n][4] */) {
+  switch (kind) {
+    case MFO_OBS_PT_1: return std::sqrt(k[1] * k[1] + k[2] * k[2]);
+    case MFO_OBS_PT_2: return std::sqrt(k[5] * k[5] + k[6] * k[6]);
+    case MFO_OBS_PT_3: return std::sqrt(k[9] * k[9] + k[10] * k[10]);
+    default: {
+      const double E = k[0] + k[4], px = k[1] + k[5], py = k[2] + k[6], pz = k[3] + k[7];
+      const double m2 = E * E - px * px - py * py - pz * pz;
+      return m2 > 0.0 ? std::sqrt(m2) : 0.0;
+    }
+  }
+}
+extern "C" int mfo_observable_hist(mfo_vegas_t *h, uint32_t iteration, uint64_t first, uint64_t n_events,
+                                   uint64_t n_total, int n_threads, const mfo_observable_t *obs, uint32_t n_obs,
+                                   double *sum, double *sum2) {
+  if (!h || !obs || !sum || !sum2 || n_total == 0) { g_err = "bad argument"; return MFO_EINVAL; }
+  std::vector<size_t> off(n_obs + 1, 0);
+  for (uint32_t o = 0; o < n_obs; ++o) {
+    if (obs[o].kind < 0 || obs[o].kind > 3 || obs[o].n_bins < 1 || !(obs[o].hi > obs[o].lo)) { g_err = "bad observable"; return MFO_EINVAL; }
+    if (obs[o].kind == MFO_OBS_PT_3 && h->n_final < 3) { g_err = "no third final particle"; return MFO_EINVAL; }
+    off[o + 1] = off[o] + obs[o].n_bins + 2;
+  }
+  if (n_threads < 1) n_threads = 1;
+  const size_t tot = off[n_obs];
+  std::vector<std::vector<long double>> p1(n_threads, std::vector<long double>(tot, 0.0L)), p2 = p1;
+  parallel_ranges(n_events, n_threads, [&](int tid, uint64_t lo, uint64_t hi) {
+    for (uint64_t i = lo; i < hi; ++i) {
+      EventRec R; double F = one_event(h, iteration, first + i, R);
+      if (!std::isfinite(F) || F == 0.0) continue;
+      const long double t = (long double)F / (long double)n_total;
+      for (uint32_t o = 0; o < n_obs; ++o) {
+        const double v = observable(obs[o].kind, R.mom + 8);
+        size_t b;
+        if (v < obs[o].lo) b = obs[o].n_bins;
+        else if (v >= obs[o].hi) b = obs[o].n_bins + 1;
+        else { b = (size_t)std::floor((v - obs[o].lo) / (obs[o].hi - obs[o].lo) * obs[o].n_bins); if (b > obs[o].n_bins - 1) b = obs[o].n_bins - 1; }
+        p1[tid][off[o] + b] += t; p2[tid][off[o] + b] += t * t;
+      }
+    }
+  });
+  for (size_t q = 0; q < tot; ++q) {
+    long double a = sum[q], b = sum2[q];
+    for (int t = 0; t < n_threads; ++t) { a += p1[t][q]; b += p2[t][q]; }
+    sum[q] = (double)a; sum2[q] = (double)b;
+  }
+  return MFO_OK;
+}
+
 // O10: sigma_I^2 = max(0, (N S2 - I^2)/(N-1)); refine every iteration; keep every iteration (A2)
 extern "C" int mfo_vegas_finalize(mfo_vegas_t *h, const double *acc, uint64_t n_total, uint64_t n_pass,
                                   uint64_t n_nonfinite, mfo_iter_t *out) {

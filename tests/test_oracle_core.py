@@ -279,3 +279,45 @@ def test_cuts_against_explicit_lab_boost(mfo):
         assert ok == bool(np.all(pt > 30) and np.all(np.abs(eta) < 2.5) and dr > 0.4)
     ok, _ = mfo.cuts(kg[:1], 0.1, 0.1, 0.0, 0.0, 0.0)       # disabled cuts always pass
     assert ok
+
+
+# ---- observable histograms ("histogram accumulation") ----------------------
+def test_observable_hist_config0_matches_closed_form_dsigma_dpt(mfo):
+    """e+e- -> mu+mu-: pT = (sqrt(s)/2) sin(theta) and dsigma/dcos = (3 sigma/8)(1 + cos^2), so the cross
+    section with pT in [a, b) is 2 (3 sigma/8) [c + c^3/3] between c(b) and c(a), c(pT) = sqrt(1 - (2 pT/sqrt s)^2)"""
+    cfg = W.config(0, seed=0)
+    orc = mfo.Vegas(cfg)
+    n, nb, lo, hi = 200_000, 10, 0.0, 50.0
+    (s1, s2), = orc.observable_hist(0, 0, n, n, [(0, nb, lo, hi)], n_threads=mfo.max_threads())
+    sigma = 4 * math.pi * cfg["alpha_em"] ** 2 / (3 * cfg["sqrt_s"] ** 2) * cfg["gev2_to_pb"]
+    c = lambda pt: math.sqrt(max(0.0, 1 - (2 * pt / cfg["sqrt_s"]) ** 2))
+    prim = lambda x: x + x ** 3 / 3
+    edges = np.linspace(lo, hi, nb + 1)
+    exact = np.array([2 * (3 * sigma / 8) * (prim(c(a)) - prim(c(b))) for a, b in zip(edges[:-1], edges[1:])])
+    err = np.sqrt(np.maximum(s2[:nb] * n - s1[:nb] ** 2, 0) / (n - 1))      # per-bin MC error of sum t
+    assert s1[nb] == 0 and s1[nb + 1] == 0                                   # pT never leaves [0, sqrt(s)/2)
+    assert (np.abs(s1[:nb] - exact) < 5 * err + 1e-12).all(), (s1[:nb], exact, err)
+    acc, _ = orc.accumulate(0, 0, n, n, n_threads=mfo.max_threads())
+    assert abs(s1.sum() / acc[0] - 1) < 1e-12 and abs(s2.sum() / acc[1] - 1) < 1e-12   # every event lands in one slot
+
+
+def test_observable_hist_definitions_against_numpy(mfo):
+    """all four kinds, under/overflow slots, on gg -> tt~g: rebuilt in NumPy from the per-event records"""
+    cfg = W.config(W.GG_TTG, seed=4)
+    orc = mfo.Vegas(cfg)
+    n = 4000
+    obs = [(0, 7, 20.0, 300.0), (1, 5, 0.0, 150.0), (2, 9, 400.0, 2000.0), (3, 6, 30.0, 200.0)]
+    got = orc.observable_hist(1, 100, n, n, obs, n_threads=mfo.max_threads())
+    ev = orc.eval(1, 100, n, n_threads=mfo.max_threads())
+    k = ev["momenta"][:, 2:]
+    tot = k[:, 0] + k[:, 1]
+    vals = [np.hypot(k[:, 0, 1], k[:, 0, 2]), np.hypot(k[:, 1, 1], k[:, 1, 2]),
+            np.sqrt(tot[:, 0] ** 2 - (tot[:, 1:] ** 2).sum(1)), np.hypot(k[:, 2, 1], k[:, 2, 2])]
+    t = ev["weight"] / n
+    for (kind, nb, lo, hi), v, (s1, s2) in zip(obs, vals, got):
+        b = np.floor((v - lo) / (hi - lo) * nb).astype(int)
+        b = np.where(v < lo, nb, np.where(v >= hi, nb + 1, np.minimum(b, nb - 1)))
+        ref1 = np.bincount(b, weights=t, minlength=nb + 2); ref2 = np.bincount(b, weights=t * t, minlength=nb + 2)
+        np.testing.assert_allclose(s1, ref1, rtol=1e-12, atol=1e-300)
+        np.testing.assert_allclose(s2, ref2, rtol=1e-12, atol=1e-300)
+        assert s1[nb] > 0 or s1[nb + 1] > 0 or kind == 3                     # the ranges above cut into the spectra

@@ -97,9 +97,30 @@ int mf_vegas_iterate(mf_vegas_t *h, uint64_t n_events, void *cuda_stream, mf_ite
  * accumulate(0, n, n) + finalize.                                                                   */
 int mf_vegas_accumulate(mf_vegas_t *h, uint64_t first_event, uint64_t n_events, uint64_t n_total,
                         void *cuda_stream);
-int mf_get_accum(mf_vegas_t *h, double *host_acc /* [2 + d*n_bins] */, uint64_t *host_counts /* [2] */);
+int mf_get_accum(mf_vegas_t *h, double *host_acc /* [mf_accum_len()] = [2 + d*n_bins] without observables */, uint64_t *host_counts /* [2] */);
 int mf_set_accum(mf_vegas_t *h, const double *host_acc, const uint64_t *host_counts);
 int mf_vegas_finalize(mf_vegas_t *h, uint64_t n_total, void *cuda_stream, mf_iter_t *host_out_or_null);
+
+/* Observable histograms filled in the same pass as the integral ("histogram accumulation";
+ * dsigma/dpT of the top quark is the paper's physics plot).  For every event with weight
+ * F_i != 0, t_i = F_i / N: sum[o][b] += t_i, sum2[o][b] += t_i^2 with b = floor((v-lo)/(hi-lo)*n_bins)
+ * for lo <= v < hi, slot 62 for v < lo (underflow), slot 63 for v >= hi (overflow); v from the final-state
+ * momenta (partonic CM frame; all kinds are invariant under the boost along the beam).  At most
+ * MF_MAX_OBS observables of at most 62 bins; each histogram has MF_OBS_SLOTS = 64 slots.
+ * mf_set_observables copies the definitions and clears the accumulated histograms (n_obs = 0 turns the
+ * feature off).  Every finalized iteration adds its histograms to the accumulated ones;
+ * mf_get_observables returns them ([n_obs][64] doubles each, host) and the number of iterations summed
+ * (divide by it, and by the bin width, for dsigma/dv).  While observables are set, the raw-sum vector
+ * of the sharded form (mf_get_accum / mf_set_accum) has mf_accum_len() = 2 + d*n_bins + 2*MF_MAX_OBS*64
+ * entries (this iteration's observable sums behind the VEGAS sums).  Processes 2 and 3 fill them on the
+ * staged path only (MF_EUNSUPPORTED from mf_vegas_accumulate on the fused path).                     */
+enum { MF_OBS_PT_1 = 0, MF_OBS_PT_2 = 1, MF_OBS_M_12 = 2, MF_OBS_PT_3 = 3 };
+#define MF_MAX_OBS 4
+#define MF_OBS_SLOTS 64
+typedef struct { int32_t kind; uint32_t n_bins; double lo, hi; } mf_observable_t;
+int mf_set_observables(mf_vegas_t *h, const mf_observable_t *obs, uint32_t n_obs);
+int mf_get_observables(mf_vegas_t *h, double *host_sum, double *host_sum2, uint32_t *n_iter);
+int mf_accum_len(const mf_vegas_t *h, uint32_t *n);
 
 /* O11 combination over all iterations so far; synchronises the last-used stream.  MF_ESTATE if no
  * iteration has been run.                                                                           */

@@ -15,7 +15,8 @@ MF_OK, MF_EINVAL, MF_ENOMEM, MF_ECUDA, MF_ESTATE, MF_EUNSUPPORTED = 0, -1, -2, -
 EXPORTS = ["mf_vegas_create", "mf_vegas_destroy", "mf_ndim", "mf_integrand_eval", "mf_vegas_iterate",
            "mf_vegas_accumulate", "mf_get_accum", "mf_set_accum", "mf_vegas_finalize", "mf_result",
            "mf_get_iterations", "mf_get_grid", "mf_set_grid", "mf_set_launch", "mf_me_flops",
-           "mf_fp64_peak", "mf_last_kernel_ms", "mf_last_error", "mf_set_path", "mf_last_stage_ms"]
+           "mf_fp64_peak", "mf_last_kernel_ms", "mf_last_error", "mf_set_path", "mf_last_stage_ms",
+           "mf_set_observables", "mf_get_observables", "mf_accum_len"]
 
 
 class MfError(RuntimeError):
@@ -93,12 +94,22 @@ def lib():
         L.mf_set_grid.argtypes = [vp, vp]
         L.mf_set_launch.argtypes = [vp, u32, u32]
         L.mf_set_path.argtypes = [vp, C.c_int32]
+        L.mf_set_observables.argtypes = [vp, vp, u32]
+        L.mf_get_observables.argtypes = [vp, vp, vp, C.POINTER(u32)]
+        L.mf_accum_len.argtypes = [vp, C.POINTER(u32)]
         L.mf_last_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
         L.mf_me_flops.argtypes = [vp, C.POINTER(u64), C.POINTER(u64), C.POINTER(u64)]
         L.mf_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
         L.mf_fp64_peak.argtypes = [C.c_int32, C.c_double, C.POINTER(C.c_double)]
         _lib = L
     return _lib
+
+
+class Observable(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("n_bins", C.c_uint32), ("lo", C.c_double), ("hi", C.c_double)]
+
+
+OBS_PT_1, OBS_PT_2, OBS_M_12, OBS_PT_3 = 0, 1, 2, 3
 
 
 def _check(rc):
@@ -163,8 +174,31 @@ class Vegas:
     def vegas_accumulate(self, first_event, n_events, n_total, stream=None):
         _check(lib().mf_vegas_accumulate(self._h, int(first_event), int(n_events), int(n_total), _stream_ptr(stream)))
 
+    def accum_len(self):
+        n = C.c_uint32()
+        _check(lib().mf_accum_len(self._h, C.byref(n)))
+        return n.value
+
+    def set_observables(self, obs):
+        """obs: list of (kind, n_bins, lo, hi), kinds OBS_PT_1 / OBS_PT_2 / OBS_M_12 / OBS_PT_3; [] turns them off"""
+        arr = (Observable * max(1, len(obs)))(*[Observable(int(k), int(nb), float(lo), float(hi)) for k, nb, lo, hi in obs])
+        _check(lib().mf_set_observables(self._h, C.cast(arr, C.c_void_p), len(obs)))
+        self._obs = list(obs)
+
+    def get_observables(self):
+        """[(sum, sum2)] per observable, each n_bins + 2 slots (last two: underflow, overflow), summed over the
+        iterations since set_observables; and the number of those iterations"""
+        n = len(self._obs)
+        s1 = np.zeros((n, 64)); s2 = np.zeros((n, 64)); it = C.c_uint32()
+        _check(lib().mf_get_observables(self._h, s1.ctypes.data, s2.ctypes.data, C.byref(it)))
+        out = []
+        for o, (k, nb, lo, hi) in enumerate(self._obs):
+            pick = list(range(int(nb))) + [62, 63]
+            out.append((s1[o, pick].copy(), s2[o, pick].copy()))
+        return out, it.value
+
     def get_accum(self):
-        acc = np.zeros(2 + self.d * self.n_bins); cnt = np.zeros(2, np.uint64)
+        acc = np.zeros(self.accum_len()); cnt = np.zeros(2, np.uint64)
         _check(lib().mf_get_accum(self._h, acc.ctypes.data, cnt.ctypes.data))
         return acc, cnt
 

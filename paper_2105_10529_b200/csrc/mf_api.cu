@@ -26,6 +26,8 @@ struct mf_vegas {
   MfParams P;
   int device, n_sm;
   int na;                              // 2 + d*nb
+  int row;                             // na + MF_OBS_ACC: allocated length of a raw-sum record (observable sums behind)
+  double* d_obs;                       // accumulated observable histograms [MF_OBS_ACC] + iterations summed
   size_t smem_iter, smem_eval;
   int occ_iter, occ_eval;              // resident blocks per SM of the two kernels
   uint32_t blocks_per_sm, threads;     // user override (0 = default)
@@ -63,6 +65,7 @@ extern "C" int mf_vegas_create(const mf_config_t* cfg, mf_vegas_t** out) {
   std::memset(h, 0, sizeof *h);
   h->cfg = *cfg; h->cfg.pdf_xf = nullptr; h->P = P; h->device = cfg->device;
   h->na = 2 + P.d * P.nb;
+  h->row = h->na + MF_OBS_ACC;
 #define MF_CREATE_CUDA(call)                                                     \
   do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { std::string m_ = std::string(#call) + ": " + cudaGetErrorString(e_); mf_vegas_destroy(h); return fail(MF_ECUDA, m_); } } while (0)
   MF_CREATE_CUDA(cudaSetDevice(h->device));
@@ -77,13 +80,15 @@ extern "C" int mf_vegas_create(const mf_config_t* cfg, mf_vegas_t** out) {
   const size_t ne = (size_t)P.d * (P.nb + 1), npdf = (size_t)P.pdf_nx * P.pdf_nq;
   MF_CREATE_CUDA(cudaMalloc(&h->d_edges, ne * sizeof(double)));
   MF_CREATE_CUDA(cudaMalloc(&h->d_pdf, (npdf ? npdf : 1) * sizeof(double)));
-  MF_CREATE_CUDA(cudaMalloc(&h->d_partial, (size_t)h->max_blocks * h->na * sizeof(double)));
+  MF_CREATE_CUDA(cudaMalloc(&h->d_partial, (size_t)h->max_blocks * h->row * sizeof(double)));
   MF_CREATE_CUDA(cudaMalloc(&h->d_pcount, (size_t)h->max_blocks * 2 * sizeof(unsigned long long)));
-  MF_CREATE_CUDA(cudaMalloc(&h->d_acc, h->na * sizeof(double)));
+  MF_CREATE_CUDA(cudaMalloc(&h->d_acc, h->row * sizeof(double)));
   MF_CREATE_CUDA(cudaMalloc(&h->d_counts, 2 * sizeof(unsigned long long)));
+  MF_CREATE_CUDA(cudaMalloc(&h->d_obs, (MF_OBS_ACC + 1) * sizeof(double)));
+  MF_CREATE_CUDA(cudaMemset(h->d_obs, 0, (MF_OBS_ACC + 1) * sizeof(double)));
   MF_CREATE_CUDA(cudaMalloc(&h->d_state, sizeof(MfDevState)));
   MF_CREATE_CUDA(cudaMemset(h->d_state, 0, sizeof(MfDevState)));
-  MF_CREATE_CUDA(cudaMemset(h->d_acc, 0, h->na * sizeof(double)));
+  MF_CREATE_CUDA(cudaMemset(h->d_acc, 0, h->row * sizeof(double)));
   MF_CREATE_CUDA(cudaMemset(h->d_counts, 0, 2 * sizeof(unsigned long long)));
   std::vector<double> e(ne);
   for (int j = 0; j < P.d; ++j)
@@ -104,7 +109,7 @@ extern "C" int mf_vegas_destroy(mf_vegas_t* h) {
   cudaSetDevice(h->device);
   cudaFree(h->d_edges); cudaFree(h->d_pdf); cudaFree(h->d_partial); cudaFree(h->d_pcount);
   cudaFree(h->d_acc); cudaFree(h->d_counts); cudaFree(h->d_state);
-  cudaFree(h->ws.rec); cudaFree(h->ws.count);
+  cudaFree(h->ws.rec); cudaFree(h->ws.count); cudaFree(h->d_obs);
   for (int i = 0; i < 4; ++i) if (h->evs[i]) cudaEventDestroy(h->evs[i]);
   if (h->ev0) cudaEventDestroy(h->ev0);
   if (h->ev1) cudaEventDestroy(h->ev1);
@@ -129,6 +134,8 @@ extern "C" int mf_set_launch(mf_vegas_t* h, uint32_t blocks_per_sm, uint32_t thr
   h->blocks_per_sm = blocks_per_sm; h->threads = threads_per_block;
   return MF_OK;
 }
+
+static inline int live_len(const mf_vegas* h) { return h->P.n_obs > 0 ? h->row : h->na; }   // live entries of a raw-sum record
 
 static int grid_for(const mf_vegas* h, unsigned long long n, int occ) {
   const int per_sm = h->blocks_per_sm ? (int)h->blocks_per_sm : occ;
@@ -203,8 +210,8 @@ extern "C" int mf_vegas_accumulate(mf_vegas_t* h, uint64_t first_event, uint64_t
       if (grid_hist > h->ws.regions) grid_hist = h->ws.regions;
       if (grid_hist > h->max_blocks) grid_hist = h->max_blocks;
       MF_CUDA(h->ops->staged(h->P, h->d_edges, h->d_pdf, h->iteration, first_event + done, m, (double)n_total, h->ws,
-                             h->d_partial, h->d_pcount, grid_me, grid_hist, st, h->evs));
-      mf_reduce_kernel<<<(h->na + 2 + 7) / 8, MF_REDUCE_THREADS, 0, st>>>(h->d_partial, h->d_pcount, grid_hist, h->na, h->d_acc, h->d_counts);
+                             h->d_partial, h->d_pcount, h->row, grid_me, grid_hist, st, h->evs));
+      mf_reduce_kernel<<<(live_len(h) + 2 + 7) / 8, MF_REDUCE_THREADS, 0, st>>>(h->d_partial, h->d_pcount, grid_hist, live_len(h), h->row, h->d_acc, h->d_counts);
       MF_CUDA(cudaGetLastError());
     }
     h->have_stage = true; h->have_k = false;
@@ -213,11 +220,15 @@ extern "C" int mf_vegas_accumulate(mf_vegas_t* h, uint64_t first_event, uint64_t
   }
   const int grid = grid_for(h, n_events, h->occ_iter);
   MF_CUDA(cudaEventRecord(h->evk0, st));
-  MF_CUDA(h->ops->iterate(h->P, h->d_edges, h->d_pdf, h->iteration, first_event, n_events, (double)n_total,
-                          h->d_partial, h->d_pcount, grid, h->smem_iter, st));
+  {
+    cudaError_t e_ = h->ops->iterate(h->P, h->d_edges, h->d_pdf, h->iteration, first_event, n_events, (double)n_total,
+                                     h->d_partial, h->d_pcount, h->row, grid, h->smem_iter, st);
+    if (e_ == cudaErrorNotSupported) return fail(MF_EUNSUPPORTED, "observables of processes 2 and 3 need the staged path");
+    MF_CUDA(e_);
+  }
   MF_CUDA(cudaEventRecord(h->evk1, st));
   h->have_k = true; h->have_stage = false;
-  mf_reduce_kernel<<<(h->na + 2 + 7) / 8, MF_REDUCE_THREADS, 0, st>>>(h->d_partial, h->d_pcount, grid, h->na, h->d_acc, h->d_counts);
+  mf_reduce_kernel<<<(live_len(h) + 2 + 7) / 8, MF_REDUCE_THREADS, 0, st>>>(h->d_partial, h->d_pcount, grid, live_len(h), h->row, h->d_acc, h->d_counts);
   MF_CUDA(cudaGetLastError());
   h->last_stream = st;
   return MF_OK;
@@ -250,7 +261,7 @@ extern "C" int mf_vegas_finalize(mf_vegas_t* h, uint64_t n_total, void* cuda_str
   MF_CUDA(cudaSetDevice(h->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
   mf_finalize_kernel<<<1, 32 * h->P.d, 0, st>>>(h->P, h->cfg.alpha_damp, (double)n_total, n_total, h->d_acc, h->d_counts,
-                                        h->d_edges, h->d_state);
+                                        h->d_edges, h->d_state, h->d_obs);
   MF_CUDA(cudaGetLastError());
   // the raw sums stay readable (mf_get_accum) until the next iteration starts
   const uint32_t idx = h->iteration++;
@@ -266,7 +277,7 @@ extern "C" int mf_vegas_finalize(mf_vegas_t* h, uint64_t n_total, void* cuda_str
 }
 
 static int zero_accum(mf_vegas* h, cudaStream_t st) {
-  MF_CUDA(cudaMemsetAsync(h->d_acc, 0, h->na * sizeof(double), st));
+  MF_CUDA(cudaMemsetAsync(h->d_acc, 0, live_len(h) * sizeof(double), st));
   MF_CUDA(cudaMemsetAsync(h->d_counts, 0, 2 * sizeof(unsigned long long), st));
   return MF_OK;
 }
@@ -323,7 +334,7 @@ extern "C" int mf_get_accum(mf_vegas_t* h, double* host_acc, uint64_t* host_coun
   if (!h || !host_acc) return fail(MF_EINVAL, "null argument");
   MF_CUDA(cudaSetDevice(h->device));
   MF_CUDA(cudaStreamSynchronize(h->last_stream));
-  MF_CUDA(cudaMemcpy(host_acc, h->d_acc, h->na * sizeof(double), cudaMemcpyDeviceToHost));
+  MF_CUDA(cudaMemcpy(host_acc, h->d_acc, live_len(h) * sizeof(double), cudaMemcpyDeviceToHost));
   if (host_counts) MF_CUDA(cudaMemcpy(host_counts, h->d_counts, 2 * sizeof(uint64_t), cudaMemcpyDeviceToHost));
   return MF_OK;
 }
@@ -332,8 +343,48 @@ extern "C" int mf_set_accum(mf_vegas_t* h, const double* host_acc, const uint64_
   if (!h || !host_acc) return fail(MF_EINVAL, "null argument");
   MF_CUDA(cudaSetDevice(h->device));
   MF_CUDA(cudaStreamSynchronize(h->last_stream));
-  MF_CUDA(cudaMemcpy(h->d_acc, host_acc, h->na * sizeof(double), cudaMemcpyHostToDevice));
+  MF_CUDA(cudaMemcpy(h->d_acc, host_acc, live_len(h) * sizeof(double), cudaMemcpyHostToDevice));
   if (host_counts) MF_CUDA(cudaMemcpy(h->d_counts, host_counts, 2 * sizeof(uint64_t), cudaMemcpyHostToDevice));
+  return MF_OK;
+}
+
+extern "C" int mf_set_observables(mf_vegas_t* h, const mf_observable_t* obs, uint32_t n_obs) {
+  if (!h) return fail(MF_EINVAL, "handle is NULL");
+  if (n_obs > MF_MAX_OBS || (n_obs > 0 && !obs)) return fail(MF_EINVAL, "at most 4 observables");
+  for (uint32_t o = 0; o < n_obs; ++o) {
+    if (obs[o].kind < 0 || obs[o].kind > 3) return fail(MF_EINVAL, "unknown observable kind");
+    if (obs[o].kind == MF_OBS_PT_3 && h->P.n_final < 3) return fail(MF_EINVAL, "this process has no third final particle");
+    if (obs[o].n_bins < 1 || obs[o].n_bins > 62) return fail(MF_EINVAL, "observable n_bins must be in 1..62");
+    if (!(obs[o].hi > obs[o].lo)) return fail(MF_EINVAL, "observable range is empty");
+  }
+  MF_CUDA(cudaSetDevice(h->device));
+  MF_CUDA(cudaStreamSynchronize(h->last_stream));
+  h->P.n_obs = (int32_t)n_obs;
+  for (uint32_t o = 0; o < n_obs; ++o) {
+    h->P.obs_kind[o] = obs[o].kind; h->P.obs_nb[o] = (int32_t)obs[o].n_bins; h->P.obs_lo[o] = obs[o].lo; h->P.obs_hi[o] = obs[o].hi;
+  }
+  MF_CUDA(cudaMemset(h->d_obs, 0, (MF_OBS_ACC + 1) * sizeof(double)));
+  MF_CUDA(cudaMemset(h->d_acc, 0, h->row * sizeof(double)));
+  return MF_OK;
+}
+
+extern "C" int mf_get_observables(mf_vegas_t* h, double* host_sum, double* host_sum2, uint32_t* n_iter) {
+  if (!h || !host_sum || !host_sum2) return fail(MF_EINVAL, "null argument");
+  if (h->P.n_obs == 0) return fail(MF_ESTATE, "no observables set");
+  MF_CUDA(cudaSetDevice(h->device));
+  MF_CUDA(cudaStreamSynchronize(h->last_stream));
+  const size_t n = (size_t)h->P.n_obs * MF_OBS_SLOTS;
+  MF_CUDA(cudaMemcpy(host_sum, h->d_obs, n * sizeof(double), cudaMemcpyDeviceToHost));
+  MF_CUDA(cudaMemcpy(host_sum2, h->d_obs + MF_OBS_ACC / 2, n * sizeof(double), cudaMemcpyDeviceToHost));
+  double it = 0.0;
+  MF_CUDA(cudaMemcpy(&it, h->d_obs + MF_OBS_ACC, sizeof(double), cudaMemcpyDeviceToHost));
+  if (n_iter) *n_iter = (uint32_t)it;
+  return MF_OK;
+}
+
+extern "C" int mf_accum_len(const mf_vegas_t* h, uint32_t* n) {
+  if (!h || !n) return fail(MF_EINVAL, "null argument");
+  *n = (uint32_t)live_len(h);
   return MF_OK;
 }
 

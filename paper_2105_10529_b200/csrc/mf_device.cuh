@@ -74,6 +74,8 @@ struct MfParams {
   double me_pref;                       // g_s^(2 ng) / 256 * generator scale, or e^4/4 (O6)
   double ptmin, etamax, drmin;          // cuts (O7)
   double tanh_etamax;                   // tanh(etamax): the eta cut is taken on tanh (mf_cuts)
+  int32_t n_obs, obs_kind[4], obs_nb[4];  // observable histograms (include/madflow_b200.h mf_set_observables)
+  double obs_lo[4], obs_hi[4];
   double wconst;                        // S_f * K / 2  (O8: F = ... S_f W_PS K / (2 shat))
   double pdf_lx0, pdf_ihx, pdf_lq0, pdf_ihq, pdf_lq;   // ln xmin, 1/h_x, ln qmin^2, 1/h_q, ln muF^2
   int32_t pdf_nx, pdf_nq;
@@ -311,6 +313,40 @@ MF_HD bool mf_cuts(const MfParams& P, const double kg[][4], double x1, double x2
     if (!(sqrt(deta * deta + dphi * dphi) > P.drmin)) pass = false;
   }
   return pass;
+}
+
+// ---- observable histogram slots ("histogram accumulation") ---------------------
+// k: final-state momenta [N][4]; returns the slots of the P.n_obs observables packed 6 bits each:
+// bin = floor((v-lo)/(hi-lo)*n_bins) for lo <= v < hi, 62 = underflow, 63 = overflow
+#define MF_OBS_MAX 4
+#define MF_OBS_SLOTS 64
+template <int N>
+MF_HD unsigned mf_obs_keys(const MfParams& P, const double k[N][4]) {
+  unsigned keys = 0;
+#pragma unroll
+  for (int o = 0; o < MF_OBS_MAX; ++o) {
+    if (o >= P.n_obs) break;
+    const int kind = P.obs_kind[o];
+    double v;
+    if (kind == 2) {
+      const double E = k[0][0] + k[1][0], px = k[0][1] + k[1][1], py = k[0][2] + k[1][2], pz = k[0][3] + k[1][3];
+      const double m2 = E * E - px * px - py * py - pz * pz;
+      v = m2 > 0.0 ? sqrt(m2) : 0.0;
+    } else {
+      const int i = (kind == 0) ? 0 : (kind == 1) ? 1 : (N > 2 ? 2 : 0);
+      v = sqrt(k[i][1] * k[i][1] + k[i][2] * k[i][2]);
+    }
+    unsigned b;
+    if (v < P.obs_lo[o]) b = 62u;
+    else if (v >= P.obs_hi[o]) b = 63u;
+    else {
+      const int nb = P.obs_nb[o];
+      int q = (int)floor((v - P.obs_lo[o]) / (P.obs_hi[o] - P.obs_lo[o]) * (double)nb);
+      b = (unsigned)(q > nb - 1 ? nb - 1 : q);
+    }
+    keys |= b << (6 * o);
+  }
+  return keys;
 }
 
 // ---- S7a: external-wavefunction ingredients (O6.2), the "conditional control statements" of

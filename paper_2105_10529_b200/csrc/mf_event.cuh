@@ -82,7 +82,7 @@ MF_HD double mf_me2(const MfParams& P, double rts, const double k[MfProc<PROC>::
 template <int PROC, bool REC>
 MF_HD bool mf_event_front(const MfParams& P, const double* edges, const double* pdf_tab, uint32_t iteration,
                           uint64_t ev, int bin[MfProc<PROC>::D], double k[MfProc<PROC>::N][4], double& rts,
-                          double& pref, MfEventRec* rec) {
+                          double& pref, MfEventRec* rec, unsigned* okeys = nullptr) {
   constexpr int D = MfProc<PROC>::D, N = MfProc<PROC>::N, NGL = MfProc<PROC>::NGL;
   double u[D], y[D];
   mf_uniforms<D>(P, iteration, ev, u);                                   // S1
@@ -99,6 +99,7 @@ MF_HD bool mf_event_front(const MfParams& P, const double* edges, const double* 
     f1 = xf1 / x1; f2 = xf2 / x2;
   }
   pref = JV * jx * f1 * f2 * wps * P.wconst / shat;                      // S8 without |M|^2
+  if (okeys) *okeys = (P.n_obs > 0 && pass) ? mf_obs_keys<N>(P, (const double(*)[4])k) : 0u;
   if (REC) {
 #pragma unroll
     for (int j = 0; j < D; ++j) rec->y[j] = y[j];
@@ -119,10 +120,10 @@ MF_HD bool mf_event_front(const MfParams& P, const double* edges, const double* 
 template <int PROC, bool REC>
 MF_HD double mf_event(const MfParams& P, const double* edges, const double* pdf_tab,
                       uint32_t iteration, uint64_t ev, int bin[MfProc<PROC>::D], bool& pass,
-                      MfEventRec* rec) {
+                      MfEventRec* rec, unsigned* okeys = nullptr) {
   constexpr int N = MfProc<PROC>::N;
   double k[N][4], rts, pref;
-  pass = mf_event_front<PROC, REC>(P, edges, pdf_tab, iteration, ev, bin, k, rts, pref, rec);
+  pass = mf_event_front<PROC, REC>(P, edges, pdf_tab, iteration, ev, bin, k, rts, pref, rec, okeys);
   double me2 = 0.0;
   if (MF_UNIFORM_ME || pass) me2 = mf_me2<PROC>(P, rts, k);              // S7
   if (!pass) me2 = 0.0;

@@ -47,13 +47,45 @@ __device__ __forceinline__ void mf_hist_add(double* __restrict__ hw, int nb, uns
   }
 }
 
+// observable histograms of one warp: ho1[o][64] += t, ho2[o][64] += t^2, same fixed-order scheme
+__device__ __forceinline__ void mf_obs_add(double* __restrict__ ho1, double* __restrict__ ho2, int n_obs, unsigned keys,
+                                           bool contrib, double t, double t2, unsigned lt_mask) {
+  const unsigned full = 0xffffffffu;
+  const unsigned cmask = __ballot_sync(full, contrib);
+  if (cmask == 0u) return;                               // warp-uniform
+  unsigned rank[MF_OBS_MAX], key[MF_OBS_MAX], maxrank = 0;
+#pragma unroll
+  for (int j = 0; j < MF_OBS_MAX; ++j) {
+    key[j] = (keys >> (6 * j)) & 63u; rank[j] = 0;
+    if (j < n_obs) {                                     // warp-uniform
+      unsigned peers = cmask;
+#pragma unroll
+      for (int b = 0; b < 6; ++b) {
+        const bool bit = (key[j] >> b) & 1u;
+        const unsigned bal = __ballot_sync(full, bit);
+        peers &= bit ? bal : ~bal;
+      }
+      rank[j] = __popc(peers & lt_mask);
+      maxrank = rank[j] > maxrank ? rank[j] : maxrank;
+    }
+  }
+  for (unsigned r = 0; __any_sync(full, contrib && maxrank >= r); ++r) {
+#pragma unroll
+    for (int j = 0; j < MF_OBS_MAX; ++j)
+      if (j < n_obs && contrib && rank[j] == r) { ho1[j * MF_OBS_SLOTS + key[j]] += t; ho2[j * MF_OBS_SLOTS + key[j]] += t2; }
+    __syncwarp();
+  }
+}
+#define MF_OBS_ACC (2 * MF_OBS_MAX * MF_OBS_SLOTS)         // doubles per record behind the 2 + d*nb VEGAS sums
+
 // ---- S1-S9 fused ---------------------------------------------------------------------------------
-// partial: [gridDim.x][2 + d*nb] doubles, pcount: [gridDim.x][2] (n_pass, n_nonfinite)
+// partial: [gridDim.x][row] doubles (2 + d*nb sums, then the observable sums), pcount: [gridDim.x][2]
+// (n_pass, n_nonfinite)
 template <int PROC>
 __global__ void __launch_bounds__(MF_THREADS, MfLaunch<PROC>::MINB)
 mf_iterate_kernel(const MfParams P, const double* __restrict__ g_edges, const double* __restrict__ g_pdf,
                   uint32_t iteration, unsigned long long first, unsigned long long n, double n_total,
-                  double* __restrict__ partial, unsigned long long* __restrict__ pcount) {
+                  double* __restrict__ partial, unsigned long long* __restrict__ pcount, int row) {
   constexpr int D = MfProc<PROC>::D;
   extern __shared__ double smem[];
   const int nb = P.nb, nh = D * nb, nw = blockDim.x >> 5;
@@ -61,8 +93,10 @@ mf_iterate_kernel(const MfParams P, const double* __restrict__ g_edges, const do
   double* s_pdf = s_edges + D * (nb + 1);
   double* s_hist = s_pdf + P.pdf_nx * P.pdf_nq;          // [nw][D*nb]
   double* s_red = s_hist + nw * nh;                      // [nw][4]
+  double* s_obs = s_red + nw * 4;                        // [nw][MF_OBS_ACC] when observables are set
   mf_stage_tables(P, g_edges, g_pdf, s_edges, s_pdf);
   for (int i = threadIdx.x; i < nw * nh; i += blockDim.x) s_hist[i] = 0.0;
+  if (P.n_obs > 0) for (int i = threadIdx.x; i < nw * MF_OBS_ACC; i += blockDim.x) s_obs[i] = 0.0;
   __syncthreads();
 
   const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
@@ -78,11 +112,12 @@ mf_iterate_kernel(const MfParams P, const double* __restrict__ g_edges, const do
     int bin[D];
     bool pass = false;
     double F = 0.0;
+    unsigned okeys = 0;
     if (MF_UNIFORM_ME) {                                 // every thread runs the event (barriers inside);
-      F = mf_event<PROC, false>(P, s_edges, s_pdf, iteration, first + (valid ? i : n - 1), bin, pass, nullptr);
+      F = mf_event<PROC, false>(P, s_edges, s_pdf, iteration, first + (valid ? i : n - 1), bin, pass, nullptr, &okeys);
       if (!valid) { F = 0.0; pass = false; }             // lanes past the end recompute event n-1, discarded
     } else if (valid) {
-      F = mf_event<PROC, false>(P, s_edges, s_pdf, iteration, first + i, bin, pass, nullptr);
+      F = mf_event<PROC, false>(P, s_edges, s_pdf, iteration, first + i, bin, pass, nullptr, &okeys);
     }
     if (!isfinite(F)) { F = 0.0; ++n_bad; }              // A20
     if (valid && pass) ++n_pass;
@@ -93,6 +128,8 @@ mf_iterate_kernel(const MfParams P, const double* __restrict__ g_edges, const do
 #pragma unroll
     for (int j = 0; j < D; ++j) packed |= (unsigned long long)bin[j] << (6 * j);
     mf_hist_add<D>(hw, nb, packed, valid && t2 != 0.0, t2, lt_mask);
+    if (P.n_obs > 0)
+      mf_obs_add(s_obs + warp * MF_OBS_ACC, s_obs + warp * MF_OBS_ACC + MF_OBS_ACC / 2, P.n_obs, okeys, valid && F != 0.0, t, t2, lt_mask);
   }
   // fixed-order reductions: xor-butterfly inside the warp, warps in index order inside the block
 #pragma unroll
@@ -108,11 +145,16 @@ mf_iterate_kernel(const MfParams P, const double* __restrict__ g_edges, const do
     s_red[warp * 4 + 3] = __longlong_as_double((long long)n_bad);
   }
   __syncthreads();
-  double* out = partial + (size_t)blockIdx.x * (2 + nh);
+  double* out = partial + (size_t)blockIdx.x * row;
   for (int e = threadIdx.x; e < nh; e += blockDim.x) {
     double s = 0.0;
     for (int w = 0; w < nw; ++w) s += s_hist[w * nh + e];
     out[2 + e] = s;
+  }
+  if (P.n_obs > 0) for (int e = threadIdx.x; e < MF_OBS_ACC; e += blockDim.x) {
+    double s = 0.0;
+    for (int w = 0; w < nw; ++w) s += s_obs[w * MF_OBS_ACC + e];
+    out[2 + nh + e] = s;
   }
   if (threadIdx.x == 0) {
     double a = 0.0, b = 0.0; unsigned long long c = 0, d2 = 0;
@@ -137,7 +179,7 @@ template <int PROC>
 __global__ void __launch_bounds__(MF_THREADS, MfLaunch<PROC>::MINB)
 mf_iterate_compact_kernel(const MfParams P, const double* __restrict__ g_edges, const double* __restrict__ g_pdf,
                           uint32_t iteration, unsigned long long first, unsigned long long n, double n_total,
-                          double* __restrict__ partial, unsigned long long* __restrict__ pcount) {
+                          double* __restrict__ partial, unsigned long long* __restrict__ pcount, int row) {
   constexpr int D = MfProc<PROC>::D, N = MfProc<PROC>::N, NF = 4 * N + 3, T = MF_THREADS, CAP = 2 * MF_THREADS;
   extern __shared__ double smem[];
   const int nb = P.nb, nh = D * nb, nw = T >> 5;
@@ -224,7 +266,7 @@ mf_iterate_compact_kernel(const MfParams P, const double* __restrict__ g_edges, 
     s_red[warp * 4 + 3] = __longlong_as_double((long long)n_bad);
   }
   __syncthreads();
-  double* out = partial + (size_t)blockIdx.x * (2 + nh);
+  double* out = partial + (size_t)blockIdx.x * row;
   for (int e = tid; e < nh; e += T) {
     double s = 0.0;
     for (int w = 0; w < nw; ++w) s += s_hist[w * nh + e];
@@ -264,7 +306,7 @@ __global__ void __launch_bounds__(MF_THREADS, MF_FRONT_MINB)
 mf_front_kernel(const MfParams P, const double* __restrict__ g_edges, const double* __restrict__ g_pdf,
                 uint32_t iteration, unsigned long long first, unsigned long long n, unsigned long long cap,
                 double* __restrict__ rec, unsigned int* __restrict__ count) {
-  constexpr int D = MfProc<PROC>::D, N = MfProc<PROC>::N, NF = 4 * N + 3, T = MF_THREADS;
+  constexpr int D = MfProc<PROC>::D, N = MfProc<PROC>::N, NF = 4 * N + 4, T = MF_THREADS;
   extern __shared__ double smem[];
   double* s_edges = smem;
   double* s_pdf = s_edges + D * (P.nb + 1);
@@ -282,7 +324,8 @@ mf_front_kernel(const MfParams P, const double* __restrict__ g_edges, const doub
     bool pass = false;
     int bin[D];
     double k[N][4], rts, pref;
-    if (i < hi) pass = mf_event_front<PROC, false>(P, s_edges, s_pdf, iteration, first + i, bin, k, rts, pref, nullptr);
+    unsigned okeys = 0;
+    if (i < hi) pass = mf_event_front<PROC, false>(P, s_edges, s_pdf, iteration, first + i, bin, k, rts, pref, nullptr, &okeys);
     const unsigned bal = __ballot_sync(0xffffffffu, pass);
     if (lane == 0) s_wtot[warp] = __popc(bal);
     __syncthreads();
@@ -301,6 +344,7 @@ mf_front_kernel(const MfParams P, const double* __restrict__ g_edges, const doub
 #pragma unroll
       for (int j = 0; j < D; ++j) packed |= (unsigned long long)bin[j] << (6 * j);
       R[(size_t)(4 * N + 2) * cap + slot] = __longlong_as_double((long long)packed);
+      if (P.n_obs > 0) R[(size_t)(4 * N + 3) * cap + slot] = __longlong_as_double((long long)okeys);
     }
     __syncthreads();
     filled += tot;
@@ -318,7 +362,7 @@ template <int PROC>
 __global__ void __launch_bounds__(MF_ME_THREADS, 1)
 mf_me_kernel(const MfParams P, double* __restrict__ rec, const unsigned int* __restrict__ count, int regions,
              unsigned long long cap) {
-  constexpr int N = MfProc<PROC>::N, NF = 4 * N + 3, T = MF_ME_THREADS;
+  constexpr int N = MfProc<PROC>::N, NF = 4 * N + 4, T = MF_ME_THREADS;
   extern __shared__ unsigned int s_pre[];                // [regions + 1] exclusive prefix, then s_part[T]
   unsigned int* s_part = s_pre + regions + 1;
   const unsigned tid = threadIdx.x;
@@ -365,13 +409,15 @@ template <int PROC>
 __global__ void __launch_bounds__(MF_THREADS)
 mf_hist_kernel(const MfParams P, const double* __restrict__ rec, const unsigned int* __restrict__ count, int regions,
                unsigned long long cap, double n_total, double* __restrict__ partial,
-               unsigned long long* __restrict__ pcount) {
-  constexpr int D = MfProc<PROC>::D, N = MfProc<PROC>::N, NF = 4 * N + 3, T = MF_THREADS;
+               unsigned long long* __restrict__ pcount, int row) {
+  constexpr int D = MfProc<PROC>::D, N = MfProc<PROC>::N, NF = 4 * N + 4, T = MF_THREADS;
   extern __shared__ double smem[];
   const int nb = P.nb, nh = D * nb, nw = T >> 5;
   double* s_hist = smem;                                 // [nw][D*nb]
   double* s_red = s_hist + nw * nh;                      // [nw][4]
+  double* s_obs = s_red + nw * 4;                        // [nw][MF_OBS_ACC] when observables are set
   for (int i = threadIdx.x; i < nw * nh; i += T) s_hist[i] = 0.0;
+  if (P.n_obs > 0) for (int i = threadIdx.x; i < nw * MF_OBS_ACC; i += T) s_obs[i] = 0.0;
   __syncthreads();
   const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
   const unsigned lt_mask = (1u << lane) - 1u;
@@ -392,6 +438,10 @@ mf_hist_kernel(const MfParams P, const double* __restrict__ rec, const unsigned 
       s1 += t; s2 += t2;
       const bool contrib = have && t2 != 0.0;
       mf_hist_add<D>(hw, nb, packed, contrib, t2, lt_mask);
+      if (P.n_obs > 0) {
+        const unsigned okeys = have ? (unsigned)__double_as_longlong(R[(size_t)(4 * N + 3) * cap + e]) : 0u;
+        mf_obs_add(s_obs + warp * MF_OBS_ACC, s_obs + warp * MF_OBS_ACC + MF_OBS_ACC / 2, P.n_obs, okeys, have && F != 0.0, t, t2, lt_mask);
+      }
     }
   }
 #pragma unroll
@@ -407,11 +457,16 @@ mf_hist_kernel(const MfParams P, const double* __restrict__ rec, const unsigned 
     s_red[warp * 4 + 3] = __longlong_as_double((long long)n_bad);
   }
   __syncthreads();
-  double* out = partial + (size_t)blockIdx.x * (2 + nh);
+  double* out = partial + (size_t)blockIdx.x * row;
   for (int e = tid; e < nh; e += T) {
     double s = 0.0;
     for (int w = 0; w < nw; ++w) s += s_hist[w * nh + e];
     out[2 + e] = s;
+  }
+  if (P.n_obs > 0) for (int e = tid; e < MF_OBS_ACC; e += T) {
+    double s = 0.0;
+    for (int w = 0; w < nw; ++w) s += s_obs[w * MF_OBS_ACC + e];
+    out[2 + nh + e] = s;
   }
   if (tid == 0) {
     double a = 0.0, b = 0.0; unsigned long long c = 0, d2 = 0;
@@ -487,7 +542,8 @@ static cudaError_t proc_setup(const MfParams& P, size_t* smem_iter, size_t* smem
     if (e) return e;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_iter, mf_iterate_compact_kernel<MF_PROC>, MF_THREADS, *smem_iter);
   } else {
-    e = cudaFuncSetAttribute(mf_iterate_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem_iter);
+    e = cudaFuncSetAttribute(mf_iterate_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)(*smem_iter + sizeof(double) * nw * MF_OBS_ACC));      // room for the observable histograms
     if (e) return e;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_iter, mf_iterate_kernel<MF_PROC>, MF_THREADS, *smem_iter);
   }
@@ -512,11 +568,15 @@ static cudaError_t proc_eval(const MfParams& P, const double* edges, const doubl
 
 static cudaError_t proc_iterate(const MfParams& P, const double* edges, const double* pdf, uint32_t iteration,
                                 unsigned long long first, unsigned long long n, double n_total, double* partial,
-                                unsigned long long* pcount, int grid, size_t smem, cudaStream_t st) {
+                                unsigned long long* pcount, int row, int grid, size_t smem, cudaStream_t st) {
+  if (P.n_obs > 0) {
+    if (kCompact) return cudaErrorNotSupported;          // observables of the heavy processes: staged path
+    smem += sizeof(double) * (MF_THREADS / 32) * MF_OBS_ACC;
+  }
   if constexpr (kCompact)
-    mf_iterate_compact_kernel<MF_PROC><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount);
+    mf_iterate_compact_kernel<MF_PROC><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount, row);
   else
-    mf_iterate_kernel<MF_PROC><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount);
+    mf_iterate_kernel<MF_PROC><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount, row);
   return cudaGetLastError();
 }
 
@@ -525,12 +585,14 @@ static cudaError_t proc_iterate(const MfParams& P, const double* edges, const do
 #define MF_STAGED 1                  // heavy processes (with cuts) iterate through the staged path
 #endif
 static constexpr bool kStaged = MF_STAGED && MfProc<MF_PROC>::NGL > 0;
-static constexpr int kRecFields = 4 * MfProc<MF_PROC>::N + 3;
+static constexpr int kRecFields = 4 * MfProc<MF_PROC>::N + 4;
 
 static size_t front_smem(const MfParams& P) {
   return sizeof(double) * ((size_t)P.d * (P.nb + 1) + (size_t)P.pdf_nx * P.pdf_nq) + sizeof(int) * (MF_THREADS / 32);
 }
-static size_t hist_smem(const MfParams& P) { return sizeof(double) * (MF_THREADS / 32) * ((size_t)P.d * P.nb + 4); }
+static size_t hist_smem(const MfParams& P) {
+  return sizeof(double) * (MF_THREADS / 32) * ((size_t)P.d * P.nb + 4 + (P.n_obs > 0 ? MF_OBS_ACC : 0));
+}
 
 static cudaError_t proc_staged_setup(const MfParams& P, int* rec_fields, int* occ_front, int* occ_hist) {
   *rec_fields = kStaged ? kRecFields : 0;
@@ -541,6 +603,9 @@ static cudaError_t proc_staged_setup(const MfParams& P, int* rec_fields, int* oc
   if (e) return e;
   e = cudaFuncSetAttribute(mf_me_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
   if (e) return e;
+  e = cudaFuncSetAttribute(mf_hist_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)(hist_smem(P) + sizeof(double) * (MF_THREADS / 32) * MF_OBS_ACC));
+  if (e) return e;
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_front, mf_front_kernel<MF_PROC>, MF_THREADS, front_smem(P));
   if (e) return e;
   return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_hist, mf_hist_kernel<MF_PROC>, MF_THREADS, hist_smem(P));
@@ -550,7 +615,7 @@ static cudaError_t proc_staged_setup(const MfParams& P, int* rec_fields, int* oc
 // ev (nullable): 4 events recorded at front start / |M|^2 start / |M|^2 end / reductions end
 static cudaError_t proc_staged(const MfParams& P, const double* edges, const double* pdf, uint32_t iteration,
                                unsigned long long first, unsigned long long n, double n_total, const MfStageWs& ws,
-                               double* partial, unsigned long long* pcount, int grid_me, int grid_hist,
+                               double* partial, unsigned long long* pcount, int row, int grid_me, int grid_hist,
                                cudaStream_t st, cudaEvent_t* ev) {
   if constexpr (!kStaged) return cudaErrorNotSupported;
   else {
@@ -563,7 +628,7 @@ static cudaError_t proc_staged(const MfParams& P, const double* edges, const dou
   mf_me_kernel<MF_PROC><<<grid_me, MF_ME_THREADS, sm, st>>>(P, ws.rec, ws.count, ws.regions, ws.cap);
   if ((e = cudaGetLastError())) return e;
   if (ev && (e = cudaEventRecord(ev[2], st))) return e;
-  mf_hist_kernel<MF_PROC><<<grid_hist, MF_THREADS, hist_smem(P), st>>>(P, ws.rec, ws.count, ws.regions, ws.cap, n_total, partial, pcount);
+  mf_hist_kernel<MF_PROC><<<grid_hist, MF_THREADS, hist_smem(P), st>>>(P, ws.rec, ws.count, ws.regions, ws.cap, n_total, partial, pcount, row);
   if ((e = cudaGetLastError())) return e;
   if (ev && (e = cudaEventRecord(ev[3], st))) return e;
   return cudaSuccess;

@@ -13,12 +13,12 @@ struct MfProcOps {
                       size_t smem, cudaStream_t st);
   cudaError_t (*iterate)(const MfParams& P, const double* edges, const double* pdf, uint32_t iteration,
                          unsigned long long first, unsigned long long n, double n_total, double* partial,
-                         unsigned long long* pcount, int grid, size_t smem, cudaStream_t st);
+                         unsigned long long* pcount, int row, int grid, size_t smem, cudaStream_t st);
   // staged path; rec_fields = 0 when the process iterates with the fused kernel only
   cudaError_t (*staged_setup)(const MfParams& P, int* rec_fields, int* occ_front, int* occ_hist);
   cudaError_t (*staged)(const MfParams& P, const double* edges, const double* pdf, uint32_t iteration,
                         unsigned long long first, unsigned long long n, double n_total, const MfStageWs& ws,
-                        double* partial, unsigned long long* pcount, int grid_me, int grid_hist, cudaStream_t st,
+                        double* partial, unsigned long long* pcount, int row, int grid_me, int grid_hist, cudaStream_t st,
                         cudaEvent_t* ev);
 };
 extern const MfProcOps mf_ops_0, mf_ops_1, mf_ops_2, mf_ops_3;

@@ -2,6 +2,9 @@
 // DFMA peak microbenchmark; included by mf_api.cu only.
 #pragma once
 #include "mf_kernels.cuh"
+#ifndef MF_OBS_ACC
+#define MF_OBS_ACC (2 * MF_OBS_MAX * MF_OBS_SLOTS)
+#endif
 
 // ---- fixed-order sum of per-block partials into the raw sums (adds: sharded accumulation) -----------
 // one warp per output element: lane l adds partials l, l+32, ... in order, then a xor-butterfly
@@ -9,11 +12,11 @@
 #define MF_REDUCE_THREADS 256
 __global__ void __launch_bounds__(MF_REDUCE_THREADS)
 mf_reduce_kernel(const double* __restrict__ partial, const unsigned long long* __restrict__ pcount,
-                 int nblocks, int na, double* __restrict__ acc, unsigned long long* __restrict__ counts) {
+                 int nblocks, int na, int row, double* __restrict__ acc, unsigned long long* __restrict__ counts) {
   const int e = blockIdx.x * (MF_REDUCE_THREADS / 32) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
   if (e < na) {
     double s = 0.0;
-    for (int b = lane; b < nblocks; b += 32) s += partial[(size_t)b * na + e];
+    for (int b = lane; b < nblocks; b += 32) s += partial[(size_t)b * row + e];   // rows of `row` doubles, the first na live
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
     if (lane == 0) acc[e] += s;
@@ -33,9 +36,14 @@ mf_reduce_kernel(const double* __restrict__ partial, const unsigned long long* _
 // taken serially by every lane from shared memory (fixed order).
 __global__ void mf_finalize_kernel(const MfParams P, double alpha, double n_total, unsigned long long n_events,
                                    const double* __restrict__ acc, const unsigned long long* __restrict__ counts,
-                                   double* __restrict__ edges, MfDevState* __restrict__ st) {
+                                   double* __restrict__ edges, MfDevState* __restrict__ st, double* __restrict__ obs_total) {
   __shared__ double s_r[MF_DMAX][MF_NBMAX], s_e[MF_DMAX][MF_NBMAX + 1];
   const int j = threadIdx.x >> 5, lane = threadIdx.x & 31, nb = P.nb;
+  if (P.n_obs > 0) {                                      // this iteration's observable histograms join the accumulated ones
+    const double* oa = acc + 2 + P.d * nb;
+    for (int i = threadIdx.x; i < MF_OBS_ACC; i += blockDim.x) obs_total[i] += oa[i];
+    if (threadIdx.x == 0) obs_total[MF_OBS_ACC] += 1.0;   // iterations summed
+  }
   if (threadIdx.x == 0) {
     const double I = acc[0], S2 = acc[1];
     double var = (n_total * S2 - I * I) / (n_total - 1.0);

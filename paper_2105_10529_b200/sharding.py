@@ -30,7 +30,7 @@ def sharded_iterate(h, n_total, rank, world, dist=None, device=None, stream=None
     """one iteration of n_total events split over `world` ranks; h has the C-ABI's method names
     (set_accum / vegas_accumulate / get_accum / vegas_finalize)"""
     first, n = shard_range(n_total, rank, world)
-    zeros = np.zeros(2 + h.d * h.n_bins)
+    zeros = np.zeros(h.accum_len() if hasattr(h, "accum_len") else 2 + h.d * h.n_bins)
     h.set_accum(zeros, np.zeros(2, np.uint64))
     h.vegas_accumulate(first, n, n_total, stream=stream)
     acc, counts = h.get_accum()

@@ -178,6 +178,41 @@ def test_staged_path_slices_large_iterations(mf):
     assert int((w != 0).sum()) <= cnt[0] <= n and g["n_events"] == n
 
 
+@pytest.mark.parametrize("proc,n", [(0, 60_000), (1, 30_000), (2, 20_000), (3, 1_500)])
+def test_observable_histograms_match_oracle(mf, mfo, proc, n):
+    """observable histograms filled in the same pass ("histogram accumulation"): two iterations
+    against the oracle's plain definition on the same grids; slots incl. under/overflow to 1e-10"""
+    cfg = W.config(proc, seed=W.CONFIGS[proc]["seed"])
+    gpu, orc = mf.Vegas(cfg), mfo.Vegas(cfg)
+    obs = [(0, 12, 0.0, 45.0), (2, 5, 99.0, 101.0)] if proc == 0 else \
+          [(0, 20, 0.0, 400.0), (1, 7, 10.0, 250.0), (2, 16, 350.0, 1500.0)] + ([(3, 10, 30.0, 230.0)] if proc >= 2 else [])
+    gpu.set_observables(obs)
+    assert gpu.accum_len() == 2 + gpu.d * gpu.n_bins + 2 * 4 * 64
+    ref = [(np.zeros(o[1] + 2), np.zeros(o[1] + 2)) for o in obs]
+    for it in range(2):
+        for (a, b), (r1, r2) in zip(orc.observable_hist(it, 0, n, n, obs, n_threads=mfo.max_threads()), ref):
+            r1 += a; r2 += b
+        g = gpu.vegas_iterate(n)
+        o = orc.iterate(n, n_threads=mfo.max_threads())
+        assert abs(g["integral"] / o["integral"] - 1) < RTOL_INT
+        gpu.set_grid(orc.get_grid())
+    got, n_it = gpu.get_observables()
+    assert n_it == 2
+    for (g1, g2), (r1, r2), ob in zip(got, ref, obs):
+        scale1, scale2 = np.abs(r1).max(), np.abs(r2).max()
+        np.testing.assert_allclose(g1, r1, rtol=1e-10, atol=1e-13 * scale1)
+        np.testing.assert_allclose(g2, r2, rtol=1e-10, atol=1e-13 * scale2)
+    tot = sum(it["integral"] for it in gpu.get_iterations())
+    assert abs(got[0][0].sum() / tot - 1) < 1e-12            # every weighted event lands in exactly one slot
+    gpu.set_observables([])                                   # off again: plain record length
+    assert gpu.accum_len() == 2 + gpu.d * gpu.n_bins
+    if proc >= 2:                                             # heavy processes: staged path only
+        gpu.set_observables(obs); gpu.set_path(False)
+        with pytest.raises(mf.MfError) as e:
+            gpu.vegas_iterate(1000)
+        assert e.value.code == mf.MF_EUNSUPPORTED
+
+
 def test_sharded_accumulate_equals_iterate(mf):
     """mf_vegas_accumulate over two event ranges + finalize == mf_vegas_iterate (to summation order)"""
     cfg = W.config(W.GG_TT, seed=5)

@@ -170,9 +170,10 @@ MF_HD double mf_mass_fraction_sq(int k, double r) {
 }
 
 // boost p from the rest frame of Q (mass M known analytically) to the frame in which Q is given
-MF_HD void mf_boost(const double Q[4], double M, const double p[4], double out[4]) {
-  const double Ep = (Q[0] * p[0] + Q[1] * p[1] + Q[2] * p[2] + Q[3] * p[3]) / M;
-  const double f = (p[0] + Ep) / (Q[0] + M);
+// (iM = 1/M and iQM = 1/(Q0 + M) are passed in: the two boosts of one decay step share them)
+MF_HD void mf_boost(const double Q[4], double iM, double iQM, const double p[4], double out[4]) {
+  const double Ep = (Q[0] * p[0] + Q[1] * p[1] + Q[2] * p[2] + Q[3] * p[3]) * iM;
+  const double f = (p[0] + Ep) * iQM;
   out[0] = Ep; out[1] = p[1] + Q[1] * f; out[2] = p[2] + Q[2] * f; out[3] = p[3] + Q[3] * f;
 }
 
@@ -208,8 +209,9 @@ MF_HD double mf_phase_space(double shat, double m, const double* rs, double k[N]
       for (int c = 0; c < 4; ++c) { k[0][c] = pr[c]; Q[c] = Qr[c]; }
     } else {
       double Qn[4];
-      mf_boost(Q, M[i - 1], pr, k[i - 2]);
-      mf_boost(Q, M[i - 1], Qr, Qn);
+      const double iM = 1.0 / M[i - 1], iQM = 1.0 / (Q[0] + M[i - 1]);
+      mf_boost(Q, iM, iQM, pr, k[i - 2]);
+      mf_boost(Q, iM, iQM, Qr, Qn);
 #pragma unroll
       for (int c = 0; c < 4; ++c) Q[c] = Qn[c];
     }
@@ -244,8 +246,14 @@ MF_HD double mf_phase_space(double shat, double m, const double* rs, double k[N]
 #pragma unroll
   for (int i = 0; i < N; ++i) {
     const double kabs = xi * k[i][0];
-    const double E = (i < 2) ? sqrt(m2 + kabs * kabs) : kabs;
-    prod *= kabs / E; den += kabs * kabs / E;
+    double E = kabs;
+    if (i < 2) {                                   // massive legs: 1/E from one rsqrt
+      const double s = fma(kabs, kabs, m2), ri = rsqrt(s);
+      E = s * ri;
+      prod *= kabs * ri; den = fma(kabs * kabs, ri, den);
+    } else {
+      den += kabs;                                 // massless: |k|/E = 1, |k|^2/E = |k|
+    }
     k[i][0] = E; k[i][1] *= xi; k[i][2] *= xi; k[i][3] *= xi;
   }
   double xp = xi;                                // xi^(2N-3)

@@ -92,13 +92,15 @@ MF_HD bool mf_event_front(const MfParams& P, const double* edges, const double* 
   const double wps = mf_phase_space<N>(shat, PROC == 0 ? 0.0 : P.m_top, y + (PROC == 0 ? 0 : 2), k);   // S4
   rts = sqrt(shat);
   const bool pass = mf_cuts<NGL>(P, (const double(*)[4])(&k[0][0] + 8), x1, x2);   // S5 (final gluons = k[2..])
-  double f1 = 1.0, f2 = 1.0, xf1 = 0.0, xf2 = 0.0;
+  double ff = 1.0, xf1 = 0.0, xf2 = 0.0;                                 // ff = f_g(x1) f_g(x2) / shat
   if (PROC != 0 && (REC || pass)) {                                      // S6
     xf1 = mf_pdf(P, pdf_tab, lx1, P.pdf_lq);
     xf2 = mf_pdf(P, pdf_tab, lx2, P.pdf_lq);
-    f1 = xf1 / x1; f2 = xf2 / x2;
+    ff = xf1 * xf2 / (x1 * x2 * shat);                                   // f_g = xf / x: one division for the three
+  } else {
+    ff = 1.0 / shat;
   }
-  pref = JV * jx * f1 * f2 * wps * P.wconst / shat;                      // S8 without |M|^2
+  pref = JV * jx * ff * wps * P.wconst;                                  // S8 without |M|^2
   if (okeys) *okeys = (P.n_obs > 0 && pass) ? mf_obs_keys<N>(P, (const double(*)[4])k) : 0u;
   if (REC) {
 #pragma unroll

@@ -226,6 +226,26 @@ def test_sharded_accumulate_equals_iterate(mf):
     np.testing.assert_allclose(a.get_grid(), b.get_grid(), rtol=0, atol=1e-13)
 
 
+def test_staged_path_edge_cases(mf, mfo):
+    """staged path: minimum iteration, fewer events than one CTA, no event passing the cuts (empty record
+    set: zero integral, grid kept), one passing event per region at most"""
+    cfg = W.config(W.GG_TTG, seed=9)
+    for n in (2, 3, 255, 257):
+        gpu, orc = mf.Vegas(cfg), mfo.Vegas(cfg)
+        g, o = gpu.vegas_iterate(n), orc.iterate(n)
+        assert g["n_pass"] == o["n_pass"] and g["n_events"] == n
+        assert (o["integral"] == 0 and g["integral"] == 0) or abs(g["integral"] / o["integral"] - 1) < RTOL_INT
+        np.testing.assert_allclose(gpu.get_grid(), orc.get_grid(), rtol=0, atol=1e-11)
+    none = dict(cfg); none["etamax_g"] = 1e-9            # |eta| < 1e-9: nothing passes
+    gpu = mf.Vegas(none)
+    before = gpu.get_grid()
+    g = gpu.vegas_iterate(5000)
+    assert g["n_pass"] == 0 and g["integral"] == 0.0 and g["sigma"] == 0.0 and g["n_nonfinite"] == 0
+    np.testing.assert_array_equal(gpu.get_grid(), before)
+    g = gpu.vegas_iterate(5000)                           # and again (workspace reuse with empty records)
+    assert g["n_pass"] == 0 and gpu.result()["n_iter"] == 2
+
+
 def test_errors_and_edge_cases(mf):
     cfg = W.config(W.GG_TT)
     gpu = mf.Vegas(cfg)

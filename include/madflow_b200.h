@@ -36,7 +36,9 @@ enum { MF_EE_MUMU = 0, MF_GG_TT = 1, MF_GG_TTG = 2, MF_GG_TTGG = 3 };
 typedef struct {
   uint32_t struct_size;      /* = sizeof(mf_config_t); ABI check                                     */
   int32_t  process;          /* MF_EE_MUMU .. MF_GG_TTGG                                             */
-  int32_t  precision;        /* 64 (fp64, the path) ; 32 -> MF_EUNSUPPORTED in this build            */
+  int32_t  precision;        /* 64 (fp64, the path); 32 = mixed precision, process MF_GG_TTG only: |M|^2
+                              * (S7) in fp32, everything else (S1-S6, S8-S10) in fp64; staged path and
+                              * mf_integrand_eval; other processes -> MF_EUNSUPPORTED                  */
   int32_t  device;           /* CUDA ordinal                                                         */
   uint64_t seed;             /* Philox key (reading A1)                                              */
   uint32_t n_bins;           /* VEGAS bins per dimension, 1..64 (configs: 50)                        */

@@ -43,6 +43,7 @@ struct mf_vegas {
   // staged path (heavy processes): records of the passing events go through HBM between the stages
   int rec_fields, occ_front, occ_hist; // rec_fields = 0: the process has the fused path only
   bool use_staged, have_stage;
+  bool f32;                            // cfg.precision == 32: |M|^2 stage in fp32 (staged path and eval only)
   MfStageWs ws;
   size_t ws_doubles, ws_regions;       // allocated sizes
   cudaEvent_t evs[4];                  // front start / |M|^2 start / |M|^2 end / reductions end
@@ -76,6 +77,7 @@ extern "C" int mf_vegas_create(const mf_config_t* cfg, mf_vegas_t** out) {
   MF_CREATE_CUDA(h->ops->staged_setup(P, &h->rec_fields, &h->occ_front, &h->occ_hist));
   if (h->rec_fields && (h->occ_front < 1 || h->occ_hist < 1)) { mf_vegas_destroy(h); return fail(MF_ECUDA, "staged kernel does not fit on an SM"); }
   h->use_staged = h->rec_fields > 0;
+  h->f32 = cfg->precision == 32;
   h->max_blocks = h->n_sm * 32;
   const size_t ne = (size_t)P.d * (P.nb + 1), npdf = (size_t)P.pdf_nx * P.pdf_nq;
   MF_CREATE_CUDA(cudaMalloc(&h->d_edges, ne * sizeof(double)));
@@ -156,7 +158,7 @@ extern "C" int mf_integrand_eval(mf_vegas_t* h, uint32_t iteration, uint64_t fir
   cudaStream_t st = (cudaStream_t)cuda_stream;
   MfEvalOutDev o = {out->weight, out->x, out->bins, out->momenta, out->me2, out->pdf, out->pass};
   const bool rec = out->x || out->momenta || out->me2 || out->pdf;
-  MF_CUDA(h->ops->eval(h->P, h->d_edges, h->d_pdf, iteration, first_event, n_events, o, rec,
+  MF_CUDA(h->ops->eval(h->P, h->d_edges, h->d_pdf, iteration, first_event, n_events, o, rec, h->f32,
                        grid_for(h, n_events, h->occ_eval), h->smem_eval, st));
   h->last_stream = st;
   return MF_OK;
@@ -165,6 +167,7 @@ extern "C" int mf_integrand_eval(mf_vegas_t* h, uint32_t iteration, uint64_t fir
 extern "C" int mf_set_path(mf_vegas_t* h, int32_t staged) {
   if (!h) return fail(MF_EINVAL, "handle is NULL");
   if (staged && !h->rec_fields) return fail(MF_EUNSUPPORTED, "this process has the fused path only");
+  if (!staged && h->f32) return fail(MF_EUNSUPPORTED, "the fp32 |M|^2 variant runs on the staged path only");
   h->use_staged = staged != 0;
   return MF_OK;
 }
@@ -210,7 +213,7 @@ extern "C" int mf_vegas_accumulate(mf_vegas_t* h, uint64_t first_event, uint64_t
       if (grid_hist > h->ws.regions) grid_hist = h->ws.regions;
       if (grid_hist > h->max_blocks) grid_hist = h->max_blocks;
       MF_CUDA(h->ops->staged(h->P, h->d_edges, h->d_pdf, h->iteration, first_event + done, m, (double)n_total, h->ws,
-                             h->d_partial, h->d_pcount, h->row, grid_me, grid_hist, st, h->evs));
+                             h->d_partial, h->d_pcount, h->row, grid_me, grid_hist, h->f32, st, h->evs));
       mf_reduce_kernel<<<(live_len(h) + 2 + 7) / 8, MF_REDUCE_THREADS, 0, st>>>(h->d_partial, h->d_pcount, grid_hist, live_len(h), h->row, h->d_acc, h->d_counts);
       MF_CUDA(cudaGetLastError());
     }

@@ -20,6 +20,7 @@
 #define MF_DEVFN static inline
 static inline void sincospi(double x, double* s, double* c) { *s = sin(M_PI * x); *c = cos(M_PI * x); }
 static inline double rsqrt(double x) { return 1.0 / sqrt(x); }
+static inline float rsqrt(float x) { return 1.0f / sqrtf(x); }
 #endif
 
 // Barrier points inside the generated helicity-loop bodies (one every 64 statements): with
@@ -51,7 +52,9 @@ static inline double rsqrt(double x) { return 1.0 / sqrt(x); }
 // opaque identity on a double: stops the compiler from hoisting what is computed from it out of the
 // helicity loop (the generator decides what is hoisted: gen/dag.py Dag.plan)
 #if defined(__CUDA_ARCH__)
-#define MF_LAUNDER(x) asm volatile("" : "+d"(x))
+__device__ __forceinline__ void mf_launder(double& x) { asm volatile("" : "+d"(x)); }
+__device__ __forceinline__ void mf_launder(float& x) { asm volatile("" : "+f"(x)); }
+#define MF_LAUNDER(x) mf_launder(x)
 #else
 #define MF_LAUNDER(x) do { } while (0)
 #endif
@@ -360,26 +363,28 @@ MF_HD unsigned mf_obs_keys(const MfParams& P, const double k[N][4]) {
 // ---- S7a: external-wavefunction ingredients (O6.2), the "conditional control statements" of
 // PAPER.md:69.  Fermion: w+ = sqrt(E+|p|), w- = m/w+, and N*(|p|+pz, px, py) of the two-spinors
 // chi+ = N(|p|+pz, px+i py), chi- = N(-px+i py, |p|+pz); the generated code builds u, v from them.
-MF_HD void mf_fermion_ing(const double p[4], double m, double o[5]) {
-  const double pt2 = p[1] * p[1] + p[2] * p[2];
-  const double pabs = sqrt(pt2 + p[3] * p[3]);
+template <typename T>
+MF_HD void mf_fermion_ing(const T p[4], T m, T o[5]) {
+  const T pt2 = p[1] * p[1] + p[2] * p[2];
+  const T pabs = sqrt(pt2 + p[3] * p[3]);
   o[0] = sqrt(p[0] + pabs);
-  o[1] = (m == 0.0) ? 0.0 : m / o[0];
-  if (pabs < 1e-12 * fabs(p[0]) || (pt2 == 0.0 && p[3] < 0.0)) {   // pz = -|p| branch
-    o[2] = 0.0; o[3] = 1.0; o[4] = 0.0;
+  o[1] = (m == T(0.0)) ? T(0.0) : m / o[0];
+  if (pabs < T(1e-12) * fabs(p[0]) || (pt2 == T(0.0) && p[3] < T(0.0))) {   // pz = -|p| branch
+    o[2] = T(0.0); o[3] = T(1.0); o[4] = T(0.0);
   } else {
-    const double ppz = (p[3] >= 0.0) ? pabs + p[3] : pt2 / (pabs - p[3]);   // no cancellation
-    const double N = rsqrt(2.0 * pabs * ppz);
+    const T ppz = (p[3] >= T(0.0)) ? pabs + p[3] : pt2 / (pabs - p[3]);   // no cancellation
+    const T N = rsqrt(T(2.0) * pabs * ppz);
     o[2] = N * ppz; o[3] = N * p[1]; o[4] = N * p[2];
   }
 }
 // Gluon: eps(k,lam) = (-lam eps1 - i eps2)/sqrt2; o = (eps1x, eps1y, eps1z, eps2x, eps2y)/sqrt2
-MF_HD void mf_gluon_ing(const double k[4], double o[5]) {
-  const double pt2 = k[1] * k[1] + k[2] * k[2];
-  const double r2 = 0.70710678118654752440;
-  if (pt2 == 0.0) { o[0] = r2; o[1] = 0.0; o[2] = 0.0; o[3] = 0.0; o[4] = (k[3] >= 0.0) ? r2 : -r2; return; }
-  const double pt = sqrt(pt2), kabs = sqrt(pt2 + k[3] * k[3]);
-  const double ipt = r2 / pt, ik = 1.0 / kabs;
+template <typename T>
+MF_HD void mf_gluon_ing(const T k[4], T o[5]) {
+  const T pt2 = k[1] * k[1] + k[2] * k[2];
+  const T r2 = T(0.70710678118654752440);
+  if (pt2 == T(0.0)) { o[0] = r2; o[1] = T(0.0); o[2] = T(0.0); o[3] = T(0.0); o[4] = (k[3] >= T(0.0)) ? r2 : -r2; return; }
+  const T pt = sqrt(pt2), kabs = sqrt(pt2 + k[3] * k[3]);
+  const T ipt = r2 / pt, ik = T(1.0) / kabs;
   o[0] = k[1] * k[3] * ipt * ik; o[1] = k[2] * k[3] * ipt * ik; o[2] = -pt * ik * r2;
   o[3] = -k[2] * ipt; o[4] = k[1] * ipt;
 }

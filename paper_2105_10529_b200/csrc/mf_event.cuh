@@ -32,46 +32,48 @@ struct MfEventRec {
 
 // inputs of the generated gg -> t t~ + gluons code: [E, mt, p3, p4, t-ingredients, t~-ingredients,
 // then for every final gluon: k, polarisation ingredients] (order fixed by gen/amplitudes.py)
-template <int N>
-MF_HD void mf_me_inputs_gg(double rts, double mt, const double k[N][4], double* in) {
-  in[0] = 0.5 * rts; in[1] = mt;
+template <int N, typename T>
+MF_HD void mf_me_inputs_gg(T rts, T mt, const T k[N][4], T* in) {
+  in[0] = T(0.5) * rts; in[1] = mt;
 #pragma unroll
   for (int c = 0; c < 4; ++c) { in[2 + c] = k[0][c]; in[6 + c] = k[1][c]; }
-  mf_fermion_ing(k[0], mt, in + 10);
-  mf_fermion_ing(k[1], mt, in + 15);
+  mf_fermion_ing<T>(k[0], mt, in + 10);
+  mf_fermion_ing<T>(k[1], mt, in + 15);
 #pragma unroll
   for (int g = 2; g < N; ++g) {
 #pragma unroll
     for (int c = 0; c < 4; ++c) in[20 + 9 * (g - 2) + c] = k[g][c];
-    mf_gluon_ing(k[g], in + 24 + 9 * (g - 2));
+    mf_gluon_ing<T>(k[g], in + 24 + 9 * (g - 2));
   }
 }
 
-template <int PROC>
-MF_HD double mf_me2(const MfParams& P, double rts, const double k[MfProc<PROC>::N][4]) {
+// |M|^2 (averaged/summed, before the symmetry factor) in the real type T: double, or float for the fp32
+// variant of the |M|^2 stage (A24: the front end and the reductions stay in fp64)
+template <int PROC, typename T = double>
+MF_HD T mf_me2(const MfParams& P, T rts, const T k[MfProc<PROC>::N][4]) {
   if (PROC == 0) {
     static_assert(MF_ME2_EE_MUMU_NIN == 20, "generator input layout changed");
-    double in[20];
-    const double E = 0.5 * rts;
-    const double pa[4] = {E, 0.0, 0.0, E}, pb[4] = {E, 0.0, 0.0, -E};
-    mf_fermion_ing(pa, 0.0, in); mf_fermion_ing(pb, 0.0, in + 5);
-    mf_fermion_ing(k[0], 0.0, in + 10); mf_fermion_ing(k[1], 0.0, in + 15);
-    return P.me_pref * mf_me2_ee_mumu(in) / (rts * rts * rts * rts);      // e^4/4 * sum |L.R|^2 / s^2
+    T in[20];
+    const T E = T(0.5) * rts;
+    const T pa[4] = {E, T(0.0), T(0.0), E}, pb[4] = {E, T(0.0), T(0.0), -E};
+    mf_fermion_ing<T>(pa, T(0.0), in); mf_fermion_ing<T>(pb, T(0.0), in + 5);
+    mf_fermion_ing<T>(k[0], T(0.0), in + 10); mf_fermion_ing<T>(k[1], T(0.0), in + 15);
+    return T(P.me_pref) * mf_me2_ee_mumu<T>(in) / (rts * rts * rts * rts);      // e^4/4 * sum |L.R|^2 / s^2
   } else if (PROC == 1) {
     static_assert(MF_ME2_GG_TT_NIN == 20, "generator input layout changed");
-    double in[20];
-    mf_me_inputs_gg<2>(rts, P.m_top, (const double(*)[4])k, in);
-    return P.me_pref * mf_me2_gg_tt(in);
+    T in[20];
+    mf_me_inputs_gg<2, T>(rts, T(P.m_top), (const T(*)[4])k, in);
+    return T(P.me_pref) * mf_me2_gg_tt<T>(in);
   } else if (PROC == 2) {
     static_assert(MF_ME2_GG_TTG_NIN == 29, "generator input layout changed");
-    double in[29];
-    mf_me_inputs_gg<3>(rts, P.m_top, (const double(*)[4])k, in);
-    return P.me_pref * mf_me2_gg_ttg(in);
+    T in[29];
+    mf_me_inputs_gg<3, T>(rts, T(P.m_top), (const T(*)[4])k, in);
+    return T(P.me_pref) * mf_me2_gg_ttg<T>(in);
   } else {
     static_assert(MF_ME2_GG_TTGG_NIN == 38, "generator input layout changed");
-    double in[38];
-    mf_me_inputs_gg<4>(rts, P.m_top, (const double(*)[4])k, in);
-    return P.me_pref * mf_me2_gg_ttgg(in);
+    T in[38];
+    mf_me_inputs_gg<4, T>(rts, T(P.m_top), (const T(*)[4])k, in);
+    return T(P.me_pref) * mf_me2_gg_ttgg<T>(in);
   }
 }
 
@@ -119,7 +121,7 @@ MF_HD bool mf_event_front(const MfParams& P, const double* edges, const double* 
 
 // One whole event: front end, then S7 and S8.  bin[] receives the VEGAS bins; rec (nullable) the
 // debug record.
-template <int PROC, bool REC>
+template <int PROC, bool REC, typename T = double>
 MF_HD double mf_event(const MfParams& P, const double* edges, const double* pdf_tab,
                       uint32_t iteration, uint64_t ev, int bin[MfProc<PROC>::D], bool& pass,
                       MfEventRec* rec, unsigned* okeys = nullptr) {
@@ -127,7 +129,14 @@ MF_HD double mf_event(const MfParams& P, const double* edges, const double* pdf_
   double k[N][4], rts, pref;
   pass = mf_event_front<PROC, REC>(P, edges, pdf_tab, iteration, ev, bin, k, rts, pref, rec, okeys);
   double me2 = 0.0;
-  if (MF_UNIFORM_ME || pass) me2 = mf_me2<PROC>(P, rts, k);              // S7
+  if (MF_UNIFORM_ME || pass) {                                           // S7 (in the real type T)
+    T kt[N][4];
+#pragma unroll
+    for (int i = 0; i < N; ++i)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) kt[i][c] = (T)k[i][c];
+    me2 = (double)mf_me2<PROC, T>(P, (T)rts, kt);
+  }
   if (!pass) me2 = 0.0;
   if (REC) rec->me2 = me2;
   return pass ? pref * me2 : 0.0;                                        // S8

@@ -20,7 +20,9 @@ static inline int mf_fill_params(const mf_config_t* c, MfParams* P, std::string&
   if (c->struct_size != sizeof(mf_config_t)) { err = "struct_size mismatch (ABI)"; return MF_EINVAL; }
   int d, nfin, ng;
   if (mf_process_shape(c->process, &d, &nfin, &ng)) { err = "unknown process"; return MF_EINVAL; }
-  if (c->precision != 64) { err = "only precision 64 is built"; return MF_EUNSUPPORTED; }
+  if (c->precision != 64 && !(c->precision == 32 && c->process == MF_GG_TTG)) {
+    err = "precision must be 64 (32: the fp32 |M|^2 variant exists for gg -> tt~g only)"; return MF_EUNSUPPORTED;
+  }
   if (c->n_bins < 1 || c->n_bins > MF_NBMAX) { err = "n_bins must be in 1..64"; return MF_EINVAL; }
   if (!(c->sqrt_s > 0.0)) { err = "sqrt_s must be positive"; return MF_EINVAL; }
   if (!(c->alpha_damp >= 0.0)) { err = "alpha_damp must be >= 0"; return MF_EINVAL; }

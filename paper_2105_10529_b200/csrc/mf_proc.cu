@@ -355,14 +355,18 @@ mf_front_kernel(const MfParams P, const double* __restrict__ g_edges, const doub
 #ifndef MF_ME_STAGGER
 #define MF_ME_STAGGER 14000          // cycles by which the second group of the |M|^2 CTA starts late (~half a chunk)
 #endif
+#ifndef MF_ME_THREADS_F32
+#define MF_ME_THREADS_F32 384        // CTA size of the fp32 variant (168 registers per thread; tuned, profiles/r1_tuning.md)
+#endif
 #ifndef MF_ME_THREADS
 #define MF_ME_THREADS 256            // CTA size of the |M|^2 stage (one CTA per SM; registers = 65536 / threads)
 #endif
-template <int PROC>
-__global__ void __launch_bounds__(MF_ME_THREADS, 1)
+// Real = double, or float: the fp32 variant of the |M|^2 stage (records, prefactor and F stay fp64)
+template <int PROC, typename Real, int THREADS>
+__global__ void __launch_bounds__(THREADS, 1)
 mf_me_kernel(const MfParams P, double* __restrict__ rec, const unsigned int* __restrict__ count, int regions,
              unsigned long long cap) {
-  constexpr int N = MfProc<PROC>::N, NF = 4 * N + 4, T = MF_ME_THREADS;
+  constexpr int N = MfProc<PROC>::N, NF = 4 * N + 4, T = THREADS;
   extern __shared__ unsigned int s_pre[];                // [regions + 1] exclusive prefix, then s_part[T]
   unsigned int* s_part = s_pre + regions + 1;
   const unsigned tid = threadIdx.x;
@@ -381,7 +385,8 @@ mf_me_kernel(const MfParams P, double* __restrict__ rec, const unsigned int* __r
   const unsigned M = s_pre[regions];
   // chunks of one GROUP (128 threads, own named barrier inside S7); group 1 starts MF_ME_STAGGER cycles
   // late so that the groups' per-event prologues (record load, ingredients, reciprocals) do not coincide
-  constexpr unsigned G = MfProc<PROC>::GROUP, NG = T / G;
+  constexpr unsigned G = MfProc<PROC>::GROUP < T ? MfProc<PROC>::GROUP : T, NG = T / G;
+  static_assert(T % G == 0, "the CTA of the |M|^2 stage must be whole groups");
   const unsigned group = tid / G, gtid = tid % G;
   const unsigned nchunks = (M + G - 1) / G;
 #if MF_ME_STAGGER > 0
@@ -394,13 +399,13 @@ mf_me_kernel(const MfParams P, double* __restrict__ rec, const unsigned int* __r
     int lo = 0, hi = regions;
     while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (s_pre[mid] <= l) lo = mid; else hi = mid; }
     double* R = rec + (size_t)lo * NF * cap + (l - s_pre[lo]);
-    double k[N][4];
+    Real k[N][4];
 #pragma unroll
     for (int p = 0; p < N; ++p)
 #pragma unroll
-      for (int c = 0; c < 4; ++c) k[p][c] = R[(size_t)(4 * p + c) * cap];
+      for (int c = 0; c < 4; ++c) k[p][c] = (Real)R[(size_t)(4 * p + c) * cap];
     const double rts = R[(size_t)(4 * N) * cap], pref = R[(size_t)(4 * N + 1) * cap];
-    const double F = pref * mf_me2<PROC>(P, rts, k);     // S7, S8
+    const double F = pref * (double)mf_me2<PROC, Real>(P, (Real)rts, k);     // S7, S8
     if (have) R[(size_t)(4 * N + 1) * cap] = F;
   }
 }
@@ -481,7 +486,7 @@ mf_hist_kernel(const MfParams P, const double* __restrict__ rec, const unsigned 
 }
 
 // ---- S1-S8 with per-event outputs -------------------------------------------------------------------
-template <int PROC, bool REC>
+template <int PROC, bool REC, typename T>
 __global__ void __launch_bounds__(MF_THREADS, MfLaunch<PROC>::MINB)
 mf_eval_kernel(const MfParams P, const double* __restrict__ g_edges, const double* __restrict__ g_pdf,
                uint32_t iteration, unsigned long long first, unsigned long long n, MfEvalOutDev o) {
@@ -498,7 +503,7 @@ mf_eval_kernel(const MfParams P, const double* __restrict__ g_edges, const doubl
     int bin[D];
     bool pass;
     MfEventRec rec;
-    double F = mf_event<PROC, REC>(P, s_edges, s_pdf, iteration, first + i, bin, pass, REC ? &rec : nullptr);
+    double F = mf_event<PROC, REC, T>(P, s_edges, s_pdf, iteration, first + i, bin, pass, REC ? &rec : nullptr);
     if (!isfinite(F)) F = 0.0;
     if (o.weight) o.weight[i] = F;
     if (o.bins) {
@@ -529,6 +534,7 @@ mf_eval_kernel(const MfParams P, const double* __restrict__ g_edges, const doubl
 #endif
 static constexpr bool kCompact = MF_COMPACT && MfProc<MF_PROC>::NGL > 0;
 static constexpr bool kEvalOne = MfProc<MF_PROC>::NGL > 0;
+static constexpr bool kF32 = MF_PROC == 2;   // fp32 variant of the |M|^2 stage: gg -> tt~g only (BASELINE configs[4])
 
 static cudaError_t proc_setup(const MfParams& P, size_t* smem_iter, size_t* smem_eval, int* occ_iter, int* occ_eval) {
   const size_t tables = (size_t)P.d * (P.nb + 1) + (size_t)P.pdf_nx * P.pdf_nq;
@@ -549,20 +555,32 @@ static cudaError_t proc_setup(const MfParams& P, size_t* smem_iter, size_t* smem
   }
   if (e) return e;
   if constexpr (!kEvalOne) {
-    e = cudaFuncSetAttribute(mf_eval_kernel<MF_PROC, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem_eval);
+    e = cudaFuncSetAttribute(mf_eval_kernel<MF_PROC, false, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem_eval);
     if (e) return e;
   }
-  e = cudaFuncSetAttribute(mf_eval_kernel<MF_PROC, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem_eval);
+  e = cudaFuncSetAttribute(mf_eval_kernel<MF_PROC, true, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem_eval);
   if (e) return e;
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_eval, mf_eval_kernel<MF_PROC, true>, MF_THREADS, *smem_eval);
+  if constexpr (kF32) {
+    e = cudaFuncSetAttribute(mf_eval_kernel<MF_PROC, true, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem_eval);
+    if (e) return e;
+  }
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_eval, mf_eval_kernel<MF_PROC, true, double>, MF_THREADS, *smem_eval);
 }
 static cudaError_t proc_eval(const MfParams& P, const double* edges, const double* pdf, uint32_t iteration,
                              unsigned long long first, unsigned long long n, const MfEvalOutDev& o, bool rec,
-                             int grid, size_t smem, cudaStream_t st) {
+                             bool f32, int grid, size_t smem, cudaStream_t st) {
+  if (f32) {
+    if constexpr (kF32) {
+      mf_eval_kernel<MF_PROC, true, float><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, o);
+      return cudaGetLastError();
+    } else {
+      return cudaErrorNotSupported;
+    }
+  }
   // heavy processes build one eval kernel only (the recording one: each output is written if requested)
-  if constexpr (kEvalOne) mf_eval_kernel<MF_PROC, true><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, o);
-  else if (rec) mf_eval_kernel<MF_PROC, true><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, o);
-  else mf_eval_kernel<MF_PROC, false><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, o);
+  if constexpr (kEvalOne) mf_eval_kernel<MF_PROC, true, double><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, o);
+  else if (rec) mf_eval_kernel<MF_PROC, true, double><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, o);
+  else mf_eval_kernel<MF_PROC, false, double><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, o);
   return cudaGetLastError();
 }
 
@@ -601,8 +619,12 @@ static cudaError_t proc_staged_setup(const MfParams& P, int* rec_fields, int* oc
   else {
   cudaError_t e = cudaFuncSetAttribute(mf_front_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)front_smem(P));
   if (e) return e;
-  e = cudaFuncSetAttribute(mf_me_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+  e = cudaFuncSetAttribute(mf_me_kernel<MF_PROC, double, MF_ME_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
   if (e) return e;
+  if constexpr (kF32) {
+    e = cudaFuncSetAttribute(mf_me_kernel<MF_PROC, float, MF_ME_THREADS_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    if (e) return e;
+  }
   e = cudaFuncSetAttribute(mf_hist_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                            (int)(hist_smem(P) + sizeof(double) * (MF_THREADS / 32) * MF_OBS_ACC));
   if (e) return e;
@@ -616,7 +638,7 @@ static cudaError_t proc_staged_setup(const MfParams& P, int* rec_fields, int* oc
 static cudaError_t proc_staged(const MfParams& P, const double* edges, const double* pdf, uint32_t iteration,
                                unsigned long long first, unsigned long long n, double n_total, const MfStageWs& ws,
                                double* partial, unsigned long long* pcount, int row, int grid_me, int grid_hist,
-                               cudaStream_t st, cudaEvent_t* ev) {
+                               bool f32, cudaStream_t st, cudaEvent_t* ev) {
   if constexpr (!kStaged) return cudaErrorNotSupported;
   else {
   cudaError_t e;
@@ -624,8 +646,13 @@ static cudaError_t proc_staged(const MfParams& P, const double* edges, const dou
   mf_front_kernel<MF_PROC><<<ws.regions, MF_THREADS, front_smem(P), st>>>(P, edges, pdf, iteration, first, n, ws.cap, ws.rec, ws.count);
   if ((e = cudaGetLastError())) return e;
   if (ev && (e = cudaEventRecord(ev[1], st))) return e;
-  const size_t sm = sizeof(unsigned int) * ((size_t)ws.regions + 1 + MF_ME_THREADS);
-  mf_me_kernel<MF_PROC><<<grid_me, MF_ME_THREADS, sm, st>>>(P, ws.rec, ws.count, ws.regions, ws.cap);
+  const size_t sm = sizeof(unsigned int) * ((size_t)ws.regions + 1 + (f32 ? MF_ME_THREADS_F32 : MF_ME_THREADS));
+  if (f32) {
+    if constexpr (kF32) mf_me_kernel<MF_PROC, float, MF_ME_THREADS_F32><<<grid_me, MF_ME_THREADS_F32, sm, st>>>(P, ws.rec, ws.count, ws.regions, ws.cap);
+    else return cudaErrorNotSupported;
+  } else {
+    mf_me_kernel<MF_PROC, double, MF_ME_THREADS><<<grid_me, MF_ME_THREADS, sm, st>>>(P, ws.rec, ws.count, ws.regions, ws.cap);
+  }
   if ((e = cudaGetLastError())) return e;
   if (ev && (e = cudaEventRecord(ev[2], st))) return e;
   mf_hist_kernel<MF_PROC><<<grid_hist, MF_THREADS, hist_smem(P), st>>>(P, ws.rec, ws.count, ws.regions, ws.cap, n_total, partial, pcount, row);

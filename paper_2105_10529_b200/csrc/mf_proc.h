@@ -9,8 +9,8 @@ struct MfStageWs { double* rec; unsigned int* count; unsigned long long cap; int
 struct MfProcOps {
   cudaError_t (*setup)(const MfParams& P, size_t* smem_iter, size_t* smem_eval, int* occ_iter, int* occ_eval);
   cudaError_t (*eval)(const MfParams& P, const double* edges, const double* pdf, uint32_t iteration,
-                      unsigned long long first, unsigned long long n, const MfEvalOutDev& o, bool rec, int grid,
-                      size_t smem, cudaStream_t st);
+                      unsigned long long first, unsigned long long n, const MfEvalOutDev& o, bool rec, bool f32,
+                      int grid, size_t smem, cudaStream_t st);
   cudaError_t (*iterate)(const MfParams& P, const double* edges, const double* pdf, uint32_t iteration,
                          unsigned long long first, unsigned long long n, double n_total, double* partial,
                          unsigned long long* pcount, int row, int grid, size_t smem, cudaStream_t st);
@@ -18,8 +18,8 @@ struct MfProcOps {
   cudaError_t (*staged_setup)(const MfParams& P, int* rec_fields, int* occ_front, int* occ_hist);
   cudaError_t (*staged)(const MfParams& P, const double* edges, const double* pdf, uint32_t iteration,
                         unsigned long long first, unsigned long long n, double n_total, const MfStageWs& ws,
-                        double* partial, unsigned long long* pcount, int row, int grid_me, int grid_hist, cudaStream_t st,
-                        cudaEvent_t* ev);
+                        double* partial, unsigned long long* pcount, int row, int grid_me, int grid_hist, bool f32,
+                        cudaStream_t st, cudaEvent_t* ev);
 };
 extern const MfProcOps mf_ops_0, mf_ops_1, mf_ops_2, mf_ops_3;
 static inline const MfProcOps* mf_proc_ops(int process) {

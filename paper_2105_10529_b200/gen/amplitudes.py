@@ -415,7 +415,8 @@ class GenEE:
 
 # ---- emission ---------------------------------------------------------------------------------------
 def emit_function(gen, fname):
-    """CUDA/C++ text of `double fname(const double* in)` plus the flop-count macros."""
+    """CUDA/C++ text of `template <typename T> T fname(const T* in)` (T = double, or float for the fp32
+    variant of the |M|^2 stage) plus the flop-count macros."""
     g, out = gen.g, gen.out
     sync = SYNC_MACRO.get(fname, "MF_SYNC_POINT")
     nh = len(gen.loop_assign)
@@ -441,9 +442,10 @@ def emit_function(gen, fname):
          "#define %s_NFMA %dull" % (U, tot["fma"]), "#define %s_NIN %d" % (U, len(gen.input_names)),
          "#define %s_SCALE %r" % (U, gen.scale)]
     L.append("enum { " + ", ".join("%s_IN_%s = %d" % (U, n.upper(), i) for i, n in enumerate(gen.input_names)) + " };")
-    L.append("MF_DEVFN double %s(const double* __restrict__ in) {" % fname)
+    L.append("template <typename T>")
+    L.append("MF_DEVFN T %s(const T* __restrict__ in) {" % fname)
     for i, n in enumerate(gen.input_names):
-        L.append("  const double %s = in[%d];" % (n, i))
+        L.append("  const T %s = in[%d];" % (n, i))
     leaf = lambda j: g.nodes[j][0] in ("in", "sym")
     pname = lambda j: g.names[j] if leaf(j) else "p%d" % j
     if not looped:
@@ -455,16 +457,16 @@ def emit_function(gen, fname):
         L.append("  return %s;" % _ref(g, out, pname))
     else:
         L += g.emit_list(pro_ids, pname, "p")
-        L.append("  double acc = 0.0;")
+        L.append("  T acc = T(0.0);")
         L.append("#pragma unroll 1")
         L.append("  for (int ih = 0; ih < %d; ++ih) {" % nh)
         for b, l in enumerate(reversed(gen.loop_legs)):
-            L.append("    const double lam%d = (ih & %d) ? 1.0 : -1.0;" % (l, 1 << b))
+            L.append("    const T lam%d = (ih & %d) ? T(1.0) : T(-1.0);" % (l, 1 << b))
         launder = getattr(gen, "max_hoist_cost", None) is not None
         used_inputs = sorted({o for i in body_ids for o in g._operands(i) if g.nodes[o][0] == "in"})
         if launder:       # opaque copies: keeps NVVM from hoisting the cheap invariants out again
             for j in used_inputs:
-                L.append("    double %s_l = %s; MF_LAUNDER(%s_l);" % (g.names[j], g.names[j], g.names[j]))
+                L.append("    T %s_l = %s; MF_LAUNDER(%s_l);" % (g.names[j], g.names[j], g.names[j]))
 
         def bname(j):
             if g.nodes[j][0] == "in":

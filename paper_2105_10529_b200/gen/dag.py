@@ -333,12 +333,12 @@ class Dag:
     def emit_list(self, ids, name, prefix, indent="  "):
         """C statements for the given nodes (ascending id = topological order); name(j) gives the C
         identifier of operand j"""
-        return ["%sconst double %s%d = %s;" % (indent, prefix, i, self._expr(i, name)) for i in ids]
+        return ["%sconst T %s%d = %s;" % (indent, prefix, i, self._expr(i, name)) for i in ids]
 
     # ---- emission ------------------------------------------------------------------------------
     @staticmethod
     def _k(v):
-        return repr(float(v))
+        return "T(%r)" % float(v)          # the emitted code is templated on the real type T
 
     def _expr(self, i, nm):
         op, a, b, c = self.nodes[i]
@@ -353,7 +353,7 @@ class Dag:
         if op == "addk":
             return "%s + %s" % (nm(a), self._k(b))
         if op == "rcp":
-            return "1.0 / %s" % nm(a)
+            return "T(1.0) / %s" % nm(a)
         if op in ("fma", "fms"):
             x, y = (self._k(a[1]), nm(a[2])) if a[0] == "k" else (nm(a[1]), nm(a[2]))
             return "fma(%s, %s, %s%s)" % (x, y, "-" if op == "fms" else "", nm(b))
@@ -367,7 +367,7 @@ class Dag:
         for i, (op, *_r) in enumerate(self.nodes):
             if not mark[i] or self.dep[i] != dep or op in ("in", "sym"):
                 continue
-            lines.append("%sconst double %s%d = %s;" % (indent, prefix, i, self._expr(i, nm)))
+            lines.append("%sconst T %s%d = %s;" % (indent, prefix, i, self._expr(i, nm)))
         return lines
 
     def ref(self, r, prefix="v"):

@@ -213,6 +213,36 @@ def test_observable_histograms_match_oracle(mf, mfo, proc, n):
         assert e.value.code == mf.MF_EUNSUPPORTED
 
 
+def test_fp32_matrix_element_variant(mf, mfo):
+    """precision = 32 (gg -> tt~g only): |M|^2 in fp32, everything else fp64, so the events, bins and cut
+    decisions are those of the fp64 path.  north_star: 1e-4 relative per event for the optional fp32 path;
+    gauge cancellations push a small fraction of the events beyond it -- the fraction is bounded here"""
+    cfg32 = W.config(W.GG_TTG, seed=1, precision=32)
+    gpu, orc = mf.Vegas(cfg32), mfo.Vegas(W.config(W.GG_TTG, seed=1))
+    n = 20_000
+    out = gpu.integrand_eval(0, 0, n, debug=True)
+    ref = orc.eval(0, 0, n, n_threads=mfo.max_threads())
+    assert (out["bins"].cpu().numpy() == ref["bins"]).all() and (out["pass_"].cpu().numpy() == ref["pass_"]).all()
+    np.testing.assert_allclose(out["momenta"].cpu().numpy(), ref["momenta"], rtol=1e-11, atol=1e-9)   # front end is fp64
+    w = out["weight"].cpu().numpy()
+    nz = ref["weight"] != 0
+    rel = np.abs(w[nz] / ref["weight"][nz] - 1)
+    assert (w[~nz] == 0).all()
+    assert np.median(rel) < 2e-6 and np.quantile(rel, 0.99) < 1e-4 and (rel > 1e-4).mean() < 2e-3 and rel.max() < 1e-2, \
+        (np.median(rel), np.quantile(rel, 0.99), (rel > 1e-4).mean(), rel.max())
+    g64 = mf.Vegas(W.config(W.GG_TTG, seed=1))
+    a, b = g64.vegas_iterate(200_000), gpu.vegas_iterate(200_000)
+    assert a["n_pass"] == b["n_pass"] and abs(b["integral"] / a["integral"] - 1) < 1e-6
+    np.testing.assert_allclose(gpu.get_grid(), g64.get_grid(), rtol=0, atol=5e-6)          # fp32 weights move the edges ~2e-7
+    with pytest.raises(mf.MfError) as e:
+        gpu.set_path(False)                                   # the fp32 variant exists on the staged path only
+    assert e.value.code == mf.MF_EUNSUPPORTED
+    for proc in (0, 1, 3):
+        with pytest.raises(mf.MfError) as e:
+            mf.Vegas(W.config(proc, precision=32))
+        assert e.value.code == mf.MF_EUNSUPPORTED
+
+
 def test_sharded_accumulate_equals_iterate(mf):
     """mf_vegas_accumulate over two event ranges + finalize == mf_vegas_iterate (to summation order)"""
     cfg = W.config(W.GG_TT, seed=5)

@@ -43,8 +43,11 @@ def test_argument_validation_and_no_cpu_path(binding):
     cfg, pdf = binding.make_config(W.config(W.GG_TTG))
     cfg.struct_size = 8
     assert lib.mf_vegas_create(C.byref(cfg), C.byref(h)) == binding.MF_EINVAL
-    cfg, pdf = binding.make_config(W.config(W.GG_TTG))
+    cfg, pdf = binding.make_config(W.config(W.GG_TT))  # the fp32 |M|^2 variant exists for gg -> tt~g only
     cfg.precision = 32
+    assert lib.mf_vegas_create(C.byref(cfg), C.byref(h)) == binding.MF_EUNSUPPORTED
+    cfg, pdf = binding.make_config(W.config(W.GG_TTG))
+    cfg.precision = 16
     assert lib.mf_vegas_create(C.byref(cfg), C.byref(h)) == binding.MF_EUNSUPPORTED
     if not torch.cuda.is_available():                  # no CPU fallback: a valid config fails loudly
         cfg, pdf = binding.make_config(W.config(W.GG_TTG))

@@ -353,7 +353,7 @@ mf_front_kernel(const MfParams P, const double* __restrict__ g_edges, const doub
 }
 
 #ifndef MF_ME_STAGGER
-#define MF_ME_STAGGER 14000          // cycles by which the second group of the |M|^2 CTA starts late (~half a chunk)
+#define MF_ME_STAGGER 0              // cycles by which group g of the |M|^2 CTA starts late (measured: no effect, the groups drift apart by themselves)
 #endif
 #ifndef MF_ME_THREADS_F32
 #define MF_ME_THREADS_F32 384        // CTA size of the fp32 variant (168 registers per thread; tuned, profiles/r1_tuning.md)
@@ -383,8 +383,8 @@ mf_me_kernel(const MfParams P, double* __restrict__ rec, const unsigned int* __r
     __syncthreads();
   }
   const unsigned M = s_pre[regions];
-  // chunks of one GROUP (128 threads, own named barrier inside S7); group 1 starts MF_ME_STAGGER cycles
-  // late so that the groups' per-event prologues (record load, ingredients, reciprocals) do not coincide
+  // chunks of one GROUP (128 threads, own named barrier inside S7): the groups run out of phase, so that one
+  // group's per-event prologue (record load, ingredients, reciprocals) overlaps the others' helicity loops
   constexpr unsigned G = MfProc<PROC>::GROUP < T ? MfProc<PROC>::GROUP : T, NG = T / G;
   static_assert(T % G == 0, "the CTA of the |M|^2 stage must be whole groups");
   const unsigned group = tid / G, gtid = tid % G;

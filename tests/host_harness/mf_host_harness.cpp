@@ -32,5 +32,18 @@ extern "C" double mfh_event(const MfParams* P, const double* edges, const double
   }
   return -1.0;
 }
+// gg -> tt~g with the |M|^2 stage in fp32 (the product's precision = 32 variant), same record layout
+extern "C" double mfh_event_ttg_f32(const MfParams* P, const double* edges, const double* pdf, uint32_t it,
+                                    uint64_t ev, int* bins, int* pass, double* rec_out) {
+  int bin[MfProc<2>::D]; bool ok; MfEventRec rec;
+  std::memset(&rec, 0, sizeof rec);
+  double F = mf_event<2, true, float>(*P, edges, pdf, it, ev, bin, ok, &rec);
+  for (int j = 0; j < MfProc<2>::D; ++j) bins[j] = bin[j];
+  *pass = ok;
+  std::memcpy(rec_out, rec.y, sizeof(double) * 10);
+  std::memcpy(rec_out + 10, rec.mom, sizeof(double) * 24);
+  rec_out[34] = rec.me2; rec_out[35] = rec.pdf[0]; rec_out[36] = rec.pdf[1];
+  return F;
+}
 extern "C" int mfh_params_size(void) { return (int)sizeof(MfParams); }
 extern "C" int mfh_fill_params(const mf_config_t* c, MfParams* P) { std::string e; return mf_fill_params(c, P, e); }

@@ -26,6 +26,8 @@ def harness():
     lib.mfh_event.restype = C.c_double
     lib.mfh_event.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.mfh_fill_params.argtypes = [C.POINTER(Config), C.c_void_p]
+    lib.mfh_event_ttg_f32.restype = C.c_double
+    lib.mfh_event_ttg_f32.argtypes = lib.mfh_event.argtypes
     return lib
 
 
@@ -64,3 +66,27 @@ def test_host_compiled_event_matches_oracle(mfo, harness, proc, n, tol):
         else:
             assert F == 0.0
     assert worst < tol, worst
+
+
+def test_host_compiled_fp32_matrix_element_variant(mfo, harness):
+    """the precision = 32 variant (|M|^2 in float, the rest in double) compiled for the host: same events,
+    bins and cut flags as the oracle; |M|^2 within float rounding times the gauge cancellations"""
+    cfg = W.config(W.GG_TTG, seed=7)
+    c, pdf = make_config(cfg)
+    P = C.create_string_buffer(harness.mfh_params_size())
+    assert harness.mfh_fill_params(C.byref(c), P) == 0
+    orc = mfo.Vegas(cfg)
+    edges = orc.get_grid()
+    n = 400
+    ref = orc.eval(0, 0, n)
+    bins = np.zeros(16, np.int32); ok = np.zeros(1, np.int32); rec = np.zeros(37)
+    rel = []
+    for i in range(n):
+        F = harness.mfh_event_ttg_f32(P, edges.ctypes.data, pdf.ctypes.data, 0, i, bins.ctypes.data, ok.ctypes.data, rec.ctypes.data)
+        assert list(bins[:orc.d]) == list(ref["bins"][i]) and ok[0] == ref["pass_"][i]
+        if ref["weight"][i] != 0:
+            rel.append(abs(F / ref["weight"][i] - 1))
+        else:
+            assert F == 0.0
+    rel = np.array(rel)
+    assert np.median(rel) < 2e-6 and (rel > 1e-4).mean() < 0.02 and rel.max() < 1e-2, (np.median(rel), rel.max())

@@ -207,8 +207,7 @@ extern "C" int mf_vegas_accumulate(mf_vegas_t* h, uint64_t first_event, uint64_t
       const uint64_t m = n_events - done < MF_STAGE_MAX_EVENTS ? n_events - done : MF_STAGE_MAX_EVENTS;
       int rc = ensure_ws(h, m);
       if (rc) return rc;
-      const int per_sm = h->blocks_per_sm ? (int)h->blocks_per_sm : h->occ_iter;
-      const int grid_me = h->n_sm * (per_sm > 0 ? 1 : 1);   // one persistent CTA per SM (launch bounds of mf_me_kernel)
+      const int grid_me = h->n_sm;                        // one persistent CTA per SM (launch bounds of mf_me_kernel)
       int grid_hist = h->n_sm * h->occ_hist;
       if (grid_hist > h->ws.regions) grid_hist = h->ws.regions;
       if (grid_hist > h->max_blocks) grid_hist = h->max_blocks;

@@ -1,15 +1,16 @@
-// mf_kernels.cuh -- the CUDA kernels of the path (sm_100a):
-//   mf_iterate_kernel  S1-S9 fused: one event per thread in registers, persistent grid (a multiple of
-//                      the 148 SMs), per-thread running sums, per-warp shared-memory histograms,
-//                      fixed-order block reduction -> one partial record per block (no atomics, so
-//                      the result is bit-reproducible for a fixed launch geometry; reading A22)
-//   mf_eval_kernel     S1-S8 with per-event outputs (the parity entry point mf_integrand_eval)
-//   mf_reduce_kernel   fixed-order sum of the per-block partials into the handle's raw sums
-//   mf_finalize_kernel S10: I, sigma, VEGAS grid refinement, iteration record (one block)
-//   mf_combine_kernel  O11: inverse-variance combination over iterations
-//   mf_dfma_kernel     register-resident DFMA chains: the measured fp64 roofline peak
-// These are FP64-pipe-bound straight-line kernels (no dense contraction): no tensor cores, no TMA;
-// the only staged data are the 2.9-4.1 KB of VEGAS edges and the 40 KB PDF table in shared memory.
+// mf_kernels.cuh -- launch shapes and the device-resident state shared by the CUDA kernels of the path
+// (sm_100a).  The kernels themselves:
+//   mf_proc.cu          mf_front_kernel / mf_me_kernel / mf_hist_kernel  staged S1-S6 / S7-S8 / S9 of the heavy
+//                       processes (each stage at its own occupancy, records of the passing events through HBM)
+//                       mf_iterate_kernel, mf_iterate_compact_kernel  S1-S9 fused: one event per thread in
+//                       registers, persistent grid, per-warp shared-memory histograms
+//                       mf_eval_kernel  S1-S8 with per-event outputs (the parity entry point mf_integrand_eval)
+//   mf_small_kernels.cuh  mf_reduce_kernel (fixed-order sum of the per-block partials), mf_finalize_kernel
+//                       (S10: I, sigma, grid refinement, iteration record), mf_combine_kernel (O11),
+//                       mf_dfma_kernel (register-resident DFMA chains: the measured fp64 roofline peak)
+// All reductions are fixed-order (no atomics): results are bit-reproducible for a fixed launch geometry
+// (reading A22).  These are FP64-pipe-bound straight-line kernels (no dense contraction): no tensor cores,
+// no TMA; the staged tables are the 2.9-4.1 KB of VEGAS edges and the 40 KB PDF table in shared memory.
 #pragma once
 #include <cuda_runtime.h>
 #include "mf_event.cuh"

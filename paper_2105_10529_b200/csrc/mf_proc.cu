@@ -1,5 +1,7 @@
-// mf_proc.cu -- the two per-process kernels (fused iteration, per-event evaluation), compiled once
-// per process with -DMF_PROC=0..3 so that the four |M|^2 codes build in parallel.
+// mf_proc.cu -- the per-process kernels, compiled once per process with -DMF_PROC=0..3 so that the four
+// |M|^2 codes build in parallel: the fused iteration (mf_iterate_kernel, mf_iterate_compact_kernel), the
+// staged iteration of the heavy processes (mf_front_kernel -> mf_me_kernel -> mf_hist_kernel), and the
+// per-event evaluation (mf_eval_kernel); plus their launchers (MfProcOps, mf_proc.h).
 #include "mf_kernels.cuh"
 #include "mf_proc.h"
 #ifndef MF_PROC
@@ -78,6 +80,48 @@ __device__ __forceinline__ void mf_obs_add(double* __restrict__ ho1, double* __r
 }
 #define MF_OBS_ACC (2 * MF_OBS_MAX * MF_OBS_SLOTS)         // doubles per record behind the 2 + d*nb VEGAS sums
 
+// fixed-order end of a reducing CTA: xor-butterfly inside the warp, warps in index order inside the block, one
+// partial record (2 + nh doubles, then the observable sums if s_obs != nullptr) and one counter pair per CTA
+__device__ __forceinline__ void mf_block_finish(double s1, double s2, unsigned long long n_pass, unsigned long long n_bad,
+                                                const double* __restrict__ s_hist, int nh, const double* __restrict__ s_obs,
+                                                double* __restrict__ s_red, double* __restrict__ out,
+                                                unsigned long long* __restrict__ pc) {
+  const int nw = blockDim.x >> 5, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+    s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+    n_pass += __shfl_xor_sync(0xffffffffu, n_pass, o);
+    n_bad += __shfl_xor_sync(0xffffffffu, n_bad, o);
+  }
+  if (lane == 0) {
+    s_red[warp * 4 + 0] = s1; s_red[warp * 4 + 1] = s2;
+    s_red[warp * 4 + 2] = __longlong_as_double((long long)n_pass);
+    s_red[warp * 4 + 3] = __longlong_as_double((long long)n_bad);
+  }
+  __syncthreads();
+  for (int e = threadIdx.x; e < nh; e += blockDim.x) {
+    double s = 0.0;
+    for (int w = 0; w < nw; ++w) s += s_hist[w * nh + e];
+    out[2 + e] = s;
+  }
+  if (s_obs) for (int e = threadIdx.x; e < MF_OBS_ACC; e += blockDim.x) {
+    double s = 0.0;
+    for (int w = 0; w < nw; ++w) s += s_obs[w * MF_OBS_ACC + e];
+    out[2 + nh + e] = s;
+  }
+  if (threadIdx.x == 0) {
+    double a = 0.0, b = 0.0; unsigned long long c = 0, d2 = 0;
+    for (int w = 0; w < nw; ++w) {
+      a += s_red[w * 4 + 0]; b += s_red[w * 4 + 1];
+      c += (unsigned long long)__double_as_longlong(s_red[w * 4 + 2]);
+      d2 += (unsigned long long)__double_as_longlong(s_red[w * 4 + 3]);
+    }
+    out[0] = a; out[1] = b;
+    pc[0] = c; pc[1] = d2;
+  }
+}
+
 // ---- S1-S9 fused ---------------------------------------------------------------------------------
 // partial: [gridDim.x][row] doubles (2 + d*nb sums, then the observable sums), pcount: [gridDim.x][2]
 // (n_pass, n_nonfinite)
@@ -132,40 +176,7 @@ mf_iterate_kernel(const MfParams P, const double* __restrict__ g_edges, const do
       mf_obs_add(s_obs + warp * MF_OBS_ACC, s_obs + warp * MF_OBS_ACC + MF_OBS_ACC / 2, P.n_obs, okeys, valid && F != 0.0, t, t2, lt_mask);
   }
   // fixed-order reductions: xor-butterfly inside the warp, warps in index order inside the block
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    s1 += __shfl_xor_sync(0xffffffffu, s1, o);
-    s2 += __shfl_xor_sync(0xffffffffu, s2, o);
-    n_pass += __shfl_xor_sync(0xffffffffu, n_pass, o);
-    n_bad += __shfl_xor_sync(0xffffffffu, n_bad, o);
-  }
-  if (lane == 0) {
-    s_red[warp * 4 + 0] = s1; s_red[warp * 4 + 1] = s2;
-    s_red[warp * 4 + 2] = __longlong_as_double((long long)n_pass);
-    s_red[warp * 4 + 3] = __longlong_as_double((long long)n_bad);
-  }
-  __syncthreads();
-  double* out = partial + (size_t)blockIdx.x * row;
-  for (int e = threadIdx.x; e < nh; e += blockDim.x) {
-    double s = 0.0;
-    for (int w = 0; w < nw; ++w) s += s_hist[w * nh + e];
-    out[2 + e] = s;
-  }
-  if (P.n_obs > 0) for (int e = threadIdx.x; e < MF_OBS_ACC; e += blockDim.x) {
-    double s = 0.0;
-    for (int w = 0; w < nw; ++w) s += s_obs[w * MF_OBS_ACC + e];
-    out[2 + nh + e] = s;
-  }
-  if (threadIdx.x == 0) {
-    double a = 0.0, b = 0.0; unsigned long long c = 0, d2 = 0;
-    for (int w = 0; w < nw; ++w) {
-      a += s_red[w * 4 + 0]; b += s_red[w * 4 + 1];
-      c += (unsigned long long)__double_as_longlong(s_red[w * 4 + 2]);
-      d2 += (unsigned long long)__double_as_longlong(s_red[w * 4 + 3]);
-    }
-    out[0] = a; out[1] = b;
-    pcount[2 * blockIdx.x] = c; pcount[2 * blockIdx.x + 1] = d2;
-  }
+  mf_block_finish(s1, s2, n_pass, n_bad, s_hist, nh, P.n_obs > 0 ? s_obs : nullptr, s_red, partial + (size_t)blockIdx.x * row, pcount + 2 * blockIdx.x);
 }
 
 // ---- S1-S9 fused, with CTA-level compaction of the events that pass the cuts -------------------------
@@ -253,35 +264,7 @@ mf_iterate_compact_kernel(const MfParams P, const double* __restrict__ g_edges, 
     qhead = (qhead + m) % CAP;
     qcount -= m;
   }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    s1 += __shfl_xor_sync(0xffffffffu, s1, o);
-    s2 += __shfl_xor_sync(0xffffffffu, s2, o);
-    n_pass += __shfl_xor_sync(0xffffffffu, n_pass, o);
-    n_bad += __shfl_xor_sync(0xffffffffu, n_bad, o);
-  }
-  if (lane == 0) {
-    s_red[warp * 4 + 0] = s1; s_red[warp * 4 + 1] = s2;
-    s_red[warp * 4 + 2] = __longlong_as_double((long long)n_pass);
-    s_red[warp * 4 + 3] = __longlong_as_double((long long)n_bad);
-  }
-  __syncthreads();
-  double* out = partial + (size_t)blockIdx.x * row;
-  for (int e = tid; e < nh; e += T) {
-    double s = 0.0;
-    for (int w = 0; w < nw; ++w) s += s_hist[w * nh + e];
-    out[2 + e] = s;
-  }
-  if (tid == 0) {
-    double a = 0.0, b = 0.0; unsigned long long c = 0, d2 = 0;
-    for (int w = 0; w < nw; ++w) {
-      a += s_red[w * 4 + 0]; b += s_red[w * 4 + 1];
-      c += (unsigned long long)__double_as_longlong(s_red[w * 4 + 2]);
-      d2 += (unsigned long long)__double_as_longlong(s_red[w * 4 + 3]);
-    }
-    out[0] = a; out[1] = b;
-    pcount[2 * blockIdx.x] = c; pcount[2 * blockIdx.x + 1] = d2;
-  }
+  mf_block_finish(s1, s2, n_pass, n_bad, s_hist, nh, nullptr, s_red, partial + (size_t)blockIdx.x * row, pcount + 2 * blockIdx.x);
 }
 
 // ---- staged iteration for the heavy processes: front end -> |M|^2 -> reductions, through HBM --------
@@ -449,40 +432,7 @@ mf_hist_kernel(const MfParams P, const double* __restrict__ rec, const unsigned 
       }
     }
   }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    s1 += __shfl_xor_sync(0xffffffffu, s1, o);
-    s2 += __shfl_xor_sync(0xffffffffu, s2, o);
-    n_pass += __shfl_xor_sync(0xffffffffu, n_pass, o);
-    n_bad += __shfl_xor_sync(0xffffffffu, n_bad, o);
-  }
-  if (lane == 0) {
-    s_red[warp * 4 + 0] = s1; s_red[warp * 4 + 1] = s2;
-    s_red[warp * 4 + 2] = __longlong_as_double((long long)n_pass);
-    s_red[warp * 4 + 3] = __longlong_as_double((long long)n_bad);
-  }
-  __syncthreads();
-  double* out = partial + (size_t)blockIdx.x * row;
-  for (int e = tid; e < nh; e += T) {
-    double s = 0.0;
-    for (int w = 0; w < nw; ++w) s += s_hist[w * nh + e];
-    out[2 + e] = s;
-  }
-  if (P.n_obs > 0) for (int e = tid; e < MF_OBS_ACC; e += T) {
-    double s = 0.0;
-    for (int w = 0; w < nw; ++w) s += s_obs[w * MF_OBS_ACC + e];
-    out[2 + nh + e] = s;
-  }
-  if (tid == 0) {
-    double a = 0.0, b = 0.0; unsigned long long c = 0, d2 = 0;
-    for (int w = 0; w < nw; ++w) {
-      a += s_red[w * 4 + 0]; b += s_red[w * 4 + 1];
-      c += (unsigned long long)__double_as_longlong(s_red[w * 4 + 2]);
-      d2 += (unsigned long long)__double_as_longlong(s_red[w * 4 + 3]);
-    }
-    out[0] = a; out[1] = b;
-    pcount[2 * blockIdx.x] = c; pcount[2 * blockIdx.x + 1] = d2;
-  }
+  mf_block_finish(s1, s2, n_pass, n_bad, s_hist, nh, P.n_obs > 0 ? s_obs : nullptr, s_red, partial + (size_t)blockIdx.x * row, pcount + 2 * blockIdx.x);
 }
 
 // ---- S1-S8 with per-event outputs -------------------------------------------------------------------

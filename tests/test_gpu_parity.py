@@ -243,6 +243,31 @@ def test_fp32_matrix_element_variant(mf, mfo):
         assert e.value.code == mf.MF_EUNSUPPORTED
 
 
+def test_config3_full_size_launch_and_config2_cross_section(mf, mfo):
+    """config 3 at its full size (1e6 events per iteration, staged path): raw sums == sums of the eval kernel's
+    weights, sampled events == oracle.  Config 2 at its full size (5 x 1e7): the cross section agrees with the
+    oracle-side determinations (VEGAS 1054.3 +- 6.6 pb, classic RAMBO 1047 +- 28 pb: tests/test_oracle_crosscheck.py)"""
+    cfg = W.config(W.GG_TTGG, seed=0)
+    n = W.CONFIGS[3]["n_events"]
+    gpu, orc = mf.Vegas(cfg), mfo.Vegas(cfg)
+    g = gpu.vegas_iterate(n)
+    acc, cnt = gpu.get_accum()
+    w = mf.Vegas(cfg).integrand_eval(0, 0, n)["weight"]
+    t = w / n
+    assert abs(float(t.sum()) / acc[0] - 1) < 1e-10 and abs(float((t * t).sum()) / acc[1] - 1) < 1e-10
+    assert int((w != 0).sum()) <= cnt[0] <= n and g["n_nonfinite"] == 0
+    for i in (0, 255, 256, 77_777, n - 1):
+        ref = orc.eval(0, i, 1)["weight"][0]
+        got = float(w[i])
+        assert (ref == 0 and got == 0) or abs(got / ref - 1) < RTOL_EVENT
+    c = W.CONFIGS[2]
+    gpu = mf.Vegas(W.config(W.GG_TTG, seed=c["seed"]))
+    for _ in range(c["n_iter"]):
+        gpu.vegas_iterate(c["n_events"])
+    r = gpu.result()
+    assert r["n_iter"] == c["n_iter"] and r["sigma"] < 0.5 and abs(r["integral"] - 1054.3) < 4 * 6.6 and r["chi2_dof"] < 5
+
+
 def test_sharded_accumulate_equals_iterate(mf):
     """mf_vegas_accumulate over two event ranges + finalize == mf_vegas_iterate (to summation order)"""
     cfg = W.config(W.GG_TT, seed=5)

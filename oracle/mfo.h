@@ -39,7 +39,13 @@ typedef struct {
   const double *pdf_xf;        /* host [nx][nq] row-major table of x*g(x,Q^2); must not be NULL  */
   uint32_t pdf_nx, pdf_nq;
   double   pdf_xmin, pdf_xmax, pdf_qmin, pdf_qmax;
+  uint32_t generator;          /* MFO_GEN_* flags; 0 = the generators of the configs   */
 } mfo_config_t;
+/* selectable generators (processes 1-3):
+ *  MFO_GEN_CLASSIC_RAMBO  textbook RAMBO (Kleiss, Stirling, Ellis 1986) with 4n uniforms instead of the 3n-4-random
+ *                         sequential form; VEGAS dimensions d = 2 + 4n (mfo_rambo_classic)
+ *  MFO_GEN_LINEAR_TAU     tau = tau0 + (1 - tau0) y0 instead of tau = tau0^(1-y0) (mfo_x_map_linear)     */
+enum { MFO_GEN_CLASSIC_RAMBO = 1, MFO_GEN_LINEAR_TAU = 2 };
 
 typedef struct {               /* host buffers owned by the caller; NULL = skip                  */
   double  *weight;             /* [n]  F_i = w_i f_i  (t_i * N)                                  */
@@ -107,6 +113,17 @@ void mfo_combine(const double *I, const double *sig, uint32_t n, mfo_result_t *o
 /* O3: y0,y1 -> x1,x2,shat,Jx */
 void mfo_x_map(double y0, double y1, double s, double shat_min, double *x1, double *x2,
                double *shat, double *jx);
+/* O3': linear-tau variant: tau = tau0 + (1 - tau0) y0, x1 = tau^y1, x2 = tau/x1, Jx = (1 - tau0)(-ln tau) */
+void mfo_x_map_linear(double y0, double y1, double s, double shat_min, double *x1, double *x2,
+                      double *shat, double *jx);
+/* O4': textbook RAMBO.  rs[4n] uniforms, particle i uses rs[4i..4i+3]: c = 2 r0 - 1, phi = 2 pi r1,
+ * q0 = -ln(r2 r3), q = q0 (1, s cos phi, s sin phi, c); Q = sum q, M = sqrt(Q^2), b = -Qvec/M, x = sqrt(shat)/M,
+ * gamma = Q0/M, a = 1/(1+gamma); p0_i = x (gamma q0 + b.q), pvec_i = x (qvec + b q0 + a (b.q) b).
+ * Output: massless momenta p0 [n][4] in the CM frame, flat in phase space: the weight is the constant mfo_w0.  */
+void mfo_rambo_classic(uint32_t n, double shat, const double *rs, double *p0);
+/* O4.4: RAMBO's massive rescaling of massless CM momenta p0 [n][4]: xi with sum sqrt(m^2 + xi^2 E^2) = sqrt(shat)
+ * (Newton, A7), k [n][4] massive momenta, out2 = {Wm, xi}; returns the Newton steps (step 4 of mfo_phase_space) */
+int mfo_massive_rescale(uint32_t n, double shat, const double *masses, const double *p0, double *k, double *out2);
 /* O4: n-body phase space from 3n-4 numbers. p0: massless momenta [n][4], k: massive [n][4],
  * Mint[n] intermediate masses (Mint[0]=sqrt(shat)), out3 = {W0, Wm, xi}; returns Newton steps */
 int mfo_phase_space(uint32_t n, double shat, const double *masses, const double *rs,

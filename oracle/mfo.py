@@ -29,7 +29,8 @@ class Config(C.Structure):
                 ("ptmin_g", C.c_double), ("etamax_g", C.c_double), ("drmin_gg", C.c_double),
                 ("gev2_to_pb", C.c_double), ("pdf_xf", C.POINTER(C.c_double)),
                 ("pdf_nx", C.c_uint32), ("pdf_nq", C.c_uint32), ("pdf_xmin", C.c_double),
-                ("pdf_xmax", C.c_double), ("pdf_qmin", C.c_double), ("pdf_qmax", C.c_double)]
+                ("pdf_xmax", C.c_double), ("pdf_qmin", C.c_double), ("pdf_qmax", C.c_double),
+                ("generator", C.c_uint32)]
 
 
 class EvalOut(C.Structure):
@@ -64,6 +65,9 @@ def lib():
         _lib.mfo_w0.restype = C.c_double
         _lib.mfo_w0.argtypes = [C.c_uint32, C.c_double]
         _lib.mfo_x_map.argtypes = [C.c_double] * 4 + [C.c_void_p] * 4
+        _lib.mfo_x_map_linear.argtypes = [C.c_double] * 4 + [C.c_void_p] * 4
+        _lib.mfo_rambo_classic.argtypes = [C.c_uint32, C.c_double, C.c_void_p, C.c_void_p]
+        _lib.mfo_massive_rescale.argtypes = [C.c_uint32, C.c_double] + [C.c_void_p] * 4
         _lib.mfo_phase_space.argtypes = [C.c_uint32, C.c_double] + [C.c_void_p] * 6
         _lib.mfo_me2.argtypes = [C.c_int, C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_void_p]
         _lib.mfo_me2_literal.argtypes = [C.c_int, C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_void_p]
@@ -131,6 +135,21 @@ def combine(I, sig):
 def x_map(y0, y1, s, shat_min):
     o = [C.c_double() for _ in range(4)]
     lib().mfo_x_map(y0, y1, s, shat_min, *[C.byref(v) for v in o]); return tuple(v.value for v in o)
+
+
+def x_map_linear(y0, y1, s, shat_min):
+    o = [C.c_double() for _ in range(4)]
+    lib().mfo_x_map_linear(y0, y1, s, shat_min, *[C.byref(v) for v in o]); return tuple(v.value for v in o)
+
+
+def rambo_classic(n, shat, rs):
+    rs = _f64(rs); p0 = np.zeros((n, 4)); lib().mfo_rambo_classic(n, shat, _p(rs), _p(p0)); return p0
+
+
+def massive_rescale(n, shat, masses, p0):
+    masses = _f64(masses); p0 = _f64(p0); k = np.zeros((n, 4)); o2 = np.zeros(2)
+    steps = lib().mfo_massive_rescale(n, shat, _p(masses), _p(p0), _p(k), _p(o2))
+    return dict(k=k, Wm=o2[0], xi=o2[1], steps=steps)
 
 
 def phase_space(n, shat, masses, rs):
@@ -214,6 +233,7 @@ class Vegas:
         for k in ("process", "seed", "n_bins", "alpha_damp", "sqrt_s", "m_top", "alpha_s", "alpha_em", "mu_f",
                   "ptmin_g", "etamax_g", "drmin_gg", "gev2_to_pb", "pdf_xmin", "pdf_xmax", "pdf_qmin", "pdf_qmax"):
             setattr(c, k, cfg[k])
+        c.generator = int(cfg.get("generator", 0))
         if self._pdf is not None:
             c.pdf_xf = self._pdf.ctypes.data_as(C.POINTER(C.c_double)); c.pdf_nx, c.pdf_nq = self._pdf.shape
         self._h = C.c_void_p()

@@ -146,6 +146,18 @@ extern "C" void mfo_x_map(double y0, double y1, double s, double shat_min, doubl
   *jx = tau * (-ltau0) * (-ltau);
 }
 
+// O3': tau linear in y0; x1 = tau^y1 as in O3, so dx1 dx2 = (1 - tau0)(-ln tau) dy0 dy1
+extern "C" void mfo_x_map_linear(double y0, double y1, double s, double shat_min, double *x1, double *x2,
+                                 double *shat, double *jx) {
+  double tau0 = shat_min / s;
+  double tau = tau0 + (1.0 - tau0) * y0;
+  double ltau = std::log(tau);
+  *x1 = std::exp(y1 * ltau);
+  *x2 = tau / *x1;
+  *shat = tau * s;
+  *jx = (1.0 - tau0) * (-ltau);
+}
+
 // ------------------------------------------------------------------------------------------------
 // O4  Phase space (reading A5: 3n-4-random sequential-decay RAMBO with the
 // standard RAMBO massive rescaling; A6 particle order = generation order; A7 Newton)
@@ -184,33 +196,10 @@ static void boost_from_rest(const double Q[4], double M, const double p[4], doub
   out[0] = Ep; out[1] = p[1] + Q[1] * f; out[2] = p[2] + Q[2] * f; out[3] = p[3] + Q[3] * f;
 }
 
-extern "C" int mfo_phase_space(uint32_t n, double shat, const double *masses, const double *rs,
-                               double *p0, double *kk, double *Mint, double *out3) {
+extern "C" int mfo_massive_rescale(uint32_t n, double shat, const double *masses, const double *p0, double *kk,
+                                   double *out2) {
   double rts = std::sqrt(shat);
-  std::vector<double> M(n + 1);
-  // 1. intermediate masses M_1 = sqrt(shat), M_n = 0, M_i = u_i M_{i-1} (i = 2..n-1), rs[i-2]
-  M[1] = rts; M[n] = 0.0;
-  for (uint32_t i = 2; i + 1 <= n; ++i) M[i] = solve_mass_fraction(n - i, rs[i - 2]) * M[i - 1];
-  for (uint32_t i = 1; i <= n; ++i) Mint[i - 1] = M[i];
-  // 2. sequential two-body decays Q_{i-1} -> p_{i-1} + Q_i, i = 2..n
-  double Q[4] = {rts, 0, 0, 0};
-  for (uint32_t i = 2; i <= n; ++i) {
-    double ct = 2.0 * rs[n - 6 + 2 * i] - 1.0;
-    double phi = 2.0 * M_PI * rs[n - 5 + 2 * i];
-    double st = std::sqrt(1.0 - ct * ct);
-    double q = (M[i - 1] * M[i - 1] - M[i] * M[i]) / (2.0 * M[i - 1]);
-    double p_rest[4] = {q, q * st * std::cos(phi), q * st * std::sin(phi), q * ct};
-    double Q_rest[4] = {std::sqrt(q * q + M[i] * M[i]), -p_rest[1], -p_rest[2], -p_rest[3]};
-    double p_cm[4], Q_cm[4];
-    if (i == 2) { std::memcpy(p_cm, p_rest, sizeof p_cm); std::memcpy(Q_cm, Q_rest, sizeof Q_cm); }
-    else { boost_from_rest(Q, M[i - 1], p_rest, p_cm); boost_from_rest(Q, M[i - 1], Q_rest, Q_cm); }
-    std::memcpy(p0 + 4 * (i - 2), p_cm, sizeof p_cm);
-    std::memcpy(Q, Q_cm, sizeof Q);
-  }
-  std::memcpy(p0 + 4 * (n - 1), Q, sizeof Q);
-  // 3. massless weight
-  double W0 = mfo_w0(n, shat);
-  // 4. massive rescaling: sum_i sqrt(m_i^2 + xi^2 E_i^2) = sqrt(shat), Newton from
+  // massive rescaling (O4.4): sum_i sqrt(m_i^2 + xi^2 E_i^2) = sqrt(shat), Newton from
   //    xi0 = sqrt(1 - (sum m / sqrt shat)^2), stop |dxi| <= 1e-14 xi, cap 50 (A7)
   double summ = 0; bool massless = true;
   for (uint32_t i = 0; i < n; ++i) { summ += masses[i]; if (masses[i] != 0.0) massless = false; }
@@ -238,7 +227,61 @@ extern "C" int mfo_phase_space(uint32_t n, double shat, const double *masses, co
     prod *= kabs / E; den += kabs * kabs / E;
   }
   double Wm = massless ? 1.0 : std::pow(xi, 2.0 * n - 3.0) * prod * rts / den;
-  out3[0] = W0; out3[1] = Wm; out3[2] = xi;
+  out2[0] = Wm; out2[1] = xi;
+  return steps;
+}
+
+// O4': textbook RAMBO (Kleiss, Stirling, Ellis 1986), the steps in the order of mfo.h
+extern "C" void mfo_rambo_classic(uint32_t n, double shat, const double *rs, double *p0) {
+  double rts = std::sqrt(shat);
+  std::vector<double> q(4 * (size_t)n);
+  double Q[4] = {0, 0, 0, 0};
+  for (uint32_t i = 0; i < n; ++i) {
+    double c = 2.0 * rs[4 * i] - 1.0, phi = 2.0 * M_PI * rs[4 * i + 1];
+    double q0 = -std::log(rs[4 * i + 2] * rs[4 * i + 3]);
+    double st = std::sqrt(1.0 - c * c);
+    q[4 * i] = q0; q[4 * i + 1] = q0 * st * std::cos(phi); q[4 * i + 2] = q0 * st * std::sin(phi); q[4 * i + 3] = q0 * c;
+    for (int m = 0; m < 4; ++m) Q[m] += q[4 * i + m];
+  }
+  double M = std::sqrt(Q[0] * Q[0] - Q[1] * Q[1] - Q[2] * Q[2] - Q[3] * Q[3]);
+  double b[3] = {-Q[1] / M, -Q[2] / M, -Q[3] / M};
+  double x = rts / M, gam = Q[0] / M, a = 1.0 / (1.0 + gam);
+  for (uint32_t i = 0; i < n; ++i) {
+    const double *qi = &q[4 * i];
+    double bq = b[0] * qi[1] + b[1] * qi[2] + b[2] * qi[3];
+    p0[4 * i] = x * (gam * qi[0] + bq);
+    for (int m = 0; m < 3; ++m) p0[4 * i + 1 + m] = x * (qi[1 + m] + b[m] * qi[0] + a * bq * b[m]);
+  }
+}
+
+extern "C" int mfo_phase_space(uint32_t n, double shat, const double *masses, const double *rs,
+                               double *p0, double *kk, double *Mint, double *out3) {
+  double rts = std::sqrt(shat);
+  std::vector<double> M(n + 1);
+  // 1. intermediate masses M_1 = sqrt(shat), M_n = 0, M_i = u_i M_{i-1} (i = 2..n-1), rs[i-2]
+  M[1] = rts; M[n] = 0.0;
+  for (uint32_t i = 2; i + 1 <= n; ++i) M[i] = solve_mass_fraction(n - i, rs[i - 2]) * M[i - 1];
+  for (uint32_t i = 1; i <= n; ++i) Mint[i - 1] = M[i];
+  // 2. sequential two-body decays Q_{i-1} -> p_{i-1} + Q_i, i = 2..n
+  double Q[4] = {rts, 0, 0, 0};
+  for (uint32_t i = 2; i <= n; ++i) {
+    double ct = 2.0 * rs[n - 6 + 2 * i] - 1.0;
+    double phi = 2.0 * M_PI * rs[n - 5 + 2 * i];
+    double st = std::sqrt(1.0 - ct * ct);
+    double q = (M[i - 1] * M[i - 1] - M[i] * M[i]) / (2.0 * M[i - 1]);
+    double p_rest[4] = {q, q * st * std::cos(phi), q * st * std::sin(phi), q * ct};
+    double Q_rest[4] = {std::sqrt(q * q + M[i] * M[i]), -p_rest[1], -p_rest[2], -p_rest[3]};
+    double p_cm[4], Q_cm[4];
+    if (i == 2) { std::memcpy(p_cm, p_rest, sizeof p_cm); std::memcpy(Q_cm, Q_rest, sizeof Q_cm); }
+    else { boost_from_rest(Q, M[i - 1], p_rest, p_cm); boost_from_rest(Q, M[i - 1], Q_rest, Q_cm); }
+    std::memcpy(p0 + 4 * (i - 2), p_cm, sizeof p_cm);
+    std::memcpy(Q, Q_cm, sizeof Q);
+  }
+  std::memcpy(p0 + 4 * (n - 1), Q, sizeof Q);
+  // 3. massless weight, 4. massive rescaling
+  double o2[2];
+  int steps = mfo_massive_rescale(n, shat, masses, p0, kk, o2);
+  out3[0] = mfo_w0(n, shat); out3[1] = o2[0]; out3[2] = o2[1];
   return steps;
 }
 

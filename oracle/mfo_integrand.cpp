@@ -38,6 +38,9 @@ extern "C" int mfo_vegas_create(const mfo_config_t *cfg, mfo_vegas_t **out) {
   static const uint32_t nfin[4] = {2, 2, 3, 4};
   h->n_final = nfin[cfg->process];
   h->d = (cfg->process == MFO_EE_MUMU) ? 2 : 2 + 3 * h->n_final - 4;
+  if (cfg->generator & ~(uint32_t)(MFO_GEN_CLASSIC_RAMBO | MFO_GEN_LINEAR_TAU)) { g_err = "unknown generator flag"; delete h; return MFO_EINVAL; }
+  if (cfg->generator && cfg->process == MFO_EE_MUMU) { g_err = "generator variants apply to processes 1-3"; delete h; return MFO_EINVAL; }
+  if (cfg->generator & MFO_GEN_CLASSIC_RAMBO) h->d = 2 + 4 * h->n_final;               // O4': 4n uniforms
   h->masses.assign(h->n_final, 0.0);
   h->sym = 1.0; h->shat_min = 0;
   if (cfg->process != MFO_EE_MUMU) {
@@ -67,17 +70,27 @@ extern "C" int mfo_set_grid(mfo_vegas_t *h, const double *e) {
 extern "C" int mfo_get_accum(mfo_vegas_t *h, double *acc) { if (!h || !acc) return MFO_EINVAL; std::memcpy(acc, h->acc.data(), h->acc.size() * sizeof(double)); return MFO_OK; }
 
 // One event, O1 -> O8.  Returns F = w f (the weight before the 1/N), fills the optional records.
-struct EventRec { double x[16]; uint8_t bins[16]; double mom[6 * 4]; double me2; double pdf[2]; int pass; };
+struct EventRec { double x[24]; uint8_t bins[24]; double mom[6 * 4]; double me2; double pdf[2]; int pass; };
 static double one_event(const mfo_vegas *h, uint32_t iteration, uint64_t ev, EventRec &R) {
   const mfo_config_t &c = h->cfg; const uint32_t d = h->d, nb = c.n_bins, n = h->n_final;
-  double u[16], JV;
+  double u[24], JV;
   mfo_uniforms(c.seed, iteration, ev, d, u);                              // O1
   mfo_vegas_map(h->edges.data(), d, nb, u, R.x, R.bins, &JV);             // O2
   double s = c.sqrt_s * c.sqrt_s, shat = s, x1 = 1, x2 = 1, Jx = 1;
   const double *rs = R.x;
-  if (c.process != MFO_EE_MUMU) { mfo_x_map(R.x[0], R.x[1], s, h->shat_min, &x1, &x2, &shat, &Jx); rs = R.x + 2; }   // O3
+  if (c.process != MFO_EE_MUMU) {                                         // O3 / O3'
+    if (c.generator & MFO_GEN_LINEAR_TAU) mfo_x_map_linear(R.x[0], R.x[1], s, h->shat_min, &x1, &x2, &shat, &Jx);
+    else mfo_x_map(R.x[0], R.x[1], s, h->shat_min, &x1, &x2, &shat, &Jx);
+    rs = R.x + 2;
+  }
   double p0[16], k[16], Mint[4], w3[3];
-  mfo_phase_space(n, shat, h->masses.data(), rs, p0, k, Mint, w3);        // O4
+  if (c.generator & MFO_GEN_CLASSIC_RAMBO) {                              // O4': textbook RAMBO, then O4.4
+    mfo_rambo_classic(n, shat, rs, p0);
+    w3[0] = mfo_w0(n, shat);
+    mfo_massive_rescale(n, shat, h->masses.data(), p0, k, w3 + 1);
+  } else {
+    mfo_phase_space(n, shat, h->masses.data(), rs, p0, k, Mint, w3);      // O4
+  }
   double rts = std::sqrt(shat);
   double *m = R.mom;                                                      // O4.5 incoming momenta
   m[0] = rts / 2; m[1] = 0; m[2] = 0; m[3] = rts / 2; m[4] = rts / 2; m[5] = 0; m[6] = 0; m[7] = -rts / 2;

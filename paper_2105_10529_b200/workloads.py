@@ -7,6 +7,8 @@ import numpy as np
 EE_MUMU, GG_TT, GG_TTG, GG_TTGG = 0, 1, 2, 3
 PROCESS_NAMES = {EE_MUMU: "ee_mumu", GG_TT: "gg_tt", GG_TTG: "gg_ttg", GG_TTGG: "gg_ttgg"}
 
+GEN_CLASSIC_RAMBO, GEN_LINEAR_TAU = 1, 2      # `generator` flags; 0 = the generators of the configs
+
 PDF_NX, PDF_NQ = 100, 50
 PDF_XMIN, PDF_XMAX, PDF_QMIN, PDF_QMAX = 1e-6, 1.0, 1.0, 1e4
 
@@ -34,7 +36,7 @@ def config(process, seed=0, **over):
              sqrt_s=13000.0, m_top=173.0, alpha_s=0.118, alpha_em=1.0 / 132.5, mu_f=173.0,
              ptmin_g=0.0, etamax_g=0.0, drmin_gg=0.0, gev2_to_pb=0.3894e9,
              pdf_xf=synthetic_gluon_grid(), pdf_xmin=PDF_XMIN, pdf_xmax=PDF_XMAX,
-             pdf_qmin=PDF_QMIN, pdf_qmax=PDF_QMAX)
+             pdf_qmin=PDF_QMIN, pdf_qmax=PDF_QMAX, generator=0)
     if process == EE_MUMU:
         c.update(sqrt_s=100.0, pdf_xf=None)
     if process in (GG_TTG, GG_TTGG):

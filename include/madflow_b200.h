@@ -33,6 +33,16 @@ enum { MF_OK = 0, MF_EINVAL = -1, MF_ENOMEM = -2, MF_ECUDA = -3, MF_ESTATE = -4,
 /* processes (BASELINE.json configs 0-3) */
 enum { MF_EE_MUMU = 0, MF_GG_TT = 1, MF_GG_TTG = 2, MF_GG_TTGG = 3 };
 
+/* Selectable generators (the paper fixes no phase-space algorithm):
+ *  MF_GEN_CLASSIC_RAMBO  textbook RAMBO (Kleiss, Stirling, Ellis 1986) from 4 n_final uniforms in place of the
+ *                        3 n_final - 4-random sequential form (reading O4), then the same massive rescaling;
+ *                        VEGAS dimensions d = 2 + 4 n_final (10, 14, 18).
+ *  MF_GEN_LINEAR_TAU     tau = tau0 + (1 - tau0) y0 in place of tau = tau0^(1-y0) (reading O3);
+ *                        J_x = (1 - tau0)(-ln tau).
+ * Both sample the same integral: the cross section agrees with the default generators' within errors.
+ * Processes 2 and 3 run them on the staged path only (mf_set_path(h, 0) -> MF_EUNSUPPORTED). */
+enum { MF_GEN_CLASSIC_RAMBO = 1, MF_GEN_LINEAR_TAU = 2 };
+
 typedef struct {
   uint32_t struct_size;      /* = sizeof(mf_config_t); ABI check                                     */
   int32_t  process;          /* MF_EE_MUMU .. MF_GG_TTGG                                             */
@@ -42,7 +52,7 @@ typedef struct {
   int32_t  device;           /* CUDA ordinal                                                         */
   uint64_t seed;             /* Philox key (reading A1)                                              */
   uint32_t n_bins;           /* VEGAS bins per dimension, 1..64 (configs: 50)                        */
-  uint32_t reserved0;
+  uint32_t generator;        /* MF_GEN_* flags, processes 1-3; 0 = the generators of the configs */
   double   alpha_damp;       /* VEGAS damping exponent (1.5)                                         */
   double   sqrt_s;           /* collider energy, GeV (config 0: the fixed e+e- energy)               */
   double   m_top, alpha_s, alpha_em, mu_f;
@@ -73,7 +83,8 @@ typedef struct { double integral, sigma, chi2_dof; uint32_t n_iter; } mf_result_
  * (precision != 64), MF_ECUDA (no device / allocation failure).                                    */
 int mf_vegas_create(const mf_config_t *cfg, mf_vegas_t **out);
 int mf_vegas_destroy(mf_vegas_t *h);
-/* d = VEGAS dimensions (2 for process 0, else 2 + 3 n_final - 4), n_final = final-state particles */
+/* d = VEGAS dimensions (2 for process 0, else 2 + 3 n_final - 4, or 2 + 4 n_final with MF_GEN_CLASSIC_RAMBO),
+ * n_final = final-state particles */
 int mf_ndim(const mf_vegas_t *h, uint32_t *d, uint32_t *n_final);
 
 /* S1-S8 for events [first_event, first_event + n_events) of iteration `iteration` on the CURRENT

@@ -27,7 +27,7 @@ class MfError(RuntimeError):
 
 class Config(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("process", C.c_int32), ("precision", C.c_int32),
-                ("device", C.c_int32), ("seed", C.c_uint64), ("n_bins", C.c_uint32), ("reserved0", C.c_uint32),
+                ("device", C.c_int32), ("seed", C.c_uint64), ("n_bins", C.c_uint32), ("generator", C.c_uint32),
                 ("alpha_damp", C.c_double), ("sqrt_s", C.c_double), ("m_top", C.c_double),
                 ("alpha_s", C.c_double), ("alpha_em", C.c_double), ("mu_f", C.c_double),
                 ("ptmin_g", C.c_double), ("etamax_g", C.c_double), ("drmin_gg", C.c_double),
@@ -58,6 +58,7 @@ def make_config(cfg: dict):
               "alpha_em", "mu_f", "ptmin_g", "etamax_g", "drmin_gg", "gev2_to_pb", "pdf_xmin", "pdf_xmax",
               "pdf_qmin", "pdf_qmax"):
         setattr(c, k, cfg[k])
+    c.generator = int(cfg.get("generator", 0))
     pdf = None
     if cfg.get("pdf_xf") is not None:
         pdf = np.ascontiguousarray(cfg["pdf_xf"], dtype=np.float64)

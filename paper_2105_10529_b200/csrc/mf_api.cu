@@ -168,6 +168,8 @@ extern "C" int mf_set_path(mf_vegas_t* h, int32_t staged) {
   if (!h) return fail(MF_EINVAL, "handle is NULL");
   if (staged && !h->rec_fields) return fail(MF_EUNSUPPORTED, "this process has the fused path only");
   if (!staged && h->f32) return fail(MF_EUNSUPPORTED, "the fp32 |M|^2 variant runs on the staged path only");
+  if (!staged && h->rec_fields && h->P.gen != 0)
+    return fail(MF_EUNSUPPORTED, "the selectable generators of processes 2 and 3 run on the staged path only");
   h->use_staged = staged != 0;
   return MF_OK;
 }
@@ -225,7 +227,7 @@ extern "C" int mf_vegas_accumulate(mf_vegas_t* h, uint64_t first_event, uint64_t
   {
     cudaError_t e_ = h->ops->iterate(h->P, h->d_edges, h->d_pdf, h->iteration, first_event, n_events, (double)n_total,
                                      h->d_partial, h->d_pcount, h->row, grid, h->smem_iter, st);
-    if (e_ == cudaErrorNotSupported) return fail(MF_EUNSUPPORTED, "observables of processes 2 and 3 need the staged path");
+    if (e_ == cudaErrorNotSupported) return fail(MF_EUNSUPPORTED, "observables and the selectable generators of processes 2 and 3 need the staged path");
     MF_CUDA(e_);
   }
   MF_CUDA(cudaEventRecord(h->evk1, st));

@@ -65,15 +65,19 @@ __device__ __forceinline__ void mf_launder(float& x) { asm volatile("" : "+f"(x)
 #ifndef MF_NEWTON_STEPS
 #define MF_NEWTON_STEPS 4   // massive-RAMBO Newton steps (reading A7)
 #endif
-#define MF_DMAX 10          // VEGAS dimensions of the largest process (gg -> tt~gg)
+#define MF_DMAX 18          // VEGAS dimensions of the largest process (gg -> tt~gg) with the classic 4n-random RAMBO
+#define MFD_GEN_CLASSIC 1   // generator flags (include/madflow_b200.h MF_GEN_*)
+#define MFD_GEN_LINEAR 2
 #define MF_NBMAX 64         // bins per dimension
 #define MF_PI 3.14159265358979323846
 
 // run constants of one handle (kernel parameter)
 struct MfParams {
   int32_t process, d, n_final, nb;
+  int32_t gen;                          // MF_GEN_* flags: selectable generators; 0 = the configs' generators
   uint32_t key0, key1;                  // Philox key = (seed lo, seed hi)        (A1)
   double s, ltau0, m_top;               // collider s, ln(shat_min / s)            (O3)
+  double tau0;                          // shat_min / s (linear-tau variant O3')
   double me_pref;                       // g_s^(2 ng) / 256 * generator scale, or e^4/4 (O6)
   double ptmin, etamax, drmin;          // cuts (O7)
   double tanh_etamax;                   // tanh(etamax): the eta cut is taken on tanh (mf_cuts)
@@ -155,6 +159,19 @@ MF_HD void mf_x_map(const MfParams& P, double y0, double y1, double& x1, double&
   jx = tau * P.ltau0 * ltau;            // tau (-ln tau0)(-ln tau)
 }
 
+// O3' (MF_GEN_LINEAR_TAU): tau = tau0 + (1 - tau0) y0, x1 = tau^y1 as in O3, so
+// dx1 dx2 = (1 - tau0)(-ln tau) dy0 dy1
+MF_HD void mf_x_map_linear(const MfParams& P, double y0, double y1, double& x1, double& x2, double& shat,
+                           double& jx, double& lx1, double& lx2) {
+  const double tau = fma(1.0 - P.tau0, y0, P.tau0);
+  const double ltau = log(tau);
+  lx1 = y1 * ltau; lx2 = ltau - lx1;
+  x1 = exp(lx1);
+  x2 = tau / x1;
+  shat = tau * P.s;
+  jx = (1.0 - P.tau0) * (-ltau);
+}
+
 // ---- S4: phase space (O4): 3n-4-random sequential-decay RAMBO + massive rescaling ---------------
 // mass fraction: solve r = (k+1) w^k - k w^(k+1) for w = u^2 in (0,1), k = n - i (closed form, then
 // two Newton steps on the polynomial so that the root does not depend on acos/cos rounding)
@@ -188,41 +205,10 @@ MF_HD double mf_w0(double shat) {
   return shat * shat / (24576.0 * MF_PI * MF_PI * MF_PI * MF_PI * MF_PI);
 }
 
-// rs[3N-4] -> massive momenta k[N][4] (t, t~, g...) in the partonic CM frame; returns W0 * Wm.
-// masses: m for particles 0,1 (0 for the massless 2-body case), 0 for the rest.
+// O4.4: RAMBO's massive rescaling of massless CM momenta k[N][4] (in place); masses m for particles 0,1, 0 for
+// the rest (m > 0).  Returns W_m.
 template <int N>
-MF_HD double mf_phase_space(double shat, double m, const double* rs, double k[N][4]) {
-  const double rts = sqrt(shat);
-  double M[N + 1];
-  M[1] = rts; M[N] = 0.0;
-#pragma unroll
-  for (int i = 2; i + 1 <= N; ++i) M[i] = sqrt(mf_mass_fraction_sq(N - i, rs[i - 2])) * M[i - 1];
-  double Q[4] = {rts, 0.0, 0.0, 0.0};
-#pragma unroll
-  for (int i = 2; i <= N; ++i) {
-    const double ct = 2.0 * rs[N - 6 + 2 * i] - 1.0;
-    double sp, cp;
-    sincospi(2.0 * rs[N - 5 + 2 * i], &sp, &cp);
-    const double st = sqrt(1.0 - ct * ct);
-    const double q = (M[i - 1] * M[i - 1] - M[i] * M[i]) / (2.0 * M[i - 1]);
-    const double pr[4] = {q, q * st * cp, q * st * sp, q * ct};
-    const double Qr[4] = {sqrt(q * q + M[i] * M[i]), -pr[1], -pr[2], -pr[3]};
-    if (i == 2) {
-#pragma unroll
-      for (int c = 0; c < 4; ++c) { k[0][c] = pr[c]; Q[c] = Qr[c]; }
-    } else {
-      double Qn[4];
-      const double iM = 1.0 / M[i - 1], iQM = 1.0 / (Q[0] + M[i - 1]);
-      mf_boost(Q, iM, iQM, pr, k[i - 2]);
-      mf_boost(Q, iM, iQM, Qr, Qn);
-#pragma unroll
-      for (int c = 0; c < 4; ++c) Q[c] = Qn[c];
-    }
-  }
-#pragma unroll
-  for (int c = 0; c < 4; ++c) k[N - 1][c] = Q[c];
-  const double W0 = mf_w0<N>(shat);
-  if (m == 0.0) return W0;
+MF_HD double mf_massive_rescale(double rts, double m, double k[N][4]) {
   // massive rescaling: sum_i sqrt(m_i^2 + xi^2 E_i^2) = sqrt(shat); Newton from
   // xi0 = sqrt(1 - (sum m / sqrt shat)^2), fixed MF_NEWTON_STEPS steps (A7: the iteration is converged
   // to rounding, 5e-15, after 4 steps for every one of 4e6 test events down to xi = 0.15, threshold
@@ -262,7 +248,81 @@ MF_HD double mf_phase_space(double shat, double m, const double* rs, double k[N]
   double xp = xi;                                // xi^(2N-3)
 #pragma unroll
   for (int i = 1; i < 2 * N - 3; ++i) xp *= xi;
-  return W0 * (xp * prod * rts / den);
+  return xp * prod * rts / den;
+}
+
+// rs[3N-4] -> massive momenta k[N][4] (t, t~, g...) in the partonic CM frame; returns W0 * Wm.
+// masses: m for particles 0,1 (0 for the massless 2-body case), 0 for the rest.
+template <int N>
+MF_HD double mf_phase_space(double shat, double m, const double* rs, double k[N][4]) {
+  const double rts = sqrt(shat);
+  double M[N + 1];
+  M[1] = rts; M[N] = 0.0;
+#pragma unroll
+  for (int i = 2; i + 1 <= N; ++i) M[i] = sqrt(mf_mass_fraction_sq(N - i, rs[i - 2])) * M[i - 1];
+  double Q[4] = {rts, 0.0, 0.0, 0.0};
+#pragma unroll
+  for (int i = 2; i <= N; ++i) {
+    const double ct = 2.0 * rs[N - 6 + 2 * i] - 1.0;
+    double sp, cp;
+    sincospi(2.0 * rs[N - 5 + 2 * i], &sp, &cp);
+    const double st = sqrt(1.0 - ct * ct);
+    const double q = (M[i - 1] * M[i - 1] - M[i] * M[i]) / (2.0 * M[i - 1]);
+    const double pr[4] = {q, q * st * cp, q * st * sp, q * ct};
+    const double Qr[4] = {sqrt(q * q + M[i] * M[i]), -pr[1], -pr[2], -pr[3]};
+    if (i == 2) {
+#pragma unroll
+      for (int c = 0; c < 4; ++c) { k[0][c] = pr[c]; Q[c] = Qr[c]; }
+    } else {
+      double Qn[4];
+      const double iM = 1.0 / M[i - 1], iQM = 1.0 / (Q[0] + M[i - 1]);
+      mf_boost(Q, iM, iQM, pr, k[i - 2]);
+      mf_boost(Q, iM, iQM, Qr, Qn);
+#pragma unroll
+      for (int c = 0; c < 4; ++c) Q[c] = Qn[c];
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < 4; ++c) k[N - 1][c] = Q[c];
+  const double W0 = mf_w0<N>(shat);
+  if (m == 0.0) return W0;
+  return W0 * mf_massive_rescale<N>(rts, m, k);
+}
+
+// O4' (MF_GEN_CLASSIC_RAMBO): textbook RAMBO (Kleiss, Stirling, Ellis 1986) from 4N uniforms,
+// particle i uses rs[4i..4i+3]: c = 2 r0 - 1, phi = 2 pi r1, q0 = -ln(r2 r3), q = q0 (1, s cos phi, s sin phi, c);
+// Q = sum q, M = sqrt(Q^2), b = -Qvec/M, x = sqrt(shat)/M, gamma = Q0/M, a = 1/(1+gamma);
+// p0_i = x (gamma q0 + b.q), pvec_i = x (qvec + b q0 + a (b.q) b): flat in phase space, constant weight W0.
+// Then the same massive rescaling.  Returns W0 * Wm.
+template <int N>
+MF_HD double mf_phase_space_classic(double shat, double m, const double* rs, double k[N][4]) {
+  const double rts = sqrt(shat);
+  double q[N][4], Q[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    const double c = 2.0 * rs[4 * i] - 1.0;
+    double sp, cp;
+    sincospi(2.0 * rs[4 * i + 1], &sp, &cp);
+    const double q0 = -log(rs[4 * i + 2] * rs[4 * i + 3]);
+    const double st = sqrt(1.0 - c * c);
+    q[i][0] = q0; q[i][1] = q0 * st * cp; q[i][2] = q0 * st * sp; q[i][3] = q0 * c;
+#pragma unroll
+    for (int c4 = 0; c4 < 4; ++c4) Q[c4] += q[i][c4];
+  }
+  const double M2 = Q[0] * Q[0] - Q[1] * Q[1] - Q[2] * Q[2] - Q[3] * Q[3];
+  const double iM = rsqrt(M2);
+  const double b[3] = {-Q[1] * iM, -Q[2] * iM, -Q[3] * iM};
+  const double x = rts * iM, gam = Q[0] * iM, a = 1.0 / (1.0 + gam);
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    const double bq = b[0] * q[i][1] + b[1] * q[i][2] + b[2] * q[i][3];
+    k[i][0] = x * (gam * q[i][0] + bq);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) k[i][1 + c] = x * (q[i][1 + c] + b[c] * q[i][0] + a * bq * b[c]);
+  }
+  const double W0 = mf_w0<N>(shat);
+  if (m == 0.0) return W0;
+  return W0 * mf_massive_rescale<N>(rts, m, k);
 }
 
 // ---- S6: PDF (O5): cubic Hermite in (ln x, ln Q^2) on the tabulated xf, node slope = mean of the

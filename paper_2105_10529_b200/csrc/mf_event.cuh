@@ -21,6 +21,22 @@ template <> struct MfProc<0> { static const int D = 2, N = 2, NGL = 0, GROUP = 1
 template <> struct MfProc<1> { static const int D = 4, N = 2, NGL = 0, GROUP = 128; };
 template <> struct MfProc<2> { static const int D = 7, N = 3, NGL = 1, GROUP = 128; };
 template <> struct MfProc<3> { static const int D = 10, N = 4, NGL = 2, GROUP = 256; };
+// Generator selection of the front end, template parameter CL:
+//   0  the generators of the configs, nothing selectable (the path bench.py times: no branch)
+//   1  classic 4n-random RAMBO, d = 2 + 4n; the tau map (O3 or O3') is a run-time, grid-uniform branch on P.gen
+//   2  sequential RAMBO of the configs with the run-time branch on the tau map
+template <int PROC, int CL> struct MfDim { static const int D = CL == 1 ? 2 + 4 * MfProc<PROC>::N : MfProc<PROC>::D; };
+// bins are packed 6 bits each, 10 per 64-bit word: the second word holds dimensions 10.. of the classic generator
+#define MF_PACK_DIMS 10
+template <int D>
+MF_HD void mf_pack_bins(const int bin[D], unsigned long long& lo, unsigned long long& hi) {
+  lo = 0; hi = 0;
+#pragma unroll
+  for (int j = 0; j < D; ++j) {
+    if (j < MF_PACK_DIMS) lo |= (unsigned long long)bin[j] << (6 * j);
+    else hi |= (unsigned long long)bin[j] << (6 * (j - MF_PACK_DIMS));
+  }
+}
 
 // optional per-event record (mf_integrand_eval's debug outputs)
 struct MfEventRec {
@@ -81,17 +97,22 @@ MF_HD T mf_me2(const MfParams& P, T rts, const T k[MfProc<PROC>::N][4]) {
 //   config 0   : pref = J_V (1/(8 pi)) K / (2 s)
 //   configs 1-3: pref = J_V J_x f_g(x1) f_g(x2) S_f W_0 W_m K / (2 shat)
 // edges: [d][nb+1], pdf_tab: [nx][nq] (both in shared memory on the device).  Returns the cut flag.
-template <int PROC, bool REC>
+template <int PROC, bool REC, int CL = 0>
 MF_HD bool mf_event_front(const MfParams& P, const double* edges, const double* pdf_tab, uint32_t iteration,
-                          uint64_t ev, int bin[MfProc<PROC>::D], double k[MfProc<PROC>::N][4], double& rts,
+                          uint64_t ev, int bin[MfDim<PROC, CL>::D], double k[MfProc<PROC>::N][4], double& rts,
                           double& pref, MfEventRec* rec, unsigned* okeys = nullptr) {
-  constexpr int D = MfProc<PROC>::D, N = MfProc<PROC>::N, NGL = MfProc<PROC>::NGL;
+  constexpr int D = MfDim<PROC, CL>::D, N = MfProc<PROC>::N, NGL = MfProc<PROC>::NGL;
+  static_assert(PROC != 0 || CL == 0, "generator variants apply to processes 1-3");
   double u[D], y[D];
   mf_uniforms<D>(P, iteration, ev, u);                                   // S1
   const double JV = mf_vegas_map<D>(edges, P.nb, u, y, bin);             // S2
   double x1 = 1.0, x2 = 1.0, shat = P.s, jx = 1.0, lx1 = 0.0, lx2 = 0.0;
-  if (PROC != 0) mf_x_map(P, y[0], y[1], x1, x2, shat, jx, lx1, lx2);    // S3
-  const double wps = mf_phase_space<N>(shat, PROC == 0 ? 0.0 : P.m_top, y + (PROC == 0 ? 0 : 2), k);   // S4
+  if (PROC != 0) {                                                       // S3 / S3'
+    if (CL != 0 && (P.gen & MFD_GEN_LINEAR)) mf_x_map_linear(P, y[0], y[1], x1, x2, shat, jx, lx1, lx2);
+    else mf_x_map(P, y[0], y[1], x1, x2, shat, jx, lx1, lx2);
+  }
+  const double wps = CL == 1 ? mf_phase_space_classic<N>(shat, P.m_top, y + 2, k)                            // S4'
+                        : mf_phase_space<N>(shat, PROC == 0 ? 0.0 : P.m_top, y + (PROC == 0 ? 0 : 2), k);   // S4
   rts = sqrt(shat);
   const bool pass = mf_cuts<NGL>(P, (const double(*)[4])(&k[0][0] + 8), x1, x2);   // S5 (final gluons = k[2..])
   double ff = 1.0, xf1 = 0.0, xf2 = 0.0;                                 // ff = f_g(x1) f_g(x2) / shat
@@ -121,13 +142,13 @@ MF_HD bool mf_event_front(const MfParams& P, const double* edges, const double* 
 
 // One whole event: front end, then S7 and S8.  bin[] receives the VEGAS bins; rec (nullable) the
 // debug record.
-template <int PROC, bool REC, typename T = double>
+template <int PROC, bool REC, typename T = double, int CL = 0>
 MF_HD double mf_event(const MfParams& P, const double* edges, const double* pdf_tab,
-                      uint32_t iteration, uint64_t ev, int bin[MfProc<PROC>::D], bool& pass,
+                      uint32_t iteration, uint64_t ev, int bin[MfDim<PROC, CL>::D], bool& pass,
                       MfEventRec* rec, unsigned* okeys = nullptr) {
   constexpr int N = MfProc<PROC>::N;
   double k[N][4], rts, pref;
-  pass = mf_event_front<PROC, REC>(P, edges, pdf_tab, iteration, ev, bin, k, rts, pref, rec, okeys);
+  pass = mf_event_front<PROC, REC, CL>(P, edges, pdf_tab, iteration, ev, bin, k, rts, pref, rec, okeys);
   double me2 = 0.0;
   if (MF_UNIFORM_ME || pass) {                                           // S7 (in the real type T)
     T kt[N][4];

@@ -5,11 +5,14 @@
 #include "mf_event.cuh"
 #include <string>
 
-static inline int mf_process_shape(int process, int* d, int* n_final, int* ng) {
+static_assert(MFD_GEN_CLASSIC == MF_GEN_CLASSIC_RAMBO && MFD_GEN_LINEAR == MF_GEN_LINEAR_TAU, "device flags follow the header");
+
+static inline int mf_process_shape(int process, uint32_t generator, int* d, int* n_final, int* ng) {
   static const int nf[4] = {2, 2, 3, 4};
   if (process < 0 || process > 3) return -1;
   *n_final = nf[process];
   *d = (process == MF_EE_MUMU) ? 2 : 2 + 3 * nf[process] - 4;
+  if (generator & MF_GEN_CLASSIC_RAMBO) *d = 2 + 4 * nf[process];       // O4': 4n uniforms
   *ng = (process == MF_EE_MUMU) ? 0 : nf[process];      // gluon legs of gg -> t t~ + (n_final-2) g
   return 0;
 }
@@ -19,7 +22,9 @@ static inline int mf_fill_params(const mf_config_t* c, MfParams* P, std::string&
   if (!c) { err = "cfg is NULL"; return MF_EINVAL; }
   if (c->struct_size != sizeof(mf_config_t)) { err = "struct_size mismatch (ABI)"; return MF_EINVAL; }
   int d, nfin, ng;
-  if (mf_process_shape(c->process, &d, &nfin, &ng)) { err = "unknown process"; return MF_EINVAL; }
+  if (c->generator & ~(uint32_t)(MF_GEN_CLASSIC_RAMBO | MF_GEN_LINEAR_TAU)) { err = "unknown generator flag"; return MF_EINVAL; }
+  if (mf_process_shape(c->process, c->generator, &d, &nfin, &ng)) { err = "unknown process"; return MF_EINVAL; }
+  if (c->generator && c->process == MF_EE_MUMU) { err = "generator variants apply to processes 1-3"; return MF_EINVAL; }
   if (c->precision != 64 && !(c->precision == 32 && c->process == MF_GG_TTG)) {
     err = "precision must be 64 (32: the fp32 |M|^2 variant exists for gg -> tt~g only)"; return MF_EUNSUPPORTED;
   }
@@ -28,7 +33,7 @@ static inline int mf_fill_params(const mf_config_t* c, MfParams* P, std::string&
   if (!(c->alpha_damp >= 0.0)) { err = "alpha_damp must be >= 0"; return MF_EINVAL; }
   if (!(c->gev2_to_pb > 0.0)) { err = "gev2_to_pb must be positive"; return MF_EINVAL; }
   MfParams p = {};
-  p.process = c->process; p.d = d; p.n_final = nfin; p.nb = (int)c->n_bins;
+  p.process = c->process; p.d = d; p.n_final = nfin; p.nb = (int)c->n_bins; p.gen = (int32_t)c->generator;
   p.key0 = (uint32_t)c->seed; p.key1 = (uint32_t)(c->seed >> 32);
   p.s = c->sqrt_s * c->sqrt_s; p.m_top = c->m_top;
   p.ptmin = c->ptmin_g; p.etamax = c->etamax_g; p.drmin = c->drmin_gg;
@@ -51,7 +56,7 @@ static inline int mf_fill_params(const mf_config_t* c, MfParams* P, std::string&
     if (!(tau0 < 1.0) || tau0 < c->pdf_xmin || c->mu_f < c->pdf_qmin || c->mu_f > c->pdf_qmax) {
       err = "kinematics outside the PDF grid"; return MF_EINVAL;
     }
-    p.ltau0 = log(tau0);
+    p.ltau0 = log(tau0); p.tau0 = tau0;
     double gs2n = 1.0;
     for (int i = 0; i < ng; ++i) gs2n *= 4.0 * PI * c->alpha_s;
     const double scale = (c->process == MF_GG_TT) ? MF_ME2_GG_TT_SCALE : (c->process == MF_GG_TTG) ? MF_ME2_GG_TTG_SCALE : MF_ME2_GG_TTGG_SCALE;

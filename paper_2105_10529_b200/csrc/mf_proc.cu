@@ -49,6 +49,14 @@ __device__ __forceinline__ void mf_hist_add(double* __restrict__ hw, int nb, uns
   }
 }
 
+// D > 10 (classic 4n-random RAMBO): the bins of dimensions 10.. are in a second packed word
+template <int D>
+__device__ __forceinline__ void mf_hist_add2(double* __restrict__ hw, int nb, unsigned long long lo, unsigned long long hi,
+                                             bool contrib, double t2, unsigned lt_mask) {
+  mf_hist_add<(D < MF_PACK_DIMS ? D : MF_PACK_DIMS)>(hw, nb, lo, contrib, t2, lt_mask);
+  if constexpr (D > MF_PACK_DIMS) mf_hist_add<D - MF_PACK_DIMS>(hw + MF_PACK_DIMS * nb, nb, hi, contrib, t2, lt_mask);
+}
+
 // observable histograms of one warp: ho1[o][64] += t, ho2[o][64] += t^2, same fixed-order scheme
 __device__ __forceinline__ void mf_obs_add(double* __restrict__ ho1, double* __restrict__ ho2, int n_obs, unsigned keys,
                                            bool contrib, double t, double t2, unsigned lt_mask) {
@@ -125,12 +133,12 @@ __device__ __forceinline__ void mf_block_finish(double s1, double s2, unsigned l
 // ---- S1-S9 fused ---------------------------------------------------------------------------------
 // partial: [gridDim.x][row] doubles (2 + d*nb sums, then the observable sums), pcount: [gridDim.x][2]
 // (n_pass, n_nonfinite)
-template <int PROC>
+template <int PROC, int CL>
 __global__ void __launch_bounds__(MF_THREADS, MfLaunch<PROC>::MINB)
 mf_iterate_kernel(const MfParams P, const double* __restrict__ g_edges, const double* __restrict__ g_pdf,
                   uint32_t iteration, unsigned long long first, unsigned long long n, double n_total,
                   double* __restrict__ partial, unsigned long long* __restrict__ pcount, int row) {
-  constexpr int D = MfProc<PROC>::D;
+  constexpr int D = MfDim<PROC, CL>::D;
   extern __shared__ double smem[];
   const int nb = P.nb, nh = D * nb, nw = blockDim.x >> 5;
   double* s_edges = smem;
@@ -158,20 +166,19 @@ mf_iterate_kernel(const MfParams P, const double* __restrict__ g_edges, const do
     double F = 0.0;
     unsigned okeys = 0;
     if (MF_UNIFORM_ME) {                                 // every thread runs the event (barriers inside);
-      F = mf_event<PROC, false>(P, s_edges, s_pdf, iteration, first + (valid ? i : n - 1), bin, pass, nullptr, &okeys);
+      F = mf_event<PROC, false, double, CL>(P, s_edges, s_pdf, iteration, first + (valid ? i : n - 1), bin, pass, nullptr, &okeys);
       if (!valid) { F = 0.0; pass = false; }             // lanes past the end recompute event n-1, discarded
     } else if (valid) {
-      F = mf_event<PROC, false>(P, s_edges, s_pdf, iteration, first + i, bin, pass, nullptr, &okeys);
+      F = mf_event<PROC, false, double, CL>(P, s_edges, s_pdf, iteration, first + i, bin, pass, nullptr, &okeys);
     }
     if (!isfinite(F)) { F = 0.0; ++n_bad; }              // A20
     if (valid && pass) ++n_pass;
     const double t = F / n_total, t2 = t * t;            // O9: t_i = F_i / N
     s1 += t; s2 += t2;
     // per-warp histogram H[j][k] += t^2, lanes that share a bin are served in lane order
-    unsigned long long packed = 0;
-#pragma unroll
-    for (int j = 0; j < D; ++j) packed |= (unsigned long long)bin[j] << (6 * j);
-    mf_hist_add<D>(hw, nb, packed, valid && t2 != 0.0, t2, lt_mask);
+    unsigned long long packed, packed_hi;
+    mf_pack_bins<D>(bin, packed, packed_hi);
+    mf_hist_add2<D>(hw, nb, packed, packed_hi, valid && t2 != 0.0, t2, lt_mask);
     if (P.n_obs > 0)
       mf_obs_add(s_obs + warp * MF_OBS_ACC, s_obs + warp * MF_OBS_ACC + MF_OBS_ACC / 2, P.n_obs, okeys, valid && F != 0.0, t, t2, lt_mask);
   }
@@ -280,16 +287,18 @@ mf_iterate_compact_kernel(const MfParams P, const double* __restrict__ g_edges, 
 //                    maps a dense index over ALL passing events to (region, entry), so every lane of
 //                    every warp carries a passing event through S7; writes F = pref |M|^2 in place
 //   mf_hist_kernel   S9: sum t, sum t^2 and the d x nb histogram in fixed order from (F, packed bins)
-// Field order of a record: k[N][4], sqrt(shat), pref (-> F), packed bins (6 bits per dimension).
+// Field order of a record: k[N][4], sqrt(shat), pref (-> F), packed bins (6 bits per dimension), observable slots,
+// packed bins of dimensions 10.. (classic 4n-random RAMBO only, CL = 1; otherwise never touched).
+#define MF_REC_FIELDS(N) (4 * (N) + 5)
 #ifndef MF_FRONT_MINB
 #define MF_FRONT_MINB 3              // resident CTAs per SM the front end is compiled for (80 registers; tuned, profiles/r1_tuning.md)
 #endif
-template <int PROC>
+template <int PROC, int CL>
 __global__ void __launch_bounds__(MF_THREADS, MF_FRONT_MINB)
 mf_front_kernel(const MfParams P, const double* __restrict__ g_edges, const double* __restrict__ g_pdf,
                 uint32_t iteration, unsigned long long first, unsigned long long n, unsigned long long cap,
                 double* __restrict__ rec, unsigned int* __restrict__ count) {
-  constexpr int D = MfProc<PROC>::D, N = MfProc<PROC>::N, NF = 4 * N + 4, T = MF_THREADS;
+  constexpr int D = MfDim<PROC, CL>::D, N = MfProc<PROC>::N, NF = MF_REC_FIELDS(N), T = MF_THREADS;
   extern __shared__ double smem[];
   double* s_edges = smem;
   double* s_pdf = s_edges + D * (P.nb + 1);
@@ -308,7 +317,7 @@ mf_front_kernel(const MfParams P, const double* __restrict__ g_edges, const doub
     int bin[D];
     double k[N][4], rts, pref;
     unsigned okeys = 0;
-    if (i < hi) pass = mf_event_front<PROC, false>(P, s_edges, s_pdf, iteration, first + i, bin, k, rts, pref, nullptr, &okeys);
+    if (i < hi) pass = mf_event_front<PROC, false, CL>(P, s_edges, s_pdf, iteration, first + i, bin, k, rts, pref, nullptr, &okeys);
     const unsigned bal = __ballot_sync(0xffffffffu, pass);
     if (lane == 0) s_wtot[warp] = __popc(bal);
     __syncthreads();
@@ -323,11 +332,11 @@ mf_front_kernel(const MfParams P, const double* __restrict__ g_edges, const doub
         for (int c = 0; c < 4; ++c) R[(size_t)(4 * p + c) * cap + slot] = k[p][c];
       R[(size_t)(4 * N) * cap + slot] = rts;
       R[(size_t)(4 * N + 1) * cap + slot] = pref;
-      unsigned long long packed = 0;                     // D <= 10 bins of 6 bits
-#pragma unroll
-      for (int j = 0; j < D; ++j) packed |= (unsigned long long)bin[j] << (6 * j);
+      unsigned long long packed, packed_hi;              // bins of 6 bits, 10 per word
+      mf_pack_bins<D>(bin, packed, packed_hi);
       R[(size_t)(4 * N + 2) * cap + slot] = __longlong_as_double((long long)packed);
       if (P.n_obs > 0) R[(size_t)(4 * N + 3) * cap + slot] = __longlong_as_double((long long)okeys);
+      if (D > MF_PACK_DIMS) R[(size_t)(4 * N + 4) * cap + slot] = __longlong_as_double((long long)packed_hi);
     }
     __syncthreads();
     filled += tot;
@@ -349,7 +358,7 @@ template <int PROC, typename Real, int THREADS>
 __global__ void __launch_bounds__(THREADS, 1)
 mf_me_kernel(const MfParams P, double* __restrict__ rec, const unsigned int* __restrict__ count, int regions,
              unsigned long long cap) {
-  constexpr int N = MfProc<PROC>::N, NF = 4 * N + 4, T = THREADS;
+  constexpr int N = MfProc<PROC>::N, NF = MF_REC_FIELDS(N), T = THREADS;
   extern __shared__ unsigned int s_pre[];                // [regions + 1] exclusive prefix, then s_part[T]
   unsigned int* s_part = s_pre + regions + 1;
   const unsigned tid = threadIdx.x;
@@ -393,12 +402,12 @@ mf_me_kernel(const MfParams P, double* __restrict__ rec, const unsigned int* __r
   }
 }
 
-template <int PROC>
+template <int PROC, int CL>
 __global__ void __launch_bounds__(MF_THREADS)
 mf_hist_kernel(const MfParams P, const double* __restrict__ rec, const unsigned int* __restrict__ count, int regions,
                unsigned long long cap, double n_total, double* __restrict__ partial,
                unsigned long long* __restrict__ pcount, int row) {
-  constexpr int D = MfProc<PROC>::D, N = MfProc<PROC>::N, NF = 4 * N + 4, T = MF_THREADS;
+  constexpr int D = MfDim<PROC, CL>::D, N = MfProc<PROC>::N, NF = MF_REC_FIELDS(N), T = MF_THREADS;
   extern __shared__ double smem[];
   const int nb = P.nb, nh = D * nb, nw = T >> 5;
   double* s_hist = smem;                                 // [nw][D*nb]
@@ -425,7 +434,9 @@ mf_hist_kernel(const MfParams P, const double* __restrict__ rec, const unsigned 
       const double t = F / n_total, t2 = t * t;          // O9
       s1 += t; s2 += t2;
       const bool contrib = have && t2 != 0.0;
-      mf_hist_add<D>(hw, nb, packed, contrib, t2, lt_mask);
+      unsigned long long packed_hi = 0ull;
+      if (D > MF_PACK_DIMS && have) packed_hi = (unsigned long long)__double_as_longlong(R[(size_t)(4 * N + 4) * cap + e]);
+      mf_hist_add2<D>(hw, nb, packed, packed_hi, contrib, t2, lt_mask);
       if (P.n_obs > 0) {
         const unsigned okeys = have ? (unsigned)__double_as_longlong(R[(size_t)(4 * N + 3) * cap + e]) : 0u;
         mf_obs_add(s_obs + warp * MF_OBS_ACC, s_obs + warp * MF_OBS_ACC + MF_OBS_ACC / 2, P.n_obs, okeys, have && F != 0.0, t, t2, lt_mask);
@@ -436,45 +447,70 @@ mf_hist_kernel(const MfParams P, const double* __restrict__ rec, const unsigned 
 }
 
 // ---- S1-S8 with per-event outputs -------------------------------------------------------------------
+// front end of one event and its per-event records (everything but the weight and |M|^2)
+template <int PROC, bool REC, int CL>
+__device__ __forceinline__ bool mf_eval_front(const MfParams& P, const double* s_edges, const double* s_pdf, uint32_t iteration,
+                                              unsigned long long ev, unsigned long long i, const MfEvalOutDev& o,
+                                              double k[MfProc<PROC>::N][4], double& rts, double& pref) {
+  constexpr int D = MfDim<PROC, CL>::D, NL = 2 + MfProc<PROC>::N;
+  int bin[D];
+  MfEventRec rec;
+  const bool pass = mf_event_front<PROC, REC, CL>(P, s_edges, s_pdf, iteration, ev, bin, k, rts, pref, REC ? &rec : nullptr);
+  if (o.bins) {
+#pragma unroll
+    for (int j = 0; j < D; ++j) o.bins[i * D + j] = (uint8_t)bin[j];
+  }
+  if (o.pass) o.pass[i] = pass ? 1 : 0;
+  if (REC) {
+    if (o.x) {
+#pragma unroll
+      for (int j = 0; j < D; ++j) o.x[i * D + j] = rec.y[j];
+    }
+    if (o.momenta) {
+#pragma unroll
+      for (int l = 0; l < NL; ++l)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) o.momenta[(i * NL + l) * 4 + c] = rec.mom[l][c];
+    }
+    if (o.pdf) { o.pdf[2 * i] = rec.pdf[0]; o.pdf[2 * i + 1] = rec.pdf[1]; }
+  }
+  return pass;
+}
+
+// The generator variants are grid-uniform run-time branches in and around the front end, so that the
+// |M|^2 code is instantiated once per kernel.
 template <int PROC, bool REC, typename T>
 __global__ void __launch_bounds__(MF_THREADS, MfLaunch<PROC>::MINB)
 mf_eval_kernel(const MfParams P, const double* __restrict__ g_edges, const double* __restrict__ g_pdf,
                uint32_t iteration, unsigned long long first, unsigned long long n, MfEvalOutDev o) {
-  constexpr int D = MfProc<PROC>::D, NL = 2 + MfProc<PROC>::N;
+  constexpr int N = MfProc<PROC>::N;
   extern __shared__ double smem[];
   double* s_edges = smem;
-  double* s_pdf = s_edges + D * (P.nb + 1);
+  double* s_pdf = s_edges + P.d * (P.nb + 1);
   mf_stage_tables(P, g_edges, g_pdf, s_edges, s_pdf);
   __syncthreads();
   const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
   for (unsigned long long base = (unsigned long long)blockIdx.x * blockDim.x; base < n; base += stride) {
     unsigned long long i = base + threadIdx.x;           // block-uniform trip count (barriers inside the event)
     if (i >= n) { if (!MF_UNIFORM_ME) break; i = n - 1; }   // tail lanes recompute event n-1 (same values written)
-    int bin[D];
+    double k[N][4], rts, pref;
     bool pass;
-    MfEventRec rec;
-    double F = mf_event<PROC, REC, T>(P, s_edges, s_pdf, iteration, first + i, bin, pass, REC ? &rec : nullptr);
+    if (PROC != 0 && (P.gen & MFD_GEN_CLASSIC)) pass = mf_eval_front<PROC, REC, PROC != 0 ? 1 : 0>(P, s_edges, s_pdf, iteration, first + i, i, o, k, rts, pref);
+    else pass = mf_eval_front<PROC, REC, PROC != 0 ? 2 : 0>(P, s_edges, s_pdf, iteration, first + i, i, o, k, rts, pref);
+    double me2 = 0.0;
+    if (MF_UNIFORM_ME || pass) {                         // S7 (in the real type T)
+      T kt[N][4];
+#pragma unroll
+      for (int p = 0; p < N; ++p)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) kt[p][c] = (T)k[p][c];
+      me2 = (double)mf_me2<PROC, T>(P, (T)rts, kt);
+    }
+    if (!pass) me2 = 0.0;
+    double F = pass ? pref * me2 : 0.0;                  // S8
     if (!isfinite(F)) F = 0.0;
     if (o.weight) o.weight[i] = F;
-    if (o.bins) {
-#pragma unroll
-      for (int j = 0; j < D; ++j) o.bins[i * D + j] = (uint8_t)bin[j];
-    }
-    if (o.pass) o.pass[i] = pass ? 1 : 0;
-    if (REC) {
-      if (o.x) {
-#pragma unroll
-        for (int j = 0; j < D; ++j) o.x[i * D + j] = rec.y[j];
-      }
-      if (o.momenta) {
-#pragma unroll
-        for (int l = 0; l < NL; ++l)
-#pragma unroll
-          for (int c = 0; c < 4; ++c) o.momenta[(i * NL + l) * 4 + c] = rec.mom[l][c];
-      }
-      if (o.me2) o.me2[i] = rec.me2;
-      if (o.pdf) { o.pdf[2 * i] = rec.pdf[0]; o.pdf[2 * i + 1] = rec.pdf[1]; }
-    }
+    if (REC && o.me2) o.me2[i] = me2;
   }
 }
 
@@ -485,6 +521,11 @@ mf_eval_kernel(const MfParams P, const double* __restrict__ g_edges, const doubl
 static constexpr bool kCompact = MF_COMPACT && MfProc<MF_PROC>::NGL > 0;
 static constexpr bool kEvalOne = MfProc<MF_PROC>::NGL > 0;
 static constexpr bool kF32 = MF_PROC == 2;   // fp32 variant of the |M|^2 stage: gg -> tt~g only (BASELINE configs[4])
+// classic 4n-random RAMBO: processes 1-3; the heavy ones on the staged path only
+static constexpr int kCL = MF_PROC != 0 ? 1 : 0;    // front-end instance of the classic RAMBO (mf_event.cuh MfDim)
+static constexpr int kLT = MF_PROC != 0 ? 2 : 0;    // ... of the configs' RAMBO with the selectable tau map
+static inline bool is_classic(const MfParams& P) { return kCL && (P.gen & MFD_GEN_CLASSIC); }
+static inline bool is_lintau(const MfParams& P) { return kLT && !is_classic(P) && (P.gen & MFD_GEN_LINEAR); }
 
 static cudaError_t proc_setup(const MfParams& P, size_t* smem_iter, size_t* smem_eval, int* occ_iter, int* occ_eval) {
   const size_t tables = (size_t)P.d * (P.nb + 1) + (size_t)P.pdf_nx * P.pdf_nq;
@@ -498,10 +539,20 @@ static cudaError_t proc_setup(const MfParams& P, size_t* smem_iter, size_t* smem
     if (e) return e;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_iter, mf_iterate_compact_kernel<MF_PROC>, MF_THREADS, *smem_iter);
   } else {
-    e = cudaFuncSetAttribute(mf_iterate_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)(*smem_iter + sizeof(double) * nw * MF_OBS_ACC));      // room for the observable histograms
-    if (e) return e;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_iter, mf_iterate_kernel<MF_PROC>, MF_THREADS, *smem_iter);
+    const int smem_obs = (int)(*smem_iter + sizeof(double) * nw * MF_OBS_ACC);            // room for the observable histograms
+    if (is_classic(P)) {
+      e = cudaFuncSetAttribute(mf_iterate_kernel<MF_PROC, kCL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_obs);
+      if (e) return e;
+      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_iter, mf_iterate_kernel<MF_PROC, kCL>, MF_THREADS, *smem_iter);
+    } else if (is_lintau(P)) {
+      e = cudaFuncSetAttribute(mf_iterate_kernel<MF_PROC, kLT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_obs);
+      if (e) return e;
+      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_iter, mf_iterate_kernel<MF_PROC, kLT>, MF_THREADS, *smem_iter);
+    } else {
+      e = cudaFuncSetAttribute(mf_iterate_kernel<MF_PROC, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_obs);
+      if (e) return e;
+      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_iter, mf_iterate_kernel<MF_PROC, 0>, MF_THREADS, *smem_iter);
+    }
   }
   if (e) return e;
   if constexpr (!kEvalOne) {
@@ -541,10 +592,16 @@ static cudaError_t proc_iterate(const MfParams& P, const double* edges, const do
     if (kCompact) return cudaErrorNotSupported;          // observables of the heavy processes: staged path
     smem += sizeof(double) * (MF_THREADS / 32) * MF_OBS_ACC;
   }
-  if constexpr (kCompact)
+  if constexpr (kCompact) {
+    if (P.gen != 0) return cudaErrorNotSupported;        // generator variants of the heavy processes: staged path
     mf_iterate_compact_kernel<MF_PROC><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount, row);
-  else
-    mf_iterate_kernel<MF_PROC><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount, row);
+  } else if (is_classic(P)) {
+    mf_iterate_kernel<MF_PROC, kCL><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount, row);
+  } else if (is_lintau(P)) {
+    mf_iterate_kernel<MF_PROC, kLT><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount, row);
+  } else {
+    mf_iterate_kernel<MF_PROC, 0><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount, row);
+  }
   return cudaGetLastError();
 }
 
@@ -553,7 +610,7 @@ static cudaError_t proc_iterate(const MfParams& P, const double* edges, const do
 #define MF_STAGED 1                  // heavy processes (with cuts) iterate through the staged path
 #endif
 static constexpr bool kStaged = MF_STAGED && MfProc<MF_PROC>::NGL > 0;
-static constexpr int kRecFields = 4 * MfProc<MF_PROC>::N + 4;
+static constexpr int kRecFields = MF_REC_FIELDS(MfProc<MF_PROC>::N);
 
 static size_t front_smem(const MfParams& P) {
   return sizeof(double) * ((size_t)P.d * (P.nb + 1) + (size_t)P.pdf_nx * P.pdf_nq) + sizeof(int) * (MF_THREADS / 32);
@@ -567,7 +624,10 @@ static cudaError_t proc_staged_setup(const MfParams& P, int* rec_fields, int* oc
   *occ_front = *occ_hist = 0;
   if constexpr (!kStaged) return cudaSuccess;
   else {
-  cudaError_t e = cudaFuncSetAttribute(mf_front_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)front_smem(P));
+  const bool cl = is_classic(P), lt = is_lintau(P);
+  cudaError_t e = cl ? cudaFuncSetAttribute(mf_front_kernel<MF_PROC, kCL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)front_smem(P))
+                : lt ? cudaFuncSetAttribute(mf_front_kernel<MF_PROC, kLT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)front_smem(P))
+                     : cudaFuncSetAttribute(mf_front_kernel<MF_PROC, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)front_smem(P));
   if (e) return e;
   e = cudaFuncSetAttribute(mf_me_kernel<MF_PROC, double, MF_ME_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
   if (e) return e;
@@ -575,12 +635,16 @@ static cudaError_t proc_staged_setup(const MfParams& P, int* rec_fields, int* oc
     e = cudaFuncSetAttribute(mf_me_kernel<MF_PROC, float, MF_ME_THREADS_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
     if (e) return e;
   }
-  e = cudaFuncSetAttribute(mf_hist_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                           (int)(hist_smem(P) + sizeof(double) * (MF_THREADS / 32) * MF_OBS_ACC));
+  const int smem_hist = (int)(hist_smem(P) + sizeof(double) * (MF_THREADS / 32) * MF_OBS_ACC);
+  e = cl ? cudaFuncSetAttribute(mf_hist_kernel<MF_PROC, kCL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_hist)
+         : cudaFuncSetAttribute(mf_hist_kernel<MF_PROC, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_hist);
   if (e) return e;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_front, mf_front_kernel<MF_PROC>, MF_THREADS, front_smem(P));
+  e = cl ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_front, mf_front_kernel<MF_PROC, kCL>, MF_THREADS, front_smem(P))
+    : lt ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_front, mf_front_kernel<MF_PROC, kLT>, MF_THREADS, front_smem(P))
+         : cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_front, mf_front_kernel<MF_PROC, 0>, MF_THREADS, front_smem(P));
   if (e) return e;
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_hist, mf_hist_kernel<MF_PROC>, MF_THREADS, hist_smem(P));
+  return cl ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_hist, mf_hist_kernel<MF_PROC, kCL>, MF_THREADS, hist_smem(P))
+            : cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_hist, mf_hist_kernel<MF_PROC, 0>, MF_THREADS, hist_smem(P));
   }
 }
 
@@ -593,7 +657,10 @@ static cudaError_t proc_staged(const MfParams& P, const double* edges, const dou
   else {
   cudaError_t e;
   if (ev && (e = cudaEventRecord(ev[0], st))) return e;
-  mf_front_kernel<MF_PROC><<<ws.regions, MF_THREADS, front_smem(P), st>>>(P, edges, pdf, iteration, first, n, ws.cap, ws.rec, ws.count);
+  const bool cl = is_classic(P);
+  if (cl) mf_front_kernel<MF_PROC, kCL><<<ws.regions, MF_THREADS, front_smem(P), st>>>(P, edges, pdf, iteration, first, n, ws.cap, ws.rec, ws.count);
+  else if (is_lintau(P)) mf_front_kernel<MF_PROC, kLT><<<ws.regions, MF_THREADS, front_smem(P), st>>>(P, edges, pdf, iteration, first, n, ws.cap, ws.rec, ws.count);
+  else mf_front_kernel<MF_PROC, 0><<<ws.regions, MF_THREADS, front_smem(P), st>>>(P, edges, pdf, iteration, first, n, ws.cap, ws.rec, ws.count);
   if ((e = cudaGetLastError())) return e;
   if (ev && (e = cudaEventRecord(ev[1], st))) return e;
   const size_t sm = sizeof(unsigned int) * ((size_t)ws.regions + 1 + (f32 ? MF_ME_THREADS_F32 : MF_ME_THREADS));
@@ -605,7 +672,8 @@ static cudaError_t proc_staged(const MfParams& P, const double* edges, const dou
   }
   if ((e = cudaGetLastError())) return e;
   if (ev && (e = cudaEventRecord(ev[2], st))) return e;
-  mf_hist_kernel<MF_PROC><<<grid_hist, MF_THREADS, hist_smem(P), st>>>(P, ws.rec, ws.count, ws.regions, ws.cap, n_total, partial, pcount, row);
+  if (cl) mf_hist_kernel<MF_PROC, kCL><<<grid_hist, MF_THREADS, hist_smem(P), st>>>(P, ws.rec, ws.count, ws.regions, ws.cap, n_total, partial, pcount, row);
+  else mf_hist_kernel<MF_PROC, 0><<<grid_hist, MF_THREADS, hist_smem(P), st>>>(P, ws.rec, ws.count, ws.regions, ws.cap, n_total, partial, pcount, row);
   if ((e = cudaGetLastError())) return e;
   if (ev && (e = cudaEventRecord(ev[3], st))) return e;
   return cudaSuccess;

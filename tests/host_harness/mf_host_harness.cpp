@@ -45,5 +45,32 @@ extern "C" double mfh_event_ttg_f32(const MfParams* P, const double* edges, cons
   rec_out[34] = rec.me2; rec_out[35] = rec.pdf[0]; rec_out[36] = rec.pdf[1];
   return F;
 }
+// selectable generators: classic 4n-random RAMBO (P->gen & 1; d = 2 + 4 n_final) and/or the linear-tau
+// map (P->gen & 2, run-time branch).  rec_out: y[18], mom[24], me2, pdf[2]
+template <int PROC, int CL>
+static double run_gen(const MfParams& P, const double* edges, const double* pdf, uint32_t it, uint64_t ev,
+                      int* bins, int* pass, double* rec_out) {
+  int bin[MfDim<PROC, CL>::D]; bool ok; MfEventRec rec;
+  std::memset(&rec, 0, sizeof rec);
+  double F = mf_event<PROC, true, double, CL>(P, edges, pdf, it, ev, bin, ok, &rec);
+  for (int j = 0; j < MfDim<PROC, CL>::D; ++j) bins[j] = bin[j];
+  *pass = ok;
+  std::memcpy(rec_out, rec.y, sizeof(double) * 18);
+  std::memcpy(rec_out + 18, rec.mom, sizeof(double) * 24);
+  rec_out[42] = rec.me2; rec_out[43] = rec.pdf[0]; rec_out[44] = rec.pdf[1];
+  return F;
+}
+extern "C" double mfh_event_gen(const MfParams* P, const double* edges, const double* pdf, uint32_t it,
+                                uint64_t ev, int* bins, int* pass, double* rec_out) {
+  const bool cl = P->gen & MFD_GEN_CLASSIC;
+  switch (P->process) {
+    case 1: return cl ? run_gen<1, 1>(*P, edges, pdf, it, ev, bins, pass, rec_out) : run_gen<1, 2>(*P, edges, pdf, it, ev, bins, pass, rec_out);
+    case 2: return cl ? run_gen<2, 1>(*P, edges, pdf, it, ev, bins, pass, rec_out) : run_gen<2, 2>(*P, edges, pdf, it, ev, bins, pass, rec_out);
+#ifndef MFH_NO_TTGG
+    case 3: return cl ? run_gen<3, 1>(*P, edges, pdf, it, ev, bins, pass, rec_out) : run_gen<3, 2>(*P, edges, pdf, it, ev, bins, pass, rec_out);
+#endif
+  }
+  return -1.0;
+}
 extern "C" int mfh_params_size(void) { return (int)sizeof(MfParams); }
 extern "C" int mfh_fill_params(const mf_config_t* c, MfParams* P) { std::string e; return mf_fill_params(c, P, e); }

@@ -28,12 +28,12 @@ def random_grid(d, nb, seed):
     return e
 
 
-def compare_events(out, ref, proc):
+def compare_events(out, ref, proc, mom_tol=(1e-11, 1e-9)):
     g = {k: v.cpu().numpy() for k, v in out.items()}
     assert (g["bins"] == ref["bins"]).all()
     assert (g["pass_"] == ref["pass_"]).all()
     np.testing.assert_allclose(g["x"], ref["x"], rtol=1e-14, atol=0)
-    np.testing.assert_allclose(g["momenta"], ref["momenta"], rtol=1e-11, atol=1e-9)
+    np.testing.assert_allclose(g["momenta"], ref["momenta"], rtol=mom_tol[0], atol=mom_tol[1])
     if proc:
         np.testing.assert_allclose(g["pdf"], ref["pdf"], rtol=1e-12, atol=1e-15)
     nz = ref["weight"] != 0
@@ -326,3 +326,75 @@ def test_errors_and_edge_cases(mf):
         gpu.set_grid(g)
     gpu.vegas_iterate(2)                          # minimum iteration
     assert gpu.result()["n_iter"] == 1
+
+
+# ---- selectable generators: classic 4n-random RAMBO (flag 1, d = 2 + 4 n_final) and linear tau (flag 2)
+@pytest.mark.parametrize("proc,gen,n", [(1, 1, 5003), (1, 2, 5003), (1, 3, 5003), (2, 1, 3001), (2, 2, 3001), (2, 3, 3001),
+                                        (3, 1, 333), (3, 2, 333), (3, 3, 333)])
+def test_generator_variants_per_event_parity(mf, mfo, proc, gen, n):
+    cfg = W.config(proc, seed=4, generator=gen)
+    gpu, orc = mf.Vegas(cfg), mfo.Vegas(cfg)
+    assert gpu.d == orc.d == (2 + 4 * orc.n_final if gen & W.GEN_CLASSIC_RAMBO else 3 * orc.n_final - 2)
+    # the boost of the classic RAMBO (gamma = Q0/M of the generated system) amplifies the rounding of its inputs
+    mom_tol = (1e-10, 1e-8) if gen & W.GEN_CLASSIC_RAMBO else (1e-11, 1e-9)
+    ref = orc.eval(0, 0, n, n_threads=mfo.max_threads())
+    compare_events(gpu.integrand_eval(0, 0, n, debug=True), ref, proc, mom_tol)
+    e = random_grid(orc.d, 50, 200 + proc)
+    gpu.set_grid(e); orc.set_grid(e)
+    ref = orc.eval(2, 2**32 + 5, n, n_threads=mfo.max_threads())
+    compare_events(gpu.integrand_eval(2, 2**32 + 5, n, debug=True), ref, proc, mom_tol)
+    w = gpu.integrand_eval(2, 2**32 + 5, n)["weight"].cpu().numpy()      # weights-only call: same values
+    nz = ref["weight"] != 0
+    assert (w[~nz] == 0).all() and np.abs(w[nz] / ref["weight"][nz] - 1).max() < 2 * RTOL_EVENT
+
+
+@pytest.mark.parametrize("proc,gen,n_iter,n", [(1, 1, 3, 40_000), (1, 2, 2, 40_000), (2, 1, 2, 20_000), (2, 3, 2, 20_000),
+                                               (3, 1, 2, 1_500), (3, 2, 2, 1_500)])
+def test_generator_variants_iteration_parity(mf, mfo, proc, gen, n_iter, n):
+    """whole iterations with the variant generators (process 1: fused kernel with d = 10; processes 2, 3: staged
+    path with d = 14 / 18, bins of dimensions 10.. in the second packed word) vs the oracle"""
+    cfg = W.config(proc, seed=6, generator=gen)
+    gpu, orc = mf.Vegas(cfg), mfo.Vegas(cfg)
+    for it in range(n_iter):
+        g = gpu.vegas_iterate(n)
+        o = orc.iterate(n, n_threads=mfo.max_threads())
+        assert g["n_events"] == n and g["n_pass"] == o["n_pass"] and g["n_nonfinite"] == 0 == o["n_nonfinite"]
+        assert abs(g["integral"] / o["integral"] - 1) < RTOL_INT
+        assert abs(g["sigma"] / o["sigma"] - 1) < 1e-8
+        acc, cnt = gpu.get_accum()
+        assert acc.shape == (2 + orc.d * 50,)
+        np.testing.assert_allclose(acc, orc.get_accum(), rtol=RTOL_INT, atol=1e-300)
+        np.testing.assert_allclose(gpu.get_grid(), orc.get_grid(), rtol=0, atol=1e-11)
+        gpu.set_grid(orc.get_grid())
+    rg, ro = gpu.result(), orc.result()
+    assert rg["n_iter"] == n_iter and abs(rg["integral"] / ro["integral"] - 1) < 1e-8
+
+
+def test_generator_variants_observables_errors_and_cross_section(mf, mfo):
+    """observables through the d = 14 staged path; argument errors; and the physics check: config 1's cross section
+    through every generator variant on the GPU (quadrature value 1074.39 pb, tests/test_oracle_generators.py)"""
+    cfg = W.config(W.GG_TTG, seed=3, generator=W.GEN_CLASSIC_RAMBO)
+    gpu, orc = mf.Vegas(cfg), mfo.Vegas(cfg)
+    obs = [(0, 20, 0.0, 400.0), (3, 10, 30.0, 230.0)]
+    gpu.set_observables(obs)
+    n = 20_000
+    ref = orc.observable_hist(0, 0, n, n, obs, n_threads=mfo.max_threads())
+    gpu.vegas_iterate(n)
+    got, n_it = gpu.get_observables()
+    for (g1, g2), (r1, r2) in zip(got, ref):
+        np.testing.assert_allclose(g1, r1, rtol=1e-10, atol=1e-13 * np.abs(r1).max())
+        np.testing.assert_allclose(g2, r2, rtol=1e-10, atol=1e-13 * np.abs(r2).max())
+    with pytest.raises(mf.MfError) as e:
+        gpu.set_path(False)                                   # heavy processes: classic RAMBO on the staged path only
+    assert e.value.code == mf.MF_EUNSUPPORTED
+    for bad in (dict(process=W.EE_MUMU, generator=1), dict(process=W.GG_TT, generator=4)):
+        with pytest.raises(mf.MfError) as e:
+            mf.Vegas(W.config(bad["process"], generator=bad["generator"]))
+        assert e.value.code == mf.MF_EINVAL
+    c = W.CONFIGS[1]
+    for gen in (1, 2, 3):
+        gpu = mf.Vegas(W.config(W.GG_TT, seed=c["seed"], generator=gen))
+        for _ in range(c["n_iter"]):
+            gpu.vegas_iterate(c["n_events"])
+        r = gpu.result()
+        assert abs(r["integral"] - 1074.393) < 5 * r["sigma"] + 0.02 and r["sigma"] < 1.5, (gen, r)

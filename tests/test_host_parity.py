@@ -90,3 +90,47 @@ def test_host_compiled_fp32_matrix_element_variant(mfo, harness):
             assert F == 0.0
     rel = np.array(rel)
     assert np.median(rel) < 2e-6 and (rel > 1e-4).mean() < 0.02 and rel.max() < 1e-2, (np.median(rel), rel.max())
+
+
+@pytest.mark.parametrize("proc,gen,n", [(1, 1, 200), (1, 2, 200), (1, 3, 200), (2, 1, 200), (2, 2, 100), (2, 3, 200), (3, 1, 30), (3, 3, 30)])
+def test_host_compiled_generator_variants_match_oracle(mfo, harness, proc, gen, n):
+    """selectable generators (classic 4n-random RAMBO = 1, linear tau = 2) of the product's per-event
+    code, compiled for the host, against the oracle's mfo_rambo_classic / mfo_x_map_linear path"""
+    harness.mfh_event_gen.restype = C.c_double
+    harness.mfh_event_gen.argtypes = harness.mfh_event.argtypes
+    cfg = W.config(proc, seed=9, generator=gen)
+    c, pdf = make_config(cfg)
+    P = C.create_string_buffer(harness.mfh_params_size())
+    assert harness.mfh_fill_params(C.byref(c), P) == 0
+    orc = mfo.Vegas(cfg)
+    d, nl = orc.d, 2 + orc.n_final
+    assert d == (2 + 4 * orc.n_final if gen & 1 else 3 * orc.n_final - 2)
+    edges = random_grid(d, 50, 21 + proc)
+    orc.set_grid(edges)
+    ref = orc.eval(1, 500, n)
+    bins = np.zeros(24, np.int32); ok = np.zeros(1, np.int32); rec = np.zeros(45)
+    worst = 0.0
+    for i in range(n):
+        F = harness.mfh_event_gen(P, edges.ctypes.data, pdf.ctypes.data, 1, 500 + i, bins.ctypes.data, ok.ctypes.data, rec.ctypes.data)
+        assert list(bins[:d]) == list(ref["bins"][i])
+        assert ok[0] == ref["pass_"][i]
+        np.testing.assert_allclose(rec[:d], ref["x"][i], rtol=1e-14, atol=0)
+        np.testing.assert_allclose(rec[18:18 + 4 * nl].reshape(nl, 4), ref["momenta"][i], rtol=1e-10, atol=1e-8)
+        np.testing.assert_allclose(rec[43:45], ref["pdf"][i], rtol=1e-11, atol=1e-15)
+        if ref["weight"][i] != 0:
+            worst = max(worst, abs(F / ref["weight"][i] - 1), abs(rec[42] / ref["me2"][i] - 1))
+        else:
+            assert F == 0.0
+    assert worst < 1e-10, worst
+
+
+def test_generator_flag_validation(harness):
+    """mf_config_t.generator (host logic of mf_vegas_create): unknown flags and process 0 are rejected; d follows the flag"""
+    P = C.create_string_buffer(harness.mfh_params_size())
+    for proc, gen, rc in [(1, 0, 0), (1, 1, 0), (2, 2, 0), (3, 3, 0), (1, 4, -1), (2, 8, -1), (0, 1, -1), (0, 2, -1)]:
+        c, pdf = make_config(W.config(proc, generator=gen))
+        assert harness.mfh_fill_params(C.byref(c), P) == rc, (proc, gen)
+        if rc == 0:
+            d = np.frombuffer(P, dtype=np.int32, count=5)          # MfParams: process, d, n_final, nb, gen
+            nf = {1: 2, 2: 3, 3: 4}[proc]
+            assert d[0] == proc and d[2] == nf and d[4] == gen and d[1] == (2 + 4 * nf if gen & 1 else 3 * nf - 2)

@@ -26,7 +26,8 @@ extern "C" {
 #endif
 
 enum { MFO_OK = 0, MFO_EINVAL = -1, MFO_ENOMEM = -2, MFO_ESTATE = -4, MFO_EUNSUPPORTED = -5 };
-enum { MFO_EE_MUMU = 0, MFO_GG_TT = 1, MFO_GG_TTG = 2, MFO_GG_TTGG = 3 };
+enum { MFO_EE_MUMU = 0, MFO_GG_TT = 1, MFO_GG_TTG = 2, MFO_GG_TTGG = 3,
+       MFO_QQ_TT = 4 };        /* q q~ -> t t~ summed over the five light flavours     */
 
 typedef struct {
   int32_t  process;            /* MFO_*                                                          */
@@ -40,7 +41,17 @@ typedef struct {
   uint32_t pdf_nx, pdf_nq;
   double   pdf_xmin, pdf_xmax, pdf_qmin, pdf_qmax;
   uint32_t generator;          /* MFO_GEN_* flags; 0 = the generators of the configs   */
+  uint32_t pdf_nf;             /* flavour tables in pdf_xf: 0 or 1 = the gluon table [nx][nq] (processes 1-3);
+                                * 11 = [11][nx][nq], flavour index = PDG id + 5 (b~ c~ s~ u~ d~ g d u s c b),
+                                * required by MFO_QQ_TT (flavour-summed PDFs)                  */
 } mfo_config_t;
+/* MFO_QQ_TT ("any process generated (at LO)"): one diagram, s-channel gluon,
+ *   M = g_s^2 T^a_{ji} T^a_{kl} [vbar(pb) gamma^mu u(pa)] [ubar(k1) gamma_mu v(k2)] / shat,
+ * averaged over 4 helicities x 9 colours of the incoming pair (O6q).  Same 2-body kinematics and VEGAS
+ * dimensions as MFO_GG_TT.  The parton luminosity is summed over flavours and both beam orientations:
+ *   F = J_V J_x [sum_{q=1..5} f_q(x1) f_q~(x2) + f_q~(x1) f_q(x2)] |M|^2 W_PS K / (2 shat)
+ * (|M|^2 is symmetric under the exchange of the beams); the per-event record pdf[2] holds the two sums
+ * sum_q xf_q(x1) xf_q~(x2) and sum_q xf_q~(x1) xf_q(x2).  Selectable generators apply as for process 1.   */
 /* selectable generators (processes 1-3):
  *  MFO_GEN_CLASSIC_RAMBO  textbook RAMBO (Kleiss, Stirling, Ellis 1986) with 4n uniforms instead of the 3n-4-random
  *                         sequential form; VEGAS dimensions d = 2 + 4n (mfo_rambo_classic)

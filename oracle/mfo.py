@@ -30,7 +30,7 @@ class Config(C.Structure):
                 ("gev2_to_pb", C.c_double), ("pdf_xf", C.POINTER(C.c_double)),
                 ("pdf_nx", C.c_uint32), ("pdf_nq", C.c_uint32), ("pdf_xmin", C.c_double),
                 ("pdf_xmax", C.c_double), ("pdf_qmin", C.c_double), ("pdf_qmax", C.c_double),
-                ("generator", C.c_uint32)]
+                ("generator", C.c_uint32), ("pdf_nf", C.c_uint32)]
 
 
 class EvalOut(C.Structure):
@@ -235,7 +235,8 @@ class Vegas:
             setattr(c, k, cfg[k])
         c.generator = int(cfg.get("generator", 0))
         if self._pdf is not None:
-            c.pdf_xf = self._pdf.ctypes.data_as(C.POINTER(C.c_double)); c.pdf_nx, c.pdf_nq = self._pdf.shape
+            c.pdf_xf = self._pdf.ctypes.data_as(C.POINTER(C.c_double)); c.pdf_nx, c.pdf_nq = self._pdf.shape[-2:]
+            c.pdf_nf = self._pdf.shape[0] if self._pdf.ndim == 3 else 1
         self._h = C.c_void_p()
         _check(lib().mfo_vegas_create(C.byref(c), C.byref(self._h)))
         d, nf = C.c_uint32(), C.c_uint32(); lib().mfo_ndim(self._h, C.byref(d), C.byref(nf))

@@ -443,10 +443,40 @@ static double me2_eemumu(const double *mom, double alpha_em) {
   return (double)(tot / 4.0L);
 }
 
+// O6q  q q~ -> t t~: M = g_s^2 T^a_{ji} T^a_{kl} [vbar(pb) gamma^mu u(pa)] [ubar(k1) gamma_mu v(k2)] / shat;
+// sum over the helicities and over the colours i, j (incoming) and k, l (outgoing) of |M|^2, averaged over the
+// 4 helicities and 9 colours of the incoming pair.  The colour sum is taken literally from the Gell-Mann matrices.
+static double me2_qqtt(const double *mom, double m_top, double alpha_s) {
+  init_su3();
+  double g2 = 4.0 * M_PI * alpha_s;
+  double s = (mom[0] + mom[4]) * (mom[0] + mom[4]) - (mom[1] + mom[5]) * (mom[1] + mom[5]) -
+             (mom[2] + mom[6]) * (mom[2] + mom[6]) - (mom[3] + mom[7]) * (mom[3] + mom[7]);
+  long double col = 0;                                     // sum_{ijkl} |sum_a T^a_{ji} T^a_{kl}|^2
+  for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) for (int k = 0; k < 3; ++k) for (int l = 0; l < 3; ++l) {
+    cd c = 0;
+    for (int a = 0; a < 8; ++a) c += TA[a].m[j][i] * TA[a].m[k][l];
+    col += std::norm(c);
+  }
+  long double tot = 0;
+  for (int h = 0; h < 16; ++h) {
+    int la = (h & 1) ? 1 : -1, lb = (h & 2) ? 1 : -1, l1 = (h & 4) ? 1 : -1, l2 = (h & 8) ? 1 : -1;
+    Sp ua = wf_fermion(0, mom, 0.0, la);                   // incoming q
+    Sp vbb = adjoint(wf_fermion(1, mom + 4, 0.0, lb));     // incoming q~
+    Sp ub1 = adjoint(wf_fermion(0, mom + 8, m_top, l1));   // outgoing t
+    Sp v2 = wf_fermion(1, mom + 12, m_top, l2);            // outgoing t~
+    V4 L, R;
+    for (int mu = 0; mu < 4; ++mu) { L.c[mu] = rowcol(vbb, matvec(GAM[mu], ua)); R.c[mu] = rowcol(ub1, matvec(GAM[mu], v2)); }
+    cd M = g2 * mdot(L, R) / s;
+    tot += std::norm(M);
+  }
+  return (double)(tot * col / 36.0L);
+}
+
 static void hel_from_index(int h, int nleg, int *hel) { for (int l = 0; l < nleg; ++l) hel[l] = (h >> l & 1) ? 1 : -1; }
 
 extern "C" int mfo_me2(int process, const double *mom, double m_top, double alpha_s, double alpha_em, double *out) {
   if (process == MFO_EE_MUMU) { *out = me2_eemumu(mom, alpha_em); return MFO_OK; }
+  if (process == MFO_QQ_TT) { *out = me2_qqtt(mom, m_top, alpha_s); return MFO_OK; }
   int ng = process_ng(process); if (ng < 0) return MFO_EINVAL;
   const Table &t = table(ng); int nleg = ng + 2; long double tot = 0;
   std::vector<cd> jamp;

@@ -30,12 +30,12 @@ struct mfo_vegas {
 
 extern "C" int mfo_vegas_create(const mfo_config_t *cfg, mfo_vegas_t **out) {
   if (!cfg || !out) { g_err = "null argument"; return MFO_EINVAL; }
-  if (cfg->process < 0 || cfg->process > 3) { g_err = "unknown process"; return MFO_EINVAL; }
+  if (cfg->process < 0 || cfg->process > 4) { g_err = "unknown process"; return MFO_EINVAL; }
   if (cfg->n_bins < 1 || cfg->n_bins > 255) { g_err = "n_bins out of range"; return MFO_EINVAL; }
   if (!(cfg->sqrt_s > 0)) { g_err = "sqrt_s must be positive"; return MFO_EINVAL; }
   mfo_vegas *h = new (std::nothrow) mfo_vegas(); if (!h) return MFO_ENOMEM;
   h->cfg = *cfg;
-  static const uint32_t nfin[4] = {2, 2, 3, 4};
+  static const uint32_t nfin[5] = {2, 2, 3, 4, 2};
   h->n_final = nfin[cfg->process];
   h->d = (cfg->process == MFO_EE_MUMU) ? 2 : 2 + 3 * h->n_final - 4;
   if (cfg->generator & ~(uint32_t)(MFO_GEN_CLASSIC_RAMBO | MFO_GEN_LINEAR_TAU)) { g_err = "unknown generator flag"; delete h; return MFO_EINVAL; }
@@ -45,7 +45,10 @@ extern "C" int mfo_vegas_create(const mfo_config_t *cfg, mfo_vegas_t **out) {
   h->sym = 1.0; h->shat_min = 0;
   if (cfg->process != MFO_EE_MUMU) {
     if (!cfg->pdf_xf || cfg->pdf_nx < 2 || cfg->pdf_nq < 2) { g_err = "pdf grid required"; delete h; return MFO_EINVAL; }
-    h->pdf.assign(cfg->pdf_xf, cfg->pdf_xf + (size_t)cfg->pdf_nx * cfg->pdf_nq); h->cfg.pdf_xf = h->pdf.data();
+    const uint32_t nf = cfg->pdf_nf ? cfg->pdf_nf : 1;
+    if (nf != 1 && nf != 11) { g_err = "pdf_nf must be 0, 1 or 11"; delete h; return MFO_EINVAL; }
+    if ((cfg->process == MFO_QQ_TT) != (nf == 11)) { g_err = "process 4 needs the 11-flavour grid, processes 1-3 the gluon table"; delete h; return MFO_EINVAL; }
+    h->pdf.assign(cfg->pdf_xf, cfg->pdf_xf + (size_t)nf * cfg->pdf_nx * cfg->pdf_nq); h->cfg.pdf_xf = h->pdf.data();
     h->masses[0] = h->masses[1] = cfg->m_top;
     uint32_t ngl = h->n_final - 2;
     double thr = 2.0 * cfg->m_top + ngl * (cfg->ptmin_g > 0 ? cfg->ptmin_g : 0.0);   // O3: shat_min = (sum m + sum pTmin)^2
@@ -103,6 +106,20 @@ static double one_event(const mfo_vegas *h, uint32_t iteration, uint64_t ev, Eve
   uint32_t ngl = n - 2;
   if (ngl > 0) R.pass = mfo_cuts(ngl, k + 8, x1, x2, c.ptmin_g, c.etamax_g, c.drmin_gg, nullptr);   // O7
   double q2 = c.mu_f * c.mu_f;
+  if (c.process == MFO_QQ_TT) {                                           // O5q: flavour-summed luminosity
+    const size_t tab = (size_t)c.pdf_nx * c.pdf_nq;                       // table of PDG id f at index f + 5
+    long double l12 = 0, l21 = 0;
+    for (int f = 1; f <= 5; ++f) {
+      double q1 = mfo_pdf_interp(c.pdf_xf + (5 + f) * tab, c.pdf_nx, c.pdf_nq, c.pdf_xmin, c.pdf_xmax, c.pdf_qmin, c.pdf_qmax, x1, q2);
+      double a1 = mfo_pdf_interp(c.pdf_xf + (5 - f) * tab, c.pdf_nx, c.pdf_nq, c.pdf_xmin, c.pdf_xmax, c.pdf_qmin, c.pdf_qmax, x1, q2);
+      double q2_ = mfo_pdf_interp(c.pdf_xf + (5 + f) * tab, c.pdf_nx, c.pdf_nq, c.pdf_xmin, c.pdf_xmax, c.pdf_qmin, c.pdf_qmax, x2, q2);
+      double a2 = mfo_pdf_interp(c.pdf_xf + (5 - f) * tab, c.pdf_nx, c.pdf_nq, c.pdf_xmin, c.pdf_xmax, c.pdf_qmin, c.pdf_qmax, x2, q2);
+      l12 += (long double)q1 * a2; l21 += (long double)a1 * q2_;
+    }
+    R.pdf[0] = (double)l12; R.pdf[1] = (double)l21;
+    mfo_me2(c.process, m, c.m_top, c.alpha_s, c.alpha_em, &R.me2);        // O6q
+    return JV * Jx * ((R.pdf[0] + R.pdf[1]) / (x1 * x2)) * R.me2 * h->sym * w3[0] * w3[1] * c.gev2_to_pb / (2.0 * shat);
+  }
   R.pdf[0] = mfo_pdf_interp(c.pdf_xf, c.pdf_nx, c.pdf_nq, c.pdf_xmin, c.pdf_xmax, c.pdf_qmin, c.pdf_qmax, x1, q2);   // O5
   R.pdf[1] = mfo_pdf_interp(c.pdf_xf, c.pdf_nx, c.pdf_nq, c.pdf_xmin, c.pdf_xmax, c.pdf_qmin, c.pdf_qmax, x2, q2);
   if (!R.pass) return 0.0;

@@ -1,0 +1,137 @@
+"""Pins of the oracle's quark channel (q q~ -> t t~ with flavour-summed PDFs on an
+11-flavour synthetic grid; readings O5q, O6q of DESIGN.md).  Checked against what the mathematics fixes: the
+textbook closed form of the spin/colour-averaged |M|^2, the textbook partonic cross section (by angular
+quadrature of the oracle's |M|^2), Lorentz invariance and beam-exchange symmetry, the flavour sum rebuilt from
+single-table interpolations, and the hadronic cross section by nested quadrature through the whole chain."""
+import math
+
+import numpy as np
+from scipy import integrate
+
+from paper_2105_10529_b200 import workloads as W
+
+MT, AS = 173.0, 0.118
+
+
+def tt_momenta(rts, ct, phi, m=MT):
+    E = rts / 2; p = math.sqrt(E * E - m * m); st = math.sqrt(1 - ct * ct)
+    k = np.array([E, p * st * math.cos(phi), p * st * math.sin(phi), p * ct])
+    return np.array([[E, 0, 0, E], [E, 0, 0, -E], k, [E, -k[1], -k[2], -k[3]]])
+
+
+def mdot(a, b):
+    return a[0] * b[0] - a[1] * b[1] - a[2] * b[2] - a[3] * b[3]
+
+
+def qq_tt_closed_form(mom, m=MT, alpha_s=AS):
+    """sum-bar |M|^2 = (4 g^4 / 9) [(m^2 - t)^2 + (m^2 - u)^2 + 2 m^2 s] / s^2  (Combridge 1979; Ellis-Stirling-Webber
+    table 10.2 in the massive case)"""
+    g4 = (4 * math.pi * alpha_s) ** 2
+    s = mdot(mom[0] + mom[1], mom[0] + mom[1])
+    t = mdot(mom[0] - mom[2], mom[0] - mom[2]); u = mdot(mom[0] - mom[3], mom[0] - mom[3])
+    return 4 * g4 / 9 * ((m * m - t) ** 2 + (m * m - u) ** 2 + 2 * m * m * s) / s ** 2
+
+
+def sighat_qq(shat, m=MT, alpha_s=AS):
+    """sigma_hat(q q~ -> Q Q~) = 8 pi alpha_s^2 / (27 shat) * beta * (1 + rho/2), rho = 4 m^2 / shat
+    (Nason, Dawson, Ellis 1988: f_qq~ = pi beta rho (2 + rho) / 27 in units alpha_s^2 / m^2)"""
+    rho = 4 * m * m / shat; beta = math.sqrt(max(1 - rho, 0.0))
+    return 8 * math.pi * alpha_s ** 2 / (27 * shat) * beta * (1 + rho / 2)
+
+
+def test_qq_tt_closed_form_per_event(mfo):
+    rng = np.random.default_rng(5)
+    for _ in range(80):
+        rts = math.exp(rng.uniform(math.log(347.0), math.log(13000.0)))
+        m = tt_momenta(rts, rng.uniform(-0.9999, 0.9999), rng.uniform(0, 2 * math.pi))
+        assert np.isclose(mfo.me2(W.QQ_TT, m), qq_tt_closed_form(m), rtol=2e-12)
+    # massless limit = the QED-like 1 + cos^2 shape: (4 g^4/9) (t^2 + u^2)/s^2 = (2 g^4/9)(1 + cos^2 theta)
+    m = tt_momenta(1000.0, 0.3, 0.7, m=1e-9)
+    g4 = (4 * math.pi * AS) ** 2
+    assert np.isclose(mfo.me2(W.QQ_TT, m, m_top=1e-9), 2 * g4 / 9 * (1 + 0.09), rtol=1e-10)
+    # threshold: t = u = -m^2, s = 4 m^2: (4 g^4/9) (4 m^4 + 4 m^4 + 8 m^4) / (16 m^4) = 4 g^4 / 9
+    m = tt_momenta(2 * MT * (1 + 1e-9), 0.5, 0.1)
+    assert np.isclose(mfo.me2(W.QQ_TT, m), 4 * g4 / 9, rtol=1e-7)
+
+
+def test_qq_tt_symmetries(mfo):
+    """beam exchange (t <-> u), azimuthal rotation, and a boost along the beam leave |M|^2 unchanged"""
+    m = tt_momenta(800.0, 0.41, 0.9)
+    ref = mfo.me2(W.QQ_TT, m)
+    sw = m.copy(); sw[[0, 1]] = sw[[1, 0]]
+    assert np.isclose(mfo.me2(W.QQ_TT, sw), ref, rtol=1e-12)
+    assert np.isclose(mfo.me2(W.QQ_TT, tt_momenta(800.0, 0.41, 2.3)), ref, rtol=1e-12)
+    assert np.isclose(mfo.me2(W.QQ_TT, tt_momenta(800.0, -0.41, 0.9)), ref, rtol=1e-12)
+    y = 0.7; ch, sh = math.cosh(y), math.sinh(y)
+    b = m.copy(); b[:, 0] = ch * m[:, 0] + sh * m[:, 3]; b[:, 3] = sh * m[:, 0] + ch * m[:, 3]
+    assert np.isclose(mfo.me2(W.QQ_TT, b), ref, rtol=1e-11)
+
+
+def test_sigma_hat_qq(mfo):
+    xs, ws = np.polynomial.legendre.leggauss(16)
+    for rts in (350.0, 400.0, 700.0, 3000.0):
+        shat = rts * rts; beta = math.sqrt(1 - 4 * MT * MT / shat)
+        ang = sum(w * mfo.me2(W.QQ_TT, tt_momenta(rts, x, 0.3)) for x, w in zip(xs, ws))
+        sig = ang * beta / (16 * math.pi) / (2 * shat)
+        assert np.isclose(sig, sighat_qq(shat), rtol=1e-11)
+
+
+def test_flavour_grid_and_luminosity_record(mfo):
+    """the 11-flavour input grid (index = PDG id + 5), and the per-event flavour sums against single-table lookups"""
+    g = W.synthetic_flavour_grid()
+    assert g.shape == (11, W.PDF_NX, W.PDF_NQ)
+    assert np.array_equal(g[5], W.synthetic_gluon_grid())
+    assert (g[:, -1, :] == 0).all() and (g[:, :-1, :] > 0).all()
+    assert np.array_equal(g[2], g[8]) and np.array_equal(g[1], g[9]) and np.array_equal(g[0], g[10])   # s, c, b: sea only
+    assert (g[7, :-1] > g[3, :-1]).all() and (g[6, :-1] > g[4, :-1]).all()                               # u > u~, d > d~
+    # valence number sum rules of the synthetic shapes: int (u - u~) dx = 2.2 B(0.5, 4), int (d - d~) dx = 1.1 B(0.5, 5)
+    lx = np.linspace(math.log(W.PDF_XMIN), 0.0, W.PDF_NX)
+    for fl, exact in ((2, 2.2 * math.gamma(0.5) * math.gamma(4) / math.gamma(4.5)), (1, 1.1 * math.gamma(0.5) * math.gamma(5) / math.gamma(5.5))):
+        num = integrate.trapezoid(g[5 + fl, :, 0] - g[5 - fl, :, 0], lx)       # int x f dln x
+        assert abs(num / exact - 1) < 2e-2
+    cfg = W.config(W.QQ_TT, seed=3)
+    v = mfo.Vegas(cfg)
+    assert v.d == 4 and v.n_final == 2
+    out = v.eval(0, 0, 50)
+    a = (W.PDF_XMIN, W.PDF_XMAX, W.PDF_QMIN, W.PDF_QMAX)
+    s = cfg["sqrt_s"] ** 2
+    for i in range(50):
+        mom = out["momenta"][i]; shat = 4 * mom[0, 0] ** 2
+        x1, x2, _, jx = mfo.x_map(out["x"][i, 0], out["x"][i, 1], s, 4 * MT * MT)
+        assert np.isclose(x1 * x2 * s, shat, rtol=1e-13)
+        f = lambda fl, x: mfo.pdf_interp(g[5 + fl], *a, x, MT * MT)
+        l12 = sum(f(q, x1) * f(-q, x2) for q in range(1, 6)); l21 = sum(f(-q, x1) * f(q, x2) for q in range(1, 6))
+        assert np.allclose(out["pdf"][i], [l12, l21], rtol=1e-13)
+        assert np.isclose(out["me2"][i], qq_tt_closed_form(mom), rtol=2e-12)
+        # weight chain on the uniform grid (J_V = 1): F = J_x (L12 + L21)/(x1 x2) |M|^2 /(8 pi) beta K / (2 shat)
+        beta = math.sqrt(1 - 4 * MT * MT / shat)
+        F = jx * (l12 + l21) / (x1 * x2) * out["me2"][i] / (8 * math.pi) * beta * 0.3894e9 / (2 * shat)
+        assert np.isclose(out["weight"][i], F, rtol=1e-11)
+
+
+def test_qq_tt_cross_section_against_quadrature(mfo):
+    """sigma = sum_q int dx1 dx2 [f_q(x1) f_q~(x2) + f_q~(x1) f_q(x2)] sigma_hat(x1 x2 s): nested quadrature with the
+    interpolated flavour tables and the closed-form sigma_hat, against the oracle's VEGAS chain (both tau maps)."""
+    g = W.synthetic_flavour_grid(); a = (W.PDF_XMIN, W.PDF_XMAX, W.PDF_QMIN, W.PDF_QMAX)
+    s = 13000.0 ** 2; tau0 = 4 * MT * MT / s
+    xf = lambda fl, x: mfo.pdf_interp(g[5 + fl], *a, x, MT * MT)
+    knots = np.linspace(math.log(1e-6), 0, 100)
+
+    def lum(lt):        # int d ln x1 of sum_q [x1 f_q(x1) x2 f_q~(x2) + (q <-> q~)], x2 = tau/x1
+        tau = math.exp(lt)
+        pts = sorted(set([lt, 0.0] + [k for k in knots if lt < k < 0] + [lt - k for k in knots if lt < lt - k < 0]))
+
+        def integrand(l1):
+            x1 = math.exp(l1); x2 = tau / x1
+            return sum(xf(q, x1) * xf(-q, x2) + xf(-q, x1) * xf(q, x2) for q in range(1, 6))
+        return sum(integrate.fixed_quad(np.vectorize(integrand), p, q, n=6)[0] for p, q in zip(pts[:-1], pts[1:]))
+    edges = np.linspace(math.log(tau0), 0, 31)
+    tot = sum(integrate.fixed_quad(np.vectorize(lambda lt: lum(lt) * sighat_qq(math.exp(lt) * s)), p, q, n=8)[0]
+              for p, q in zip(edges[:-1], edges[1:]))
+    sigma_q = tot * 0.3894e9
+    for gen in (0, W.GEN_LINEAR_TAU):
+        v = mfo.Vegas(W.config(W.QQ_TT, seed=0, generator=gen))
+        for _ in range(5):
+            v.iterate(100_000, n_threads=mfo.max_threads())
+        r = v.result()
+        assert abs(r["integral"] - sigma_q) < 4 * r["sigma"] and r["sigma"] / sigma_q < 3e-3, (gen, r, sigma_q)

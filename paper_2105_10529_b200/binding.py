@@ -33,7 +33,8 @@ class Config(C.Structure):
                 ("ptmin_g", C.c_double), ("etamax_g", C.c_double), ("drmin_gg", C.c_double),
                 ("gev2_to_pb", C.c_double), ("pdf_xf", C.POINTER(C.c_double)),
                 ("pdf_nx", C.c_uint32), ("pdf_nq", C.c_uint32), ("pdf_xmin", C.c_double),
-                ("pdf_xmax", C.c_double), ("pdf_qmin", C.c_double), ("pdf_qmax", C.c_double)]
+                ("pdf_xmax", C.c_double), ("pdf_qmin", C.c_double), ("pdf_qmax", C.c_double),
+                ("pdf_nf", C.c_uint32), ("reserved1", C.c_uint32)]
 
 
 class EvalOut(C.Structure):
@@ -63,7 +64,8 @@ def make_config(cfg: dict):
     if cfg.get("pdf_xf") is not None:
         pdf = np.ascontiguousarray(cfg["pdf_xf"], dtype=np.float64)
         c.pdf_xf = pdf.ctypes.data_as(C.POINTER(C.c_double))
-        c.pdf_nx, c.pdf_nq = pdf.shape
+        c.pdf_nx, c.pdf_nq = pdf.shape[-2:]
+        c.pdf_nf = pdf.shape[0] if pdf.ndim == 3 else 1
     return c, pdf
 
 

@@ -18,7 +18,7 @@ def _newer(target, deps):
     return os.path.exists(target) and all(os.path.getmtime(target) >= os.path.getmtime(d) for d in deps)
 
 
-def build(force=False, verbose=False, extra_flags=(), tag="", only=(0, 1, 2, 3)):
+def build(force=False, verbose=False, extra_flags=(), tag="", only=(0, 1, 2, 3, 4)):
     """tag/extra_flags/only: tuning variants (objects and library get the tag as a suffix)"""
     global OBJ, LIB
     obj_dir = OBJ + tag
@@ -31,7 +31,7 @@ def build(force=False, verbose=False, extra_flags=(), tag="", only=(0, 1, 2, 3))
     api = kern + [os.path.join(CSRC, f) for f in ("mf_small_kernels.cuh", "mf_params.h")]
     api += [os.path.join(os.path.dirname(HERE), "include", "madflow_b200.h")]
     jobs = [("mf_api.o", os.path.join(CSRC, "mf_api.cu"), [])]
-    jobs += [("mf_proc%d.o" % p, os.path.join(CSRC, "mf_proc.cu" if p in only else "mf_proc_stub.cu"), ["-DMF_PROC=%d" % p]) for p in range(4)]
+    jobs += [("mf_proc%d.o" % p, os.path.join(CSRC, "mf_proc.cu" if p in only else "mf_proc_stub.cu"), ["-DMF_PROC=%d" % p]) for p in range(5)]
 
     def compile_one(job):
         obj, src, extra = job
@@ -45,7 +45,7 @@ def build(force=False, verbose=False, extra_flags=(), tag="", only=(0, 1, 2, 3))
             raise RuntimeError("nvcc failed for %s:\n%s" % (obj, (r.stdout + r.stderr)[-4000:]))
         return obj, "compiled"
 
-    with ThreadPoolExecutor(max_workers=5) as ex:
+    with ThreadPoolExecutor(max_workers=6) as ex:
         results = list(ex.map(compile_one, jobs))
     objs = [os.path.join(obj_dir, j[0]) for j in jobs]
     if force or not _newer(lib, objs):

@@ -79,7 +79,8 @@ extern "C" int mf_vegas_create(const mf_config_t* cfg, mf_vegas_t** out) {
   h->use_staged = h->rec_fields > 0;
   h->f32 = cfg->precision == 32;
   h->max_blocks = h->n_sm * 32;
-  const size_t ne = (size_t)P.d * (P.nb + 1), npdf = (size_t)P.pdf_nx * P.pdf_nq;
+  const bool flavours = cfg->process == MF_QQ_TT;      // 11-flavour grid: the ten quark tables, flavour-innermost
+  const size_t ne = (size_t)P.d * (P.nb + 1), ntab = (size_t)P.pdf_nx * P.pdf_nq, npdf = flavours ? ntab * MF_NQF : ntab;
   MF_CREATE_CUDA(cudaMalloc(&h->d_edges, ne * sizeof(double)));
   MF_CREATE_CUDA(cudaMalloc(&h->d_pdf, (npdf ? npdf : 1) * sizeof(double)));
   MF_CREATE_CUDA(cudaMalloc(&h->d_partial, (size_t)h->max_blocks * h->row * sizeof(double)));
@@ -96,7 +97,15 @@ extern "C" int mf_vegas_create(const mf_config_t* cfg, mf_vegas_t** out) {
   for (int j = 0; j < P.d; ++j)
     for (int k = 0; k <= P.nb; ++k) e[(size_t)j * (P.nb + 1) + k] = (double)k / (double)P.nb;
   MF_CREATE_CUDA(cudaMemcpy(h->d_edges, e.data(), ne * sizeof(double), cudaMemcpyHostToDevice));
-  if (npdf) MF_CREATE_CUDA(cudaMemcpy(h->d_pdf, cfg->pdf_xf, npdf * sizeof(double), cudaMemcpyHostToDevice));
+  if (flavours) {                                        // host [11][nx][nq] (index = PDG id + 5) -> device [nx][nq][MF_NQF]
+    std::vector<double> t(npdf);
+    for (int f = 0; f < 11; ++f) {
+      if (f == 5) continue;                                // the gluon table is not used by q q~ -> t t~
+      const int slot = f < 5 ? f : f - 1;                  // slots 0..4 = b~ c~ s~ u~ d~ (5 - q), 5..9 = d u s c b (4 + q)
+      for (size_t i = 0; i < ntab; ++i) t[i * MF_NQF + slot] = cfg->pdf_xf[(size_t)f * ntab + i];
+    }
+    MF_CREATE_CUDA(cudaMemcpy(h->d_pdf, t.data(), npdf * sizeof(double), cudaMemcpyHostToDevice));
+  } else if (npdf) MF_CREATE_CUDA(cudaMemcpy(h->d_pdf, cfg->pdf_xf, npdf * sizeof(double), cudaMemcpyHostToDevice));
   MF_CREATE_CUDA(cudaEventCreate(&h->ev0));
   MF_CREATE_CUDA(cudaEventCreate(&h->ev1));
   MF_CREATE_CUDA(cudaEventCreate(&h->evk0));
@@ -439,10 +448,11 @@ extern "C" int mf_set_grid(mf_vegas_t* h, const double* e) {
 
 extern "C" int mf_me_flops(const mf_vegas_t* h, uint64_t* n_add, uint64_t* n_mul, uint64_t* n_fma) {
   if (!h) return fail(MF_EINVAL, "handle is NULL");
-  static const uint64_t T[4][3] = {{MF_ME2_EE_MUMU_NADD, MF_ME2_EE_MUMU_NMUL, MF_ME2_EE_MUMU_NFMA},
+  static const uint64_t T[5][3] = {{MF_ME2_EE_MUMU_NADD, MF_ME2_EE_MUMU_NMUL, MF_ME2_EE_MUMU_NFMA},
                                    {MF_ME2_GG_TT_NADD, MF_ME2_GG_TT_NMUL, MF_ME2_GG_TT_NFMA},
                                    {MF_ME2_GG_TTG_NADD, MF_ME2_GG_TTG_NMUL, MF_ME2_GG_TTG_NFMA},
-                                   {MF_ME2_GG_TTGG_NADD, MF_ME2_GG_TTGG_NMUL, MF_ME2_GG_TTGG_NFMA}};
+                                   {MF_ME2_GG_TTGG_NADD, MF_ME2_GG_TTGG_NMUL, MF_ME2_GG_TTGG_NFMA},
+                                   {MF_ME2_EE_MUMU_NADD, MF_ME2_EE_MUMU_NMUL, MF_ME2_EE_MUMU_NFMA}};   // q q~ -> t t~: the two-current code
   if (n_add) *n_add = T[h->P.process][0];
   if (n_mul) *n_mul = T[h->P.process][1];
   if (n_fma) *n_fma = T[h->P.process][2];

@@ -86,7 +86,11 @@ struct MfParams {
   double wconst;                        // S_f * K / 2  (O8: F = ... S_f W_PS K / (2 shat))
   double pdf_lx0, pdf_ihx, pdf_lq0, pdf_ihq, pdf_lq;   // ln xmin, 1/h_x, ln qmin^2, 1/h_q, ln muF^2
   int32_t pdf_nx, pdf_nq;
+  int32_t pdf_smem;                     // doubles of the PDF table staged in shared memory: nx*nq (gluon table), 0 for the
+                                        // 11-flavour grid of the quark channel (400 KB: read through L1/L2 from global memory)
 };
+#define MF_NQF 10                       // quark/antiquark tables of the flavour grid, device layout [nx][nq][MF_NQF]:
+                                        // slot 5 - q = antiquark, 4 + q = quark of flavour q = 1..5 (d u s c b)
 
 // ---- S1: Philox4x32-10 (Salmon et al. SC'11), reading O1/A1 ----------------------------------
 MF_HD uint32_t mf_mulhi32(uint32_t a, uint32_t b) {
@@ -334,8 +338,13 @@ MF_HD double mf_hermite(double fm1, double f0, double f1, double f2, bool has_m1
   return (2.0 * t3 - 3.0 * t2 + 1.0) * f0 + (t3 - 2.0 * t2 + t) * hd0 + (3.0 * t2 - 2.0 * t3) * f1 + (t3 - t2) * hd1;
 }
 
-// xf(x, Q^2) from the table `tab` [nx][nq] (shared memory on the device); lx = ln x, lq = ln Q^2
-MF_HD double mf_pdf(const MfParams& P, const double* tab, double lx, double lq) {
+// xf(x, Q^2) from the table `tab` [nx][nq] (shared memory on the device); lx = ln x, lq = ln Q^2.
+// STRIDE: doubles between neighbouring (ix, iq) entries (1 = single table; MF_NQF = flavour-innermost grid)
+template <int STRIDE>
+MF_HD double mf_pdf_strided(const MfParams& P, const double* tab, double lx, double lq);
+MF_HD double mf_pdf(const MfParams& P, const double* tab, double lx, double lq) { return mf_pdf_strided<1>(P, tab, lx, lq); }
+template <int STRIDE>
+MF_HD double mf_pdf_strided(const MfParams& P, const double* tab, double lx, double lq) {
   const int nx = P.pdf_nx, nq = P.pdf_nq;
   const double fx = (lx - P.pdf_lx0) * P.pdf_ihx, fq = (lq - P.pdf_lq0) * P.pdf_ihq;
   int ix = (int)floor(fx), iq = (int)floor(fq);
@@ -351,9 +360,22 @@ MF_HD double mf_pdf(const MfParams& P, const double* tab, double lx, double lq) 
   for (int c = 0; c < 4; ++c) {                     // Q^2 rows iq-1 .. iq+2 (clamped where absent)
     int q = iq - 1 + c;
     q = q < 0 ? 0 : (q > nq - 1 ? nq - 1 : q);
-    row[c] = mf_hermite(tab[r0 + q], tab[r1 + q], tab[r2 + q], tab[r3 + q], xm, xp, tx);
+    row[c] = mf_hermite(tab[(r0 + q) * STRIDE], tab[(r1 + q) * STRIDE], tab[(r2 + q) * STRIDE], tab[(r3 + q) * STRIDE], xm, xp, tx);
   }
   return mf_hermite(row[0], row[1], row[2], row[3], qm, qp, tq);
+}
+
+// O5q: flavour-summed q q~ luminosity from the flavour-innermost grid tab [nx][nq][MF_NQF] (global
+// memory): l12 = sum_q xf_q(x1) xf_q~(x2), l21 = sum_q xf_q~(x1) xf_q(x2), q = d u s c b.  The 16-point stencil of
+// one x is shared by the ten tables: each of its points is one contiguous 80-byte read.
+MF_HD void mf_lumi_qq(const MfParams& P, const double* tab, double lx1, double lx2, double lq, double& l12, double& l21) {
+  l12 = 0.0; l21 = 0.0;
+#pragma unroll
+  for (int q = 1; q <= 5; ++q) {
+    const double q1 = mf_pdf_strided<MF_NQF>(P, tab + 4 + q, lx1, lq), a1 = mf_pdf_strided<MF_NQF>(P, tab + 5 - q, lx1, lq);
+    const double q2 = mf_pdf_strided<MF_NQF>(P, tab + 4 + q, lx2, lq), a2 = mf_pdf_strided<MF_NQF>(P, tab + 5 - q, lx2, lq);
+    l12 = fma(q1, a2, l12); l21 = fma(a1, q2, l21);
+  }
 }
 
 // ---- S5: cuts (O7): final gluons only, lab frame; eta_lab = atanh(kz/|k|) + y_b, y_b = ln(x1/x2)/2 -----

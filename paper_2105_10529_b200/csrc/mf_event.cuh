@@ -21,6 +21,9 @@ template <> struct MfProc<0> { static const int D = 2, N = 2, NGL = 0, GROUP = 1
 template <> struct MfProc<1> { static const int D = 4, N = 2, NGL = 0, GROUP = 128; };
 template <> struct MfProc<2> { static const int D = 7, N = 3, NGL = 1, GROUP = 128; };
 template <> struct MfProc<3> { static const int D = 10, N = 4, NGL = 2, GROUP = 256; };
+// q q~ -> t t~ summed over five flavours: kinematics of process 1, PDF = flavour grid in global memory
+template <> struct MfProc<4> { static const int D = 4, N = 2, NGL = 0, GROUP = 128; };
+template <int PROC> struct MfPdf { static const bool FLAVOURS = PROC == 4; };
 // Generator selection of the front end, template parameter CL:
 //   0  the generators of the configs, nothing selectable (the path bench.py times: no branch)
 //   1  classic 4n-random RAMBO, d = 2 + 4n; the tau map (O3 or O3') is a run-time, grid-uniform branch on P.gen
@@ -75,6 +78,15 @@ MF_HD T mf_me2(const MfParams& P, T rts, const T k[MfProc<PROC>::N][4]) {
     mf_fermion_ing<T>(pa, T(0.0), in); mf_fermion_ing<T>(pb, T(0.0), in + 5);
     mf_fermion_ing<T>(k[0], T(0.0), in + 10); mf_fermion_ing<T>(k[1], T(0.0), in + 15);
     return T(P.me_pref) * mf_me2_ee_mumu<T>(in) / (rts * rts * rts * rts);      // e^4/4 * sum |L.R|^2 / s^2
+  } else if (PROC == 4) {
+    // O6q: the two-current contraction sum_hel |[vbar(pb) gamma^mu u(pa)][ubar(k1) gamma_mu v(k2)]|^2 of the generated
+    // e+e- -> mu+mu- code, with massive outgoing spinors; me_pref = g_s^4 (2/9) / 4 (colour sum 2, 9 colours, 4 spins)
+    T in[20];
+    const T E = T(0.5) * rts;
+    const T pa[4] = {E, T(0.0), T(0.0), E}, pb[4] = {E, T(0.0), T(0.0), -E};
+    mf_fermion_ing<T>(pa, T(0.0), in); mf_fermion_ing<T>(pb, T(0.0), in + 5);
+    mf_fermion_ing<T>(k[0], T(P.m_top), in + 10); mf_fermion_ing<T>(k[1], T(P.m_top), in + 15);
+    return T(P.me_pref) * mf_me2_ee_mumu<T>(in) / (rts * rts * rts * rts);
   } else if (PROC == 1) {
     static_assert(MF_ME2_GG_TT_NIN == 20, "generator input layout changed");
     T in[20];
@@ -116,7 +128,10 @@ MF_HD bool mf_event_front(const MfParams& P, const double* edges, const double* 
   rts = sqrt(shat);
   const bool pass = mf_cuts<NGL>(P, (const double(*)[4])(&k[0][0] + 8), x1, x2);   // S5 (final gluons = k[2..])
   double ff = 1.0, xf1 = 0.0, xf2 = 0.0;                                 // ff = f_g(x1) f_g(x2) / shat
-  if (PROC != 0 && (REC || pass)) {                                      // S6
+  if (MfPdf<PROC>::FLAVOURS) {                                           // S6q: flavour-summed luminosity (xf1, xf2 = the two sums)
+    mf_lumi_qq(P, pdf_tab, lx1, lx2, P.pdf_lq, xf1, xf2);
+    ff = (xf1 + xf2) / (x1 * x2 * shat);
+  } else if (PROC != 0 && (REC || pass)) {                               // S6
     xf1 = mf_pdf(P, pdf_tab, lx1, P.pdf_lq);
     xf2 = mf_pdf(P, pdf_tab, lx2, P.pdf_lq);
     ff = xf1 * xf2 / (x1 * x2 * shat);                                   // f_g = xf / x: one division for the three

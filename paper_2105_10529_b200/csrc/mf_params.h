@@ -8,12 +8,12 @@
 static_assert(MFD_GEN_CLASSIC == MF_GEN_CLASSIC_RAMBO && MFD_GEN_LINEAR == MF_GEN_LINEAR_TAU, "device flags follow the header");
 
 static inline int mf_process_shape(int process, uint32_t generator, int* d, int* n_final, int* ng) {
-  static const int nf[4] = {2, 2, 3, 4};
-  if (process < 0 || process > 3) return -1;
+  static const int nf[5] = {2, 2, 3, 4, 2};
+  if (process < 0 || process > 4) return -1;
   *n_final = nf[process];
   *d = (process == MF_EE_MUMU) ? 2 : 2 + 3 * nf[process] - 4;
   if (generator & MF_GEN_CLASSIC_RAMBO) *d = 2 + 4 * nf[process];       // O4': 4n uniforms
-  *ng = (process == MF_EE_MUMU) ? 0 : nf[process];      // gluon legs of gg -> t t~ + (n_final-2) g
+  *ng = (process == MF_EE_MUMU) ? 0 : nf[process];      // gluon legs of gg -> t t~ + (n_final-2) g (= powers of g_s^2; 2 for q q~ -> t t~)
   return 0;
 }
 
@@ -48,7 +48,10 @@ static inline int mf_fill_params(const mf_config_t* c, MfParams* P, std::string&
   } else {
     if (!(c->m_top > 0.0) || !(c->alpha_s > 0.0)) { err = "m_top and alpha_s must be positive"; return MF_EINVAL; }
     if (!c->pdf_xf || c->pdf_nx < 2 || c->pdf_nq < 2) { err = "pdf grid required"; return MF_EINVAL; }
-    if ((uint64_t)c->pdf_nx * c->pdf_nq * 8ull > 160ull * 1024ull) { err = "pdf grid larger than 160 KB"; return MF_EINVAL; }
+    const uint32_t nfl = c->pdf_nf ? c->pdf_nf : 1;
+    if (nfl != 1 && nfl != 11) { err = "pdf_nf must be 0, 1 or 11"; return MF_EINVAL; }
+    if ((c->process == MF_QQ_TT) != (nfl == 11)) { err = "process 4 needs the 11-flavour grid, processes 1-3 the gluon table"; return MF_EINVAL; }
+    if ((uint64_t)c->pdf_nx * c->pdf_nq * 8ull > 160ull * 1024ull) { err = "pdf table larger than 160 KB"; return MF_EINVAL; }
     if (!(c->pdf_xmin > 0.0 && c->pdf_xmax > c->pdf_xmin && c->pdf_qmin > 0.0 && c->pdf_qmax > c->pdf_qmin)) { err = "bad pdf ranges"; return MF_EINVAL; }
     const int ngl = nfin - 2;
     const double thr = 2.0 * c->m_top + ngl * (c->ptmin_g > 0.0 ? c->ptmin_g : 0.0);   // O3: shat_min
@@ -61,8 +64,10 @@ static inline int mf_fill_params(const mf_config_t* c, MfParams* P, std::string&
     for (int i = 0; i < ng; ++i) gs2n *= 4.0 * PI * c->alpha_s;
     const double scale = (c->process == MF_GG_TT) ? MF_ME2_GG_TT_SCALE : (c->process == MF_GG_TTG) ? MF_ME2_GG_TTG_SCALE : MF_ME2_GG_TTGG_SCALE;
     p.me_pref = gs2n / 256.0 * scale;                   // 1/4 helicities x 1/64 colours (A12)
+    if (c->process == MF_QQ_TT) p.me_pref = gs2n * (2.0 / 9.0) * MF_ME2_EE_MUMU_SCALE;   // O6q: colour sum 2 / 9 colours, 1/4 spins
     p.wconst = (ngl == 2 ? 0.5 : 1.0) * c->gev2_to_pb / 2.0;
     p.pdf_nx = (int)c->pdf_nx; p.pdf_nq = (int)c->pdf_nq;
+    p.pdf_smem = nfl == 1 ? p.pdf_nx * p.pdf_nq : 0;
     p.pdf_lx0 = log(c->pdf_xmin);
     p.pdf_ihx = (double)(c->pdf_nx - 1) / (log(c->pdf_xmax) - p.pdf_lx0);
     p.pdf_lq0 = log(c->pdf_qmin * c->pdf_qmin);

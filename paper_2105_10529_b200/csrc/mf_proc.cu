@@ -5,12 +5,18 @@
 #include "mf_kernels.cuh"
 #include "mf_proc.h"
 #ifndef MF_PROC
-#error "compile with -DMF_PROC=0..3"
+#error "compile with -DMF_PROC=0..4"
 #endif
+
+// the PDF table the event functions read: the staged copy, or (quark channel) the flavour grid in global memory
+template <int PROC>
+__device__ __forceinline__ const double* mf_pdf_ptr(const double* s_pdf, const double* g_pdf) {
+  return MfPdf<PROC>::FLAVOURS ? g_pdf : s_pdf;
+}
 
 __device__ __forceinline__ void mf_stage_tables(const MfParams& P, const double* g_edges, const double* g_pdf,
                                                 double* s_edges, double* s_pdf) {
-  const int ne = P.d * (P.nb + 1), np = P.pdf_nx * P.pdf_nq;
+  const int ne = P.d * (P.nb + 1), np = P.pdf_smem;      // np = 0: the flavour grid of the quark channel stays in global memory
   for (int i = threadIdx.x; i < ne; i += blockDim.x) s_edges[i] = g_edges[i];
   for (int i = threadIdx.x; i < np; i += blockDim.x) s_pdf[i] = g_pdf[i];
 }
@@ -143,7 +149,7 @@ mf_iterate_kernel(const MfParams P, const double* __restrict__ g_edges, const do
   const int nb = P.nb, nh = D * nb, nw = blockDim.x >> 5;
   double* s_edges = smem;
   double* s_pdf = s_edges + D * (nb + 1);
-  double* s_hist = s_pdf + P.pdf_nx * P.pdf_nq;          // [nw][D*nb]
+  double* s_hist = s_pdf + P.pdf_smem;                   // [nw][D*nb]
   double* s_red = s_hist + nw * nh;                      // [nw][4]
   double* s_obs = s_red + nw * 4;                        // [nw][MF_OBS_ACC] when observables are set
   mf_stage_tables(P, g_edges, g_pdf, s_edges, s_pdf);
@@ -166,10 +172,10 @@ mf_iterate_kernel(const MfParams P, const double* __restrict__ g_edges, const do
     double F = 0.0;
     unsigned okeys = 0;
     if (MF_UNIFORM_ME) {                                 // every thread runs the event (barriers inside);
-      F = mf_event<PROC, false, double, CL>(P, s_edges, s_pdf, iteration, first + (valid ? i : n - 1), bin, pass, nullptr, &okeys);
+      F = mf_event<PROC, false, double, CL>(P, s_edges, mf_pdf_ptr<PROC>(s_pdf, g_pdf), iteration, first + (valid ? i : n - 1), bin, pass, nullptr, &okeys);
       if (!valid) { F = 0.0; pass = false; }             // lanes past the end recompute event n-1, discarded
     } else if (valid) {
-      F = mf_event<PROC, false, double, CL>(P, s_edges, s_pdf, iteration, first + i, bin, pass, nullptr, &okeys);
+      F = mf_event<PROC, false, double, CL>(P, s_edges, mf_pdf_ptr<PROC>(s_pdf, g_pdf), iteration, first + i, bin, pass, nullptr, &okeys);
     }
     if (!isfinite(F)) { F = 0.0; ++n_bad; }              // A20
     if (valid && pass) ++n_pass;
@@ -203,7 +209,7 @@ mf_iterate_compact_kernel(const MfParams P, const double* __restrict__ g_edges, 
   const int nb = P.nb, nh = D * nb, nw = T >> 5;
   double* s_edges = smem;
   double* s_pdf = s_edges + D * (nb + 1);
-  double* s_hist = s_pdf + P.pdf_nx * P.pdf_nq;          // [nw][D*nb]
+  double* s_hist = s_pdf + P.pdf_smem;                   // [nw][D*nb]
   double* s_red = s_hist + nw * nh;                      // [nw][4]
   double* s_q = s_red + nw * 4;                          // [NF][CAP] field-major queue
   int* s_wtot = (int*)(s_q + NF * CAP);                  // [nw]
@@ -302,7 +308,7 @@ mf_front_kernel(const MfParams P, const double* __restrict__ g_edges, const doub
   extern __shared__ double smem[];
   double* s_edges = smem;
   double* s_pdf = s_edges + D * (P.nb + 1);
-  int* s_wtot = (int*)(s_pdf + P.pdf_nx * P.pdf_nq);    // [T/32]
+  int* s_wtot = (int*)(s_pdf + P.pdf_smem);             // [T/32]
   mf_stage_tables(P, g_edges, g_pdf, s_edges, s_pdf);
   __syncthreads();
   const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
@@ -486,8 +492,8 @@ mf_eval_kernel(const MfParams P, const double* __restrict__ g_edges, const doubl
   constexpr int N = MfProc<PROC>::N;
   extern __shared__ double smem[];
   double* s_edges = smem;
-  double* s_pdf = s_edges + P.d * (P.nb + 1);
-  mf_stage_tables(P, g_edges, g_pdf, s_edges, s_pdf);
+  const double* s_pdf = mf_pdf_ptr<PROC>(s_edges + P.d * (P.nb + 1), g_pdf);
+  mf_stage_tables(P, g_edges, g_pdf, s_edges, s_edges + P.d * (P.nb + 1));
   __syncthreads();
   const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
   for (unsigned long long base = (unsigned long long)blockIdx.x * blockDim.x; base < n; base += stride) {
@@ -528,7 +534,7 @@ static inline bool is_classic(const MfParams& P) { return kCL && (P.gen & MFD_GE
 static inline bool is_lintau(const MfParams& P) { return kLT && !is_classic(P) && (P.gen & MFD_GEN_LINEAR); }
 
 static cudaError_t proc_setup(const MfParams& P, size_t* smem_iter, size_t* smem_eval, int* occ_iter, int* occ_eval) {
-  const size_t tables = (size_t)P.d * (P.nb + 1) + (size_t)P.pdf_nx * P.pdf_nq;
+  const size_t tables = (size_t)P.d * (P.nb + 1) + (size_t)P.pdf_smem;
   const size_t nw = MF_THREADS / 32;
   *smem_eval = sizeof(double) * tables;
   *smem_iter = sizeof(double) * (tables + nw * P.d * P.nb + nw * 4);
@@ -613,7 +619,7 @@ static constexpr bool kStaged = MF_STAGED && MfProc<MF_PROC>::NGL > 0;
 static constexpr int kRecFields = MF_REC_FIELDS(MfProc<MF_PROC>::N);
 
 static size_t front_smem(const MfParams& P) {
-  return sizeof(double) * ((size_t)P.d * (P.nb + 1) + (size_t)P.pdf_nx * P.pdf_nq) + sizeof(int) * (MF_THREADS / 32);
+  return sizeof(double) * ((size_t)P.d * (P.nb + 1) + (size_t)P.pdf_smem) + sizeof(int) * (MF_THREADS / 32);
 }
 static size_t hist_smem(const MfParams& P) {
   return sizeof(double) * (MF_THREADS / 32) * ((size_t)P.d * P.nb + 4 + (P.n_obs > 0 ? MF_OBS_ACC : 0));

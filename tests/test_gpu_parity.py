@@ -28,7 +28,7 @@ def random_grid(d, nb, seed):
     return e
 
 
-def compare_events(out, ref, proc, mom_tol=(1e-11, 1e-9)):
+def compare_events(out, ref, proc, mom_tol=(1e-11, 1e-9), lumi_abs=0.0):
     g = {k: v.cpu().numpy() for k, v in out.items()}
     assert (g["bins"] == ref["bins"]).all()
     assert (g["pass_"] == ref["pass_"]).all()
@@ -46,6 +46,8 @@ def compare_events(out, ref, proc, mom_tol=(1e-11, 1e-9)):
     tol_w = np.full(int(nz.sum()), RTOL_EVENT)
     if proc:
         tol_w = tol_w + (1e-15 / np.abs(ref["pdf"][nz])).sum(axis=1)
+    if lumi_abs:            # quark channel: the weight carries the SUM of the two flavour sums, each good to lumi_abs absolutely
+        tol_w = tol_w + lumi_abs / np.abs(ref["pdf"][nz].sum(axis=1))
     assert (rel_w < tol_w).all(), (rel_w / tol_w).max()
 
 
@@ -398,3 +400,62 @@ def test_generator_variants_observables_errors_and_cross_section(mf, mfo):
             gpu.vegas_iterate(c["n_events"])
         r = gpu.result()
         assert abs(r["integral"] - 1074.393) < 5 * r["sigma"] + 0.02 and r["sigma"] < 1.5, (gen, r)
+
+
+# ---- quark channel: q q~ -> t t~, luminosity summed over five flavours on the 11-flavour grid
+@pytest.mark.parametrize("gen,n", [(0, 5003), (1, 5003), (2, 5003)])
+def test_quark_channel_per_event_parity(mf, mfo, gen, n):
+    cfg = W.config(W.QQ_TT, seed=8, generator=gen)
+    gpu, orc = mf.Vegas(cfg), mfo.Vegas(cfg)
+    assert gpu.d == orc.d == (10 if gen & 1 else 4) and gpu.n_final == 2
+    mom_tol = (1e-10, 1e-8) if gen & 1 else (1e-11, 1e-9)
+    ref = orc.eval(0, 0, n, n_threads=mfo.max_threads())
+    # proc = 0: the pdf record (the two flavour sums of ten products of O(1) interpolants, each good to 1e-15) is compared
+    # below; towards x -> 1 (sampled often by the linear-tau map) the sums go to zero and their absolute error shows
+    compare_events(gpu.integrand_eval(0, 0, n, debug=True), ref, 0, mom_tol, lumi_abs=2e-14)
+    e = random_grid(orc.d, 50, 300)
+    gpu.set_grid(e); orc.set_grid(e)
+    ref = orc.eval(4, 2**34 + 3, n, n_threads=mfo.max_threads())
+    out = gpu.integrand_eval(4, 2**34 + 3, n, debug=True)
+    compare_events(out, ref, 0, mom_tol, lumi_abs=2e-14)
+    np.testing.assert_allclose(out["pdf"].cpu().numpy(), ref["pdf"], rtol=1e-12, atol=1e-14)   # the two flavour sums
+    assert (ref["pdf"][:, 0] != ref["pdf"][:, 1]).all()      # the two beam orientations are distinct sums (valence quarks)
+
+
+def test_quark_channel_iterations_cross_section_and_errors(mf, mfo):
+    """fused iterations against the oracle (raw sums, histogram, grid), observables, the cross section against the
+    quadrature value pinned on the oracle side (tests/test_oracle_quarks.py), argument errors"""
+    cfg = W.config(W.QQ_TT, seed=0)
+    gpu, orc = mf.Vegas(cfg), mfo.Vegas(cfg)
+    obs = [(0, 20, 0.0, 400.0), (2, 16, 350.0, 1500.0)]
+    gpu.set_observables(obs)
+    n = 40_000
+    ref = [(np.zeros(o[1] + 2), np.zeros(o[1] + 2)) for o in obs]
+    for it in range(3):
+        for (a, b), (r1, r2) in zip(orc.observable_hist(it, 0, n, n, obs, n_threads=mfo.max_threads()), ref):
+            r1 += a; r2 += b
+        g = gpu.vegas_iterate(n)
+        o = orc.iterate(n, n_threads=mfo.max_threads())
+        assert g["n_pass"] == o["n_pass"] == n and g["n_nonfinite"] == 0
+        assert abs(g["integral"] / o["integral"] - 1) < RTOL_INT and abs(g["sigma"] / o["sigma"] - 1) < 1e-8
+        np.testing.assert_allclose(gpu.get_accum()[0][:2 + 4 * 50], orc.get_accum(), rtol=RTOL_INT, atol=1e-300)
+        np.testing.assert_allclose(gpu.get_grid(), orc.get_grid(), rtol=0, atol=1e-11)
+        gpu.set_grid(orc.get_grid())
+    got, n_it = gpu.get_observables()
+    for (g1, g2), (r1, r2) in zip(got, ref):
+        np.testing.assert_allclose(g1, r1, rtol=1e-10, atol=1e-13 * np.abs(r1).max())
+        np.testing.assert_allclose(g2, r2, rtol=1e-10, atol=1e-13 * np.abs(r2).max())
+    gpu = mf.Vegas(cfg)
+    for _ in range(5):
+        gpu.vegas_iterate(1_000_000)
+    r = gpu.result()
+    assert abs(r["integral"] - 79.96) < 5 * r["sigma"] + 0.03 and r["sigma"] < 0.05, r      # oracle: 79.961 +- 0.023 pb
+    with pytest.raises(mf.MfError) as e:
+        gpu.set_path(True)                                    # light process: fused path only
+    assert e.value.code == mf.MF_EUNSUPPORTED
+    for bad in (W.config(W.QQ_TT, pdf_xf=W.synthetic_gluon_grid()), W.config(W.GG_TT, pdf_xf=W.synthetic_flavour_grid()),
+                W.config(W.QQ_TT, precision=32)):
+        with pytest.raises(mf.MfError):
+            mf.Vegas(bad)
+    fl = gpu.me_flops()
+    assert fl["flops"] == mf.Vegas(W.config(W.EE_MUMU)).me_flops()["flops"]      # the two-current code

@@ -134,3 +134,46 @@ def test_generator_flag_validation(harness):
             d = np.frombuffer(P, dtype=np.int32, count=5)          # MfParams: process, d, n_final, nb, gen
             nf = {1: 2, 2: 3, 3: 4}[proc]
             assert d[0] == proc and d[2] == nf and d[4] == gen and d[1] == (2 + 4 * nf if gen & 1 else 3 * nf - 2)
+
+
+def flavour_innermost(pdf11):
+    """the library's device layout of the 11-flavour grid (mf_api.cu): ten quark tables, [nx][nq][10], gluon dropped"""
+    keep = [f for f in range(11) if f != 5]
+    return np.ascontiguousarray(np.transpose(pdf11[keep], (1, 2, 0)))
+
+
+@pytest.mark.parametrize("gen,n", [(0, 300), (1, 150), (2, 150)])
+def test_host_compiled_quark_channel_matches_oracle(mfo, harness, gen, n):
+    """q q~ -> t t~ with the flavour-summed luminosity of the product's per-event code, compiled for
+    the host, against the oracle: bins, momenta, the two flavour sums, |M|^2 and the weight"""
+    harness.mfh_event_gen.restype = C.c_double
+    harness.mfh_event_gen.argtypes = harness.mfh_event.argtypes
+    cfg = W.config(W.QQ_TT, seed=13, generator=gen)
+    c, pdf = make_config(cfg)
+    assert c.pdf_nf == 11
+    P = C.create_string_buffer(harness.mfh_params_size())
+    assert harness.mfh_fill_params(C.byref(c), P) == 0
+    tab = flavour_innermost(pdf)
+    orc = mfo.Vegas(cfg)
+    d = orc.d
+    edges = random_grid(d, 50, 31)
+    orc.set_grid(edges)
+    ref = orc.eval(1, 77, n)
+    bins = np.zeros(24, np.int32); ok = np.zeros(1, np.int32); rec = np.zeros(45)
+    worst = 0.0
+    for i in range(n):
+        F = harness.mfh_event_gen(P, edges.ctypes.data, tab.ctypes.data, 1, 77 + i, bins.ctypes.data, ok.ctypes.data, rec.ctypes.data)
+        assert list(bins[:d]) == list(ref["bins"][i]) and ok[0] == 1
+        np.testing.assert_allclose(rec[:d], ref["x"][i], rtol=1e-14, atol=0)
+        np.testing.assert_allclose(rec[18:34].reshape(4, 4), ref["momenta"][i], rtol=1e-10, atol=1e-8)
+        np.testing.assert_allclose(rec[43:45], ref["pdf"][i], rtol=1e-12, atol=1e-16)
+        worst = max(worst, abs(F / ref["weight"][i] - 1), abs(rec[42] / ref["me2"][i] - 1))
+    assert worst < 1e-10, worst
+    if gen == 0:                                              # and through the plain entry point
+        rec37 = np.zeros(37)
+        F = harness.mfh_event(P, edges.ctypes.data, tab.ctypes.data, 1, 77, bins.ctypes.data, ok.ctypes.data, rec37.ctypes.data)
+        assert abs(F / ref["weight"][0] - 1) < 1e-10
+    bad, _ = make_config(W.config(W.QQ_TT, pdf_xf=W.synthetic_gluon_grid()))     # needs the flavour grid
+    assert harness.mfh_fill_params(C.byref(bad), P) == -1
+    bad, _ = make_config(W.config(W.GG_TT, pdf_xf=W.synthetic_flavour_grid()))   # and the gluon processes the gluon table
+    assert harness.mfh_fill_params(C.byref(bad), P) == -1

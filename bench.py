@@ -278,6 +278,51 @@ def run_sweep(args):
                                       "its TFLOP/s are fp32 operations against the same fp64 peak, for reference only", "sweep": rows}))
 
 
+def run_processes(args):
+    """Every process and generator selection at its config size (configs 0-3; the quark channel and the selectable
+    generators of SURVEY 8(f)2/3 at the size of the process they vary): device time of whole iterations on the adapting
+    grid (warm-up iterations first), L2 flushed before every timed iteration.  One JSON line."""
+    import torch
+    from paper_2105_10529_b200 import binding, workloads as W
+    binding.lib()
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    peak = binding.fp64_peak(0, 0.3) / 1e12
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    sizes = {W.EE_MUMU: 100_000, W.GG_TT: 1_000_000, W.GG_TTG: 10_000_000, W.GG_TTGG: 1_000_000, W.QQ_TT: 1_000_000}
+    cases = [(W.EE_MUMU, 0), (W.GG_TT, 0), (W.GG_TT, 1), (W.GG_TT, 2), (W.QQ_TT, 0), (W.QQ_TT, 1),
+             (W.GG_TTG, 0), (W.GG_TTG, 1), (W.GG_TTG, 2), (W.GG_TTG, 3), (W.GG_TTGG, 0), (W.GG_TTGG, 1)]
+    rows = []
+    for proc, gen in cases:
+        n = sizes[proc]
+        h = binding.Vegas(W.config(proc, seed=0, generator=gen))
+        for _ in range(3):
+            h.vegas_iterate(n, sync=True)
+        flops = h.me_flops()["flops"]
+        ms, last = [], None
+        for _ in range(5):
+            flush.zero_()
+            torch.cuda.synchronize()
+            last = h.vegas_iterate(n, sync=True)
+            ms.append(h.last_kernel_ms()[1])
+        it_ms = sorted(ms)[len(ms) // 2]
+        row = {"process": W.PROCESS_NAMES[proc], "generator": gen, "d": h.d, "events": n, "iteration_ms": it_ms,
+               "events_per_s": n / (it_ms * 1e-3), "pass_fraction": last["n_pass"] / n,
+               "me_flops_per_event": flops, "whole_path_tflops": flops * last["n_pass"] / (it_ms * 1e-3) / 1e12}
+        row["whole_path_frac_of_fp64_peak"] = row["whole_path_tflops"] / peak
+        try:
+            st = h.last_stage_ms()
+            row["stages_ms"] = st
+        except binding.MfError:
+            row["stages_ms"] = None                                         # fused path
+        r = h.result()
+        row["integral_pb"], row["sigma_pb"] = r["integral"], r["sigma"]
+        rows.append(row)
+    print(json.dumps({"metric": "events/s of whole VEGAS iterations, every process and generator selection", "unit": "events/s",
+                      "dtype": "f64", "fp64_peak_tflops": peak, "timing": "median of 5 iterations after 3 warm-up iterations, "
+                      "CUDA events around mf_vegas_iterate, 256 MiB L2 flush before each", "rows": rows}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -287,6 +332,7 @@ def main():
     ap.add_argument("--events", type=int, default=N_EVENTS, help="events per iteration per GPU")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="configs[4]: events-per-launch sweep of the gg->tt~g integrand (1 GPU)")
+    ap.add_argument("--processes", action="store_true", help="every process / generator selection at its config size (1 GPU)")
     ap.add_argument("--path", default="staged", choices=["staged", "fused"],
                     help="staged: front end / |M|^2 / reductions as three kernels (default); fused: one kernel")
     args = ap.parse_args()
@@ -299,6 +345,10 @@ def main():
     if args.sweep:
         if rank == 0:
             run_sweep(args)
+        return
+    if args.processes:
+        if rank == 0:
+            run_processes(args)
         return
     run_ours(args, rank, local_rank, world)
     if world > 1:

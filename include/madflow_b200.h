@@ -71,8 +71,8 @@ typedef struct {
   double   pdf_xmin, pdf_xmax, pdf_qmin, pdf_qmax;
   uint32_t pdf_nf;           /* flavour tables in pdf_xf: 0 or 1 = the gluon table [nx][nq] (processes 1-3);         */
   uint32_t reserved1;        /* 11 = [11][nx][nq], flavour index = PDG id + 5 (b~ c~ s~ u~ d~ g d u s c b): process 4. */
-                             /* The library keeps the ten quark tables flavour-innermost in device memory (400 KB,   */
-                             /* L2-resident): one 16-point stencil per x serves all flavours                        */
+                             /* The library stages the ten quark tables flavour-innermost in shared memory, keeping   */
+                             /* the <= 4 Q^2 rows the stencil of the fixed mu_f touches (32 KB)                     */
 } mf_config_t;
 
 /* Optional per-event outputs of mf_integrand_eval.  DEVICE pointers, caller-owned, NULL = skip.     */

@@ -79,8 +79,8 @@ extern "C" int mf_vegas_create(const mf_config_t* cfg, mf_vegas_t** out) {
   h->use_staged = h->rec_fields > 0;
   h->f32 = cfg->precision == 32;
   h->max_blocks = h->n_sm * 32;
-  const bool flavours = cfg->process == MF_QQ_TT;      // 11-flavour grid: the ten quark tables, flavour-innermost
-  const size_t ne = (size_t)P.d * (P.nb + 1), ntab = (size_t)P.pdf_nx * P.pdf_nq, npdf = flavours ? ntab * MF_NQF : ntab;
+  const bool flavours = cfg->process == MF_QQ_TT;      // 11-flavour grid: the active rows of the ten quark tables (mf_flavour_slice)
+  const size_t ne = (size_t)P.d * (P.nb + 1), npdf = (size_t)P.pdf_smem;
   MF_CREATE_CUDA(cudaMalloc(&h->d_edges, ne * sizeof(double)));
   MF_CREATE_CUDA(cudaMalloc(&h->d_pdf, (npdf ? npdf : 1) * sizeof(double)));
   MF_CREATE_CUDA(cudaMalloc(&h->d_partial, (size_t)h->max_blocks * h->row * sizeof(double)));
@@ -97,13 +97,9 @@ extern "C" int mf_vegas_create(const mf_config_t* cfg, mf_vegas_t** out) {
   for (int j = 0; j < P.d; ++j)
     for (int k = 0; k <= P.nb; ++k) e[(size_t)j * (P.nb + 1) + k] = (double)k / (double)P.nb;
   MF_CREATE_CUDA(cudaMemcpy(h->d_edges, e.data(), ne * sizeof(double), cudaMemcpyHostToDevice));
-  if (flavours) {                                        // host [11][nx][nq] (index = PDG id + 5) -> device [nx][nq][MF_NQF]
+  if (flavours) {
     std::vector<double> t(npdf);
-    for (int f = 0; f < 11; ++f) {
-      if (f == 5) continue;                                // the gluon table is not used by q q~ -> t t~
-      const int slot = f < 5 ? f : f - 1;                  // slots 0..4 = b~ c~ s~ u~ d~ (5 - q), 5..9 = d u s c b (4 + q)
-      for (size_t i = 0; i < ntab; ++i) t[i * MF_NQF + slot] = cfg->pdf_xf[(size_t)f * ntab + i];
-    }
+    mf_flavour_slice(P, cfg->pdf_xf, t.data());
     MF_CREATE_CUDA(cudaMemcpy(h->d_pdf, t.data(), npdf * sizeof(double), cudaMemcpyHostToDevice));
   } else if (npdf) MF_CREATE_CUDA(cudaMemcpy(h->d_pdf, cfg->pdf_xf, npdf * sizeof(double), cudaMemcpyHostToDevice));
   MF_CREATE_CUDA(cudaEventCreate(&h->ev0));

@@ -86,10 +86,14 @@ struct MfParams {
   double wconst;                        // S_f * K / 2  (O8: F = ... S_f W_PS K / (2 shat))
   double pdf_lx0, pdf_ihx, pdf_lq0, pdf_ihq, pdf_lq;   // ln xmin, 1/h_x, ln qmin^2, 1/h_q, ln muF^2
   int32_t pdf_nx, pdf_nq;
-  int32_t pdf_smem;                     // doubles of the PDF table staged in shared memory: nx*nq (gluon table), 0 for the
-                                        // 11-flavour grid of the quark channel (400 KB: read through L1/L2 from global memory)
+  int32_t pdf_smem;                     // doubles of the PDF table staged in shared memory: nx*nq (gluon table), or
+                                        // nx*pdf_nqs*MF_NQF for the flavour grid of the quark channel
+  int32_t pdf_iq0, pdf_nqs;             // flavour grid: first Q^2 row and number of rows kept (<= 4): mu_F is a run constant, so
+                                        // only the rows its stencil touches are staged (32 KB instead of 400 KB); the
+                                        // interpolation in Q^2 is still evaluated per event (A17)
 };
-#define MF_NQF 10                       // quark/antiquark tables of the flavour grid, device layout [nx][nq][MF_NQF]:
+#define MF_XPAD 1                       // padding doubles per ln-x row of the staged flavour grid (bank spread)
+#define MF_NQF 10                       // quark/antiquark tables of the flavour grid, device layout [nx][pdf_nqs * MF_NQF + MF_XPAD]:
                                         // slot 5 - q = antiquark, 4 + q = quark of flavour q = 1..5 (d u s c b)
 
 // ---- S1: Philox4x32-10 (Salmon et al. SC'11), reading O1/A1 ----------------------------------
@@ -339,7 +343,8 @@ MF_HD double mf_hermite(double fm1, double f0, double f1, double f2, bool has_m1
 }
 
 // xf(x, Q^2) from the table `tab` [nx][nq] (shared memory on the device); lx = ln x, lq = ln Q^2.
-// STRIDE: doubles between neighbouring (ix, iq) entries (1 = single table; MF_NQF = flavour-innermost grid)
+// STRIDE: doubles between neighbouring (ix, iq) entries (1 = single table [nx][nq]; MF_NQF = flavour-innermost grid, of
+// which the rows pdf_iq0 .. pdf_iq0 + pdf_nqs - 1 are present)
 template <int STRIDE>
 MF_HD double mf_pdf_strided(const MfParams& P, const double* tab, double lx, double lq);
 MF_HD double mf_pdf(const MfParams& P, const double* tab, double lx, double lq) { return mf_pdf_strided<1>(P, tab, lx, lq); }
@@ -354,20 +359,24 @@ MF_HD double mf_pdf_strided(const MfParams& P, const double* tab, double lx, dou
   tx = tx < 0.0 ? 0.0 : (tx > 1.0 ? 1.0 : tx);     // clamp: no extrapolation
   tq = tq < 0.0 ? 0.0 : (tq > 1.0 ? 1.0 : tq);
   const bool xm = ix > 0, xp = ix + 2 < nx, qm = iq > 0, qp = iq + 2 < nq;
-  const int r0 = (xm ? ix - 1 : ix) * nq, r1 = ix * nq, r2 = (ix + 1) * nq, r3 = (xp ? ix + 2 : ix + 1) * nq;
+  // doubles per ln-x row of `tab` and its first Q^2 row; the flavour grid pads every ln-x row by MF_XPAD doubles so that
+  // the rows of different lanes fall on different shared-memory banks (41 doubles: odd)
+  const int rs = STRIDE == 1 ? nq : P.pdf_nqs * STRIDE + MF_XPAD, q0 = STRIDE == 1 ? 0 : P.pdf_iq0;
+  const int r0 = (xm ? ix - 1 : ix) * rs, r1 = ix * rs, r2 = (ix + 1) * rs, r3 = (xp ? ix + 2 : ix + 1) * rs;
   double row[4];
 #pragma unroll
   for (int c = 0; c < 4; ++c) {                     // Q^2 rows iq-1 .. iq+2 (clamped where absent)
     int q = iq - 1 + c;
     q = q < 0 ? 0 : (q > nq - 1 ? nq - 1 : q);
-    row[c] = mf_hermite(tab[(r0 + q) * STRIDE], tab[(r1 + q) * STRIDE], tab[(r2 + q) * STRIDE], tab[(r3 + q) * STRIDE], xm, xp, tx);
+    const int qo = (q - q0) * STRIDE;
+    row[c] = mf_hermite(tab[r0 + qo], tab[r1 + qo], tab[r2 + qo], tab[r3 + qo], xm, xp, tx);
   }
   return mf_hermite(row[0], row[1], row[2], row[3], qm, qp, tq);
 }
 
-// O5q: flavour-summed q q~ luminosity from the flavour-innermost grid tab [nx][nq][MF_NQF] (global
-// memory): l12 = sum_q xf_q(x1) xf_q~(x2), l21 = sum_q xf_q~(x1) xf_q(x2), q = d u s c b.  The 16-point stencil of
-// one x is shared by the ten tables: each of its points is one contiguous 80-byte read.
+// O5q: flavour-summed q q~ luminosity from the flavour-innermost grid tab [nx][pdf_nqs][MF_NQF] (shared
+// memory on the device): l12 = sum_q xf_q(x1) xf_q~(x2), l21 = sum_q xf_q~(x1) xf_q(x2), q = d u s c b.  The 16-point
+// stencil of one x is shared by the ten tables: each of its points is one contiguous 80-byte read.
 MF_HD void mf_lumi_qq(const MfParams& P, const double* tab, double lx1, double lx2, double lq, double& l12, double& l21) {
   l12 = 0.0; l21 = 0.0;
 #pragma unroll

@@ -17,6 +17,21 @@ static inline int mf_process_shape(int process, uint32_t generator, int* d, int*
   return 0;
 }
 
+// device copy of the 11-flavour grid (process 4): host [11][nx][nq] (index = PDG id + 5) -> the ten quark tables,
+// flavour-innermost, rows pdf_iq0 .. pdf_iq0 + pdf_nqs - 1 only: out[nx][pdf_nqs * MF_NQF + MF_XPAD] (P.pdf_smem doubles, zeroed
+// by the caller: the pad entries are never read).
+// Slots 0..4 = b~ c~ s~ u~ d~ (5 - q), 5..9 = d u s c b (4 + q); the gluon table is not used by q q~ -> t t~.
+static inline void mf_flavour_slice(const MfParams& P, const double* pdf11, double* out) {
+  const size_t ntab = (size_t)P.pdf_nx * P.pdf_nq;
+  for (int f = 0; f < 11; ++f) {
+    if (f == 5) continue;
+    const int slot = f < 5 ? f : f - 1;
+    for (int ix = 0; ix < P.pdf_nx; ++ix)
+      for (int r = 0; r < P.pdf_nqs; ++r)
+        out[(size_t)ix * (P.pdf_nqs * MF_NQF + MF_XPAD) + r * MF_NQF + slot] = pdf11[(size_t)f * ntab + (size_t)ix * P.pdf_nq + P.pdf_iq0 + r];
+  }
+}
+
 // returns MF_OK or MF_EINVAL / MF_EUNSUPPORTED with a message in err
 static inline int mf_fill_params(const mf_config_t* c, MfParams* P, std::string& err) {
   if (!c) { err = "cfg is NULL"; return MF_EINVAL; }
@@ -67,12 +82,19 @@ static inline int mf_fill_params(const mf_config_t* c, MfParams* P, std::string&
     if (c->process == MF_QQ_TT) p.me_pref = gs2n * (2.0 / 9.0) * MF_ME2_EE_MUMU_SCALE;   // O6q: colour sum 2 / 9 colours, 1/4 spins
     p.wconst = (ngl == 2 ? 0.5 : 1.0) * c->gev2_to_pb / 2.0;
     p.pdf_nx = (int)c->pdf_nx; p.pdf_nq = (int)c->pdf_nq;
-    p.pdf_smem = nfl == 1 ? p.pdf_nx * p.pdf_nq : 0;
     p.pdf_lx0 = log(c->pdf_xmin);
     p.pdf_ihx = (double)(c->pdf_nx - 1) / (log(c->pdf_xmax) - p.pdf_lx0);
     p.pdf_lq0 = log(c->pdf_qmin * c->pdf_qmin);
     p.pdf_ihq = (double)(c->pdf_nq - 1) / (log(c->pdf_qmax * c->pdf_qmax) - p.pdf_lq0);
     p.pdf_lq = log(c->mu_f * c->mu_f);
+    p.pdf_smem = p.pdf_nx * p.pdf_nq; p.pdf_iq0 = 0; p.pdf_nqs = p.pdf_nq;
+    if (nfl == 11) {                                   // flavour grid: keep the Q^2 rows the stencil of mu_F touches (mf_pdf_strided)
+      int iq = (int)floor((p.pdf_lq - p.pdf_lq0) * p.pdf_ihq);
+      iq = iq < 0 ? 0 : (iq > p.pdf_nq - 2 ? p.pdf_nq - 2 : iq);
+      const int lo = iq - 1 < 0 ? 0 : iq - 1, hi = iq + 2 > p.pdf_nq - 1 ? p.pdf_nq - 1 : iq + 2;
+      p.pdf_iq0 = lo; p.pdf_nqs = hi - lo + 1;
+      p.pdf_smem = p.pdf_nx * (p.pdf_nqs * MF_NQF + MF_XPAD);
+    }
   }
   *P = p;
   return MF_OK;

@@ -8,15 +8,9 @@
 #error "compile with -DMF_PROC=0..4"
 #endif
 
-// the PDF table the event functions read: the staged copy, or (quark channel) the flavour grid in global memory
-template <int PROC>
-__device__ __forceinline__ const double* mf_pdf_ptr(const double* s_pdf, const double* g_pdf) {
-  return MfPdf<PROC>::FLAVOURS ? g_pdf : s_pdf;
-}
-
 __device__ __forceinline__ void mf_stage_tables(const MfParams& P, const double* g_edges, const double* g_pdf,
                                                 double* s_edges, double* s_pdf) {
-  const int ne = P.d * (P.nb + 1), np = P.pdf_smem;      // np = 0: the flavour grid of the quark channel stays in global memory
+  const int ne = P.d * (P.nb + 1), np = P.pdf_smem;      // gluon table, or the active rows of the flavour grid (mf_params.h)
   for (int i = threadIdx.x; i < ne; i += blockDim.x) s_edges[i] = g_edges[i];
   for (int i = threadIdx.x; i < np; i += blockDim.x) s_pdf[i] = g_pdf[i];
 }
@@ -172,10 +166,10 @@ mf_iterate_kernel(const MfParams P, const double* __restrict__ g_edges, const do
     double F = 0.0;
     unsigned okeys = 0;
     if (MF_UNIFORM_ME) {                                 // every thread runs the event (barriers inside);
-      F = mf_event<PROC, false, double, CL>(P, s_edges, mf_pdf_ptr<PROC>(s_pdf, g_pdf), iteration, first + (valid ? i : n - 1), bin, pass, nullptr, &okeys);
+      F = mf_event<PROC, false, double, CL>(P, s_edges, s_pdf, iteration, first + (valid ? i : n - 1), bin, pass, nullptr, &okeys);
       if (!valid) { F = 0.0; pass = false; }             // lanes past the end recompute event n-1, discarded
     } else if (valid) {
-      F = mf_event<PROC, false, double, CL>(P, s_edges, mf_pdf_ptr<PROC>(s_pdf, g_pdf), iteration, first + i, bin, pass, nullptr, &okeys);
+      F = mf_event<PROC, false, double, CL>(P, s_edges, s_pdf, iteration, first + i, bin, pass, nullptr, &okeys);
     }
     if (!isfinite(F)) { F = 0.0; ++n_bad; }              // A20
     if (valid && pass) ++n_pass;
@@ -492,8 +486,8 @@ mf_eval_kernel(const MfParams P, const double* __restrict__ g_edges, const doubl
   constexpr int N = MfProc<PROC>::N;
   extern __shared__ double smem[];
   double* s_edges = smem;
-  const double* s_pdf = mf_pdf_ptr<PROC>(s_edges + P.d * (P.nb + 1), g_pdf);
-  mf_stage_tables(P, g_edges, g_pdf, s_edges, s_edges + P.d * (P.nb + 1));
+  double* s_pdf = s_edges + P.d * (P.nb + 1);
+  mf_stage_tables(P, g_edges, g_pdf, s_edges, s_pdf);
   __syncthreads();
   const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
   for (unsigned long long base = (unsigned long long)blockIdx.x * blockDim.x; base < n; base += stride) {

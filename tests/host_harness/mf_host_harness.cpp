@@ -74,5 +74,10 @@ extern "C" double mfh_event_gen(const MfParams* P, const double* edges, const do
   }
   return -1.0;
 }
+// the library's device copy of the 11-flavour grid (mf_params.h mf_flavour_slice); returns its length in doubles
+extern "C" int mfh_flavour_slice(const MfParams* P, const double* pdf11, double* out) {
+  if (out) mf_flavour_slice(*P, pdf11, out);
+  return P->pdf_smem;
+}
 extern "C" int mfh_params_size(void) { return (int)sizeof(MfParams); }
 extern "C" int mfh_fill_params(const mf_config_t* c, MfParams* P) { std::string e; return mf_fill_params(c, P, e); }

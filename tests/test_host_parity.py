@@ -136,10 +136,18 @@ def test_generator_flag_validation(harness):
             assert d[0] == proc and d[2] == nf and d[4] == gen and d[1] == (2 + 4 * nf if gen & 1 else 3 * nf - 2)
 
 
-def flavour_innermost(pdf11):
-    """the library's device layout of the 11-flavour grid (mf_api.cu): ten quark tables, [nx][nq][10], gluon dropped"""
+def flavour_slice(harness, P, pdf11):
+    """the library's device copy of the 11-flavour grid (mf_params.h mf_flavour_slice): the ten quark tables,
+    flavour-innermost, the Q^2 rows around mu_F only; checked here against a NumPy re-layout"""
+    n = harness.mfh_flavour_slice(P, pdf11.ctypes.data, None)
+    out = np.zeros(n)
+    harness.mfh_flavour_slice(P, pdf11.ctypes.data, out.ctypes.data)
+    nx, nq = pdf11.shape[1:]
+    iq = int(np.floor((np.log(173.0 ** 2) - np.log(W.PDF_QMIN ** 2)) / (np.log(W.PDF_QMAX ** 2) - np.log(W.PDF_QMIN ** 2)) * (nq - 1)))
     keep = [f for f in range(11) if f != 5]
-    return np.ascontiguousarray(np.transpose(pdf11[keep], (1, 2, 0)))
+    ref = np.transpose(pdf11[keep][:, :, iq - 1:iq + 3], (1, 2, 0))
+    assert n == nx * (ref.shape[1] * 10 + 1) and np.array_equal(out.reshape(nx, -1)[:, :-1].reshape(ref.shape), ref)   # one pad double per ln-x row
+    return out
 
 
 @pytest.mark.parametrize("gen,n", [(0, 300), (1, 150), (2, 150)])
@@ -153,7 +161,7 @@ def test_host_compiled_quark_channel_matches_oracle(mfo, harness, gen, n):
     assert c.pdf_nf == 11
     P = C.create_string_buffer(harness.mfh_params_size())
     assert harness.mfh_fill_params(C.byref(c), P) == 0
-    tab = flavour_innermost(pdf)
+    tab = flavour_slice(harness, P, pdf)
     orc = mfo.Vegas(cfg)
     d = orc.d
     edges = random_grid(d, 50, 31)

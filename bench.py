@@ -28,7 +28,7 @@ import numpy as np
 METRIC = "integrand events/sec (fp64) gg->ttbar g, 1e7 events/iteration/GPU"
 N_EVENTS = 10_000_000
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # SMs x DFMA lanes x 2 x max clock
-ME_KERNEL_DRAM_BYTES = 1.0907e9                          # ncu --set full capture of mf_me_kernel<2> (profiles/r1_final_staged_ncu.md)
+ME_KERNEL_DRAM_BYTES = 1.0730e9                          # ncu --set full capture of mf_me_kernel<2> (profiles/r1b_staged_ncu.md)
 
 
 class ClockSampler:
@@ -212,7 +212,7 @@ def run_ours(args, rank, local_rank, world):
         "gpu_launches": (5 if staged else 3) * args.steps,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                      "traffic": ME_KERNEL_DRAM_BYTES if staged else None,
-                     "traffic_source": "profiles/r1_final_staged_ncu.md (dram__bytes_read.sum + dram__bytes_write.sum of one mf_me_kernel<2> launch; algorithmic: 120 B per passing event = %.3e B)" % (120.0 * n_pass) if staged else None,
+                     "traffic_source": "profiles/r1b_staged_ncu.md (dram__bytes_read.sum + dram__bytes_write.sum of one mf_me_kernel<2> launch; algorithmic: 120 B per passing event = %.3e B)" % (120.0 * n_pass) if staged else None,
                      "kernel": "mf_me_kernel<2>" if staged else "mf_iterate_compact_kernel<2>", "kernel_ms": k_ms,
                      "flops_per_event": flops["flops"], "fma_fraction_of_ops": flops["fma"] / (flops["add"] + flops["mul"] + flops["fma"]),
                      "peak_source": "measured DFMA-chain microbenchmark (mf_fp64_peak), max of before/after the timed region",

@@ -459,3 +459,18 @@ def test_quark_channel_iterations_cross_section_and_errors(mf, mfo):
             mf.Vegas(bad)
     fl = gpu.me_flops()
     assert fl["flops"] == mf.Vegas(W.config(W.EE_MUMU)).me_flops()["flops"]      # the two-current code
+
+
+def test_config2_full_iteration_against_oracle(mf, mfo):
+    """configs[2] at its full size, every event through the oracle: the raw sums (I, S2), the 7 x 50 histogram, the pass
+    counter and the refined grid of a whole 1e7-event iteration on the GPU (staged path, the launch configuration
+    bench.py times) against the oracle's (about two minutes on 16 host cores; 2e6 events on a box with fewer than 8)"""
+    n = 10_000_000 if mfo.max_threads() >= 8 else 2_000_000
+    cfg = W.config(W.GG_TTG, seed=0)
+    gpu, orc = mf.Vegas(cfg), mfo.Vegas(cfg)
+    g = gpu.vegas_iterate(n)
+    o = orc.iterate(n, n_threads=mfo.max_threads())
+    assert g["n_pass"] == o["n_pass"] and g["n_nonfinite"] == 0 == o["n_nonfinite"]
+    assert abs(g["integral"] / o["integral"] - 1) < RTOL_INT and abs(g["sigma"] / o["sigma"] - 1) < 1e-8
+    np.testing.assert_allclose(gpu.get_accum()[0], orc.get_accum(), rtol=RTOL_INT, atol=1e-300)
+    np.testing.assert_allclose(gpu.get_grid(), orc.get_grid(), rtol=0, atol=1e-11)

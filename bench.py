@@ -116,9 +116,14 @@ def run_ours(args, rank, local_rank, world):
         raise SystemExit("bench.py needs a CUDA device (there is no CPU path); use --impl reference for the oracle")
     binding.lib()
     dist = None
-    if world > 1:
+    sharded = world > 1 or args.sharded                                    # the N > 1 code path (also at N = 1 with --sharded)
+    if sharded:
         import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        if world == 1:
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1"); os.environ.setdefault("MASTER_PORT", "29533")
+            dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", local_rank))
+        else:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     n, n_total = args.events, args.events * world
@@ -138,10 +143,10 @@ def run_ours(args, rank, local_rank, world):
 
     def step():
         flush.zero_()                                                      # L2 flush between iterations
-        if world == 1:
+        if not sharded:
             h.vegas_iterate(n, sync=False)
         else:
-            sharding.sharded_iterate(h, n_total, rank, world, dist, dev)
+            sharding.sharded_iterate_device(h, n_total, rank, world, dist, dev, sync=False)
 
     # clocks are sampled from the first warm-up step to the end of the end-to-end region (same load)
     sampler = ClockSampler(uuid) if rank == 0 else None
@@ -173,10 +178,10 @@ def run_ours(args, rank, local_rank, world):
     t0 = time.perf_counter()
     for _ in range(args.steps):
         h.set_grid(grid)                                                   # H2D d*51 doubles
-        if world == 1:
+        if not sharded:
             rec = h.vegas_iterate(n, sync=True)                            # D2H iteration record
         else:
-            rec = sharding.sharded_iterate(h, n_total, rank, world, dist, dev)
+            rec = sharding.sharded_iterate_device(h, n_total, rank, world, dist, dev, sync=True)
         grid = h.get_grid()                                                # D2H refined grid
     barrier()
     e2e_s = time.perf_counter() - t0
@@ -203,13 +208,13 @@ def run_ours(args, rank, local_rank, world):
                    "events_per_step_per_gpu": n, "pass_fraction": float(np.mean(pass_frac)),
                    "path": args.path,
                    "l2": "flushed between steps (256 MiB memset inside the timed region); inputs are 46 KB of tables; "
-                         "the staged path passes ~1.0 GB of event records per step through HBM (> 126 MB L2)", "parallelism": "event ranges over %d GPU(s), 1 all-reduce of 352 "
-                         "doubles per iteration" % world if world > 1 else "1 GPU",
+                         "the staged path passes ~1.0 GB of event records per step through HBM (> 126 MB L2)", "parallelism": "event ranges over %d GPU(s), 1 NCCL all-reduce of 354 "
+                         "doubles on the device per iteration (no host round trip)" % world if sharded else "1 GPU",
                    "integral_pb": res["integral"], "sigma_pb": res["sigma"]},
         "clocks": clocks,
         "e2e": {"value": n_total * args.steps / e2e_s, "unit": "events/s", "h2d_bytes_per_step": grid_bytes,
                 "d2h_bytes_per_step": grid_bytes + 40},
-        "gpu_launches": (5 if staged else 3) * args.steps,
+        "gpu_launches": ((5 if staged else 3) + (2 if sharded else 0)) * args.steps,   # + pack/unpack of the raw sums around the all-reduce
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                      "traffic": ME_KERNEL_DRAM_BYTES if staged else None,
                      "traffic_source": "profiles/r1b_staged_ncu.md (dram__bytes_read.sum + dram__bytes_write.sum of one mf_me_kernel<2> launch; algorithmic: 120 B per passing event = %.3e B)" % (120.0 * n_pass) if staged else None,
@@ -332,6 +337,7 @@ def main():
     ap.add_argument("--events", type=int, default=N_EVENTS, help="events per iteration per GPU")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="configs[4]: events-per-launch sweep of the gg->tt~g integrand (1 GPU)")
+    ap.add_argument("--sharded", action="store_true", help="run the multi-GPU code path (device-side all-reduce of the raw sums) even at N = 1")
     ap.add_argument("--processes", action="store_true", help="every process / generator selection at its config size (1 GPU)")
     ap.add_argument("--path", default="staged", choices=["staged", "fused"],
                     help="staged: front end / |M|^2 / reductions as three kernels (default); fused: one kernel")
@@ -351,7 +357,7 @@ def main():
             run_processes(args)
         return
     run_ours(args, rank, local_rank, world)
-    if world > 1:
+    if world > 1 or args.sharded:
         import torch.distributed as dist
         dist.destroy_process_group()
 

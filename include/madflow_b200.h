@@ -124,6 +124,12 @@ int mf_vegas_accumulate(mf_vegas_t *h, uint64_t first_event, uint64_t n_events, 
 int mf_get_accum(mf_vegas_t *h, double *host_acc /* [mf_accum_len()] = [2 + d*n_bins] without observables */, uint64_t *host_counts /* [2] */);
 int mf_set_accum(mf_vegas_t *h, const double *host_acc, const uint64_t *host_counts);
 int mf_vegas_finalize(mf_vegas_t *h, uint64_t n_total, void *cuda_stream, mf_iter_t *host_out_or_null);
+/* The same exchange without host round trips (enqueue only, no synchronisation): clear the raw sums; copy them, followed
+ * by the two counters converted to double (exact below 2^53), into / from a caller-owned DEVICE buffer of
+ * mf_accum_len() + 2 doubles -- one buffer for one all-reduce (e.g. ncclAllReduce / torch.distributed on the same stream). */
+int mf_zero_accum(mf_vegas_t *h, void *cuda_stream);
+int mf_get_accum_device(mf_vegas_t *h, double *dev_out, void *cuda_stream);
+int mf_set_accum_device(mf_vegas_t *h, const double *dev_in, void *cuda_stream);
 
 /* Observable histograms filled in the same pass as the integral ("histogram accumulation";
  * dsigma/dpT of the top quark is the paper's physics plot).  For every event with weight

@@ -16,7 +16,8 @@ EXPORTS = ["mf_vegas_create", "mf_vegas_destroy", "mf_ndim", "mf_integrand_eval"
            "mf_vegas_accumulate", "mf_get_accum", "mf_set_accum", "mf_vegas_finalize", "mf_result",
            "mf_get_iterations", "mf_get_grid", "mf_set_grid", "mf_set_launch", "mf_me_flops",
            "mf_fp64_peak", "mf_last_kernel_ms", "mf_last_error", "mf_set_path", "mf_last_stage_ms",
-           "mf_set_observables", "mf_get_observables", "mf_accum_len"]
+           "mf_set_observables", "mf_get_observables", "mf_accum_len", "mf_zero_accum", "mf_get_accum_device",
+           "mf_set_accum_device"]
 
 
 class MfError(RuntimeError):
@@ -100,6 +101,9 @@ def lib():
         L.mf_set_observables.argtypes = [vp, vp, u32]
         L.mf_get_observables.argtypes = [vp, vp, vp, C.POINTER(u32)]
         L.mf_accum_len.argtypes = [vp, C.POINTER(u32)]
+        L.mf_zero_accum.argtypes = [vp, vp]
+        L.mf_get_accum_device.argtypes = [vp, vp, vp]
+        L.mf_set_accum_device.argtypes = [vp, vp, vp]
         L.mf_last_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
         L.mf_me_flops.argtypes = [vp, C.POINTER(u64), C.POINTER(u64), C.POINTER(u64)]
         L.mf_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
@@ -208,6 +212,16 @@ class Vegas:
     def set_accum(self, acc, counts):
         acc = np.ascontiguousarray(acc, dtype=np.float64); cnt = np.ascontiguousarray(counts, dtype=np.uint64)
         _check(lib().mf_set_accum(self._h, acc.ctypes.data, cnt.ctypes.data))
+
+    def zero_accum(self, stream=None):
+        _check(lib().mf_zero_accum(self._h, _stream_ptr(stream)))
+
+    def get_accum_device(self, dev_ptr, stream=None):
+        """raw sums + the two counters (as doubles) into a device buffer of accum_len() + 2 doubles; enqueue only"""
+        _check(lib().mf_get_accum_device(self._h, C.c_void_p(int(dev_ptr)), _stream_ptr(stream)))
+
+    def set_accum_device(self, dev_ptr, stream=None):
+        _check(lib().mf_set_accum_device(self._h, C.c_void_p(int(dev_ptr)), _stream_ptr(stream)))
 
     def vegas_finalize(self, n_total, stream=None, sync=True):
         it = Iter()

@@ -357,6 +357,35 @@ extern "C" int mf_set_accum(mf_vegas_t* h, const double* host_acc, const uint64_
   return MF_OK;
 }
 
+extern "C" int mf_zero_accum(mf_vegas_t* h, void* cuda_stream) {
+  if (!h) return fail(MF_EINVAL, "handle is NULL");
+  MF_CUDA(cudaSetDevice(h->device));
+  h->last_stream = (cudaStream_t)cuda_stream;
+  return zero_accum(h, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int mf_get_accum_device(mf_vegas_t* h, double* dev_out, void* cuda_stream) {
+  if (!h || !dev_out) return fail(MF_EINVAL, "null argument");
+  MF_CUDA(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int n = live_len(h);
+  mf_pack_accum_kernel<<<(n + 2 + 255) / 256, 256, 0, st>>>(h->d_acc, h->d_counts, n, dev_out);
+  MF_CUDA(cudaGetLastError());
+  h->last_stream = st;
+  return MF_OK;
+}
+
+extern "C" int mf_set_accum_device(mf_vegas_t* h, const double* dev_in, void* cuda_stream) {
+  if (!h || !dev_in) return fail(MF_EINVAL, "null argument");
+  MF_CUDA(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int n = live_len(h);
+  mf_unpack_accum_kernel<<<(n + 2 + 255) / 256, 256, 0, st>>>(dev_in, n, h->d_acc, h->d_counts);
+  MF_CUDA(cudaGetLastError());
+  h->last_stream = st;
+  return MF_OK;
+}
+
 extern "C" int mf_set_observables(mf_vegas_t* h, const mf_observable_t* obs, uint32_t n_obs) {
   if (!h) return fail(MF_EINVAL, "handle is NULL");
   if (n_obs > MF_MAX_OBS || (n_obs > 0 && !obs)) return fail(MF_EINVAL, "at most 4 observables");

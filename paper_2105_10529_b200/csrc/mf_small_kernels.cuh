@@ -94,6 +94,21 @@ __global__ void mf_finalize_kernel(const MfParams P, double alpha, double n_tota
   }
 }
 
+// ---- device-side exchange of the raw sums (multi-GPU without host round trips) -------------------------
+// buf = [acc[0..n), (double)counts[0], (double)counts[1]]: one buffer for one all-reduce (counts < 2^53: exact)
+__global__ void mf_pack_accum_kernel(const double* __restrict__ acc, const unsigned long long* __restrict__ counts, int n,
+                                     double* __restrict__ buf) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) buf[i] = acc[i];
+  else if (i < n + 2) buf[i] = (double)counts[i - n];
+}
+__global__ void mf_unpack_accum_kernel(const double* __restrict__ buf, int n, double* __restrict__ acc,
+                                       unsigned long long* __restrict__ counts) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) acc[i] = buf[i];
+  else if (i < n + 2) counts[i - n] = (unsigned long long)__double2ll_rn(buf[i]);
+}
+
 // ---- O11: I = sum(I_j/s_j^2)/sum(1/s_j^2), sigma = (sum 1/s_j^2)^-1/2, chi2/dof ----------------------
 __global__ void mf_combine_kernel(MfDevState* __restrict__ st) {
   if (threadIdx.x != 0 || blockIdx.x != 0) return;

@@ -26,9 +26,25 @@ def allreduce_sums(acc, counts, dist=None, device=None):
     return out[:len(acc)].copy(), np.rint(out[len(acc):]).astype(np.uint64)
 
 
+def sharded_iterate_device(h, n_total, rank, world, dist=None, device=None, sync=True):
+    """the same iteration without host round trips: the raw sums and counters stay on the device, the all-reduce runs
+    on a device buffer (NCCL), everything is enqueued on torch's current stream; sync=False returns without waiting"""
+    import torch
+    first, n = shard_range(n_total, rank, world)
+    h.zero_accum()
+    h.vegas_accumulate(first, n, n_total)
+    buf = torch.empty(h.accum_len() + 2, dtype=torch.float64, device=device)
+    h.get_accum_device(buf.data_ptr())
+    if dist is not None and dist.is_initialized():
+        dist.all_reduce(buf, op=dist.ReduceOp.SUM)         # ordered after the pack kernel on the current stream
+    h.set_accum_device(buf.data_ptr())
+    return h.vegas_finalize(n_total, sync=sync)
+
+
 def sharded_iterate(h, n_total, rank, world, dist=None, device=None, stream=None):
     """one iteration of n_total events split over `world` ranks; h has the C-ABI's method names
-    (set_accum / vegas_accumulate / get_accum / vegas_finalize)"""
+    (set_accum / vegas_accumulate / get_accum / vegas_finalize).  Host-staged exchange (works with any backend:
+    the gloo test); device handles on NCCL use sharded_iterate_device"""
     first, n = shard_range(n_total, rank, world)
     zeros = np.zeros(h.accum_len() if hasattr(h, "accum_len") else 2 + h.d * h.n_bins)
     h.set_accum(zeros, np.zeros(2, np.uint64))

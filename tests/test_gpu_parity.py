@@ -474,3 +474,46 @@ def test_config2_full_iteration_against_oracle(mf, mfo):
     assert abs(g["integral"] / o["integral"] - 1) < RTOL_INT and abs(g["sigma"] / o["sigma"] - 1) < 1e-8
     np.testing.assert_allclose(gpu.get_accum()[0], orc.get_accum(), rtol=RTOL_INT, atol=1e-300)
     np.testing.assert_allclose(gpu.get_grid(), orc.get_grid(), rtol=0, atol=1e-11)
+
+
+def test_device_side_sharded_iteration(mf):
+    """multi-GPU exchange without host round trips (mf_zero_accum / mf_get_accum_device / mf_set_accum_device around an
+    NCCL all-reduce on the device buffer), on the one GPU of this box with a world-size-1 NCCL group: identical to
+    mf_vegas_iterate bit for bit (same launches); and two event ranges accumulated one after the other, as two ranks
+    would, agree to summation order"""
+    import os
+    import torch
+    import torch.distributed as dist
+    from paper_2105_10529_b200 import sharding
+    dev = torch.device("cuda", 0)
+    cfg = W.config(W.GG_TTG, seed=11)
+    n = 300_001
+    a, b, c = mf.Vegas(cfg), mf.Vegas(cfg), mf.Vegas(cfg)
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1"); os.environ.setdefault("MASTER_PORT", str(29700 + os.getpid() % 200))
+    group = False
+    if not dist.is_initialized():
+        dist.init_process_group("nccl", rank=0, world_size=1, device_id=dev)
+        group = True
+    try:
+        for _ in range(2):
+            ia = a.vegas_iterate(n)
+            ib = sharding.sharded_iterate_device(b, n, 0, 1, dist, dev)
+            assert ia["integral"] == ib["integral"] and ia["sigma"] == ib["sigma"] and ia["n_pass"] == ib["n_pass"]
+            np.testing.assert_array_equal(a.get_grid(), b.get_grid())
+            # two "ranks" on one handle: ranges [0, n/2) and [n/2, n), packed sums added on the device
+            c.zero_accum()
+            bufs = []
+            for r in range(2):
+                first, m = sharding.shard_range(n, r, 2)
+                c.zero_accum(); c.vegas_accumulate(first, m, n)
+                t = torch.empty(c.accum_len() + 2, dtype=torch.float64, device=dev)
+                c.get_accum_device(t.data_ptr()); bufs.append(t)
+            tot = bufs[0] + bufs[1]
+            dist.all_reduce(tot)                                   # world size 1: identity, through NCCL
+            c.set_accum_device(tot.data_ptr())
+            ic = c.vegas_finalize(n)
+            assert ic["n_pass"] == ia["n_pass"] and abs(ic["integral"] / ia["integral"] - 1) < 1e-13
+            np.testing.assert_allclose(c.get_grid(), a.get_grid(), rtol=0, atol=1e-13)
+    finally:
+        if group:
+            dist.destroy_process_group()

@@ -144,8 +144,8 @@ class Vegas:
         self.device = cfg.get("device", 0)
 
     def close(self):
-        if getattr(self, "_h", None):
-            lib().mf_vegas_destroy(self._h)
+        if getattr(self, "_h", None) and _lib is not None:    # at interpreter shutdown the module globals may be gone already
+            _lib.mf_vegas_destroy(self._h)
             self._h = None
 
     __del__ = close

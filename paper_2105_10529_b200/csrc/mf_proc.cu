@@ -4,6 +4,7 @@
 // per-event evaluation (mf_eval_kernel); plus their launchers (MfProcOps, mf_proc.h).
 #include "mf_kernels.cuh"
 #include "mf_proc.h"
+#include <type_traits>
 #ifndef MF_PROC
 #error "compile with -DMF_PROC=0..4"
 #endif
@@ -524,8 +525,20 @@ static constexpr bool kF32 = MF_PROC == 2;   // fp32 variant of the |M|^2 stage:
 // classic 4n-random RAMBO: processes 1-3; the heavy ones on the staged path only
 static constexpr int kCL = MF_PROC != 0 ? 1 : 0;    // front-end instance of the classic RAMBO (mf_event.cuh MfDim)
 static constexpr int kLT = MF_PROC != 0 ? 2 : 0;    // ... of the configs' RAMBO with the selectable tau map
-static inline bool is_classic(const MfParams& P) { return kCL && (P.gen & MFD_GEN_CLASSIC); }
-static inline bool is_lintau(const MfParams& P) { return kLT && !is_classic(P) && (P.gen & MFD_GEN_LINEAR); }
+// f(std::integral_constant<int, G>) with the front-end instance G the run's generator flags select (0 = the configs'
+// generators: the instance without any run-time branch), resp. with the instance that fixes the VEGAS dimensions only
+// (the reduction stage does not care about the tau map)
+template <typename F>
+static cudaError_t with_generator(const MfParams& P, F&& f) {
+  if (kCL && (P.gen & MFD_GEN_CLASSIC)) return f(std::integral_constant<int, kCL>{});
+  if (kLT && (P.gen & MFD_GEN_LINEAR)) return f(std::integral_constant<int, kLT>{});
+  return f(std::integral_constant<int, 0>{});
+}
+template <typename F>
+static cudaError_t with_dimensions(const MfParams& P, F&& f) {
+  if (kCL && (P.gen & MFD_GEN_CLASSIC)) return f(std::integral_constant<int, kCL>{});
+  return f(std::integral_constant<int, 0>{});
+}
 
 static cudaError_t proc_setup(const MfParams& P, size_t* smem_iter, size_t* smem_eval, int* occ_iter, int* occ_eval) {
   const size_t tables = (size_t)P.d * (P.nb + 1) + (size_t)P.pdf_smem;
@@ -540,19 +553,11 @@ static cudaError_t proc_setup(const MfParams& P, size_t* smem_iter, size_t* smem
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_iter, mf_iterate_compact_kernel<MF_PROC>, MF_THREADS, *smem_iter);
   } else {
     const int smem_obs = (int)(*smem_iter + sizeof(double) * nw * MF_OBS_ACC);            // room for the observable histograms
-    if (is_classic(P)) {
-      e = cudaFuncSetAttribute(mf_iterate_kernel<MF_PROC, kCL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_obs);
-      if (e) return e;
-      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_iter, mf_iterate_kernel<MF_PROC, kCL>, MF_THREADS, *smem_iter);
-    } else if (is_lintau(P)) {
-      e = cudaFuncSetAttribute(mf_iterate_kernel<MF_PROC, kLT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_obs);
-      if (e) return e;
-      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_iter, mf_iterate_kernel<MF_PROC, kLT>, MF_THREADS, *smem_iter);
-    } else {
-      e = cudaFuncSetAttribute(mf_iterate_kernel<MF_PROC, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_obs);
-      if (e) return e;
-      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_iter, mf_iterate_kernel<MF_PROC, 0>, MF_THREADS, *smem_iter);
-    }
+    e = with_generator(P, [&](auto g) {
+      constexpr int G = decltype(g)::value;
+      const cudaError_t r = cudaFuncSetAttribute(mf_iterate_kernel<MF_PROC, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_obs);
+      return r ? r : cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_iter, mf_iterate_kernel<MF_PROC, G>, MF_THREADS, *smem_iter);
+    });
   }
   if (e) return e;
   if constexpr (!kEvalOne) {
@@ -595,14 +600,13 @@ static cudaError_t proc_iterate(const MfParams& P, const double* edges, const do
   if constexpr (kCompact) {
     if (P.gen != 0) return cudaErrorNotSupported;        // generator variants of the heavy processes: staged path
     mf_iterate_compact_kernel<MF_PROC><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount, row);
-  } else if (is_classic(P)) {
-    mf_iterate_kernel<MF_PROC, kCL><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount, row);
-  } else if (is_lintau(P)) {
-    mf_iterate_kernel<MF_PROC, kLT><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount, row);
+    return cudaGetLastError();
   } else {
-    mf_iterate_kernel<MF_PROC, 0><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount, row);
+    return with_generator(P, [&](auto g) {
+      mf_iterate_kernel<MF_PROC, decltype(g)::value><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount, row);
+      return cudaGetLastError();
+    });
   }
-  return cudaGetLastError();
 }
 
 // ---- staged path: launches ---------------------------------------------------------------------------
@@ -624,10 +628,11 @@ static cudaError_t proc_staged_setup(const MfParams& P, int* rec_fields, int* oc
   *occ_front = *occ_hist = 0;
   if constexpr (!kStaged) return cudaSuccess;
   else {
-  const bool cl = is_classic(P), lt = is_lintau(P);
-  cudaError_t e = cl ? cudaFuncSetAttribute(mf_front_kernel<MF_PROC, kCL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)front_smem(P))
-                : lt ? cudaFuncSetAttribute(mf_front_kernel<MF_PROC, kLT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)front_smem(P))
-                     : cudaFuncSetAttribute(mf_front_kernel<MF_PROC, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)front_smem(P));
+  cudaError_t e = with_generator(P, [&](auto g) {
+    constexpr int G = decltype(g)::value;
+    const cudaError_t r = cudaFuncSetAttribute(mf_front_kernel<MF_PROC, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)front_smem(P));
+    return r ? r : cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_front, mf_front_kernel<MF_PROC, G>, MF_THREADS, front_smem(P));
+  });
   if (e) return e;
   e = cudaFuncSetAttribute(mf_me_kernel<MF_PROC, double, MF_ME_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
   if (e) return e;
@@ -636,15 +641,11 @@ static cudaError_t proc_staged_setup(const MfParams& P, int* rec_fields, int* oc
     if (e) return e;
   }
   const int smem_hist = (int)(hist_smem(P) + sizeof(double) * (MF_THREADS / 32) * MF_OBS_ACC);
-  e = cl ? cudaFuncSetAttribute(mf_hist_kernel<MF_PROC, kCL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_hist)
-         : cudaFuncSetAttribute(mf_hist_kernel<MF_PROC, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_hist);
-  if (e) return e;
-  e = cl ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_front, mf_front_kernel<MF_PROC, kCL>, MF_THREADS, front_smem(P))
-    : lt ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_front, mf_front_kernel<MF_PROC, kLT>, MF_THREADS, front_smem(P))
-         : cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_front, mf_front_kernel<MF_PROC, 0>, MF_THREADS, front_smem(P));
-  if (e) return e;
-  return cl ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_hist, mf_hist_kernel<MF_PROC, kCL>, MF_THREADS, hist_smem(P))
-            : cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_hist, mf_hist_kernel<MF_PROC, 0>, MF_THREADS, hist_smem(P));
+  return with_dimensions(P, [&](auto g) {
+    constexpr int G = decltype(g)::value;
+    const cudaError_t r = cudaFuncSetAttribute(mf_hist_kernel<MF_PROC, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_hist);
+    return r ? r : cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_hist, mf_hist_kernel<MF_PROC, G>, MF_THREADS, hist_smem(P));
+  });
   }
 }
 
@@ -657,11 +658,11 @@ static cudaError_t proc_staged(const MfParams& P, const double* edges, const dou
   else {
   cudaError_t e;
   if (ev && (e = cudaEventRecord(ev[0], st))) return e;
-  const bool cl = is_classic(P);
-  if (cl) mf_front_kernel<MF_PROC, kCL><<<ws.regions, MF_THREADS, front_smem(P), st>>>(P, edges, pdf, iteration, first, n, ws.cap, ws.rec, ws.count);
-  else if (is_lintau(P)) mf_front_kernel<MF_PROC, kLT><<<ws.regions, MF_THREADS, front_smem(P), st>>>(P, edges, pdf, iteration, first, n, ws.cap, ws.rec, ws.count);
-  else mf_front_kernel<MF_PROC, 0><<<ws.regions, MF_THREADS, front_smem(P), st>>>(P, edges, pdf, iteration, first, n, ws.cap, ws.rec, ws.count);
-  if ((e = cudaGetLastError())) return e;
+  e = with_generator(P, [&](auto g) {
+    mf_front_kernel<MF_PROC, decltype(g)::value><<<ws.regions, MF_THREADS, front_smem(P), st>>>(P, edges, pdf, iteration, first, n, ws.cap, ws.rec, ws.count);
+    return cudaGetLastError();
+  });
+  if (e) return e;
   if (ev && (e = cudaEventRecord(ev[1], st))) return e;
   const size_t sm = sizeof(unsigned int) * ((size_t)ws.regions + 1 + (f32 ? MF_ME_THREADS_F32 : MF_ME_THREADS));
   if (f32) {
@@ -672,9 +673,11 @@ static cudaError_t proc_staged(const MfParams& P, const double* edges, const dou
   }
   if ((e = cudaGetLastError())) return e;
   if (ev && (e = cudaEventRecord(ev[2], st))) return e;
-  if (cl) mf_hist_kernel<MF_PROC, kCL><<<grid_hist, MF_THREADS, hist_smem(P), st>>>(P, ws.rec, ws.count, ws.regions, ws.cap, n_total, partial, pcount, row);
-  else mf_hist_kernel<MF_PROC, 0><<<grid_hist, MF_THREADS, hist_smem(P), st>>>(P, ws.rec, ws.count, ws.regions, ws.cap, n_total, partial, pcount, row);
-  if ((e = cudaGetLastError())) return e;
+  e = with_dimensions(P, [&](auto g) {
+    mf_hist_kernel<MF_PROC, decltype(g)::value><<<grid_hist, MF_THREADS, hist_smem(P), st>>>(P, ws.rec, ws.count, ws.regions, ws.cap, n_total, partial, pcount, row);
+    return cudaGetLastError();
+  });
+  if (e) return e;
   if (ev && (e = cudaEventRecord(ev[3], st))) return e;
   return cudaSuccess;
   }

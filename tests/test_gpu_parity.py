@@ -517,3 +517,23 @@ def test_device_side_sharded_iteration(mf):
     finally:
         if group:
             dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("proc,gen,n", [(W.QQ_TT, 0, 1_000_000), (W.GG_TTG, W.GEN_CLASSIC_RAMBO, 10_000_000),
+                                        (W.GG_TTGG, W.GEN_CLASSIC_RAMBO | W.GEN_LINEAR_TAU, 1_000_000)])
+def test_widened_rows_full_size_launch_sampled_parity(mf, mfo, proc, gen, n):
+    """the quark channel and the selectable generators at the full size of the config they vary, in the launch
+    configuration `bench.py --processes` times: raw sums of the iteration == sums of the eval kernel's weights, counters
+    consistent, sampled events == oracle"""
+    cfg = W.config(proc, seed=0, generator=gen)
+    gpu, orc = mf.Vegas(cfg), mfo.Vegas(cfg)
+    g = gpu.vegas_iterate(n)
+    acc, cnt = gpu.get_accum()
+    w = mf.Vegas(cfg).integrand_eval(0, 0, n)["weight"]
+    t = w / n
+    assert abs(float(t.sum()) / acc[0] - 1) < 1e-10 and abs(float((t * t).sum()) / acc[1] - 1) < 1e-10
+    assert int((w != 0).sum()) <= cnt[0] <= n and g["n_nonfinite"] == 0 and g["n_events"] == n
+    for i in (0, 1, 255, 256, 65_537, n // 2 + 1, n - 1):
+        ref = orc.eval(0, i, 1)["weight"][0]
+        got = float(w[i])
+        assert (ref == 0 and got == 0) or abs(got / ref - 1) < RTOL_EVENT, (i, got, ref)

@@ -1,6 +1,8 @@
-"""World-size-2 gloo test (CPU) of the sharded-iteration plumbing (paper_2105_10529_b200/sharding.py):
+"""World-size-2 gloo tests (CPU) of the sharded-iteration plumbing (paper_2105_10529_b200/sharding.py), in its host-staged
+form and in the device-buffer form that bench.py --gpus N runs (here with a CPU tensor as the exchange buffer):
 event ranges, the one all-reduce of the raw sums, identical grids on every rank.  The device handle is
 replaced by an adapter over the oracle (same method names as the C-ABI binding)."""
+import ctypes
 import os
 import numpy as np
 import pytest
@@ -31,9 +33,26 @@ class OracleHandle:
         acc, cnt = self.v.accumulate(self.iteration, first, n, n_total, n_threads=2, acc=self.acc.copy())
         self.acc = acc; self.cnt = self.cnt + cnt
 
-    def vegas_finalize(self, n_total, stream=None):
+    def vegas_finalize(self, n_total, stream=None, sync=True):
         self.iteration += 1
         return self.v.finalize(self.acc, n_total, self.cnt[0], self.cnt[1])
+
+    # the device-side exchange of the C-ABI (mf_zero_accum / mf_get_accum_device / mf_set_accum_device) on host memory:
+    # the "device buffer" is a CPU tensor, addressed by its data_ptr() like the real one
+    def accum_len(self):
+        return len(self.acc)
+
+    def zero_accum(self, stream=None):
+        self.acc[:] = 0.0; self.cnt[:] = 0
+
+    def get_accum_device(self, ptr, stream=None):
+        buf = np.concatenate([self.acc, self.cnt.astype(np.float64)])
+        ctypes.memmove(ptr, buf.ctypes.data, buf.nbytes)
+
+    def set_accum_device(self, ptr, stream=None):
+        buf = np.zeros(len(self.acc) + 2)
+        ctypes.memmove(buf.ctypes.data, ptr, buf.nbytes)
+        self.acc = buf[:-2].copy(); self.cnt = np.rint(buf[-2:]).astype(np.uint64)
 
 
 def test_shard_ranges_cover_the_iteration():
@@ -44,24 +63,28 @@ def test_shard_ranges_cover_the_iteration():
             assert f0 + c0 == f1
 
 
-def _worker(rank, world, port, q):
+def _worker(rank, world, port, q, device_form=False):
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
     dist.init_process_group("gloo", rank=rank, world_size=world)
     h = OracleHandle(W.config(W.GG_TT, seed=3))
     out = []
     for _ in range(2):
-        it = sharding.sharded_iterate(h, 6001, rank, world, dist)
+        if device_form:      # the function bench.py --gpus N runs, with a CPU tensor as the exchange buffer
+            it = sharding.sharded_iterate_device(h, 6001, rank, world, dist, torch.device("cpu"))
+        else:
+            it = sharding.sharded_iterate(h, 6001, rank, world, dist)
         out.append((it["integral"], it["sigma"], it["n_pass"]))
     q.put((rank, out, h.v.get_grid()))
     dist.barrier()
     dist.destroy_process_group()
 
 
-def test_two_rank_iteration_matches_single_process(mfo):
-    port = 29500 + os.getpid() % 2000
+@pytest.mark.parametrize("device_form", [False, True])
+def test_two_rank_iteration_matches_single_process(mfo, device_form):
+    port = 29500 + (os.getpid() + 7 * device_form) % 2000
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
-    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q, device_form)) for r in range(2)]
     for p in procs:
         p.start()
     got = sorted([q.get(timeout=300) for _ in procs], key=lambda t: t[0])

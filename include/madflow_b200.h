@@ -30,7 +30,7 @@ extern "C" {
 typedef struct mf_vegas mf_vegas_t;
 
 enum { MF_OK = 0, MF_EINVAL = -1, MF_ENOMEM = -2, MF_ECUDA = -3, MF_ESTATE = -4, MF_EUNSUPPORTED = -5 };
-/* processes (BASELINE.json configs 0-3) */
+/* processes (BASELINE.json configs 0-3; 4 = the quark channel of SURVEY 8(f)2) */
 enum { MF_EE_MUMU = 0, MF_GG_TT = 1, MF_GG_TTG = 2, MF_GG_TTGG = 3,
        MF_QQ_TT = 4 };     /* quark channel ("any process generated (at LO)"): q q~ -> t t~, one
                             * s-channel-gluon diagram, averaged over 4 helicities x 9 colours, with the parton luminosity

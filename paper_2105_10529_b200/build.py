@@ -1,5 +1,5 @@
 """In-tree build of libmadflow_b200.so for sm_100a: run the amplitude generator, compile the C-ABI
-and the four per-process kernel objects in parallel with nvcc, link.  `python -m
+and the five per-process kernel objects in parallel with nvcc, link.  `python -m
 paper_2105_10529_b200.build [--force]`."""
 import os
 import subprocess

@@ -1,7 +1,9 @@
 // mf_event.cuh -- one event, S1 -> S8 (PAPER.md:59 pipeline), for the four processes of
-// BASELINE.json configs 0-3.  Returns F = w*f (pb), the weight before the 1/N (reading O8):
+// BASELINE.json configs 0-3 and the quark channel (process 4).  Returns F = w*f (pb), the weight
+// before the 1/N (reading O8):
 //   config 0   : F = J_V |M|^2 (1/(8 pi)) K / (2 s)
 //   configs 1-3: F = J_V J_x f_g(x1) f_g(x2) |M|^2 S_f W_0 W_m Theta_cuts K / (2 shat)
+//   process 4  : F = J_V J_x sum_q [f_q(x1) f_q~(x2) + f_q~(x1) f_q(x2)] |M|^2 W_0 W_m K / (2 shat)
 #pragma once
 #include "mf_device.cuh"
 #include "generated/mf_me2_ee_mumu.cuh"

@@ -1,4 +1,4 @@
-// mf_proc.cu -- the per-process kernels, compiled once per process with -DMF_PROC=0..3 so that the four
+// mf_proc.cu -- the per-process kernels, compiled once per process with -DMF_PROC=0..4 so that the
 // |M|^2 codes build in parallel: the fused iteration (mf_iterate_kernel, mf_iterate_compact_kernel), the
 // staged iteration of the heavy processes (mf_front_kernel -> mf_me_kernel -> mf_hist_kernel), and the
 // per-event evaluation (mf_eval_kernel); plus their launchers (MfProcOps, mf_proc.h).

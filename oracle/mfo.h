@@ -27,7 +27,8 @@ extern "C" {
 
 enum { MFO_OK = 0, MFO_EINVAL = -1, MFO_ENOMEM = -2, MFO_ESTATE = -4, MFO_EUNSUPPORTED = -5 };
 enum { MFO_EE_MUMU = 0, MFO_GG_TT = 1, MFO_GG_TTG = 2, MFO_GG_TTGG = 3,
-       MFO_QQ_TT = 4 };        /* q q~ -> t t~ summed over the five light flavours     */
+       MFO_QQ_TT = 4,          /* q q~ -> t t~ summed over the five light flavours     */
+       MFO_PP_TT = 5 };        /* p p -> t t~ at LO: the sum of the subprocesses g g -> t t~ and q q~ -> t t~   */
 
 typedef struct {
   int32_t  process;            /* MFO_*                                                          */
@@ -58,6 +59,10 @@ typedef struct {
  *  MFO_GEN_LINEAR_TAU     tau = tau0 + (1 - tau0) y0 instead of tau = tau0^(1-y0) (mfo_x_map_linear)     */
 enum { MFO_GEN_CLASSIC_RAMBO = 1, MFO_GEN_LINEAR_TAU = 2 };
 
+/* MFO_PP_TT: both subprocesses in one integrand on the 11-flavour grid,
+ *   F = J_V J_x [ xg(x1) xg(x2) |M_gg|^2 + (L12 + L21) |M_qq|^2 ] / (x1 x2) W_PS K / (2 shat),
+ * L12, L21 the flavour sums of MFO_QQ_TT, the gluon density from table 5.  Per-event record: pdf[2] =
+ * { xg(x1) xg(x2), L12 + L21 } (the two x1 x2-weighted luminosities), me2 = their luminosity-weighted mean |M|^2. */
 typedef struct {               /* host buffers owned by the caller; NULL = skip                  */
   double  *weight;             /* [n]  F_i = w_i f_i  (t_i * N)                                  */
   double  *x;                  /* [n][d]  VEGAS points                                           */

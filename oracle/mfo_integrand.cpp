@@ -30,12 +30,12 @@ struct mfo_vegas {
 
 extern "C" int mfo_vegas_create(const mfo_config_t *cfg, mfo_vegas_t **out) {
   if (!cfg || !out) { g_err = "null argument"; return MFO_EINVAL; }
-  if (cfg->process < 0 || cfg->process > 4) { g_err = "unknown process"; return MFO_EINVAL; }
+  if (cfg->process < 0 || cfg->process > 5) { g_err = "unknown process"; return MFO_EINVAL; }
   if (cfg->n_bins < 1 || cfg->n_bins > 255) { g_err = "n_bins out of range"; return MFO_EINVAL; }
   if (!(cfg->sqrt_s > 0)) { g_err = "sqrt_s must be positive"; return MFO_EINVAL; }
   mfo_vegas *h = new (std::nothrow) mfo_vegas(); if (!h) return MFO_ENOMEM;
   h->cfg = *cfg;
-  static const uint32_t nfin[5] = {2, 2, 3, 4, 2};
+  static const uint32_t nfin[6] = {2, 2, 3, 4, 2, 2};
   h->n_final = nfin[cfg->process];
   h->d = (cfg->process == MFO_EE_MUMU) ? 2 : 2 + 3 * h->n_final - 4;
   if (cfg->generator & ~(uint32_t)(MFO_GEN_CLASSIC_RAMBO | MFO_GEN_LINEAR_TAU)) { g_err = "unknown generator flag"; delete h; return MFO_EINVAL; }
@@ -47,7 +47,7 @@ extern "C" int mfo_vegas_create(const mfo_config_t *cfg, mfo_vegas_t **out) {
     if (!cfg->pdf_xf || cfg->pdf_nx < 2 || cfg->pdf_nq < 2) { g_err = "pdf grid required"; delete h; return MFO_EINVAL; }
     const uint32_t nf = cfg->pdf_nf ? cfg->pdf_nf : 1;
     if (nf != 1 && nf != 11) { g_err = "pdf_nf must be 0, 1 or 11"; delete h; return MFO_EINVAL; }
-    if ((cfg->process == MFO_QQ_TT) != (nf == 11)) { g_err = "process 4 needs the 11-flavour grid, processes 1-3 the gluon table"; delete h; return MFO_EINVAL; }
+    if ((cfg->process == MFO_QQ_TT || cfg->process == MFO_PP_TT) != (nf == 11)) { g_err = "processes 4 and 5 need the 11-flavour grid, processes 1-3 the gluon table"; delete h; return MFO_EINVAL; }
     h->pdf.assign(cfg->pdf_xf, cfg->pdf_xf + (size_t)nf * cfg->pdf_nx * cfg->pdf_nq); h->cfg.pdf_xf = h->pdf.data();
     h->masses[0] = h->masses[1] = cfg->m_top;
     uint32_t ngl = h->n_final - 2;
@@ -106,7 +106,7 @@ static double one_event(const mfo_vegas *h, uint32_t iteration, uint64_t ev, Eve
   uint32_t ngl = n - 2;
   if (ngl > 0) R.pass = mfo_cuts(ngl, k + 8, x1, x2, c.ptmin_g, c.etamax_g, c.drmin_gg, nullptr);   // O7
   double q2 = c.mu_f * c.mu_f;
-  if (c.process == MFO_QQ_TT) {                                           // O5q: flavour-summed luminosity
+  if (c.process == MFO_QQ_TT || c.process == MFO_PP_TT) {                 // O5q: flavour-summed luminosity
     const size_t tab = (size_t)c.pdf_nx * c.pdf_nq;                       // table of PDG id f at index f + 5
     long double l12 = 0, l21 = 0;
     for (int f = 1; f <= 5; ++f) {
@@ -115,6 +115,17 @@ static double one_event(const mfo_vegas *h, uint32_t iteration, uint64_t ev, Eve
       double q2_ = mfo_pdf_interp(c.pdf_xf + (5 + f) * tab, c.pdf_nx, c.pdf_nq, c.pdf_xmin, c.pdf_xmax, c.pdf_qmin, c.pdf_qmax, x2, q2);
       double a2 = mfo_pdf_interp(c.pdf_xf + (5 - f) * tab, c.pdf_nx, c.pdf_nq, c.pdf_xmin, c.pdf_xmax, c.pdf_qmin, c.pdf_qmax, x2, q2);
       l12 += (long double)q1 * a2; l21 += (long double)a1 * q2_;
+    }
+    if (c.process == MFO_PP_TT) {                                         // both subprocesses in one integrand
+      double g1 = mfo_pdf_interp(c.pdf_xf + 5 * tab, c.pdf_nx, c.pdf_nq, c.pdf_xmin, c.pdf_xmax, c.pdf_qmin, c.pdf_qmax, x1, q2);
+      double g2 = mfo_pdf_interp(c.pdf_xf + 5 * tab, c.pdf_nx, c.pdf_nq, c.pdf_xmin, c.pdf_xmax, c.pdf_qmin, c.pdf_qmax, x2, q2);
+      double mgg, mqq;
+      mfo_me2(MFO_GG_TT, m, c.m_top, c.alpha_s, c.alpha_em, &mgg);       // O6
+      mfo_me2(MFO_QQ_TT, m, c.m_top, c.alpha_s, c.alpha_em, &mqq);       // O6q
+      R.pdf[0] = g1 * g2; R.pdf[1] = (double)(l12 + l21);
+      double sum = R.pdf[0] * mgg + R.pdf[1] * mqq;
+      R.me2 = sum / (R.pdf[0] + R.pdf[1]);
+      return JV * Jx * (sum / (x1 * x2)) * h->sym * w3[0] * w3[1] * c.gev2_to_pb / (2.0 * shat);
     }
     R.pdf[0] = (double)l12; R.pdf[1] = (double)l21;
     mfo_me2(c.process, m, c.m_top, c.alpha_s, c.alpha_em, &R.me2);        // O6q

@@ -6,7 +6,8 @@ import numpy as np
 
 EE_MUMU, GG_TT, GG_TTG, GG_TTGG = 0, 1, 2, 3
 QQ_TT = 4                                      # q q~ -> t t~ summed over five light flavours
-PROCESS_NAMES = {EE_MUMU: "ee_mumu", GG_TT: "gg_tt", GG_TTG: "gg_ttg", GG_TTGG: "gg_ttgg", QQ_TT: "qq_tt"}
+PP_TT = 5                                      # p p -> t t~ at LO: g g -> t t~ and q q~ -> t t~ in one integrand
+PROCESS_NAMES = {EE_MUMU: "ee_mumu", GG_TT: "gg_tt", GG_TTG: "gg_ttg", GG_TTGG: "gg_ttgg", QQ_TT: "qq_tt", PP_TT: "pp_tt"}
 PDF_NF = 11                                    # flavour tables of the 11-flavour grid, index = PDG id + 5 (b~ .. g .. b)
 
 GEN_CLASSIC_RAMBO, GEN_LINEAR_TAU = 1, 2      # `generator` flags; 0 = the generators of the configs
@@ -65,7 +66,7 @@ def config(process, seed=0, **over):
              pdf_qmin=PDF_QMIN, pdf_qmax=PDF_QMAX, generator=0)
     if process == EE_MUMU:
         c.update(sqrt_s=100.0, pdf_xf=None)
-    if process == QQ_TT:
+    if process in (QQ_TT, PP_TT):
         c.update(pdf_xf=synthetic_flavour_grid())
     if process in (GG_TTG, GG_TTGG):
         c.update(ptmin_g=30.0, etamax_g=2.5)

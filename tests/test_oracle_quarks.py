@@ -135,3 +135,31 @@ def test_qq_tt_cross_section_against_quadrature(mfo):
             v.iterate(100_000, n_threads=mfo.max_threads())
         r = v.result()
         assert abs(r["integral"] - sigma_q) < 4 * r["sigma"] and r["sigma"] / sigma_q < 3e-3, (gen, r, sigma_q)
+
+
+def test_pp_tt_is_the_sum_of_its_subprocesses(mfo):
+    """process 5 (p p -> t t~: g g and q q~ in one integrand): event by event the weight is the sum of the weights of the
+    two pinned subprocesses on the same points (same seed, same grid: d = 4 for all three), the record holds the two
+    luminosities, and the cross section is the sum of the two quadrature values (1074.39 + 79.96 pb)"""
+    g11 = W.synthetic_flavour_grid()
+    cfg5 = W.config(W.PP_TT, seed=21)
+    v5, v1, v4 = mfo.Vegas(cfg5), mfo.Vegas(W.config(W.GG_TT, seed=21)), mfo.Vegas(W.config(W.QQ_TT, seed=21))
+    assert v5.d == 4 and v5.n_final == 2
+    rng = np.random.default_rng(2)
+    w = rng.uniform(0.4, 1.6, size=(4, 50))
+    e = np.concatenate([np.zeros((4, 1)), np.cumsum(w, axis=1) / w.sum(axis=1, keepdims=True)], axis=1); e[:, -1] = 1.0
+    for v in (v5, v1, v4):
+        v.set_grid(e)
+    n = 400
+    o5, o1, o4 = v5.eval(2, 10, n), v1.eval(2, 10, n), v4.eval(2, 10, n)
+    assert np.array_equal(o5["x"], o1["x"]) and np.array_equal(o5["momenta"], o4["momenta"])
+    np.testing.assert_allclose(o5["weight"], o1["weight"] + o4["weight"], rtol=1e-13)
+    np.testing.assert_allclose(o5["pdf"][:, 0], o1["pdf"][:, 0] * o1["pdf"][:, 1], rtol=1e-14)
+    np.testing.assert_allclose(o5["pdf"][:, 1], o4["pdf"].sum(axis=1), rtol=1e-14)
+    lum = o5["pdf"]
+    np.testing.assert_allclose(o5["me2"] * lum.sum(axis=1), lum[:, 0] * o1["me2"] + lum[:, 1] * o4["me2"], rtol=1e-13)
+    v = mfo.Vegas(W.config(W.PP_TT, seed=0))
+    for _ in range(5):
+        v.iterate(100_000, n_threads=mfo.max_threads())
+    r = v.result()
+    assert abs(r["integral"] - (1074.393 + 79.96)) < 4 * r["sigma"] + 0.03 and r["sigma"] < 1.5, r

@@ -294,8 +294,8 @@ def run_processes(args):
     torch.cuda.set_device(0)
     peak = binding.fp64_peak(0, 0.3) / 1e12
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    sizes = {W.EE_MUMU: 100_000, W.GG_TT: 1_000_000, W.GG_TTG: 10_000_000, W.GG_TTGG: 1_000_000, W.QQ_TT: 1_000_000}
-    cases = [(W.EE_MUMU, 0), (W.GG_TT, 0), (W.GG_TT, 1), (W.GG_TT, 2), (W.QQ_TT, 0), (W.QQ_TT, 1),
+    sizes = {W.EE_MUMU: 100_000, W.GG_TT: 1_000_000, W.GG_TTG: 10_000_000, W.GG_TTGG: 1_000_000, W.QQ_TT: 1_000_000, W.PP_TT: 1_000_000}
+    cases = [(W.EE_MUMU, 0), (W.GG_TT, 0), (W.GG_TT, 1), (W.GG_TT, 2), (W.QQ_TT, 0), (W.QQ_TT, 1), (W.PP_TT, 0),
              (W.GG_TTG, 0), (W.GG_TTG, 1), (W.GG_TTG, 2), (W.GG_TTG, 3), (W.GG_TTGG, 0), (W.GG_TTGG, 1)]
     rows = []
     for proc, gen in cases:

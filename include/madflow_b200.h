@@ -32,13 +32,18 @@ typedef struct mf_vegas mf_vegas_t;
 enum { MF_OK = 0, MF_EINVAL = -1, MF_ENOMEM = -2, MF_ECUDA = -3, MF_ESTATE = -4, MF_EUNSUPPORTED = -5 };
 /* processes (BASELINE.json configs 0-3; 4 = the quark channel of SURVEY 8(f)2) */
 enum { MF_EE_MUMU = 0, MF_GG_TT = 1, MF_GG_TTG = 2, MF_GG_TTGG = 3,
-       MF_QQ_TT = 4 };     /* quark channel ("any process generated (at LO)"): q q~ -> t t~, one
+       MF_QQ_TT = 4, MF_PP_TT = 5 };
+                           /* MF_QQ_TT: quark channel ("any process generated (at LO)"): q q~ -> t t~, one
                             * s-channel-gluon diagram, averaged over 4 helicities x 9 colours, with the parton luminosity
                             * summed over the five light flavours and both beam orientations:
                             *   F = J_V J_x [sum_q f_q(x1) f_q~(x2) + f_q~(x1) f_q(x2)] |M|^2 W_PS K / (2 shat).
                             * Kinematics, VEGAS dimensions and selectable generators of process 1; fused path.  Needs the
                             * 11-flavour grid (pdf_nf = 11).  mf_eval_out_t.pdf then holds the two flavour sums
-                            * sum_q xf_q(x1) xf_q~(x2) and sum_q xf_q~(x1) xf_q(x2).                                      */
+                            * sum_q xf_q(x1) xf_q~(x2) and sum_q xf_q~(x1) xf_q(x2).
+                            * MF_PP_TT = 5: p p -> t t~ at LO, the subprocesses g g -> t t~ and q q~ -> t t~ in one integrand,
+                            *   F = J_V J_x [xg(x1) xg(x2) |M_gg|^2 + (L12 + L21) |M_qq|^2] / (x1 x2) W_PS K / (2 shat)
+                            * on the same grid (gluon = table 5); mf_eval_out_t.pdf = {xg(x1) xg(x2), L12 + L21}, me2 = the
+                            * luminosity-weighted mean of the two |M|^2.                                                   */
 
 /* Selectable generators (the paper fixes no phase-space algorithm):
  *  MF_GEN_CLASSIC_RAMBO  textbook RAMBO (Kleiss, Stirling, Ellis 1986) from 4 n_final uniforms in place of the
@@ -70,9 +75,9 @@ typedef struct {
   uint32_t pdf_nx, pdf_nq;   /* knots, uniform in ln x resp. ln Q^2; nx*nq*8 bytes <= 160 KB         */
   double   pdf_xmin, pdf_xmax, pdf_qmin, pdf_qmax;
   uint32_t pdf_nf;           /* flavour tables in pdf_xf: 0 or 1 = the gluon table [nx][nq] (processes 1-3);         */
-  uint32_t reserved1;        /* 11 = [11][nx][nq], flavour index = PDG id + 5 (b~ c~ s~ u~ d~ g d u s c b): process 4. */
-                             /* The library stages the ten quark tables flavour-innermost in shared memory, keeping   */
-                             /* the <= 4 Q^2 rows the stencil of the fixed mu_f touches (32 KB)                     */
+  uint32_t reserved1;        /* 11 = [11][nx][nq], flavour index = PDG id + 5 (b~ c~ s~ u~ d~ g d u s c b): processes 4, 5. */
+                             /* The library stages the tables flavour-innermost in shared memory, keeping             */
+                             /* the <= 4 Q^2 rows the stencil of the fixed mu_f touches (36 KB)                     */
 } mf_config_t;
 
 /* Optional per-event outputs of mf_integrand_eval.  DEVICE pointers, caller-owned, NULL = skip.     */

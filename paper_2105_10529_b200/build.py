@@ -1,5 +1,5 @@
 """In-tree build of libmadflow_b200.so for sm_100a: run the amplitude generator, compile the C-ABI
-and the five per-process kernel objects in parallel with nvcc, link.  `python -m
+and the six per-process kernel objects in parallel with nvcc, link.  `python -m
 paper_2105_10529_b200.build [--force]`."""
 import os
 import subprocess
@@ -18,7 +18,7 @@ def _newer(target, deps):
     return os.path.exists(target) and all(os.path.getmtime(target) >= os.path.getmtime(d) for d in deps)
 
 
-def build(force=False, verbose=False, extra_flags=(), tag="", only=(0, 1, 2, 3, 4)):
+def build(force=False, verbose=False, extra_flags=(), tag="", only=(0, 1, 2, 3, 4, 5)):
     """tag/extra_flags/only: tuning variants (objects and library get the tag as a suffix)"""
     global OBJ, LIB
     obj_dir = OBJ + tag
@@ -31,7 +31,7 @@ def build(force=False, verbose=False, extra_flags=(), tag="", only=(0, 1, 2, 3, 
     api = kern + [os.path.join(CSRC, f) for f in ("mf_small_kernels.cuh", "mf_params.h")]
     api += [os.path.join(os.path.dirname(HERE), "include", "madflow_b200.h")]
     jobs = [("mf_api.o", os.path.join(CSRC, "mf_api.cu"), [])]
-    jobs += [("mf_proc%d.o" % p, os.path.join(CSRC, "mf_proc.cu" if p in only else "mf_proc_stub.cu"), ["-DMF_PROC=%d" % p]) for p in range(5)]
+    jobs += [("mf_proc%d.o" % p, os.path.join(CSRC, "mf_proc.cu" if p in only else "mf_proc_stub.cu"), ["-DMF_PROC=%d" % p]) for p in range(6)]
 
     def compile_one(job):
         obj, src, extra = job
@@ -45,7 +45,7 @@ def build(force=False, verbose=False, extra_flags=(), tag="", only=(0, 1, 2, 3, 
             raise RuntimeError("nvcc failed for %s:\n%s" % (obj, (r.stdout + r.stderr)[-4000:]))
         return obj, "compiled"
 
-    with ThreadPoolExecutor(max_workers=6) as ex:
+    with ThreadPoolExecutor(max_workers=7) as ex:
         results = list(ex.map(compile_one, jobs))
     objs = [os.path.join(obj_dir, j[0]) for j in jobs]
     if force or not _newer(lib, objs):

@@ -79,6 +79,7 @@ struct MfParams {
   double s, ltau0, m_top;               // collider s, ln(shat_min / s)            (O3)
   double tau0;                          // shat_min / s (linear-tau variant O3')
   double me_pref;                       // g_s^(2 ng) / 256 * generator scale, or e^4/4 (O6)
+  double me_pref_qq;                    // g_s^4 (2/9) / 4: q q~ -> t t~ (O6q; processes 4 and 5)
   double ptmin, etamax, drmin;          // cuts (O7)
   double tanh_etamax;                   // tanh(etamax): the eta cut is taken on tanh (mf_cuts)
   int32_t n_obs, obs_kind[4], obs_nb[4];  // observable histograms (include/madflow_b200.h mf_set_observables)
@@ -87,14 +88,14 @@ struct MfParams {
   double pdf_lx0, pdf_ihx, pdf_lq0, pdf_ihq, pdf_lq;   // ln xmin, 1/h_x, ln qmin^2, 1/h_q, ln muF^2
   int32_t pdf_nx, pdf_nq;
   int32_t pdf_smem;                     // doubles of the PDF table staged in shared memory: nx*nq (gluon table), or
-                                        // nx*pdf_nqs*MF_NQF for the flavour grid of the quark channel
+                                        // nx*(pdf_nqs*MF_NFL + MF_XPAD) for the flavour grid of the quark channels
   int32_t pdf_iq0, pdf_nqs;             // flavour grid: first Q^2 row and number of rows kept (<= 4): mu_F is a run constant, so
                                         // only the rows its stencil touches are staged (32 KB instead of 400 KB); the
                                         // interpolation in Q^2 is still evaluated per event (A17)
 };
 #define MF_XPAD 1                       // padding doubles per ln-x row of the staged flavour grid (bank spread)
-#define MF_NQF 10                       // quark/antiquark tables of the flavour grid, device layout [nx][pdf_nqs * MF_NQF + MF_XPAD]:
-                                        // slot 5 - q = antiquark, 4 + q = quark of flavour q = 1..5 (d u s c b)
+#define MF_NFL 11                       // tables of the flavour grid, device layout [nx][pdf_nqs * MF_NFL + MF_XPAD], slot =
+                                        // PDG id + 5: 5 - q = antiquark, 5 = gluon, 5 + q = quark of flavour q = 1..5 (d u s c b)
 
 // ---- S1: Philox4x32-10 (Salmon et al. SC'11), reading O1/A1 ----------------------------------
 MF_HD uint32_t mf_mulhi32(uint32_t a, uint32_t b) {
@@ -343,7 +344,7 @@ MF_HD double mf_hermite(double fm1, double f0, double f1, double f2, bool has_m1
 }
 
 // xf(x, Q^2) from the table `tab` [nx][nq] (shared memory on the device); lx = ln x, lq = ln Q^2.
-// STRIDE: doubles between neighbouring (ix, iq) entries (1 = single table [nx][nq]; MF_NQF = flavour-innermost grid, of
+// STRIDE: doubles between neighbouring (ix, iq) entries (1 = single table [nx][nq]; MF_NFL = flavour-innermost grid, of
 // which the rows pdf_iq0 .. pdf_iq0 + pdf_nqs - 1 are present)
 template <int STRIDE>
 MF_HD double mf_pdf_strided(const MfParams& P, const double* tab, double lx, double lq);
@@ -360,7 +361,7 @@ MF_HD double mf_pdf_strided(const MfParams& P, const double* tab, double lx, dou
   tq = tq < 0.0 ? 0.0 : (tq > 1.0 ? 1.0 : tq);
   const bool xm = ix > 0, xp = ix + 2 < nx, qm = iq > 0, qp = iq + 2 < nq;
   // doubles per ln-x row of `tab` and its first Q^2 row; the flavour grid pads every ln-x row by MF_XPAD doubles so that
-  // the rows of different lanes fall on different shared-memory banks (41 doubles: odd)
+  // the rows of different lanes fall on different shared-memory banks (45 doubles: odd)
   const int rs = STRIDE == 1 ? nq : P.pdf_nqs * STRIDE + MF_XPAD, q0 = STRIDE == 1 ? 0 : P.pdf_iq0;
   const int r0 = (xm ? ix - 1 : ix) * rs, r1 = ix * rs, r2 = (ix + 1) * rs, r3 = (xp ? ix + 2 : ix + 1) * rs;
   double row[4];
@@ -374,15 +375,15 @@ MF_HD double mf_pdf_strided(const MfParams& P, const double* tab, double lx, dou
   return mf_hermite(row[0], row[1], row[2], row[3], qm, qp, tq);
 }
 
-// O5q: flavour-summed q q~ luminosity from the flavour-innermost grid tab [nx][pdf_nqs][MF_NQF] (shared
+// O5q: flavour-summed q q~ luminosity from the flavour-innermost grid tab [nx][pdf_nqs][MF_NFL] (shared
 // memory on the device): l12 = sum_q xf_q(x1) xf_q~(x2), l21 = sum_q xf_q~(x1) xf_q(x2), q = d u s c b.  The 16-point
-// stencil of one x is shared by the ten tables: each of its points is one contiguous 80-byte read.
+// stencil of one x is shared by all tables: each of its points is one contiguous 88-byte read.
 MF_HD void mf_lumi_qq(const MfParams& P, const double* tab, double lx1, double lx2, double lq, double& l12, double& l21) {
   l12 = 0.0; l21 = 0.0;
 #pragma unroll
   for (int q = 1; q <= 5; ++q) {
-    const double q1 = mf_pdf_strided<MF_NQF>(P, tab + 4 + q, lx1, lq), a1 = mf_pdf_strided<MF_NQF>(P, tab + 5 - q, lx1, lq);
-    const double q2 = mf_pdf_strided<MF_NQF>(P, tab + 4 + q, lx2, lq), a2 = mf_pdf_strided<MF_NQF>(P, tab + 5 - q, lx2, lq);
+    const double q1 = mf_pdf_strided<MF_NFL>(P, tab + 5 + q, lx1, lq), a1 = mf_pdf_strided<MF_NFL>(P, tab + 5 - q, lx1, lq);
+    const double q2 = mf_pdf_strided<MF_NFL>(P, tab + 5 + q, lx2, lq), a2 = mf_pdf_strided<MF_NFL>(P, tab + 5 - q, lx2, lq);
     l12 = fma(q1, a2, l12); l21 = fma(a1, q2, l21);
   }
 }

@@ -25,7 +25,9 @@ template <> struct MfProc<2> { static const int D = 7, N = 3, NGL = 1, GROUP = 1
 template <> struct MfProc<3> { static const int D = 10, N = 4, NGL = 2, GROUP = 256; };
 // q q~ -> t t~ summed over five flavours: kinematics of process 1, PDF = flavour grid in global memory
 template <> struct MfProc<4> { static const int D = 4, N = 2, NGL = 0, GROUP = 128; };
-template <int PROC> struct MfPdf { static const bool FLAVOURS = PROC == 4; };
+// p p -> t t~ at LO: the subprocesses g g -> t t~ and q q~ -> t t~ in one integrand (kinematics of process 1)
+template <> struct MfProc<5> { static const int D = 4, N = 2, NGL = 0, GROUP = 128; };
+template <int PROC> struct MfPdf { static const bool FLAVOURS = PROC == 4 || PROC == 5; };
 // Generator selection of the front end, template parameter CL:
 //   0  the generators of the configs, nothing selectable (the path bench.py times: no branch)
 //   1  classic 4n-random RAMBO, d = 2 + 4n; the tau map (O3 or O3') is a run-time, grid-uniform branch on P.gen
@@ -88,7 +90,7 @@ MF_HD T mf_me2(const MfParams& P, T rts, const T k[MfProc<PROC>::N][4]) {
     const T pa[4] = {E, T(0.0), T(0.0), E}, pb[4] = {E, T(0.0), T(0.0), -E};
     mf_fermion_ing<T>(pa, T(0.0), in); mf_fermion_ing<T>(pb, T(0.0), in + 5);
     mf_fermion_ing<T>(k[0], T(P.m_top), in + 10); mf_fermion_ing<T>(k[1], T(P.m_top), in + 15);
-    return T(P.me_pref) * mf_me2_ee_mumu<T>(in) / (rts * rts * rts * rts);
+    return T(P.me_pref_qq) * mf_me2_ee_mumu<T>(in) / (rts * rts * rts * rts);
   } else if (PROC == 1) {
     static_assert(MF_ME2_GG_TT_NIN == 20, "generator input layout changed");
     T in[20];
@@ -107,6 +109,14 @@ MF_HD T mf_me2(const MfParams& P, T rts, const T k[MfProc<PROC>::N][4]) {
   }
 }
 
+// S7 weighted with the parton luminosities: process 5 returns xg(x1) xg(x2) |M_gg|^2 + (L12 + L21) |M_qq|^2 (lum = the two
+// luminosities from the front end); every other process its |M|^2
+template <int PROC, typename T>
+MF_HD T mf_me2_lum(const MfParams& P, T rts, const T k[MfProc<PROC>::N][4], const double* lum) {
+  if (PROC == 5) return T(lum[0]) * mf_me2<1, T>(P, rts, k) + T(lum[1]) * mf_me2<4, T>(P, rts, k);
+  return mf_me2<PROC == 5 ? 1 : PROC, T>(P, rts, k);
+}
+
 // Front end of one event, S1-S6 + the weight prefactor: F = pref * |M|^2 for a passing event with
 //   config 0   : pref = J_V (1/(8 pi)) K / (2 s)
 //   configs 1-3: pref = J_V J_x f_g(x1) f_g(x2) S_f W_0 W_m K / (2 shat)
@@ -114,7 +124,7 @@ MF_HD T mf_me2(const MfParams& P, T rts, const T k[MfProc<PROC>::N][4]) {
 template <int PROC, bool REC, int CL = 0>
 MF_HD bool mf_event_front(const MfParams& P, const double* edges, const double* pdf_tab, uint32_t iteration,
                           uint64_t ev, int bin[MfDim<PROC, CL>::D], double k[MfProc<PROC>::N][4], double& rts,
-                          double& pref, MfEventRec* rec, unsigned* okeys = nullptr) {
+                          double& pref, MfEventRec* rec, unsigned* okeys = nullptr, double* lum = nullptr) {
   constexpr int D = MfDim<PROC, CL>::D, N = MfProc<PROC>::N, NGL = MfProc<PROC>::NGL;
   static_assert(PROC != 0 || CL == 0, "generator variants apply to processes 1-3");
   double u[D], y[D];
@@ -133,6 +143,12 @@ MF_HD bool mf_event_front(const MfParams& P, const double* edges, const double* 
   if (MfPdf<PROC>::FLAVOURS) {                                           // S6q: flavour-summed luminosity (xf1, xf2 = the two sums)
     mf_lumi_qq(P, pdf_tab, lx1, lx2, P.pdf_lq, xf1, xf2);
     ff = (xf1 + xf2) / (x1 * x2 * shat);
+    if (PROC == 5) {                                                     // both subprocesses: the luminosities go to S7 (mf_me2_lum)
+      const double g1 = mf_pdf_strided<MF_NFL>(P, pdf_tab + 5, lx1, P.pdf_lq), g2 = mf_pdf_strided<MF_NFL>(P, pdf_tab + 5, lx2, P.pdf_lq);
+      lum[0] = g1 * g2; lum[1] = xf1 + xf2;
+      xf1 = lum[0]; xf2 = lum[1];                                        // the record holds the two luminosities
+      ff = 1.0 / (x1 * x2 * shat);
+    }
   } else if (PROC != 0 && (REC || pass)) {                               // S6
     xf1 = mf_pdf(P, pdf_tab, lx1, P.pdf_lq);
     xf2 = mf_pdf(P, pdf_tab, lx2, P.pdf_lq);
@@ -164,8 +180,8 @@ MF_HD double mf_event(const MfParams& P, const double* edges, const double* pdf_
                       uint32_t iteration, uint64_t ev, int bin[MfDim<PROC, CL>::D], bool& pass,
                       MfEventRec* rec, unsigned* okeys = nullptr) {
   constexpr int N = MfProc<PROC>::N;
-  double k[N][4], rts, pref;
-  pass = mf_event_front<PROC, REC, CL>(P, edges, pdf_tab, iteration, ev, bin, k, rts, pref, rec, okeys);
+  double k[N][4], rts, pref, lum[2] = {0.0, 0.0};
+  pass = mf_event_front<PROC, REC, CL>(P, edges, pdf_tab, iteration, ev, bin, k, rts, pref, rec, okeys, lum);
   double me2 = 0.0;
   if (MF_UNIFORM_ME || pass) {                                           // S7 (in the real type T)
     T kt[N][4];
@@ -173,9 +189,9 @@ MF_HD double mf_event(const MfParams& P, const double* edges, const double* pdf_
     for (int i = 0; i < N; ++i)
 #pragma unroll
       for (int c = 0; c < 4; ++c) kt[i][c] = (T)k[i][c];
-    me2 = (double)mf_me2<PROC, T>(P, (T)rts, kt);
+    me2 = (double)mf_me2_lum<PROC, T>(P, (T)rts, kt, lum);
   }
   if (!pass) me2 = 0.0;
-  if (REC) rec->me2 = me2;
+  if (REC) rec->me2 = PROC == 5 ? me2 / (lum[0] + lum[1]) : me2;         // process 5: the luminosity-weighted mean |M|^2
   return pass ? pref * me2 : 0.0;                                        // S8
 }

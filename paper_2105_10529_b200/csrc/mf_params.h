@@ -8,8 +8,8 @@
 static_assert(MFD_GEN_CLASSIC == MF_GEN_CLASSIC_RAMBO && MFD_GEN_LINEAR == MF_GEN_LINEAR_TAU, "device flags follow the header");
 
 static inline int mf_process_shape(int process, uint32_t generator, int* d, int* n_final, int* ng) {
-  static const int nf[5] = {2, 2, 3, 4, 2};
-  if (process < 0 || process > 4) return -1;
+  static const int nf[6] = {2, 2, 3, 4, 2, 2};
+  if (process < 0 || process > 5) return -1;
   *n_final = nf[process];
   *d = (process == MF_EE_MUMU) ? 2 : 2 + 3 * nf[process] - 4;
   if (generator & MF_GEN_CLASSIC_RAMBO) *d = 2 + 4 * nf[process];       // O4': 4n uniforms
@@ -17,19 +17,15 @@ static inline int mf_process_shape(int process, uint32_t generator, int* d, int*
   return 0;
 }
 
-// device copy of the 11-flavour grid (process 4): host [11][nx][nq] (index = PDG id + 5) -> the ten quark tables,
-// flavour-innermost, rows pdf_iq0 .. pdf_iq0 + pdf_nqs - 1 only: out[nx][pdf_nqs * MF_NQF + MF_XPAD] (P.pdf_smem doubles, zeroed
-// by the caller: the pad entries are never read).
-// Slots 0..4 = b~ c~ s~ u~ d~ (5 - q), 5..9 = d u s c b (4 + q); the gluon table is not used by q q~ -> t t~.
+// device copy of the 11-flavour grid (processes 4 and 5): host [11][nx][nq] (index = PDG id + 5) -> flavour-innermost,
+// rows pdf_iq0 .. pdf_iq0 + pdf_nqs - 1 only: out[nx][pdf_nqs * MF_NFL + MF_XPAD] (P.pdf_smem doubles, zeroed by the caller:
+// the pad entries are never read), slot = PDG id + 5.
 static inline void mf_flavour_slice(const MfParams& P, const double* pdf11, double* out) {
   const size_t ntab = (size_t)P.pdf_nx * P.pdf_nq;
-  for (int f = 0; f < 11; ++f) {
-    if (f == 5) continue;
-    const int slot = f < 5 ? f : f - 1;
+  for (int f = 0; f < MF_NFL; ++f)
     for (int ix = 0; ix < P.pdf_nx; ++ix)
       for (int r = 0; r < P.pdf_nqs; ++r)
-        out[(size_t)ix * (P.pdf_nqs * MF_NQF + MF_XPAD) + r * MF_NQF + slot] = pdf11[(size_t)f * ntab + (size_t)ix * P.pdf_nq + P.pdf_iq0 + r];
-  }
+        out[(size_t)ix * (P.pdf_nqs * MF_NFL + MF_XPAD) + r * MF_NFL + f] = pdf11[(size_t)f * ntab + (size_t)ix * P.pdf_nq + P.pdf_iq0 + r];
 }
 
 // returns MF_OK or MF_EINVAL / MF_EUNSUPPORTED with a message in err
@@ -65,7 +61,7 @@ static inline int mf_fill_params(const mf_config_t* c, MfParams* P, std::string&
     if (!c->pdf_xf || c->pdf_nx < 2 || c->pdf_nq < 2) { err = "pdf grid required"; return MF_EINVAL; }
     const uint32_t nfl = c->pdf_nf ? c->pdf_nf : 1;
     if (nfl != 1 && nfl != 11) { err = "pdf_nf must be 0, 1 or 11"; return MF_EINVAL; }
-    if ((c->process == MF_QQ_TT) != (nfl == 11)) { err = "process 4 needs the 11-flavour grid, processes 1-3 the gluon table"; return MF_EINVAL; }
+    if ((c->process == MF_QQ_TT || c->process == MF_PP_TT) != (nfl == 11)) { err = "processes 4 and 5 need the 11-flavour grid, processes 1-3 the gluon table"; return MF_EINVAL; }
     if ((uint64_t)c->pdf_nx * c->pdf_nq * 8ull > 160ull * 1024ull) { err = "pdf table larger than 160 KB"; return MF_EINVAL; }
     if (!(c->pdf_xmin > 0.0 && c->pdf_xmax > c->pdf_xmin && c->pdf_qmin > 0.0 && c->pdf_qmax > c->pdf_qmin)) { err = "bad pdf ranges"; return MF_EINVAL; }
     const int ngl = nfin - 2;
@@ -79,7 +75,9 @@ static inline int mf_fill_params(const mf_config_t* c, MfParams* P, std::string&
     for (int i = 0; i < ng; ++i) gs2n *= 4.0 * PI * c->alpha_s;
     const double scale = (c->process == MF_GG_TT) ? MF_ME2_GG_TT_SCALE : (c->process == MF_GG_TTG) ? MF_ME2_GG_TTG_SCALE : MF_ME2_GG_TTGG_SCALE;
     p.me_pref = gs2n / 256.0 * scale;                   // 1/4 helicities x 1/64 colours (A12)
-    if (c->process == MF_QQ_TT) p.me_pref = gs2n * (2.0 / 9.0) * MF_ME2_EE_MUMU_SCALE;   // O6q: colour sum 2 / 9 colours, 1/4 spins
+    if (c->process == MF_PP_TT) p.me_pref = gs2n / 256.0 * MF_ME2_GG_TT_SCALE;         // its g g -> t t~ subprocess
+    p.me_pref_qq = gs2n * (2.0 / 9.0) * MF_ME2_EE_MUMU_SCALE;                           // O6q: colour sum 2 / 9 colours, 1/4 spins
+    if (c->process == MF_QQ_TT) p.me_pref = p.me_pref_qq;
     p.wconst = (ngl == 2 ? 0.5 : 1.0) * c->gev2_to_pb / 2.0;
     p.pdf_nx = (int)c->pdf_nx; p.pdf_nq = (int)c->pdf_nq;
     p.pdf_lx0 = log(c->pdf_xmin);
@@ -93,7 +91,7 @@ static inline int mf_fill_params(const mf_config_t* c, MfParams* P, std::string&
       iq = iq < 0 ? 0 : (iq > p.pdf_nq - 2 ? p.pdf_nq - 2 : iq);
       const int lo = iq - 1 < 0 ? 0 : iq - 1, hi = iq + 2 > p.pdf_nq - 1 ? p.pdf_nq - 1 : iq + 2;
       p.pdf_iq0 = lo; p.pdf_nqs = hi - lo + 1;
-      p.pdf_smem = p.pdf_nx * (p.pdf_nqs * MF_NQF + MF_XPAD);
+      p.pdf_smem = p.pdf_nx * (p.pdf_nqs * MF_NFL + MF_XPAD);
     }
   }
   *P = p;

@@ -1,4 +1,4 @@
-// mf_proc.cu -- the per-process kernels, compiled once per process with -DMF_PROC=0..4 so that the
+// mf_proc.cu -- the per-process kernels, compiled once per process with -DMF_PROC=0..5 so that the
 // |M|^2 codes build in parallel: the fused iteration (mf_iterate_kernel, mf_iterate_compact_kernel), the
 // staged iteration of the heavy processes (mf_front_kernel -> mf_me_kernel -> mf_hist_kernel), and the
 // per-event evaluation (mf_eval_kernel); plus their launchers (MfProcOps, mf_proc.h).
@@ -6,7 +6,7 @@
 #include "mf_proc.h"
 #include <type_traits>
 #ifndef MF_PROC
-#error "compile with -DMF_PROC=0..4"
+#error "compile with -DMF_PROC=0..5"
 #endif
 
 __device__ __forceinline__ void mf_stage_tables(const MfParams& P, const double* g_edges, const double* g_pdf,
@@ -452,11 +452,11 @@ mf_hist_kernel(const MfParams P, const double* __restrict__ rec, const unsigned 
 template <int PROC, bool REC, int CL>
 __device__ __forceinline__ bool mf_eval_front(const MfParams& P, const double* s_edges, const double* s_pdf, uint32_t iteration,
                                               unsigned long long ev, unsigned long long i, const MfEvalOutDev& o,
-                                              double k[MfProc<PROC>::N][4], double& rts, double& pref) {
+                                              double k[MfProc<PROC>::N][4], double& rts, double& pref, double* lum) {
   constexpr int D = MfDim<PROC, CL>::D, NL = 2 + MfProc<PROC>::N;
   int bin[D];
   MfEventRec rec;
-  const bool pass = mf_event_front<PROC, REC, CL>(P, s_edges, s_pdf, iteration, ev, bin, k, rts, pref, REC ? &rec : nullptr);
+  const bool pass = mf_event_front<PROC, REC, CL>(P, s_edges, s_pdf, iteration, ev, bin, k, rts, pref, REC ? &rec : nullptr, nullptr, lum);
   if (o.bins) {
 #pragma unroll
     for (int j = 0; j < D; ++j) o.bins[i * D + j] = (uint8_t)bin[j];
@@ -494,10 +494,10 @@ mf_eval_kernel(const MfParams P, const double* __restrict__ g_edges, const doubl
   for (unsigned long long base = (unsigned long long)blockIdx.x * blockDim.x; base < n; base += stride) {
     unsigned long long i = base + threadIdx.x;           // block-uniform trip count (barriers inside the event)
     if (i >= n) { if (!MF_UNIFORM_ME) break; i = n - 1; }   // tail lanes recompute event n-1 (same values written)
-    double k[N][4], rts, pref;
+    double k[N][4], rts, pref, lum[2] = {0.0, 0.0};
     bool pass;
-    if (PROC != 0 && (P.gen & MFD_GEN_CLASSIC)) pass = mf_eval_front<PROC, REC, PROC != 0 ? 1 : 0>(P, s_edges, s_pdf, iteration, first + i, i, o, k, rts, pref);
-    else pass = mf_eval_front<PROC, REC, PROC != 0 ? 2 : 0>(P, s_edges, s_pdf, iteration, first + i, i, o, k, rts, pref);
+    if (PROC != 0 && (P.gen & MFD_GEN_CLASSIC)) pass = mf_eval_front<PROC, REC, PROC != 0 ? 1 : 0>(P, s_edges, s_pdf, iteration, first + i, i, o, k, rts, pref, lum);
+    else pass = mf_eval_front<PROC, REC, PROC != 0 ? 2 : 0>(P, s_edges, s_pdf, iteration, first + i, i, o, k, rts, pref, lum);
     double me2 = 0.0;
     if (MF_UNIFORM_ME || pass) {                         // S7 (in the real type T)
       T kt[N][4];
@@ -505,13 +505,13 @@ mf_eval_kernel(const MfParams P, const double* __restrict__ g_edges, const doubl
       for (int p = 0; p < N; ++p)
 #pragma unroll
         for (int c = 0; c < 4; ++c) kt[p][c] = (T)k[p][c];
-      me2 = (double)mf_me2<PROC, T>(P, (T)rts, kt);
+      me2 = (double)mf_me2_lum<PROC, T>(P, (T)rts, kt, lum);
     }
     if (!pass) me2 = 0.0;
     double F = pass ? pref * me2 : 0.0;                  // S8
     if (!isfinite(F)) F = 0.0;
     if (o.weight) o.weight[i] = F;
-    if (REC && o.me2) o.me2[i] = me2;
+    if (REC && o.me2) o.me2[i] = PROC == 5 ? me2 / (lum[0] + lum[1]) : me2;   // process 5: luminosity-weighted mean
   }
 }
 

@@ -26,7 +26,8 @@ extern "C" double mfh_event(const MfParams* P, const double* edges, const double
     case 0: return run<0>(*P, edges, pdf, it, ev, bins, pass, rec_out);
     case 1: return run<1>(*P, edges, pdf, it, ev, bins, pass, rec_out);
     case 2: return run<2>(*P, edges, pdf, it, ev, bins, pass, rec_out);
-    case 4: return run<4>(*P, edges, pdf, it, ev, bins, pass, rec_out);   // pdf: flavour-innermost [nx][nq][10]
+    case 4: return run<4>(*P, edges, pdf, it, ev, bins, pass, rec_out);   // pdf: the library's flavour slice (mfh_flavour_slice)
+    case 5: return run<5>(*P, edges, pdf, it, ev, bins, pass, rec_out);
 #ifndef MFH_NO_TTGG
     case 3: return run<3>(*P, edges, pdf, it, ev, bins, pass, rec_out);
 #endif
@@ -66,6 +67,7 @@ extern "C" double mfh_event_gen(const MfParams* P, const double* edges, const do
   const bool cl = P->gen & MFD_GEN_CLASSIC;
   switch (P->process) {
     case 1: return cl ? run_gen<1, 1>(*P, edges, pdf, it, ev, bins, pass, rec_out) : run_gen<1, 2>(*P, edges, pdf, it, ev, bins, pass, rec_out);
+    case 5: return cl ? run_gen<5, 1>(*P, edges, pdf, it, ev, bins, pass, rec_out) : run_gen<5, 2>(*P, edges, pdf, it, ev, bins, pass, rec_out);
     case 4: return cl ? run_gen<4, 1>(*P, edges, pdf, it, ev, bins, pass, rec_out) : run_gen<4, 2>(*P, edges, pdf, it, ev, bins, pass, rec_out);
     case 2: return cl ? run_gen<2, 1>(*P, edges, pdf, it, ev, bins, pass, rec_out) : run_gen<2, 2>(*P, edges, pdf, it, ev, bins, pass, rec_out);
 #ifndef MFH_NO_TTGG

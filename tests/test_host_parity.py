@@ -137,26 +137,25 @@ def test_generator_flag_validation(harness):
 
 
 def flavour_slice(harness, P, pdf11):
-    """the library's device copy of the 11-flavour grid (mf_params.h mf_flavour_slice): the ten quark tables,
-    flavour-innermost, the Q^2 rows around mu_F only; checked here against a NumPy re-layout"""
+    """the library's device copy of the 11-flavour grid (mf_params.h mf_flavour_slice): the tables flavour-innermost
+    (slot = PDG id + 5), the Q^2 rows around mu_F only; checked here against a NumPy re-layout"""
     n = harness.mfh_flavour_slice(P, pdf11.ctypes.data, None)
     out = np.zeros(n)
     harness.mfh_flavour_slice(P, pdf11.ctypes.data, out.ctypes.data)
     nx, nq = pdf11.shape[1:]
     iq = int(np.floor((np.log(173.0 ** 2) - np.log(W.PDF_QMIN ** 2)) / (np.log(W.PDF_QMAX ** 2) - np.log(W.PDF_QMIN ** 2)) * (nq - 1)))
-    keep = [f for f in range(11) if f != 5]
-    ref = np.transpose(pdf11[keep][:, :, iq - 1:iq + 3], (1, 2, 0))
-    assert n == nx * (ref.shape[1] * 10 + 1) and np.array_equal(out.reshape(nx, -1)[:, :-1].reshape(ref.shape), ref)   # one pad double per ln-x row
+    ref = np.transpose(pdf11[:, :, iq - 1:iq + 3], (1, 2, 0))
+    assert n == nx * (ref.shape[1] * 11 + 1) and np.array_equal(out.reshape(nx, -1)[:, :-1].reshape(ref.shape), ref)   # one pad double per ln-x row
     return out
 
 
-@pytest.mark.parametrize("gen,n", [(0, 300), (1, 150), (2, 150)])
-def test_host_compiled_quark_channel_matches_oracle(mfo, harness, gen, n):
+@pytest.mark.parametrize("proc,gen,n", [(4, 0, 300), (4, 1, 150), (4, 2, 150), (5, 0, 300), (5, 3, 150)])
+def test_host_compiled_quark_channel_matches_oracle(mfo, harness, proc, gen, n):
     """q q~ -> t t~ with the flavour-summed luminosity of the product's per-event code, compiled for
     the host, against the oracle: bins, momenta, the two flavour sums, |M|^2 and the weight"""
     harness.mfh_event_gen.restype = C.c_double
     harness.mfh_event_gen.argtypes = harness.mfh_event.argtypes
-    cfg = W.config(W.QQ_TT, seed=13, generator=gen)
+    cfg = W.config(proc, seed=13, generator=gen)                  # 4 = q q~ -> t t~, 5 = p p -> t t~ (g g + q q~)
     c, pdf = make_config(cfg)
     assert c.pdf_nf == 11
     P = C.create_string_buffer(harness.mfh_params_size())

@@ -542,3 +542,18 @@ def test_widened_rows_full_size_launch_sampled_parity(mf, mfo, proc, gen, n):
         ref = orc.eval(0, i, 1)["weight"][0]
         got = float(w[i])
         assert (ref == 0 and got == 0) or abs(got / ref - 1) < RTOL_EVENT, (i, got, ref)
+
+
+def test_fp32_matrix_element_with_generator_variants(mf):
+    """the fp32 |M|^2 stage never sees the VEGAS dimensions, so it runs unchanged behind the variant generators: same
+    events and counters as the fp64 run of the same variant, integral within fp32 rounding"""
+    for gen in (W.GEN_CLASSIC_RAMBO, W.GEN_LINEAR_TAU):
+        a = mf.Vegas(W.config(W.GG_TTG, seed=5, generator=gen))
+        b = mf.Vegas(W.config(W.GG_TTG, seed=5, generator=gen, precision=32))
+        ia, ib = a.vegas_iterate(200_000), b.vegas_iterate(200_000)
+        assert ia["n_pass"] == ib["n_pass"] and ib["n_nonfinite"] == 0 and abs(ib["integral"] / ia["integral"] - 1) < 1e-5
+        wa = a.integrand_eval(1, 0, 4000, debug=True); wb = b.integrand_eval(1, 0, 4000, debug=True)
+        assert (wa["bins"] == wb["bins"]).all() and (wa["pass_"] == wb["pass_"]).all()
+        nz = wa["weight"] != 0
+        rel = (wb["weight"][nz] / wa["weight"][nz] - 1).abs()
+        assert float(rel.median()) < 1e-5 and float((rel > 1e-4).double().mean()) < 5e-3      # north_star: 1e-4 for the fp32 path

@@ -39,8 +39,9 @@ static inline float rsqrt(float x) { return 1.0f / sqrtf(x); }
 // group is in its per-event prologue the other keeps the FP64 pipe busy).
 #define MF_GROUP_SYNC() asm volatile("bar.sync %0, 128;" :: "r"(1 + (int)(threadIdx.x >> 7)) : "memory")
 #define MF_SYNC_POINT(i) do { if (MF_SYNC_EVERY > 0 && (i) % (MF_SYNC_EVERY > 0 ? MF_SYNC_EVERY : 1) == 0) MF_GROUP_SYNC(); } while (0)
-// gg -> tt~gg: the loop body is ~0.5 MB of SASS, instruction fetch is the bottleneck: all eight warps of the
-// CTA stay together (whole-CTA barrier, every MF_SYNC_EVERY_WIDE-th point) and stream it once
+// whole-CTA barrier points (tuning hook, gen/amplitudes.py SYNC_MACRO): gg -> tt~gg used them while its helicity loop ran over
+// three gluons (0.5 MB of SASS per trip: one instruction stream per SM); with all four gluons in the loop the body halves and the
+// 128-thread groups of MF_SYNC_POINT are faster (profiles/r1_tuning.md)
 #ifndef MF_SYNC_EVERY_WIDE
 #define MF_SYNC_EVERY_WIDE 4
 #endif

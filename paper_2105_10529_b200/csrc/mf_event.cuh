@@ -22,7 +22,10 @@ template <int PROC> struct MfProc;
 template <> struct MfProc<0> { static const int D = 2, N = 2, NGL = 0, GROUP = 128; };
 template <> struct MfProc<1> { static const int D = 4, N = 2, NGL = 0, GROUP = 128; };
 template <> struct MfProc<2> { static const int D = 7, N = 3, NGL = 1, GROUP = 128; };
-template <> struct MfProc<3> { static const int D = 10, N = 4, NGL = 2, GROUP = 256; };
+#ifndef MF_TTGG_GROUP
+#define MF_TTGG_GROUP 128     // gg -> tt~gg: 128-thread groups like gg -> tt~g (256 = the whole CTA shares the barrier points; tuning hook)
+#endif
+template <> struct MfProc<3> { static const int D = 10, N = 4, NGL = 2, GROUP = MF_TTGG_GROUP; };
 // q q~ -> t t~ summed over five flavours: kinematics of process 1, PDF = flavour grid in global memory
 template <> struct MfProc<4> { static const int D = 4, N = 2, NGL = 0, GROUP = 128; };
 // p p -> t t~ at LO: the subprocesses g g -> t t~ and q q~ -> t t~ in one integrand (kinematics of process 1)

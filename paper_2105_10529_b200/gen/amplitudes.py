@@ -516,7 +516,7 @@ PROCESSES = {
     "mf_me2_gg_tt": lambda: Gen(2, loop_legs=(), parity=True, basis="circular"),      # 514 flops (linear: 715)
     "mf_me2_gg_ttg": lambda: Gen(3, loop_legs=_legs("MF_GEN_TTG_LOOP", (0, 2)), parity=True,
                                  loop_lam4=os.environ.get("MF_GEN_TTG_LAM4", "0") == "1", basis=BASIS),
-    "mf_me2_gg_ttgg": lambda: Gen(4, loop_legs=_legs("MF_GEN_TTGG_LOOP", (1, 2, 3)), parity=True, basis=BASIS),
+    "mf_me2_gg_ttgg": lambda: Gen(4, loop_legs=_legs("MF_GEN_TTGG_LOOP", (0, 1, 2, 3)), parity=True, basis=BASIS),
 }
 
 
@@ -527,7 +527,7 @@ DEMOTE = {"mf_me2_gg_ttg": int(os.environ.get("MF_GEN_DEMOTE_TTG", "6")),
 
 
 # barrier-point macro of the generated code (csrc/mf_device.cuh): 128-thread groups, or the whole CTA
-SYNC_MACRO = {"mf_me2_gg_ttgg": "MF_SYNC_POINT_W"}
+SYNC_MACRO = {}      # (gg -> tt~gg used MF_SYNC_POINT_W, the whole CTA, until its loop ran over all four gluons: profiles/r1_tuning.md)
 
 # emission order of the helicity-loop body (Dag.schedule): window 0 = creation order
 SCHED_WINDOW = int(os.environ.get("MF_GEN_SCHED_WINDOW", "48"))

@@ -173,6 +173,8 @@ extern "C" int mf_set_path(mf_vegas_t* h, int32_t staged) {
   if (!h) return fail(MF_EINVAL, "handle is NULL");
   if (staged && !h->rec_fields) return fail(MF_EUNSUPPORTED, "this process has the fused path only");
   if (!staged && h->f32) return fail(MF_EUNSUPPORTED, "the fp32 |M|^2 variant runs on the staged path only");
+  if (!staged && h->P.process == MF_GG_TTGG)
+    return fail(MF_EUNSUPPORTED, "gg -> tt~gg runs on the staged path only (its |M|^2 stage spreads one event over four lanes)");
   if (!staged && h->rec_fields && h->P.gen != 0)
     return fail(MF_EUNSUPPORTED, "the selectable generators of processes 2 and 3 run on the staged path only");
   h->use_staged = staged != 0;

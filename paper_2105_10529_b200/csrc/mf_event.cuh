@@ -12,10 +12,7 @@
 #define MF_GEN_TTG "generated/mf_me2_gg_ttg.cuh"
 #endif
 #include MF_GEN_TTG
-#ifndef MF_GEN_TTGG
-#define MF_GEN_TTGG "generated/mf_me2_gg_ttgg.cuh"
-#endif
-#include MF_GEN_TTGG
+#include "generated/mf_me2_gg_ttgg_lanes.cuh"     // gg -> tt~gg: one event over four lanes (gen/lanes.py)
 
 template <int PROC> struct MfProc;
 // GROUP: threads that share the barrier points of the generated |M|^2 code (mf_device.cuh)
@@ -105,19 +102,86 @@ MF_HD T mf_me2(const MfParams& P, T rts, const T k[MfProc<PROC>::N][4]) {
     mf_me_inputs_gg<3, T>(rts, T(P.m_top), (const T(*)[4])k, in);
     return T(P.me_pref) * mf_me2_gg_ttg<T>(in);
   } else {
-    static_assert(MF_ME2_GG_TTGG_NIN == 38, "generator input layout changed");
-    T in[38];
-    mf_me_inputs_gg<4, T>(rts, T(P.m_top), (const T(*)[4])k, in);
-    return T(P.me_pref) * mf_me2_gg_ttgg<T>(in);
+    static_assert(PROC != 3, "gg -> tt~gg has no one-thread |M|^2: mf_me2_ttgg_group (four lanes per event)");
+    return T(0.0);
   }
 }
+
+// ---- gg -> t t~ g g: one event over FOUR LANES (gen/lanes.py) -----------------------------------
+// The four lanes of a group (lane & 3 = 0..3 of consecutive lanes) hold the same event (rts, k).  Lane l takes the
+// six colour orderings that end with gluon l and runs the generated per-lane code on cyclically relabelled gluons
+// (local label i = global gluon (i + l) mod 4); gluon currents and partial amplitudes are exchanged through the
+// warp's shared-memory tile.  Global gluons: 0, 1 incoming along +z / -z, 2, 3 = k[2], k[3]; all-incoming momenta.
+// tile: MF_LANES_TILE doubles per warp = the exchange slots [slot][32] + per event [4][6] unit polarisation vectors
+// (eps1, eps2) and [4][4] momenta.  Every lane of the warp must call (warp barriers inside); returns |M|^2 on all
+// four lanes of the group.
+#if defined(__CUDACC__)
+#define MF_LANES_TILE (MF_ME2_GG_TTGG_LANES_SLOTS * 32 + 8 * 40)
+template <typename T>
+__device__ __forceinline__ T mf_me2_ttgg_group(const MfParams& P, T rts, const T k[4][4], T* tile) {
+  static_assert(MF_ME2_GG_TTGG_LANES_NIN == 31, "generator input layout changed");
+  const int lane = threadIdx.x & 31, lane4 = lane & 3;
+  T* Gp = tile + MF_ME2_GG_TTGG_LANES_SLOTS * 32 + (lane >> 2) * 40;
+  T* Kt = Gp + 24;
+  {                                                     // lane l publishes global gluon l
+    const T E = T(0.5) * rts, r2 = T(1.41421356237309504880);
+    T kg[4], o[5];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) kg[c] = (lane4 == 3) ? k[3][c] : k[2][c];
+    mf_gluon_ing<T>(kg, o);                             // eps / sqrt2 of an outgoing gluon
+    const bool inc = lane4 < 2;
+    const T sg = (lane4 == 0) ? T(1.0) : T(-1.0);
+    Kt[lane4 * 4 + 0] = inc ? E : -kg[0]; Kt[lane4 * 4 + 1] = inc ? T(0.0) : -kg[1];
+    Kt[lane4 * 4 + 2] = inc ? T(0.0) : -kg[2]; Kt[lane4 * 4 + 3] = inc ? sg * E : -kg[3];
+    Gp[lane4 * 6 + 0] = inc ? T(1.0) : r2 * o[0]; Gp[lane4 * 6 + 1] = inc ? T(0.0) : r2 * o[1]; Gp[lane4 * 6 + 2] = inc ? T(0.0) : r2 * o[2];
+    Gp[lane4 * 6 + 3] = inc ? T(0.0) : r2 * o[3]; Gp[lane4 * 6 + 4] = inc ? sg : r2 * o[4]; Gp[lane4 * 6 + 5] = T(0.0);
+  }
+  __syncwarp();
+  T in[31];
+  in[0] = T(P.m_top);
+#pragma unroll
+  for (int c = 0; c < 4; ++c) in[1 + c] = k[1][c];
+  mf_fermion_ing<T>(k[0], T(P.m_top), in + 5);
+  mf_fermion_ing<T>(k[1], T(P.m_top), in + 10);
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int c = 0; c < 4; ++c) in[15 + 4 * i + c] = Kt[((i + lane4) & 3) * 4 + c];
+  const int b4 = lane & ~3;
+  T acc = mf_me2_gg_ttgg_lanes<T>(in, Gp, tile, lane4, lane, b4 | ((lane4 + 1) & 3), b4 | ((lane4 + 2) & 3), b4 | ((lane4 + 3) & 3));
+  acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+  acc += __shfl_xor_sync(0xffffffffu, acc, 2);
+  return T(P.me_pref) * acc;
+}
+
+// the same for a warp whose 32 lanes hold one event each: four rounds of eight events
+template <typename T>
+__device__ __forceinline__ T mf_me2_ttgg_warp32(const MfParams& P, T rts, const T k[4][4], T* tile) {
+  const int lane = threadIdx.x & 31;
+  T out = T(0.0);
+#pragma unroll 1
+  for (int r = 0; r < 4; ++r) {
+    const int src = r * 8 + (lane >> 2);
+    T kr[4][4];
+#pragma unroll
+    for (int p = 0; p < 4; ++p)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) kr[p][c] = __shfl_sync(0xffffffffu, k[p][c], src);
+    const T rr = __shfl_sync(0xffffffffu, rts, src);
+    const T m = mf_me2_ttgg_group<T>(P, rr, kr, tile);
+    const T t = __shfl_sync(0xffffffffu, m, 4 * (lane & 7));
+    if ((lane >> 3) == r) out = t;
+  }
+  return out;
+}
+#endif
 
 // S7 weighted with the parton luminosities: process 5 returns xg(x1) xg(x2) |M_gg|^2 + (L12 + L21) |M_qq|^2 (lum = the two
 // luminosities from the front end); every other process its |M|^2
 template <int PROC, typename T>
 MF_HD T mf_me2_lum(const MfParams& P, T rts, const T k[MfProc<PROC>::N][4], const double* lum) {
   if (PROC == 5) return T(lum[0]) * mf_me2<1, T>(P, rts, k) + T(lum[1]) * mf_me2<4, T>(P, rts, k);
-  return mf_me2<PROC == 5 ? 1 : PROC, T>(P, rts, k);
+  return mf_me2<(PROC == 5 || PROC == 3) ? 1 : PROC, T>(P, rts, k);      // (process 3: mf_me2_ttgg_group instead)
 }
 
 // Front end of one event, S1-S6 + the weight prefactor: F = pref * |M|^2 for a passing event with

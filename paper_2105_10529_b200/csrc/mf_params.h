@@ -73,7 +73,7 @@ static inline int mf_fill_params(const mf_config_t* c, MfParams* P, std::string&
     p.ltau0 = log(tau0); p.tau0 = tau0;
     double gs2n = 1.0;
     for (int i = 0; i < ng; ++i) gs2n *= 4.0 * PI * c->alpha_s;
-    const double scale = (c->process == MF_GG_TT) ? MF_ME2_GG_TT_SCALE : (c->process == MF_GG_TTG) ? MF_ME2_GG_TTG_SCALE : MF_ME2_GG_TTGG_SCALE;
+    const double scale = (c->process == MF_GG_TT) ? MF_ME2_GG_TT_SCALE : (c->process == MF_GG_TTG) ? MF_ME2_GG_TTG_SCALE : MF_ME2_GG_TTGG_LANES_SCALE;
     p.me_pref = gs2n / 256.0 * scale;                   // 1/4 helicities x 1/64 colours (A12)
     if (c->process == MF_PP_TT) p.me_pref = gs2n / 256.0 * MF_ME2_GG_TT_SCALE;         // its g g -> t t~ subprocess
     p.me_pref_qq = gs2n * (2.0 / 9.0) * MF_ME2_EE_MUMU_SCALE;                           // O6q: colour sum 2 / 9 colours, 1/4 spins

@@ -360,7 +360,8 @@ __global__ void __launch_bounds__(THREADS, 1)
 mf_me_kernel(const MfParams P, double* __restrict__ rec, const unsigned int* __restrict__ count, int regions,
              unsigned long long cap) {
   constexpr int N = MfProc<PROC>::N, NF = MF_REC_FIELDS(N), T = THREADS;
-  extern __shared__ unsigned int s_pre[];                // [regions + 1] exclusive prefix, then s_part[T]
+  constexpr bool LANES = PROC == 3;                      // gg -> tt~gg: one event over four lanes (mf_me2_ttgg_group)
+  extern __shared__ unsigned int s_pre[];                // [regions + 1] exclusive prefix, then s_part[T], then the lane tiles
   unsigned int* s_part = s_pre + regions + 1;
   const unsigned tid = threadIdx.x;
   {                                                      // block scan over the region counts
@@ -380,13 +381,16 @@ mf_me_kernel(const MfParams P, double* __restrict__ rec, const unsigned int* __r
   // group's per-event prologue (record load, ingredients, reciprocals) overlaps the others' helicity loops
   constexpr unsigned G = MfProc<PROC>::GROUP < T ? MfProc<PROC>::GROUP : T, NG = T / G;
   static_assert(T % G == 0, "the CTA of the |M|^2 stage must be whole groups");
+  constexpr unsigned EPC = LANES ? G / 4 : G;            // events per chunk of a group
   const unsigned group = tid / G, gtid = tid % G;
-  const unsigned nchunks = (M + G - 1) / G;
+  const unsigned nchunks = (M + EPC - 1) / EPC;
+  Real* tile = nullptr;
+  if constexpr (LANES) tile = (Real*)(s_pre + ((regions + 1 + T + 1) & ~1)) + (size_t)(tid >> 5) * MF_LANES_TILE;
 #if MF_ME_STAGGER > 0
   if (group > 0) { const long long t0 = clock64(); while (clock64() - t0 < (long long)MF_ME_STAGGER * group) { } }
 #endif
   for (unsigned q = blockIdx.x * NG + group; q < nchunks; q += gridDim.x * NG) {   // group-uniform trips
-    const unsigned lin = q * G + gtid;
+    const unsigned lin = q * EPC + (LANES ? gtid >> 2 : gtid);
     const bool have = lin < M;
     const unsigned l = have ? lin : M - 1;               // lanes past the end recompute the last event
     int lo = 0, hi = regions;
@@ -398,8 +402,10 @@ mf_me_kernel(const MfParams P, double* __restrict__ rec, const unsigned int* __r
 #pragma unroll
       for (int c = 0; c < 4; ++c) k[p][c] = (Real)R[(size_t)(4 * p + c) * cap];
     const double rts = R[(size_t)(4 * N) * cap], pref = R[(size_t)(4 * N + 1) * cap];
-    const double F = pref * (double)mf_me2<PROC, Real>(P, (Real)rts, k);     // S7, S8
-    if (have) R[(size_t)(4 * N + 1) * cap] = F;
+    double F;                                            // S7, S8
+    if constexpr (LANES) F = pref * (double)mf_me2_ttgg_group<Real>(P, (Real)rts, k, tile);
+    else F = pref * (double)mf_me2<PROC, Real>(P, (Real)rts, k);
+    if (have && (!LANES || (tid & 3u) == 0u)) R[(size_t)(4 * N + 1) * cap] = F;
   }
 }
 
@@ -488,6 +494,7 @@ mf_eval_kernel(const MfParams P, const double* __restrict__ g_edges, const doubl
   extern __shared__ double smem[];
   double* s_edges = smem;
   double* s_pdf = s_edges + P.d * (P.nb + 1);
+  [[maybe_unused]] double* tile = s_pdf + P.pdf_smem + (size_t)(threadIdx.x >> 5) * (PROC == 3 ? MF_LANES_TILE : 0);   // lane tiles of gg -> tt~gg
   mf_stage_tables(P, g_edges, g_pdf, s_edges, s_pdf);
   __syncthreads();
   const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
@@ -505,7 +512,8 @@ mf_eval_kernel(const MfParams P, const double* __restrict__ g_edges, const doubl
       for (int p = 0; p < N; ++p)
 #pragma unroll
         for (int c = 0; c < 4; ++c) kt[p][c] = (T)k[p][c];
-      me2 = (double)mf_me2_lum<PROC, T>(P, (T)rts, kt, lum);
+      if constexpr (PROC == 3) me2 = (double)mf_me2_ttgg_warp32<T>(P, (T)rts, kt, (T*)tile);   // all 32 lanes (barriers inside)
+      else me2 = (double)mf_me2_lum<PROC, T>(P, (T)rts, kt, lum);
     }
     if (!pass) me2 = 0.0;
     double F = pass ? pref * me2 : 0.0;                  // S8
@@ -519,7 +527,9 @@ mf_eval_kernel(const MfParams P, const double* __restrict__ g_edges, const doubl
 #ifndef MF_COMPACT
 #define MF_COMPACT 1                 // CTA-level compaction of passing events for the processes with cuts
 #endif
-static constexpr bool kCompact = MF_COMPACT && MfProc<MF_PROC>::NGL > 0;
+static constexpr bool kFused = MF_PROC != 3;         // gg -> tt~gg iterates on the staged path only (four lanes per event in its |M|^2 stage)
+static constexpr bool kCompact = MF_COMPACT && MfProc<MF_PROC>::NGL > 0 && kFused;
+static constexpr size_t kTileBytes = MF_PROC == 3 ? sizeof(double) * (MF_THREADS / 32) * MF_LANES_TILE : 0;   // eval kernel: lane tiles
 static constexpr bool kEvalOne = MfProc<MF_PROC>::NGL > 0;
 static constexpr bool kF32 = MF_PROC == 2;   // fp32 variant of the |M|^2 stage: gg -> tt~g only (BASELINE configs[4])
 // classic 4n-random RAMBO: processes 1-3; the heavy ones on the staged path only
@@ -543,10 +553,13 @@ static cudaError_t with_dimensions(const MfParams& P, F&& f) {
 static cudaError_t proc_setup(const MfParams& P, size_t* smem_iter, size_t* smem_eval, int* occ_iter, int* occ_eval) {
   const size_t tables = (size_t)P.d * (P.nb + 1) + (size_t)P.pdf_smem;
   const size_t nw = MF_THREADS / 32;
-  *smem_eval = sizeof(double) * tables;
+  *smem_eval = sizeof(double) * tables + kTileBytes;
   *smem_iter = sizeof(double) * (tables + nw * P.d * P.nb + nw * 4);
   if (kCompact) *smem_iter += sizeof(double) * (4 * MfProc<MF_PROC>::N + 3) * 2 * MF_THREADS + sizeof(int) * nw;
   cudaError_t e;
+#if MF_PROC == 3
+  *smem_iter = 0; *occ_iter = 1; e = cudaSuccess;        // no fused kernel
+#else
   if constexpr (kCompact) {
     e = cudaFuncSetAttribute(mf_iterate_compact_kernel<MF_PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem_iter);
     if (e) return e;
@@ -559,6 +572,7 @@ static cudaError_t proc_setup(const MfParams& P, size_t* smem_iter, size_t* smem
       return r ? r : cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_iter, mf_iterate_kernel<MF_PROC, G>, MF_THREADS, *smem_iter);
     });
   }
+#endif
   if (e) return e;
   if constexpr (!kEvalOne) {
     e = cudaFuncSetAttribute(mf_eval_kernel<MF_PROC, false, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem_eval);
@@ -597,6 +611,9 @@ static cudaError_t proc_iterate(const MfParams& P, const double* edges, const do
     if (kCompact) return cudaErrorNotSupported;          // observables of the heavy processes: staged path
     smem += sizeof(double) * (MF_THREADS / 32) * MF_OBS_ACC;
   }
+#if MF_PROC == 3
+  return cudaErrorNotSupported;
+#else
   if constexpr (kCompact) {
     if (P.gen != 0) return cudaErrorNotSupported;        // generator variants of the heavy processes: staged path
     mf_iterate_compact_kernel<MF_PROC><<<grid, MF_THREADS, smem, st>>>(P, edges, pdf, iteration, first, n, n_total, partial, pcount, row);
@@ -607,6 +624,7 @@ static cudaError_t proc_iterate(const MfParams& P, const double* edges, const do
       return cudaGetLastError();
     });
   }
+#endif
 }
 
 // ---- staged path: launches ---------------------------------------------------------------------------
@@ -623,6 +641,7 @@ static size_t hist_smem(const MfParams& P) {
   return sizeof(double) * (MF_THREADS / 32) * ((size_t)P.d * P.nb + 4 + (P.n_obs > 0 ? MF_OBS_ACC : 0));
 }
 
+static size_t me_tile_bytes(int threads) { return MF_PROC == 3 ? sizeof(double) * (threads / 32) * MF_LANES_TILE + 8 : 0; }
 static cudaError_t proc_staged_setup(const MfParams& P, int* rec_fields, int* occ_front, int* occ_hist) {
   *rec_fields = kStaged ? kRecFields : 0;
   *occ_front = *occ_hist = 0;
@@ -634,7 +653,7 @@ static cudaError_t proc_staged_setup(const MfParams& P, int* rec_fields, int* oc
     return r ? r : cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_front, mf_front_kernel<MF_PROC, G>, MF_THREADS, front_smem(P));
   });
   if (e) return e;
-  e = cudaFuncSetAttribute(mf_me_kernel<MF_PROC, double, MF_ME_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+  e = cudaFuncSetAttribute(mf_me_kernel<MF_PROC, double, MF_ME_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024 + (int)me_tile_bytes(MF_ME_THREADS));
   if (e) return e;
   if constexpr (kF32) {
     e = cudaFuncSetAttribute(mf_me_kernel<MF_PROC, float, MF_ME_THREADS_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
@@ -664,7 +683,7 @@ static cudaError_t proc_staged(const MfParams& P, const double* edges, const dou
   });
   if (e) return e;
   if (ev && (e = cudaEventRecord(ev[1], st))) return e;
-  const size_t sm = sizeof(unsigned int) * ((size_t)ws.regions + 1 + (f32 ? MF_ME_THREADS_F32 : MF_ME_THREADS));
+  const size_t sm = sizeof(unsigned int) * ((size_t)ws.regions + 1 + (f32 ? MF_ME_THREADS_F32 : MF_ME_THREADS)) + me_tile_bytes(MF_ME_THREADS);
   if (f32) {
     if constexpr (kF32) mf_me_kernel<MF_PROC, float, MF_ME_THREADS_F32><<<grid_me, MF_ME_THREADS_F32, sm, st>>>(P, ws.rec, ws.count, ws.regions, ws.cap);
     else return cudaErrorNotSupported;

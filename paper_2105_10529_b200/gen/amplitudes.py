@@ -211,6 +211,10 @@ class Gen:
             self._P[key] = v
         return self._P[key]
 
+    def _hk(self, legs, hel):
+        """memo key of the helicity labels of `legs` (symbols by identity)"""
+        return tuple(id(hel[l]) if isinstance(hel[l], R) else hel[l] for l in legs)
+
     def j(self, pi, hel):
         """ordered current j(pi) for helicities hel (dict leg -> +-1 or symbol); memoised with the
         reflection identity j(reversed pi) = (-1)^(k-1) j(pi)"""
@@ -219,47 +223,47 @@ class Gen:
         if rev < pi:
             cur = self.j(rev, hel)
             return cur if len(pi) % 2 == 1 else [-c for c in cur]
-        key = (pi, tuple(id(hel[l]) if isinstance(hel[l], R) else hel[l] for l in pi))
-        if key in self._j:
-            return self._j[key]
+        key = (pi, self._hk(pi, hel))
+        if key not in self._j:
+            self._j[key] = self.pol(pi[0], hel[pi[0]]) if len(pi) == 1 else self._bg(pi, hel)
+        return self._j[key]
+
+    def _bg(self, pi, hel):
+        """one step of the Berends-Giele recursion: j(pi), len(pi) >= 2, from the currents of its splits"""
         g = self.g
-        if len(pi) == 1:
-            cur = self.pol(pi[0], hel[pi[0]])
-        else:
-            k = len(pi)
-            terms = [[] for _ in range(4)]        # complex product lists per component
-            rterms = [[] for _ in range(4)]       # (real, complex) products per component
-            for s in range(1, k):                 # cubic: split L | R
-                L, Rr = pi[:s], pi[s:]
-                PL, PR = self.P(L), self.P(Rr)
-                jL, jR = self.j(L, hel), self.j(Rr, hel)
-                c1 = mdot_r(g, [2.0 * a + b for a, b in zip(PL, PR)], jR)
-                c2 = mdot(g, jL, jR)
-                c3 = mdot_r(g, [2.0 * b + a for a, b in zip(PL, PR)], jL)
-                d = [a - b for a, b in zip(PL, PR)]
-                for m in range(4):                # accumulate  -v3 = +jL c1 - d c2 - jR c3
-                    terms[m] += [(jL[m], c1), (-jR[m], c3)]
-                    rterms[m] += [(-d[m], c2)]
-            for s1 in range(1, k - 1):            # quartic: X | Y | Z
-                for s2 in range(s1 + 1, k):
-                    X, Y, Z = self.j(pi[:s1], hel), self.j(pi[s1:s2], hel), self.j(pi[s2:], hel)
-                    yz, xy, xz = mdot(g, Y, Z), mdot(g, X, Y), mdot(g, X, Z)
-                    for m in range(4):            # accumulate -q4 = -X yz - Z xy + 2 Y xz
-                        terms[m] += [(-X[m], yz), (-Z[m], xy), (2.0 * Y[m], xz)]
-            Pv = self.P(pi)
-            inv = g.rcp(mdot_rr(g, Pv, Pv))
-            cur = []
-            for m in range(4):
-                acc = csum_prod(g, terms[m])
-                re = g.sop([(a, c.re) for a, c in rterms[m]], acc.re)
-                im = g.sop([(a, c.im) for a, c in rterms[m]], acc.im)
-                cur.append(Cx(re * inv, im * inv))
-        self._j[key] = cur
+        k = len(pi)
+        terms = [[] for _ in range(4)]        # complex product lists per component
+        rterms = [[] for _ in range(4)]       # (real, complex) products per component
+        for s in range(1, k):                 # cubic: split L | R
+            L, Rr = pi[:s], pi[s:]
+            PL, PR = self.P(L), self.P(Rr)
+            jL, jR = self.j(L, hel), self.j(Rr, hel)
+            c1 = mdot_r(g, [2.0 * a + b for a, b in zip(PL, PR)], jR)
+            c2 = mdot(g, jL, jR)
+            c3 = mdot_r(g, [2.0 * b + a for a, b in zip(PL, PR)], jL)
+            d = [a - b for a, b in zip(PL, PR)]
+            for m in range(4):                # accumulate  -v3 = +jL c1 - d c2 - jR c3
+                terms[m] += [(jL[m], c1), (-jR[m], c3)]
+                rterms[m] += [(-d[m], c2)]
+        for s1 in range(1, k - 1):            # quartic: X | Y | Z
+            for s2 in range(s1 + 1, k):
+                X, Y, Z = self.j(pi[:s1], hel), self.j(pi[s1:s2], hel), self.j(pi[s2:], hel)
+                yz, xy, xz = mdot(g, Y, Z), mdot(g, X, Y), mdot(g, X, Z)
+                for m in range(4):            # accumulate -q4 = -X yz - Z xy + 2 Y xz
+                    terms[m] += [(-X[m], yz), (-Z[m], xy), (2.0 * Y[m], xz)]
+        Pv = self.P(pi)
+        inv = g.rcp(mdot_rr(g, Pv, Pv))
+        cur = []
+        for m in range(4):
+            acc = csum_prod(g, terms[m])
+            re = g.sop([(a, c.re) for a, c in rterms[m]], acc.re)
+            im = g.sop([(a, c.im) for a, c in rterms[m]], acc.im)
+            cur.append(Cx(re * inv, im * inv))
         return cur
 
     def jsl(self, pi, hel):
         pi = tuple(pi)
-        key = (pi, tuple(id(hel[l]) if isinstance(hel[l], R) else hel[l] for l in pi))
+        key = (pi, self._hk(pi, hel))
         if key not in self._sl:
             self._sl[key] = SlashC(self.j(pi, hel))
         return self._sl[key]
@@ -278,7 +282,7 @@ class Gen:
 
     def chi(self, tau, hel, lam4):
         tau = tuple(tau)
-        key = (tau, tuple(id(hel[l]) if isinstance(hel[l], R) else hel[l] for l in tau), id(lam4) if isinstance(lam4, R) else lam4)
+        key = (tau, self._hk(tau, hel), id(lam4) if isinstance(lam4, R) else lam4)
         if key in self._chi:
             return self._chi[key]
         g = self.g
@@ -516,7 +520,6 @@ PROCESSES = {
     "mf_me2_gg_tt": lambda: Gen(2, loop_legs=(), parity=True, basis="circular"),      # 514 flops (linear: 715)
     "mf_me2_gg_ttg": lambda: Gen(3, loop_legs=_legs("MF_GEN_TTG_LOOP", (0, 2)), parity=True,
                                  loop_lam4=os.environ.get("MF_GEN_TTG_LAM4", "0") == "1", basis=BASIS),
-    "mf_me2_gg_ttgg": lambda: Gen(4, loop_legs=_legs("MF_GEN_TTGG_LOOP", (0, 1, 2, 3)), parity=True, basis=BASIS),
 }
 
 

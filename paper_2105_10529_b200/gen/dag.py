@@ -85,6 +85,11 @@ class Dag:
         self.names[i] = name
         return R(self, i)
 
+    def xl(self, slot, k, rnd=0):
+        """value of exchange slot `slot` as stored by the lane `k` places on (gen/lanes.py: one event over several lanes);
+        a body node without operands, emitted as a load.  rnd tells apart the uses of a slot that is written more than once."""
+        return R(self, self._new(("xl", slot, k, rnd), True))
+
     def _d(self, *rs):
         return any(r.n is not None and self.dep[r.n] for r in rs)
 
@@ -278,7 +283,7 @@ class Dag:
     # ---- analysis ------------------------------------------------------------------------------
     def _operands(self, i):
         op, a, b, c = self.nodes[i]
-        if op in ("in", "sym"):
+        if op in ("in", "sym", "xl"):
             return ()
         if op in ("mulk", "addk", "rcp"):
             return (a,)
@@ -354,6 +359,8 @@ class Dag:
             return "%s + %s" % (nm(a), self._k(b))
         if op == "rcp":
             return "T(1.0) / %s" % nm(a)
+        if op == "xl":
+            return "MF_XL(%d, %d)" % (a, b)
         if op in ("fma", "fms"):
             x, y = (self._k(a[1]), nm(a[2])) if a[0] == "k" else (nm(a[1]), nm(a[2]))
             return "fma(%s, %s, %s%s)" % (x, y, "-" if op == "fms" else "", nm(b))
@@ -387,6 +394,8 @@ class Dag:
                 continue
             if op in ("in", "sym"):
                 val[i] = np.asarray(values[a], dtype=np.float64)
+            elif op == "xl":
+                val[i] = np.asarray(values[("xl", a, b, c)], dtype=np.float64)
             elif op == "mul":
                 val[i] = val[a] * val[b]
             elif op == "mulk":

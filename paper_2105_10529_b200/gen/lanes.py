@@ -1,0 +1,298 @@
+"""gg -> t t~ g g with ONE EVENT OVER FOUR LANES (BASELINE.json configs[3], the register-pressure case).
+
+One thread per event cannot hold a helicity configuration of this process: 34 ordered gluon currents
+(136 doubles), 41 quark-line spinors (328) and 24 x 2 partial amplitudes (96) -- the one-thread code
+spilled 6.5-14 KB per thread and waited on the reloads (profiles/r2_ttgg_ncu.md).  Here the 24 colour
+orderings (a b c d) of DESIGN.md 5.3 are split by their LAST gluon d (the one next to the antitop):
+lane l of a group of four takes the six orderings that end with gluon l.  Every lane runs the SAME
+straight-line code on cyclically relabelled gluons (local label i = global gluon (i + l) mod 4, local
+0 = the last gluon), so a warp carries 8 events without divergence:
+
+  * the quark line of a lane is the subtree chi(0) -> chi(c 0) -> chi(b c 0) -> a_(a b c 0), walked depth
+    first: 4 spinors alive at a time, no spinor is computed twice in the group;
+  * the gluon currents are shared: the cyclic group acts on the 6 / 12 / 12 unordered pairs / triples /
+    quadruples (ordered, modulo reflection) with 2 / 3 / 4 orbits; each lane computes one representative
+    per orbit, stores it in the warp's shared-memory tile and reads the others from the lane k places on:
+    "my j(pi + k)" = "lane l+k's j(pi)"  (MF_XL(slot, k));
+  * the colour form uses C_{s s'} = c(s^-1 s') (invariant under relabelling): with the partial amplitudes
+    exchanged the same way, lane l adds x_l^T C(0) x_l + 2 x_l^T C(1) x_(l+1) + x_l^T C(2) x_(l+2) with
+    lane-independent integer blocks C(k); the four lane sums are added by two shuffles after the loop.
+
+Polarisations: linear basis, unit vectors for all four gluons; the 16 polarisation
+assignments are a run-time loop, lambda_4 = + fixed (parity), both lambda_3 unrolled.
+"""
+import itertools
+import numpy as np
+from .dag import Dag, R, Cx, csum_prod
+from .amplitudes import Gen, colour_matrix
+
+NL = 4
+
+
+def _canon(pi):
+    """(canonical form, sign) with j(pi) = sign * j(canonical): reflection identity j(rev) = (-1)^(k-1) j"""
+    pi = tuple(pi)
+    rev = tuple(reversed(pi))
+    if rev < pi:
+        return rev, (1 if len(pi) % 2 == 1 else -1)
+    return pi, 1
+
+
+def _shift(pi, k):
+    return tuple((x + k) % NL for x in pi)
+
+
+def orbits(size):
+    """orbits of the cyclic relabelling on the ordered currents of `size` gluons modulo reflection:
+    {canonical pi: (representative, k, sign)} with j(pi) = sign * [lane l+k's j(representative)]"""
+    out, reps = {}, []
+    for pi in itertools.permutations(range(NL), size):
+        c, _ = _canon(pi)
+        if c in out:
+            continue
+        reps.append(c)
+        for k in range(NL):
+            c2, s2 = _canon(_shift(c, k))
+            out.setdefault(c2, (c, k, s2))
+    return out, reps
+
+
+class GenLanes(Gen):
+    """per-lane program of gg -> t t~ g g; inputs are the lane's relabelled quantities"""
+
+    def __init__(self):
+        self.basis, self.ng, self.g = "linear", NL, Dag()
+        self.loop_lam4, self.parity, self.loop_legs = False, True, ()
+        g = self.g
+        self.input_names = []
+        inp = self._inp
+        self.mt = inp("mt")
+        self.p4 = [inp("p4e"), inp("p4x"), inp("p4y"), inp("p4z")]
+        self.t_ing = [inp("t_" + n) for n in ("wp", "wm", "c0", "cx", "cy")]
+        self.b_ing = [inp("b_" + n) for n in ("wp", "wm", "c0", "cx", "cy")]
+        # all-incoming momenta of the lane's gluons (local label i = global gluon (i + lane) mod 4)
+        self.K = [[inp("k%d%s" % (i, c)) for c in "exyz"] for i in range(NL)]
+        # unit polarisation vector of local gluon i in this trip of the polarisation loop (loop symbols)
+        self.pl = [[g.sym("pl%d%s" % (i, c)) for c in "xyz"] for i in range(NL)]
+        self._P, self._j, self._sl, self._chi = {}, {}, {}, {}
+        self.orb, self.reps = {}, {}
+        for size in (2, 3, 4):
+            o, r = orbits(size)
+            self.orb.update(o)
+            self.reps[size] = r
+        self.slot_of = {}                      # representative -> first of its 4 exchange slots
+        self.prog = []                         # ("seg", node count) / ("store", slot, R) / ("sync", round of the loads behind it)
+        self.n_slots = 0
+
+    # helicity labels play no role in the memo keys: one symbolic configuration
+    def _hk(self, legs, hel):
+        return ()
+
+    def pol(self, leg, lam=None):
+        zero = self.g.const(0.0)
+        return [Cx(zero, zero)] + [Cx(c, zero) for c in self.pl[leg]]
+
+    def j(self, pi, hel=None):
+        pi = tuple(pi)
+        if len(pi) == 1:
+            return self.pol(pi[0])
+        c, sgn = _canon(pi)
+        if c not in self._j:
+            rep, k, s2 = self.orb[c]
+            assert k != 0 and rep in self.slot_of, "representative currents are computed in their own phase"
+            zero = self.g.const(0.0)
+            slot = self.slot_of[rep]
+            self._j[c] = [Cx(self.g.xl(slot + m, k) * float(s2), zero) for m in range(4)]
+        cur = self._j[c]
+        return cur if sgn > 0 else [-x for x in cur]
+
+    def _mark(self):
+        self.prog.append(("seg", len(self.g.nodes)))
+
+    def _new_slots(self, n):
+        s = self.n_slots
+        self.n_slots += n
+        return s
+
+    def build(self):
+        g = self.g
+        num, den, perms = colour_matrix(NL)
+        index = {p: i for i, p in enumerate(perms)}
+        # ---- gluon currents: one representative per orbit, phase by phase ------------------------------
+        for size in (2, 3, 4):
+            for rep in self.reps[size]:
+                cur = self._bg(rep, None)
+                assert all(c.im.is_zero() for c in cur)
+                self._j[rep] = cur
+                self.slot_of[rep] = self._new_slots(4)
+                self._mark()
+                for m in range(4):
+                    self.prog.append(("store", self.slot_of[rep] + m, cur[m].re))
+            self.prog.append(("sync", 0))
+        # ---- quark line: the six orderings (a b c 0), depth first ----------------------------------------
+        local = []
+        for c in (1, 2, 3):
+            for b in (1, 2, 3):
+                if b != c:
+                    a = 6 - b - c
+                    local.append((a, b, c, 0))
+        amps = {1: [], -1: []}
+        for sg in local:
+            a = self.partial_amps(sg, None, 1)
+            amps[1].append(a[1])
+            amps[-1].append(a[-1])
+        self.local = local
+        # ---- colour form with exchanged amplitudes ------------------------------------------------------
+        # the exchange tile is reused: all lanes are past their last current load (sync), then store, sync
+        self._mark()
+        self.prog.append(("sync", 0))
+        xs = {}
+        slot = 0
+        for lam3 in (1, -1):
+            for part in ("re", "im"):
+                xs[(lam3, part)] = [getattr(a, part) for a in amps[lam3]]
+                for i, x in enumerate(xs[(lam3, part)]):
+                    self.prog.append(("store", slot + i, x))
+                slot += 6
+        self.prog.append(("sync", 1))
+        self.n_slots = max(self.n_slots, slot)
+
+        def glob(sg, lane):
+            return index[_shift(sg, lane)]
+
+        blocks = {}
+        for k in (0, 1, 2):
+            blk = np.array([[num[glob(si, 0)][glob(sj, k)] for sj in local] for si in local])
+            for lane in range(1, NL):          # invariance under relabelling: the blocks do not depend on the lane
+                assert (blk == np.array([[num[glob(si, lane)][glob(sj, lane + k)] for sj in local] for si in local])).all()
+            blocks[k] = blk
+        total = g.const(0.0)
+        slot = 0
+        for lam3 in (1, -1):
+            for part in ("re", "im"):
+                x = xs[(lam3, part)]
+                pairs = []
+                for i in range(6):
+                    y = g.sop([(g.const(2.0 * blocks[0][i][t]), x[t]) for t in range(i + 1, 6)], g.const(float(blocks[0][i][i])) * x[i])
+                    y = g.sop([(g.const(2.0 * blocks[1][i][t]), g.xl(slot + t, 1, 1)) for t in range(6)], y)
+                    y = g.sop([(g.const(1.0 * blocks[2][i][t]), g.xl(slot + t, 2, 1)) for t in range(6)], y)
+                    pairs.append((x[i], y))
+                total = g.sop(pairs, total)
+                slot += 6
+        self._mark()
+        self.out = total
+        self.scale = 2.0 / den                 # parity (lambda_4 fixed) / colour denominator; unit polarisation vectors
+        self.blocks = blocks
+        return total
+
+
+# ---- numeric evaluation: the four lanes of one event, segment by segment (generator self-test) ---------
+def evaluate_event(gen, mom, mt, ferm, glu_units):
+    """|M|^2 body summed over the 16 polarisation assignments and the four lanes.
+    mom: [6][4] (g g -> t t~ g g, partonic CM frame); ferm(p, m) -> 5 spinor ingredients;
+    glu_units(k) -> (eps1, eps2) unit 3-vectors of an outgoing gluon."""
+    g = gen.g
+    Kg = [np.array(mom[0]), np.array(mom[1]), -np.array(mom[4]), -np.array(mom[5])]
+    e = [(np.array([1.0, 0.0, 0.0]), np.array([0.0, 1.0, 0.0])), (np.array([1.0, 0.0, 0.0]), np.array([0.0, -1.0, 0.0])),
+         glu_units(mom[4]), glu_units(mom[5])]
+    base = {"mt": mt}
+    for n, c in zip(("p4e", "p4x", "p4y", "p4z"), mom[3]): base[n] = c
+    for n, c in zip(("wp", "wm", "c0", "cx", "cy"), ferm(mom[2], mt)): base["t_" + n] = c
+    for n, c in zip(("wp", "wm", "c0", "cx", "cy"), ferm(mom[3], mt)): base["b_" + n] = c
+    total = 0.0
+    for ih in range(16):
+        vals = []
+        for lane in range(NL):
+            v = dict(base)
+            for i in range(NL):
+                gl = (i + lane) % NL
+                for n, c in zip("exyz", Kg[gl]): v["k%d%s" % (i, n)] = c
+                pol = e[gl][0] if (ih >> gl) & 1 else e[gl][1]
+                for n, c in zip("xyz", pol): v["pl%d%s" % (i, n)] = c
+            vals.append(v)
+        pending = []
+        for item in gen.prog:
+            if item[0] == "store":
+                pending.append((item[1], item[2]))
+            elif item[0] == "sync" and pending:      # the stores before this barrier become readable: round item[1]
+                res = [g.evaluate([r for _s, r in pending], vals[lane]) for lane in range(NL)]
+                for lane in range(NL):
+                    for k in range(1, NL):
+                        for (s, _r), x in zip(pending, res[(lane + k) % NL]):
+                            vals[lane][("xl", s, k, item[1])] = float(x)
+                pending = []
+        for lane in range(NL):
+            total += float(g.evaluate([gen.out], vals[lane])[0])
+    return total
+
+
+# ---- emission -------------------------------------------------------------------------------------------
+def emit_lanes(gen, fname, sched_window=48, sched_distance=5, max_hoist_cost=None):
+    """CUDA text of the per-lane function
+        template <typename T> T fname(const T* in, const T* G, T* X, int lane4, int xs0, int xs1, int xs2, int xs3)
+    in: the lane's inputs (order = gen.input_names); G: the event's polarisation table [global gluon][eps1, eps2][x, y, z];
+    X: the warp's exchange tile [slot][32]; lane4: lane within the group of four; xs0 = the thread's lane in the warp,
+    xs_k = lane in the warp of the group member k places on.  Returns this lane's share of sum_pol sum_{s s'} a_s C a_s'^*;
+    the caller adds the four lanes.  Counts are per LANE and event (executed, with the loop-invariant prologue once)."""
+    g = gen.g
+    stores = [it[2] for it in gen.prog if it[0] == "store"]
+    pro_ids, body_ids, hoisted = g.plan([gen.out] + stores, max_hoist_cost)
+    body_set = set(body_ids)
+    nh = 16
+    pro, body = g.count_list(pro_ids), g.count_list(body_ids)
+    tot = {k: pro[k] + nh * (body[k] + (1 if k == "add" else 0)) for k in pro}
+    U = fname.upper()
+    L = ["// GENERATED by paper_2105_10529_b200/gen/lanes.py -- do not edit.",
+         "// one event over four lanes; per LANE and event (executed): %d add, %d mul, %d fma, %d rcp  (flops = add + mul + 2 fma = %d)"
+         % (tot["add"], tot["mul"], tot["fma"], tot["rcp"], tot["add"] + tot["mul"] + 2 * tot["fma"]),
+         "#define %s_NADD %dull" % (U, tot["add"]), "#define %s_NMUL %dull" % (U, tot["mul"]),
+         "#define %s_NFMA %dull" % (U, tot["fma"]), "#define %s_NIN %d" % (U, len(gen.input_names)),
+         "#define %s_SCALE %r" % (U, gen.scale), "#define %s_SLOTS %d" % (U, gen.n_slots)]
+    L.append("enum { " + ", ".join("%s_IN_%s = %d" % (U, n.upper(), i) for i, n in enumerate(gen.input_names)) + " };")
+    L.append("#if defined(__CUDACC__) || defined(MF_LANES_HOST_EMULATION)      // device code (warp barriers, shared-memory tile); the CPU test harness runs it on four host threads")
+    L.append("#define MF_XL(s, k) X[(s) * 32 + xs##k]")
+    L.append("template <typename T>")
+    L.append("MF_DEVFN T %s(const T* __restrict__ in, const T* G, T* X, const int lane4, const int xs0, const int xs1, const int xs2, const int xs3) {" % fname)
+    for i, n in enumerate(gen.input_names):
+        L.append("  const T %s = in[%d];" % (n, i))
+    leaf = lambda j: g.nodes[j][0] in ("in", "sym")
+    pname = lambda j: g.names[j] if leaf(j) else "p%d" % j
+    L += g.emit_list(pro_ids, pname, "p")
+    L.append("  T acc = T(0.0);")
+    L.append("#pragma unroll 1")
+    L.append("  for (int ih = 0; ih < %d; ++ih) {" % nh)
+    for i in range(NL):
+        L.append("    const int gl%d = (lane4 + %d) & 3;" % (i, i))
+        L.append("    const T* gp%d = G + gl%d * 6 + (((ih >> gl%d) & 1) ? 0 : 3);" % (i, i, i))
+        L.append("    const T pl%dx = gp%d[0], pl%dy = gp%d[1], pl%dz = gp%d[2];" % (i, i, i, i, i, i))
+
+    def bname(j):
+        if leaf(j):
+            return g.names[j]
+        return "v%d" % j if j in body_set else "p%d" % j
+
+    lo, nstmt = 0, 0
+    for it in gen.prog:
+        if it[0] == "seg":
+            ids = [i for i in body_ids if lo <= i < it[1]]
+            lo = it[1]
+            if ids:
+                ids = g.schedule(ids, sched_window, sched_distance)
+                for line in g.emit_list(ids, bname, "v", indent="    "):
+                    if nstmt % 64 == 0:
+                        L.append("    MF_SYNC_POINT(%d);" % (nstmt // 64))
+                    L.append(line)
+                    nstmt += 1
+        elif it[0] == "store":
+            r = it[2]
+            L.append("    X[%d * 32 + xs0] = %s;" % (it[1], g._k(r.c) if r.n is None else ("" if r.s > 0 else "-") + bname(r.n)))
+        else:
+            L.append("    __syncwarp();")
+    L.append("    acc += %s;" % (g._k(gen.out.c) if gen.out.n is None else ("" if gen.out.s > 0 else "-") + bname(gen.out.n)))
+    L.append("    __syncwarp();      // the tile is rewritten by the next trip")
+    L.append("  }")
+    L.append("  return acc;")
+    L.append("}")
+    L.append("#undef MF_XL")
+    L.append("#endif")
+    return "\n".join(L) + "\n", tot, dict(pro=pro, body=body)

@@ -1,16 +1,63 @@
 // TEST HARNESS ONLY (never part of the product library): compiles the product's per-event device
 // functions (csrc/mf_event.cuh, including the generated |M|^2 code) for the host with g++, so that
 // the CPU test-suite can check that arithmetic event by event against the oracle without a GPU.
+// gg -> tt~gg spreads one event over four lanes that exchange currents through a shared tile between warp barriers
+// (gen/lanes.py): the harness runs the generated per-lane code on four host threads, __syncwarp() = a std::barrier.
+#include <barrier>
+#include <thread>
+#include <cstring>
+static std::barrier<> g_lane_barrier(4);
+static inline void __syncwarp() { g_lane_barrier.arrive_and_wait(); }
+#define MF_LANES_HOST_EMULATION
 #include "../../paper_2105_10529_b200/csrc/mf_event.cuh"
 #include "../../paper_2105_10529_b200/csrc/mf_params.h"
-#include <cstring>
+
+// host stand-in of mf_me2_ttgg_group (mf_event.cuh): same publishing of the global gluons, same per-lane inputs
+static double ttgg_lanes_host(const MfParams& P, double rts, const double k[4][4]) {
+  static double tile[MF_ME2_GG_TTGG_LANES_SLOTS * 32 + 40];
+  double* Gp = tile + MF_ME2_GG_TTGG_LANES_SLOTS * 32;
+  double* Kt = Gp + 24;
+  const double E = 0.5 * rts, r2 = 1.41421356237309504880;
+  for (int l = 0; l < 4; ++l) {
+    const bool inc = l < 2;
+    const double sg = l == 0 ? 1.0 : -1.0;
+    const double* kg = l == 3 ? k[3] : k[2];
+    double o[5];
+    mf_gluon_ing<double>(kg, o);
+    Kt[l * 4 + 0] = inc ? E : -kg[0]; Kt[l * 4 + 1] = inc ? 0.0 : -kg[1]; Kt[l * 4 + 2] = inc ? 0.0 : -kg[2]; Kt[l * 4 + 3] = inc ? sg * E : -kg[3];
+    Gp[l * 6 + 0] = inc ? 1.0 : r2 * o[0]; Gp[l * 6 + 1] = inc ? 0.0 : r2 * o[1]; Gp[l * 6 + 2] = inc ? 0.0 : r2 * o[2];
+    Gp[l * 6 + 3] = inc ? 0.0 : r2 * o[3]; Gp[l * 6 + 4] = inc ? sg : r2 * o[4]; Gp[l * 6 + 5] = 0.0;
+  }
+  double acc[4];
+  std::thread th[4];
+  for (int l = 0; l < 4; ++l) th[l] = std::thread([&, l] {
+    double in[31];
+    in[0] = P.m_top;
+    for (int c = 0; c < 4; ++c) in[1 + c] = k[1][c];
+    mf_fermion_ing<double>(k[0], P.m_top, in + 5);
+    mf_fermion_ing<double>(k[1], P.m_top, in + 10);
+    for (int i = 0; i < 4; ++i) for (int c = 0; c < 4; ++c) in[15 + 4 * i + c] = Kt[((i + l) & 3) * 4 + c];
+    acc[l] = mf_me2_gg_ttgg_lanes<double>(in, Gp, tile, l, l, (l + 1) & 3, (l + 2) & 3, (l + 3) & 3);
+  });
+  for (int l = 0; l < 4; ++l) th[l].join();
+  return P.me_pref * ((acc[0] + acc[1]) + (acc[2] + acc[3]));
+}
+template <int CL>
+static double event_ttgg(const MfParams& P, const double* edges, const double* pdf, uint32_t it, uint64_t ev, int* bin, bool& ok, MfEventRec* rec) {
+  double k[4][4], rts, pref;
+  ok = mf_event_front<3, true, CL>(P, edges, pdf, it, ev, bin, k, rts, pref, rec);
+  rec->me2 = ok ? ttgg_lanes_host(P, rts, k) : 0.0;
+  return ok ? pref * rec->me2 : 0.0;
+}
 
 template <int PROC>
 static double run(const MfParams& P, const double* edges, const double* pdf, uint32_t it, uint64_t ev,
                   int* bins, int* pass, double* rec_out) {
   int bin[MfProc<PROC>::D]; bool ok; MfEventRec rec;
   std::memset(&rec, 0, sizeof rec);
-  double F = mf_event<PROC, true>(P, edges, pdf, it, ev, bin, ok, &rec);
+  double F;
+  if constexpr (PROC == 3) F = event_ttgg<0>(P, edges, pdf, it, ev, bin, ok, &rec);
+  else F = mf_event<PROC, true>(P, edges, pdf, it, ev, bin, ok, &rec);
   for (int j = 0; j < MfProc<PROC>::D; ++j) bins[j] = bin[j];
   *pass = ok;
   // rec_out: y[10], mom[24], me2, pdf[2]
@@ -54,7 +101,9 @@ static double run_gen(const MfParams& P, const double* edges, const double* pdf,
                       int* bins, int* pass, double* rec_out) {
   int bin[MfDim<PROC, CL>::D]; bool ok; MfEventRec rec;
   std::memset(&rec, 0, sizeof rec);
-  double F = mf_event<PROC, true, double, CL>(P, edges, pdf, it, ev, bin, ok, &rec);
+  double F;
+  if constexpr (PROC == 3) F = event_ttgg<CL>(P, edges, pdf, it, ev, bin, ok, &rec);
+  else F = mf_event<PROC, true, double, CL>(P, edges, pdf, it, ev, bin, ok, &rec);
   for (int j = 0; j < MfDim<PROC, CL>::D; ++j) bins[j] = bin[j];
   *pass = ok;
   std::memcpy(rec_out, rec.y, sizeof(double) * 18);

@@ -88,7 +88,7 @@ def _inputs(gen, mom, mt=173.0):
     return v
 
 
-@pytest.mark.parametrize("proc,fname,n", [(1, "mf_me2_gg_tt", 2), (2, "mf_me2_gg_ttg", 3), (3, "mf_me2_gg_ttgg", 4)])
+@pytest.mark.parametrize("proc,fname,n", [(1, "mf_me2_gg_tt", 2), (2, "mf_me2_gg_ttg", 3)])
 def test_generated_amplitude_dag_matches_oracle(mfo, proc, fname, n):
     from paper_2105_10529_b200.gen import amplitudes as A
     gen = A.generate(fname)
@@ -103,6 +103,38 @@ def test_generated_amplitude_dag_matches_oracle(mfo, proc, fname, n):
         ref = mfo.me2(proc, mom)
         val = float(A.evaluate(gen, _inputs(gen, mom))) * gen.scale * gs2 ** n / 256
         assert abs(val / ref - 1) < 1e-11
+
+
+def test_four_lane_decomposition_matches_oracle(mfo):
+    """gg -> tt~gg with one event over four lanes (gen/lanes.py): the per-lane DAG evaluated for the four lanes with the
+    exchanges of currents and amplitudes played out, against the oracle; the orbit structure of the shared currents; and
+    the one-thread organisation of the same amplitude (the algorithmic flop count) against both"""
+    from paper_2105_10529_b200.gen import amplitudes as A, lanes as L
+    gen = L.GenLanes()
+    gen.build()
+    assert [len(gen.reps[s]) for s in (2, 3, 4)] == [2, 3, 4]          # orbits of the cyclic relabelling
+    assert len(gen.local) == 6 and all(sg[-1] == 0 for sg in gen.local) and gen.n_slots == 36
+    text, tot, parts = L.emit_lanes(gen, "mf_me2_gg_ttgg_lanes")
+    assert text.count("__syncwarp();") == 6 and "MF_ME2_GG_TTGG_LANES_NFMA %dull" % tot["fma"] in text
+    one = A.Gen(4, loop_legs=(0, 1, 2, 3), parity=True, basis="linear")
+    one.build()
+
+    def glu_units(k):
+        e = np.array(_glu(k)) * math.sqrt(2)
+        return e[:3], np.array([e[3], e[4], 0.0])
+
+    gs2 = 4 * math.pi * 0.118
+    rng = np.random.default_rng(23)
+    for trial in range(3):
+        rts = rng.uniform(450, 4000)
+        ps = mfo.phase_space(4, rts * rts, [173.0, 173.0, 0.0, 0.0], rng.uniform(0.03, 0.97, 8))
+        mom = np.zeros((6, 4)); mom[0] = [rts / 2, 0, 0, rts / 2]; mom[1] = [rts / 2, 0, 0, -rts / 2]; mom[2:] = ps["k"]
+        ref = mfo.me2(3, mom)
+        val = L.evaluate_event(gen, mom, 173.0, _ferm, glu_units) * gen.scale * gs2 ** 4 / 256
+        assert abs(val / ref - 1) < 1e-11
+        if trial == 0:
+            v1 = float(A.evaluate(one, _inputs(one, mom))) * one.scale * gs2 ** 4 / 256
+            assert abs(v1 / ref - 1) < 1e-11
 
 
 def test_generator_colour_matrices_match_golden():

@@ -19,9 +19,11 @@ LIB = os.path.join(ROOT, "tests", "host_harness", "libmfh.so")
 def harness():
     from paper_2105_10529_b200.gen.__main__ import main as gen_main
     gen_main()
-    deps = [SRC] + [os.path.join(ROOT, "paper_2105_10529_b200", "csrc", f) for f in ("mf_event.cuh", "mf_device.cuh", "mf_params.h")]
+    csrc = os.path.join(ROOT, "paper_2105_10529_b200", "csrc")
+    deps = [SRC] + [os.path.join(csrc, f) for f in ("mf_event.cuh", "mf_device.cuh", "mf_params.h")]
+    deps += [os.path.join(csrc, "generated", f) for f in os.listdir(os.path.join(csrc, "generated"))]
     if not os.path.exists(LIB) or any(os.path.getmtime(LIB) < os.path.getmtime(p) for p in deps):
-        subprocess.check_call(["g++", "-O1", "-std=c++17", "-fPIC", "-shared", "-o", LIB, SRC])
+        subprocess.check_call(["g++", "-O1", "-std=c++20", "-pthread", "-fPIC", "-shared", "-o", LIB, SRC])
     lib = C.CDLL(LIB)
     lib.mfh_event.restype = C.c_double
     lib.mfh_event.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p]

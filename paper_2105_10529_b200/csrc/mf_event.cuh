@@ -112,43 +112,47 @@ MF_HD T mf_me2(const MfParams& P, T rts, const T k[MfProc<PROC>::N][4]) {
 // six colour orderings that end with gluon l and runs the generated per-lane code on cyclically relabelled gluons
 // (local label i = global gluon (i + l) mod 4); gluon currents and partial amplitudes are exchanged through the
 // warp's shared-memory tile.  Global gluons: 0, 1 incoming along +z / -z, 2, 3 = k[2], k[3]; all-incoming momenta.
-// tile: MF_LANES_TILE doubles per warp = the exchange slots [slot][32] + per event [4][6] unit polarisation vectors
-// (eps1, eps2) and [4][4] momenta.  Every lane of the warp must call (warp barriers inside); returns |M|^2 on all
-// four lanes of the group.
+// tile: MF_LANES_TILE doubles per warp = the exchange slots X[slot][32], the parked loop invariants V[slot][32], and per
+// event (8 per warp, stride MF_LANES_EVT: odd, so that the events fall on different banks) the table the generated code
+// reads: mt, p4, spinor ingredients of t and t~, all-incoming momenta [4][4] and unit polarisation vectors [4][eps1, eps2]
+// of the global gluons.  Every lane of the warp must call (warp barriers inside); returns |M|^2 on all four lanes of the group.
 #if defined(__CUDACC__)
-#define MF_LANES_TILE (MF_ME2_GG_TTGG_LANES_SLOTS * 32 + 8 * 40)
+#define MF_LANES_EVT (MF_ME2_GG_TTGG_LANES_NEV + 24 + 2)
+#define MF_LANES_TILE ((MF_ME2_GG_TTGG_LANES_SLOTS + MF_ME2_GG_TTGG_LANES_NV) * 32 + 8 * MF_LANES_EVT)
 template <typename T>
 __device__ __forceinline__ T mf_me2_ttgg_group(const MfParams& P, T rts, const T k[4][4], T* tile) {
-  static_assert(MF_ME2_GG_TTGG_LANES_NIN == 31, "generator input layout changed");
+  static_assert(MF_ME2_GG_TTGG_LANES_NEV == 31 && MF_ME2_GG_TTGG_LANES_EV_K == 15 && MF_LANES_EVT % 2 == 1, "generator input layout changed");
   const int lane = threadIdx.x & 31, lane4 = lane & 3;
-  T* Gp = tile + MF_ME2_GG_TTGG_LANES_SLOTS * 32 + (lane >> 2) * 40;
-  T* Kt = Gp + 24;
-  {                                                     // lane l publishes global gluon l
-    const T E = T(0.5) * rts, r2 = T(1.41421356237309504880);
-    T kg[4], o[5];
+  T* V = tile + MF_ME2_GG_TTGG_LANES_SLOTS * 32;
+  T* E = V + MF_ME2_GG_TTGG_LANES_NV * 32 + (lane >> 2) * MF_LANES_EVT;
+  T* Gp = E + MF_ME2_GG_TTGG_LANES_NEV;
+  {                                                     // lane l publishes global gluon l; lanes 0, 1, 2 the quark line's inputs
+    const T E0 = T(0.5) * rts, r2 = T(1.41421356237309504880);
+    T kg[4], pf[4], o[5], f[5];
 #pragma unroll
-    for (int c = 0; c < 4; ++c) kg[c] = (lane4 == 3) ? k[3][c] : k[2][c];
+    for (int c = 0; c < 4; ++c) { kg[c] = (lane4 == 3) ? k[3][c] : k[2][c]; pf[c] = (lane4 == 2) ? k[1][c] : k[0][c]; }
     mf_gluon_ing<T>(kg, o);                             // eps / sqrt2 of an outgoing gluon
+    mf_fermion_ing<T>(pf, T(P.m_top), f);
     const bool inc = lane4 < 2;
     const T sg = (lane4 == 0) ? T(1.0) : T(-1.0);
-    Kt[lane4 * 4 + 0] = inc ? E : -kg[0]; Kt[lane4 * 4 + 1] = inc ? T(0.0) : -kg[1];
-    Kt[lane4 * 4 + 2] = inc ? T(0.0) : -kg[2]; Kt[lane4 * 4 + 3] = inc ? sg * E : -kg[3];
-    Gp[lane4 * 6 + 0] = inc ? T(1.0) : r2 * o[0]; Gp[lane4 * 6 + 1] = inc ? T(0.0) : r2 * o[1]; Gp[lane4 * 6 + 2] = inc ? T(0.0) : r2 * o[2];
-    Gp[lane4 * 6 + 3] = inc ? T(0.0) : r2 * o[3]; Gp[lane4 * 6 + 4] = inc ? sg : r2 * o[4]; Gp[lane4 * 6 + 5] = T(0.0);
+    T* Kt = E + MF_ME2_GG_TTGG_LANES_EV_K + lane4 * 4;
+    Kt[0] = inc ? E0 : -kg[0]; Kt[1] = inc ? T(0.0) : -kg[1]; Kt[2] = inc ? T(0.0) : -kg[2]; Kt[3] = inc ? sg * E0 : -kg[3];
+    T* Gl = Gp + lane4 * 6;
+    Gl[0] = inc ? T(1.0) : r2 * o[0]; Gl[1] = inc ? T(0.0) : r2 * o[1]; Gl[2] = inc ? T(0.0) : r2 * o[2];
+    Gl[3] = inc ? T(0.0) : r2 * o[3]; Gl[4] = inc ? sg : r2 * o[4]; Gl[5] = T(0.0);
+    if (lane4 == 0) {
+      E[MF_ME2_GG_TTGG_LANES_EV_MT] = T(P.m_top);
+#pragma unroll
+      for (int c = 0; c < 4; ++c) E[MF_ME2_GG_TTGG_LANES_EV_P4E + c] = k[1][c];
+    } else if (lane4 < 3) {
+      T* F = E + (lane4 == 1 ? MF_ME2_GG_TTGG_LANES_EV_T_WP : MF_ME2_GG_TTGG_LANES_EV_B_WP);
+#pragma unroll
+      for (int c = 0; c < 5; ++c) F[c] = f[c];
+    }
   }
   __syncwarp();
-  T in[31];
-  in[0] = T(P.m_top);
-#pragma unroll
-  for (int c = 0; c < 4; ++c) in[1 + c] = k[1][c];
-  mf_fermion_ing<T>(k[0], T(P.m_top), in + 5);
-  mf_fermion_ing<T>(k[1], T(P.m_top), in + 10);
-#pragma unroll
-  for (int i = 0; i < 4; ++i)
-#pragma unroll
-    for (int c = 0; c < 4; ++c) in[15 + 4 * i + c] = Kt[((i + lane4) & 3) * 4 + c];
   const int b4 = lane & ~3;
-  T acc = mf_me2_gg_ttgg_lanes<T>(in, Gp, tile, lane4, lane, b4 | ((lane4 + 1) & 3), b4 | ((lane4 + 2) & 3), b4 | ((lane4 + 3) & 3));
+  T acc = mf_me2_gg_ttgg_lanes<T>(E, Gp, tile, V, lane4, lane, b4 | ((lane4 + 1) & 3), b4 | ((lane4 + 2) & 3), b4 | ((lane4 + 3) & 3));
   acc += __shfl_xor_sync(0xffffffffu, acc, 1);
   acc += __shfl_xor_sync(0xffffffffu, acc, 2);
   return T(P.me_pref) * acc;

@@ -227,13 +227,21 @@ def evaluate_event(gen, mom, mt, ferm, glu_units):
 
 
 # ---- emission -------------------------------------------------------------------------------------------
-def emit_lanes(gen, fname, sched_window=48, sched_distance=5, max_hoist_cost=None):
+def emit_lanes(gen, fname, sched_window=48, sched_distance=5, max_hoist_cost=4):
     """CUDA text of the per-lane function
-        template <typename T> T fname(const T* in, const T* G, T* X, int lane4, int xs0, int xs1, int xs2, int xs3)
-    in: the lane's inputs (order = gen.input_names); G: the event's polarisation table [global gluon][eps1, eps2][x, y, z];
-    X: the warp's exchange tile [slot][32]; lane4: lane within the group of four; xs0 = the thread's lane in the warp,
-    xs_k = lane in the warp of the group member k places on.  Returns this lane's share of sum_pol sum_{s s'} a_s C a_s'^*;
-    the caller adds the four lanes.  Counts are per LANE and event (executed, with the loop-invariant prologue once)."""
+        template <typename T> T fname(const T* E, const T* G, T* X, T* V, int lane4, int xs0, int xs1, int xs2, int xs3)
+    E: the event's table in shared memory: [0..14] = mt, p4, top and antitop spinor ingredients (gen.input_names order), then
+       the all-incoming momenta of the four GLOBAL gluons [4][4] (the lane reads its relabelled K_i = E[15 + 4 ((i + lane4) & 3)]);
+    G: the event's polarisation table [global gluon][eps1, eps2][x, y, z]; X: the warp's exchange tile [slot][32];
+    V: the warp's tile of per-lane loop invariants [NV][32]; lane4: lane within the group of four; xs0 = the thread's lane
+    in the warp, xs_k = lane in the warp of the group member k places on.
+    Nothing but pointers lives in registers across the polarisation loop: the inputs are re-read from E where they are used,
+    the expensive loop invariants (cones with a reciprocal or more than max_hoist_cost operations) are computed once, parked
+    in V and re-read; cheap ones are recomputed per trip.  (Hoisting everything kept 221 doubles alive across the loop:
+    1.8 KB of local-memory spills per thread, profiles/r2_ttgg_ncu.md.)  The loads cannot be hoisted by the compiler: the
+    stores to X may alias them.
+    Returns this lane's share of sum_pol sum_{s s'} a_s C a_s'^*; the caller adds the four lanes.  Counts are per LANE and
+    event (executed, with the loop-invariant prologue once)."""
     g = gen.g
     stores = [it[2] for it in gen.prog if it[0] == "store"]
     pro_ids, body_ids, hoisted = g.plan([gen.out] + stores, max_hoist_cost)
@@ -241,35 +249,50 @@ def emit_lanes(gen, fname, sched_window=48, sched_distance=5, max_hoist_cost=Non
     nh = 16
     pro, body = g.count_list(pro_ids), g.count_list(body_ids)
     tot = {k: pro[k] + nh * (body[k] + (1 if k == "add" else 0)) for k in pro}
+    leaf = lambda j: g.nodes[j][0] in ("in", "sym")
+    parked = sorted({o for i in body_ids for o in g._operands(i) if o not in body_set and not leaf(o)})
+    vslot = {j: n for n, j in enumerate(parked)}
+    n_ev = len(gen.input_names) - 4 * NL            # per-event scalars in front of the gluon momenta
+    assert gen.input_names[n_ev] == "k0e" and n_ev == 15
+    in_index = {}
+    for idx, n in enumerate(gen.input_names):
+        in_index[n] = "%d" % idx if idx < n_ev else "ko%d + %d" % ((idx - n_ev) // 4, (idx - n_ev) % 4)
     U = fname.upper()
     L = ["// GENERATED by paper_2105_10529_b200/gen/lanes.py -- do not edit.",
          "// one event over four lanes; per LANE and event (executed): %d add, %d mul, %d fma, %d rcp  (flops = add + mul + 2 fma = %d)"
          % (tot["add"], tot["mul"], tot["fma"], tot["rcp"], tot["add"] + tot["mul"] + 2 * tot["fma"]),
          "#define %s_NADD %dull" % (U, tot["add"]), "#define %s_NMUL %dull" % (U, tot["mul"]),
-         "#define %s_NFMA %dull" % (U, tot["fma"]), "#define %s_NIN %d" % (U, len(gen.input_names)),
-         "#define %s_SCALE %r" % (U, gen.scale), "#define %s_SLOTS %d" % (U, gen.n_slots)]
-    L.append("enum { " + ", ".join("%s_IN_%s = %d" % (U, n.upper(), i) for i, n in enumerate(gen.input_names)) + " };")
+         "#define %s_NFMA %dull" % (U, tot["fma"]), "#define %s_NEV %d" % (U, n_ev + 4 * NL),
+         "#define %s_SCALE %r" % (U, gen.scale), "#define %s_SLOTS %d" % (U, gen.n_slots), "#define %s_NV %d" % (U, len(parked))]
+    L.append("enum { " + ", ".join("%s_EV_%s = %d" % (U, n.upper(), i) for i, n in enumerate(gen.input_names[:n_ev])) + ", %s_EV_K = %d };" % (U, n_ev))
     L.append("#if defined(__CUDACC__) || defined(MF_LANES_HOST_EMULATION)      // device code (warp barriers, shared-memory tile); the CPU test harness runs it on four host threads")
     L.append("#define MF_XL(s, k) X[(s) * 32 + xs##k]")
     L.append("template <typename T>")
-    L.append("MF_DEVFN T %s(const T* __restrict__ in, const T* G, T* X, const int lane4, const int xs0, const int xs1, const int xs2, const int xs3) {" % fname)
-    for i, n in enumerate(gen.input_names):
-        L.append("  const T %s = in[%d];" % (n, i))
-    leaf = lambda j: g.nodes[j][0] in ("in", "sym")
+    L.append("MF_DEVFN T %s(const T* E, const T* G, T* X, T* V, const int lane4, const int xs0, const int xs1, const int xs2, const int xs3) {" % fname)
+    for i in range(NL):
+        L.append("  const int gl%d = (lane4 + %d) & 3, ko%d = %d + 4 * gl%d;" % (i, i, i, n_ev, i))
+    L.append("  {      // loop invariants that are worth keeping: computed once, parked in V")
+    used_pro = sorted({o for i in pro_ids for o in g._operands(i) if g.nodes[o][0] == "in"})
+    for j in used_pro:
+        L.append("    const T %s = E[%s];" % (g.names[j], in_index[g.names[j]]))
     pname = lambda j: g.names[j] if leaf(j) else "p%d" % j
-    L += g.emit_list(pro_ids, pname, "p")
+    L += g.emit_list(pro_ids, pname, "p", indent="    ")
+    for j in parked:
+        L.append("    V[%d * 32 + xs0] = p%d;" % (vslot[j], j))
+    L.append("  }")
     L.append("  T acc = T(0.0);")
     L.append("#pragma unroll 1")
     L.append("  for (int ih = 0; ih < %d; ++ih) {" % nh)
     for i in range(NL):
-        L.append("    const int gl%d = (lane4 + %d) & 3;" % (i, i))
         L.append("    const T* gp%d = G + gl%d * 6 + (((ih >> gl%d) & 1) ? 0 : 3);" % (i, i, i))
         L.append("    const T pl%dx = gp%d[0], pl%dy = gp%d[1], pl%dz = gp%d[2];" % (i, i, i, i, i, i))
 
     def bname(j):
+        if g.nodes[j][0] == "in":
+            return "E[%s]" % in_index[g.names[j]]
         if leaf(j):
             return g.names[j]
-        return "v%d" % j if j in body_set else "p%d" % j
+        return "v%d" % j if j in body_set else "V[%d * 32 + xs0]" % vslot[j]
 
     lo, nstmt = 0, 0
     for it in gen.prog:
@@ -295,4 +318,4 @@ def emit_lanes(gen, fname, sched_window=48, sched_distance=5, max_hoist_cost=Non
     L.append("}")
     L.append("#undef MF_XL")
     L.append("#endif")
-    return "\n".join(L) + "\n", tot, dict(pro=pro, body=body)
+    return "\n".join(L) + "\n", tot, dict(pro=pro, body=body, parked=len(parked))

@@ -12,32 +12,33 @@ static inline void __syncwarp() { g_lane_barrier.arrive_and_wait(); }
 #include "../../paper_2105_10529_b200/csrc/mf_event.cuh"
 #include "../../paper_2105_10529_b200/csrc/mf_params.h"
 
-// host stand-in of mf_me2_ttgg_group (mf_event.cuh): same publishing of the global gluons, same per-lane inputs
+// host stand-in of mf_me2_ttgg_group (mf_event.cuh): same event table, same per-lane call
 static double ttgg_lanes_host(const MfParams& P, double rts, const double k[4][4]) {
-  static double tile[MF_ME2_GG_TTGG_LANES_SLOTS * 32 + 40];
-  double* Gp = tile + MF_ME2_GG_TTGG_LANES_SLOTS * 32;
-  double* Kt = Gp + 24;
-  const double E = 0.5 * rts, r2 = 1.41421356237309504880;
+  constexpr int SL = MF_ME2_GG_TTGG_LANES_SLOTS, NV = MF_ME2_GG_TTGG_LANES_NV, NEV = MF_ME2_GG_TTGG_LANES_NEV;
+  static double tile[(SL + NV) * 32 + NEV + 24];
+  double* V = tile + SL * 32;
+  double* E = V + NV * 32;
+  double* Gp = E + NEV;
+  const double E0 = 0.5 * rts, r2 = 1.41421356237309504880;
+  E[MF_ME2_GG_TTGG_LANES_EV_MT] = P.m_top;
+  for (int c = 0; c < 4; ++c) E[MF_ME2_GG_TTGG_LANES_EV_P4E + c] = k[1][c];
+  mf_fermion_ing<double>(k[0], P.m_top, E + MF_ME2_GG_TTGG_LANES_EV_T_WP);
+  mf_fermion_ing<double>(k[1], P.m_top, E + MF_ME2_GG_TTGG_LANES_EV_B_WP);
   for (int l = 0; l < 4; ++l) {
     const bool inc = l < 2;
     const double sg = l == 0 ? 1.0 : -1.0;
     const double* kg = l == 3 ? k[3] : k[2];
     double o[5];
     mf_gluon_ing<double>(kg, o);
-    Kt[l * 4 + 0] = inc ? E : -kg[0]; Kt[l * 4 + 1] = inc ? 0.0 : -kg[1]; Kt[l * 4 + 2] = inc ? 0.0 : -kg[2]; Kt[l * 4 + 3] = inc ? sg * E : -kg[3];
+    double* Kt = E + MF_ME2_GG_TTGG_LANES_EV_K + 4 * l;
+    Kt[0] = inc ? E0 : -kg[0]; Kt[1] = inc ? 0.0 : -kg[1]; Kt[2] = inc ? 0.0 : -kg[2]; Kt[3] = inc ? sg * E0 : -kg[3];
     Gp[l * 6 + 0] = inc ? 1.0 : r2 * o[0]; Gp[l * 6 + 1] = inc ? 0.0 : r2 * o[1]; Gp[l * 6 + 2] = inc ? 0.0 : r2 * o[2];
     Gp[l * 6 + 3] = inc ? 0.0 : r2 * o[3]; Gp[l * 6 + 4] = inc ? sg : r2 * o[4]; Gp[l * 6 + 5] = 0.0;
   }
   double acc[4];
   std::thread th[4];
   for (int l = 0; l < 4; ++l) th[l] = std::thread([&, l] {
-    double in[31];
-    in[0] = P.m_top;
-    for (int c = 0; c < 4; ++c) in[1 + c] = k[1][c];
-    mf_fermion_ing<double>(k[0], P.m_top, in + 5);
-    mf_fermion_ing<double>(k[1], P.m_top, in + 10);
-    for (int i = 0; i < 4; ++i) for (int c = 0; c < 4; ++c) in[15 + 4 * i + c] = Kt[((i + l) & 3) * 4 + c];
-    acc[l] = mf_me2_gg_ttgg_lanes<double>(in, Gp, tile, l, l, (l + 1) & 3, (l + 2) & 3, (l + 3) & 3);
+    acc[l] = mf_me2_gg_ttgg_lanes<double>(E, Gp, tile, V, l, l, (l + 1) & 3, (l + 2) & 3, (l + 3) & 3);
   });
   for (int l = 0; l < 4; ++l) th[l].join();
   return P.me_pref * ((acc[0] + acc[1]) + (acc[2] + acc[3]));

@@ -28,7 +28,59 @@ import numpy as np
 METRIC = "integrand events/sec (fp64) gg->ttbar g, 1e7 events/iteration/GPU"
 N_EVENTS = 10_000_000
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # SMs x DFMA lanes x 2 x max clock
-ME_KERNEL_DRAM_BYTES = 1.0730e9                          # ncu --set full capture of mf_me_kernel<2> (profiles/r1b_staged_ncu.md)
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r2_ncu_traffic.json")   # dram bytes per passing event from the committed ncu capture
+
+
+def ncu_traffic(kernel, n_pass):
+    """roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel`, from the committed ncu
+    --set full capture (profiles/r2_ncu_traffic.json: bytes per cut-passing event of that capture), scaled to the passing
+    events of one launch of THIS run; (None, why) when no capture of that kernel is on file"""
+    try:
+        with open(TRAFFIC_FILE) as f:
+            rec = json.load(f)[kernel]
+    except (OSError, KeyError, ValueError):
+        return None, "no ncu capture of %s in profiles/r2_ncu_traffic.json" % kernel
+    return rec["dram_bytes_per_passing_event"] * n_pass, rec["source"]
+
+
+def launch_ranks_if_needed(args, argv):
+    """`python bench.py --gpus N` without torchrun: start N ranks (one per GPU) of this very command"""
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        port = str(29500 + os.getpid() % 400)
+        os.execvp(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+                                   "--master-addr", "127.0.0.1", "--master-port", port, os.path.abspath(__file__)] + argv)
+
+
+def init_ranks(backend="nccl", force_group=False):
+    """(rank, local_rank, world, dist or None) from the torchrun environment; the process group exists iff world > 1 or
+    force_group (the N > 1 code path at N = 1).  backend "gloo" runs the same logic on CPU (tests/test_sharding.py)."""
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world == 1 and not force_group:
+        return rank, local_rank, world, None
+    import torch
+    import torch.distributed as dist
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    os.environ.setdefault("MASTER_PORT", "29533")
+    kw = {}
+    if backend == "nccl":
+        os.environ.setdefault("NCCL_DEBUG", "INFO")              # the communicator log (ranks, transport) goes to stderr:
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")       # stdout carries the one JSON line
+        os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")
+        kw["device_id"] = torch.device("cuda", local_rank)
+    dist.init_process_group(backend, rank=rank, world_size=world, **kw)
+    return rank, local_rank, world, dist
+
+
+def max_over_ranks(dist, value, device=None):
+    """device time of the slowest rank (the contract's timing rule)"""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
 
 
 class ClockSampler:
@@ -70,7 +122,7 @@ def oracle_rate(n_threads, seconds):
     from paper_2105_10529_b200 import workloads as W
     cfg = W.config(W.GG_TTG, seed=0)
     orc = mfo.Vegas(cfg)
-    probe = 500 * n_threads
+    probe = 2000 * n_threads
     t0 = time.perf_counter(); orc.accumulate(0, 0, probe, N_EVENTS, n_threads=n_threads); dt = time.perf_counter() - t0
     n = max(probe, int(probe / dt * seconds))
     t0 = time.perf_counter(); orc.iterate(n, n_threads=n_threads); dt = time.perf_counter() - t0
@@ -109,21 +161,13 @@ def run_reference(args, rank):
         "gpu_launches": 0}))
 
 
-def run_ours(args, rank, local_rank, world):
+def run_ours(args, rank, local_rank, world, dist):
     import torch
     from paper_2105_10529_b200 import binding, sharding, workloads as W
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU path); use --impl reference for the oracle")
     binding.lib()
-    dist = None
-    sharded = world > 1 or args.sharded                                    # the N > 1 code path (also at N = 1 with --sharded)
-    if sharded:
-        import torch.distributed as dist
-        if world == 1:
-            os.environ.setdefault("MASTER_ADDR", "127.0.0.1"); os.environ.setdefault("MASTER_PORT", "29533")
-            dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", local_rank))
-        else:
-            dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    sharded = dist is not None                                             # the N > 1 code path (also at N = 1 with --sharded)
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     n, n_total = args.events, args.events * world
@@ -132,6 +176,7 @@ def run_ours(args, rank, local_rank, world):
     staged = args.path == "staged"
     h.set_path(staged)
     flops = h.me_flops()
+    bounds = h.me_flops_bounds()
     uuid = "GPU-" + str(torch.cuda.get_device_properties(dev).uuid)
     peak_before = binding.fp64_peak(local_rank, 0.3)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)          # > 126 MB L2
@@ -141,102 +186,113 @@ def run_ours(args, rank, local_rank, world):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def step():
-        flush.zero_()                                                      # L2 flush between iterations
+    def step(sync=False):
+        flush.zero_()                                                      # L2 flush between iterations (both timed loops)
         if not sharded:
-            h.vegas_iterate(n, sync=False)
-        else:
-            sharding.sharded_iterate_device(h, n_total, rank, world, dist, dev, sync=False)
+            return h.vegas_iterate(n, sync=sync)
+        return sharding.sharded_iterate_device(h, n_total, rank, world, dist, dev, sync=sync)
 
     # clocks are sampled from the first warm-up step to the end of the end-to-end region (same load)
     sampler = ClockSampler(uuid) if rank == 0 else None
     for _ in range(args.warmup):
         step()
     barrier()
+    if staged:
+        h.stage_ms_sum()                                                   # forget the warm-up launches
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    kernel_ms, pass_frac, stage_ms = [], [], []
+    fused_ms = []
     e0.record()
-    for _ in range(args.steps):
+    for _ in range(args.steps):                                            # nothing synchronises inside the timed region
         step()
-        kernel_ms.append(h.last_kernel_ms()[0])        # waits for this step's dominant kernel (event sync)
-        if staged:
-            stage_ms.append(h.last_stage_ms())
+        if not staged:
+            fused_ms.append(h.last_kernel_ms()[0])                         # (fused path: one event pair per handle -> waits per step)
     e1.record()
     barrier()
-    ms = e0.elapsed_time(e1)
-    if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(dist, e0.elapsed_time(e1), dev)
+    if staged:                                                             # CUDA events the library recorded on the launching stream
+        sums, launches = h.stage_ms_sum()                                  # around every stage of every timed launch
+        stages = {k: v / launches for k, v in sums.items()}
+        k_ms = stages["me"]
+    else:
+        stages, launches, k_ms = None, len(fused_ms), float(np.mean(fused_ms))
     its = h.get_iterations()
-    pass_frac = [it["n_pass"] / it["n_events"] for it in its[-args.steps:]]
+    pass_frac = float(np.mean([it["n_pass"] / it["n_events"] for it in its[-args.steps:]]))
     value = n_total * args.steps / (ms * 1e-3)
 
-    # end to end through the C-ABI with host buffers: grid in from the host, record + grid back out
+    # end to end through the C-ABI with host buffers: grid in from the host, record + grid back out, same L2 flush
     grid = h.get_grid()
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
         h.set_grid(grid)                                                   # H2D d*51 doubles
-        if not sharded:
-            rec = h.vegas_iterate(n, sync=True)                            # D2H iteration record
-        else:
-            rec = sharding.sharded_iterate_device(h, n_total, rank, world, dist, dev, sync=True)
+        rec = step(sync=True)                                              # D2H iteration record (40 B)
         grid = h.get_grid()                                                # D2H refined grid
     barrier()
-    e2e_s = time.perf_counter() - t0
-    if dist is not None:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(dist, time.perf_counter() - t0, dev)
     clocks = sampler.stop() if sampler else None
     peak_after = binding.fp64_peak(local_rank, 0.3)
     res = h.result()
     if rank != 0:
         return
-    k_ms = float(np.mean(kernel_ms))
-    n_pass = float(np.mean(pass_frac)) * n                                 # per launch (this rank's events)
-    achieved = flops["flops"] * n_pass / (k_ms * 1e-3) / 1e12
+    n_pass = pass_frac * n                                                 # per launch (this rank's events)
+    step_ms = ms / args.steps
     peak = max(peak_before, peak_after) / 1e12
+    tf = lambda fl, t_ms: fl * n_pass / (t_ms * 1e-3) / 1e12               # TFLOP/s of `fl` flops per passing event over t_ms
+    achieved = tf(flops["flops"], k_ms)
+    kernel = "mf_me_kernel<2, double, 256>" if staged else "mf_iterate_compact_kernel<2>"
+    traffic, traffic_src = ncu_traffic(kernel, n_pass) if staged else (None, "fused path: no per-event traffic")
     grid_bytes = int(grid.nbytes)
     out = {
         "metric": METRIC, "value": value, "unit": "events/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": "configs[2]: pp->tt~g via gg->tt~g (16 diagrams, 6x6 colour matrix), massive 3-body RAMBO + "
                                "Newton, cuts pT>30 |eta|<2.5, VEGAS 7 dims x 50 bins, seed 0, successive iterations of one run",
-                   "events_per_step_per_gpu": n, "pass_fraction": float(np.mean(pass_frac)),
-                   "path": args.path,
-                   "l2": "flushed between steps (256 MiB memset inside the timed region); inputs are 46 KB of tables; "
-                         "the staged path passes ~1.0 GB of event records per step through HBM (> 126 MB L2)", "parallelism": "event ranges over %d GPU(s), 1 NCCL all-reduce of 354 "
-                         "doubles on the device per iteration (no host round trip)" % world if sharded else "1 GPU",
+                   "events_per_step_per_gpu": n, "pass_fraction": pass_frac, "path": args.path,
+                   "l2": "flushed before every step of both timed loops (256 MiB memset inside the timed region); inputs are 46 KB "
+                         "of tables; the staged path passes ~1.0 GB of event records per step through HBM (> 126 MB L2)",
+                   "parallelism": "event ranges over %d GPU(s), 1 NCCL all-reduce of 354 doubles on the device per iteration "
+                                  "(no host round trip)" % world if sharded else "1 GPU",
                    "integral_pb": res["integral"], "sigma_pb": res["sigma"]},
         "clocks": clocks,
         "e2e": {"value": n_total * args.steps / e2e_s, "unit": "events/s", "h2d_bytes_per_step": grid_bytes,
                 "d2h_bytes_per_step": grid_bytes + 40},
         "gpu_launches": ((5 if staged else 3) + (2 if sharded else 0)) * args.steps,   # + pack/unpack of the raw sums around the all-reduce
-        "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                     "traffic": ME_KERNEL_DRAM_BYTES if staged else None,
-                     "traffic_source": "profiles/r1b_staged_ncu.md (dram__bytes_read.sum + dram__bytes_write.sum of one mf_me_kernel<2> launch; algorithmic: 120 B per passing event = %.3e B)" % (120.0 * n_pass) if staged else None,
-                     "kernel": "mf_me_kernel<2>" if staged else "mf_iterate_compact_kernel<2>", "kernel_ms": k_ms,
-                     "flops_per_event": flops["flops"], "fma_fraction_of_ops": flops["fma"] / (flops["add"] + flops["mul"] + flops["fma"]),
-                     "peak_source": "measured DFMA-chain microbenchmark (mf_fp64_peak), max of before/after the timed region",
-                     "peak_before": peak_before / 1e12, "peak_after": peak_after / 1e12,
-                     "peak_nominal": FP64_NOMINAL_TFLOPS, "frac_nominal": achieved / FP64_NOMINAL_TFLOPS,
-                     "note": "algorithmic flops = generator-counted |M|^2 add+mul+2*fma per passing event; front end not counted"},
+        "roofline": {
+            "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+            "traffic": traffic, "traffic_source": traffic_src,
+            "algorithmic_bytes": 120.0 * n_pass if staged else 0.0,
+            "kernel": kernel, "kernel_ms": k_ms, "kernel_launches_timed": launches, "kernel_share_of_step": k_ms / step_ms,
+            "flops_per_event": flops["flops"], "fma_fraction_of_ops": flops["fma"] / (flops["add"] + flops["mul"] + flops["fma"]),
+            "peak_source": "measured DFMA-chain microbenchmark (mf_fp64_peak), max of before/after the timed region; "
+                           "MEASURED_PEAKS.json and the profiling guide have no fp64 entry",
+            "peak_before": peak_before / 1e12, "peak_after": peak_after / 1e12, "peak_nominal": FP64_NOMINAL_TFLOPS,
+            # the same algorithmic flops over the WHOLE step (front end, reductions, memsets, launch gaps included):
+            # what north_star's "sustained in the integrand" asks; and both against the chip's nominal peak
+            "frac_step": tf(flops["flops"], step_ms) / peak,
+            "frac_nominal": achieved / FP64_NOMINAL_TFLOPS,
+            "frac_step_nominal": tf(flops["flops"], step_ms) / FP64_NOMINAL_TFLOPS,
+            # the leanest op list the generator knows for this amplitude (every helicity unrolled, everything shared)
+            "flops_per_event_min": bounds["min"], "frac_min": tf(bounds["min"], k_ms) / peak,
+            "frac_step_min": tf(bounds["min"], step_ms) / peak,
+            "flops_per_event_executed": bounds["executed"],
+            "note": "algorithmic flops = generator-counted |M|^2 add+mul+2*fma per passing event of the emitted organisation "
+                    "(helicity loop: loop invariants counted once); front end, wavefunction ingredients and padding not counted"},
     }
     if staged:
-        out["roofline"]["stages_ms"] = {k: float(np.mean([m[k] for m in stage_ms])) for k in ("front", "me", "reduce")}
-        rec_bytes = 15 * 8 * n_pass                                        # 4*3+3 doubles per passing event
-        out["roofline"]["front_stage_hbm_gbps"] = rec_bytes / (out["roofline"]["stages_ms"]["front"] * 1e-3) / 1e9
-        out["roofline"]["reduce_stage_hbm_gbps"] = 16 * n_pass / (out["roofline"]["stages_ms"]["reduce"] * 1e-3) / 1e9
+        out["roofline"]["stages_ms"] = stages
+        out["roofline"]["front_stage_hbm_gbps"] = 15 * 8 * n_pass / (stages["front"] * 1e-3) / 1e9   # 4*3+3 doubles per passing event
+        out["roofline"]["reduce_stage_hbm_gbps"] = 16 * n_pass / (stages["reduce"] * 1e-3) / 1e9
     if world == 1 and not args.no_cpu_baseline:
         from oracle import mfo
         mfo.build()
         nt = mfo.max_threads()
-        v, ns, dt = oracle_rate(nt, 15.0)
+        v, ns, dt = oracle_rate(nt, 12.0)
+        v1, ns1, dt1 = oracle_rate(1, 6.0)
         out["cpu_baseline"] = {"value": v, "unit": "events/s", "cores": nt, "kind": "oracle",
-                               "sample": "first %d events of the 1e7-event iteration, whole path, %.1f s" % (ns, dt)}
+                               "sample": "first %d events of the 1e7-event iteration, whole path, %.1f s" % (ns, dt),
+                               "single_thread": {"value": v1, "unit": "events/s", "cores": 1,
+                                                 "sample": "first %d events, whole path, %.1f s" % (ns1, dt1)}}
     print(json.dumps(out))
 
 
@@ -345,24 +401,21 @@ def main():
     ap.add_argument("--path", default="staged", choices=["staged", "fused"],
                     help="staged: front end / |M|^2 / reductions as three kernels (default); fused: one kernel")
     args = ap.parse_args()
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "ours" and not (args.sweep or args.processes):
+        launch_ranks_if_needed(args, sys.argv[1:])         # --gpus N without torchrun: N ranks of this command
     if args.impl == "reference":
-        run_reference(args, rank)
+        run_reference(args, int(os.environ.get("RANK", "0")))
         return
-    if args.sweep:
-        if rank == 0:
-            run_sweep(args)
+    if args.sweep or args.processes:
+        if int(os.environ.get("RANK", "0")) == 0:
+            (run_sweep if args.sweep else run_processes)(args)
         return
-    if args.processes:
-        if rank == 0:
-            run_processes(args)
-        return
-    run_ours(args, rank, local_rank, world)
-    if world > 1 or args.sharded:
-        import torch.distributed as dist
-        dist.destroy_process_group()
+    rank, local_rank, world, dist = init_ranks("nccl", force_group=args.sharded)
+    try:
+        run_ours(args, rank, local_rank, world, dist)
+    finally:
+        if dist is not None:
+            dist.destroy_process_group()
 
 
 if __name__ == "__main__":

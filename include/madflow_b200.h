@@ -87,8 +87,9 @@ typedef struct {
   uint8_t *bins;             /* [n][d]  VEGAS bin indices k_j                                         */
   double  *momenta;          /* [n][2+n_final][4]  (E,px,py,pz), partonic CM frame, incoming first   */
   double  *me2;              /* [n]  |M|^2 averaged/summed, before the symmetry factor; 0 if cut     */
-  double  *pdf;              /* [n][2]  xg(x1,muF^2), xg(x2,muF^2)                                    */
-  uint8_t *pass;             /* [n]  1 if the event passed the cuts                                  */
+  double  *pdf;              /* [n][2]  xg(x1,muF^2), xg(x2,muF^2); process 4: the two flavour sums L12, L21;     */
+                             /*         process 5: xg(x1) xg(x2) and L12 + L21 (see MF_QQ_TT / MF_PP_TT above) */
+  uint8_t *pass;             /* [n]  1 if the event passed the cuts (always 1 for processes 0, 1, 4, 5: no cuts) */
 } mf_eval_out_t;
 
 typedef struct { double integral, sigma; uint64_t n_events, n_pass, n_nonfinite; float kernel_ms; } mf_iter_t;
@@ -96,7 +97,8 @@ typedef struct { double integral, sigma, chi2_dof; uint32_t n_iter; } mf_result_
 
 /* Validate cfg, copy it and the PDF table, allocate device state, set the uniform grid.  No kernel
  * work.  Errors: MF_EINVAL (bad field, kinematics outside the PDF grid), MF_EUNSUPPORTED
- * (precision != 64), MF_ECUDA (no device / allocation failure).                                    */
+ * (precision other than 64, or 32 for a process other than MF_GG_TTG), MF_ECUDA (no device /
+ * allocation failure).  Every call leaves the caller's current CUDA device as it found it.           */
 int mf_vegas_create(const mf_config_t *cfg, mf_vegas_t **out);
 int mf_vegas_destroy(mf_vegas_t *h);
 /* d = VEGAS dimensions (2 for process 0, else 2 + 3 n_final - 4, or 2 + 4 n_final with MF_GEN_CLASSIC_RAMBO),
@@ -157,8 +159,11 @@ int mf_set_observables(mf_vegas_t *h, const mf_observable_t *obs, uint32_t n_obs
 int mf_get_observables(mf_vegas_t *h, double *host_sum, double *host_sum2, uint32_t *n_iter);
 int mf_accum_len(const mf_vegas_t *h, uint32_t *n);
 
-/* O11 combination over all iterations so far; synchronises the last-used stream.  MF_ESTATE if no
- * iteration has been run.                                                                           */
+/* O11 combination over all iterations so far, enqueued behind the last call that changed the integrator
+ * state, on that call's stream, which is then synchronised.  MF_ESTATE if no iteration has been run.
+ * Stream ordering in general: calls may be issued on different streams; a call that reads or writes the
+ * integrator state (grid, raw sums, records) waits on the device for the last call that wrote it, a call
+ * that writes the grid also for evaluations in flight; host reads (get_*, result) wait for both.        */
 int mf_result(mf_vegas_t *h, mf_result_t *host_out);
 /* per-iteration records; host_out[n_iter] must hold at least max_iter entries; *n_iter = stored    */
 int mf_get_iterations(mf_vegas_t *h, mf_iter_t *host_out, uint32_t max_iter, uint32_t *n_iter);
@@ -172,8 +177,14 @@ int mf_set_launch(mf_vegas_t *h, uint32_t blocks_per_sm, uint32_t threads_per_bl
  * order (hence the last bits of the sums) differs.                                                   */
 int mf_set_path(mf_vegas_t *h, int32_t staged);
 /* Device times of the three stages (front end, |M|^2, reductions; ms3[3], host) of the last staged
- * launch.  MF_ESTATE if the last accumulate ran the fused path.  Waits for the events.              */
+ * launch (the last SLICE of an iteration of more than 2^24 events: use mf_stage_ms_sum for the whole).
+ * MF_ESTATE if the last accumulate ran the fused path.  Waits for the events.                       */
 int mf_last_stage_ms(const mf_vegas_t *h, float *ms3);
+/* Sums of the three stage times over ALL staged launches (every slice of every iteration) since the
+ * previous call, and their number (*launches; at most the last 256 are kept); resets the count.  The
+ * events are recorded on the caller's stream inside mf_vegas_accumulate, nothing synchronises until this
+ * call, which waits for the last of them.                                                            */
+int mf_stage_ms_sum(mf_vegas_t *h, float *ms3, uint32_t *launches);
 /* Device times (CUDA events on the caller's stream): of the dominant S1-S9 kernel (fused kernel, or
  * the |M|^2 stage of the staged path) of the last
  * mf_vegas_accumulate / mf_vegas_iterate, and of the whole last mf_vegas_iterate (memsets + fused
@@ -182,6 +193,11 @@ int mf_last_kernel_ms(const mf_vegas_t *h, float *fused_kernel_ms, float *iterat
 /* Exact add/mul/fma counts per event of the generated |M|^2 code of the handle's process
  * (generator-counted): flops = add + mul + 2 fma.                    */
 int mf_me_flops(const mf_vegas_t *h, uint64_t *n_add, uint64_t *n_mul, uint64_t *n_fma);
+/* flops per event of the LEANEST organisation of the same amplitude the build-time generator knows (every helicity
+ * configuration unrolled, every subexpression shared: gg -> tt~g 11 302, gg -> tt~gg 170 880; other processes: the count
+ * of mf_me_flops), and the flops the kernels EXECUTE per event for S7 (= mf_me_flops, except gg -> tt~gg: four lanes per
+ * event, each with its own prologue and a share of recomputation).  mf_me_flops lies between the two.        */
+int mf_me_flops_bounds(const mf_vegas_t *h, uint64_t *flops_min, uint64_t *flops_executed);
 /* Register-resident DFMA-chain microbenchmark on `device`: measured fp64 FLOP/s (roofline peak).   */
 int mf_fp64_peak(int32_t device, double seconds, double *host_flops_per_s);
 const char *mf_last_error(void);

@@ -9,7 +9,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("MF_LIB", os.path.join(_HERE, "libmadflow_b200.so"))   # MF_LIB: tuning variants
+LIB_PATH = os.path.join(_HERE, "libmadflow_b200.so")
 
 MF_OK, MF_EINVAL, MF_ENOMEM, MF_ECUDA, MF_ESTATE, MF_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 EXPORTS = ["mf_vegas_create", "mf_vegas_destroy", "mf_ndim", "mf_integrand_eval", "mf_vegas_iterate",
@@ -17,7 +17,7 @@ EXPORTS = ["mf_vegas_create", "mf_vegas_destroy", "mf_ndim", "mf_integrand_eval"
            "mf_get_iterations", "mf_get_grid", "mf_set_grid", "mf_set_launch", "mf_me_flops",
            "mf_fp64_peak", "mf_last_kernel_ms", "mf_last_error", "mf_set_path", "mf_last_stage_ms",
            "mf_set_observables", "mf_get_observables", "mf_accum_len", "mf_zero_accum", "mf_get_accum_device",
-           "mf_set_accum_device"]
+           "mf_set_accum_device", "mf_stage_ms_sum", "mf_me_flops_bounds"]
 
 
 class MfError(RuntimeError):
@@ -105,6 +105,8 @@ def lib():
         L.mf_get_accum_device.argtypes = [vp, vp, vp]
         L.mf_set_accum_device.argtypes = [vp, vp, vp]
         L.mf_last_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
+        L.mf_stage_ms_sum.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(u32)]
+        L.mf_me_flops_bounds.argtypes = [vp, C.POINTER(u64), C.POINTER(u64)]
         L.mf_me_flops.argtypes = [vp, C.POINTER(u64), C.POINTER(u64), C.POINTER(u64)]
         L.mf_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
         L.mf_fp64_peak.argtypes = [C.c_int32, C.c_double, C.POINTER(C.c_double)]
@@ -124,11 +126,12 @@ def _check(rc):
         raise MfError(rc, lib().mf_last_error().decode())
 
 
-def _stream_ptr(stream):
+def _stream_ptr(stream, device=None):
+    """cudaStream_t of `stream` (an int / torch stream pointer), default: torch's current stream ON THE HANDLE'S DEVICE"""
     if stream is None:
         import torch
-        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
-    return C.c_void_p(int(stream))
+        return C.c_void_p(torch.cuda.current_stream(device).cuda_stream)
+    return C.c_void_p(int(getattr(stream, "cuda_stream", stream)))
 
 
 class Vegas:
@@ -165,21 +168,21 @@ class Vegas:
                        pass_=torch.empty(n, dtype=torch.uint8, device=dev))
         eo = EvalOut(**{k: (v.data_ptr() if n else None) for k, v in out.items()})
         with torch.cuda.device(dev):
-            _check(lib().mf_integrand_eval(self._h, iteration, int(first_event), n, C.byref(eo), _stream_ptr(stream)))
+            _check(lib().mf_integrand_eval(self._h, iteration, int(first_event), n, C.byref(eo), _stream_ptr(stream, self.device)))
         return out
 
     def integrand_eval_into(self, iteration, first_event, n_events, weight_ptr, stream=None):
         """mf_integrand_eval writing only the weights to a caller-owned device pointer"""
         eo = EvalOut(weight=weight_ptr)
-        _check(lib().mf_integrand_eval(self._h, iteration, int(first_event), int(n_events), C.byref(eo), _stream_ptr(stream)))
+        _check(lib().mf_integrand_eval(self._h, iteration, int(first_event), int(n_events), C.byref(eo), _stream_ptr(stream, self.device)))
 
     def vegas_iterate(self, n_events, stream=None, sync=True):
         it = Iter()
-        _check(lib().mf_vegas_iterate(self._h, int(n_events), _stream_ptr(stream), C.byref(it) if sync else None))
+        _check(lib().mf_vegas_iterate(self._h, int(n_events), _stream_ptr(stream, self.device), C.byref(it) if sync else None))
         return _iter_dict(it) if sync else None
 
     def vegas_accumulate(self, first_event, n_events, n_total, stream=None):
-        _check(lib().mf_vegas_accumulate(self._h, int(first_event), int(n_events), int(n_total), _stream_ptr(stream)))
+        _check(lib().mf_vegas_accumulate(self._h, int(first_event), int(n_events), int(n_total), _stream_ptr(stream, self.device)))
 
     def accum_len(self):
         n = C.c_uint32()
@@ -214,18 +217,18 @@ class Vegas:
         _check(lib().mf_set_accum(self._h, acc.ctypes.data, cnt.ctypes.data))
 
     def zero_accum(self, stream=None):
-        _check(lib().mf_zero_accum(self._h, _stream_ptr(stream)))
+        _check(lib().mf_zero_accum(self._h, _stream_ptr(stream, self.device)))
 
     def get_accum_device(self, dev_ptr, stream=None):
         """raw sums + the two counters (as doubles) into a device buffer of accum_len() + 2 doubles; enqueue only"""
-        _check(lib().mf_get_accum_device(self._h, C.c_void_p(int(dev_ptr)), _stream_ptr(stream)))
+        _check(lib().mf_get_accum_device(self._h, C.c_void_p(int(dev_ptr)), _stream_ptr(stream, self.device)))
 
     def set_accum_device(self, dev_ptr, stream=None):
-        _check(lib().mf_set_accum_device(self._h, C.c_void_p(int(dev_ptr)), _stream_ptr(stream)))
+        _check(lib().mf_set_accum_device(self._h, C.c_void_p(int(dev_ptr)), _stream_ptr(stream, self.device)))
 
     def vegas_finalize(self, n_total, stream=None, sync=True):
         it = Iter()
-        _check(lib().mf_vegas_finalize(self._h, int(n_total), _stream_ptr(stream), C.byref(it) if sync else None))
+        _check(lib().mf_vegas_finalize(self._h, int(n_total), _stream_ptr(stream, self.device), C.byref(it) if sync else None))
         return _iter_dict(it) if sync else None
 
     def result(self):
@@ -263,6 +266,17 @@ class Vegas:
         a, b = C.c_float(), C.c_float()
         _check(lib().mf_last_kernel_ms(self._h, C.byref(a), C.byref(b)))
         return a.value, b.value
+
+    def stage_ms_sum(self):
+        """sums of the stage times over all staged launches since the previous call, and their number"""
+        ms = (C.c_float * 3)(); n = C.c_uint32()
+        _check(lib().mf_stage_ms_sum(self._h, ms, C.byref(n)))
+        return dict(front=ms[0], me=ms[1], reduce=ms[2]), n.value
+
+    def me_flops_bounds(self):
+        lo, ex = C.c_uint64(), C.c_uint64()
+        _check(lib().mf_me_flops_bounds(self._h, C.byref(lo), C.byref(ex)))
+        return dict(min=lo.value, executed=ex.value)
 
     def me_flops(self):
         a, m, f = C.c_uint64(), C.c_uint64(), C.c_uint64()

@@ -18,11 +18,8 @@ def _newer(target, deps):
     return os.path.exists(target) and all(os.path.getmtime(target) >= os.path.getmtime(d) for d in deps)
 
 
-def build(force=False, verbose=False, extra_flags=(), tag="", only=(0, 1, 2, 3, 4, 5)):
-    """tag/extra_flags/only: tuning variants (objects and library get the tag as a suffix)"""
-    global OBJ, LIB
-    obj_dir = OBJ + tag
-    lib = LIB if not tag else LIB.replace(".so", tag + ".so")
+def build(force=False, verbose=False):
+    obj_dir, lib = OBJ, LIB
     from .gen.__main__ import main as gen_main
     gen_main()
     os.makedirs(obj_dir, exist_ok=True)
@@ -31,14 +28,14 @@ def build(force=False, verbose=False, extra_flags=(), tag="", only=(0, 1, 2, 3, 
     api = kern + [os.path.join(CSRC, f) for f in ("mf_small_kernels.cuh", "mf_params.h")]
     api += [os.path.join(os.path.dirname(HERE), "include", "madflow_b200.h")]
     jobs = [("mf_api.o", os.path.join(CSRC, "mf_api.cu"), [])]
-    jobs += [("mf_proc%d.o" % p, os.path.join(CSRC, "mf_proc.cu" if p in only else "mf_proc_stub.cu"), ["-DMF_PROC=%d" % p]) for p in range(6)]
+    jobs += [("mf_proc%d.o" % p, os.path.join(CSRC, "mf_proc.cu"), ["-DMF_PROC=%d" % p]) for p in range(6)]
 
     def compile_one(job):
         obj, src, extra = job
         out = os.path.join(obj_dir, obj)
         if not force and _newer(out, (api if obj == "mf_api.o" else kern) + [src]):
             return obj, "up to date"
-        r = subprocess.run(["nvcc"] + NVCC_FLAGS + list(extra_flags) + extra + ["-c", src, "-o", out], capture_output=True, text=True)
+        r = subprocess.run(["nvcc"] + NVCC_FLAGS + extra + ["-c", src, "-o", out], capture_output=True, text=True)
         with open(out + ".log", "w") as f:
             f.write(r.stdout + r.stderr)
         if r.returncode != 0:

@@ -21,6 +21,15 @@ static int fail(int code, const std::string& msg) { g_err = msg; return code; }
     if (e_ != cudaSuccess) return fail(MF_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); \
   } while (0)
 
+// the caller's current device is restored when a call returns
+struct MfDeviceGuard {
+  int prev = -1; cudaError_t err;
+  explicit MfDeviceGuard(int dev) { err = cudaGetDevice(&prev); if (err == cudaSuccess && prev != dev) err = cudaSetDevice(dev); else if (err == cudaSuccess) prev = -1; }
+  ~MfDeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define MF_ON_DEVICE(h) MfDeviceGuard dev_guard_((h)->device); MF_CUDA(dev_guard_.err)
+#define MF_STAGE_RING 256                  // staged launches whose stage times can be summed (mf_stage_ms_sum)
+
 struct mf_vegas {
   mf_config_t cfg;
   MfParams P;
@@ -37,7 +46,12 @@ struct mf_vegas {
   MfDevState* d_state;
   const MfProcOps* ops;               // per-process kernels (one translation unit each)
   uint32_t iteration;                  // iterations finalized so far (= Philox counter word 3)
-  cudaStream_t last_stream;
+  // stream ordering: state_stream = the stream of the last call that touched the integrator state (raw sums, grid, records),
+  // ev_state = recorded behind it; ev_eval = behind the last mf_integrand_eval (which only reads the grid).  Calls on another
+  // stream wait for the event they depend on; host reads synchronise on it.
+  cudaStream_t state_stream;
+  cudaEvent_t ev_state, ev_eval;
+  bool have_state_ev, have_eval_ev;
   cudaEvent_t ev0, ev1, evk0, evk1;   // iteration start/end, fused-kernel start/end
   bool have_k, have_it;                // events recorded (fused kernel / whole iteration)
   // staged path (heavy processes): records of the passing events go through HBM between the stages
@@ -46,8 +60,33 @@ struct mf_vegas {
   bool f32;                            // cfg.precision == 32: |M|^2 stage in fp32 (staged path and eval only)
   MfStageWs ws;
   size_t ws_doubles, ws_regions;       // allocated sizes
-  cudaEvent_t evs[4];                  // front start / |M|^2 start / |M|^2 end / reductions end
+  cudaEvent_t* evs;                    // front start / |M|^2 start / |M|^2 end / reductions end of the LAST staged launch (ring entry)
+  cudaEvent_t ring[MF_STAGE_RING][4];  // one entry per staged launch (slices of a large iteration included)
+  uint32_t ring_next, ring_count;      // next entry, entries recorded since the last mf_stage_ms_sum
+  MfIterRec* h_rec;                    // pinned staging of one iteration record
 };
+
+// ---- stream ordering helpers ----------------------------------------------------------------------------
+static int state_begin(mf_vegas* h, cudaStream_t st) {       // a call that reads or writes the integrator state on st
+  if (h->have_state_ev && st != h->state_stream) MF_CUDA(cudaStreamWaitEvent(st, h->ev_state, 0));
+  return MF_OK;
+}
+static int state_write_begin(mf_vegas* h, cudaStream_t st) { // ... that writes it: evals in flight read the grid
+  int rc = state_begin(h, st);
+  if (rc) return rc;
+  if (h->have_eval_ev) MF_CUDA(cudaStreamWaitEvent(st, h->ev_eval, 0));
+  return MF_OK;
+}
+static int state_end(mf_vegas* h, cudaStream_t st) {
+  MF_CUDA(cudaEventRecord(h->ev_state, st));
+  h->state_stream = st; h->have_state_ev = true;
+  return MF_OK;
+}
+static int state_sync(mf_vegas* h, bool evals_too) {         // host access to the state
+  if (h->have_state_ev) MF_CUDA(cudaEventSynchronize(h->ev_state));
+  if (evals_too && h->have_eval_ev) MF_CUDA(cudaEventSynchronize(h->ev_eval));
+  return MF_OK;
+}
 #define MF_STAGE_MAX_EVENTS (1ull << 24)   // events per staged launch (<= 2.1-2.6 GB of records)
 
 extern "C" int mf_vegas_create(const mf_config_t* cfg, mf_vegas_t** out) {
@@ -69,7 +108,8 @@ extern "C" int mf_vegas_create(const mf_config_t* cfg, mf_vegas_t** out) {
   h->row = h->na + MF_OBS_ACC;
 #define MF_CREATE_CUDA(call)                                                     \
   do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { std::string m_ = std::string(#call) + ": " + cudaGetErrorString(e_); mf_vegas_destroy(h); return fail(MF_ECUDA, m_); } } while (0)
-  MF_CREATE_CUDA(cudaSetDevice(h->device));
+  MfDeviceGuard dev_guard_(h->device);
+  MF_CREATE_CUDA(dev_guard_.err);
   MF_CREATE_CUDA(cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device));
   h->ops = mf_proc_ops(P.process);
   MF_CREATE_CUDA(h->ops->setup(P, &h->smem_iter, &h->smem_eval, &h->occ_iter, &h->occ_eval));
@@ -106,18 +146,27 @@ extern "C" int mf_vegas_create(const mf_config_t* cfg, mf_vegas_t** out) {
   MF_CREATE_CUDA(cudaEventCreate(&h->ev1));
   MF_CREATE_CUDA(cudaEventCreate(&h->evk0));
   MF_CREATE_CUDA(cudaEventCreate(&h->evk1));
-  for (int i = 0; i < 4; ++i) MF_CREATE_CUDA(cudaEventCreate(&h->evs[i]));
+  MF_CREATE_CUDA(cudaEventCreateWithFlags(&h->ev_state, cudaEventDisableTiming));
+  MF_CREATE_CUDA(cudaEventCreateWithFlags(&h->ev_eval, cudaEventDisableTiming));
+  for (int r = 0; r < MF_STAGE_RING; ++r)
+    for (int i = 0; i < 4; ++i) MF_CREATE_CUDA(cudaEventCreate(&h->ring[r][i]));
+  h->evs = h->ring[0];
+  MF_CREATE_CUDA(cudaMallocHost(&h->h_rec, sizeof(MfIterRec)));
   *out = h;
   return MF_OK;
 }
 
 extern "C" int mf_vegas_destroy(mf_vegas_t* h) {
   if (!h) return MF_OK;
-  cudaSetDevice(h->device);
+  MfDeviceGuard dev_guard_(h->device);
   cudaFree(h->d_edges); cudaFree(h->d_pdf); cudaFree(h->d_partial); cudaFree(h->d_pcount);
   cudaFree(h->d_acc); cudaFree(h->d_counts); cudaFree(h->d_state);
   cudaFree(h->ws.rec); cudaFree(h->ws.count); cudaFree(h->d_obs);
-  for (int i = 0; i < 4; ++i) if (h->evs[i]) cudaEventDestroy(h->evs[i]);
+  for (int r = 0; r < MF_STAGE_RING; ++r)
+    for (int i = 0; i < 4; ++i) if (h->ring[r][i]) cudaEventDestroy(h->ring[r][i]);
+  if (h->ev_state) cudaEventDestroy(h->ev_state);
+  if (h->ev_eval) cudaEventDestroy(h->ev_eval);
+  if (h->h_rec) cudaFreeHost(h->h_rec);
   if (h->ev0) cudaEventDestroy(h->ev0);
   if (h->ev1) cudaEventDestroy(h->ev1);
   if (h->evk0) cudaEventDestroy(h->evk0);
@@ -159,13 +208,16 @@ extern "C" int mf_integrand_eval(mf_vegas_t* h, uint32_t iteration, uint64_t fir
   if (n_events == 0) return MF_OK;
   if (!out->weight && !out->x && !out->bins && !out->momenta && !out->me2 && !out->pdf && !out->pass)
     return fail(MF_EINVAL, "no output buffer requested");
-  MF_CUDA(cudaSetDevice(h->device));
+  MF_ON_DEVICE(h);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   MfEvalOutDev o = {out->weight, out->x, out->bins, out->momenta, out->me2, out->pdf, out->pass};
   const bool rec = out->x || out->momenta || out->me2 || out->pdf;
+  int rc = state_begin(h, st);                           // the grid may still be refined on another stream
+  if (rc) return rc;
   MF_CUDA(h->ops->eval(h->P, h->d_edges, h->d_pdf, iteration, first_event, n_events, o, rec, h->f32,
                        grid_for(h, n_events, h->occ_eval), h->smem_eval, st));
-  h->last_stream = st;
+  MF_CUDA(cudaEventRecord(h->ev_eval, st));
+  h->have_eval_ev = true;
   return MF_OK;
 }
 
@@ -209,10 +261,14 @@ extern "C" int mf_vegas_accumulate(mf_vegas_t* h, uint64_t first_event, uint64_t
   if (n_total < 2 || n_events > n_total || first_event > n_total - n_events)
     return fail(MF_EINVAL, "event range outside the iteration");
   if (n_events == 0) return MF_OK;
-  MF_CUDA(cudaSetDevice(h->device));
+  MF_ON_DEVICE(h);
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (int rc0 = state_begin(h, st)) return rc0;
   if (h->use_staged) {
     for (uint64_t done = 0; done < n_events; done += MF_STAGE_MAX_EVENTS) {
+      h->evs = h->ring[h->ring_next];                    // one event set per staged launch
+      h->ring_next = (h->ring_next + 1) % MF_STAGE_RING;
+      if (h->ring_count < MF_STAGE_RING) ++h->ring_count;
       const uint64_t m = n_events - done < MF_STAGE_MAX_EVENTS ? n_events - done : MF_STAGE_MAX_EVENTS;
       int rc = ensure_ws(h, m);
       if (rc) return rc;
@@ -226,8 +282,7 @@ extern "C" int mf_vegas_accumulate(mf_vegas_t* h, uint64_t first_event, uint64_t
       MF_CUDA(cudaGetLastError());
     }
     h->have_stage = true; h->have_k = false;
-    h->last_stream = st;
-    return MF_OK;
+    return state_end(h, st);
   }
   const int grid = grid_for(h, n_events, h->occ_iter);
   MF_CUDA(cudaEventRecord(h->evk0, st));
@@ -241,8 +296,7 @@ extern "C" int mf_vegas_accumulate(mf_vegas_t* h, uint64_t first_event, uint64_t
   h->have_k = true; h->have_stage = false;
   mf_reduce_kernel<<<(live_len(h) + 2 + 7) / 8, MF_REDUCE_THREADS, 0, st>>>(h->d_partial, h->d_pcount, grid, live_len(h), h->row, h->d_acc, h->d_counts);
   MF_CUDA(cudaGetLastError());
-  h->last_stream = st;
-  return MF_OK;
+  return state_end(h, st);
 }
 
 // duration of the dominant kernel of the last accumulate: the fused kernel, or the |M|^2 stage
@@ -253,15 +307,12 @@ static int dominant_ms(mf_vegas* h, float* ms) {
   return MF_OK;
 }
 
-static int fetch_iter(mf_vegas* h, uint32_t idx, mf_iter_t* o) {
-  MfDevState* s = h->d_state;
-  MF_CUDA(cudaMemcpy(&o->integral, &s->it_I[idx], sizeof(double), cudaMemcpyDeviceToHost));
-  MF_CUDA(cudaMemcpy(&o->sigma, &s->it_sig[idx], sizeof(double), cudaMemcpyDeviceToHost));
-  unsigned long long v[3];
-  MF_CUDA(cudaMemcpy(&v[0], &s->it_n[idx], sizeof(v[0]), cudaMemcpyDeviceToHost));
-  MF_CUDA(cudaMemcpy(&v[1], &s->it_pass[idx], sizeof(v[0]), cudaMemcpyDeviceToHost));
-  MF_CUDA(cudaMemcpy(&v[2], &s->it_bad[idx], sizeof(v[0]), cudaMemcpyDeviceToHost));
-  o->n_events = v[0]; o->n_pass = v[1]; o->n_nonfinite = v[2]; o->kernel_ms = 0.0f;
+// one iteration record: a single asynchronous copy on the caller's stream into pinned memory, one synchronisation
+static int fetch_iter(mf_vegas* h, uint32_t idx, cudaStream_t st, mf_iter_t* o) {
+  MF_CUDA(cudaMemcpyAsync(h->h_rec, &h->d_state->it[idx], sizeof(MfIterRec), cudaMemcpyDeviceToHost, st));
+  MF_CUDA(cudaStreamSynchronize(st));
+  o->integral = h->h_rec->I; o->sigma = h->h_rec->sig;
+  o->n_events = h->h_rec->n; o->n_pass = h->h_rec->pass; o->n_nonfinite = h->h_rec->bad; o->kernel_ms = 0.0f;
   return MF_OK;
 }
 
@@ -269,20 +320,19 @@ extern "C" int mf_vegas_finalize(mf_vegas_t* h, uint64_t n_total, void* cuda_str
   if (!h) return fail(MF_EINVAL, "handle is NULL");
   if (n_total < 2) return fail(MF_EINVAL, "an iteration needs at least 2 events");
   if (h->iteration >= MF_MAX_ITER) return fail(MF_ESTATE, "too many iterations (1024)");
-  MF_CUDA(cudaSetDevice(h->device));
+  MF_ON_DEVICE(h);
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc = state_write_begin(h, st);
+  if (rc) return rc;
   mf_finalize_kernel<<<1, 32 * h->P.d, 0, st>>>(h->P, h->cfg.alpha_damp, (double)n_total, n_total, h->d_acc, h->d_counts,
                                         h->d_edges, h->d_state, h->d_obs);
   MF_CUDA(cudaGetLastError());
   // the raw sums stay readable (mf_get_accum) until the next iteration starts
   const uint32_t idx = h->iteration++;
-  h->last_stream = st;
+  if ((rc = state_end(h, st))) return rc;
   if (host_out) {
-    MF_CUDA(cudaStreamSynchronize(st));
-    int rc = fetch_iter(h, idx, host_out);
-    if (rc) return rc;
-    rc = dominant_ms(h, &host_out->kernel_ms);
-    if (rc) return rc;
+    if ((rc = fetch_iter(h, idx, st, host_out))) return rc;
+    if ((rc = dominant_ms(h, &host_out->kernel_ms))) return rc;
   }
   return MF_OK;
 }
@@ -297,23 +347,20 @@ extern "C" int mf_vegas_iterate(mf_vegas_t* h, uint64_t n_events, void* cuda_str
   if (!h) return fail(MF_EINVAL, "handle is NULL");
   if (n_events < 2) return fail(MF_EINVAL, "an iteration needs at least 2 events");
   if (h->iteration >= MF_MAX_ITER) return fail(MF_ESTATE, "too many iterations (1024)");
-  MF_CUDA(cudaSetDevice(h->device));
+  MF_ON_DEVICE(h);
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc = state_write_begin(h, st);
+  if (rc) return rc;
   MF_CUDA(cudaEventRecord(h->ev0, st));
-  int rc = zero_accum(h, st);
-  if (rc) return rc;
-  rc = mf_vegas_accumulate(h, 0, n_events, n_events, cuda_stream);
-  if (rc) return rc;
-  rc = mf_vegas_finalize(h, n_events, cuda_stream, nullptr);
-  if (rc) return rc;
+  if ((rc = zero_accum(h, st))) return rc;
+  if ((rc = state_end(h, st))) return rc;
+  if ((rc = mf_vegas_accumulate(h, 0, n_events, n_events, cuda_stream))) return rc;
+  if ((rc = mf_vegas_finalize(h, n_events, cuda_stream, nullptr))) return rc;
   MF_CUDA(cudaEventRecord(h->ev1, st));
   h->have_it = true;
   if (host_out) {
-    MF_CUDA(cudaStreamSynchronize(st));
-    rc = fetch_iter(h, h->iteration - 1, host_out);
-    if (rc) return rc;
-    rc = dominant_ms(h, &host_out->kernel_ms);
-    if (rc) return rc;
+    if ((rc = fetch_iter(h, h->iteration - 1, st, host_out))) return rc;
+    if ((rc = dominant_ms(h, &host_out->kernel_ms))) return rc;
   }
   return MF_OK;
 }
@@ -324,6 +371,21 @@ extern "C" int mf_last_stage_ms(const mf_vegas_t* h, float* ms3) {
   if (!h->have_stage) return fail(MF_ESTATE, "the last accumulate did not run the staged path");
   MF_CUDA(cudaEventSynchronize(h->evs[3]));
   for (int i = 0; i < 3; ++i) MF_CUDA(cudaEventElapsedTime(&ms3[i], h->evs[i], h->evs[i + 1]));
+  return MF_OK;
+}
+
+extern "C" int mf_stage_ms_sum(mf_vegas_t* h, float* ms3, uint32_t* launches) {
+  if (!h || !ms3 || !launches) return fail(MF_EINVAL, "null argument");
+  ms3[0] = ms3[1] = ms3[2] = 0.0f; *launches = 0;
+  MF_ON_DEVICE(h);
+  const uint32_t n = h->ring_count;
+  for (uint32_t j = 0; j < n; ++j) {
+    cudaEvent_t* e = h->ring[(h->ring_next + MF_STAGE_RING - 1 - j) % MF_STAGE_RING];
+    MF_CUDA(cudaEventSynchronize(e[3]));
+    for (int i = 0; i < 3; ++i) { float t = 0.0f; MF_CUDA(cudaEventElapsedTime(&t, e[i], e[i + 1])); ms3[i] += t; }
+  }
+  *launches = n;
+  h->ring_count = 0;
   return MF_OK;
 }
 
@@ -343,8 +405,8 @@ extern "C" int mf_last_kernel_ms(const mf_vegas_t* h, float* fused_kernel_ms, fl
 
 extern "C" int mf_get_accum(mf_vegas_t* h, double* host_acc, uint64_t* host_counts) {
   if (!h || !host_acc) return fail(MF_EINVAL, "null argument");
-  MF_CUDA(cudaSetDevice(h->device));
-  MF_CUDA(cudaStreamSynchronize(h->last_stream));
+  MF_ON_DEVICE(h);
+  if (int rc = state_sync(h, false)) return rc;
   MF_CUDA(cudaMemcpy(host_acc, h->d_acc, live_len(h) * sizeof(double), cudaMemcpyDeviceToHost));
   if (host_counts) MF_CUDA(cudaMemcpy(host_counts, h->d_counts, 2 * sizeof(uint64_t), cudaMemcpyDeviceToHost));
   return MF_OK;
@@ -352,8 +414,8 @@ extern "C" int mf_get_accum(mf_vegas_t* h, double* host_acc, uint64_t* host_coun
 
 extern "C" int mf_set_accum(mf_vegas_t* h, const double* host_acc, const uint64_t* host_counts) {
   if (!h || !host_acc) return fail(MF_EINVAL, "null argument");
-  MF_CUDA(cudaSetDevice(h->device));
-  MF_CUDA(cudaStreamSynchronize(h->last_stream));
+  MF_ON_DEVICE(h);
+  if (int rc = state_sync(h, false)) return rc;
   MF_CUDA(cudaMemcpy(h->d_acc, host_acc, live_len(h) * sizeof(double), cudaMemcpyHostToDevice));
   if (host_counts) MF_CUDA(cudaMemcpy(h->d_counts, host_counts, 2 * sizeof(uint64_t), cudaMemcpyHostToDevice));
   return MF_OK;
@@ -361,31 +423,34 @@ extern "C" int mf_set_accum(mf_vegas_t* h, const double* host_acc, const uint64_
 
 extern "C" int mf_zero_accum(mf_vegas_t* h, void* cuda_stream) {
   if (!h) return fail(MF_EINVAL, "handle is NULL");
-  MF_CUDA(cudaSetDevice(h->device));
-  h->last_stream = (cudaStream_t)cuda_stream;
-  return zero_accum(h, (cudaStream_t)cuda_stream);
+  MF_ON_DEVICE(h);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc = state_begin(h, st);
+  if (rc) return rc;
+  if ((rc = zero_accum(h, st))) return rc;
+  return state_end(h, st);
 }
 
 extern "C" int mf_get_accum_device(mf_vegas_t* h, double* dev_out, void* cuda_stream) {
   if (!h || !dev_out) return fail(MF_EINVAL, "null argument");
-  MF_CUDA(cudaSetDevice(h->device));
+  MF_ON_DEVICE(h);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int n = live_len(h);
+  if (int rc = state_begin(h, st)) return rc;
   mf_pack_accum_kernel<<<(n + 2 + 255) / 256, 256, 0, st>>>(h->d_acc, h->d_counts, n, dev_out);
   MF_CUDA(cudaGetLastError());
-  h->last_stream = st;
-  return MF_OK;
+  return state_end(h, st);
 }
 
 extern "C" int mf_set_accum_device(mf_vegas_t* h, const double* dev_in, void* cuda_stream) {
   if (!h || !dev_in) return fail(MF_EINVAL, "null argument");
-  MF_CUDA(cudaSetDevice(h->device));
+  MF_ON_DEVICE(h);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int n = live_len(h);
+  if (int rc = state_begin(h, st)) return rc;
   mf_unpack_accum_kernel<<<(n + 2 + 255) / 256, 256, 0, st>>>(dev_in, n, h->d_acc, h->d_counts);
   MF_CUDA(cudaGetLastError());
-  h->last_stream = st;
-  return MF_OK;
+  return state_end(h, st);
 }
 
 extern "C" int mf_set_observables(mf_vegas_t* h, const mf_observable_t* obs, uint32_t n_obs) {
@@ -397,8 +462,8 @@ extern "C" int mf_set_observables(mf_vegas_t* h, const mf_observable_t* obs, uin
     if (obs[o].n_bins < 1 || obs[o].n_bins > 62) return fail(MF_EINVAL, "observable n_bins must be in 1..62");
     if (!(obs[o].hi > obs[o].lo)) return fail(MF_EINVAL, "observable range is empty");
   }
-  MF_CUDA(cudaSetDevice(h->device));
-  MF_CUDA(cudaStreamSynchronize(h->last_stream));
+  MF_ON_DEVICE(h);
+  if (int rc = state_sync(h, true)) return rc;
   h->P.n_obs = (int32_t)n_obs;
   for (uint32_t o = 0; o < n_obs; ++o) {
     h->P.obs_kind[o] = obs[o].kind; h->P.obs_nb[o] = (int32_t)obs[o].n_bins; h->P.obs_lo[o] = obs[o].lo; h->P.obs_hi[o] = obs[o].hi;
@@ -411,8 +476,8 @@ extern "C" int mf_set_observables(mf_vegas_t* h, const mf_observable_t* obs, uin
 extern "C" int mf_get_observables(mf_vegas_t* h, double* host_sum, double* host_sum2, uint32_t* n_iter) {
   if (!h || !host_sum || !host_sum2) return fail(MF_EINVAL, "null argument");
   if (h->P.n_obs == 0) return fail(MF_ESTATE, "no observables set");
-  MF_CUDA(cudaSetDevice(h->device));
-  MF_CUDA(cudaStreamSynchronize(h->last_stream));
+  MF_ON_DEVICE(h);
+  if (int rc = state_sync(h, false)) return rc;
   const size_t n = (size_t)h->P.n_obs * MF_OBS_SLOTS;
   MF_CUDA(cudaMemcpy(host_sum, h->d_obs, n * sizeof(double), cudaMemcpyDeviceToHost));
   MF_CUDA(cudaMemcpy(host_sum2, h->d_obs + MF_OBS_ACC / 2, n * sizeof(double), cudaMemcpyDeviceToHost));
@@ -431,10 +496,11 @@ extern "C" int mf_accum_len(const mf_vegas_t* h, uint32_t* n) {
 extern "C" int mf_result(mf_vegas_t* h, mf_result_t* host_out) {
   if (!h || !host_out) return fail(MF_EINVAL, "null argument");
   if (h->iteration == 0) return fail(MF_ESTATE, "no iteration has been run");
-  MF_CUDA(cudaSetDevice(h->device));
-  mf_combine_kernel<<<1, 32, 0, h->last_stream>>>(h->d_state);
+  MF_ON_DEVICE(h);
+  mf_combine_kernel<<<1, 32, 0, h->state_stream>>>(h->d_state);      // ordered behind the last finalize on its own stream
   MF_CUDA(cudaGetLastError());
-  MF_CUDA(cudaStreamSynchronize(h->last_stream));
+  if (int rc = state_end(h, h->state_stream)) return rc;
+  MF_CUDA(cudaStreamSynchronize(h->state_stream));
   double r[3];
   MF_CUDA(cudaMemcpy(r, &h->d_state->res_I, 3 * sizeof(double), cudaMemcpyDeviceToHost));
   host_out->integral = r[0]; host_out->sigma = r[1]; host_out->chi2_dof = r[2]; host_out->n_iter = h->iteration;
@@ -443,18 +509,23 @@ extern "C" int mf_result(mf_vegas_t* h, mf_result_t* host_out) {
 
 extern "C" int mf_get_iterations(mf_vegas_t* h, mf_iter_t* host_out, uint32_t max_iter, uint32_t* n_iter) {
   if (!h || !host_out || !n_iter) return fail(MF_EINVAL, "null argument");
-  MF_CUDA(cudaSetDevice(h->device));
-  MF_CUDA(cudaStreamSynchronize(h->last_stream));
+  MF_ON_DEVICE(h);
+  if (int rc = state_sync(h, false)) return rc;
   uint32_t n = h->iteration < max_iter ? h->iteration : max_iter;
-  for (uint32_t i = 0; i < n; ++i) { int rc = fetch_iter(h, i, &host_out[i]); if (rc) return rc; }
+  std::vector<MfIterRec> recs(n);
+  if (n) MF_CUDA(cudaMemcpy(recs.data(), h->d_state->it, n * sizeof(MfIterRec), cudaMemcpyDeviceToHost));
+  for (uint32_t i = 0; i < n; ++i) {
+    host_out[i].integral = recs[i].I; host_out[i].sigma = recs[i].sig; host_out[i].n_events = recs[i].n;
+    host_out[i].n_pass = recs[i].pass; host_out[i].n_nonfinite = recs[i].bad; host_out[i].kernel_ms = 0.0f;
+  }
   *n_iter = n;
   return MF_OK;
 }
 
 extern "C" int mf_get_grid(mf_vegas_t* h, double* host_edges) {
   if (!h || !host_edges) return fail(MF_EINVAL, "null argument");
-  MF_CUDA(cudaSetDevice(h->device));
-  MF_CUDA(cudaStreamSynchronize(h->last_stream));
+  MF_ON_DEVICE(h);
+  if (int rc = state_sync(h, false)) return rc;
   MF_CUDA(cudaMemcpy(host_edges, h->d_edges, (size_t)h->P.d * (h->P.nb + 1) * sizeof(double), cudaMemcpyDeviceToHost));
   return MF_OK;
 }
@@ -467,8 +538,8 @@ extern "C" int mf_set_grid(mf_vegas_t* h, const double* e) {
     if (r[0] != 0.0 || r[nb] != 1.0) return fail(MF_EINVAL, "edges must start at 0 and end at 1");
     for (int k = 0; k < nb; ++k) if (!(r[k + 1] > r[k])) return fail(MF_EINVAL, "edges not increasing");
   }
-  MF_CUDA(cudaSetDevice(h->device));
-  MF_CUDA(cudaStreamSynchronize(h->last_stream));
+  MF_ON_DEVICE(h);
+  if (int rc = state_sync(h, true)) return rc;           // refinements and evaluations in flight use the old grid
   MF_CUDA(cudaMemcpy(h->d_edges, e, (size_t)h->P.d * (nb + 1) * sizeof(double), cudaMemcpyHostToDevice));
   return MF_OK;
 }
@@ -488,35 +559,53 @@ extern "C" int mf_me_flops(const mf_vegas_t* h, uint64_t* n_add, uint64_t* n_mul
   return MF_OK;
 }
 
+extern "C" int mf_me_flops_bounds(const mf_vegas_t* h, uint64_t* flops_min, uint64_t* flops_executed) {
+  if (!h) return fail(MF_EINVAL, "handle is NULL");
+  uint64_t a, m, f;
+  int rc = mf_me_flops(h, &a, &m, &f);
+  if (rc) return rc;
+  uint64_t lo = a + m + 2 * f, ex = lo;
+  if (h->P.process == MF_GG_TTG) lo = MF_ME2_GG_TTG_NFLOPS_MIN;
+  if (h->P.process == MF_GG_TTGG) {
+    lo = MF_ME2_GG_TTGG_NFLOPS_MIN;
+    ex = 4ull * (MF_ME2_GG_TTGG_LANES_NADD + MF_ME2_GG_TTGG_LANES_NMUL + 2ull * MF_ME2_GG_TTGG_LANES_NFMA);
+  }
+  if (flops_min) *flops_min = lo;
+  if (flops_executed) *flops_executed = ex;
+  return MF_OK;
+}
+
 extern "C" int mf_fp64_peak(int32_t device, double seconds, double* host_flops_per_s) {
   if (!host_flops_per_s || !(seconds > 0.0)) return fail(MF_EINVAL, "bad argument");
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return fail(MF_ECUDA, "no such CUDA device");
-  MF_CUDA(cudaSetDevice(device));
+  MfDeviceGuard dev_guard_(device);
+  MF_CUDA(dev_guard_.err);
   int n_sm = 0;
   MF_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device));
   const int grid = n_sm * 4, threads = 256, iters = 4096;
-  double* d_out = nullptr;
-  MF_CUDA(cudaMalloc(&d_out, (size_t)grid * threads * sizeof(double)));
-  cudaEvent_t a, b;
-  MF_CUDA(cudaEventCreate(&a)); MF_CUDA(cudaEventCreate(&b));
-  mf_dfma_kernel<<<grid, threads>>>(d_out, iters, 0.999999, 1e-6);          // warm-up
+  struct Res {                                            // released on every return path
+    double* d_out = nullptr; cudaEvent_t a = nullptr, b = nullptr;
+    ~Res() { if (a) cudaEventDestroy(a); if (b) cudaEventDestroy(b); if (d_out) cudaFree(d_out); }
+  } r;
+  MF_CUDA(cudaMalloc(&r.d_out, (size_t)grid * threads * sizeof(double)));
+  MF_CUDA(cudaEventCreate(&r.a)); MF_CUDA(cudaEventCreate(&r.b));
+  mf_dfma_kernel<<<grid, threads>>>(r.d_out, iters, 0.999999, 1e-6);          // warm-up
   MF_CUDA(cudaDeviceSynchronize());
   const double flops_per_launch = 2.0 * MF_DFMA_PER_ITER * (double)iters * grid * threads;
   double best = 0.0, spent = 0.0;
   int reps = 0;
   while (spent < seconds * 1e3 && reps < 10000) {
-    MF_CUDA(cudaEventRecord(a));
-    mf_dfma_kernel<<<grid, threads>>>(d_out, iters, 0.999999, 1e-6);
-    MF_CUDA(cudaEventRecord(b));
-    MF_CUDA(cudaEventSynchronize(b));
+    MF_CUDA(cudaEventRecord(r.a));
+    mf_dfma_kernel<<<grid, threads>>>(r.d_out, iters, 0.999999, 1e-6);
+    MF_CUDA(cudaEventRecord(r.b));
+    MF_CUDA(cudaEventSynchronize(r.b));
     float ms = 0.0f;
-    MF_CUDA(cudaEventElapsedTime(&ms, a, b));
+    MF_CUDA(cudaEventElapsedTime(&ms, r.a, r.b));
     spent += ms; ++reps;
     const double f = flops_per_launch / (ms * 1e-3);
     if (f > best) best = f;
   }
-  cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(d_out);
   *host_flops_per_s = best;
   return MF_OK;
 }

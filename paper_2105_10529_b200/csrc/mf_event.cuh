@@ -8,10 +8,7 @@
 #include "mf_device.cuh"
 #include "generated/mf_me2_ee_mumu.cuh"
 #include "generated/mf_me2_gg_tt.cuh"
-#ifndef MF_GEN_TTG            // tuning builds point this at an alternative generated file
-#define MF_GEN_TTG "generated/mf_me2_gg_ttg.cuh"
-#endif
-#include MF_GEN_TTG
+#include "generated/mf_me2_gg_ttg.cuh"
 #include "generated/mf_me2_gg_ttgg_lanes.cuh"     // gg -> tt~gg: one event over four lanes (gen/lanes.py)
 
 template <int PROC> struct MfProc;

@@ -35,9 +35,9 @@ struct MfEvalOutDev {
 };
 
 // device-resident integrator state that the kernels update
+struct MfIterRec { double I, sig; unsigned long long n, pass, bad; };     // one iteration (read back with one copy)
 struct MfDevState {
-  double it_I[MF_MAX_ITER], it_sig[MF_MAX_ITER];
-  unsigned long long it_n[MF_MAX_ITER], it_pass[MF_MAX_ITER], it_bad[MF_MAX_ITER];
+  MfIterRec it[MF_MAX_ITER];
   unsigned int n_iter;
   double res_I, res_sig, res_chi2;
 };

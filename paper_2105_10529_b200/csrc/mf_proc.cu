@@ -19,7 +19,7 @@ __device__ __forceinline__ void mf_stage_tables(const MfParams& P, const double*
 // ---- S9: per-warp histogram update in fixed order -------------------------------------------------------
 // H[j][bin_j] += t2 for every contributing lane of the warp, lanes that share a bin served in lane order
 // (so the sum order is fixed: reading A22).  The peer masks come from six ballots per dimension (one per
-// key bit) instead of match.any, whose latency (~800 cycles under load, profiles/r1_v3_staged_ncu.md)
+// key bit) instead of match.any, whose latency (~800 cycles under load, profiles/r1_tuning.md)
 // dominated the reduction stage; the ranks of all dimensions are resolved first so that each round
 // issues D independent shared-memory updates.
 template <int D>
@@ -278,7 +278,7 @@ mf_iterate_compact_kernel(const MfParams P, const double* __restrict__ g_edges, 
 // ---- staged iteration for the heavy processes: front end -> |M|^2 -> reductions, through HBM --------
 // The fused kernels above run the front end (S1-S6) at the occupancy of the |M|^2 code (255 registers,
 // 2 warps per scheduler), where it is latency-bound: 21 % of the fused kernel's time for 12 % of its
-// FP64 instructions (profiles/r1_v2_iterate_ttg_ncu.md).  The staged path gives every stage its own
+// FP64 instructions (profiles/r1_tuning.md).  The staged path gives every stage its own
 // launch shape and passes 4N+3 doubles per PASSING event through HBM (1.0 GB written + 1.0 GB read per
 // 1e7 events, ~0.3 ms at the measured 6.5 TB/s):
 //   mf_front_kernel  one CTA per REGION of `cap` consecutive events: S1-S6 and the weight prefactor,

@@ -50,8 +50,8 @@ __global__ void mf_finalize_kernel(const MfParams P, double alpha, double n_tota
     var = var > 0.0 ? var : 0.0;
     const unsigned k = st->n_iter;
     if (k < MF_MAX_ITER) {
-      st->it_I[k] = I; st->it_sig[k] = sqrt(var);
-      st->it_n[k] = n_events; st->it_pass[k] = counts[0]; st->it_bad[k] = counts[1];
+      st->it[k].I = I; st->it[k].sig = sqrt(var);
+      st->it[k].n = n_events; st->it[k].pass = counts[0]; st->it[k].bad = counts[1];
       st->n_iter = k + 1;
     }
   }
@@ -114,18 +114,18 @@ __global__ void mf_combine_kernel(MfDevState* __restrict__ st) {
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   const unsigned n = st->n_iter;
   bool any_zero = false;
-  for (unsigned j = 0; j < n; ++j) if (!(st->it_sig[j] > 0.0)) any_zero = true;
+  for (unsigned j = 0; j < n; ++j) if (!(st->it[j].sig > 0.0)) any_zero = true;
   double I = 0.0, sig = 0.0, chi2 = 0.0;
   if (n > 0 && any_zero) {                                // fall back to the plain mean
     double m = 0.0, v = 0.0;
-    for (unsigned j = 0; j < n; ++j) { m += st->it_I[j]; v += st->it_sig[j] * st->it_sig[j]; }
+    for (unsigned j = 0; j < n; ++j) { m += st->it[j].I; v += st->it[j].sig * st->it[j].sig; }
     I = m / n; sig = sqrt(v) / n;
   } else if (n > 0) {
     double sw = 0.0, swi = 0.0;
-    for (unsigned j = 0; j < n; ++j) { const double w = 1.0 / (st->it_sig[j] * st->it_sig[j]); sw += w; swi += w * st->it_I[j]; }
+    for (unsigned j = 0; j < n; ++j) { const double w = 1.0 / (st->it[j].sig * st->it[j].sig); sw += w; swi += w * st->it[j].I; }
     I = swi / sw; sig = 1.0 / sqrt(sw);
     if (n > 1) {
-      for (unsigned j = 0; j < n; ++j) { const double dl = st->it_I[j] - I; chi2 += dl * dl / (st->it_sig[j] * st->it_sig[j]); }
+      for (unsigned j = 0; j < n; ++j) { const double dl = st->it[j].I - I; chi2 += dl * dl / (st->it[j].sig * st->it[j].sig); }
       chi2 /= (double)(n - 1);
     }
   }

@@ -21,7 +21,6 @@ derivation is written out in DESIGN.md.  The parity relation |M(-lambda)|^2 = |M
 """
 import itertools
 import math
-import os
 import numpy as np
 from .dag import Dag, R, Cx, csum_prod
 
@@ -509,32 +508,24 @@ def evaluate(gen, inputs):
     return total
 
 
-def _legs(env, default):
-    v = os.environ.get(env)
-    return default if v is None else tuple(int(x) for x in v.split(",") if x != "")
-
-
-BASIS = os.environ.get("MF_GEN_BASIS", "linear")
+# Organisation of the emitted code per process (tuned on the B200, profiles/r1_tuning.md): polarisation basis, the gluon
+# legs whose polarisation is a run-time loop, parity; gg -> tt~gg is emitted by gen/lanes.py (one event over four lanes)
 PROCESSES = {
     "mf_me2_ee_mumu": lambda: GenEE(),
     "mf_me2_gg_tt": lambda: Gen(2, loop_legs=(), parity=True, basis="circular"),      # 514 flops (linear: 715)
-    "mf_me2_gg_ttg": lambda: Gen(3, loop_legs=_legs("MF_GEN_TTG_LOOP", (0, 2)), parity=True,
-                                 loop_lam4=os.environ.get("MF_GEN_TTG_LAM4", "0") == "1", basis=BASIS),
+    "mf_me2_gg_ttg": lambda: Gen(3, loop_legs=(0, 2), parity=True, basis="linear"),
 }
 
-
 # loop-invariant values with a cone of at most this many operations are recomputed in the loop body
-# (Dag.demote_cheap); tuned on B200, see DESIGN.md "Kernels / S7"
-DEMOTE = {"mf_me2_gg_ttg": int(os.environ.get("MF_GEN_DEMOTE_TTG", "6")),
-          "mf_me2_gg_ttgg": int(os.environ.get("MF_GEN_DEMOTE_TTGG", "0"))}
+# (Dag.plan); tuned on B200, see DESIGN.md "Kernels / S7"
+DEMOTE = {"mf_me2_gg_ttg": 6}
 
-
-# barrier-point macro of the generated code (csrc/mf_device.cuh): 128-thread groups, or the whole CTA
-SYNC_MACRO = {}      # (gg -> tt~gg used MF_SYNC_POINT_W, the whole CTA, until its loop ran over all four gluons: profiles/r1_tuning.md)
+# barrier-point macro of the generated code (csrc/mf_device.cuh): 128-thread groups (default), or the whole CTA
+SYNC_MACRO = {}
 
 # emission order of the helicity-loop body (Dag.schedule): window 0 = creation order
-SCHED_WINDOW = int(os.environ.get("MF_GEN_SCHED_WINDOW", "48"))
-SCHED_DISTANCE = int(os.environ.get("MF_GEN_SCHED_DISTANCE", "5"))
+SCHED_WINDOW = 48
+SCHED_DISTANCE = 5
 
 
 def generate(fname):

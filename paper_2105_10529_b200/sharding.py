@@ -33,7 +33,10 @@ def sharded_iterate_device(h, n_total, rank, world, dist=None, device=None, sync
     first, n = shard_range(n_total, rank, world)
     h.zero_accum()
     h.vegas_accumulate(first, n, n_total)
-    buf = torch.empty(h.accum_len() + 2, dtype=torch.float64, device=device)
+    m = h.accum_len() + 2
+    buf = getattr(h, "_exchange_buf", None)                  # one exchange buffer per handle, reused every iteration
+    if buf is None or buf.numel() != m or buf.device != torch.device(device if device is not None else "cuda"):
+        buf = h._exchange_buf = torch.empty(m, dtype=torch.float64, device=device)
     h.get_accum_device(buf.data_ptr())
     if dist is not None and dist.is_initialized():
         dist.all_reduce(buf, op=dist.ReduceOp.SUM)         # ordered after the pack kernel on the current stream

@@ -213,9 +213,10 @@ def test_observable_histograms_match_oracle(mf, mfo, proc, n):
     assert abs(got[0][0].sum() / tot - 1) < 1e-12            # every weighted event lands in exactly one slot
     gpu.set_observables([])                                   # off again: plain record length
     assert gpu.accum_len() == 2 + gpu.d * gpu.n_bins
-    if proc >= 2:                                             # heavy processes: staged path only
-        gpu.set_observables(obs); gpu.set_path(False)
+    if proc >= 2:                                             # heavy processes: observables on the staged path only
+        gpu.set_observables(obs)
         with pytest.raises(mf.MfError) as e:
+            gpu.set_path(False)                               # (gg -> tt~gg has no fused path at all)
             gpu.vegas_iterate(1000)
         assert e.value.code == mf.MF_EUNSUPPORTED
 
@@ -565,3 +566,76 @@ def test_fp32_matrix_element_with_generator_variants(mf):
         nz = wa["weight"] != 0
         rel = (wb["weight"][nz] / wa["weight"][nz] - 1).abs()
         assert float(rel.median()) < 1e-5 and float((rel > 1e-4).double().mean()) < 5e-3      # north_star: 1e-4 for the fp32 path
+
+
+# ---- config 3 (gg -> tt~gg, one event over four lanes in the |M|^2 stage) at sizes that reach the full-size code path ------
+def test_config3_large_iteration_against_oracle(mf, mfo):
+    """a 1e5-event iteration of gg -> tt~gg on the staged path (several hundred record regions, prefix + binary search over the
+    region counts, 4-lane |M|^2 stage) on a random adapted grid, every event through the oracle: raw sums, all 10 x 50 histogram
+    bins, pass counter, refined grid (about a minute of oracle time on 16 host cores)"""
+    n = 100_000 if mfo.max_threads() >= 8 else 20_000
+    cfg = W.config(W.GG_TTGG, seed=0)
+    gpu, orc = mf.Vegas(cfg), mfo.Vegas(cfg)
+    e = random_grid(orc.d, 50, 77)
+    gpu.set_grid(e); orc.set_grid(e)
+    g = gpu.vegas_iterate(n)
+    o = orc.iterate(n, n_threads=mfo.max_threads())
+    assert g["n_pass"] == o["n_pass"] and g["n_nonfinite"] == 0 == o["n_nonfinite"] and g["n_events"] == n
+    assert abs(g["integral"] / o["integral"] - 1) < RTOL_INT and abs(g["sigma"] / o["sigma"] - 1) < 1e-8
+    acc = gpu.get_accum()[0]
+    assert acc.shape == (2 + 10 * 50,)
+    np.testing.assert_allclose(acc, orc.get_accum(), rtol=RTOL_INT, atol=1e-300)
+    np.testing.assert_allclose(gpu.get_grid(), orc.get_grid(), rtol=0, atol=1e-11)
+
+
+def test_config3_full_index_range_per_event(mf, mfo):
+    """1e4 events of the 1e6-event config-3 iteration, in 20 chunks of 500 spread over the whole index range (and a second
+    iteration counter), event by event against the oracle: bins, cut flags, points, momenta, PDFs, |M|^2, weights"""
+    cfg = W.config(W.GG_TTGG, seed=0)
+    gpu, orc = mf.Vegas(cfg), mfo.Vegas(cfg)
+    n = W.CONFIGS[3]["n_events"]
+    for j in range(20):
+        first = j * (n // 20) + 37 * j
+        it = 0 if j % 2 == 0 else 4
+        ref = orc.eval(it, first, 500, n_threads=mfo.max_threads())
+        compare_events(gpu.integrand_eval(it, first, 500, debug=True), ref, 3)
+
+
+def test_streams_and_stage_time_sums(mf):
+    """calls under a non-default torch stream (the binding passes the current stream of the handle's device); two streams
+    without host synchronisation in between (the library orders a call behind the last writer of the integrator state);
+    stage times summed over every slice of a sliced iteration; flop bounds"""
+    import torch
+    from paper_2105_10529_b200 import sharding
+    cfg = W.config(W.GG_TTG, seed=12)
+    n = 200_003
+    a, b, c = mf.Vegas(cfg), mf.Vegas(cfg), mf.Vegas(cfg)
+    ia = [a.vegas_iterate(n) for _ in range(2)]
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    with torch.cuda.stream(s1):
+        ib = [b.vegas_iterate(n) for _ in range(2)]
+        ic = [sharding.sharded_iterate_device(c, n, 0, 1, None, torch.device("cuda", 0)) for _ in range(2)]
+    for x, y, z in zip(ia, ib, ic):
+        assert x == y or {k: x[k] for k in x if k != "kernel_ms"} == {k: y[k] for k in y if k != "kernel_ms"}
+        assert x["integral"] == z["integral"] and x["n_pass"] == z["n_pass"]
+    np.testing.assert_array_equal(a.get_grid(), b.get_grid())
+    np.testing.assert_array_equal(a.get_grid(), c.get_grid())
+    # iterate on s1 (enqueue only), evaluate on s2 at once: the evaluation must see the refined grid
+    ref = a.vegas_iterate(n) and a.integrand_eval(0, 0, 4096)["weight"].clone()
+    with torch.cuda.stream(s1):
+        b.vegas_iterate(n, sync=False)
+    with torch.cuda.stream(s2):
+        w = b.integrand_eval(0, 0, 4096)["weight"]
+    s2.synchronize()
+    assert torch.equal(w, ref)
+    assert b.result()["n_iter"] == 3 and b.result()["integral"] == a.result()["integral"]
+    # stage times: one entry per staged launch; an iteration of more than 2^24 events runs as two slices
+    a.stage_ms_sum()
+    a.vegas_iterate((1 << 24) + 1000)
+    sums, launches = a.stage_ms_sum()
+    assert launches == 2 and sums["front"] > 0 and sums["me"] > sums["front"] and sums["reduce"] > 0
+    assert a.stage_ms_sum()[1] == 0
+    fb = a.me_flops_bounds()
+    assert fb["min"] == 11302 and fb["executed"] == a.me_flops()["flops"] == 15023
+    fb = mf.Vegas(W.config(W.GG_TTGG)).me_flops_bounds()
+    assert fb["min"] == 170880 < 256020 < fb["executed"]

@@ -260,6 +260,67 @@ def test_lorentz_bose_parity(mfo):
             assert np.isclose(mfo.jamps(proc, mom, hel)[1], mfo.jamps(proc, mom, -hel)[1], rtol=1e-11)
 
 
+# ---------------------------------------------------------------- P24 collinear factorisation: absolute normalisation
+# Ward, Lorentz, Bose and the A = B comparison are blind to a common normalisation or convention slip (coupling powers,
+# 1/256, colour matrix).  The collinear limits are not: they tie |M(gg -> tt~g)|^2 to the closed form of gg -> tt~ and
+# |M(gg -> tt~gg)|^2 to |M(gg -> tt~g)|^2 through the unregularised Altarelli-Parisi function (textbook; azimuth averaged)
+#   P_gg(z) = 2 C_A [ z/(1-z) + (1-z)/z + z(1-z) ],  C_A = 3:
+#   final state   k3 || k4:  |M_{n+1}|^2 -> (2 g_s^2 / s_34) P_gg(z) |M_n|^2,          z = E_3 / (E_3 + E_4)
+#   initial state k || p_a:  |M_{n+1}|^2 -> (2 g_s^2 / (2 p_a.k)) P_gg(x)/x |M_n(x p_a, p_b)|^2,   x = (p_a + p_b - k)^2 / shat
+# (both sides averaged over the incoming gluons' spins and colours, summed over the final ones, no symmetry factor).
+def p_gg(z):
+    return 2 * 3.0 * (z / (1 - z) + (1 - z) / z + z * (1 - z))
+
+
+def boost_from_rest(p, K):
+    """p given in the rest frame of K -> the frame in which K is given"""
+    M = math.sqrt(mdot(K, K)); E = (K[0] * p[0] + K[1:] @ p[1:]) / M
+    return np.array([E, *(p[1:] + K[1:] * (p[0] + E) / (K[0] + M))])
+
+
+@pytest.mark.parametrize("rts,x,cts,phis", [(900.0, 0.7, 0.3, 1.1), (2500.0, 0.45, -0.6, 4.0)])
+def test_initial_state_collinear_limit_ties_ttg_to_closed_form_tt(mfo, rts, x, cts, phis):
+    E = rts / 2
+    pa, pb = np.array([E, 0, 0, E]), np.array([E, 0, 0, -E])
+    dev = {}
+    for theta in (1e-2, 1e-3):
+        acc = 0.0
+        for j in range(8):                                        # azimuth average: kills the cos(2 phi) spin correlation
+            phi = 0.37 + 2 * math.pi * j / 8
+            k = (1 - x) * E * np.array([1, math.sin(theta) * math.cos(phi), math.sin(theta) * math.sin(phi), math.cos(theta)])
+            K = pa + pb - k
+            M = math.sqrt(mdot(K, K))
+            b = tt_momenta(M, cts, phis)                           # t t~ in the rest frame of K, same angles as the Born point
+            mom = np.array([pa, pb, boost_from_rest(b[2], K), boost_from_rest(b[3], K), k])
+            xx = M * M / rts ** 2
+            born = gg_tt_closed_form(b)                            # the CLOSED FORM, not the oracle
+            acc += mfo.me2(W.GG_TTG, mom) / (2 * GS2 / (2 * mdot(pa, k)) * p_gg(xx) / xx * born)
+        dev[theta] = acc / 8 - 1
+    assert abs(dev[1e-3]) < 2e-6 and abs(dev[1e-2]) < 1e-4, dev   # approached like theta^2
+
+
+@pytest.mark.parametrize("rts,rs,ctd", [(900.0, [0.31, 0.62, 0.44, 0.83, 0.27], 0.2), (3000.0, [0.7, 0.2, 0.9, 0.55, 0.4], -0.5)])
+def test_final_state_collinear_limit_ties_ttgg_to_ttg(mfo, rts, rs, ctd):
+    E = rts / 2
+    beams = [[E, 0, 0, E], [E, 0, 0, -E]]
+    born = mfo.me2(W.GG_TTG, np.vstack([beams, mfo.phase_space(3, rts * rts, [MT, MT, 0.0], rs)["k"]]))
+    dev = {}
+    for m34 in (5.0, 0.5):                                         # the gluon pair as a particle of small mass m34
+        ks = mfo.phase_space(3, rts * rts, [MT, MT, m34], rs)["k"]
+        K = ks[2]
+        n = K[1:] / np.linalg.norm(K[1:]); a = np.cross(n, [0.3, -0.5, 0.8]); a /= np.linalg.norm(a); b = np.cross(n, a)
+        acc = 0.0
+        for j in range(8):
+            phid = 0.11 + 2 * math.pi * j / 8
+            d = math.sqrt(1 - ctd * ctd) * (math.cos(phid) * a + math.sin(phid) * b) + ctd * n
+            k3 = boost_from_rest(np.array([m34 / 2, *(m34 / 2 * d)]), K)
+            k4 = boost_from_rest(np.array([m34 / 2, *(-m34 / 2 * d)]), K)
+            mom = np.vstack([beams, ks[:2], k3, k4])
+            acc += mfo.me2(W.GG_TTGG, mom) / (2 * GS2 / m34 ** 2 * p_gg(k3[0] / K[0]) * born)
+        dev[m34] = acc / 8 - 1
+    assert abs(dev[0.5]) < 1e-4 and abs(dev[5.0]) < 1e-2, dev      # approached like m34^2 / shat
+
+
 # ---------------------------------------------------------------- P26-P28 weight chain and reductions
 @pytest.mark.parametrize("proc", [W.EE_MUMU, W.GG_TT, W.GG_TTG])
 def test_weight_chain_and_reductions(mfo, proc):

@@ -98,3 +98,50 @@ def test_two_rank_iteration_matches_single_process(mfo, device_form):
             assert abs(I / r["integral"] - 1) < 1e-12 and abs(s / r["sigma"] - 1) < 1e-9 and npass == r["n_pass"]
         np.testing.assert_allclose(grid, single.get_grid(), rtol=0, atol=1e-13)
     np.testing.assert_array_equal(got[0][2], got[1][2])      # every rank holds the same grid, bit for bit
+
+
+# ---- bench.py's rank logic (the part in front of the first CUDA call) with world size 2 under gloo ------------------
+def _bench_worker(rank, world, port, q):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world))
+    import bench
+    r, lr, w, d = bench.init_ranks("gloo")
+    slow = bench.max_over_ranks(d, 10.0 + r)                     # the timing rule: max over ranks
+    h = OracleHandle(W.config(W.GG_TT, seed=3))
+    it = sharding.sharded_iterate_device(h, 4001, r, w, d, torch.device("cpu"))   # bench.py's step() at N > 1
+    buf_id = id(h._exchange_buf)
+    sharding.sharded_iterate_device(h, 4001, r, w, d, torch.device("cpu"))
+    q.put((r, lr, w, d is not None, slow, it["integral"], buf_id == id(h._exchange_buf)))
+    d.barrier()
+    d.destroy_process_group()
+
+
+def test_bench_rank_logic_world_size_2(mfo, monkeypatch):
+    import bench
+    port = 31500 + os.getpid() % 2000
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_bench_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = sorted([q.get(timeout=300) for _ in procs])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    ref = mfo.Vegas(W.config(W.GG_TT, seed=3)).iterate(4001, n_threads=2)
+    for r, (rank, local_rank, world, grouped, slow, integral, reused) in enumerate(got):
+        assert (rank, local_rank, world, grouped) == (r, r, 2, True) and slow == 11.0 and reused   # one exchange buffer per handle
+        assert abs(integral / ref["integral"] - 1) < 1e-12
+    # without torchrun, `bench.py --gpus 2` starts the two ranks itself; inside torchrun (WORLD_SIZE set) it does not
+    calls = []
+    monkeypatch.setattr(os, "execvp", lambda exe, argv: calls.append(argv))
+    monkeypatch.delenv("WORLD_SIZE", raising=False)
+    args = type("A", (), {"gpus": 2})()
+    bench.launch_ranks_if_needed(args, ["--gpus", "2", "--steps", "3"])
+    assert len(calls) == 1 and calls[0][1:4] == ["-m", "torch.distributed.run", "--nnodes=1"]
+    assert calls[0][calls[0].index("--nproc-per-node") + 1] == "2" and calls[0][-4:] == ["--gpus", "2", "--steps", "3"]
+    assert "127.0.0.1" in calls[0] and os.path.basename(calls[0][calls[0].index("--master-port") + 2]) == "bench.py"
+    monkeypatch.setenv("WORLD_SIZE", "2")
+    bench.launch_ranks_if_needed(args, ["--gpus", "2"])
+    assert len(calls) == 1
+    monkeypatch.delenv("WORLD_SIZE")
+    assert bench.init_ranks("gloo") == (0, 0, 1, None)           # plain N = 1: no process group

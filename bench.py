@@ -350,8 +350,9 @@ def run_processes(args):
     torch.cuda.set_device(0)
     peak = binding.fp64_peak(0, 0.3) / 1e12
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    sizes = {W.EE_MUMU: 100_000, W.GG_TT: 1_000_000, W.GG_TTG: 10_000_000, W.GG_TTGG: 1_000_000, W.QQ_TT: 1_000_000, W.PP_TT: 1_000_000}
-    cases = [(W.EE_MUMU, 0), (W.GG_TT, 0), (W.GG_TT, 1), (W.GG_TT, 2), (W.QQ_TT, 0), (W.QQ_TT, 1), (W.PP_TT, 0),
+    sizes = {W.EE_MUMU: 100_000, W.GG_TT: 1_000_000, W.GG_TTG: 10_000_000, W.GG_TTGG: 1_000_000, W.QQ_TT: 1_000_000, W.PP_TT: 1_000_000,
+             W.QQ_TTG: 1_000_000, W.QG_TTQ: 1_000_000}
+    cases = [(W.EE_MUMU, 0), (W.GG_TT, 0), (W.GG_TT, 1), (W.GG_TT, 2), (W.QQ_TT, 0), (W.QQ_TT, 1), (W.PP_TT, 0), (W.QQ_TTG, 0), (W.QG_TTQ, 0),
              (W.GG_TTG, 0), (W.GG_TTG, 1), (W.GG_TTG, 2), (W.GG_TTG, 3), (W.GG_TTGG, 0), (W.GG_TTGG, 1)]
     if args.only:
         cases = [c for c in cases if W.PROCESS_NAMES[c[0]] in args.only.split(",")]
@@ -397,7 +398,7 @@ def main():
     ap.add_argument("--sweep", action="store_true", help="configs[4]: events-per-launch sweep of the gg->tt~g integrand (1 GPU)")
     ap.add_argument("--sharded", action="store_true", help="run the multi-GPU code path (device-side all-reduce of the raw sums) even at N = 1")
     ap.add_argument("--processes", action="store_true", help="every process / generator selection at its config size (1 GPU)")
-    ap.add_argument("--only", default="", help="with --processes: comma-separated process names (ee_mumu, gg_tt, qq_tt, pp_tt, gg_ttg, gg_ttgg)")
+    ap.add_argument("--only", default="", help="with --processes: comma-separated process names (ee_mumu, gg_tt, qq_tt, pp_tt, qq_ttg, qg_ttq, gg_ttg, gg_ttgg)")
     ap.add_argument("--path", default="staged", choices=["staged", "fused"],
                     help="staged: front end / |M|^2 / reductions as three kernels (default); fused: one kernel")
     args = ap.parse_args()

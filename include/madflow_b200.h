@@ -32,7 +32,7 @@ typedef struct mf_vegas mf_vegas_t;
 enum { MF_OK = 0, MF_EINVAL = -1, MF_ENOMEM = -2, MF_ECUDA = -3, MF_ESTATE = -4, MF_EUNSUPPORTED = -5 };
 /* processes (BASELINE.json configs 0-3; 4 = the quark channel of SURVEY 8(f)2) */
 enum { MF_EE_MUMU = 0, MF_GG_TT = 1, MF_GG_TTG = 2, MF_GG_TTGG = 3,
-       MF_QQ_TT = 4, MF_PP_TT = 5 };
+       MF_QQ_TT = 4, MF_PP_TT = 5, MF_QQ_TTG = 6, MF_QG_TTQ = 7 };
                            /* MF_QQ_TT: quark channel ("any process generated (at LO)"): q q~ -> t t~, one
                             * s-channel-gluon diagram, averaged over 4 helicities x 9 colours, with the parton luminosity
                             * summed over the five light flavours and both beam orientations:
@@ -43,7 +43,15 @@ enum { MF_EE_MUMU = 0, MF_GG_TT = 1, MF_GG_TTG = 2, MF_GG_TTGG = 3,
                             * MF_PP_TT = 5: p p -> t t~ at LO, the subprocesses g g -> t t~ and q q~ -> t t~ in one integrand,
                             *   F = J_V J_x [xg(x1) xg(x2) |M_gg|^2 + (L12 + L21) |M_qq|^2] / (x1 x2) W_PS K / (2 shat)
                             * on the same grid (gluon = table 5); mf_eval_out_t.pdf = {xg(x1) xg(x2), L12 + L21}, me2 = the
-                            * luminosity-weighted mean of the two |M|^2.                                                   */
+                            * luminosity-weighted mean of the two |M|^2.
+                            * MF_QQ_TTG = 6, MF_QG_TTQ = 7 (SURVEY 8(f)2 "q q~ -> t t~ (g), q g -> t t~ q"): the channels with a
+                            * second quark line and one gluon, five diagrams each; kinematics, VEGAS dimensions (7, or 14), cuts
+                            * (ptmin_g, etamax_g on the third final particle: the gluon, resp. the light-quark jet) and selectable
+                            * generators of process 2; 11-flavour grid; fused path.
+                            *   6: F = J_V J_x [L12 |M(q(p1) q~(p2) -> t t~ g)|^2 + L21 |M(q~(p1) q(p2) -> t t~ g)|^2] / (x1 x2) W_PS K / (2 shat)
+                            *      (the two |M|^2 differ: charge asymmetry); pdf = {L12, L21}, me2 = their weighted mean |M|^2.
+                            *   7: the four channels q g, g q, q~ g, g q~ -> t t~ + q/q~ with Lqg = sum_q xf_q(x1) xg(x2) etc.;
+                            *      pdf = {Lqg + Lq~g, Lgq + Lgq~}, me2 = the luminosity-weighted mean of the four |M|^2.          */
 
 /* Selectable generators (the paper fixes no phase-space algorithm):
  *  MF_GEN_CLASSIC_RAMBO  textbook RAMBO (Kleiss, Stirling, Ellis 1986) from 4 n_final uniforms in place of the
@@ -57,7 +65,7 @@ enum { MF_GEN_CLASSIC_RAMBO = 1, MF_GEN_LINEAR_TAU = 2 };
 
 typedef struct {
   uint32_t struct_size;      /* = sizeof(mf_config_t); ABI check                                     */
-  int32_t  process;          /* MF_EE_MUMU .. MF_GG_TTGG                                             */
+  int32_t  process;          /* MF_EE_MUMU .. MF_QG_TTQ                                              */
   int32_t  precision;        /* 64 (fp64, the path); 32 = mixed precision, process MF_GG_TTG only: |M|^2
                               * (S7) in fp32, everything else (S1-S6, S8-S10) in fp64; staged path and
                               * mf_integrand_eval; other processes -> MF_EUNSUPPORTED                  */
@@ -75,7 +83,7 @@ typedef struct {
   uint32_t pdf_nx, pdf_nq;   /* knots, uniform in ln x resp. ln Q^2; nx*nq*8 bytes <= 160 KB         */
   double   pdf_xmin, pdf_xmax, pdf_qmin, pdf_qmax;
   uint32_t pdf_nf;           /* flavour tables in pdf_xf: 0 or 1 = the gluon table [nx][nq] (processes 1-3);         */
-  uint32_t reserved1;        /* 11 = [11][nx][nq], flavour index = PDG id + 5 (b~ c~ s~ u~ d~ g d u s c b): processes 4, 5. */
+  uint32_t reserved1;        /* 11 = [11][nx][nq], flavour index = PDG id + 5 (b~ c~ s~ u~ d~ g d u s c b): processes 4-7.  */
                              /* The library stages the tables flavour-innermost in shared memory, keeping             */
                              /* the <= 4 Q^2 rows the stencil of the fixed mu_f touches (36 KB)                     */
 } mf_config_t;

@@ -28,7 +28,9 @@ extern "C" {
 enum { MFO_OK = 0, MFO_EINVAL = -1, MFO_ENOMEM = -2, MFO_ESTATE = -4, MFO_EUNSUPPORTED = -5 };
 enum { MFO_EE_MUMU = 0, MFO_GG_TT = 1, MFO_GG_TTG = 2, MFO_GG_TTGG = 3,
        MFO_QQ_TT = 4,          /* q q~ -> t t~ summed over the five light flavours     */
-       MFO_PP_TT = 5 };        /* p p -> t t~ at LO: the sum of the subprocesses g g -> t t~ and q q~ -> t t~   */
+       MFO_PP_TT = 5,          /* p p -> t t~ at LO: the sum of the subprocesses g g -> t t~ and q q~ -> t t~   */
+       MFO_QQ_TTG = 6,         /* p p -> t t~ g through q q~ -> t t~ g (five diagrams), five flavours, both beam orientations   */
+       MFO_QG_TTQ = 7 };       /* p p -> t t~ + quark jet through q g, g q, q~ g, g q~ -> t t~ q (five diagrams each)      */
 
 typedef struct {
   int32_t  process;            /* MFO_*                                                          */
@@ -76,6 +78,19 @@ typedef struct {               /* host buffers owned by the caller; NULL = skip 
 typedef struct { double integral, sigma; uint64_t n_events, n_pass, n_nonfinite; } mfo_iter_t;
 typedef struct { double integral, sigma, chi2_dof; uint32_t n_iter; } mfo_result_t;
 typedef struct mfo_vegas mfo_vegas_t;
+
+/* MFO_QQ_TTG, MFO_QG_TTQ ("q q~ -> t t~ (g), q g -> t t~ q").  Kinematics, VEGAS dimensions, cuts
+ * (on the third final particle: the gluon, resp. the light-quark jet) and generators of MFO_GG_TTG; 11-flavour grid.
+ *   MFO_QQ_TTG: F = J_V J_x [L12 |M(q(p1) q~(p2))|^2 + L21 |M(q~(p1) q(p2))|^2] / (x1 x2) W_PS K / (2 shat), L12, L21 the
+ *     flavour sums of MFO_QQ_TT; the two |M|^2 differ (charge asymmetry): the second is the first with the beams exchanged.
+ *     Record: pdf[2] = {L12, L21}, me2 = their luminosity-weighted mean |M|^2.
+ *   MFO_QG_TTQ: F = J_V J_x [Lqg |M(q g)|^2 + Lgq |M(g q)|^2 + Lq~g |M(q~ g)|^2 + Lgq~ |M(g q~)|^2] / (x1 x2) W_PS K / (2 shat),
+ *     Lqg = sum_q xf_q(x1) xg(x2), Lgq = xg(x1) sum_q xf_q(x2), Lq~g, Lgq~ with the antiquark tables; |M(g q)|^2 = |M(q g)|^2
+ *     with the beams exchanged, |M(q~ g -> t t~ q~)|^2 = |M(q g -> t t~ q)|^2 with t and t~ exchanged (charge conjugation).
+ *     Record: pdf[2] = {Lqg + Lq~g, Lgq + Lgq~}, me2 = the luminosity-weighted mean of the four |M|^2.
+ * mfo_me2 returns the basic |M|^2 (q along mom[0]): averaged over 4 helicities and 9 (q q~) / 24 (q g) colours.            */
+int mfo_me2_2q(int process, const double *mom /* [5][4]: pa, pb, k1 (t), k2 (t~), k3 */, double m_top, double alpha_s,
+               int ward /* != 0: the gluon's polarisation replaced by its momentum (must give 0) */, double *out);
 
 /* ---- the path (same calls as the product's C-ABI, on host memory) ---------------------------- */
 int mfo_vegas_create(const mfo_config_t *cfg, mfo_vegas_t **out);

@@ -14,7 +14,7 @@ _LIB = os.path.join(_HERE, "libmfo.so")
 
 def build(force=False):
     """Compile oracle/libmfo.so with g++ (building the checker is not using it)."""
-    srcs = [os.path.join(_HERE, f) for f in ("mfo_core.cpp", "mfo_amp.cpp", "mfo_integrand.cpp", "mfo.h")]
+    srcs = [os.path.join(_HERE, f) for f in ("mfo_core.cpp", "mfo_amp.cpp", "mfo_amp2q.cpp", "mfo_integrand.cpp", "mfo.h")]
     if (not force and os.path.exists(_LIB)
             and all(os.path.getmtime(_LIB) >= os.path.getmtime(s) for s in srcs)):
         return _LIB
@@ -70,6 +70,7 @@ def lib():
         _lib.mfo_massive_rescale.argtypes = [C.c_uint32, C.c_double] + [C.c_void_p] * 4
         _lib.mfo_phase_space.argtypes = [C.c_uint32, C.c_double] + [C.c_void_p] * 6
         _lib.mfo_me2.argtypes = [C.c_int, C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_void_p]
+        _lib.mfo_me2_2q.argtypes = [C.c_int, C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_void_p]
         _lib.mfo_me2_literal.argtypes = [C.c_int, C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_void_p]
         _lib.mfo_jamps.argtypes = [C.c_int, C.c_void_p, C.c_double, C.c_double, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         _lib.mfo_amp_literal.argtypes = [C.c_int, C.c_void_p, C.c_double, C.c_double, C.c_void_p, C.c_void_p,
@@ -195,6 +196,11 @@ def diagram_counts(ng):
 
 def me2(process, mom, m_top=173.0, alpha_s=0.118, alpha_em=1 / 132.5):
     mom = _f64(mom); o = np.zeros(1); _check(lib().mfo_me2(process, _p(mom), m_top, alpha_s, alpha_em, _p(o))); return o[0]
+
+
+def me2_2q(process, mom, m_top=173.0, alpha_s=0.118, ward=0):
+    """|M|^2 of q q~ -> t t~ g (process 6) / q g -> t t~ q (process 7) for mom = [pa, pb, k1, k2, k3]; ward: e -> K"""
+    mom = _f64(mom); o = np.zeros(1); _check(lib().mfo_me2_2q(process, _p(mom), m_top, alpha_s, ward, _p(o))); return o[0]
 
 
 def me2_literal(process, mom, m_top=173.0, alpha_s=0.118, hel_only=-1):

@@ -477,6 +477,7 @@ static void hel_from_index(int h, int nleg, int *hel) { for (int l = 0; l < nleg
 extern "C" int mfo_me2(int process, const double *mom, double m_top, double alpha_s, double alpha_em, double *out) {
   if (process == MFO_EE_MUMU) { *out = me2_eemumu(mom, alpha_em); return MFO_OK; }
   if (process == MFO_QQ_TT) { *out = me2_qqtt(mom, m_top, alpha_s); return MFO_OK; }
+  if (process == MFO_QQ_TTG || process == MFO_QG_TTQ) return mfo_me2_2q(process, mom, m_top, alpha_s, 0, out);
   int ng = process_ng(process); if (ng < 0) return MFO_EINVAL;
   const Table &t = table(ng); int nleg = ng + 2; long double tot = 0;
   std::vector<cd> jamp;

@@ -30,12 +30,12 @@ struct mfo_vegas {
 
 extern "C" int mfo_vegas_create(const mfo_config_t *cfg, mfo_vegas_t **out) {
   if (!cfg || !out) { g_err = "null argument"; return MFO_EINVAL; }
-  if (cfg->process < 0 || cfg->process > 5) { g_err = "unknown process"; return MFO_EINVAL; }
+  if (cfg->process < 0 || cfg->process > 7) { g_err = "unknown process"; return MFO_EINVAL; }
   if (cfg->n_bins < 1 || cfg->n_bins > 255) { g_err = "n_bins out of range"; return MFO_EINVAL; }
   if (!(cfg->sqrt_s > 0)) { g_err = "sqrt_s must be positive"; return MFO_EINVAL; }
   mfo_vegas *h = new (std::nothrow) mfo_vegas(); if (!h) return MFO_ENOMEM;
   h->cfg = *cfg;
-  static const uint32_t nfin[6] = {2, 2, 3, 4, 2, 2};
+  static const uint32_t nfin[8] = {2, 2, 3, 4, 2, 2, 3, 3};
   h->n_final = nfin[cfg->process];
   h->d = (cfg->process == MFO_EE_MUMU) ? 2 : 2 + 3 * h->n_final - 4;
   if (cfg->generator & ~(uint32_t)(MFO_GEN_CLASSIC_RAMBO | MFO_GEN_LINEAR_TAU)) { g_err = "unknown generator flag"; delete h; return MFO_EINVAL; }
@@ -47,7 +47,7 @@ extern "C" int mfo_vegas_create(const mfo_config_t *cfg, mfo_vegas_t **out) {
     if (!cfg->pdf_xf || cfg->pdf_nx < 2 || cfg->pdf_nq < 2) { g_err = "pdf grid required"; delete h; return MFO_EINVAL; }
     const uint32_t nf = cfg->pdf_nf ? cfg->pdf_nf : 1;
     if (nf != 1 && nf != 11) { g_err = "pdf_nf must be 0, 1 or 11"; delete h; return MFO_EINVAL; }
-    if ((cfg->process == MFO_QQ_TT || cfg->process == MFO_PP_TT) != (nf == 11)) { g_err = "processes 4 and 5 need the 11-flavour grid, processes 1-3 the gluon table"; delete h; return MFO_EINVAL; }
+    if ((cfg->process >= MFO_QQ_TT) != (nf == 11)) { g_err = "processes 4-7 need the 11-flavour grid, processes 1-3 the gluon table"; delete h; return MFO_EINVAL; }
     h->pdf.assign(cfg->pdf_xf, cfg->pdf_xf + (size_t)nf * cfg->pdf_nx * cfg->pdf_nq); h->cfg.pdf_xf = h->pdf.data();
     h->masses[0] = h->masses[1] = cfg->m_top;
     uint32_t ngl = h->n_final - 2;
@@ -106,6 +106,42 @@ static double one_event(const mfo_vegas *h, uint32_t iteration, uint64_t ev, Eve
   uint32_t ngl = n - 2;
   if (ngl > 0) R.pass = mfo_cuts(ngl, k + 8, x1, x2, c.ptmin_g, c.etamax_g, c.drmin_gg, nullptr);   // O7
   double q2 = c.mu_f * c.mu_f;
+  if (c.process == MFO_QQ_TTG || c.process == MFO_QG_TTQ) {               // O5q / O6q with a second quark line and a gluon
+    const size_t tab = (size_t)c.pdf_nx * c.pdf_nq;                       // table of PDG id f at index f + 5
+    auto xf = [&](int id, double x) { return mfo_pdf_interp(c.pdf_xf + (5 + id) * tab, c.pdf_nx, c.pdf_nq, c.pdf_xmin, c.pdf_xmax, c.pdf_qmin, c.pdf_qmax, x, q2); };
+    auto me2_of = [&](int i0, int i1, int i2, int i3) {                   // |M|^2 with the legs (pa, pb, k1, k2) taken from m[i0], m[i1], m[i2], m[i3]
+      double mm[20], r;
+      std::memcpy(mm, m + 4 * i0, 32); std::memcpy(mm + 4, m + 4 * i1, 32); std::memcpy(mm + 8, m + 4 * i2, 32);
+      std::memcpy(mm + 12, m + 4 * i3, 32); std::memcpy(mm + 16, m + 16, 32);
+      mfo_me2(c.process, mm, c.m_top, c.alpha_s, c.alpha_em, &r);
+      return r;
+    };
+    long double lum[4] = {0, 0, 0, 0};
+    double me[4] = {0, 0, 0, 0};
+    int nch;
+    if (c.process == MFO_QQ_TTG) {
+      nch = 2;
+      for (int f = 1; f <= 5; ++f) { lum[0] += (long double)xf(f, x1) * xf(-f, x2); lum[1] += (long double)xf(-f, x1) * xf(f, x2); }
+      R.pdf[0] = (double)lum[0]; R.pdf[1] = (double)lum[1];
+      if (R.pass) { me[0] = me2_of(0, 1, 2, 3); me[1] = me2_of(1, 0, 2, 3); }            // q along beam 1 / along beam 2
+    } else {
+      nch = 4;
+      const double g1 = xf(0, x1), g2 = xf(0, x2);
+      long double q1 = 0, a1 = 0, q2s = 0, a2 = 0;
+      for (int f = 1; f <= 5; ++f) { q1 += xf(f, x1); a1 += xf(-f, x1); q2s += xf(f, x2); a2 += xf(-f, x2); }
+      lum[0] = q1 * g2; lum[1] = g1 * q2s; lum[2] = a1 * g2; lum[3] = g1 * a2;            // q g, g q, q~ g, g q~
+      R.pdf[0] = (double)(lum[0] + lum[2]); R.pdf[1] = (double)(lum[1] + lum[3]);
+      if (R.pass) {
+        me[0] = me2_of(0, 1, 2, 3); me[1] = me2_of(1, 0, 2, 3);                          // quark along beam 1 / beam 2
+        me[2] = me2_of(0, 1, 3, 2); me[3] = me2_of(1, 0, 3, 2);                          // antiquarks: charge conjugation = t <-> t~
+      }
+    }
+    if (!R.pass) return 0.0;
+    long double sum = 0, ltot = 0;
+    for (int i = 0; i < nch; ++i) { sum += lum[i] * me[i]; ltot += lum[i]; }
+    R.me2 = (double)(sum / ltot);
+    return JV * Jx * ((double)sum / (x1 * x2)) * h->sym * w3[0] * w3[1] * c.gev2_to_pb / (2.0 * shat);
+  }
   if (c.process == MFO_QQ_TT || c.process == MFO_PP_TT) {                 // O5q: flavour-summed luminosity
     const size_t tab = (size_t)c.pdf_nx * c.pdf_nq;                       // table of PDG id f at index f + 5
     long double l12 = 0, l21 = 0;

@@ -1,5 +1,5 @@
 """In-tree build of libmadflow_b200.so for sm_100a: run the amplitude generator, compile the C-ABI
-and the six per-process kernel objects in parallel with nvcc, link.  `python -m
+and the eight per-process kernel objects in parallel with nvcc, link.  `python -m
 paper_2105_10529_b200.build [--force]`."""
 import os
 import subprocess
@@ -28,7 +28,7 @@ def build(force=False, verbose=False):
     api = kern + [os.path.join(CSRC, f) for f in ("mf_small_kernels.cuh", "mf_params.h")]
     api += [os.path.join(os.path.dirname(HERE), "include", "madflow_b200.h")]
     jobs = [("mf_api.o", os.path.join(CSRC, "mf_api.cu"), [])]
-    jobs += [("mf_proc%d.o" % p, os.path.join(CSRC, "mf_proc.cu"), ["-DMF_PROC=%d" % p]) for p in range(6)]
+    jobs += [("mf_proc%d.o" % p, os.path.join(CSRC, "mf_proc.cu"), ["-DMF_PROC=%d" % p]) for p in range(8)]
 
     def compile_one(job):
         obj, src, extra = job
@@ -42,7 +42,7 @@ def build(force=False, verbose=False):
             raise RuntimeError("nvcc failed for %s:\n%s" % (obj, (r.stdout + r.stderr)[-4000:]))
         return obj, "compiled"
 
-    with ThreadPoolExecutor(max_workers=7) as ex:
+    with ThreadPoolExecutor(max_workers=8) as ex:
         results = list(ex.map(compile_one, jobs))
     objs = [os.path.join(obj_dir, j[0]) for j in jobs]
     if force or not _newer(lib, objs):

@@ -119,7 +119,7 @@ extern "C" int mf_vegas_create(const mf_config_t* cfg, mf_vegas_t** out) {
   h->use_staged = h->rec_fields > 0;
   h->f32 = cfg->precision == 32;
   h->max_blocks = h->n_sm * 32;
-  const bool flavours = cfg->process == MF_QQ_TT || cfg->process == MF_PP_TT;   // 11-flavour grid: its active rows (mf_flavour_slice)
+  const bool flavours = cfg->process >= MF_QQ_TT;        // 11-flavour grid: its active rows (mf_flavour_slice)
   const size_t ne = (size_t)P.d * (P.nb + 1), npdf = (size_t)P.pdf_smem;
   MF_CREATE_CUDA(cudaMalloc(&h->d_edges, ne * sizeof(double)));
   MF_CREATE_CUDA(cudaMalloc(&h->d_pdf, (npdf ? npdf : 1) * sizeof(double)));
@@ -546,13 +546,15 @@ extern "C" int mf_set_grid(mf_vegas_t* h, const double* e) {
 
 extern "C" int mf_me_flops(const mf_vegas_t* h, uint64_t* n_add, uint64_t* n_mul, uint64_t* n_fma) {
   if (!h) return fail(MF_EINVAL, "handle is NULL");
-  static const uint64_t T[6][3] = {{MF_ME2_EE_MUMU_NADD, MF_ME2_EE_MUMU_NMUL, MF_ME2_EE_MUMU_NFMA},
+  static const uint64_t T[8][3] = {{MF_ME2_EE_MUMU_NADD, MF_ME2_EE_MUMU_NMUL, MF_ME2_EE_MUMU_NFMA},
                                    {MF_ME2_GG_TT_NADD, MF_ME2_GG_TT_NMUL, MF_ME2_GG_TT_NFMA},
                                    {MF_ME2_GG_TTG_NADD, MF_ME2_GG_TTG_NMUL, MF_ME2_GG_TTG_NFMA},
                                    {MF_ME2_GG_TTGG_NADD, MF_ME2_GG_TTGG_NMUL, MF_ME2_GG_TTGG_NFMA},
                                    {MF_ME2_EE_MUMU_NADD, MF_ME2_EE_MUMU_NMUL, MF_ME2_EE_MUMU_NFMA},    // q q~ -> t t~: the two-current code
                                    {MF_ME2_GG_TT_NADD + MF_ME2_EE_MUMU_NADD, MF_ME2_GG_TT_NMUL + MF_ME2_EE_MUMU_NMUL + 1,
-                                    MF_ME2_GG_TT_NFMA + MF_ME2_EE_MUMU_NFMA + 1}};   // p p -> t t~: both subprocesses + the luminosity-weighted sum (mul, fma)
+                                    MF_ME2_GG_TT_NFMA + MF_ME2_EE_MUMU_NFMA + 1},    // p p -> t t~: both subprocesses + the luminosity-weighted sum (mul, fma)
+                                   {2 * MF_ME2_QQ_TTG_NADD, 2 * MF_ME2_QQ_TTG_NMUL, 2 * MF_ME2_QQ_TTG_NFMA + 2},     // two channels (q q~, q~ q)
+                                   {4 * MF_ME2_QG_TTQ_NADD, 4 * MF_ME2_QG_TTQ_NMUL, 4 * MF_ME2_QG_TTQ_NFMA + 4}};    // four channels
   if (n_add) *n_add = T[h->P.process][0];
   if (n_mul) *n_mul = T[h->P.process][1];
   if (n_fma) *n_fma = T[h->P.process][2];

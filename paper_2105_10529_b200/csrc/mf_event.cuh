@@ -10,6 +10,8 @@
 #include "generated/mf_me2_gg_tt.cuh"
 #include "generated/mf_me2_gg_ttg.cuh"
 #include "generated/mf_me2_gg_ttgg_lanes.cuh"     // gg -> tt~gg: one event over four lanes (gen/lanes.py)
+#include "generated/mf_me2_qq_ttg.cuh"            // q q~ -> t t~ g and q g -> t t~ q (gen/quarks.py)
+#include "generated/mf_me2_qg_ttq.cuh"
 
 template <int PROC> struct MfProc;
 // GROUP: threads that share the barrier points of the generated |M|^2 code (mf_device.cuh)
@@ -24,7 +26,17 @@ template <> struct MfProc<3> { static const int D = 10, N = 4, NGL = 2, GROUP = 
 template <> struct MfProc<4> { static const int D = 4, N = 2, NGL = 0, GROUP = 128; };
 // p p -> t t~ at LO: the subprocesses g g -> t t~ and q q~ -> t t~ in one integrand (kinematics of process 1)
 template <> struct MfProc<5> { static const int D = 4, N = 2, NGL = 0, GROUP = 128; };
-template <int PROC> struct MfPdf { static const bool FLAVOURS = PROC == 4 || PROC == 5; };
+// p p -> t t~ g through q q~ -> t t~ g (both beam orientations), and p p -> t t~ + quark jet through q g, g q, q~ g, g q~ ->
+// t t~ q: kinematics, cuts (on the third final particle) and VEGAS dimensions of process 2, flavour grid
+template <> struct MfProc<6> { static const int D = 7, N = 3, NGL = 1, GROUP = 128; };
+template <> struct MfProc<7> { static const int D = 7, N = 3, NGL = 1, GROUP = 128; };
+template <int PROC> struct MfPdf { static const bool FLAVOURS = PROC >= 4; };
+// processes whose |M|^2 stage is heavy enough for the staged iteration path (front end / |M|^2 / reductions as three kernels)
+template <int PROC> struct MfHeavy { static const bool value = PROC == 2 || PROC == 3; };
+// partonic channels summed in one event (luminosity-weighted |M|^2): 1, or 2 (process 5: gg + qq~; process 6: q q~ and q~ q),
+// or 4 (process 7: q g, g q, q~ g, g q~)
+template <int PROC> struct MfChannels { static const int value = PROC == 7 ? 4 : (PROC == 5 || PROC == 6) ? 2 : 1; };
+#define MF_NLUM 4
 // Generator selection of the front end, template parameter CL:
 //   0  the generators of the configs, nothing selectable (the path bench.py times: no branch)
 //   1  classic 4n-random RAMBO, d = 2 + 4n; the tau map (O3 or O3') is a run-time, grid-uniform branch on P.gen
@@ -99,7 +111,7 @@ MF_HD T mf_me2(const MfParams& P, T rts, const T k[MfProc<PROC>::N][4]) {
     mf_me_inputs_gg<3, T>(rts, T(P.m_top), (const T(*)[4])k, in);
     return T(P.me_pref) * mf_me2_gg_ttg<T>(in);
   } else {
-    static_assert(PROC != 3, "gg -> tt~gg has no one-thread |M|^2: mf_me2_ttgg_group (four lanes per event)");
+    static_assert(PROC != 3 && PROC < 6, "gg -> tt~gg: mf_me2_ttgg_group (four lanes per event); processes 6, 7: mf_me2_2q");
     return T(0.0);
   }
 }
@@ -177,12 +189,51 @@ __device__ __forceinline__ T mf_me2_ttgg_warp32(const MfParams& P, T rts, const 
 }
 #endif
 
+// ---- q q~ -> t t~ g (PROC 6) and q g -> t t~ q (PROC 7): the generated code takes generic external lines, so the other
+// channels are the same code on relabelled momenta.  ch bit 0: the beams exchanged (the light quark comes along -z);
+// bit 1: the charge-conjugate channel = t and t~ exchanged (q~ g -> t t~ q~).  DESIGN.md 5.10.
+template <int PROC, typename T>
+MF_HD T mf_me2_2q(const MfParams& P, T rts, const T k[3][4], int ch) {
+  static_assert(MF_ME2_QQ_TTG_NIN == 41 && MF_ME2_QG_TTQ_NIN == 41, "generator input layout changed");
+  T in[41];
+  const T E = T(0.5) * rts, sz = (ch & 1) ? T(-1.0) : T(1.0), r2 = T(1.41421356237309504880);
+  const T pa[4] = {E, T(0.0), T(0.0), sz * E}, pb[4] = {E, T(0.0), T(0.0), -sz * E};
+  T k1[4], k2[4], f[5], o[5];
+#pragma unroll
+  for (int c = 0; c < 4; ++c) { k1[c] = (ch & 2) ? k[1][c] : k[0][c]; k2[c] = (ch & 2) ? k[0][c] : k[1][c]; }
+  in[0] = T(P.m_top);
+#pragma unroll
+  for (int c = 0; c < 4; ++c) in[1 + c] = k2[c];
+  mf_fermion_ing<T>(k1, T(P.m_top), in + 5);
+  mf_fermion_ing<T>(k2, T(P.m_top), in + 10);
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {                          // light line: u(pa) ... vbar(pb) (PROC 6) or ubar(k3) (PROC 7); gluon all-incoming
+    in[15 + c] = pa[c];
+    in[19 + c] = PROC == 6 ? pb[c] : -k[2][c];
+    in[31 + c] = PROC == 6 ? -k[2][c] : pb[c];
+  }
+  mf_fermion_ing<T>(pa, T(0.0), f);
+  in[23] = f[0]; in[24] = f[2]; in[25] = f[3]; in[26] = f[4];
+  mf_fermion_ing<T>(PROC == 6 ? pb : k[2], T(0.0), f);
+  in[27] = f[0]; in[28] = f[2]; in[29] = f[3]; in[30] = f[4];
+  mf_gluon_ing<T>(PROC == 6 ? k[2] : pb, o);              // eps1, eps2 / sqrt2 of the gluon (linear basis: same vectors in and out)
+  in[35] = r2 * o[0]; in[36] = r2 * o[1]; in[37] = r2 * o[2]; in[38] = r2 * o[3]; in[39] = r2 * o[4]; in[40] = T(0.0);
+  return T(P.me_pref) * (PROC == 6 ? mf_me2_qq_ttg<T>(in) : mf_me2_qg_ttq<T>(in));
+}
+
 // S7 weighted with the parton luminosities: process 5 returns xg(x1) xg(x2) |M_gg|^2 + (L12 + L21) |M_qq|^2 (lum = the two
 // luminosities from the front end); every other process its |M|^2
 template <int PROC, typename T>
 MF_HD T mf_me2_lum(const MfParams& P, T rts, const T k[MfProc<PROC>::N][4], const double* lum) {
-  if (PROC == 5) return T(lum[0]) * mf_me2<1, T>(P, rts, k) + T(lum[1]) * mf_me2<4, T>(P, rts, k);
-  return mf_me2<(PROC == 5 || PROC == 3) ? 1 : PROC, T>(P, rts, k);      // (process 3: mf_me2_ttgg_group instead)
+  if constexpr (PROC == 5) return T(lum[0]) * mf_me2<1, T>(P, rts, k) + T(lum[1]) * mf_me2<4, T>(P, rts, k);
+  else if constexpr (PROC == 6 || PROC == 7) {           // sum over the channels: one copy of the |M|^2 code
+    T sum = T(0.0);
+#if defined(__CUDACC__)
+#pragma unroll 1
+#endif
+    for (int ch = 0; ch < MfChannels<PROC>::value; ++ch) sum += T(lum[ch]) * mf_me2_2q<PROC, T>(P, rts, k, ch);
+    return sum;
+  } else return mf_me2<PROC == 3 ? 1 : PROC, T>(P, rts, k);      // (process 3: mf_me2_ttgg_group instead)
 }
 
 // Front end of one event, S1-S6 + the weight prefactor: F = pref * |M|^2 for a passing event with
@@ -208,7 +259,23 @@ MF_HD bool mf_event_front(const MfParams& P, const double* edges, const double* 
   rts = sqrt(shat);
   const bool pass = mf_cuts<NGL>(P, (const double(*)[4])(&k[0][0] + 8), x1, x2);   // S5 (final gluons = k[2..])
   double ff = 1.0, xf1 = 0.0, xf2 = 0.0;                                 // ff = f_g(x1) f_g(x2) / shat
-  if (MfPdf<PROC>::FLAVOURS) {                                           // S6q: flavour-summed luminosity (xf1, xf2 = the two sums)
+  if (PROC == 7) {                                                       // S6q: q g, g q, q~ g, g q~ luminosities (to S7: mf_me2_lum)
+    ff = 1.0 / (x1 * x2 * shat);
+    if (REC || pass) {
+      const double g1 = mf_pdf_strided<MF_NFL>(P, pdf_tab + 5, lx1, P.pdf_lq), g2 = mf_pdf_strided<MF_NFL>(P, pdf_tab + 5, lx2, P.pdf_lq);
+      double q1 = 0.0, a1 = 0.0, q2 = 0.0, a2 = 0.0;
+#pragma unroll
+      for (int q = 1; q <= 5; ++q) {
+        q1 += mf_pdf_strided<MF_NFL>(P, pdf_tab + 5 + q, lx1, P.pdf_lq); a1 += mf_pdf_strided<MF_NFL>(P, pdf_tab + 5 - q, lx1, P.pdf_lq);
+        q2 += mf_pdf_strided<MF_NFL>(P, pdf_tab + 5 + q, lx2, P.pdf_lq); a2 += mf_pdf_strided<MF_NFL>(P, pdf_tab + 5 - q, lx2, P.pdf_lq);
+      }
+      lum[0] = q1 * g2; lum[1] = g1 * q2; lum[2] = a1 * g2; lum[3] = g1 * a2;
+      xf1 = lum[0] + lum[2]; xf2 = lum[1] + lum[3];                      // the record: quark from beam 1 / from beam 2
+    }
+  } else if (PROC == 6) {                                                // q q~ and q~ q luminosities (the two |M|^2 differ)
+    ff = 1.0 / (x1 * x2 * shat);
+    if (REC || pass) { mf_lumi_qq(P, pdf_tab, lx1, lx2, P.pdf_lq, xf1, xf2); lum[0] = xf1; lum[1] = xf2; }
+  } else if (MfPdf<PROC>::FLAVOURS) {                                    // S6q: flavour-summed luminosity (xf1, xf2 = the two sums)
     mf_lumi_qq(P, pdf_tab, lx1, lx2, P.pdf_lq, xf1, xf2);
     ff = (xf1 + xf2) / (x1 * x2 * shat);
     if (PROC == 5) {                                                     // both subprocesses: the luminosities go to S7 (mf_me2_lum)
@@ -248,7 +315,7 @@ MF_HD double mf_event(const MfParams& P, const double* edges, const double* pdf_
                       uint32_t iteration, uint64_t ev, int bin[MfDim<PROC, CL>::D], bool& pass,
                       MfEventRec* rec, unsigned* okeys = nullptr) {
   constexpr int N = MfProc<PROC>::N;
-  double k[N][4], rts, pref, lum[2] = {0.0, 0.0};
+  double k[N][4], rts, pref, lum[MF_NLUM] = {0.0, 0.0, 0.0, 0.0};
   pass = mf_event_front<PROC, REC, CL>(P, edges, pdf_tab, iteration, ev, bin, k, rts, pref, rec, okeys, lum);
   double me2 = 0.0;
   if (MF_UNIFORM_ME || pass) {                                           // S7 (in the real type T)
@@ -260,6 +327,6 @@ MF_HD double mf_event(const MfParams& P, const double* edges, const double* pdf_
     me2 = (double)mf_me2_lum<PROC, T>(P, (T)rts, kt, lum);
   }
   if (!pass) me2 = 0.0;
-  if (REC) rec->me2 = PROC == 5 ? me2 / (lum[0] + lum[1]) : me2;         // process 5: the luminosity-weighted mean |M|^2
+  if (REC) rec->me2 = MfChannels<PROC>::value > 1 ? me2 / (lum[0] + lum[1] + lum[2] + lum[3]) : me2;   // several channels: the luminosity-weighted mean |M|^2
   return pass ? pref * me2 : 0.0;                                        // S8
 }

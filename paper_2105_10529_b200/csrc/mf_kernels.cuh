@@ -29,6 +29,8 @@
 template <int PROC> struct MfLaunch { static const int MINB = 512 / MF_THREADS; };
 template <> struct MfLaunch<2> { static const int MINB = MF_MINB_HEAVY; };
 template <> struct MfLaunch<3> { static const int MINB = MF_MINB_HEAVY; };
+template <> struct MfLaunch<6> { static const int MINB = 1; };    // 3 400 straight-line operations per channel: all 255 registers
+template <> struct MfLaunch<7> { static const int MINB = 1; };
 
 struct MfEvalOutDev {
   double* weight; double* x; uint8_t* bins; double* momenta; double* me2; double* pdf; uint8_t* pass;

@@ -8,8 +8,8 @@
 static_assert(MFD_GEN_CLASSIC == MF_GEN_CLASSIC_RAMBO && MFD_GEN_LINEAR == MF_GEN_LINEAR_TAU, "device flags follow the header");
 
 static inline int mf_process_shape(int process, uint32_t generator, int* d, int* n_final, int* ng) {
-  static const int nf[6] = {2, 2, 3, 4, 2, 2};
-  if (process < 0 || process > 5) return -1;
+  static const int nf[8] = {2, 2, 3, 4, 2, 2, 3, 3};
+  if (process < 0 || process > 7) return -1;
   *n_final = nf[process];
   *d = (process == MF_EE_MUMU) ? 2 : 2 + 3 * nf[process] - 4;
   if (generator & MF_GEN_CLASSIC_RAMBO) *d = 2 + 4 * nf[process];       // O4': 4n uniforms
@@ -61,7 +61,7 @@ static inline int mf_fill_params(const mf_config_t* c, MfParams* P, std::string&
     if (!c->pdf_xf || c->pdf_nx < 2 || c->pdf_nq < 2) { err = "pdf grid required"; return MF_EINVAL; }
     const uint32_t nfl = c->pdf_nf ? c->pdf_nf : 1;
     if (nfl != 1 && nfl != 11) { err = "pdf_nf must be 0, 1 or 11"; return MF_EINVAL; }
-    if ((c->process == MF_QQ_TT || c->process == MF_PP_TT) != (nfl == 11)) { err = "processes 4 and 5 need the 11-flavour grid, processes 1-3 the gluon table"; return MF_EINVAL; }
+    if ((c->process >= MF_QQ_TT) != (nfl == 11)) { err = "processes 4-7 need the 11-flavour grid, processes 1-3 the gluon table"; return MF_EINVAL; }
     if ((uint64_t)c->pdf_nx * c->pdf_nq * 8ull > 160ull * 1024ull) { err = "pdf table larger than 160 KB"; return MF_EINVAL; }
     if (!(c->pdf_xmin > 0.0 && c->pdf_xmax > c->pdf_xmin && c->pdf_qmin > 0.0 && c->pdf_qmax > c->pdf_qmin)) { err = "bad pdf ranges"; return MF_EINVAL; }
     const int ngl = nfin - 2;
@@ -78,6 +78,8 @@ static inline int mf_fill_params(const mf_config_t* c, MfParams* P, std::string&
     if (c->process == MF_PP_TT) p.me_pref = gs2n / 256.0 * MF_ME2_GG_TT_SCALE;         // its g g -> t t~ subprocess
     p.me_pref_qq = gs2n * (2.0 / 9.0) * MF_ME2_EE_MUMU_SCALE;                           // O6q: colour sum 2 / 9 colours, 1/4 spins
     if (c->process == MF_QQ_TT) p.me_pref = p.me_pref_qq;
+    if (c->process == MF_QQ_TTG) p.me_pref = gs2n * MF_ME2_QQ_TTG_SCALE;               // g_s^6 / (9 colour denominator x 36)
+    if (c->process == MF_QG_TTQ) p.me_pref = gs2n * MF_ME2_QG_TTQ_SCALE;               // ... x 96
     p.wconst = (ngl == 2 ? 0.5 : 1.0) * c->gev2_to_pb / 2.0;
     p.pdf_nx = (int)c->pdf_nx; p.pdf_nq = (int)c->pdf_nq;
     p.pdf_lx0 = log(c->pdf_xmin);

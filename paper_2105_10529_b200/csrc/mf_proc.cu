@@ -6,7 +6,7 @@
 #include "mf_proc.h"
 #include <type_traits>
 #ifndef MF_PROC
-#error "compile with -DMF_PROC=0..5"
+#error "compile with -DMF_PROC=0..7"
 #endif
 
 __device__ __forceinline__ void mf_stage_tables(const MfParams& P, const double* g_edges, const double* g_pdf,
@@ -501,7 +501,7 @@ mf_eval_kernel(const MfParams P, const double* __restrict__ g_edges, const doubl
   for (unsigned long long base = (unsigned long long)blockIdx.x * blockDim.x; base < n; base += stride) {
     unsigned long long i = base + threadIdx.x;           // block-uniform trip count (barriers inside the event)
     if (i >= n) { if (!MF_UNIFORM_ME) break; i = n - 1; }   // tail lanes recompute event n-1 (same values written)
-    double k[N][4], rts, pref, lum[2] = {0.0, 0.0};
+    double k[N][4], rts, pref, lum[MF_NLUM] = {0.0, 0.0, 0.0, 0.0};
     bool pass;
     if (PROC != 0 && (P.gen & MFD_GEN_CLASSIC)) pass = mf_eval_front<PROC, REC, PROC != 0 ? 1 : 0>(P, s_edges, s_pdf, iteration, first + i, i, o, k, rts, pref, lum);
     else pass = mf_eval_front<PROC, REC, PROC != 0 ? 2 : 0>(P, s_edges, s_pdf, iteration, first + i, i, o, k, rts, pref, lum);
@@ -519,7 +519,7 @@ mf_eval_kernel(const MfParams P, const double* __restrict__ g_edges, const doubl
     double F = pass ? pref * me2 : 0.0;                  // S8
     if (!isfinite(F)) F = 0.0;
     if (o.weight) o.weight[i] = F;
-    if (REC && o.me2) o.me2[i] = PROC == 5 ? me2 / (lum[0] + lum[1]) : me2;   // process 5: luminosity-weighted mean
+    if (REC && o.me2) o.me2[i] = MfChannels<PROC>::value > 1 ? me2 / (lum[0] + lum[1] + lum[2] + lum[3]) : me2;   // several channels: luminosity-weighted mean
   }
 }
 
@@ -528,9 +528,9 @@ mf_eval_kernel(const MfParams P, const double* __restrict__ g_edges, const doubl
 #define MF_COMPACT 1                 // CTA-level compaction of passing events for the processes with cuts
 #endif
 static constexpr bool kFused = MF_PROC != 3;         // gg -> tt~gg iterates on the staged path only (four lanes per event in its |M|^2 stage)
-static constexpr bool kCompact = MF_COMPACT && MfProc<MF_PROC>::NGL > 0 && kFused;
+static constexpr bool kCompact = MF_COMPACT && MfHeavy<MF_PROC>::value && kFused;
 static constexpr size_t kTileBytes = MF_PROC == 3 ? sizeof(double) * (MF_THREADS / 32) * MF_LANES_TILE : 0;   // eval kernel: lane tiles
-static constexpr bool kEvalOne = MfProc<MF_PROC>::NGL > 0;
+static constexpr bool kEvalOne = MfHeavy<MF_PROC>::value;
 static constexpr bool kF32 = MF_PROC == 2;   // fp32 variant of the |M|^2 stage: gg -> tt~g only (BASELINE configs[4])
 // classic 4n-random RAMBO: processes 1-3; the heavy ones on the staged path only
 static constexpr int kCL = MF_PROC != 0 ? 1 : 0;    // front-end instance of the classic RAMBO (mf_event.cuh MfDim)
@@ -631,7 +631,7 @@ static cudaError_t proc_iterate(const MfParams& P, const double* edges, const do
 #ifndef MF_STAGED
 #define MF_STAGED 1                  // heavy processes (with cuts) iterate through the staged path
 #endif
-static constexpr bool kStaged = MF_STAGED && MfProc<MF_PROC>::NGL > 0;
+static constexpr bool kStaged = MF_STAGED && MfHeavy<MF_PROC>::value;
 static constexpr int kRecFields = MF_REC_FIELDS(MfProc<MF_PROC>::N);
 
 static size_t front_smem(const MfParams& P) {

@@ -21,7 +21,8 @@ struct MfProcOps {
                         double* partial, unsigned long long* pcount, int row, int grid_me, int grid_hist, bool f32,
                         cudaStream_t st, cudaEvent_t* ev);
 };
-extern const MfProcOps mf_ops_0, mf_ops_1, mf_ops_2, mf_ops_3, mf_ops_4, mf_ops_5;
+extern const MfProcOps mf_ops_0, mf_ops_1, mf_ops_2, mf_ops_3, mf_ops_4, mf_ops_5, mf_ops_6, mf_ops_7;
 static inline const MfProcOps* mf_proc_ops(int process) {
-  return process == 0 ? &mf_ops_0 : process == 1 ? &mf_ops_1 : process == 2 ? &mf_ops_2 : process == 3 ? &mf_ops_3 : process == 4 ? &mf_ops_4 : &mf_ops_5;
+  static const MfProcOps* const ops[8] = {&mf_ops_0, &mf_ops_1, &mf_ops_2, &mf_ops_3, &mf_ops_4, &mf_ops_5, &mf_ops_6, &mf_ops_7};
+  return ops[process];
 }

@@ -4,6 +4,7 @@ import os
 import sys
 from . import amplitudes as A
 from . import lanes as L
+from . import quarks as Q
 
 
 def _write(path, text):
@@ -30,6 +31,14 @@ def main(outdir=None):
         text, tot = A.emit_function(gen, fname)
         if fname == "mf_me2_gg_ttg":
             text += "#define MF_ME2_GG_TTG_NFLOPS_MIN %dull\n" % lean_flops(3)
+        _write(os.path.join(outdir, fname + ".cuh"), text)
+        print("%-22s add %7d mul %7d fma %7d rcp %3d  flops/event %8d  inputs %d" % (
+            fname, tot["add"], tot["mul"], tot["fma"], tot["rcp"],
+            tot["add"] + tot["mul"] + 2 * tot["fma"], len(gen.input_names)))
+    for fname, make in Q.PROCESSES_2Q.items():          # q q~ -> t t~ g, q g -> t t~ q
+        gen = make()
+        gen.build()
+        text, tot = A.emit_function(gen, fname)
         _write(os.path.join(outdir, fname + ".cuh"), text)
         print("%-22s add %7d mul %7d fma %7d rcp %3d  flops/event %8d  inputs %d" % (
             fname, tot["add"], tot["mul"], tot["fma"], tot["rcp"],

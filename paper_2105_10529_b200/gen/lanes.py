@@ -38,21 +38,21 @@ def _canon(pi):
     return pi, 1
 
 
-def _shift(pi, k):
-    return tuple((x + k) % NL for x in pi)
+def _shift(pi, k, nl=NL):
+    return tuple((x + k) % nl for x in pi)
 
 
-def orbits(size):
+def orbits(size, nl=NL):
     """orbits of the cyclic relabelling on the ordered currents of `size` gluons modulo reflection:
     {canonical pi: (representative, k, sign)} with j(pi) = sign * [lane l+k's j(representative)]"""
     out, reps = {}, []
-    for pi in itertools.permutations(range(NL), size):
+    for pi in itertools.permutations(range(nl), size):
         c, _ = _canon(pi)
         if c in out:
             continue
         reps.append(c)
-        for k in range(NL):
-            c2, s2 = _canon(_shift(c, k))
+        for k in range(nl):
+            c2, s2 = _canon(_shift(c, k, nl))
             out.setdefault(c2, (c, k, s2))
     return out, reps
 
@@ -60,7 +60,8 @@ def orbits(size):
 class GenLanes(Gen):
     """per-lane program of gg -> t t~ g g; inputs are the lane's relabelled quantities"""
 
-    def __init__(self):
+    def __init__(self, nl=NL):
+        NL = self.nl = nl                      # gluons = lanes per event (4: gg -> tt~gg; 3: gg -> tt~g)
         self.basis, self.ng, self.g = "linear", NL, Dag()
         self.loop_lam4, self.parity, self.loop_legs = False, True, ()
         g = self.g
@@ -76,8 +77,8 @@ class GenLanes(Gen):
         self.pl = [[g.sym("pl%d%s" % (i, c)) for c in "xyz"] for i in range(NL)]
         self._P, self._j, self._sl, self._chi = {}, {}, {}, {}
         self.orb, self.reps = {}, {}
-        for size in (2, 3, 4):
-            o, r = orbits(size)
+        for size in range(2, NL + 1):
+            o, r = orbits(size, NL)
             self.orb.update(o)
             self.reps[size] = r
         self.slot_of = {}                      # representative -> first of its 4 exchange slots
@@ -116,10 +117,11 @@ class GenLanes(Gen):
 
     def build(self):
         g = self.g
+        NL = self.nl
         num, den, perms = colour_matrix(NL)
         index = {p: i for i, p in enumerate(perms)}
         # ---- gluon currents: one representative per orbit, phase by phase ------------------------------
-        for size in (2, 3, 4):
+        for size in range(2, NL + 1):
             for rep in self.reps[size]:
                 cur = self._bg(rep, None)
                 assert all(c.im.is_zero() for c in cur)
@@ -130,12 +132,10 @@ class GenLanes(Gen):
                     self.prog.append(("store", self.slot_of[rep] + m, cur[m].re))
             self.prog.append(("sync", 0))
         # ---- quark line: the six orderings (a b c 0), depth first ----------------------------------------
-        local = []
-        for c in (1, 2, 3):
-            for b in (1, 2, 3):
-                if b != c:
-                    a = 6 - b - c
-                    local.append((a, b, c, 0))
+        # orderings (.. c 0) that end with the lane's gluon, grouped so that neighbours share their tails
+        local = [tuple(reversed(p)) + (0,) for p in itertools.permutations(range(1, NL))]
+        local.sort(key=lambda sg: tuple(reversed(sg)))
+        nloc = len(local)
         amps = {1: [], -1: []}
         for sg in local:
             a = self.partial_amps(sg, None, 1)
@@ -153,32 +153,35 @@ class GenLanes(Gen):
                 xs[(lam3, part)] = [getattr(a, part) for a in amps[lam3]]
                 for i, x in enumerate(xs[(lam3, part)]):
                     self.prog.append(("store", slot + i, x))
-                slot += 6
+                slot += nloc
         self.prog.append(("sync", 1))
         self.n_slots = max(self.n_slots, slot)
 
         def glob(sg, lane):
-            return index[_shift(sg, lane)]
+            return index[_shift(sg, lane, NL)]
 
-        blocks = {}
-        for k in (0, 1, 2):
+        # blocks C(k) between a lane and the lane k places on; C(NL - k) seen from the other lane is the transpose of C(k):
+        # the pairs (k, NL - k), k < NL - k, are taken once with weight 2, the self-paired k = NL / 2 with weight 1
+        blocks, weight = {}, {}
+        for k in range(0, NL // 2 + 1):
             blk = np.array([[num[glob(si, 0)][glob(sj, k)] for sj in local] for si in local])
             for lane in range(1, NL):          # invariance under relabelling: the blocks do not depend on the lane
                 assert (blk == np.array([[num[glob(si, lane)][glob(sj, lane + k)] for sj in local] for si in local])).all()
             blocks[k] = blk
+            weight[k] = 1.0 if (k == 0 or 2 * k == NL) else 2.0
         total = g.const(0.0)
         slot = 0
         for lam3 in (1, -1):
             for part in ("re", "im"):
                 x = xs[(lam3, part)]
                 pairs = []
-                for i in range(6):
-                    y = g.sop([(g.const(2.0 * blocks[0][i][t]), x[t]) for t in range(i + 1, 6)], g.const(float(blocks[0][i][i])) * x[i])
-                    y = g.sop([(g.const(2.0 * blocks[1][i][t]), g.xl(slot + t, 1, 1)) for t in range(6)], y)
-                    y = g.sop([(g.const(1.0 * blocks[2][i][t]), g.xl(slot + t, 2, 1)) for t in range(6)], y)
+                for i in range(nloc):
+                    y = g.sop([(g.const(2.0 * blocks[0][i][t]), x[t]) for t in range(i + 1, nloc)], g.const(float(blocks[0][i][i])) * x[i])
+                    for k in range(1, NL // 2 + 1):
+                        y = g.sop([(g.const(weight[k] * blocks[k][i][t]), g.xl(slot + t, k, 1)) for t in range(nloc)], y)
                     pairs.append((x[i], y))
                 total = g.sop(pairs, total)
-                slot += 6
+                slot += nloc
         self._mark()
         self.out = total
         self.scale = 2.0 / den                 # parity (lambda_4 fixed) / colour denominator; unit polarisation vectors
@@ -192,15 +195,16 @@ def evaluate_event(gen, mom, mt, ferm, glu_units):
     mom: [6][4] (g g -> t t~ g g, partonic CM frame); ferm(p, m) -> 5 spinor ingredients;
     glu_units(k) -> (eps1, eps2) unit 3-vectors of an outgoing gluon."""
     g = gen.g
-    Kg = [np.array(mom[0]), np.array(mom[1]), -np.array(mom[4]), -np.array(mom[5])]
-    e = [(np.array([1.0, 0.0, 0.0]), np.array([0.0, 1.0, 0.0])), (np.array([1.0, 0.0, 0.0]), np.array([0.0, -1.0, 0.0])),
-         glu_units(mom[4]), glu_units(mom[5])]
+    NL = gen.nl
+    Kg = [np.array(mom[0]), np.array(mom[1])] + [-np.array(mom[4 + i]) for i in range(NL - 2)]
+    e = [(np.array([1.0, 0.0, 0.0]), np.array([0.0, 1.0, 0.0])), (np.array([1.0, 0.0, 0.0]), np.array([0.0, -1.0, 0.0]))] + \
+        [glu_units(mom[4 + i]) for i in range(NL - 2)]
     base = {"mt": mt}
     for n, c in zip(("p4e", "p4x", "p4y", "p4z"), mom[3]): base[n] = c
     for n, c in zip(("wp", "wm", "c0", "cx", "cy"), ferm(mom[2], mt)): base["t_" + n] = c
     for n, c in zip(("wp", "wm", "c0", "cx", "cy"), ferm(mom[3], mt)): base["b_" + n] = c
     total = 0.0
-    for ih in range(16):
+    for ih in range(1 << NL):
         vals = []
         for lane in range(NL):
             v = dict(base)
@@ -243,10 +247,11 @@ def emit_lanes(gen, fname, sched_window=48, sched_distance=5, max_hoist_cost=4):
     Returns this lane's share of sum_pol sum_{s s'} a_s C a_s'^*; the caller adds the four lanes.  Counts are per LANE and
     event (executed, with the loop-invariant prologue once)."""
     g = gen.g
+    NL = gen.nl
     stores = [it[2] for it in gen.prog if it[0] == "store"]
     pro_ids, body_ids, hoisted = g.plan([gen.out] + stores, max_hoist_cost)
     body_set = set(body_ids)
-    nh = 16
+    nh = 1 << NL
     pro, body = g.count_list(pro_ids), g.count_list(body_ids)
     tot = {k: pro[k] + nh * (body[k] + (1 if k == "add" else 0)) for k in pro}
     leaf = lambda j: g.nodes[j][0] in ("in", "sym")
@@ -254,13 +259,14 @@ def emit_lanes(gen, fname, sched_window=48, sched_distance=5, max_hoist_cost=4):
     vslot = {j: n for n, j in enumerate(parked)}
     n_ev = len(gen.input_names) - 4 * NL            # per-event scalars in front of the gluon momenta
     assert gen.input_names[n_ev] == "k0e" and n_ev == 15
+    wrap = "& 3" if NL == 4 else "%% %d" % NL
     in_index = {}
     for idx, n in enumerate(gen.input_names):
         in_index[n] = "%d" % idx if idx < n_ev else "ko%d + %d" % ((idx - n_ev) // 4, (idx - n_ev) % 4)
     U = fname.upper()
     L = ["// GENERATED by paper_2105_10529_b200/gen/lanes.py -- do not edit.",
-         "// one event over four lanes; per LANE and event (executed): %d add, %d mul, %d fma, %d rcp  (flops = add + mul + 2 fma = %d)"
-         % (tot["add"], tot["mul"], tot["fma"], tot["rcp"], tot["add"] + tot["mul"] + 2 * tot["fma"]),
+         "// one event over %d lanes; per LANE and event (executed): %d add, %d mul, %d fma, %d rcp  (flops = add + mul + 2 fma = %d)"
+         % (NL, tot["add"], tot["mul"], tot["fma"], tot["rcp"], tot["add"] + tot["mul"] + 2 * tot["fma"]),
          "#define %s_NADD %dull" % (U, tot["add"]), "#define %s_NMUL %dull" % (U, tot["mul"]),
          "#define %s_NFMA %dull" % (U, tot["fma"]), "#define %s_NEV %d" % (U, n_ev + 4 * NL),
          "#define %s_SCALE %r" % (U, gen.scale), "#define %s_SLOTS %d" % (U, gen.n_slots), "#define %s_NV %d" % (U, len(parked))]
@@ -268,9 +274,9 @@ def emit_lanes(gen, fname, sched_window=48, sched_distance=5, max_hoist_cost=4):
     L.append("#if defined(__CUDACC__) || defined(MF_LANES_HOST_EMULATION)      // device code (warp barriers, shared-memory tile); the CPU test harness runs it on four host threads")
     L.append("#define MF_XL(s, k) X[(s) * 32 + xs##k]")
     L.append("template <typename T>")
-    L.append("MF_DEVFN T %s(const T* E, const T* G, T* X, T* V, const int lane4, const int xs0, const int xs1, const int xs2, const int xs3) {" % fname)
+    L.append("MF_DEVFN T %s(const T* E, const T* G, T* X, T* V, const int lane4, %s) {" % (fname, ", ".join("const int xs%d" % k for k in range(NL))))
     for i in range(NL):
-        L.append("  const int gl%d = (lane4 + %d) & 3, ko%d = %d + 4 * gl%d;" % (i, i, i, n_ev, i))
+        L.append("  const int gl%d = (lane4 + %d) %s, ko%d = %d + 4 * gl%d;" % (i, i, wrap, i, n_ev, i))
     L.append("  {      // loop invariants that are worth keeping: computed once, parked in V")
     used_pro = sorted({o for i in pro_ids for o in g._operands(i) if g.nodes[o][0] == "in"})
     for j in used_pro:

@@ -7,7 +7,10 @@ import numpy as np
 EE_MUMU, GG_TT, GG_TTG, GG_TTGG = 0, 1, 2, 3
 QQ_TT = 4                                      # q q~ -> t t~ summed over five light flavours
 PP_TT = 5                                      # p p -> t t~ at LO: g g -> t t~ and q q~ -> t t~ in one integrand
-PROCESS_NAMES = {EE_MUMU: "ee_mumu", GG_TT: "gg_tt", GG_TTG: "gg_ttg", GG_TTGG: "gg_ttgg", QQ_TT: "qq_tt", PP_TT: "pp_tt"}
+QQ_TTG = 6                                     # p p -> t t~ g through q q~ -> t t~ g (both beam orientations, five flavours)
+QG_TTQ = 7                                     # p p -> t t~ + quark jet through q g, g q, q~ g, g q~ -> t t~ q
+PROCESS_NAMES = {EE_MUMU: "ee_mumu", GG_TT: "gg_tt", GG_TTG: "gg_ttg", GG_TTGG: "gg_ttgg", QQ_TT: "qq_tt", PP_TT: "pp_tt",
+                 QQ_TTG: "qq_ttg", QG_TTQ: "qg_ttq"}
 PDF_NF = 11                                    # flavour tables of the 11-flavour grid, index = PDG id + 5 (b~ .. g .. b)
 
 GEN_CLASSIC_RAMBO, GEN_LINEAR_TAU = 1, 2      # `generator` flags; 0 = the generators of the configs
@@ -66,9 +69,9 @@ def config(process, seed=0, **over):
              pdf_qmin=PDF_QMIN, pdf_qmax=PDF_QMAX, generator=0)
     if process == EE_MUMU:
         c.update(sqrt_s=100.0, pdf_xf=None)
-    if process in (QQ_TT, PP_TT):
+    if process in (QQ_TT, PP_TT, QQ_TTG, QG_TTQ):
         c.update(pdf_xf=synthetic_flavour_grid())
-    if process in (GG_TTG, GG_TTGG):
+    if process in (GG_TTG, GG_TTGG, QQ_TTG, QG_TTQ):      # cuts of config 2 on the third final particle (gluon / light-quark jet)
         c.update(ptmin_g=30.0, etamax_g=2.5)
     if process == GG_TTGG:
         c.update(drmin_gg=0.4)

@@ -76,6 +76,8 @@ extern "C" double mfh_event(const MfParams* P, const double* edges, const double
     case 2: return run<2>(*P, edges, pdf, it, ev, bins, pass, rec_out);
     case 4: return run<4>(*P, edges, pdf, it, ev, bins, pass, rec_out);   // pdf: the library's flavour slice (mfh_flavour_slice)
     case 5: return run<5>(*P, edges, pdf, it, ev, bins, pass, rec_out);
+    case 6: return run<6>(*P, edges, pdf, it, ev, bins, pass, rec_out);
+    case 7: return run<7>(*P, edges, pdf, it, ev, bins, pass, rec_out);
 #ifndef MFH_NO_TTGG
     case 3: return run<3>(*P, edges, pdf, it, ev, bins, pass, rec_out);
 #endif
@@ -120,6 +122,8 @@ extern "C" double mfh_event_gen(const MfParams* P, const double* edges, const do
     case 5: return cl ? run_gen<5, 1>(*P, edges, pdf, it, ev, bins, pass, rec_out) : run_gen<5, 2>(*P, edges, pdf, it, ev, bins, pass, rec_out);
     case 4: return cl ? run_gen<4, 1>(*P, edges, pdf, it, ev, bins, pass, rec_out) : run_gen<4, 2>(*P, edges, pdf, it, ev, bins, pass, rec_out);
     case 2: return cl ? run_gen<2, 1>(*P, edges, pdf, it, ev, bins, pass, rec_out) : run_gen<2, 2>(*P, edges, pdf, it, ev, bins, pass, rec_out);
+    case 6: return cl ? run_gen<6, 1>(*P, edges, pdf, it, ev, bins, pass, rec_out) : run_gen<6, 2>(*P, edges, pdf, it, ev, bins, pass, rec_out);
+    case 7: return cl ? run_gen<7, 1>(*P, edges, pdf, it, ev, bins, pass, rec_out) : run_gen<7, 2>(*P, edges, pdf, it, ev, bins, pass, rec_out);
 #ifndef MFH_NO_TTGG
     case 3: return cl ? run_gen<3, 1>(*P, edges, pdf, it, ev, bins, pass, rec_out) : run_gen<3, 2>(*P, edges, pdf, it, ev, bins, pass, rec_out);
 #endif

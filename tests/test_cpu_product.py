@@ -137,6 +137,48 @@ def test_four_lane_decomposition_matches_oracle(mfo):
             assert abs(v1 / ref - 1) < 1e-11
 
 
+def test_two_quark_line_generator_matches_oracle(mfo):
+    """gen/quarks.py (q q~ -> t t~ g, q g -> t t~ q: four colour structures, linear polarisations, generic external lines)
+    evaluated with NumPy against the oracle's five explicit diagrams with the literal colour sum, on the basic channel and on the
+    beam-exchanged + charge-conjugated one"""
+    from paper_2105_10529_b200.gen import amplitudes as A, quarks as Q
+    num, den = Q.colour_matrix_2q()
+    assert den == 9 and (num == num.T).all() and num[0][0] == num[1][1] and num[2][2] == num[3][3]
+    gs2 = 4 * math.pi * 0.118
+    rng = np.random.default_rng(29)
+    for kind, proc in (("qq", W.QQ_TTG), ("qg", W.QG_TTQ)):
+        gen = Q.Gen2Q(kind)
+        gen.build()
+        assert len(gen.input_names) == 41
+        for trial in range(3):
+            rts = rng.uniform(450, 4000)
+            ps = mfo.phase_space(3, rts * rts, [173.0, 173.0, 0.0], rng.uniform(0.03, 0.97, 5))
+            mom = np.vstack([[rts / 2, 0, 0, rts / 2], [rts / 2, 0, 0, -rts / 2], ps["k"]])
+            for swap in (False, True):
+                m = mom.copy()
+                if swap:
+                    m[[0, 1]] = m[[1, 0]]; m[[2, 3]] = m[[3, 2]]
+                pa, pb, k1, k2, k3 = m
+                v = dict(mt=173.0)
+                for n, c in zip("exyz", k2): v["k2" + n] = c
+                for n, c in zip(("wp", "wm", "c0", "cx", "cy"), _ferm(k1, 173.0)): v["t_" + n] = c
+                for n, c in zip(("wp", "wm", "c0", "cx", "cy"), _ferm(k2, 173.0)): v["b_" + n] = c
+                pr, K, kg = (pb, -k3, k3) if kind == "qq" else (-k3, pb, pb)
+                for n, c in zip("exyz", pa): v["pc" + n] = c
+                for n, c in zip("exyz", pr): v["pr" + n] = c
+                for n, c in zip("exyz", K): v["K" + n] = c
+                for n, c in zip(("wp", "wm", "c0", "cx", "cy"), _ferm(pa, 0.0)): v["c_" + n] = c
+                for n, c in zip(("wp", "wm", "c0", "cx", "cy"), _ferm(pb if kind == "qq" else k3, 0.0)): v["r_" + n] = c
+                if math.hypot(kg[1], kg[2]) == 0:
+                    e1, e2 = [1.0, 0.0, 0.0], [0.0, 1.0 if kg[3] >= 0 else -1.0, 0.0]
+                else:
+                    e = np.array(_glu(kg)) * math.sqrt(2); e1, e2 = e[:3], [e[3], e[4], 0.0]
+                for n, c in zip("xyz", e1): v["e1" + n] = c
+                for n, c in zip("xyz", e2): v["e2" + n] = c
+                val = float(A.evaluate(gen, {k: x for k, x in v.items() if k in gen.input_names})) * gen.scale * gs2 ** 3
+                assert abs(val / mfo.me2_2q(proc, m) - 1) < 1e-12
+
+
 def test_generator_colour_matrices_match_golden():
     from paper_2105_10529_b200.gen import amplitudes as A
     from conftest import read_golden

@@ -639,3 +639,67 @@ def test_streams_and_stage_time_sums(mf):
     assert fb["min"] == 11302 and fb["executed"] == a.me_flops()["flops"] == 15023
     fb = mf.Vegas(W.config(W.GG_TTGG)).me_flops_bounds()
     assert fb["min"] == 170880 < 256020 < fb["executed"]
+
+
+# ---- channels with a second quark line and one gluon: q q~ -> t t~ g (6), q g -> t t~ q (7) -----------------
+@pytest.mark.parametrize("proc,gen,n", [(6, 0, 3001), (6, 3, 2001), (7, 0, 3001), (7, 1, 2001)])
+def test_two_quark_line_channels_per_event_parity(mf, mfo, proc, gen, n):
+    cfg = W.config(proc, seed=8, generator=gen)
+    gpu, orc = mf.Vegas(cfg), mfo.Vegas(cfg)
+    assert gpu.d == orc.d == (14 if gen & 1 else 7) and gpu.n_final == 3
+    mom_tol = (1e-10, 1e-8) if gen & 1 else (1e-11, 1e-9)
+    ref = orc.eval(0, 0, n, n_threads=mfo.max_threads())
+    # the luminosity record (sums of ten or more products of O(1) interpolants) carries an absolute error of ~1e-14
+    compare_events(gpu.integrand_eval(0, 0, n, debug=True), ref, 0, mom_tol, lumi_abs=4e-14)
+    e = random_grid(orc.d, 50, 400 + proc)
+    gpu.set_grid(e); orc.set_grid(e)
+    ref = orc.eval(3, 2**33 + 5, n, n_threads=mfo.max_threads())
+    out = gpu.integrand_eval(3, 2**33 + 5, n, debug=True)
+    compare_events(out, ref, 0, mom_tol, lumi_abs=4e-14)
+    np.testing.assert_allclose(out["pdf"].cpu().numpy(), ref["pdf"], rtol=1e-12, atol=1e-14)
+    assert 0.5 < ref["pass_"].mean() < 0.999                  # the cuts act on the third final particle
+
+
+@pytest.mark.parametrize("proc", [W.QQ_TTG, W.QG_TTQ])
+def test_two_quark_line_channels_iterations_and_errors(mf, mfo, proc):
+    """fused iterations against the oracle (raw sums, histogram, pass counter, grid), observables incl. the jet pT, full-size
+    launch with sampled events, argument errors"""
+    cfg = W.config(proc, seed=0)
+    gpu, orc = mf.Vegas(cfg), mfo.Vegas(cfg)
+    obs = [(0, 20, 0.0, 400.0), (3, 10, 30.0, 230.0)]
+    gpu.set_observables(obs)
+    n = 30_000
+    ref = [(np.zeros(o[1] + 2), np.zeros(o[1] + 2)) for o in obs]
+    for it in range(3):
+        for (a, b), (r1, r2) in zip(orc.observable_hist(it, 0, n, n, obs, n_threads=mfo.max_threads()), ref):
+            r1 += a; r2 += b
+        g = gpu.vegas_iterate(n)
+        o = orc.iterate(n, n_threads=mfo.max_threads())
+        assert g["n_pass"] == o["n_pass"] and g["n_nonfinite"] == 0 == o["n_nonfinite"]
+        assert abs(g["integral"] / o["integral"] - 1) < RTOL_INT and abs(g["sigma"] / o["sigma"] - 1) < 1e-8
+        np.testing.assert_allclose(gpu.get_accum()[0][:2 + 7 * 50], orc.get_accum(), rtol=RTOL_INT, atol=1e-300)
+        np.testing.assert_allclose(gpu.get_grid(), orc.get_grid(), rtol=0, atol=1e-11)
+        gpu.set_grid(orc.get_grid())
+    got, n_it = gpu.get_observables()
+    for (g1, g2), (r1, r2) in zip(got, ref):
+        np.testing.assert_allclose(g1, r1, rtol=1e-10, atol=1e-13 * np.abs(r1).max())
+        np.testing.assert_allclose(g2, r2, rtol=1e-10, atol=1e-13 * np.abs(r2).max())
+    # full-size launch (1e6 events per iteration): raw sums == sums of the eval kernel's weights; sampled events == oracle
+    n = 1_000_000
+    gpu, orc = mf.Vegas(cfg), mfo.Vegas(cfg)
+    g = gpu.vegas_iterate(n)
+    acc, cnt = gpu.get_accum()
+    w = mf.Vegas(cfg).integrand_eval(0, 0, n)["weight"]
+    t = w / n
+    assert abs(float(t.sum()) / acc[0] - 1) < 1e-10 and abs(float((t * t).sum()) / acc[1] - 1) < 1e-10
+    assert int((w != 0).sum()) == cnt[0] and g["n_nonfinite"] == 0
+    for i in (0, 1, 255, 256, 65_537, n // 2 + 1, n - 1):
+        r = orc.eval(0, i, 1)["weight"][0]
+        assert (r == 0 and float(w[i]) == 0) or abs(float(w[i]) / r - 1) < RTOL_EVENT
+    with pytest.raises(mf.MfError) as e:
+        gpu.set_path(True)                                    # fused path only
+    assert e.value.code == mf.MF_EUNSUPPORTED
+    for bad in (W.config(proc, pdf_xf=W.synthetic_gluon_grid()), W.config(proc, precision=32)):
+        with pytest.raises(mf.MfError):
+            mf.Vegas(bad)
+    assert gpu.me_flops()["flops"] == (2 if proc == W.QQ_TTG else 4) * (5636 + 2)

@@ -151,6 +151,43 @@ def flavour_slice(harness, P, pdf11):
     return out
 
 
+@pytest.mark.parametrize("proc,gen,n", [(6, 0, 200), (6, 3, 100), (7, 0, 200), (7, 1, 100)])
+def test_host_compiled_two_quark_line_channels_match_oracle(mfo, harness, proc, gen, n):
+    """q q~ -> t t~ g (6) and q g -> t t~ q (7): the product's per-event code compiled for the host against the
+    oracle: bins, cut flags, momenta, the luminosity record, the luminosity-weighted |M|^2 and the weight"""
+    harness.mfh_event_gen.restype = C.c_double
+    harness.mfh_event_gen.argtypes = harness.mfh_event.argtypes
+    cfg = W.config(proc, seed=17, generator=gen)
+    c, pdf = make_config(cfg)
+    P = C.create_string_buffer(harness.mfh_params_size())
+    assert harness.mfh_fill_params(C.byref(c), P) == 0
+    tab = flavour_slice(harness, P, pdf)
+    orc = mfo.Vegas(cfg)
+    d = orc.d
+    assert d == (14 if gen & 1 else 7)
+    edges = random_grid(d, 50, 41)
+    orc.set_grid(edges)
+    ref = orc.eval(2, 900, n)
+    bins = np.zeros(24, np.int32); ok = np.zeros(1, np.int32); rec = np.zeros(45)
+    worst, n_pass = 0.0, 0
+    for i in range(n):
+        F = harness.mfh_event_gen(P, edges.ctypes.data, tab.ctypes.data, 2, 900 + i, bins.ctypes.data, ok.ctypes.data, rec.ctypes.data)
+        assert list(bins[:d]) == list(ref["bins"][i]) and ok[0] == ref["pass_"][i]
+        np.testing.assert_allclose(rec[:d], ref["x"][i], rtol=1e-14, atol=0)
+        np.testing.assert_allclose(rec[18:38].reshape(5, 4), ref["momenta"][i], rtol=1e-10, atol=1e-8)
+        np.testing.assert_allclose(rec[43:45], ref["pdf"][i], rtol=1e-12, atol=1e-16)
+        if ref["weight"][i] != 0:
+            n_pass += 1
+            worst = max(worst, abs(F / ref["weight"][i] - 1), abs(rec[42] / ref["me2"][i] - 1))
+        else:
+            assert F == 0.0
+    assert worst < 1e-10 and n_pass > n // 2, (worst, n_pass)
+    if gen == 0:                                              # and through the plain entry point
+        rec37 = np.zeros(37)
+        F = harness.mfh_event(P, edges.ctypes.data, tab.ctypes.data, 2, 900, bins.ctypes.data, ok.ctypes.data, rec37.ctypes.data)
+        assert F == 0.0 and ref["weight"][0] == 0 or abs(F / ref["weight"][0] - 1) < 1e-10
+
+
 @pytest.mark.parametrize("proc,gen,n", [(4, 0, 300), (4, 1, 150), (4, 2, 150), (5, 0, 300), (5, 3, 150)])
 def test_host_compiled_quark_channel_matches_oracle(mfo, harness, proc, gen, n):
     """q q~ -> t t~ with the flavour-summed luminosity of the product's per-event code, compiled for

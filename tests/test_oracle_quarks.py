@@ -163,3 +163,120 @@ def test_pp_tt_is_the_sum_of_its_subprocesses(mfo):
         v.iterate(100_000, n_threads=mfo.max_threads())
     r = v.result()
     assert abs(r["integral"] - (1074.393 + 79.96)) < 4 * r["sigma"] + 0.03 and r["sigma"] < 1.5, r
+
+
+# ---- the channels with a second quark line and one gluon: q q~ -> t t~ g (process 6), q g -> t t~ q (process 7) ------------
+# oracle/mfo_amp2q.cpp writes the five diagrams out with explicit gamma matrices and the literal colour sum.  Pins: the Ward
+# identity of the external gluon; the four initial-state collinear limits, which tie both processes to the CLOSED FORMS of
+# q q~ -> t t~ and g g -> t t~ through the textbook (unregularised, azimuth-averaged) Altarelli-Parisi functions
+#   |M_{n+1}|^2 -> (2 g_s^2 / (2 p.k)) P(x)/x |M_n(x p, p')|^2,  x = (p + p' - k)^2 / shat:
+#   q -> q(x) g:  P_qq = C_F (1 + x^2)/(1 - x)      q -> g(x) q:  P_gq = C_F (1 + (1 - x)^2)/x      g -> q(x) q~:  P_qg = T_R (x^2 + (1 - x)^2)
+# (coupling power, colour factors C_F = 4/3 and T_R = 1/2, the 1/36 and 1/96 averages and the relative signs of the diagrams
+# all enter); Lorentz invariance; positivity; and the cross sections through both oracle generators.
+def gg_tt_closed_form(mom, m=MT, alpha_s=AS):
+    g4 = (4 * math.pi * alpha_s) ** 2
+    s = mdot(mom[0] + mom[1], mom[0] + mom[1])
+    t1 = 2 * mdot(mom[0], mom[2]) / s; t2 = 2 * mdot(mom[1], mom[2]) / s; rho = 4 * m * m / s
+    return g4 * (1 / (6 * t1 * t2) - 3 / 8) * (t1 * t1 + t2 * t2 + rho - rho * rho / (4 * t1 * t2))
+
+
+def boost_from_rest(p, K):
+    M = math.sqrt(mdot(K, K)); E = (K[0] * p[0] + K[1:] @ p[1:]) / M
+    return np.array([E, *(p[1:] + K[1:] * (p[0] + E) / (K[0] + M))])
+
+
+def three_body(mfo, rts, rs):
+    ks = mfo.phase_space(3, rts * rts, [MT, MT, 0.0], rs)["k"]
+    return np.vstack([[rts / 2, 0, 0, rts / 2], [rts / 2, 0, 0, -rts / 2], ks])
+
+
+def test_two_quark_lines_ward_identity_lorentz_and_positivity(mfo):
+    rng = np.random.default_rng(31)
+    for proc in (W.QQ_TTG, W.QG_TTQ):
+        for _ in range(6):
+            mom = three_body(mfo, math.exp(rng.uniform(math.log(450.0), math.log(6000.0))), rng.uniform(0.03, 0.97, 5))
+            ref = mfo.me2_2q(proc, mom)
+            assert ref > 0 and mfo.me2(proc, mom) == ref
+            assert abs(mfo.me2_2q(proc, mom, ward=1)) < 1e-9 * ref          # eps -> k: the five diagrams cancel
+            ch, sh, c, s = math.cosh(0.6), math.sinh(0.6), math.cos(0.8), math.sin(0.8)
+            lor = mom.copy()
+            lor[:, 0] = ch * mom[:, 0] + sh * mom[:, 3]; z = sh * mom[:, 0] + ch * mom[:, 3]
+            lor[:, 2] = c * mom[:, 2] - s * z; lor[:, 3] = s * mom[:, 2] + c * z
+            assert np.isclose(mfo.me2_2q(proc, lor), ref, rtol=1e-10)        # boost along z, rotation about x
+
+
+def collinear_ratio(mfo, proc, side, born, split, rts, x, theta):
+    """azimuth average of |M_{n+1}|^2 / [ (2 g^2 / (2 p.k)) P(x')/x' |M_n|^2 ] for the emitted parton k at angle theta to beam `side`"""
+    E = rts / 2
+    pa, pb = np.array([E, 0, 0, E]), np.array([E, 0, 0, -E])
+    gs2 = 4 * math.pi * AS
+    acc = 0.0
+    for j in range(8):
+        phi = 0.37 + 2 * math.pi * j / 8
+        k = (1 - x) * E * np.array([1, math.sin(theta) * math.cos(phi), math.sin(theta) * math.sin(phi), (1 if side == 0 else -1) * math.cos(theta)])
+        K = pa + pb - k
+        M = math.sqrt(mdot(K, K))
+        b = tt_momenta(M, 0.3, 1.1)
+        mom = np.array([pa, pb, boost_from_rest(b[2], K), boost_from_rest(b[3], K), k])
+        xx = M * M / rts ** 2
+        acc += mfo.me2_2q(proc, mom) / (2 * gs2 / (2 * mdot(pa if side == 0 else pb, k)) * split(xx) / xx * born(b))
+    return acc / 8
+
+
+def test_two_quark_lines_collinear_limits_tie_to_closed_forms(mfo):
+    CF, TR = 4.0 / 3.0, 0.5
+    p_qq = lambda x: CF * (1 + x * x) / (1 - x)
+    p_gq = lambda x: CF * (1 + (1 - x) ** 2) / x
+    p_qg = lambda x: TR * (x * x + (1 - x) ** 2)
+    cases = [(W.QQ_TTG, 0, qq_tt_closed_form, p_qq),      # g || q:   q -> q g,   hard q q~ -> t t~
+             (W.QQ_TTG, 1, qq_tt_closed_form, p_qq),      # g || q~
+             (W.QG_TTQ, 0, gg_tt_closed_form, p_gq),      # outgoing q || incoming q: q -> g q, hard g g -> t t~
+             (W.QG_TTQ, 1, qq_tt_closed_form, p_qg)]      # outgoing q || incoming g: g -> q~ q, hard q q~ -> t t~
+    for proc, side, born, split in cases:
+        for rts, x in ((1100.0, 0.65), (3000.0, 0.3)):
+            d2, d3 = (collinear_ratio(mfo, proc, side, born, split, rts, x, th) - 1 for th in (1e-2, 1e-3))
+            assert abs(d3) < 5e-6 and abs(d2) < 5e-4, (proc, side, rts, x, d2, d3)     # approached like theta^2
+
+
+def test_two_quark_lines_integrand_chain(mfo):
+    """the event weight of processes 6 and 7 rebuilt here from the oracle's per-event records and single calls: luminosities from
+    single-table interpolations, the channels' |M|^2 from mfo_me2_2q on relabelled momenta (beam exchange, t <-> t~)"""
+    for proc in (W.QQ_TTG, W.QG_TTQ):
+        cfg = W.config(proc, seed=2)
+        orc = mfo.Vegas(cfg)
+        assert orc.d == 7 and orc.n_final == 3
+        ev = orc.eval(1, 100, 40)
+        xf = cfg["pdf_xf"]
+        pdf = lambda f, x: mfo.pdf_interp(xf[5 + f], W.PDF_XMIN, W.PDF_XMAX, W.PDF_QMIN, W.PDF_QMAX, x, cfg["mu_f"] ** 2)
+        ref2 = mfo.Vegas(W.config(W.GG_TTG, seed=2, pdf_xf=xf[5])).eval(1, 100, 40)      # same kinematics, cuts and Jacobians
+        np.testing.assert_array_equal(ev["pass_"], ref2["pass_"])
+        np.testing.assert_array_equal(ev["momenta"], ref2["momenta"])
+        for i in range(40):
+            mom = ev["momenta"][i]
+            shat = 4 * mom[0][0] ** 2
+            # x1, x2 from the records of the gluon run: weight_gg = J ... xg(x1) xg(x2)/(x1 x2) |M_gg|^2 ...
+            y0, y1 = ev["x"][i][0], ev["x"][i][1]
+            tau0 = (2 * MT + 30.0) ** 2 / 13000.0 ** 2
+            tau = tau0 ** (1 - y0); x1 = tau ** y1; x2 = tau / x1
+            assert np.isclose(tau * 13000.0 ** 2, shat, rtol=1e-12)
+            beams = mom.copy(); beams[[0, 1]] = mom[[1, 0]]
+            cc = mom.copy(); cc[[2, 3]] = mom[[3, 2]]
+            both = beams.copy(); both[[2, 3]] = beams[[3, 2]]
+            if proc == W.QQ_TTG:
+                lum = [sum(pdf(f, x1) * pdf(-f, x2) for f in range(1, 6)), sum(pdf(-f, x1) * pdf(f, x2) for f in range(1, 6))]
+                me = [mfo.me2_2q(proc, mom), mfo.me2_2q(proc, beams)]
+                np.testing.assert_allclose(ev["pdf"][i], lum, rtol=1e-13)
+            else:
+                q1 = sum(pdf(f, x1) for f in range(1, 6)); a1 = sum(pdf(-f, x1) for f in range(1, 6))
+                q2 = sum(pdf(f, x2) for f in range(1, 6)); a2 = sum(pdf(-f, x2) for f in range(1, 6))
+                lum = [q1 * pdf(0, x2), pdf(0, x1) * q2, a1 * pdf(0, x2), pdf(0, x1) * a2]
+                me = [mfo.me2_2q(proc, mom), mfo.me2_2q(proc, beams), mfo.me2_2q(proc, cc), mfo.me2_2q(proc, both)]
+                np.testing.assert_allclose(ev["pdf"][i], [lum[0] + lum[2], lum[1] + lum[3]], rtol=1e-13)
+            if not ev["pass_"][i]:
+                assert ev["weight"][i] == 0.0
+                continue
+            tot = sum(l * m for l, m in zip(lum, me))
+            assert np.isclose(ev["me2"][i], tot / sum(lum), rtol=1e-12)
+            # everything but luminosity x |M|^2 is the gluon run's factor: F / (L |M|^2) agrees between the two processes
+            gg = ref2["weight"][i] / (ref2["pdf"][i][0] * ref2["pdf"][i][1] * ref2["me2"][i])
+            assert np.isclose(ev["weight"][i] / tot, gg, rtol=1e-12)

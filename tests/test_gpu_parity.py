@@ -649,13 +649,13 @@ def test_two_quark_line_channels_per_event_parity(mf, mfo, proc, gen, n):
     assert gpu.d == orc.d == (14 if gen & 1 else 7) and gpu.n_final == 3
     mom_tol = (1e-10, 1e-8) if gen & 1 else (1e-11, 1e-9)
     ref = orc.eval(0, 0, n, n_threads=mfo.max_threads())
-    # the luminosity record (sums of ten or more products of O(1) interpolants) carries an absolute error of ~1e-14
-    compare_events(gpu.integrand_eval(0, 0, n, debug=True), ref, 0, mom_tol, lumi_abs=4e-14)
+    # the luminosity record: the absolute-error term of the quark channel (DESIGN.md 5.9 / section 6)
+    compare_events(gpu.integrand_eval(0, 0, n, debug=True), ref, 0, mom_tol, lumi_abs=2e-14)
     e = random_grid(orc.d, 50, 400 + proc)
     gpu.set_grid(e); orc.set_grid(e)
     ref = orc.eval(3, 2**33 + 5, n, n_threads=mfo.max_threads())
     out = gpu.integrand_eval(3, 2**33 + 5, n, debug=True)
-    compare_events(out, ref, 0, mom_tol, lumi_abs=4e-14)
+    compare_events(out, ref, 0, mom_tol, lumi_abs=2e-14)
     np.testing.assert_allclose(out["pdf"].cpu().numpy(), ref["pdf"], rtol=1e-12, atol=1e-14)
     assert 0.5 < ref["pass_"].mean() < 0.999                  # the cuts act on the third final particle
 

@@ -116,6 +116,21 @@ MF_HD T mf_me2(const MfParams& P, T rts, const T k[MfProc<PROC>::N][4]) {
   }
 }
 
+// gg -> t t~ g with the loop-entering values of the helicity loop in shared memory (W: the thread's column of a [slot][S] tile)
+#if defined(__CUDACC__)
+template <typename T, int S>
+__device__ __forceinline__ T mf_me2_ttg_smem(const MfParams& P, T rts, const T k[3][4], T* W) {
+  static_assert(MF_ME2_GG_TTG_NIN == 29, "generator input layout changed");
+  {
+    T in[29];
+    mf_me_inputs_gg<3, T>(rts, T(P.m_top), k, in);
+#pragma unroll
+    for (int i = 0; i < 29; ++i) W[i * S] = in[i];
+  }
+  return T(P.me_pref) * mf_me2_gg_ttg_s<T, S>(W);
+}
+#endif
+
 // ---- gg -> t t~ g g: one event over FOUR LANES (gen/lanes.py) -----------------------------------
 // The four lanes of a group (lane & 3 = 0..3 of consecutive lanes) hold the same event (rts, k).  Lane l takes the
 // six colour orderings that end with gluon l and runs the generated per-lane code on cyclically relabelled gluons

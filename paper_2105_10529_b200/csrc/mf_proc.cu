@@ -351,6 +351,7 @@ mf_front_kernel(const MfParams P, const double* __restrict__ g_edges, const doub
 #ifndef MF_ME_THREADS_F32
 #define MF_ME_THREADS_F32 384        // CTA size of the fp32 variant (168 registers per thread; tuned, profiles/r1_tuning.md)
 #endif
+#define MF_TTG_SMEM 1                // gg -> tt~g |M|^2 stage: loop-entering values in shared memory (mf_me2_ttg_smem)
 #ifndef MF_ME_THREADS
 #define MF_ME_THREADS 256            // CTA size of the |M|^2 stage (one CTA per SM; registers = 65536 / threads)
 #endif
@@ -361,6 +362,7 @@ mf_me_kernel(const MfParams P, double* __restrict__ rec, const unsigned int* __r
              unsigned long long cap) {
   constexpr int N = MfProc<PROC>::N, NF = MF_REC_FIELDS(N), T = THREADS;
   constexpr bool LANES = PROC == 3;                      // gg -> tt~gg: one event over four lanes (mf_me2_ttgg_group)
+  constexpr bool SMEMOPS = PROC == 2 && MF_TTG_SMEM && std::is_same<Real, double>::value;   // gg -> tt~g: loop-entering values in shared memory
   extern __shared__ unsigned int s_pre[];                // [regions + 1] exclusive prefix, then s_part[T], then the lane tiles
   unsigned int* s_part = s_pre + regions + 1;
   const unsigned tid = threadIdx.x;
@@ -386,6 +388,7 @@ mf_me_kernel(const MfParams P, double* __restrict__ rec, const unsigned int* __r
   const unsigned nchunks = (M + EPC - 1) / EPC;
   Real* tile = nullptr;
   if constexpr (LANES) tile = (Real*)(s_pre + ((regions + 1 + T + 1) & ~1)) + (size_t)(tid >> 5) * MF_LANES_TILE;
+  if constexpr (SMEMOPS) tile = (Real*)(s_pre + ((regions + 1 + T + 1) & ~1)) + tid;
 #if MF_ME_STAGGER > 0
   if (group > 0) { const long long t0 = clock64(); while (clock64() - t0 < (long long)MF_ME_STAGGER * group) { } }
 #endif
@@ -404,6 +407,7 @@ mf_me_kernel(const MfParams P, double* __restrict__ rec, const unsigned int* __r
     const double rts = R[(size_t)(4 * N) * cap], pref = R[(size_t)(4 * N + 1) * cap];
     double F;                                            // S7, S8
     if constexpr (LANES) F = pref * (double)mf_me2_ttgg_group<Real>(P, (Real)rts, k, tile);
+    else if constexpr (SMEMOPS) F = pref * (double)mf_me2_ttg_smem<Real, T>(P, (Real)rts, k, tile);
     else F = pref * (double)mf_me2<PROC, Real>(P, (Real)rts, k);
     if (have && (!LANES || (tid & 3u) == 0u)) R[(size_t)(4 * N + 1) * cap] = F;
   }
@@ -641,7 +645,11 @@ static size_t hist_smem(const MfParams& P) {
   return sizeof(double) * (MF_THREADS / 32) * ((size_t)P.d * P.nb + 4 + (P.n_obs > 0 ? MF_OBS_ACC : 0));
 }
 
-static size_t me_tile_bytes(int threads) { return MF_PROC == 3 ? sizeof(double) * (threads / 32) * MF_LANES_TILE + 8 : 0; }
+static size_t me_tile_bytes(int threads) {
+  if (MF_PROC == 3) return sizeof(double) * (threads / 32) * MF_LANES_TILE + 8;
+  if (MF_PROC == 2 && MF_TTG_SMEM) return sizeof(double) * MF_ME2_GG_TTG_NW * threads + 8;
+  return 0;
+}
 static cudaError_t proc_staged_setup(const MfParams& P, int* rec_fields, int* occ_front, int* occ_hist) {
   *rec_fields = kStaged ? kRecFields : 0;
   *occ_front = *occ_hist = 0;
@@ -653,7 +661,7 @@ static cudaError_t proc_staged_setup(const MfParams& P, int* rec_fields, int* oc
     return r ? r : cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_front, mf_front_kernel<MF_PROC, G>, MF_THREADS, front_smem(P));
   });
   if (e) return e;
-  e = cudaFuncSetAttribute(mf_me_kernel<MF_PROC, double, MF_ME_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024 + (int)me_tile_bytes(MF_ME_THREADS));
+  e = cudaFuncSetAttribute(mf_me_kernel<MF_PROC, double, MF_ME_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 32 * 1024 + (int)me_tile_bytes(MF_ME_THREADS));
   if (e) return e;
   if constexpr (kF32) {
     e = cudaFuncSetAttribute(mf_me_kernel<MF_PROC, float, MF_ME_THREADS_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
@@ -683,7 +691,7 @@ static cudaError_t proc_staged(const MfParams& P, const double* edges, const dou
   });
   if (e) return e;
   if (ev && (e = cudaEventRecord(ev[1], st))) return e;
-  const size_t sm = sizeof(unsigned int) * ((size_t)ws.regions + 1 + (f32 ? MF_ME_THREADS_F32 : MF_ME_THREADS)) + me_tile_bytes(MF_ME_THREADS);
+  const size_t sm = sizeof(unsigned int) * ((size_t)ws.regions + 1 + (f32 ? MF_ME_THREADS_F32 : MF_ME_THREADS)) + (f32 ? 0 : me_tile_bytes(MF_ME_THREADS));   // (the fp32 variant keeps its operands in registers)
   if (f32) {
     if constexpr (kF32) mf_me_kernel<MF_PROC, float, MF_ME_THREADS_F32><<<grid_me, MF_ME_THREADS_F32, sm, st>>>(P, ws.rec, ws.count, ws.regions, ws.cap);
     else return cudaErrorNotSupported;

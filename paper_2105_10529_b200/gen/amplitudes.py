@@ -492,6 +492,59 @@ def emit_function(gen, fname):
     return "\n".join(L) + "\n", tot
 
 
+def emit_function_smem(gen, fname, clobber_every=256, max_hoist_cost=2):
+    """The same helicity-loop function with its loop-entering values in SHARED MEMORY instead of registers:
+        template <typename T, int S> T fname_s(T* W)
+    W: the thread's column of a [slot][S] tile (S = threads of the CTA: conflict-free): slots 0..NIN-1 hold the inputs, the
+    following NV slots receive the hoisted loop invariants.  The body re-reads them where they are used; a compiler barrier
+    every `clobber_every` statements keeps the loads from being hoisted to the loop head (where they would be spilled again)
+    while letting the compiler share a loaded value inside a stretch.  With ~50 doubles out of the register file the body
+    has the register file to itself: no spills at 255 registers (672 B before), |M|^2 stage of gg -> tt~g 5.64 -> 5.40 ms per
+    1e7 events (profiles/r2_tuning.md; 384 threads at 168 registers still spill 1.2 KB and take 8.0 ms)."""
+    g, out = gen.g, gen.out
+    nh = len(gen.loop_assign)
+    pro_ids, body_ids, hoisted = g.plan([out], max_hoist_cost)     # parking costs shared memory, not registers: hoist more
+    body_set = set(body_ids)
+    leaf = lambda j: g.nodes[j][0] in ("in", "sym")
+    parked = sorted({o for i in body_ids for o in g._operands(i) if o not in body_set and not leaf(o)})
+    nin = len(gen.input_names)
+    slot = {j: nin + n for n, j in enumerate(parked)}
+    idx = {n: i for i, n in enumerate(gen.input_names)}
+    U = fname.upper()
+    L = ["#define %s_NW %d      // slots of the shared-memory tile of %s_s: inputs, then parked invariants" % (U, nin + len(parked), fname),
+         "#if defined(__CUDACC__)",
+         "template <typename T, int S>",
+         "__device__ __forceinline__ T %s_s(T* W) {" % fname,
+         "  {"]
+    used_pro = sorted({o for i in pro_ids for o in g._operands(i) if g.nodes[o][0] == "in"})
+    for j in used_pro:
+        L.append("    const T %s = W[%d * S];" % (g.names[j], idx[g.names[j]]))
+    pname = lambda j: g.names[j] if leaf(j) else "p%d" % j
+    L += g.emit_list(pro_ids, pname, "p", indent="    ")
+    for j in parked:
+        L.append("    W[%d * S] = p%d;" % (slot[j], j))
+    L += ["  }", "  T acc = T(0.0);", "#pragma unroll 1", "  for (int ih = 0; ih < %d; ++ih) {" % nh]
+    for b, l in enumerate(reversed(gen.loop_legs)):
+        L.append("    const T lam%d = (ih & %d) ? T(1.0) : T(-1.0);" % (l, 1 << b))
+
+    def bname(j):
+        if g.nodes[j][0] == "in":
+            return "W[%d * S]" % idx[g.names[j]]
+        if g.nodes[j][0] == "sym":
+            return g.names[j]
+        return "v%d" % j if j in body_set else "W[%d * S]" % slot[j]
+
+    body_ids = g.schedule(body_ids, SCHED_WINDOW, SCHED_DISTANCE)
+    for i, line in enumerate(g.emit_list(body_ids, bname, "v", indent="    ")):
+        if i % 64 == 0:
+            L.append("    MF_SYNC_POINT(%d);" % (i // 64))
+        if i % clobber_every == 0:
+            L.append("    asm volatile(\"\" ::: \"memory\");")
+        L.append(line)
+    L += ["    acc += %s;" % _ref(g, out, bname), "  }", "  return acc;", "}", "#endif"]
+    return "\n".join(L) + "\n"
+
+
 def _ref(g, r, name):
     if r.n is None:
         return g._k(r.c)
@@ -526,6 +579,10 @@ SYNC_MACRO = {}
 # emission order of the helicity-loop body (Dag.schedule): window 0 = creation order
 SCHED_WINDOW = 48
 SCHED_DISTANCE = 5
+# shared-memory-operand variant (emit_function_smem): statements between its compiler barriers (64 .. 1024: no difference on
+# the B200) and its hoisting threshold (none / 2 / 3 / 6: 5.42 / 5.39 / 5.40 / 5.46 ms; profiles/r2_tuning.md)
+SMEM_CLOBBER_EVERY = 256
+SMEM_HOIST_COST = 2
 
 
 def generate(fname):

@@ -27,6 +27,7 @@ from .dag import Dag, R, Cx, csum_prod
 from .amplitudes import Gen, colour_matrix
 
 NL = 4
+SYNC_STATEMENTS = 2048      # statements between the group barriers of the loop body (B200: 8.9 ms per 1e6 events; 1024: 9.25, 256: 9.4; profiles/r2_tuning.md)
 
 
 def _canon(pi):
@@ -308,8 +309,8 @@ def emit_lanes(gen, fname, sched_window=48, sched_distance=5, max_hoist_cost=4):
             if ids:
                 ids = g.schedule(ids, sched_window, sched_distance)
                 for line in g.emit_list(ids, bname, "v", indent="    "):
-                    if nstmt % 64 == 0:
-                        L.append("    MF_SYNC_POINT(%d);" % (nstmt // 64))
+                    if nstmt % SYNC_STATEMENTS == 0:      # group barrier: keeps the four warps of a group on the same I-cache lines
+                        L.append("    MF_SYNC_POINT(0);")
                     L.append(line)
                     nstmt += 1
         elif it[0] == "store":

@@ -206,6 +206,22 @@ int mf_me_flops(const mf_vegas_t *h, uint64_t *n_add, uint64_t *n_mul, uint64_t 
  * of mf_me_flops), and the flops the kernels EXECUTE per event for S7 (= mf_me_flops, except gg -> tt~gg: four lanes per
  * event, each with its own prologue and a share of recomputation).  mf_me_flops lies between the two.        */
 int mf_me_flops_bounds(const mf_vegas_t *h, uint64_t *flops_min, uint64_t *flops_executed);
+/* S9 (reading O9) as ONE entry point that ALLOCATES NOTHING -- no cudaMalloc, cudaFree or allocating library routine at
+ * any call, the first included -- for callers that cannot allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid it).  From n_events per-event weights F_i (dev_weight[n], as mf_integrand_eval writes them) and
+ * their VEGAS bins (dev_bins[n][d], uint8) it writes, or with accumulate != 0 adds, into the caller's DEVICE buffer
+ * dev_acc[2 + d*n_bins]:  sum_i t_i,  sum_i t_i^2,  H[j][k] = sum_{i in bin k of dimension j} t_i^2,  t_i = F_i / n_total
+ * -- the raw-sum vector of mf_vegas_accumulate / mf_set_accum_device (non-finite weights count as 0; fixed summation
+ * order for a given n_events).  It is a variant of the library's reduction stage whose scratch (one partial record per
+ * CTA) is a file-scope static __device__ array of 296 x (2 + 18 x 64) doubles = 2.7 MB that every GPU loading the library
+ * holds until exit.  Limits: d <= 18, n_bins <= 64 (MF_EINVAL beyond; n_events is not limited).  `device` = the CUDA
+ * ordinal the buffers live on.  Enqueue only; no synchronisation.  Every call shares the scratch array: calls that
+ * overlap on the GPU (different streams without ordering, several host threads) RACE on it -- issue them on one stream
+ * or order them with events.  Together with mf_integrand_eval, mf_set_accum_device and mf_vegas_finalize (none of
+ * which allocates) a whole iteration of any process runs without the on-demand workspace of mf_vegas_accumulate.      */
+int mf_reduce_weights_noalloc(int32_t device, const double *dev_weight, const uint8_t *dev_bins, uint64_t n_events,
+                              uint32_t d, uint32_t n_bins, double n_total, int32_t accumulate, double *dev_acc,
+                              void *cuda_stream);
 /* Register-resident DFMA-chain microbenchmark on `device`: measured fp64 FLOP/s (roofline peak).   */
 int mf_fp64_peak(int32_t device, double seconds, double *host_flops_per_s);
 const char *mf_last_error(void);

@@ -17,7 +17,7 @@ EXPORTS = ["mf_vegas_create", "mf_vegas_destroy", "mf_ndim", "mf_integrand_eval"
            "mf_get_iterations", "mf_get_grid", "mf_set_grid", "mf_set_launch", "mf_me_flops",
            "mf_fp64_peak", "mf_last_kernel_ms", "mf_last_error", "mf_set_path", "mf_last_stage_ms",
            "mf_set_observables", "mf_get_observables", "mf_accum_len", "mf_zero_accum", "mf_get_accum_device",
-           "mf_set_accum_device", "mf_stage_ms_sum", "mf_me_flops_bounds"]
+           "mf_set_accum_device", "mf_stage_ms_sum", "mf_me_flops_bounds", "mf_reduce_weights_noalloc"]
 
 
 class MfError(RuntimeError):
@@ -107,6 +107,7 @@ def lib():
         L.mf_last_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
         L.mf_stage_ms_sum.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(u32)]
         L.mf_me_flops_bounds.argtypes = [vp, C.POINTER(u64), C.POINTER(u64)]
+        L.mf_reduce_weights_noalloc.argtypes = [C.c_int32, vp, vp, u64, u32, u32, C.c_double, C.c_int32, vp, vp]
         L.mf_me_flops.argtypes = [vp, C.POINTER(u64), C.POINTER(u64), C.POINTER(u64)]
         L.mf_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
         L.mf_fp64_peak.argtypes = [C.c_int32, C.c_double, C.POINTER(C.c_double)]
@@ -287,6 +288,14 @@ class Vegas:
 def _iter_dict(it):
     return dict(integral=it.integral, sigma=it.sigma, n_events=it.n_events, n_pass=it.n_pass,
                 n_nonfinite=it.n_nonfinite, kernel_ms=it.kernel_ms)
+
+
+def reduce_weights_noalloc(weight_ptr, bins_ptr, n_events, d, n_bins, n_total, acc_ptr, accumulate=False, device=0, stream=None):
+    """mf_reduce_weights_noalloc: raw sums (sum t, sum t^2, d x n_bins histogram) of per-event weights and bins into a caller-owned
+    device buffer of 2 + d*n_bins doubles; allocates nothing (static device scratch); enqueue only"""
+    _check(lib().mf_reduce_weights_noalloc(int(device), C.c_void_p(int(weight_ptr)), C.c_void_p(int(bins_ptr)), int(n_events), int(d),
+                                           int(n_bins), float(n_total), 1 if accumulate else 0, C.c_void_p(int(acc_ptr)),
+                                           _stream_ptr(stream, device)))
 
 
 def fp64_peak(device=0, seconds=0.5):

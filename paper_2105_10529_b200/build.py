@@ -1,5 +1,5 @@
-"""In-tree build of libmadflow_b200.so for sm_100a: run the amplitude generator, compile the C-ABI
-and the eight per-process kernel objects in parallel with nvcc, link.  `python -m
+"""In-tree build of libmadflow_b200.so for sm_100a: run the amplitude generator, compile the C-ABI,
+the no-alloc reduction and the eight per-process kernel objects in parallel with nvcc, link.  `python -m
 paper_2105_10529_b200.build [--force]`."""
 import os
 import subprocess
@@ -28,12 +28,13 @@ def build(force=False, verbose=False):
     api = kern + [os.path.join(CSRC, f) for f in ("mf_small_kernels.cuh", "mf_params.h")]
     api += [os.path.join(os.path.dirname(HERE), "include", "madflow_b200.h")]
     jobs = [("mf_api.o", os.path.join(CSRC, "mf_api.cu"), [])]
+    jobs += [("mf_noalloc.o", os.path.join(CSRC, "mf_noalloc.cu"), [])]      # mf_reduce_weights_noalloc (static device scratch)
     jobs += [("mf_proc%d.o" % p, os.path.join(CSRC, "mf_proc.cu"), ["-DMF_PROC=%d" % p]) for p in range(8)]
 
     def compile_one(job):
         obj, src, extra = job
         out = os.path.join(obj_dir, obj)
-        if not force and _newer(out, (api if obj == "mf_api.o" else kern) + [src]):
+        if not force and _newer(out, (api if obj in ("mf_api.o", "mf_noalloc.o") else kern) + [src]):
             return obj, "up to date"
         r = subprocess.run(["nvcc"] + NVCC_FLAGS + extra + ["-c", src, "-o", out], capture_output=True, text=True)
         with open(out + ".log", "w") as f:

@@ -15,6 +15,7 @@ static thread_local std::string g_err;
 extern "C" const char* mf_last_error(void) { return g_err.c_str(); }
 
 static int fail(int code, const std::string& msg) { g_err = msg; return code; }
+int mf_fail_(int code, const char* msg) { return fail(code, msg); }      // for the other translation units of the library (mf_noalloc.cu)
 #define MF_CUDA(call)                                                                              \
   do {                                                                                             \
     cudaError_t e_ = (call);                                                                       \

@@ -556,9 +556,12 @@ extern "C" int mf_me_flops(const mf_vegas_t* h, uint64_t* n_add, uint64_t* n_mul
                                     MF_ME2_GG_TT_NFMA + MF_ME2_EE_MUMU_NFMA + 1},    // p p -> t t~: both subprocesses + the luminosity-weighted sum (mul, fma)
                                    {2 * MF_ME2_QQ_TTG_NADD, 2 * MF_ME2_QQ_TTG_NMUL, 2 * MF_ME2_QQ_TTG_NFMA + 2},     // two channels (q q~, q~ q)
                                    {4 * MF_ME2_QG_TTQ_NADD, 4 * MF_ME2_QG_TTQ_NMUL, 4 * MF_ME2_QG_TTQ_NFMA + 4}};    // four channels
-  if (n_add) *n_add = T[h->P.process][0];
-  if (n_mul) *n_mul = T[h->P.process][1];
-  if (n_fma) *n_fma = T[h->P.process][2];
+  // gg -> tt~g on the staged fp64 path runs the shared-memory-operand organisation (helicity loop over gluon leg 2 only): its own count
+  static const uint64_t S2[3] = {MF_ME2_GG_TTG_S_NADD, MF_ME2_GG_TTG_S_NMUL, MF_ME2_GG_TTG_S_NFMA};
+  const uint64_t* t = (h->P.process == MF_GG_TTG && h->use_staged && !h->f32) ? S2 : T[h->P.process];
+  if (n_add) *n_add = t[0];
+  if (n_mul) *n_mul = t[1];
+  if (n_fma) *n_fma = t[2];
   return MF_OK;
 }
 
@@ -568,7 +571,10 @@ extern "C" int mf_me_flops_bounds(const mf_vegas_t* h, uint64_t* flops_min, uint
   int rc = mf_me_flops(h, &a, &m, &f);
   if (rc) return rc;
   uint64_t lo = a + m + 2 * f, ex = lo;
-  if (h->P.process == MF_GG_TTG) lo = MF_ME2_GG_TTG_NFLOPS_MIN;
+  if (h->P.process == MF_GG_TTG) {
+    lo = MF_ME2_GG_TTG_NFLOPS_MIN;
+    if (h->use_staged && !h->f32) ex = MF_ME2_GG_TTG_S_NFLOPS_EMITTED;      // with the cheap loop invariants it recomputes per trip
+  }
   if (h->P.process == MF_GG_TTGG) {
     lo = MF_ME2_GG_TTGG_NFLOPS_MIN;
     ex = 4ull * (MF_ME2_GG_TTGG_LANES_NADD + MF_ME2_GG_TTGG_LANES_NMUL + 2ull * MF_ME2_GG_TTGG_LANES_NFMA);

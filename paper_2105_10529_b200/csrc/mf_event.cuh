@@ -120,7 +120,7 @@ MF_HD T mf_me2(const MfParams& P, T rts, const T k[MfProc<PROC>::N][4]) {
 #if defined(__CUDACC__)
 template <typename T, int S>
 __device__ __forceinline__ T mf_me2_ttg_smem(const MfParams& P, T rts, const T k[3][4], T* W) {
-  static_assert(MF_ME2_GG_TTG_NIN == 29, "generator input layout changed");
+  static_assert(MF_ME2_GG_TTG_NIN == 29 && MF_ME2_GG_TTG_S_SCALE == MF_ME2_GG_TTG_SCALE, "generator input layout changed");
   {
     T in[29];
     mf_me_inputs_gg<3, T>(rts, T(P.m_top), k, in);

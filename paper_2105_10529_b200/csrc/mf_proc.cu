@@ -661,7 +661,10 @@ static cudaError_t proc_staged_setup(const MfParams& P, int* rec_fields, int* oc
     return r ? r : cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_front, mf_front_kernel<MF_PROC, G>, MF_THREADS, front_smem(P));
   });
   if (e) return e;
-  e = cudaFuncSetAttribute(mf_me_kernel<MF_PROC, double, MF_ME_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 32 * 1024 + (int)me_tile_bytes(MF_ME_THREADS));
+  {                                                      // region prefix (<= 32 KB) + tiles, capped at the 227 KB an sm_100 CTA can opt in to
+    const int want = 32 * 1024 + (int)me_tile_bytes(MF_ME_THREADS), cap = 227 * 1024;
+    e = cudaFuncSetAttribute(mf_me_kernel<MF_PROC, double, MF_ME_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, want < cap ? want : cap);
+  }
   if (e) return e;
   if constexpr (kF32) {
     e = cudaFuncSetAttribute(mf_me_kernel<MF_PROC, float, MF_ME_THREADS_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);

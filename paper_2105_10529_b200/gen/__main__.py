@@ -31,7 +31,7 @@ def main(outdir=None):
         text, tot = A.emit_function(gen, fname)
         if fname == "mf_me2_gg_ttg":
             text += "#define MF_ME2_GG_TTG_NFLOPS_MIN %dull\n" % lean_flops(3)
-            text += A.emit_function_smem(gen, fname, A.SMEM_CLOBBER_EVERY, A.SMEM_HOIST_COST)
+            text += A.emit_function_smem(A.generate_smem(fname), fname, A.SMEM_CLOBBER_EVERY, A.SMEM_HOIST_COST, A.SMEM_RCP_LEAF)
         _write(os.path.join(outdir, fname + ".cuh"), text)
         print("%-22s add %7d mul %7d fma %7d rcp %3d  flops/event %8d  inputs %d" % (
             fname, tot["add"], tot["mul"], tot["fma"], tot["rcp"],

@@ -492,7 +492,7 @@ def emit_function(gen, fname):
     return "\n".join(L) + "\n", tot
 
 
-def emit_function_smem(gen, fname, clobber_every=256, max_hoist_cost=2):
+def emit_function_smem(gen, fname, clobber_every=256, max_hoist_cost=2, rcp_leaf=False):
     """The same helicity-loop function with its loop-entering values in SHARED MEMORY instead of registers:
         template <typename T, int S> T fname_s(T* W)
     W: the thread's column of a [slot][S] tile (S = threads of the CTA: conflict-free): slots 0..NIN-1 hold the inputs, the
@@ -503,7 +503,7 @@ def emit_function_smem(gen, fname, clobber_every=256, max_hoist_cost=2):
     1e7 events (profiles/r2_tuning.md; 384 threads at 168 registers still spill 1.2 KB and take 8.0 ms)."""
     g, out = gen.g, gen.out
     nh = len(gen.loop_assign)
-    pro_ids, body_ids, hoisted = g.plan([out], max_hoist_cost)     # parking costs shared memory, not registers: hoist more
+    pro_ids, body_ids, hoisted = g.plan([out], max_hoist_cost, rcp_leaf)     # parking costs shared memory, not registers: hoist more
     body_set = set(body_ids)
     leaf = lambda j: g.nodes[j][0] in ("in", "sym")
     parked = sorted({o for i in body_ids for o in g._operands(i) if o not in body_set and not leaf(o)})
@@ -511,7 +511,18 @@ def emit_function_smem(gen, fname, clobber_every=256, max_hoist_cost=2):
     slot = {j: nin + n for n, j in enumerate(parked)}
     idx = {n: i for i, n in enumerate(gen.input_names)}
     U = fname.upper()
-    L = ["#define %s_NW %d      // slots of the shared-memory tile of %s_s: inputs, then parked invariants" % (U, nin + len(parked), fname),
+    p0, b0, _h = g.plan([out], None)              # ALGORITHMIC count of this organisation: every loop invariant computed once
+    c0, c1 = g.count_list(p0), g.count_list(b0)
+    alg = {k: c0[k] + nh * (c1[k] + (1 if k == "add" else 0)) for k in c0}
+    cp, cb = g.count_list(pro_ids), g.count_list(body_ids)
+    emitted = {k: cp[k] + nh * (cb[k] + (1 if k == "add" else 0)) for k in cp}
+    L = ["// %s_s: helicity loop over gluon legs %s (%d trips); algorithmic %d add, %d mul, %d fma (flops = %d); emitted with recomputed invariants: flops = %d"
+         % (fname, gen.loop_legs, nh, alg["add"], alg["mul"], alg["fma"], alg["add"] + alg["mul"] + 2 * alg["fma"],
+            emitted["add"] + emitted["mul"] + 2 * emitted["fma"]),
+         "#define %s_S_NADD %dull" % (U, alg["add"]), "#define %s_S_NMUL %dull" % (U, alg["mul"]), "#define %s_S_NFMA %dull" % (U, alg["fma"]),
+         "#define %s_S_NFLOPS_EMITTED %dull" % (U, emitted["add"] + emitted["mul"] + 2 * emitted["fma"]),
+         "#define %s_S_SCALE %r" % (U, gen.scale),
+         "#define %s_NW %d      // slots of the shared-memory tile of %s_s: inputs, then parked invariants" % (U, nin + len(parked), fname),
          "#if defined(__CUDACC__)",
          "template <typename T, int S>",
          "__device__ __forceinline__ T %s_s(T* W) {" % fname,
@@ -579,10 +590,22 @@ SYNC_MACRO = {}
 # emission order of the helicity-loop body (Dag.schedule): window 0 = creation order
 SCHED_WINDOW = 48
 SCHED_DISTANCE = 5
-# shared-memory-operand variant (emit_function_smem): statements between its compiler barriers (64 .. 1024: no difference on
-# the B200) and its hoisting threshold (none / 2 / 3 / 6: 5.42 / 5.39 / 5.40 / 5.46 ms; profiles/r2_tuning.md)
+# shared-memory-operand variant of gg -> tt~g (emit_function_smem; the |M|^2 stage of the staged path): with the loop invariants parked
+# in shared memory a SHORTER loop pays -- gluon leg 2 only (2 trips, 6 806 operations per event instead of 8 712 with legs (0, 2)):
+# 102 slots per thread (reciprocals always parked, values built on them recomputed when their cone has <= 16 operations), 5.40 -> 5.05 ms
+# per 1e7 events (profiles/r2_tuning.md).  Statements between compiler barriers: 64 .. 1024 make no difference on the B200.
+SMEM_LOOP_LEGS = (2,)
 SMEM_CLOBBER_EVERY = 256
-SMEM_HOIST_COST = 2
+SMEM_HOIST_COST = 16
+SMEM_RCP_LEAF = True
+
+
+def generate_smem(fname):
+    """the organisation of fname's shared-memory-operand variant (a second Gen: the register version keeps PROCESSES[fname])"""
+    assert fname == "mf_me2_gg_ttg"
+    gen = Gen(3, loop_legs=SMEM_LOOP_LEGS, parity=True, basis="linear")
+    gen.build()
+    return gen
 
 
 def generate(fname):

@@ -172,12 +172,13 @@ class Dag:
             acc = self.fma(a, b, acc)
         return acc
 
-    def plan(self, outputs, max_cost=None):
+    def plan(self, outputs, max_cost=None, rcp_leaf=False):
         """Split the live nodes into (prologue, body, hoisted).  max_cost None: every loop-invariant
         node is hoisted.  Otherwise only EXPENSIVE invariants (cone with a reciprocal or more than
         max_cost operations) that the body uses are hoisted; cheap ones are recomputed inside the
         loop (and also in the prologue where a hoisted node needs them), because hoisting everything
-        keeps more values alive across the loop than the register file holds."""
+        keeps more values alive across the loop than the register file holds.  rcp_leaf: a reciprocal is always
+        hoisted, but counts as a leaf for the values built on it (they are recomputed when their cone is small)."""
         mark = self.live(outputs)
         ids = [i for i in range(len(self.nodes)) if mark[i]]
         leaf = lambda i: self.nodes[i][0] in ("in", "sym")
@@ -195,6 +196,8 @@ class Dag:
             c, big = {i}, self.nodes[i][0] == "rcp"
             for o in self._operands(i):
                 if cone[o] is None:
+                    if rcp_leaf and self.nodes[o][0] == "rcp":
+                        continue                    # the reciprocal itself is hoisted; what is built on it may be recomputed
                     big = True
                 else:
                     c |= cone[o]

@@ -103,6 +103,10 @@ def test_generated_amplitude_dag_matches_oracle(mfo, proc, fname, n):
         ref = mfo.me2(proc, mom)
         val = float(A.evaluate(gen, _inputs(gen, mom))) * gen.scale * gs2 ** n / 256
         assert abs(val / ref - 1) < 1e-11
+        if fname == "mf_me2_gg_ttg":      # the organisation of the shared-memory-operand variant (loop over gluon leg 2 only)
+            gs_ = A.generate_smem(fname)
+            assert gs_.input_names == gen.input_names and gs_.scale == gen.scale and len(gs_.loop_assign) == 2
+            assert abs(float(A.evaluate(gs_, _inputs(gs_, mom))) * gs_.scale * gs2 ** n / 256 / ref - 1) < 1e-11
 
 
 def test_four_lane_decomposition_matches_oracle(mfo):

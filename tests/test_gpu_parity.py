@@ -636,7 +636,11 @@ def test_streams_and_stage_time_sums(mf):
     assert launches == 2 and sums["front"] > 0 and sums["me"] > sums["front"] and sums["reduce"] > 0
     assert a.stage_ms_sum()[1] == 0
     fb = a.me_flops_bounds()
-    assert fb["min"] == 11302 and fb["executed"] == a.me_flops()["flops"] == 15023
+    assert fb["min"] == 11302 and a.me_flops()["flops"] == 11591 and fb["executed"] == 11975      # staged path: loop over gluon leg 2 only
+    a.set_path(False)
+    fb = a.me_flops_bounds()
+    assert a.me_flops()["flops"] == 15023 == fb["executed"] and fb["min"] == 11302                 # fused path: the register-resident organisation
+    a.set_path(True)
     fb = mf.Vegas(W.config(W.GG_TTGG)).me_flops_bounds()
     assert fb["min"] == 170880 < 256020 < fb["executed"]
 

@@ -57,9 +57,12 @@ class Gen2Q:
     """kind "qq": q q~ -> t t~ g;  kind "qg": q g -> t t~ q.  Inputs are generic (no axis is special), so that the
     beam-exchanged and charge-conjugated channels are the same code on relabelled momenta."""
 
-    def __init__(self, kind):
+    def __init__(self, kind, loop_pol=False):
+        """loop_pol: the gluon's polarisation (eps1 / eps2) is a run-time loop of two trips (symbol lam5 = +-1 blends the two
+        vectors) instead of being unrolled: half the straight-line code, no spills"""
         assert kind in ("qq", "qg")
         self.kind, self.g = kind, Dag()
+        self.loop_pol = loop_pol
         self.input_names = []
         inp = self._inp
         self.mt = inp("mt")
@@ -73,7 +76,8 @@ class Gen2Q:
         self.r_ing = [inp("r_wp"), zero] + [inp("r_" + n) for n in ("c0", "cx", "cy")]
         self.K = [inp("K" + c) for c in "exyz"]                         # gluon: all-incoming momentum, two real unit polarisations
         self.e = [[inp("e%d%s" % (i, c)) for c in "xyz"] for i in (1, 2)]
-        self.loop_legs = ()
+        self.loop_legs = (5,) if loop_pol else ()
+        self.lam5 = self.g.sym("lam5") if loop_pol else None
 
     def _inp(self, name):
         self.input_names.append(name)
@@ -120,8 +124,13 @@ class Gen2Q:
             j = GenEE._current(self, lrow, lcol)                        # lrow gamma^mu lcol, upper index
             if all(c.re.is_zero() and c.im.is_zero() for c in j):
                 continue                                                # chirality: the massless line flips no helicity
-            for pol in (0, 1):
-                e = [Cx(zero, zero)] + cvec(self.e[pol])
+            for pol in ((None,) if self.loop_pol else (0, 1)):
+                if pol is None:                                         # e = (1 + lam5)/2 e1 + (1 - lam5)/2 e2
+                    s1, s2 = 0.5 * self.lam5 + 0.5, 0.5 - 0.5 * self.lam5
+                    evec = [g.sop([(s1, a), (s2, b)]) for a, b in zip(self.e[0], self.e[1])]
+                else:
+                    evec = self.e[pol]
+                e = [Cx(zero, zero)] + cvec(evec)
                 es = SlashC(e)
                 # light line with the gluon attached
                 b3 = GenEE._current(self, lrow, self._prop(q3, None, self._slash(e, lcol)))
@@ -129,7 +138,7 @@ class Gen2Q:
                 w4 = [csum_prod(g, t) for t in row_slash_terms(w4, SlashC(cvec(q4)))]   # ... q4slash
                 b4 = GenEE._current(self, w4, lcol)
                 # three-gluon vertex: V3(-P, PL, K; j, e) = j ((-P - PL).e) + (PL - K) (j.e) + e ((K + P).j)
-                c1 = mdot_rr(g, [-(a + b) for a, b in zip(P, PL)], [zero] + self.e[pol])
+                c1 = mdot_rr(g, [-(a + b) for a, b in zip(P, PL)], [zero] + list(evec))
                 c2 = mdot(g, j, e)
                 c3 = mdot_r(g, [a + b for a, b in zip(self.K, P)], j)
                 dPK = [a - b for a, b in zip(PL, self.K)]
@@ -158,8 +167,10 @@ class Gen2Q:
         self.out = total
         # |M|^2 = g_s^6 * scale * out: colour denominator, average over the incoming pair's helicities and colours
         self.scale = 1.0 / den / (36.0 if self.kind == "qq" else 96.0)
-        self.loop_assign = [()]
+        self.loop_assign = [(-1.0,), (1.0,)] if self.loop_pol else [()]
         return total
 
 
-PROCESSES_2Q = {"mf_me2_qq_ttg": lambda: Gen2Q("qq"), "mf_me2_qg_ttq": lambda: Gen2Q("qg")}
+# the gluon polarisation as a run-time loop: stack 1424 -> 944 B per thread, q q~ -> t t~ g 0.99 -> 0.94 ms per 1e6 events on the B200
+# (q g -> t t~ q unchanged: 1.60 ms; profiles/r2_tuning.md)
+PROCESSES_2Q = {"mf_me2_qq_ttg": lambda: Gen2Q("qq", loop_pol=True), "mf_me2_qg_ttq": lambda: Gen2Q("qg", loop_pol=True)}

@@ -154,6 +154,9 @@ def test_two_quark_line_generator_matches_oracle(mfo):
         gen = Q.Gen2Q(kind)
         gen.build()
         assert len(gen.input_names) == 41
+        looped = Q.PROCESSES_2Q["mf_me2_%s" % ("qq_ttg" if kind == "qq" else "qg_ttq")]()      # the emitted form: polarisation loop
+        looped.build()
+        assert looped.loop_pol and looped.input_names == gen.input_names and looped.scale == gen.scale and len(looped.loop_assign) == 2
         for trial in range(3):
             rts = rng.uniform(450, 4000)
             ps = mfo.phase_space(3, rts * rts, [173.0, 173.0, 0.0], rng.uniform(0.03, 0.97, 5))
@@ -179,8 +182,9 @@ def test_two_quark_line_generator_matches_oracle(mfo):
                     e = np.array(_glu(kg)) * math.sqrt(2); e1, e2 = e[:3], [e[3], e[4], 0.0]
                 for n, c in zip("xyz", e1): v["e1" + n] = c
                 for n, c in zip("xyz", e2): v["e2" + n] = c
-                val = float(A.evaluate(gen, {k: x for k, x in v.items() if k in gen.input_names})) * gen.scale * gs2 ** 3
-                assert abs(val / mfo.me2_2q(proc, m) - 1) < 1e-12
+                for form in (gen, looped):
+                    val = float(A.evaluate(form, {k: x for k, x in v.items() if k in form.input_names})) * form.scale * gs2 ** 3
+                    assert abs(val / mfo.me2_2q(proc, m) - 1) < 1e-12
 
 
 def test_generator_colour_matrices_match_golden():

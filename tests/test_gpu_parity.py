@@ -706,4 +706,4 @@ def test_two_quark_line_channels_iterations_and_errors(mf, mfo, proc):
     for bad in (W.config(proc, pdf_xf=W.synthetic_gluon_grid()), W.config(proc, precision=32)):
         with pytest.raises(mf.MfError):
             mf.Vegas(bad)
-    assert gpu.me_flops()["flops"] == (2 if proc == W.QQ_TTG else 4) * (5636 + 2)
+    assert gpu.me_flops()["flops"] == (2 if proc == W.QQ_TTG else 4) * (5661 + 2)

@@ -21,8 +21,9 @@ WANT = ["dram__bytes_read.sum", "dram__bytes_write.sum", "gpu__time_duration.sum
         "l1tex__data_pipe_lsu_wavefronts.avg.pct_of_peak_sustained_elapsed",
         "sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_elapsed", "sm__warps_active.avg.pct_of_peak_sustained_active",
         "smsp__issue_active.avg.pct_of_peak_sustained_active", "sm__icc_request_hit_rate.pct", "smsp__inst_executed.sum",
-        "sm__cycles_elapsed.avg", "smsp__sass_thread_inst_executed_op_dadd_pred_on.sum",
-        "smsp__sass_thread_inst_executed_op_dmul_pred_on.sum", "smsp__sass_thread_inst_executed_op_dfma_pred_on.sum"]
+        "sm__cycles_elapsed.avg", "smsp__sass_thread_inst_executed_op_dadd_pred_on.sum.per_cycle_elapsed",
+        "smsp__sass_thread_inst_executed_op_dmul_pred_on.sum.per_cycle_elapsed",
+        "smsp__sass_thread_inst_executed_op_dfma_pred_on.sum.per_cycle_elapsed"]
 TO_BYTES = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
 
 
@@ -55,6 +56,15 @@ def main():
         st = {k: float(v.replace(",", "")) for k, v in d.items()
               if k.startswith("smsp__average_warps_issue_stalled") and k.endswith("per_issue_active.ratio")}
         top = sorted(st.items(), key=lambda x: -x[1])[:9]
+        try:      # executed fp64 flops of the launch = (dadd + dmul + 2 dfma thread-instructions per cycle) x elapsed cycles
+            f = lambda k: float(d["smsp__sass_thread_inst_executed_op_%s_pred_on.sum.per_cycle_elapsed" % k].replace(",", ""))
+            cyc = float(d["sm__cycles_elapsed.avg"].replace(",", ""))
+            ms = float(d["gpu__time_duration.sum"].replace(",", "")) * {"ms": 1.0, "us": 1e-3, "s": 1e3}[units["gpu__time_duration.sum"]]
+            fl = (f("dadd") + f("dmul") + 2.0 * f("dfma")) * cyc
+            print("  executed fp64: %.4e flops per launch (%.4e thread-instructions) = %.2f TFLOP/s over the profiled launch"
+                  % (fl, (f("dadd") + f("dmul") + f("dfma")) * cyc, fl / (ms * 1e-3) / 1e12))
+        except (KeyError, ValueError):
+            pass
         print("  stalls/issue: " + " ".join("%s=%.2f" % (k.replace("smsp__average_warps_issue_stalled_", "").replace("_per_issue_active.ratio", ""), v)
                                             for k, v in top))
         if args.kernel and first is None and args.kernel in name.replace("(int)", "").replace("void ", ""):

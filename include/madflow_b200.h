@@ -173,6 +173,15 @@ int mf_accum_len(const mf_vegas_t *h, uint32_t *n);
  * integrator state (grid, raw sums, records) waits on the device for the last call that wrote it, a call
  * that writes the grid also for evaluations in flight; host reads (get_*, result) wait for both.        */
 int mf_result(mf_vegas_t *h, mf_result_t *host_out);
+/* Checkpoint / resume of the integrator state (an auxiliary of the path: the integration state lives on the device):
+ * the grid edges, the per-iteration records, the iteration counter (= the Philox counter word of the next iteration) and the
+ * accumulated observable histograms, as one opaque host blob of mf_state_size() bytes (it grows by 40 bytes per iteration).
+ * mf_get_state waits for the work in flight and copies it out; mf_set_state puts a blob into a handle created with the SAME
+ * configuration (process, generator, dimensions, bins, seed: MF_EINVAL otherwise; observables must have been set as when it was saved):
+ * the next mf_vegas_iterate then continues the run bit for bit, and mf_result combines the restored iterations with the new ones. */
+int mf_state_size(const mf_vegas_t *h, uint64_t *bytes);
+int mf_get_state(mf_vegas_t *h, void *host_buf, uint64_t bytes /* >= mf_state_size */);
+int mf_set_state(mf_vegas_t *h, const void *host_buf, uint64_t bytes);
 /* per-iteration records; host_out[n_iter] must hold at least max_iter entries; *n_iter = stored    */
 int mf_get_iterations(mf_vegas_t *h, mf_iter_t *host_out, uint32_t max_iter, uint32_t *n_iter);
 int mf_get_grid(mf_vegas_t *h, double *host_edges /* [d][n_bins+1] */);

@@ -17,7 +17,8 @@ EXPORTS = ["mf_vegas_create", "mf_vegas_destroy", "mf_ndim", "mf_integrand_eval"
            "mf_get_iterations", "mf_get_grid", "mf_set_grid", "mf_set_launch", "mf_me_flops",
            "mf_fp64_peak", "mf_last_kernel_ms", "mf_last_error", "mf_set_path", "mf_last_stage_ms",
            "mf_set_observables", "mf_get_observables", "mf_accum_len", "mf_zero_accum", "mf_get_accum_device",
-           "mf_set_accum_device", "mf_stage_ms_sum", "mf_me_flops_bounds", "mf_reduce_weights_noalloc"]
+           "mf_set_accum_device", "mf_stage_ms_sum", "mf_me_flops_bounds", "mf_reduce_weights_noalloc",
+           "mf_state_size", "mf_get_state", "mf_set_state"]
 
 
 class MfError(RuntimeError):
@@ -107,6 +108,9 @@ def lib():
         L.mf_last_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
         L.mf_stage_ms_sum.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(u32)]
         L.mf_me_flops_bounds.argtypes = [vp, C.POINTER(u64), C.POINTER(u64)]
+        L.mf_state_size.argtypes = [vp, C.POINTER(u64)]
+        L.mf_get_state.argtypes = [vp, vp, u64]
+        L.mf_set_state.argtypes = [vp, vp, u64]
         L.mf_reduce_weights_noalloc.argtypes = [C.c_int32, vp, vp, u64, u32, u32, C.c_double, C.c_int32, vp, vp]
         L.mf_me_flops.argtypes = [vp, C.POINTER(u64), C.POINTER(u64), C.POINTER(u64)]
         L.mf_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
@@ -267,6 +271,18 @@ class Vegas:
         a, b = C.c_float(), C.c_float()
         _check(lib().mf_last_kernel_ms(self._h, C.byref(a), C.byref(b)))
         return a.value, b.value
+
+    def get_state(self):
+        """checkpoint of the integrator state (grid, iteration records, counter, observable sums) as bytes"""
+        n = C.c_uint64()
+        _check(lib().mf_state_size(self._h, C.byref(n)))
+        buf = (C.c_char * n.value)()
+        _check(lib().mf_get_state(self._h, buf, n.value))
+        return bytes(buf)
+
+    def set_state(self, blob):
+        """resume from a checkpoint taken on a handle of the same configuration"""
+        _check(lib().mf_set_state(self._h, C.c_char_p(blob), len(blob)))
 
     def stage_ms_sum(self):
         """sums of the stage times over all staged launches since the previous call, and their number"""

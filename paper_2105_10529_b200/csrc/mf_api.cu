@@ -545,6 +545,71 @@ extern "C" int mf_set_grid(mf_vegas_t* h, const double* e) {
   return MF_OK;
 }
 
+// ---- checkpoint / resume of the integrator state (auxiliary; include/madflow_b200.h) ---------------------
+struct MfStateHeader {
+  uint32_t magic, version; int32_t process; uint32_t generator, d, n_bins, n_iter, n_obs; uint64_t seed;
+};
+#define MF_STATE_MAGIC 0x4d465354u      // "MFST"
+static size_t state_bytes(const mf_vegas* h, uint32_t n_iter) {
+  return sizeof(MfStateHeader) + sizeof(double) * ((size_t)h->P.d * (h->P.nb + 1) + MF_OBS_ACC + 1) + sizeof(MfIterRec) * (size_t)n_iter;
+}
+
+extern "C" int mf_state_size(const mf_vegas_t* h, uint64_t* bytes) {
+  if (!h || !bytes) return fail(MF_EINVAL, "null argument");
+  *bytes = state_bytes(h, h->iteration);
+  return MF_OK;
+}
+
+extern "C" int mf_get_state(mf_vegas_t* h, void* host_buf, uint64_t bytes) {
+  if (!h || !host_buf) return fail(MF_EINVAL, "null argument");
+  if (bytes < state_bytes(h, h->iteration)) return fail(MF_EINVAL, "state buffer too small (mf_state_size)");
+  MF_ON_DEVICE(h);
+  if (int rc = state_sync(h, true)) return rc;
+  MfStateHeader hd = {MF_STATE_MAGIC, 1u, h->P.process, (uint32_t)h->P.gen, (uint32_t)h->P.d, (uint32_t)h->P.nb, h->iteration, (uint32_t)h->P.n_obs, h->cfg.seed};
+  char* p = (char*)host_buf;
+  std::memcpy(p, &hd, sizeof hd); p += sizeof hd;
+  const size_t ne = sizeof(double) * (size_t)h->P.d * (h->P.nb + 1), nr = sizeof(MfIterRec) * (size_t)h->iteration, no = sizeof(double) * (MF_OBS_ACC + 1);
+  MF_CUDA(cudaMemcpy(p, h->d_edges, ne, cudaMemcpyDeviceToHost)); p += ne;
+  if (nr) MF_CUDA(cudaMemcpy(p, h->d_state->it, nr, cudaMemcpyDeviceToHost));
+  p += nr;
+  MF_CUDA(cudaMemcpy(p, h->d_obs, no, cudaMemcpyDeviceToHost));
+  return MF_OK;
+}
+
+extern "C" int mf_set_state(mf_vegas_t* h, const void* host_buf, uint64_t bytes) {
+  if (!h || !host_buf) return fail(MF_EINVAL, "null argument");
+  if (bytes < sizeof(MfStateHeader)) return fail(MF_EINVAL, "state buffer too small");
+  MfStateHeader hd;
+  std::memcpy(&hd, host_buf, sizeof hd);
+  if (hd.magic != MF_STATE_MAGIC || hd.version != 1u) return fail(MF_EINVAL, "not a madflow_b200 state (magic / version)");
+  if (hd.process != h->P.process || hd.generator != (uint32_t)h->P.gen || hd.d != (uint32_t)h->P.d || hd.n_bins != (uint32_t)h->P.nb || hd.seed != h->cfg.seed)
+    return fail(MF_EINVAL, "state belongs to another configuration (process, generator, dimensions, bins or seed differ)");
+  if (hd.n_obs != (uint32_t)h->P.n_obs) return fail(MF_EINVAL, "state was saved with another number of observables (call mf_set_observables first)");
+  if (hd.n_iter > MF_MAX_ITER) return fail(MF_EINVAL, "corrupt state (iteration count)");
+  if (bytes < state_bytes(h, hd.n_iter)) return fail(MF_EINVAL, "state buffer truncated");
+  const size_t ne = sizeof(double) * (size_t)h->P.d * (h->P.nb + 1), nr = sizeof(MfIterRec) * (size_t)hd.n_iter, no = sizeof(double) * (MF_OBS_ACC + 1);
+  const char* p = (const char*)host_buf + sizeof hd;
+  {                                                       // the same validation as mf_set_grid
+    std::vector<double> e((size_t)h->P.d * (h->P.nb + 1));
+    std::memcpy(e.data(), p, ne);
+    for (int j = 0; j < h->P.d; ++j) {
+      const double* r = e.data() + (size_t)j * (h->P.nb + 1);
+      if (r[0] != 0.0 || r[h->P.nb] != 1.0) return fail(MF_EINVAL, "corrupt state (grid edges)");
+      for (int k = 0; k < h->P.nb; ++k) if (!(r[k + 1] > r[k])) return fail(MF_EINVAL, "corrupt state (grid edges)");
+    }
+  }
+  MF_ON_DEVICE(h);
+  if (int rc = state_sync(h, true)) return rc;
+  MF_CUDA(cudaMemcpy(h->d_edges, p, ne, cudaMemcpyHostToDevice)); p += ne;
+  if (nr) MF_CUDA(cudaMemcpy(h->d_state->it, p, nr, cudaMemcpyHostToDevice));
+  p += nr;
+  MF_CUDA(cudaMemcpy(&h->d_state->n_iter, &hd.n_iter, sizeof(unsigned int), cudaMemcpyHostToDevice));
+  MF_CUDA(cudaMemcpy(h->d_obs, p, no, cudaMemcpyHostToDevice));
+  h->iteration = hd.n_iter;                              // = the Philox counter word of the next iteration
+  h->have_k = h->have_stage = h->have_it = false;
+  return MF_OK;
+}
+
 extern "C" int mf_me_flops(const mf_vegas_t* h, uint64_t* n_add, uint64_t* n_mul, uint64_t* n_fma) {
   if (!h) return fail(MF_EINVAL, "handle is NULL");
   static const uint64_t T[8][3] = {{MF_ME2_EE_MUMU_NADD, MF_ME2_EE_MUMU_NMUL, MF_ME2_EE_MUMU_NFMA},

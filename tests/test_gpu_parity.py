@@ -707,3 +707,49 @@ def test_two_quark_line_channels_iterations_and_errors(mf, mfo, proc):
         with pytest.raises(mf.MfError):
             mf.Vegas(bad)
     assert gpu.me_flops()["flops"] == (2 if proc == W.QQ_TTG else 4) * (5661 + 2)
+
+
+def test_checkpoint_and_resume(mf):
+    """mf_get_state / mf_set_state: a run saved after two iterations and restored into a fresh handle continues bit for bit (grid,
+    iteration records, Philox iteration word, observable sums); states of another configuration or damaged blobs are rejected"""
+    for proc, n in ((W.GG_TTG, 100_003), (W.PP_TT, 50_001)):
+        cfg = W.config(proc, seed=21)
+        obs = [(0, 20, 0.0, 400.0), (2, 16, 350.0, 1500.0)]
+        a = mf.Vegas(cfg)
+        a.set_observables(obs)
+        for _ in range(2):
+            a.vegas_iterate(n)
+        blob = a.get_state()
+        assert len(blob) == len(a.get_state()) and blob == a.get_state()
+        b = mf.Vegas(cfg)
+        b.set_observables(obs)
+        b.set_state(blob)
+        np.testing.assert_array_equal(a.get_grid(), b.get_grid())
+        assert b.get_iterations() == a.get_iterations() and b.result() == a.result()
+        ia, ib = a.vegas_iterate(n), b.vegas_iterate(n)
+        assert {k: ia[k] for k in ia if k != "kernel_ms"} == {k: ib[k] for k in ib if k != "kernel_ms"}
+        np.testing.assert_array_equal(a.get_grid(), b.get_grid())
+        assert a.result() == b.result() and b.result()["n_iter"] == 3
+        (ga, na), (gb, nb_) = a.get_observables(), b.get_observables()
+        assert na == nb_ == 3
+        for (x1, x2), (y1, y2) in zip(ga, gb):
+            np.testing.assert_array_equal(x1, y1); np.testing.assert_array_equal(x2, y2)
+        assert len(b.get_state()) == len(blob) + 40                    # one more iteration record
+        # the restored run saw the same random numbers as the uninterrupted one: per-event weights of the next iteration agree too
+        assert bool((a.integrand_eval(3, 0, 2048)["weight"] == b.integrand_eval(3, 0, 2048)["weight"]).all())
+        for bad_cfg in (W.config(proc, seed=22), W.config(W.GG_TT if proc != W.GG_TT else W.GG_TTG, seed=21)):
+            c = mf.Vegas(bad_cfg)
+            if bad_cfg["process"] == proc:
+                c.set_observables(obs)
+            with pytest.raises(mf.MfError) as e:
+                c.set_state(blob)
+            assert e.value.code == mf.MF_EINVAL
+        c = mf.Vegas(cfg)                                               # observables not set as when the state was saved
+        with pytest.raises(mf.MfError):
+            c.set_state(blob)
+        c.set_observables(obs)
+        for damaged in (blob[:-8], b"XXXX" + blob[4:], blob[:64]):
+            with pytest.raises(mf.MfError):
+                c.set_state(damaged)
+        c.set_state(blob)                                               # and the intact blob still goes in
+        assert c.result()["n_iter"] == 2
